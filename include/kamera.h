@@ -1,0 +1,218 @@
+/* kamera.h - C ABI of libkamera: the serve-time hot path of Kamera's training-free KV-reuse operator
+ * (arxiv/paper_2606_23581), hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations: P:NN = line NN of the paper text; R-n = reading n in DESIGN.md.
+ *
+ *   KV^(B|A) = R(delta) . KV(B|0) + U_m V_m^T                                           (Eq. 1)
+ *
+ * A cached, position-free chunk is relocated to any target offset by exact RoPE re-rotation (for MLA only
+ * the decoupled rope band rotates), its stored rank-m conditioning patch is added to K and V per
+ * layer and KV head, and the result is scattered into a paged KV pool through a block table (P:56,
+ * P:195-204).  Chunks are admitted / evicted at either end of a window in O(1).  The same
+ * operator is available fused-on-read inside a paged decode-attention kernel that merges per-chunk softmax
+ * states by log-sum-exp.
+ *
+ * Conventions
+ *  - "device" pointers are CUDA device memory owned by the CALLER (e.g. torch tensors); "host" pointers are
+ *    ordinary host memory.  The library owns only kam_ctx and what hangs off it.
+ *  - All device base pointers must be 16-byte aligned.
+ *  - Every call that takes a `stream` (a cudaStream_t passed as void*; NULL = legacy default stream) enqueues
+ *    its work on that stream and returns without synchronising.  Host bookkeeping (windows, free list) is
+ *    applied immediately; device effects are stream-ordered.
+ *  - Errors: every function returns a kam_status; nothing throws or aborts.  Arguments are validated before
+ *    any state changes, so a failed call leaves the context as it was.  kam_last_error() gives the reason.
+ *  - There is no CPU fallback: without a CUDA device every compute entry returns KAM_ERR_CUDA.
+ */
+#ifndef KAMERA_H_
+#define KAMERA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KAM_MAX_RANK   64    /* largest rank the paper uses: the rank-64 removal patch */
+#define KAM_MAX_LAYERS 128
+
+typedef struct kam_ctx kam_ctx;                       /* opaque; library-owned */
+
+typedef enum { KAM_OK = 0, KAM_ERR_INVALID_ARG = 1, KAM_ERR_NO_PAGES = 2, KAM_ERR_UNSUPPORTED = 3,
+               KAM_ERR_STATE = 4, KAM_ERR_CUDA = 5 } kam_status;
+typedef enum { KAM_MHA = 0, KAM_GQA = 1, KAM_MLA = 2 } kam_layout_kind;
+typedef enum { KAM_ROPE_HALF = 0, KAM_ROPE_INTERLEAVED = 1 } kam_rope_style;  /* pair (i, i+d/2) vs (2i, 2i+1); R-1 */
+typedef enum { KAM_PATCH_TARGET_FRAME = 0, KAM_PATCH_CANONICAL_FRAME = 1 } kam_patch_frame; /* Eq. 1 order = 0; R-4 */
+typedef enum { KAM_FRONT = 0, KAM_BACK = 1 } kam_end;
+typedef enum { KAM_BF16 = 0, KAM_F32 = 1 } kam_dtype;
+
+/* "layout = {MHA, GQA, MLA}" made explicit: one content | rope split covers all three (Fig. 2). */
+typedef struct kam_layout {
+  int32_t kind;            /* kam_layout_kind */
+  int32_t n_layers;        /* <= KAM_MAX_LAYERS */
+  int32_t n_q_heads;       /* multiple of n_kv_heads; query head hq reads KV head hq / (n_q_heads/n_kv_heads) (R-12) */
+  int32_t n_kv_heads;      /* 1 for MLA */
+  int32_t row_dim;         /* elements per token per KV head: head_dim; 576 for MLA (512 latent + 64 rope) */
+  int32_t rope_off;        /* first rotated column of a row: 0 for MHA/GQA, 512 for MLA */
+  int32_t rope_dim;        /* number of rotated columns (even): row_dim for MHA/GQA, 64 for MLA */
+  int32_t has_v;           /* 1: separate V pool (MHA/GQA); 0: MLA, one latent+rope row per token */
+  int32_t v_dim;           /* decode only, has_v == 0: a token's value = first v_dim columns of its row (512) */
+  int32_t page_size;       /* tokens per page */
+  int32_t rope_style;      /* kam_rope_style */
+  int32_t elem_dtype;      /* kam_dtype of canonical chunks AND pool pages */
+  int32_t factor_dtype;    /* kam_dtype of U and W */
+  double  rope_theta;      /* f_i = theta^(-2i/rope_dim) (R-2) */
+} kam_layout;
+
+/* Paged KV pool.  k_layers / v_layers: DEVICE arrays [n_layers] of device base pointers; each layer is
+ * [num_pages][page_size][n_kv_heads][row_dim] of elem_dtype (token-major pages, R-13).  v_layers NULL iff !has_v. */
+typedef struct kam_pool {
+  void *const *k_layers;
+  void *const *v_layers;
+  int32_t num_pages;
+} kam_pool;
+
+/* A position-free canonical chunk KV(B|0).  k_layers / v_layers: DEVICE arrays [n_layers] of
+ * device pointers to [n_tokens][n_kv_heads][row_dim] rows.  p_base = the RoPE position token 0's key sits
+ * at in this stored copy (0 for a chunk prefilled alone); relocation applies the uniform phase advance
+ * delta = p_target - p_base to every token (R-3). */
+typedef struct kam_chunk {
+  const void *const *k_layers;
+  const void *const *v_layers;     /* NULL iff !has_v */
+  int32_t n_tokens;
+  int64_t p_base;
+} kam_chunk;
+
+/* Rank-m patch factors {U_m S, V_m^T}: Delta ~= U W per layer and KV head.
+ * Uk/Wk/Uv/Wv: DEVICE arrays [n_layers] of device pointers.
+ *   U element (t, h, j) at  U[l] + t*u_token_stride + h*u_head_stride + j      (strides in elements;
+ *     u_head_stride == 0 => one U shared by all KV heads, the paper's per-layer form, R-6)
+ *   W[l] is [n_kv_heads][rank][row_dim], contiguous  (the paper's V_m^T).
+ * rank_per_layer: HOST array [n_layers] or NULL (=> the call's `rank` everywhere); 0 => that layer gets the
+ * rotation only (the deep-half variant). */
+typedef struct kam_patch {
+  const void *const *Uk, *const *Wk, *const *Uv, *const *Wv;     /* Uv/Wv NULL iff !has_v */
+  int64_t u_token_stride, u_head_stride;
+  const int32_t *rank_per_layer;
+  int32_t frame;                   /* kam_patch_frame */
+} kam_patch;
+
+/* The argument tuple of kam_relocate_patch as a record, so that one launch covers many chunks. */
+typedef struct kam_reloc_desc {
+  const int32_t *block_table;      /* device */
+  int64_t dst_token_start;
+  const kam_chunk *chunk;          /* host struct */
+  int64_t p_target;
+  const kam_patch *patch;          /* host struct or NULL */
+  int32_t rank;
+} kam_reloc_desc;
+
+/* One layer's factors of one (request, chunk), for patching on read inside the decode kernel. */
+typedef struct kam_patch_ref {
+  const void *Uk, *Wk, *Uv, *Wv;   /* device; this layer's U [T][..] and W [H][rank][row_dim]; all NULL => no patch */
+  int64_t u_token_stride, u_head_stride;
+  int32_t rank;
+  int32_t reserved;
+} kam_patch_ref;
+
+typedef struct kam_stats {
+  int64_t pages_free, pages_total;
+  int64_t table_entries_written;   /* page-table entries written since kam_create (O(1)-per-op evidence) */
+  int64_t chunks_live;
+  int64_t kernels_launched;        /* CUDA kernels this context has launched since kam_create */
+} kam_stats;
+
+/* ---- context -------------------------------------------------------------------------------------------------
+ * pool == NULL creates a bookkeeping-only context: window calls update and export host state but launch nothing
+ * (used to test the host logic without a GPU); every stateless compute entry then needs an explicit pool.
+ * max_requests / max_chunks_per_request / max_pages_per_chunk size the window store. */
+kam_status kam_create(const kam_layout *layout, const kam_pool *pool, int32_t max_requests,
+                      int32_t max_chunks_per_request, int32_t max_pages_per_chunk, kam_ctx **out);
+kam_status kam_destroy(kam_ctx *ctx);
+const char *kam_last_error(const kam_ctx *ctx);     /* ctx may be NULL: error of the last failed kam_create */
+const char *kam_version(void);
+
+/* ---- stateless operator: Eq. 1 written into the paged pool (`apply_reuse`) --------------------
+ * For every layer l, token t, head h:
+ *     k^ = R(p_target - p_base) k + U_k W_k ,  v^ = v + U_v W_v      (TARGET frame; CANONICAL adds U_k W_k first)
+ *     g = dst_token_start + t ; page = block_table[g / P] ; pool[l][page][g % P][h][:] = round_to_elem(k^ / v^)
+ * block_table: DEVICE int32[>= ceil((dst_token_start + n_tokens)/P)], logical page -> physical page.
+ * dst_token_start need not be page aligned.  patch == NULL or rank == 0 => pure rotation (survivors).
+ * p_target is a RoPE phase (any int64; M-RoPE positions are not sequence indices); dst_token_start is the
+ * logical index inside the block table - two different things on purpose.
+ * pool == NULL => the context's pool.  Errors: INVALID_ARG (null/misaligned pointers, rank < 0 or > KAM_MAX_RANK,
+ * n_tokens < 0), UNSUPPORTED (layout the kernels do not cover), CUDA. */
+kam_status kam_relocate_patch(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_table,
+                              int64_t dst_token_start, const kam_chunk *chunk, int64_t p_target,
+                              const kam_patch *patch, int32_t rank, void *stream);
+kam_status kam_relocate_patch_batch(kam_ctx *ctx, const kam_pool *pool, int32_t n,
+                                    const kam_reloc_desc *descs /* host array [n] */, void *stream);
+
+/* Survivors (P:26(ii)): rotate the rope band of K rows ALREADY in the pool, in place, by delta (may be
+ * negative); V is not read.  Tokens [token_start, token_start + n_tokens) of block_table (device). */
+kam_status kam_rotate_inplace(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_table,
+                              int64_t token_start, int32_t n_tokens, int64_t delta, void *stream);
+
+/* Same operator with the canonical chunk and its factors in HOST memory (a chunk recalled from an off-device
+ * canonical store): every k/v/U/W array is a HOST array [n_layers] of HOST pointers with the layouts above
+ * (U contiguous [T][H][rank]).  The library copies them to device staging it owns (H2D on `stream`), then runs
+ * kam_relocate_patch.  Pinned host memory makes the copies asynchronous. */
+kam_status kam_relocate_patch_host(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_table /* device */,
+                                   int64_t dst_token_start, int32_t n_tokens, int64_t p_base, int64_t p_target,
+                                   const void *const *k_host, const void *const *v_host,
+                                   const void *const *Uk_host, const void *const *Wk_host,
+                                   const void *const *Uv_host, const void *const *Wv_host,
+                                   int32_t rank, int32_t frame, void *stream);
+
+/* ---- the window store as a deque (allocation policy R-13) ------------------------------------------
+ * Per request: an ordered list of chunks; logical token order = list order; position of chunk i =
+ * window_base + tokens before it.  Pages come from one LIFO free list (first pops give 0,1,2,...; admit pops in
+ * logical order; evict pushes back in reverse logical order).  The first `n_front_chunks` pinned chunks (a text
+ * prefix) are exempt from FRONT operations.  Chunk lengths must be positive multiples of page_size.
+ *   kam_admit  takes pages, places the chunk at p_target = its position via Eq. 1 (relocate + patch into its pages).
+ *   kam_evict  returns the chunk's pages.
+ * Chunks whose position moved (FRONT ops): materialize = 1 rotates them in place now (delta = position - phase);
+ * materialize = 0 touches nothing - the pending delta is applied on read by kam_window_decode.
+ * Errors: INVALID_ARG, STATE (request not open / already open / window empty / too many chunks), NO_PAGES. */
+kam_status kam_window_open(kam_ctx *ctx, int32_t req, int64_t window_base);
+kam_status kam_window_pin(kam_ctx *ctx, int32_t req, int32_t n_front_chunks);
+kam_status kam_window_close(kam_ctx *ctx, int32_t req);
+kam_status kam_admit(kam_ctx *ctx, int32_t req, int32_t end /* kam_end */, const kam_chunk *chunk,
+                     const kam_patch *patch, int32_t rank, int32_t materialize, int32_t *chunk_handle_out,
+                     void *stream);
+kam_status kam_evict(kam_ctx *ctx, int32_t req, int32_t end /* kam_end */, int32_t materialize, void *stream);
+/* Linear host view of one request, for bit-exact checks.  Any output pointer may be NULL.  Capacities are in
+ * entries; too small => INVALID_ARG.  chunk_starts_out gets n_chunks + 1 entries. */
+kam_status kam_window_export(kam_ctx *ctx, int32_t req, int32_t *block_table_out, int32_t block_table_cap,
+                             int64_t *slot_mapping_out, int64_t slot_mapping_cap, int32_t *chunk_starts_out,
+                             int64_t *chunk_offsets_out, int32_t *chunk_handles_out, int32_t chunk_cap,
+                             int32_t *n_pages_out, int32_t *n_chunks_out);
+kam_status kam_get_stats(kam_ctx *ctx, kam_stats *out);
+
+/* ---- fused-on-read paged decode with LSE merge (R-12) -----------------------------------------------------
+ * For request b, query head hq (KV head h = hq / G), over all chunks c of the request:
+ *     k^_t = R(chunk_offsets[b][c]) k_t (+ U_k W_k)   v^_t = v_t (+ U_v W_v)          read from the pool, never written
+ *     s_t = sm_scale * q . k^_t ;  per chunk (o_c, lse_c) ;  lse = ln sum_c e^{lse_c} ;  out = sum_c e^{lse_c - lse} o_c
+ * q [batch][n_q_heads][row_dim] bf16 device.  block_tables device int32 [batch][max_pages].  chunk_starts device
+ * int32 [batch][max_chunks+1] (CSR token boundaries; only differences to chunk_starts[b][0] are used).
+ * chunk_offsets device int64 [batch][max_chunks] (delta to apply on read; 0 if materialised) or NULL (= all 0).
+ * n_chunks device int32 [batch].  patches: NULL, or device kam_patch_ref [batch][max_chunks].
+ * out [batch][n_q_heads][Dv] bf16 (Dv = row_dim, or v_dim for MLA), lse [batch][n_q_heads] f32 (natural log, scale
+ * inside).  A request with no tokens gives out = 0, lse = -inf.  Requires elem_dtype == KAM_BF16. */
+kam_status kam_paged_decode_merge(kam_ctx *ctx, const void *q, const kam_pool *pool, const int32_t *block_tables,
+                                  int32_t max_pages, const int32_t *chunk_starts, const int64_t *chunk_offsets,
+                                  const int32_t *n_chunks, int32_t max_chunks, const kam_patch_ref *patches,
+                                  int32_t layer, int32_t batch, float sm_scale, void *out, float *lse, void *stream);
+/* Same, over the context's own windows: request ids req_ids[0..batch) (host).  Pending lazy deltas are applied on read. */
+kam_status kam_window_decode(kam_ctx *ctx, const void *q, const int32_t *req_ids, int32_t batch, int32_t layer,
+                             float sm_scale, void *out, float *lse, void *stream);
+/* Same as kam_paged_decode_merge with q, out and lse in HOST memory (H2D / D2H on `stream`, then a stream sync). */
+kam_status kam_paged_decode_merge_host(kam_ctx *ctx, const void *q_host, const kam_pool *pool,
+                                       const int32_t *block_tables, int32_t max_pages, const int32_t *chunk_starts,
+                                       const int64_t *chunk_offsets, const int32_t *n_chunks, int32_t max_chunks,
+                                       const kam_patch_ref *patches, int32_t layer, int32_t batch, float sm_scale,
+                                       void *out_host, float *lse_host, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KAMERA_H_ */

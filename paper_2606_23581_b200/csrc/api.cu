@@ -1,0 +1,523 @@
+// libkamera C entry points: argument validation, host bookkeeping, descriptor staging, kernel launches.
+// Every step of the hot path runs in the kernels (relocate_kernel.cu, decode_kernel.cu); this file only decides
+// geometry and marshals descriptors.  No CPU fallback exists: without CUDA every compute entry fails.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ctx.h"
+
+using namespace kam;
+
+namespace { thread_local std::string g_create_error; }
+
+namespace kam {
+
+kam_status fail(kam_ctx* ctx, kam_status st, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (ctx) ctx->err = buf; else g_create_error = buf;
+  return st;
+}
+
+kam_status cuda_fail(kam_ctx* ctx, cudaError_t e, const char* what) {
+  return fail(ctx, KAM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+kam_status grow_device(kam_ctx* c, void** buf, size_t* cap, size_t bytes, const char* what) {
+  if (*cap >= bytes) return KAM_OK;
+  cudaError_t e;
+  if (*buf) { cudaDeviceSynchronize(); cudaFree(*buf); *buf = nullptr; *cap = 0; }
+  if ((e = cudaMalloc(buf, bytes)) != cudaSuccess) return cuda_fail(c, e, what);
+  *cap = bytes;
+  return KAM_OK;
+}
+
+}  // namespace kam
+
+namespace {
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline int align_up(int x, int a) { return (x + a - 1) / a * a; }
+
+// ---- column blocks of one KV head's row (what one consumer warp processes per 16 tokens) -----------------------
+bool build_head_blocks(kam_ctx* c) {
+  const kam_layout& L = c->lay;
+  c->blocks_per_head = 0;
+  if (L.elem_dtype != KAM_BF16 || L.factor_dtype != KAM_BF16) { c->fast_layout_why = "tiled kernel needs bf16 elements and factors"; return false; }
+  const int pre = L.rope_off, band = L.rope_dim, post = L.row_dim - L.rope_off - L.rope_dim;
+  if (pre % 64 || band % 64 || post % 64) { c->fast_layout_why = "row regions must be multiples of 64 columns"; return false; }
+  if (L.rope_style == KAM_ROPE_HALF && band > 128) { c->fast_layout_why = "HALF rope band wider than 128 columns"; return false; }
+  int n = 0;
+  auto add_plain = [&](int start, int len, bool rope) {
+    for (int off = 0; off < len;) {
+      const int w = std::min(128, len - off);
+      if (n >= kMaxColBlocks) return false;
+      ColBlock b{};
+      b.col_off = (int16_t)(start + off); b.w_col_off = (int16_t)(start + off);
+      b.band_col0 = (int16_t)(rope ? off : 0); b.n_groups = (int8_t)(w / 32); b.rope = rope; b.fhead = 0;
+      c->head_blocks[n++] = b;
+      off += w;
+    }
+    return true;
+  };
+  if (!add_plain(0, pre, false)) return false;
+  if (band) {
+    if (L.rope_style == KAM_ROPE_HALF) {
+      ColBlock b{};
+      b.col_off = (int16_t)pre; b.w_col_off = (int16_t)pre; b.band_col0 = 0; b.n_groups = (int8_t)(band / 32); b.rope = 1;
+      c->head_blocks[n++] = b;
+    } else if (!add_plain(pre, band, true)) return false;
+  }
+  if (!add_plain(pre + band, post, false)) return false;
+  c->blocks_per_head = n;
+  return true;
+}
+
+bool build_reloc_geom(const kam_ctx* c, int max_rank, RelocGeom* out, std::string* why) {
+  const kam_layout& L = c->lay;
+  RelocGeom g{};
+  g.L = L.n_layers; g.H = L.n_kv_heads; g.D = L.row_dim; g.P = L.page_size;
+  g.row_bytes = g.H * g.D * 2;
+  g.nkv = L.has_v ? 2 : 1;
+  g.KT_max = max_rank / 16;
+  g.rope_style = L.rope_style; g.d_r = L.rope_dim; g.half_groups = L.rope_dim / 64;
+  g.theta = L.rope_theta;
+  const int limit = 220 * 1024;
+  RelocGeom best{}; bool have = false;
+  for (int HG = std::min(g.H, 4); HG >= 1; --HG) {
+    if (g.H % HG) continue;
+    const int NB = HG * c->blocks_per_head;
+    if (NB > kMaxColBlocks) continue;
+    RelocGeom t = g;
+    t.HG = HG; t.n_hg = g.H / HG; t.n_blocks = NB;
+    t.slice_bytes = HG * g.D * 2;
+    t.s_row = t.slice_bytes + ((64 - t.slice_bytes % 128) + 128) % 128;      // == 64 (mod 128): conflict-free LDS.128
+    t.su_row = g.KT_max ? HG * max_rank * 2 + 16 : 0;                          // (su_row / 16) odd
+    t.RB = std::min(4, std::max(1, (kRelocConsumerWarps + t.nkv * NB - 1) / (t.nkv * NB)));
+    t.TT = 16 * t.RB;
+    t.st_k = 0;
+    t.st_v = t.st_k + t.TT * t.s_row;
+    t.st_uk = t.st_v + (t.nkv == 2 ? t.TT * t.s_row : 0);
+    t.st_uv = t.st_uk + t.TT * t.su_row;
+    t.st_slot = t.st_uv + (t.nkv == 2 ? t.TT * t.su_row : 0);
+    t.stage_bytes = align_up(t.st_slot + t.TT * 4, 128);
+    t.w_kv_stride = NB * g.KT_max * 4096;
+    t.off_cs = 128;
+    t.off_w = t.off_cs + align_up(std::max(1, g.d_r / 2) * 8, 128);
+    t.off_stage0 = t.off_w + t.nkv * t.w_kv_stride;
+    for (int i = 0; i < NB; ++i) {
+      ColBlock b = c->head_blocks[i % c->blocks_per_head];
+      const int h = i / c->blocks_per_head;
+      b.fhead = (int8_t)h; b.col_off = (int16_t)(b.col_off + h * g.D);
+      t.blk[i] = b;
+    }
+    for (int NS = 4; NS >= 2; --NS) {
+      t.n_stages = NS;
+      t.smem_bytes = t.off_stage0 + NS * t.stage_bytes;
+      if (t.smem_bytes > limit) continue;
+      if (NS >= 3) { *out = t; return true; }
+      if (!have) { best = t; have = true; }
+      break;
+    }
+  }
+  if (have) { *out = best; return true; }
+  *why = "no shared-memory configuration fits";
+  return false;
+}
+
+}  // namespace
+
+namespace kam {
+// ---- staging ---------------------------------------------------------------------------------------------------
+kam_status staging_acquire(kam_ctx* c, size_t bytes, Staging** out) {
+  Staging& s = c->staging[c->staging_next];
+  c->staging_next = (c->staging_next + 1) % kStagingSlots;
+  cudaError_t e;
+  if (s.in_flight) {
+    if ((e = cudaEventSynchronize(s.ev)) != cudaSuccess) return cuda_fail(c, e, "cudaEventSynchronize(staging)");
+    s.in_flight = false;
+  }
+  if (!s.ev && (e = cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming)) != cudaSuccess)
+    return cuda_fail(c, e, "cudaEventCreate");
+  if (s.cap < bytes) {
+    if (s.host) cudaFreeHost(s.host);
+    if (s.dev) cudaFree(s.dev);
+    s.host = s.dev = nullptr; s.cap = 0;
+    const size_t cap = std::max<size_t>(bytes * 2, 64 * 1024);
+    if ((e = cudaMallocHost(&s.host, cap)) != cudaSuccess) return cuda_fail(c, e, "cudaMallocHost(staging)");
+    if ((e = cudaMalloc(&s.dev, cap)) != cudaSuccess) return cuda_fail(c, e, "cudaMalloc(staging)");
+    s.cap = cap;
+  }
+  *out = &s;
+  return KAM_OK;
+}
+kam_status staging_commit(kam_ctx* c, Staging* s, size_t bytes, cudaStream_t st) {
+  cudaError_t e = cudaMemcpyAsync(s->dev, s->host, bytes, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(staging)");
+  return KAM_OK;
+}
+void staging_release(Staging* s, cudaStream_t st) {
+  if (cudaEventRecord(s->ev, st) == cudaSuccess) s->in_flight = true;
+}
+
+kam_status check_pool(kam_ctx* c, const kam_pool** pool) {
+  if (*pool == nullptr) {
+    if (!c->has_pool) return fail(c, KAM_ERR_INVALID_ARG, "no pool given and the context has none");
+    *pool = &c->pool;
+  }
+  if ((*pool)->k_layers == nullptr || (c->lay.has_v && (*pool)->v_layers == nullptr))
+    return fail(c, KAM_ERR_INVALID_ARG, "pool layer-pointer arrays must not be NULL");
+  return KAM_OK;
+}
+}  // namespace kam
+
+namespace {
+
+// ---- relocate core -----------------------------------------------------------------------------------------------
+struct HostReloc {
+  const int32_t* bt; int64_t dst0, delta;
+  const void* const* k; const void* const* v;
+  const kam_patch* patch; int32_t rank; int32_t n_tokens; int32_t flags;
+};
+
+// Checked before any state changes, by the stateless entries and by kam_admit alike.
+kam_status validate_patch(kam_ctx* c, const kam_patch* p, int32_t rank, int idx) {
+  if (rank < 0 || rank > KAM_MAX_RANK) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: rank %d outside [0, %d]", idx, rank, KAM_MAX_RANK);
+  if (!p || rank == 0) return KAM_OK;
+  if (!p->Uk || !p->Wk || (c->lay.has_v && (!p->Uv || !p->Wv)))
+    return fail(c, KAM_ERR_INVALID_ARG, "desc %d: patch factor arrays must not be NULL when rank > 0", idx);
+  if (p->frame != KAM_PATCH_TARGET_FRAME && p->frame != KAM_PATCH_CANONICAL_FRAME)
+    return fail(c, KAM_ERR_INVALID_ARG, "desc %d: unknown patch frame", idx);
+  if (p->u_token_stride <= 0 || p->u_head_stride < 0) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: bad U strides", idx);
+  if (p->rank_per_layer)
+    for (int l = 0; l < c->lay.n_layers; ++l)
+      if (p->rank_per_layer[l] < 0 || p->rank_per_layer[l] > KAM_MAX_RANK)
+        return fail(c, KAM_ERR_INVALID_ARG, "desc %d: rank_per_layer[%d] = %d outside [0, %d]", idx, l, p->rank_per_layer[l], KAM_MAX_RANK);
+  return KAM_OK;
+}
+
+kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostReloc>& hs, cudaStream_t st) {
+  const kam_layout& L = c->lay;
+  const int n = (int)hs.size();
+  // ---- validate everything before touching anything
+  int max_rank = 0, max_tokens = 0;
+  bool fast = c->fast_layout;
+  for (int i = 0; i < n; ++i) {
+    const HostReloc& h = hs[i];
+    if (h.n_tokens < 0) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: n_tokens < 0", i);
+    if (h.bt == nullptr) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: block_table is NULL", i);
+    if (h.dst0 < 0) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: negative token start", i);
+    const bool inplace = h.flags & FLAG_INPLACE;
+    if (!inplace && (h.k == nullptr || (L.has_v && h.v == nullptr)))
+      return fail(c, KAM_ERR_INVALID_ARG, "desc %d: chunk layer-pointer arrays must not be NULL", i);
+    kam_status vs = validate_patch(c, h.patch, h.rank, i);
+    if (vs != KAM_OK) return vs;
+    max_tokens = std::max(max_tokens, h.n_tokens);
+    const kam_patch* p = (h.patch && h.rank > 0) ? h.patch : nullptr;
+    for (int l = 0; l < L.n_layers && p; ++l) {
+      const int r = p->rank_per_layer ? p->rank_per_layer[l] : h.rank;
+      max_rank = std::max(max_rank, r);
+      if (r % 16) fast = false;
+    }
+    if (p && (p->u_token_stride % 8 || p->u_head_stride % 8)) fast = false;
+  }
+  if (n == 0 || max_tokens == 0) return KAM_OK;
+  if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
+
+  RelocGeom g{};
+  if (fast) { std::string why; if (!build_reloc_geom(c, max_rank, &g, &why)) fast = false; }
+
+  const size_t desc_bytes = (size_t)n * sizeof(RelocDescDev);
+  const size_t prefix_off = (desc_bytes + 15) & ~size_t(15);
+  const size_t total_bytes = prefix_off + (size_t)(n + 1) * sizeof(long long);
+  Staging* sg;
+  kam_status s = staging_acquire(c, total_bytes, &sg);
+  if (s != KAM_OK) return s;
+  RelocDescDev* dd = static_cast<RelocDescDev*>(sg->host);
+  long long* prefix = reinterpret_cast<long long*>(static_cast<char*>(sg->host) + prefix_off);
+  long long acc = 0;
+  for (int i = 0; i < n; ++i) {
+    const HostReloc& h = hs[i];
+    RelocDescDev d{};
+    const kam_patch* p = (h.patch && h.rank > 0) ? h.patch : nullptr;
+    d.k_src = h.k; d.v_src = h.v;
+    d.Uk = p ? p->Uk : nullptr; d.Wk = p ? p->Wk : nullptr;
+    d.Uv = (p && L.has_v) ? p->Uv : nullptr; d.Wv = (p && L.has_v) ? p->Wv : nullptr;
+    d.block_table = h.bt; d.dst_token_start = h.dst0; d.delta = h.delta;
+    d.u_token_stride = p ? p->u_token_stride : 0; d.u_head_stride = p ? p->u_head_stride : 0;
+    d.n_tokens = h.n_tokens;
+    d.flags = h.flags | ((p && p->frame == KAM_PATCH_CANONICAL_FRAME) ? FLAG_CANONICAL_FRAME : 0);
+    for (int l = 0; l < L.n_layers; ++l) d.rank_l[l] = (uint8_t)(p ? (p->rank_per_layer ? p->rank_per_layer[l] : h.rank) : 0);
+    dd[i] = d;
+    prefix[i] = acc;
+    if (fast) acc += (long long)L.n_layers * g.n_hg * ((h.n_tokens + g.TT - 1) / g.TT);
+  }
+  prefix[n] = acc;
+  if ((s = staging_commit(c, sg, total_bytes, st)) != KAM_OK) return s;
+  const RelocDescDev* d_descs = static_cast<const RelocDescDev*>(sg->dev);
+
+  if (fast) {
+    RelocParams p{};
+    p.descs = d_descs;
+    p.tile_prefix = reinterpret_cast<const long long*>(static_cast<const char*>(sg->dev) + prefix_off);
+    p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;
+    p.total_tiles = acc; p.n_descs = n;
+    const int grid = (int)std::min<long long>(c->sm_count, acc);
+    launch_relocate_fast(g, p, grid, st);
+  } else {
+    GenericParams p{};
+    p.descs = d_descs; p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;
+    p.n_descs = n; p.L = L.n_layers; p.H = L.n_kv_heads; p.D = L.row_dim; p.P = L.page_size;
+    p.rope_off = L.rope_off; p.d_r = L.rope_dim; p.rope_style = L.rope_style; p.has_v = L.has_v;
+    p.elem_f32 = L.elem_dtype == KAM_F32; p.factor_f32 = L.factor_dtype == KAM_F32; p.theta = L.rope_theta;
+    launch_relocate_generic(p, max_tokens, st);
+  }
+  ++c->kernels_launched;
+  cudaError_t e = cudaGetLastError();
+  staging_release(sg, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, fast ? "kam_relocate_patch_kernel launch" : "kam_relocate_patch_generic_kernel launch");
+  return KAM_OK;
+}
+
+kam_status validate_layout(const kam_layout* L) {
+  if (!L) return fail(nullptr, KAM_ERR_INVALID_ARG, "layout is NULL");
+  if (L->kind < KAM_MHA || L->kind > KAM_MLA) return fail(nullptr, KAM_ERR_INVALID_ARG, "unknown layout kind");
+  if (L->n_layers < 1 || L->n_layers > KAM_MAX_LAYERS) return fail(nullptr, KAM_ERR_INVALID_ARG, "n_layers outside [1, %d]", KAM_MAX_LAYERS);
+  if (L->n_kv_heads < 1 || L->n_q_heads < 1 || L->n_q_heads % L->n_kv_heads) return fail(nullptr, KAM_ERR_INVALID_ARG, "n_q_heads must be a positive multiple of n_kv_heads");
+  if (L->row_dim < 8 || L->row_dim % 8) return fail(nullptr, KAM_ERR_INVALID_ARG, "row_dim must be a positive multiple of 8");
+  if (L->rope_dim < 0 || L->rope_dim % 2) return fail(nullptr, KAM_ERR_INVALID_ARG, "rope_dim must be even");
+  if (L->rope_off < 0 || L->rope_off + L->rope_dim > L->row_dim) return fail(nullptr, KAM_ERR_INVALID_ARG, "rope band outside the row");
+  if (L->rope_dim > 512) return fail(nullptr, KAM_ERR_UNSUPPORTED, "rope_dim > 512");
+  if (L->page_size < 1) return fail(nullptr, KAM_ERR_INVALID_ARG, "page_size < 1");
+  if (L->rope_style != KAM_ROPE_HALF && L->rope_style != KAM_ROPE_INTERLEAVED) return fail(nullptr, KAM_ERR_INVALID_ARG, "unknown rope style");
+  if ((L->elem_dtype != KAM_BF16 && L->elem_dtype != KAM_F32) || (L->factor_dtype != KAM_BF16 && L->factor_dtype != KAM_F32))
+    return fail(nullptr, KAM_ERR_INVALID_ARG, "unknown dtype");
+  if (!(L->rope_theta > 0)) return fail(nullptr, KAM_ERR_INVALID_ARG, "rope_theta must be positive");
+  if (L->kind == KAM_MHA && L->n_q_heads != L->n_kv_heads) return fail(nullptr, KAM_ERR_INVALID_ARG, "MHA needs n_q_heads == n_kv_heads");
+  if (!L->has_v && (L->v_dim < 0 || L->v_dim > L->row_dim)) return fail(nullptr, KAM_ERR_INVALID_ARG, "v_dim outside the row");
+  return KAM_OK;
+}
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+const char* kam_version(void) { return "libkamera 0.1 (sm_100a)"; }
+
+const char* kam_last_error(const kam_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t max_requests,
+                      int32_t max_chunks_per_request, int32_t max_pages_per_chunk, kam_ctx** out) {
+  if (!out) return fail(nullptr, KAM_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  kam_status s = validate_layout(layout);
+  if (s != KAM_OK) return s;
+  if (max_requests < 0 || max_chunks_per_request < 0 || max_pages_per_chunk < 0)
+    return fail(nullptr, KAM_ERR_INVALID_ARG, "negative window-store size");
+  if (pool && (pool->num_pages < 0 || !pool->k_layers || (layout->has_v && !pool->v_layers)))
+    return fail(nullptr, KAM_ERR_INVALID_ARG, "bad pool");
+  kam_ctx* c = new (std::nothrow) kam_ctx();
+  if (!c) return fail(nullptr, KAM_ERR_STATE, "out of host memory");
+  c->lay = *layout;
+  c->fast_layout = build_head_blocks(c);
+  c->max_requests = max_requests; c->max_chunks = max_chunks_per_request; c->max_ppc = max_pages_per_chunk;
+  if (pool) { c->pool = *pool; c->has_pool = true; }
+  if (pool) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "kam_create: no usable CUDA device"); delete c; return r; }
+    c->cuda_ok = true;
+  }
+  if (max_requests > 0 && max_chunks_per_request > 0 && max_pages_per_chunk > 0) {
+    const int32_t np = pool ? pool->num_pages : max_requests * max_chunks_per_request * max_pages_per_chunk;
+    c->win.reset(new WindowStore(np, layout->page_size, max_requests, max_chunks_per_request, max_pages_per_chunk));
+    if (c->cuda_ok) {
+      const size_t bytes = (size_t)max_requests * max_chunks_per_request * max_pages_per_chunk * sizeof(int32_t);
+      cudaError_t e = cudaMalloc(&c->d_slot_pages, bytes);
+      if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "cudaMalloc(page lists)"); delete c; return r; }
+    }
+  }
+  *out = c;
+  return KAM_OK;
+}
+
+kam_status kam_destroy(kam_ctx* c) {
+  if (!c) return KAM_OK;
+  if (c->cuda_ok) {
+    for (Staging& s : c->staging) {
+      if (s.in_flight) cudaEventSynchronize(s.ev);
+      if (s.ev) cudaEventDestroy(s.ev);
+      if (s.host) cudaFreeHost(s.host);
+      if (s.dev) cudaFree(s.dev);
+    }
+    if (c->d_slot_pages) cudaFree(c->d_slot_pages);
+    if (c->d_ws) cudaFree(c->d_ws);
+    if (c->d_hstage) cudaFree(c->d_hstage);
+  }
+  delete c;
+  return KAM_OK;
+}
+
+kam_status kam_get_stats(kam_ctx* c, kam_stats* out) {
+  if (!c || !out) return fail(c, KAM_ERR_INVALID_ARG, "NULL argument");
+  kam_stats s{};
+  if (c->win) {
+    s.pages_free = c->win->pages_free(); s.pages_total = c->win->pages_total();
+    s.table_entries_written = c->win->table_entries_written(); s.chunks_live = c->win->chunks_live();
+  }
+  s.kernels_launched = c->kernels_launched;
+  *out = s;
+  return KAM_OK;
+}
+
+// ---- stateless operator -------------------------------------------------------------------------------------------
+kam_status kam_relocate_patch_batch(kam_ctx* c, const kam_pool* pool, int32_t n, const kam_reloc_desc* descs, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (n < 0 || (n > 0 && !descs)) return fail(c, KAM_ERR_INVALID_ARG, "bad descriptor array");
+  kam_status s = check_pool(c, &pool);
+  if (s != KAM_OK) return s;
+  std::vector<HostReloc> hs((size_t)n);
+  for (int i = 0; i < n; ++i) {
+    const kam_reloc_desc& d = descs[i];
+    if (!d.chunk) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: chunk is NULL", i);
+    hs[i] = HostReloc{d.block_table, d.dst_token_start, d.p_target - d.chunk->p_base, d.chunk->k_layers,
+                      d.chunk->v_layers, d.patch, d.rank, d.chunk->n_tokens, 0};
+  }
+  return run_reloc(c, pool, hs, static_cast<cudaStream_t>(stream));
+}
+
+kam_status kam_relocate_patch(kam_ctx* c, const kam_pool* pool, const int32_t* block_table, int64_t dst_token_start,
+                              const kam_chunk* chunk, int64_t p_target, const kam_patch* patch, int32_t rank, void* stream) {
+  kam_reloc_desc d{block_table, dst_token_start, chunk, p_target, patch, rank};
+  return kam_relocate_patch_batch(c, pool, 1, &d, stream);
+}
+
+kam_status kam_rotate_inplace(kam_ctx* c, const kam_pool* pool, const int32_t* block_table, int64_t token_start,
+                              int32_t n_tokens, int64_t delta, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  kam_status s = check_pool(c, &pool);
+  if (s != KAM_OK) return s;
+  std::vector<HostReloc> hs(1);
+  hs[0] = HostReloc{block_table, token_start, delta, nullptr, nullptr, nullptr, 0, n_tokens, FLAG_INPLACE};
+  return run_reloc(c, pool, hs, static_cast<cudaStream_t>(stream));
+}
+
+// ---- window store ---------------------------------------------------------------------------------------------------
+static kam_status win_status(kam_ctx* c, WindowStore::Result r, const char* what) {
+  switch (r) {
+    case WindowStore::OK: return KAM_OK;
+    case WindowStore::BAD_ARG: return fail(c, KAM_ERR_INVALID_ARG, "%s: invalid argument", what);
+    case WindowStore::BAD_STATE: return fail(c, KAM_ERR_STATE, "%s: request not open / already open / window empty or full", what);
+    case WindowStore::NO_PAGES: return fail(c, KAM_ERR_NO_PAGES, "%s: free list exhausted", what);
+  }
+  return KAM_ERR_STATE;
+}
+#define KAM_NEED_WIN(c)                                                                       \
+  if (!(c)) return KAM_ERR_INVALID_ARG;                                                       \
+  if (!(c)->win) return fail((c), KAM_ERR_STATE, "context was created without a window store")
+
+kam_status kam_window_open(kam_ctx* c, int32_t req, int64_t window_base) {
+  KAM_NEED_WIN(c);
+  return win_status(c, c->win->open(req, window_base), "kam_window_open");
+}
+kam_status kam_window_pin(kam_ctx* c, int32_t req, int32_t n_front) {
+  KAM_NEED_WIN(c);
+  return win_status(c, c->win->pin(req, n_front), "kam_window_pin");
+}
+kam_status kam_window_close(kam_ctx* c, int32_t req) {
+  KAM_NEED_WIN(c);
+  return win_status(c, c->win->close(req), "kam_window_close");
+}
+
+static kam_status rotate_survivors(kam_ctx* c, const std::vector<Rotation>& rot, cudaStream_t st) {
+  if (rot.empty() || !c->cuda_ok) return KAM_OK;
+  std::vector<HostReloc> hs(rot.size());
+  for (size_t i = 0; i < rot.size(); ++i)
+    hs[i] = HostReloc{c->d_slot_pages + (size_t)rot[i].slot * c->max_ppc, 0, rot[i].delta, nullptr, nullptr, nullptr, 0,
+                      rot[i].n_tokens, FLAG_INPLACE};
+  const kam_pool* pool = &c->pool;
+  return run_reloc(c, pool, hs, st);
+}
+
+kam_status kam_admit(kam_ctx* c, int32_t req, int32_t end, const kam_chunk* chunk, const kam_patch* patch, int32_t rank,
+                     int32_t materialize, int32_t* handle_out, void* stream) {
+  KAM_NEED_WIN(c);
+  if (!chunk) return fail(c, KAM_ERR_INVALID_ARG, "chunk is NULL");
+  { kam_status vs = validate_patch(c, patch, rank, 0); if (vs != KAM_OK) return vs; }
+  if (c->cuda_ok && (!chunk->k_layers || (c->lay.has_v && !chunk->v_layers)))
+    return fail(c, KAM_ERR_INVALID_ARG, "chunk layer-pointer arrays must not be NULL");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  ChunkRec rec; int64_t p_target = 0; std::vector<Rotation> rot;
+  kam_status s = win_status(c, c->win->admit(req, end, chunk->n_tokens, materialize != 0, &rec, &p_target, &rot), "kam_admit");
+  if (s != KAM_OK) return s;
+  if (handle_out) *handle_out = rec.handle;
+  if (!c->cuda_ok) return KAM_OK;                     // bookkeeping-only context
+  // device mirror of the chunk's page list: exactly n_tokens / P entries are written (O(1) in the window length)
+  const int32_t np = rec.n_tokens / c->lay.page_size;
+  int32_t* d_pages = c->d_slot_pages + (size_t)rec.slot * c->max_ppc;
+  Staging* sg;
+  if ((s = staging_acquire(c, (size_t)np * 4, &sg)) != KAM_OK) return s;
+  memcpy(sg->host, c->win->pages_of(rec.slot), (size_t)np * 4);
+  cudaError_t e = cudaMemcpyAsync(d_pages, sg->host, (size_t)np * 4, cudaMemcpyHostToDevice, st);
+  staging_release(sg, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(page list)");
+  // survivors first (they only touch their own pages), then Eq. 1 for the admitted chunk
+  if ((s = rotate_survivors(c, rot, st)) != KAM_OK) return s;
+  std::vector<HostReloc> hs(1);
+  hs[0] = HostReloc{d_pages, 0, p_target - chunk->p_base, chunk->k_layers, chunk->v_layers, patch, rank, chunk->n_tokens, 0};
+  const kam_pool* pool = &c->pool;
+  return run_reloc(c, pool, hs, st);
+}
+
+kam_status kam_evict(kam_ctx* c, int32_t req, int32_t end, int32_t materialize, void* stream) {
+  KAM_NEED_WIN(c);
+  std::vector<Rotation> rot;
+  kam_status s = win_status(c, c->win->evict(req, end, materialize != 0, nullptr, &rot), "kam_evict");
+  if (s != KAM_OK) return s;
+  return rotate_survivors(c, rot, static_cast<cudaStream_t>(stream));
+}
+
+kam_status kam_window_export(kam_ctx* c, int32_t req, int32_t* bt_out, int32_t bt_cap, int64_t* sm_out, int64_t sm_cap,
+                             int32_t* starts_out, int64_t* offs_out, int32_t* handles_out, int32_t chunk_cap,
+                             int32_t* n_pages_out, int32_t* n_chunks_out) {
+  KAM_NEED_WIN(c);
+  if (!c->win->is_open(req)) return fail(c, KAM_ERR_STATE, "kam_window_export: request not open");
+  const auto& ch = c->win->chunks(req);
+  const int P = c->lay.page_size;
+  int64_t n_tok = 0; int32_t n_pages = 0;
+  for (const ChunkRec& r : ch) { n_tok += r.n_tokens; n_pages += r.n_tokens / P; }
+  const int32_t nc = (int32_t)ch.size();
+  if ((bt_out && bt_cap < n_pages) || (sm_out && sm_cap < n_tok) ||
+      ((starts_out || offs_out || handles_out) && chunk_cap < nc))
+    return fail(c, KAM_ERR_INVALID_ARG, "kam_window_export: output capacity too small");
+  int64_t pos = c->win->window_base(req), tok = 0; int32_t pg = 0, i = 0;
+  for (const ChunkRec& r : ch) {
+    const int32_t* pages = c->win->pages_of(r.slot);
+    const int32_t np = r.n_tokens / P;
+    if (bt_out) memcpy(bt_out + pg, pages, (size_t)np * 4);
+    if (sm_out) for (int32_t t = 0; t < r.n_tokens; ++t) sm_out[tok + t] = (int64_t)pages[t / P] * P + t % P;
+    if (starts_out) starts_out[i] = (int32_t)tok;
+    if (offs_out) offs_out[i] = pos - r.phase;
+    if (handles_out) handles_out[i] = r.handle;
+    pg += np; tok += r.n_tokens; pos += r.n_tokens; ++i;
+  }
+  if (starts_out) starts_out[nc] = (int32_t)tok;
+  if (n_pages_out) *n_pages_out = n_pages;
+  if (n_chunks_out) *n_chunks_out = nc;
+  return KAM_OK;
+}
+
+}  // extern "C"

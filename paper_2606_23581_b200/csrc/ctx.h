@@ -1,0 +1,69 @@
+// kam_ctx and the helpers shared by the entry-point files.  Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "internal.h"
+#include "window.h"
+
+namespace kam {
+
+struct Staging {                 // pinned host + device buffer pair, reused round-robin behind an event
+  void* host = nullptr;
+  void* dev = nullptr;
+  size_t cap = 0;
+  cudaEvent_t ev = nullptr;
+  bool in_flight = false;
+};
+constexpr int kStagingSlots = 8;
+
+}  // namespace kam
+
+struct kam_ctx {
+  kam_layout lay;
+  kam_pool pool{};
+  bool has_pool = false;
+  bool cuda_ok = false;
+  int sm_count = 0;
+  std::string err;
+  int64_t kernels_launched = 0;
+
+  // relocate
+  bool fast_layout = false;
+  std::string fast_layout_why;
+  int blocks_per_head = 0;
+  kam::ColBlock head_blocks[kam::kMaxColBlocks];
+
+  kam::Staging staging[kam::kStagingSlots];
+  int staging_next = 0;
+
+  // window store
+  std::unique_ptr<kam::WindowStore> win;
+  int32_t max_requests = 0, max_chunks = 0, max_ppc = 0;
+  int32_t* d_slot_pages = nullptr;            // device mirror [n_slots][max_ppc]
+
+  // decode: workspace (grown on demand) and the cached plan of the window store
+  void* d_ws = nullptr;
+  size_t ws_cap = 0;
+  void* d_winplan = nullptr;
+  size_t winplan_cap = 0;
+  uint64_t winplan_epoch = ~0ull;
+  std::vector<int32_t> winplan_reqs;
+  int32_t winplan_items = 0, winplan_max_splits = 0;
+  // device staging of host-resident chunks (kam_relocate_patch_host) and host-resident q/out (decode host variant)
+  void* d_hstage = nullptr;
+  size_t hstage_cap = 0;
+};
+
+namespace kam {
+kam_status fail(kam_ctx* ctx, kam_status st, const char* fmt, ...);
+kam_status cuda_fail(kam_ctx* ctx, cudaError_t e, const char* what);
+kam_status staging_acquire(kam_ctx* c, size_t bytes, Staging** out);
+kam_status staging_commit(kam_ctx* c, Staging* s, size_t bytes, cudaStream_t st);
+void staging_release(Staging* s, cudaStream_t st);
+kam_status check_pool(kam_ctx* c, const kam_pool** pool);
+kam_status grow_device(kam_ctx* c, void** buf, size_t* cap, size_t bytes, const char* what);
+}  // namespace kam

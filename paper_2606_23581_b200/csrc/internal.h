@@ -1,0 +1,129 @@
+// Host/device records shared between the libkamera entry points and its kernels.  Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/kamera.h"
+
+namespace kam {
+
+// ---------------------------------------------------------------- relocate + patch
+// One chunk of a (batched) relocate call, as the kernels see it.
+struct RelocDescDev {
+  const void* const* k_src;      // device array [L] -> [T][H][D]; unused when FLAG_INPLACE
+  const void* const* v_src;
+  const void* const* Uk;         // device arrays [L] or nullptr
+  const void* const* Wk;
+  const void* const* Uv;
+  const void* const* Wv;
+  const int32_t* block_table;    // device
+  long long dst_token_start;
+  long long delta;               // p_target - p_base
+  long long u_token_stride;      // elements
+  long long u_head_stride;       // elements; 0 => U shared by all heads
+  int32_t n_tokens;
+  int32_t flags;
+  uint8_t rank_l[KAM_MAX_LAYERS];
+};
+enum : int32_t { FLAG_INPLACE = 1, FLAG_CANONICAL_FRAME = 2 };
+
+// A column block of a token's slice: what one warp processes for 16 tokens (up to 4 groups of 32 columns).
+struct ColBlock {
+  int16_t col_off;      // first column, relative to the slice
+  int16_t w_col_off;    // same column, relative to its head's row (index into W's last dim)
+  int16_t band_col0;    // column relative to the rope band start (rope blocks only)
+  int8_t n_groups;      // 2 or 4
+  int8_t fhead;         // head index inside the head group (selects U/W head)
+  int8_t rope;          // 1 if the block lies in the rope band
+  int8_t pad[3];
+};
+
+constexpr int kMaxColBlocks = 24;
+constexpr int kRelocConsumerWarps = 8;
+constexpr int kRelocThreads = (kRelocConsumerWarps + 1) * 32;
+
+struct RelocGeom {
+  int32_t L, H, D, P;
+  int32_t HG, n_hg;             // KV heads per slice, slices per token row
+  int32_t slice_bytes;          // HG * D * 2
+  int32_t row_bytes;            // H * D * 2 : one token of one layer in chunk and pool
+  int32_t s_row;                // padded shared-memory stride of a token's slice (== 64 mod 128)
+  int32_t su_row;               // padded shared-memory stride of a token's U run ((su_row/16) odd)
+  int32_t RB, TT;               // 16-token row blocks per tile; TT = 16 * RB tokens
+  int32_t nkv;                  // 2 with a V pool, 1 for MLA
+  int32_t n_blocks;
+  int32_t KT_max;               // max rank / 16 over the call
+  int32_t rope_style, d_r, half_groups;   // half_groups = d_r / 64 for HALF
+  int32_t n_stages;
+  int32_t off_cs, off_w, off_stage0, stage_bytes;   // byte offsets in dynamic shared memory
+  int32_t st_k, st_v, st_uk, st_uv, st_slot;        // offsets inside a stage
+  int32_t w_kv_stride;          // bytes of one of {K,V}'s fragment table
+  int32_t smem_bytes;
+  double theta;
+  ColBlock blk[kMaxColBlocks];
+};
+
+struct RelocParams {
+  const RelocDescDev* descs;
+  const long long* tile_prefix;  // [n_descs + 1]
+  void* const* pool_k;
+  void* const* pool_v;
+  long long total_tiles;
+  int32_t n_descs;
+};
+
+// generic (any dtype / rank / width) element-wise path
+struct GenericParams {
+  const RelocDescDev* descs;
+  void* const* pool_k;
+  void* const* pool_v;
+  int32_t n_descs, L, H, D, P, rope_off, d_r, rope_style, has_v, elem_f32, factor_f32;
+  double theta;
+};
+
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, int grid, cudaStream_t st);
+void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
+
+// ---------------------------------------------------------------- decode
+struct DecodeGeom {
+  int32_t Hq, H, G, D, Dv, P;
+  int32_t HG, n_hg;
+  int32_t rope_off, d_r, rope_style;
+  int32_t has_v;
+  int32_t row_bytes, slice_bytes, s_row;
+  int32_t TT, n_stages, stage_bytes, st_k, st_v, st_uk, st_uv, st_slot, su_row;
+  int32_t off_q, off_stage0, smem_bytes;
+  int32_t split_tokens;
+  int32_t max_rank;
+  double theta;
+};
+
+struct DecodeItem {            // one (request, chunk, split) = a contiguous token range of one chunk
+  int32_t b, chunk;            // request index in the batch, chunk index in the request
+  int32_t tok0, n_tok;         // logical tokens [tok0, tok0 + n_tok) of the request
+  int32_t split;               // partial slot within the request
+  int32_t ctok0;               // first token relative to the chunk start (indexes U on read)
+  long long delta;
+};
+
+struct DecodeParams {
+  const void* q;               // [B][Hq][D] bf16
+  const void* pool_k;          // this layer
+  const void* pool_v;
+  const int32_t* block_tables; // [B][max_pages]  (or the window store's per-request rows)
+  int32_t max_pages;
+  const DecodeItem* items;
+  const int32_t* n_items;      // device scalar
+  int32_t* work_counter;       // device scalar, zeroed by the planner
+  const kam_patch_ref* patches;// [B][max_chunks] or nullptr
+  int32_t max_chunks;
+  float* part_o;               // [B][Hq][max_splits][Dv]
+  float* part_lse;             // [B][Hq][max_splits]
+  const int32_t* n_splits;     // [B]
+  int32_t max_splits;
+  float sm_scale;
+  void* out; float* lse;
+  int32_t batch;
+};
+
+}  // namespace kam
