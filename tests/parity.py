@@ -16,7 +16,7 @@ from oracle import reuse
 from oracle.bf16 import bf16_bits, bf16_from_bits, bf16_rne, ulp_bf16
 from paper_2606_23581_b200 import binding as B
 
-SENTINEL = 1234.0
+SENTINEL = 1248.0          # exactly representable in bf16
 
 
 def layout_of(cfg, n_layers=None, style=B.KAM_ROPE_HALF, elem=None, factor=None):
