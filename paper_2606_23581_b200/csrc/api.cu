@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <memory>
 #include <new>
@@ -89,6 +90,8 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, RelocGeom* out, std::strin
   RelocGeom g{};
   g.L = L.n_layers; g.H = L.n_kv_heads; g.D = L.row_dim; g.P = L.page_size;
   g.row_bytes = g.H * g.D * 2;
+  g.P_shift = -1;
+  for (int sft = 0; sft < 31; ++sft) if ((1 << sft) == g.P) g.P_shift = sft;
   g.nkv = L.has_v ? 2 : 1;
   g.KT_max = max_rank / 16;
   g.rope_style = L.rope_style; g.d_r = L.rope_dim; g.half_groups = L.rope_dim / 64;
@@ -102,7 +105,9 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, RelocGeom* out, std::strin
     RelocGeom t = g;
     t.HG = HG; t.n_hg = g.H / HG; t.n_blocks = NB;
     t.slice_bytes = HG * g.D * 2;
-    t.s_row = t.slice_bytes + ((64 - t.slice_bytes % 128) + 128) % 128;      // == 64 (mod 128): conflict-free LDS.128
+    t.contig = (HG == g.H) && c->contig_copies;
+    // padded rows (== 64 mod 128) make the 128-bit row loads conflict-free; unpadded rows allow one copy per tile
+    t.s_row = t.contig ? t.slice_bytes : t.slice_bytes + ((64 - t.slice_bytes % 128) + 128) % 128;
     t.su_row = g.KT_max ? HG * max_rank * 2 + 16 : 0;                          // (su_row / 16) odd
     t.RB = std::min(4, std::max(1, (kRelocConsumerWarps + t.nkv * NB - 1) / (t.nkv * NB)));
     t.TT = 16 * t.RB;
@@ -112,10 +117,12 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, RelocGeom* out, std::strin
     t.st_uv = t.st_uk + t.TT * t.su_row;
     t.st_slot = t.st_uv + (t.nkv == 2 ? t.TT * t.su_row : 0);
     t.stage_bytes = align_up(t.st_slot + t.TT * 4, 128);
-    t.w_kv_stride = NB * g.KT_max * 4096;
-    t.off_cs = 128;
+    t.w_row = (g.D + 8) * 2;
+    t.w_kv_stride = HG * max_rank * t.w_row;
+    t.off_tab = 128;
+    t.off_cs = t.off_tab + 256 + align_up(NB * 16, 128);
     t.off_w = t.off_cs + align_up(std::max(1, g.d_r / 2) * 8, 128);
-    t.off_stage0 = t.off_w + t.nkv * t.w_kv_stride;
+    t.off_stage0 = align_up(t.off_w + t.nkv * t.w_kv_stride, 128);
     for (int i = 0; i < NB; ++i) {
       ColBlock b = c->head_blocks[i % c->blocks_per_head];
       const int h = i / c->blocks_per_head;
@@ -332,6 +339,7 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
   if (!c) return fail(nullptr, KAM_ERR_STATE, "out of host memory");
   c->lay = *layout;
   c->fast_layout = build_head_blocks(c);
+  if (const char* e = getenv("KAM_RELOC_CONTIG")) c->contig_copies = (e[0] != '0');
   c->max_requests = max_requests; c->max_chunks = max_chunks_per_request; c->max_ppc = max_pages_per_chunk;
   if (pool) { c->pool = *pool; c->has_pool = true; }
   if (pool) {

@@ -40,10 +40,13 @@ struct ColBlock {
 
 constexpr int kMaxColBlocks = 24;
 constexpr int kRelocConsumerWarps = 8;
-constexpr int kRelocThreads = (kRelocConsumerWarps + 1) * 32;
+constexpr int kRelocProducerWarps = 4;     // K rows | V rows | U_k | U_v
+constexpr int kRelocThreads = (kRelocConsumerWarps + kRelocProducerWarps) * 32;
 
 struct RelocGeom {
   int32_t L, H, D, P;
+  int32_t P_shift;              // log2(P) if P is a power of two, else -1
+  int32_t contig;               // 1: slice == whole token row and shared-memory rows are unpadded (one copy per tile)
   int32_t HG, n_hg;             // KV heads per slice, slices per token row
   int32_t slice_bytes;          // HG * D * 2
   int32_t row_bytes;            // H * D * 2 : one token of one layer in chunk and pool
@@ -55,7 +58,8 @@ struct RelocGeom {
   int32_t KT_max;               // max rank / 16 over the call
   int32_t rope_style, d_r, half_groups;   // half_groups = d_r / 64 for HALF
   int32_t n_stages;
-  int32_t off_cs, off_w, off_stage0, stage_bytes;   // byte offsets in dynamic shared memory
+  int32_t off_tab, off_cs, off_w, off_stage0, stage_bytes;   // byte offsets in dynamic shared memory
+  int32_t w_row;                // bytes of one k-row of W in shared memory: (D + 8) * 2
   int32_t st_k, st_v, st_uk, st_uv, st_slot;        // offsets inside a stage
   int32_t w_kv_stride;          // bytes of one of {K,V}'s fragment table
   int32_t smem_bytes;
