@@ -374,6 +374,7 @@ kam_status kam_destroy(kam_ctx* c) {
     if (c->d_slot_pages) cudaFree(c->d_slot_pages);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_hstage) cudaFree(c->d_hstage);
+    if (c->d_hstage2) cudaFree(c->d_hstage2);
   }
   delete c;
   return KAM_OK;
@@ -421,6 +422,65 @@ kam_status kam_rotate_inplace(kam_ctx* c, const kam_pool* pool, const int32_t* b
   std::vector<HostReloc> hs(1);
   hs[0] = HostReloc{block_table, token_start, delta, nullptr, nullptr, nullptr, 0, n_tokens, FLAG_INPLACE};
   return run_reloc(c, pool, hs, static_cast<cudaStream_t>(stream));
+}
+
+kam_status kam_relocate_patch_host(kam_ctx* c, const kam_pool* pool, const int32_t* block_table, int64_t dst_token_start,
+                                   int32_t n_tokens, int64_t p_base, int64_t p_target, const void* const* k_host,
+                                   const void* const* v_host, const void* const* Uk_host, const void* const* Wk_host,
+                                   const void* const* Uv_host, const void* const* Wv_host, int32_t rank, int32_t frame,
+                                   void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  kam_status s = check_pool(c, &pool);
+  if (s != KAM_OK) return s;
+  const kam_layout& L = c->lay;
+  if (!k_host || (L.has_v && !v_host)) return fail(c, KAM_ERR_INVALID_ARG, "host chunk arrays must not be NULL");
+  if (rank < 0 || rank > KAM_MAX_RANK) return fail(c, KAM_ERR_INVALID_ARG, "rank %d outside [0, %d]", rank, KAM_MAX_RANK);
+  if (rank > 0 && (!Uk_host || !Wk_host || (L.has_v && (!Uv_host || !Wv_host))))
+    return fail(c, KAM_ERR_INVALID_ARG, "host factor arrays must not be NULL when rank > 0");
+  if (n_tokens < 0 || !block_table || dst_token_start < 0) return fail(c, KAM_ERR_INVALID_ARG, "bad token range / block table");
+  if (n_tokens == 0) return KAM_OK;
+  if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t eb = L.elem_dtype == KAM_BF16 ? 2 : 4, fb = L.factor_dtype == KAM_BF16 ? 2 : 4;
+  const size_t rows = ((size_t)n_tokens * L.n_kv_heads * L.row_dim * eb + 255) & ~size_t(255);
+  const size_t ub = ((size_t)n_tokens * L.n_kv_heads * rank * fb + 255) & ~size_t(255);
+  const size_t wb = ((size_t)L.n_kv_heads * rank * L.row_dim * fb + 255) & ~size_t(255);
+  const int nkv = L.has_v ? 2 : 1;
+  const size_t per_layer = nkv * (rows + ub + wb);
+  if ((s = grow_device(c, &c->d_hstage, &c->hstage_cap, per_layer * L.n_layers, "cudaMalloc(host-chunk staging)")) != KAM_OK) return s;
+  // device pointer tables for the staged copy: [k | v | Uk | Wk | Uv | Wv][n_layers]
+  Staging* sg;
+  if ((s = staging_acquire(c, (size_t)6 * L.n_layers * sizeof(void*), &sg)) != KAM_OK) return s;
+  const void** tabs = static_cast<const void**>(sg->host);
+  char* d = static_cast<char*>(c->d_hstage);
+  cudaError_t e = cudaSuccess;
+  auto put = [&](int which, int l, const void* const* src, size_t bytes, size_t& off) {
+    tabs[which * L.n_layers + l] = nullptr;
+    if (!src || bytes == 0) return;
+    tabs[which * L.n_layers + l] = d + off;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d + off, src[l], bytes, cudaMemcpyHostToDevice, st);
+  };
+  for (int l = 0; l < L.n_layers; ++l) {
+    size_t off = per_layer * l;
+    put(0, l, k_host, (size_t)n_tokens * L.n_kv_heads * L.row_dim * eb, off); off += rows;
+    if (L.has_v) { put(1, l, v_host, (size_t)n_tokens * L.n_kv_heads * L.row_dim * eb, off); off += rows; } else tabs[1 * L.n_layers + l] = nullptr;
+    put(2, l, rank ? Uk_host : nullptr, (size_t)n_tokens * L.n_kv_heads * rank * fb, off); off += ub;
+    put(3, l, rank ? Wk_host : nullptr, (size_t)L.n_kv_heads * rank * L.row_dim * fb, off); off += wb;
+    if (L.has_v) {
+      put(4, l, rank ? Uv_host : nullptr, (size_t)n_tokens * L.n_kv_heads * rank * fb, off); off += ub;
+      put(5, l, rank ? Wv_host : nullptr, (size_t)L.n_kv_heads * rank * L.row_dim * fb, off);
+    } else { tabs[4 * L.n_layers + l] = nullptr; tabs[5 * L.n_layers + l] = nullptr; }
+  }
+  if (e != cudaSuccess) { staging_release(sg, st); return cuda_fail(c, e, "cudaMemcpyAsync(host chunk)"); }
+  if ((s = staging_commit(c, sg, (size_t)6 * L.n_layers * sizeof(void*), st)) != KAM_OK) return s;
+  staging_release(sg, st);          // NOTE: the tables stay valid until this staging slot is reused (8 calls later)
+  const void* const* dt = static_cast<const void* const*>(sg->dev);
+  kam_chunk ch{dt, L.has_v ? dt + L.n_layers : nullptr, n_tokens, p_base};
+  kam_patch pa{dt + 2 * L.n_layers, dt + 3 * L.n_layers, L.has_v ? dt + 4 * L.n_layers : nullptr,
+               L.has_v ? dt + 5 * L.n_layers : nullptr, (int64_t)L.n_kv_heads * rank, rank, nullptr, frame};
+  std::vector<HostReloc> hs(1);
+  hs[0] = HostReloc{block_table, dst_token_start, p_target - p_base, ch.k_layers, ch.v_layers, rank ? &pa : nullptr, rank, n_tokens, 0};
+  return run_reloc(c, pool, hs, st);
 }
 
 // ---- window store ---------------------------------------------------------------------------------------------------

@@ -57,6 +57,8 @@ struct kam_ctx {
   // device staging of host-resident chunks (kam_relocate_patch_host) and host-resident q/out (decode host variant)
   void* d_hstage = nullptr;
   size_t hstage_cap = 0;
+  void* d_hstage2 = nullptr;
+  size_t hstage2_cap = 0;
 };
 
 namespace kam {

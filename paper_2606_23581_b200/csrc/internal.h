@@ -89,45 +89,56 @@ void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, int grid, cu
 void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
 
 // ---------------------------------------------------------------- decode
+constexpr int kDecTT = 32;                 // tokens per pipeline stage
+constexpr int kDecMaxHG = 4;               // KV heads (= compute warps) per CTA
+
 struct DecodeGeom {
-  int32_t Hq, H, G, D, Dv, P;
-  int32_t HG, n_hg;
+  int32_t Hq, H, G, D, Dv, P, P_shift;
+  int32_t HG, n_hg;              // KV heads per work unit, units per token row
   int32_t rope_off, d_r, rope_style;
-  int32_t has_v;
-  int32_t row_bytes, slice_bytes, s_row;
-  int32_t TT, n_stages, stage_bytes, st_k, st_v, st_uk, st_uv, st_slot, su_row;
-  int32_t off_q, off_stage0, smem_bytes;
+  int32_t row_bytes, slice_bytes, s_row;      // s_row: padded stride of a token's slice in shared memory ((s_row/16) odd)
+  int32_t n_stages, stage_bytes, st_k, st_v, st_uk, st_uv, st_hdr, su_row;
+  int32_t off_warp, off_stage0, smem_bytes;   // off_warp: per-warp scratch (sin/cos table, z / y staging)
+  int32_t warp_bytes;
   int32_t split_tokens;
-  int32_t max_rank;
+  int32_t max_rank;              // 0: no on-read patch in this call
   double theta;
 };
 
-struct DecodeItem {            // one (request, chunk, split) = a contiguous token range of one chunk
-  int32_t b, chunk;            // request index in the batch, chunk index in the request
-  int32_t tok0, n_tok;         // logical tokens [tok0, tok0 + n_tok) of the request
-  int32_t split;               // partial slot within the request
-  int32_t ctok0;               // first token relative to the chunk start (indexes U on read)
-  long long delta;
+struct DecodeItem {              // one split = a contiguous token range inside ONE chunk of one request
+  long long bt_off;              // index of the page list's first entry in the block-table array
+  long long delta;               // RoPE offset to apply on read
+  int32_t b, chunk;              // request index in the batch, chunk index in the request
+  int32_t tok0, n_tok;           // tokens [tok0, tok0 + n_tok) of that page list
+  int32_t split;                 // partial slot within the request
+  int32_t ctok0;                 // first token relative to the chunk start (indexes U when patching on read)
 };
 
 struct DecodeParams {
-  const void* q;               // [B][Hq][D] bf16
-  const void* pool_k;          // this layer
-  const void* pool_v;
-  const int32_t* block_tables; // [B][max_pages]  (or the window store's per-request rows)
-  int32_t max_pages;
+  const void* q;                 // [B][Hq][D] bf16
+  void* const* pool_k_layers;    // device arrays of per-layer page bases; the kernel reads entry `layer`
+  void* const* pool_v_layers;
+  int32_t layer;
+  const int32_t* block_tables;
   const DecodeItem* items;
-  const int32_t* n_items;      // device scalar
-  int32_t* work_counter;       // device scalar, zeroed by the planner
-  const kam_patch_ref* patches;// [B][max_chunks] or nullptr
+  const int32_t* n_items;        // device scalar
+  int32_t* work_counter;         // device scalar, zero on entry
+  const kam_patch_ref* patches;  // [B][max_chunks] or nullptr
   int32_t max_chunks;
-  float* part_o;               // [B][Hq][max_splits][Dv]
-  float* part_lse;             // [B][Hq][max_splits]
-  const int32_t* n_splits;     // [B]
+  float* part_o;                 // [B][Hq][max_splits][Dv]
+  float* part_lse;               // [B][Hq][max_splits]
+  const int32_t* n_splits;       // [B]
   int32_t max_splits;
   float sm_scale;
-  void* out; float* lse;
+  void* out;                     // [B][Hq][Dv] bf16
+  float* lse;                    // [B][Hq]
   int32_t batch;
 };
+
+void launch_decode_plan(const int32_t* chunk_starts, const long long* chunk_offsets, const int32_t* n_chunks,
+                        int32_t max_chunks, int32_t max_pages, int32_t batch, int32_t split_tokens, int32_t max_splits,
+                        DecodeItem* items, int32_t* n_items, int32_t* n_splits, int32_t* work_counter, cudaStream_t st);
+void launch_decode(const DecodeGeom& g, const DecodeParams& p, int grid, cudaStream_t st);
+void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st);
 
 }  // namespace kam
