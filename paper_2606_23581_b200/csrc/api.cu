@@ -1,6 +1,7 @@
 // libkamera C entry points: argument validation, host bookkeeping, descriptor staging, kernel launches.
 // Every step of the hot path runs in the kernels (relocate_kernel.cu, decode_kernel.cu); this file only decides
 // geometry and marshals descriptors.  No CPU fallback exists: without CUDA every compute entry fails.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -297,6 +298,52 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
   return KAM_OK;
 }
 
+// TMA tensor maps over the pool, one per (layer, K|V): dims (64 columns, slots, 64-column blocks) so that a box of
+// (64, 16 tokens, column blocks of a head group) lands in shared memory as [column block][token][128 B], SWIZZLE_128B.
+typedef CUresult (*PFN_tmapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                        const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                        CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+void build_pool_tensor_maps(kam_ctx* c) {
+  const kam_layout& L = c->lay;
+  if (getenv("KAM_DECODE_NO_TMA")) { c->tmap_why = "disabled by KAM_DECODE_NO_TMA"; return; }
+  if (L.elem_dtype != KAM_BF16 || !L.has_v) { c->tmap_why = "needs a bf16 K/V pool"; return; }
+  if (L.page_size % 16 || (L.row_dim != 64 && L.row_dim != 128)) { c->tmap_why = "needs page_size % 16 == 0 and head_dim 64/128"; return; }
+  if (c->pool.num_pages < 1) { c->tmap_why = "empty pool"; return; }
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError(); c->tmap_why = "cuTensorMapEncodeTiled not available"; return;
+  }
+  PFN_tmapEncodeTiled encode = reinterpret_cast<PFN_tmapEncodeTiled>(fn);
+  std::vector<void*> kp(L.n_layers), vp(L.n_layers);
+  if (cudaMemcpy(kp.data(), c->pool.k_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess ||
+      cudaMemcpy(vp.data(), c->pool.v_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess) {
+    cudaGetLastError(); c->tmap_why = "could not read the pool's layer pointers"; return;
+  }
+  int HG = 1;
+  for (int h = std::min(L.n_kv_heads, kDecMaxHG); h >= 1; --h) if (L.n_kv_heads % h == 0) { HG = h; break; }
+  const cuuint64_t gdim[3] = {64, (cuuint64_t)c->pool.num_pages * L.page_size, (cuuint64_t)L.n_kv_heads * L.row_dim / 64};
+  const cuuint64_t gstride[2] = {(cuuint64_t)L.n_kv_heads * L.row_dim * 2, 128};
+  const cuuint32_t box[3] = {64, 16, (cuuint32_t)(HG * L.row_dim / 64)};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  std::vector<CUtensorMap> maps((size_t)2 * L.n_layers);
+  for (int l = 0; l < L.n_layers; ++l)
+    for (int kv = 0; kv < 2; ++kv) {
+      CUresult r = encode(&maps[2 * l + kv], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv ? vp[l] : kp[l], gdim, gstride, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) { c->tmap_why = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r); return; }
+    }
+  static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
+  if (cudaMalloc(&c->d_tmaps, maps.size() * sizeof(CUtensorMap)) != cudaSuccess ||
+      cudaMemcpy(c->d_tmaps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaGetLastError();
+    if (c->d_tmaps) { cudaFree(c->d_tmaps); c->d_tmaps = nullptr; }
+    c->tmap_why = "could not upload tensor maps";
+  }
+}
+
 kam_status validate_layout(const kam_layout* L) {
   if (!L) return fail(nullptr, KAM_ERR_INVALID_ARG, "layout is NULL");
   if (L->kind < KAM_MHA || L->kind > KAM_MLA) return fail(nullptr, KAM_ERR_INVALID_ARG, "unknown layout kind");
@@ -348,6 +395,7 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "kam_create: no usable CUDA device"); delete c; return r; }
     c->cuda_ok = true;
+    build_pool_tensor_maps(c);
   }
   if (max_requests > 0 && max_chunks_per_request > 0 && max_pages_per_chunk > 0) {
     const int32_t np = pool ? pool->num_pages : max_requests * max_chunks_per_request * max_pages_per_chunk;
@@ -375,6 +423,7 @@ kam_status kam_destroy(kam_ctx* c) {
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_hstage) cudaFree(c->d_hstage);
     if (c->d_hstage2) cudaFree(c->d_hstage2);
+    if (c->d_tmaps) cudaFree(c->d_tmaps);
   }
   delete c;
   return KAM_OK;

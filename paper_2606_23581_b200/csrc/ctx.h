@@ -46,6 +46,9 @@ struct kam_ctx {
   int32_t max_requests = 0, max_chunks = 0, max_ppc = 0;
   int32_t* d_slot_pages = nullptr;            // device mirror [n_slots][max_ppc]
 
+  // decode: TMA tensor maps over the context's pool ([n_layers][K,V], 128 bytes each, device memory)
+  void* d_tmaps = nullptr;
+  std::string tmap_why;                        // why the TMA path is off, if it is
   // decode: workspace (grown on demand) and the cached plan of the window store
   void* d_ws = nullptr;
   size_t ws_cap = 0;

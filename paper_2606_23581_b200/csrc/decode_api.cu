@@ -11,7 +11,7 @@ namespace {
 
 inline int align_up(int x, int a) { return (x + a - 1) / a * a; }
 
-kam_status decode_geom(kam_ctx* c, DecodeGeom* out) {
+kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
   const kam_layout& L = c->lay;
   if (L.elem_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "decode needs a bf16 pool");
   if (!L.has_v) return fail(c, KAM_ERR_UNSUPPORTED, "decode over an MLA latent pool is not built yet (SURVEY.md 8(f) f1)");
@@ -28,12 +28,20 @@ kam_status decode_geom(kam_ctx* c, DecodeGeom* out) {
   g.n_hg = g.H / g.HG;
   g.rope_off = L.rope_off; g.d_r = L.rope_dim; g.rope_style = L.rope_style; g.theta = L.rope_theta;
   g.row_bytes = g.H * g.D * 2; g.slice_bytes = g.HG * g.D * 2;
+  g.use_tma = c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers;
+  g.ncb = g.HG * g.D / 64; g.box_bytes = 2048 * g.ncb;
   g.s_row = g.slice_bytes + 16;                                   // (s_row / 16) odd: ldmatrix rows never share a bank group
-  g.st_k = 0; g.st_v = kDecTT * g.s_row; g.st_hdr = 2 * kDecTT * g.s_row;
-  g.stage_bytes = align_up(g.st_hdr + 16, 128);
   g.off_warp = 128;
   g.warp_bytes = align_up(std::max(1, g.d_r / 2) * 8, 128);
-  g.off_stage0 = align_up(g.off_warp + g.HG * g.warp_bytes, 128);
+  if (g.use_tma) {                                                // two 16-token boxes for K, two for V, 1024-byte aligned
+    g.st_k = 0; g.st_v = 2 * g.box_bytes; g.st_hdr = 4 * g.box_bytes;
+    g.stage_bytes = align_up(g.st_hdr + 16, 1024);
+    g.off_stage0 = align_up(g.off_warp + g.HG * g.warp_bytes, 1024);
+  } else {
+    g.st_k = 0; g.st_v = kDecTT * g.s_row; g.st_hdr = 2 * kDecTT * g.s_row;
+    g.stage_bytes = align_up(g.st_hdr + 16, 128);
+    g.off_stage0 = align_up(g.off_warp + g.HG * g.warp_bytes, 128);
+  }
   g.n_stages = std::min(6, (220 * 1024 - g.off_stage0) / g.stage_bytes);
   if (g.n_stages < 2) return fail(c, KAM_ERR_UNSUPPORTED, "decode tile does not fit shared memory");
   g.smem_bytes = g.off_stage0 + g.n_stages * g.stage_bytes;
@@ -81,7 +89,7 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   if (batch == 0) return KAM_OK;
   if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
   DecodeGeom g;
-  if ((s = decode_geom(c, &g)) != KAM_OK) return s;
+  if ((s = decode_geom(c, pool, &g)) != KAM_OK) return s;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
 
   g.split_tokens = pick_split(c, g, (long long)batch * max_pages * g.P);
@@ -92,7 +100,7 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
 
   DecodeParams p{};
   p.q = q; p.pool_k_layers = pool->k_layers; p.pool_v_layers = pool->v_layers; p.layer = layer;
-  p.block_tables = block_tables;
+  p.block_tables = block_tables; p.tmaps = c->d_tmaps;
   p.items = reinterpret_cast<DecodeItem*>(ws + w.items);
   p.n_items = reinterpret_cast<int32_t*>(ws + w.scalars);
   p.work_counter = reinterpret_cast<int32_t*>(ws + w.scalars) + 1;
@@ -125,7 +133,7 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
     if (!c->win->is_open(req_ids[b])) return fail(c, KAM_ERR_STATE, "request %d is not open", req_ids[b]);
   if (batch == 0) return KAM_OK;
   DecodeGeom g;
-  kam_status s = decode_geom(c, &g);
+  kam_status s = decode_geom(c, &c->pool, &g);
   if (s != KAM_OK) return s;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
 
@@ -170,7 +178,7 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
 
   DecodeParams p{};
   p.q = q; p.pool_k_layers = c->pool.k_layers; p.pool_v_layers = c->pool.v_layers; p.layer = layer;
-  p.block_tables = c->d_slot_pages;
+  p.block_tables = c->d_slot_pages; p.tmaps = c->d_tmaps;
   p.items = reinterpret_cast<DecodeItem*>(ws + w.items);
   p.n_items = reinterpret_cast<int32_t*>(ws + w.scalars);
   p.work_counter = reinterpret_cast<int32_t*>(ws + w.scalars) + 1;

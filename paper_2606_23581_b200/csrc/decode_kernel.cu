@@ -99,8 +99,14 @@ __device__ __forceinline__ float quad_sum(float v) {
 }
 }  // namespace
 
-// KS = D / 16 (k-steps of QK^T; D = Dv).
-template <int KS>
+// KS = D / 16 (k-steps of QK^T; D = Dv).  TMA: pool pages arrive as swizzled 16-token tensor-map boxes.
+//
+// TMA path shared-memory layout of one box: [64-column block c][token r (16)][128 bytes], SWIZZLE_128B, i.e. the 16-byte
+// chunk j of (c, r) sits at (c*16 + r)*128 + ((j ^ (r & 7)) << 4): eight consecutive tokens of one chunk hit eight
+// different bank groups, so ldmatrix (K) and ldmatrix.trans (V) are conflict-free without padding.  Tiles are aligned
+// to 16 tokens of the page list (a box never straddles a page because P % 16 == 0); rows outside the split's token
+// range are masked in the softmax.
+template <int KS, bool TMA>
 __global__ void __launch_bounds__((kDecMaxHG + 1) * 32, 1)
 kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
   extern __shared__ __align__(128) uint8_t smem[];
@@ -140,8 +146,40 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
       }
       const int item_idx = w / g.n_hg, hg = w - item_idx * g.n_hg;
       const DecodeItem it = p.items[item_idx];
-      const int n_tiles = (it.n_tok + kDecTT - 1) / kDecTT;
       const int32_t* bt = p.block_tables + it.bt_off;
+      if constexpr (TMA) {
+        const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * 256;
+        const char* tm_v = tm_k + 128;
+        const int a0 = it.tok0 & ~15, end = it.tok0 + it.n_tok;
+        const int n_tiles = (end - a0 + kDecTT - 1) / kDecTT;
+        for (int t = 0; t < n_tiles; ++t) {
+          const int base = a0 + t * kDecTT;
+          const int n_box = min(2, (end - base + 15) >> 4);
+          int slot0 = 0;
+          if (lane < n_box) {
+            const int tok = base + lane * 16;
+            const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
+            slot0 = bt[pg] * g.P + (tok - pg * g.P);
+          }
+          const int slot1 = __shfl_sync(0xffffffffu, slot0, 1);
+          mbar_wait(&empty_bar[stage], phase ^ 1);
+          if (lane == 0) {
+            uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
+            const int lo = max(it.tok0 - base, 0), hi = min(end - base, kDecTT);
+            *reinterpret_cast<int4*>(st + g.st_hdr) = make_int4(w, t, lo | (hi << 16), (t == 0 ? HDR_FIRST : 0) | (t == n_tiles - 1 ? HDR_LAST : 0));
+            mbar_arrive_expect_tx(&full_bar[stage], static_cast<uint32_t>(n_box) * g.box_bytes * 2u);
+            tma_load_3d(st + g.st_k, tm_k, 0, slot0, hg * g.ncb, &full_bar[stage]);
+            tma_load_3d(st + g.st_v, tm_v, 0, slot0, hg * g.ncb, &full_bar[stage]);
+            if (n_box > 1) {
+              tma_load_3d(st + g.st_k + g.box_bytes, tm_k, 0, slot1, hg * g.ncb, &full_bar[stage]);
+              tma_load_3d(st + g.st_v + g.box_bytes, tm_v, 0, slot1, hg * g.ncb, &full_bar[stage]);
+            }
+          }
+          if (++stage == g.n_stages) { stage = 0; phase ^= 1; }
+        }
+        continue;
+      }
+      const int n_tiles = (it.n_tok + kDecTT - 1) / kDecTT;
       const size_t off = static_cast<size_t>(hg) * g.slice_bytes;
       for (int t = 0; t < n_tiles; ++t) {
         // A1 slot mapping for the tile's 32 tokens, one per lane (issued before waiting for the stage)
@@ -156,7 +194,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
         mbar_wait(&empty_bar[stage], phase ^ 1);
         uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
         if (lane == 0) {
-          *reinterpret_cast<int4*>(st + g.st_hdr) = make_int4(w, t, nvalid, (t == 0 ? HDR_FIRST : 0) | (t == n_tiles - 1 ? HDR_LAST : 0));
+          *reinterpret_cast<int4*>(st + g.st_hdr) = make_int4(w, t, nvalid << 16, (t == 0 ? HDR_FIRST : 0) | (t == n_tiles - 1 ? HDR_LAST : 0));
           mbar_arrive_expect_tx(&full_bar[stage], static_cast<uint32_t>(nvalid) * g.slice_bytes * 2u);
         }
         __syncwarp();
@@ -187,8 +225,14 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
   int item_b = 0, item_split = 0, head = 0;
 
   // ldmatrix lane addressing inside a stage (bytes relative to the K / V region)
-  const uint32_t k_lane = ((lane & 7) + ((lane >> 4) & 1) * 8) * g.s_row + warp * D * 2 + ((lane >> 3) & 1) * 16;
-  const uint32_t v_lane = ((lane & 7) + ((lane >> 3) & 1) * 8) * g.s_row + warp * D * 2 + ((lane >> 4) & 1) * 16;
+  //   K (non-trans): matrices = (tokens 0-7 | 8-15 of a 16-token block) x (first | second 16-byte chunk of the k-step)
+  //   V (trans):     matrices = (tokens 0-7 | 8-15) x (first | second d n-tile of the pair)
+  const int k_row = (lane & 7) + ((lane >> 4) & 1) * 8, k_hi = (lane >> 3) & 1;
+  const int v_row = (lane & 7) + ((lane >> 3) & 1) * 8, v_hi = (lane >> 4) & 1;
+  const uint32_t k_lane = TMA ? (warp * (D / 64) * 16 + k_row) * 128 : k_row * g.s_row + warp * D * 2 + k_hi * 16;
+  const uint32_t v_lane = TMA ? (warp * (D / 64) * 16 + v_row) * 128 : v_row * g.s_row + warp * D * 2 + v_hi * 16;
+  const uint32_t k_sw = (k_hi ^ (lane & 7)) << 4, v_sw = (v_hi ^ (lane & 7)) << 4;   // swizzled chunk of k-step 0
+  const uint32_t blk16 = TMA ? g.box_bytes : 16 * g.s_row;                            // bytes between 16-token blocks
 
   int stage = 0; uint32_t phase = 0;
   while (true) {
@@ -196,7 +240,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
     const uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
     const int4 hdr = *reinterpret_cast<const int4*>(st + g.st_hdr);
     if (hdr.x < 0) break;
-    const int nvalid = hdr.z;
+    const int row_lo = hdr.z & 0xffff, row_hi = hdr.z >> 16;        // valid token rows of this tile
 
     if (hdr.w & HDR_FIRST) {
       // ---- new work unit: load the G query rows of this KV head, rotate them by -delta, split into bf16 hi + lo
@@ -274,7 +318,9 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
 #pragma unroll
       for (int np = 0; np < 2; ++np) {
         uint32_t b0, b1, b2, b3;
-        ldmatrix_x4(b0, b1, b2, b3, kb + np * 16 * g.s_row + ks * 32);
+        // chunk index of this k-step inside its 64-column block: (ks & 3) * 2 (+ k_hi), XOR-swizzled on the TMA path
+        ldmatrix_x4(b0, b1, b2, b3, TMA ? kb + np * blk16 + (ks >> 2) * 2048 + (k_sw ^ ((ks & 3) << 5))
+                                        : kb + np * blk16 + ks * 32);
         mma_bf16_16816(S[2 * np][0], S[2 * np][1], S[2 * np][2], S[2 * np][3], qhi[ks][0], qhi[ks][1], qhi[ks][2], qhi[ks][3], b0, b1);
         mma_bf16_16816(S[2 * np + 1][0], S[2 * np + 1][1], S[2 * np + 1][2], S[2 * np + 1][3], qhi[ks][0], qhi[ks][1], qhi[ks][2], qhi[ks][3], b2, b3);
         if (use_lo) {
@@ -289,7 +335,8 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
     for (int n = 0; n < 4; ++n) {
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
-        const bool ok = (n * 8 + 2 * t4 + e) < nvalid;
+        const int tr = n * 8 + 2 * t4 + e;
+        const bool ok = tr >= row_lo && tr < row_hi;
         S[n][e] = ok ? S[n][e] * scale_log2 : -CUDART_INF_F;
         S[n][2 + e] = ok ? S[n][2 + e] * scale_log2 : -CUDART_INF_F;
         mx0 = fmaxf(mx0, S[n][e]); mx1 = fmaxf(mx1, S[n][2 + e]);
@@ -321,7 +368,8 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
 #pragma unroll
       for (int dp = 0; dp < KS; ++dp) {
         uint32_t v0, v1, v2, v3;
-        ldmatrix_x4_trans(v0, v1, v2, v3, vb + j * 16 * g.s_row + dp * 32);
+        ldmatrix_x4_trans(v0, v1, v2, v3, TMA ? vb + j * blk16 + (dp >> 2) * 2048 + (v_sw ^ ((dp & 3) << 5))
+                                              : vb + j * blk16 + dp * 32);
         mma_bf16_16816(O[2 * dp][0], O[2 * dp][1], O[2 * dp][2], O[2 * dp][3], pa0, pa1, pa2, pa3, v0, v1);
         mma_bf16_16816(O[2 * dp + 1][0], O[2 * dp + 1][1], O[2 * dp + 1][2], O[2 * dp + 1][3], pa0, pa1, pa2, pa3, v2, v3);
       }
@@ -356,13 +404,12 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
 
 void launch_decode(const DecodeGeom& g, const DecodeParams& p, int grid, cudaStream_t st) {
   const int threads = (g.HG + 1) * 32;
-  if (g.D == 128) {
-    cudaFuncSetAttribute(kam_paged_decode_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    kam_paged_decode_kernel<8><<<grid, threads, g.smem_bytes, st>>>(g, p);
-  } else {
-    cudaFuncSetAttribute(kam_paged_decode_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    kam_paged_decode_kernel<4><<<grid, threads, g.smem_bytes, st>>>(g, p);
-  }
+  auto go = [&](auto kern) {
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    kern<<<grid, threads, g.smem_bytes, st>>>(g, p);
+  };
+  if (g.D == 128) { if (g.use_tma) go(kam_paged_decode_kernel<8, true>); else go(kam_paged_decode_kernel<8, false>); }
+  else            { if (g.use_tma) go(kam_paged_decode_kernel<4, true>); else go(kam_paged_decode_kernel<4, false>); }
 }
 
 // ---------------------------------------------------------------------------------------------------- merge

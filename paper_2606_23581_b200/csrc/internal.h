@@ -102,6 +102,8 @@ struct DecodeGeom {
   int32_t warp_bytes;
   int32_t split_tokens;
   int32_t max_rank;              // 0: no on-read patch in this call
+  int32_t use_tma;               // 1: pool pages arrive as 16-token swizzled TMA boxes; 0: one padded bulk copy per token
+  int32_t ncb, box_bytes;        // TMA path: 64-column blocks per slice, bytes of one 16-token box
   double theta;
 };
 
@@ -120,6 +122,7 @@ struct DecodeParams {
   void* const* pool_v_layers;
   int32_t layer;
   const int32_t* block_tables;
+  const void* tmaps;             // device array of CUtensorMap [n_layers][2] over the context's pool (TMA path)
   const DecodeItem* items;
   const int32_t* n_items;        // device scalar
   int32_t* work_counter;         // device scalar, zero on entry
