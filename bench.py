@@ -1,0 +1,413 @@
+#!/usr/bin/env python
+"""bench.py - the Kamera hot path on BASELINE.json configs[1] (GQA Qwen2-VL-7B-like, bf16), one JSON line.
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference]
+
+A STEP is one pass of the whole hot path over one batch of synthetic input:
+  phase A  kam_relocate_patch_batch : 8 chunks x 1024 tokens x 28 layers relocated to p ~ U[0, 32768) with their rank-16
+                                      patches into one request's pages, ONE launch           (A1-A5)   <- the headline metric
+  phase B  kam_evict + kam_admit    : the request's window slides: oldest chunk out (its 7 survivors re-rotate in place by
+                                      -1024), one evicted chunk recalled by relocate+patch      (A6, A7)
+  phase C  kam_window_decode        : fused paged decode over every request's 8192-token window, 28 layers, LSE merge (A8, A9)
+Inputs are resident in HBM before the timed region; every step touches > 1 GB of fresh source and destination memory
+(the B200 L2 is 126 MB), and the request / canonical set rotate from step to step.
+
+metric = relocate+patch GB/s: ALGORITHMIC bytes of phase A (page read + page write + U + W + block table)
+divided by the device time of phase A.  The other two headline figures (us per 1024-token chunk, decode tokens/s) and all
+three kernels' roofline fractions ride along in the same line.  N > 1: requests are sharded over ranks, no data-path
+collective (the path partitions by request), time = max over ranks, value = all ranks' bytes / that.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+CFG_ID = 2
+N_REQ = 8               # requests per GPU (decode batch; each owns an 8-chunk window)
+N_SETS = 2              # canonical chunk sets cycled so that sources miss L2
+
+
+def algorithmic_bytes_relocate(T, H, D, m, P, has_v=True):
+    """bytes(chunk, layer) = 2*nkv*T*H*D*2 + nkv*H*T*m*2 + nkv*H*m*D*2 + 4*T/P."""
+    nkv = 2 if has_v else 1
+    return 2 * nkv * T * H * D * 2 + nkv * H * T * m * 2 + nkv * H * m * D * 2 + 4 * (T // P)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.idx = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 9 for n, v in zip(names, r[5:9]) if v.lower().startswith("active")})
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------------- the workload
+class Workload:
+    def __init__(self, device, rank):
+        import numpy as np
+        import torch
+
+        import paper_2606_23581_b200 as kam
+        from paper_2606_23581_b200 import binding as B
+        from synth import CONFIGS, randn_device
+        self.torch, self.kam, self.B = torch, kam, B
+        cfg = self.cfg = CONFIGS[CFG_ID]
+        L, H, D, P, T, m = cfg.n_layers, cfg.n_kv_heads, cfg.row_dim, cfg.page_size, cfg.chunk_tokens, cfg.rank
+        self.n_chunks = cfg.chunks_per_step
+        self.rng = np.random.Generator(np.random.PCG64(cfg.seed + 1000 * rank))
+        seed = [cfg.seed * 100003 + 7919 * rank]
+
+        def rnd(shape, std):
+            seed[0] += 1
+            return randn_device(shape, seed[0], std, torch.bfloat16, device)
+
+        # canonical store: N_SETS x 8 position-free chunks + rank-16 factors, resident in HBM (K,V ~ N(0,1); U ~ N(0,1); W ~ N(0,.05))
+        self.sets = []
+        for _ in range(N_SETS):
+            cs = []
+            for _ in range(self.n_chunks):
+                ch = kam.Chunk([rnd((T, H, D), 1.0) for _ in range(L)], [rnd((T, H, D), 1.0) for _ in range(L)])
+                pa = kam.Patch([rnd((T, H, m), 1.0) for _ in range(L)], [rnd((H, m, D), cfg.w_std) for _ in range(L)],
+                               [rnd((T, H, m), 1.0) for _ in range(L)], [rnd((H, m, D), cfg.w_std) for _ in range(L)])
+                cs.append((ch, pa))
+            self.sets.append(cs)
+        ppc = T // P
+        lay = kam.make_layout(B.KAM_GQA, L, cfg.n_q_heads, H, D, cfg.rope_off, cfg.rope_dim, True, P, cfg.theta)
+        # pool A: target of the stateless batched operator (phase A); block table = random permutation of its pages
+        npa = N_REQ * self.n_chunks * ppc
+        self.pool_a = kam.Pool([torch.zeros((npa, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(L)],
+                               [torch.zeros((npa, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(L)])
+        self.ctx_a = kam.Context(lay, self.pool_a)
+        self.bt_a = torch.from_numpy(self.rng.permutation(npa).astype(np.int32)).to(device)
+        # pool B: the window store (phases B, C): N_REQ windows of 8 chunks (+1 chunk of slack while sliding)
+        npb = N_REQ * (self.n_chunks + 1) * ppc
+        self.pool_b = kam.Pool([torch.zeros((npb, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(L)],
+                               [torch.zeros((npb, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(L)])
+        self.ctx_b = kam.Context(lay, self.pool_b, max_requests=N_REQ, max_chunks_per_request=self.n_chunks + 1,
+                                 max_pages_per_chunk=ppc)
+        for r in range(N_REQ):
+            self.ctx_b.kam_window_open(r, 0)
+            for c in range(self.n_chunks):
+                ch, pa = self.sets[r % N_SETS][c]
+                self.ctx_b.kam_admit(r, B.KAM_BACK, ch, pa, m, 1)
+        self.q = rnd((N_REQ, cfg.n_q_heads, D), 1.0)
+        self.out = torch.zeros((N_REQ, cfg.n_q_heads, D), dtype=torch.bfloat16, device=device)
+        self.lse = torch.zeros((N_REQ, cfg.n_q_heads), dtype=torch.float32, device=device)
+        self.sm_scale = D ** -0.5
+        self.req_ids = list(range(N_REQ))
+        # algorithmic bytes
+        self.bytes_a = self.n_chunks * L * algorithmic_bytes_relocate(T, H, D, m, P)
+        self.bytes_b = (self.n_chunks - 1) * L * (2 * T * H * D * 2) + L * algorithmic_bytes_relocate(T, H, D, m, P)
+        self.bytes_c_layer = N_REQ * 2 * self.n_chunks * T * H * D * 2
+        self.bytes_c = L * self.bytes_c_layer
+        torch.cuda.synchronize()
+
+    def launches(self):
+        return self.ctx_a.kam_get_stats()["kernels_launched"] + self.ctx_b.kam_get_stats()["kernels_launched"]
+
+    def step(self, i, ev=None):
+        cfg, B, T, m = self.cfg, self.B, self.cfg.chunk_tokens, self.cfg.rank
+        r, cs = i % N_REQ, self.sets[i % N_SETS]
+        rec = (lambda k: ev[k].record()) if ev is not None else (lambda k: None)
+        rec(0)
+        # phase A: 8 chunks relocated+patched to random offsets, one launch
+        p = self.rng.integers(0, cfg.max_pos, size=self.n_chunks)
+        base = r * self.n_chunks * T
+        self.ctx_a.kam_relocate_patch_batch([(self.bt_a, base + c * T, cs[c][0], int(p[c]), cs[c][1], m) for c in range(self.n_chunks)])
+        rec(1)
+        # phase B: the window of request r slides by one chunk
+        self.ctx_b.kam_evict(r, B.KAM_FRONT, 1)
+        ch, pa = cs[i % self.n_chunks]
+        self.ctx_b.kam_admit(r, B.KAM_BACK, ch, pa, m, 1)
+        rec(2)
+        # phase C: every request decodes one token over its window, all layers
+        for l in range(cfg.n_layers):
+            self.ctx_b.kam_window_decode(self.q, self.req_ids, l, self.sm_scale, self.out, self.lse)
+        rec(3)
+
+
+class E2E:
+    """The same path through the C-ABI entries that take HOST buffers: canonical chunks and factors live in pinned host
+    memory (an off-device canonical store), H2D inside kam_relocate_patch_host; the decode query comes from the host
+    and out / lse go back to it inside kam_paged_decode_merge_host."""
+
+    def __init__(self, wl, device):
+        torch = wl.torch
+        cfg = wl.cfg
+        L, T = cfg.n_layers, cfg.chunk_tokens
+        self.wl = wl
+
+        def host(ts):
+            return [t.to("cpu").pin_memory() for t in ts]
+        self.chunks = []
+        for ch, pa in wl.sets[0]:
+            self.chunks.append((host(ch.k_layers), host(ch.v_layers), host(pa.t[0]), host(pa.t[1]), host(pa.t[2]), host(pa.t[3])))
+        self.h2d = sum(sum(t.numel() * t.element_size() for t in grp) for c in self.chunks for grp in c)
+        P = cfg.page_size
+        n_pages = wl.n_chunks * T // P
+        self.bt = wl.bt_a[:n_pages].contiguous().reshape(1, -1)
+        self.starts = torch.arange(0, (wl.n_chunks + 1) * T, T, dtype=torch.int32, device=device).reshape(1, -1)
+        self.nc = torch.tensor([wl.n_chunks], dtype=torch.int32, device=device)
+        self.q_h = wl.q[:1].to("cpu").pin_memory()
+        self.out_h = torch.zeros((1, cfg.n_q_heads, cfg.row_dim), dtype=torch.bfloat16).pin_memory()
+        self.lse_h = torch.zeros((1, cfg.n_q_heads), dtype=torch.float32).pin_memory()
+        self.h2d += L * self.q_h.numel() * 2
+        self.d2h = L * (self.out_h.numel() * 2 + self.lse_h.numel() * 4)
+
+    def step(self, i):
+        wl, cfg = self.wl, self.wl.cfg
+        T, m = cfg.chunk_tokens, cfg.rank
+        p = wl.rng.integers(0, cfg.max_pos, size=wl.n_chunks)
+        for c, (k, v, uk, wk, uv, wv) in enumerate(self.chunks):
+            wl.ctx_a.kam_relocate_patch_host(self.bt.reshape(-1), c * T, T, 0, int(p[c]), k, v, uk, wk, uv, wv, m)
+        for l in range(cfg.n_layers):
+            wl.ctx_a.kam_paged_decode_merge_host(self.q_h, self.bt, self.starts, None, self.nc, l, wl.sm_scale, self.out_h, self.lse_h)
+
+
+# ------------------------------------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample(n_chunks, n_layers, seed=1):
+    """Times oracle/reuse.py (as it stands) on n_chunks x n_layers (chunk, layer) units of config 2.  Returns (GB/s, seconds)."""
+    import numpy as np
+    import torch
+
+    from oracle import reuse
+    from synth import CONFIGS, make_chunk
+    cfg = CONFIGS[CFG_ID]
+    rng = np.random.Generator(np.random.PCG64(seed))
+    T, H, D, P, m = cfg.chunk_tokens, cfg.n_kv_heads, cfg.row_dim, cfg.page_size, cfg.rank
+    chunks = [make_chunk(cfg, rng, n_layers=n_layers) for _ in range(n_chunks)]
+    f = lambda t: t.to(torch.float64).numpy()
+    pool_k = np.zeros((T // P, P, H, D), np.uint16); pool_v = np.zeros_like(pool_k)
+    bt = rng.permutation(T // P).astype(np.int32)
+    t0 = time.perf_counter()
+    for ch in chunks:
+        p = int(rng.integers(0, cfg.max_pos))
+        for l in range(n_layers):
+            reuse.relocate_patch_layer(pool_k, pool_v, bt, 0, f(ch["K"][l]), f(ch["V"][l]), p, f(ch["Uk"][l]), f(ch["Wk"][l]),
+                                       f(ch["Uv"][l]), f(ch["Wv"][l]), theta=cfg.theta, rope_off=cfg.rope_off, d_r=cfg.rope_dim)
+    dt = time.perf_counter() - t0
+    nbytes = n_chunks * n_layers * algorithmic_bytes_relocate(T, H, D, m, P)
+    return nbytes / dt / 1e9, dt
+
+
+def cpu_threads():
+    try:
+        import torch
+        return int(torch.get_num_threads())
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    """--impl reference: this tier has no reference implementation; the arm is the fp64 CPU oracle, as it stands, on the
+    host cores, each step a bounded sample (1 chunk x 2 layers) of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vals = []
+    for i in range(args.warmup + args.steps):
+        gbs, dt = oracle_sample(1, 2, seed=i)
+        if i >= args.warmup:
+            vals.append((gbs, dt))
+    tot_t = sum(d for _, d in vals)
+    value = sum(g * d for g, d in vals) / tot_t
+    sample = "1 chunk x 2 layers of config 2 per step (of 8 chunks x 28 layers)"
+    print(json.dumps({
+        "impl": "reference", "metric": "relocate+patch GB/s", "value": value, "unit": "GB/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(1, len(vals)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": "BASELINE.json configs[1] GQA Qwen2-VL-7B-like", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "GB/s", "cores": cpu_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------------------- main
+def max_over_ranks(x, world):
+    """Largest value of x over all ranks (device timing is reduced this way; works on NCCL and gloo alike)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([x], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x, world):
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([x], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(3, args.warmup)
+
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libkamera has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+
+    wl = Workload(device, rank)
+    peak, peak_src = peaks()
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        wl.step(i)
+    barrier()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    l0 = wl.launches()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record()
+    for i in range(args.steps):
+        wl.step(args.warmup + i, ev[i])
+    t_end.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = (wl.launches() - l0) // args.steps
+    total_ms = max_over_ranks(t_start.elapsed_time(t_end), world)
+    ms = {k: sum(e[k].elapsed_time(e[k + 1]) for e in ev) / args.steps for k in range(3)}
+    ms_a = max_over_ranks(ms[0], world); ms_b = max_over_ranks(ms[1], world); ms_c = max_over_ranks(ms[2], world)
+    n_ranks_bytes_a = sum_over_ranks(wl.bytes_a, world)
+    value = n_ranks_bytes_a / (ms_a * 1e-3) / 1e9
+
+    # e2e: same path through the host-buffer entries
+    e2e = None
+    if not args.no_e2e:
+        ee = E2E(wl, device)
+        for i in range(2):
+            ee.step(i)
+        barrier()
+        n_e = max(2, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for i in range(n_e):
+            ee.step(i)
+        torch.cuda.synchronize()
+        dt = max_over_ranks((time.perf_counter() - t0) / n_e, world)
+        e2e = {"value": sum_over_ranks(wl.bytes_a, world) / dt / 1e9, "unit": "GB/s", "h2d_bytes_per_step": ee.h2d, "d2h_bytes_per_step": ee.d2h,
+               "ms_per_step": dt * 1e3, "what": "8 x kam_relocate_patch_host (pinned host chunks+factors -> H2D -> kernel) + 28 x "
+               "kam_paged_decode_merge_host (q H2D, out/lse D2H) per step; relocate+patch bytes / whole region"}
+
+    cfg = wl.cfg
+    L, T = cfg.n_layers, cfg.chunk_tokens
+    gb = lambda b, t_ms: b / (t_ms * 1e-3) / 1e9
+    kernels = {
+        "kam_relocate_patch_kernel": {"bound": "hbm", "achieved": gb(wl.bytes_a, ms[0]), "bytes_per_launch": wl.bytes_a, "ms_per_launch": ms[0],
+                                      "share_of_step": ms[0] / (ms[0] + ms[1] + ms[2])},
+        "window_slide(evict+admit)": {"bound": "hbm", "achieved": gb(wl.bytes_b, ms[1]), "bytes_per_launch": wl.bytes_b / 2, "ms_per_launch": ms[1] / 2,
+                                      "share_of_step": ms[1] / (ms[0] + ms[1] + ms[2])},
+        "kam_paged_decode_kernel(+merge)": {"bound": "hbm", "achieved": gb(wl.bytes_c, ms[2]), "bytes_per_launch": wl.bytes_c_layer, "ms_per_launch": ms[2] / L,
+                                            "share_of_step": ms[2] / (ms[0] + ms[1] + ms[2])},
+    }
+    for k in kernels.values():
+        k.update({"peak": peak, "unit": "GB/s", "frac": k["achieved"] / peak})
+    dom = max(kernels, key=lambda k: kernels[k]["share_of_step"])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic_r01.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(dom.split("(")[0])
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["achieved"], "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": traffic}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        gbs, dt = oracle_sample(2, L)
+        cpu = {"value": gbs, "unit": "GB/s", "cores": cpu_threads(), "kind": "oracle", "seconds": dt,
+               "sample": "relocate+patch of 2 chunks x 28 layers of config 2 (of 8 chunks per step), oracle/reuse.py in numpy fp64"}
+
+    if rank == 0:
+        out = {
+            "metric": "relocate+patch GB/s", "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[1]: GQA Qwen2-VL-7B-like, 28 layers, 28q/4kv heads, head_dim 128, theta 1e6, "
+                                   "8 chunks x 1024 tokens per slide, rank-16 patch, page 16, offsets U[0,32768)",
+                       "requests_per_gpu": N_REQ, "decode_batch": N_REQ, "window_tokens": wl.n_chunks * T,
+                       "l2": "inputs larger than L2: each step streams >1 GB of fresh source and destination; request and canonical set rotate",
+                       "parallelism": "requests sharded over ranks, no collective"},
+            "phases_ms": {"relocate_patch_batch": ms_a, "window_slide": ms_b, "decode_all_layers": ms_c},
+            "us_per_1024tok_chunk": 1e3 * ms_a / wl.n_chunks,
+            "decode_tok_per_s": world * N_REQ / (ms_c * 1e-3),
+            "decode_note": "attention only: batch / (per-layer attention time x 28 layers); projections and MLP are not part of the method",
+            "step_gbs": sum_over_ranks(wl.bytes_a + wl.bytes_b + wl.bytes_c, world) / (total_ms / args.steps * 1e-3) / 1e9 if world == 1 else None,
+            "roofline": roofline, "roofline_all": kernels, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        }
+        print(json.dumps(out))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
