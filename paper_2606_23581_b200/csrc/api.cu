@@ -8,6 +8,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <memory>
 #include <new>
@@ -321,8 +322,7 @@ void build_pool_tensor_maps(kam_ctx* c) {
       cudaMemcpy(vp.data(), c->pool.v_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess) {
     cudaGetLastError(); c->tmap_why = "could not read the pool's layer pointers"; return;
   }
-  int HG = 1;
-  for (int h = std::min(L.n_kv_heads, kDecMaxHG); h >= 1; --h) if (L.n_kv_heads % h == 0) { HG = h; break; }
+  const int HG = decode_head_group(L);
   const cuuint64_t gdim[3] = {64, (cuuint64_t)c->pool.num_pages * L.page_size, (cuuint64_t)L.n_kv_heads * L.row_dim / 64};
   const cuuint64_t gstride[2] = {(cuuint64_t)L.n_kv_heads * L.row_dim * 2, 128};
   const cuuint32_t box[3] = {64, 16, (cuuint32_t)(HG * L.row_dim / 64)};
@@ -396,6 +396,15 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
     if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "kam_create: no usable CUDA device"); delete c; return r; }
     c->cuda_ok = true;
     build_pool_tensor_maps(c);
+    if (const char* ev = getenv("KAM_DEC_CTAS_PER_SM")) c->dec_ctas_per_sm = atoi(ev);
+    if (const char* ev = getenv("KAM_DEC_BOXES")) c->dec_boxes = atoi(ev);
+    if (layout->rope_dim > 0) {                // f_i = theta^(-2i/d_r) in fp64, once (R-2)
+      std::vector<double> f((size_t)layout->rope_dim / 2);
+      for (size_t i = 0; i < f.size(); ++i) f[i] = pow(layout->rope_theta, -2.0 * (double)i / layout->rope_dim);
+      e = cudaMalloc(&c->d_inv_freq, f.size() * sizeof(double));
+      if (e == cudaSuccess) e = cudaMemcpy(c->d_inv_freq, f.data(), f.size() * sizeof(double), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "kam_create: inverse-frequency table"); kam_destroy(c); return r; }
+    }
   }
   if (max_requests > 0 && max_chunks_per_request > 0 && max_pages_per_chunk > 0) {
     const int32_t np = pool ? pool->num_pages : max_requests * max_chunks_per_request * max_pages_per_chunk;
@@ -424,6 +433,7 @@ kam_status kam_destroy(kam_ctx* c) {
     if (c->d_hstage) cudaFree(c->d_hstage);
     if (c->d_hstage2) cudaFree(c->d_hstage2);
     if (c->d_tmaps) cudaFree(c->d_tmaps);
+    if (c->d_inv_freq) cudaFree(c->d_inv_freq);
   }
   delete c;
   return KAM_OK;

@@ -49,14 +49,14 @@ struct kam_ctx {
   // decode: TMA tensor maps over the context's pool ([n_layers][K,V], 128 bytes each, device memory)
   void* d_tmaps = nullptr;
   std::string tmap_why;                        // why the TMA path is off, if it is
-  // decode: workspace (grown on demand) and the cached plan of the window store
+  // decode: workspace (grown on demand); the plan of the window store stays cached in it between layers
   void* d_ws = nullptr;
   size_t ws_cap = 0;
-  void* d_winplan = nullptr;
-  size_t winplan_cap = 0;
-  uint64_t winplan_epoch = ~0ull;
+  uint64_t winplan_epoch = ~0ull;              // window epoch the plan in d_ws was built for (~0 = none)
   std::vector<int32_t> winplan_reqs;
-  int32_t winplan_items = 0, winplan_max_splits = 0;
+  int32_t winplan_chunks = 0;
+  double* d_inv_freq = nullptr;                // [rope_dim / 2] f_i = theta^(-2i/d_r), fp64
+  int dec_ctas_per_sm = 0, dec_boxes = 0;      // tuning switches (KAM_DEC_CTAS_PER_SM, KAM_DEC_BOXES); 0 = automatic
   // device staging of host-resident chunks (kam_relocate_patch_host) and host-resident q/out (decode host variant)
   void* d_hstage = nullptr;
   size_t hstage_cap = 0;

@@ -9,8 +9,9 @@ using namespace kam;
 
 namespace {
 
-inline int align_up(int x, int a) { return (x + a - 1) / a * a; }
+inline size_t align_up_sz(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Geometry of the decode kernel for this context's layout; `ctas_per_sm` = 0 picks the densest configuration that fits.
 kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
   const kam_layout& L = c->lay;
   if (L.elem_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "decode needs a bf16 pool");
@@ -23,52 +24,75 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
   g.Hq = L.n_q_heads; g.H = L.n_kv_heads; g.G = G; g.D = L.row_dim; g.Dv = L.row_dim; g.P = L.page_size;
   g.P_shift = -1;
   for (int s = 0; s < 31; ++s) if ((1 << s) == g.P) g.P_shift = s;
-  g.HG = 1;
-  for (int hgc = std::min(g.H, kDecMaxHG); hgc >= 1; --hgc) if (g.H % hgc == 0) { g.HG = hgc; break; }
+  g.HG = decode_head_group(L);
   g.n_hg = g.H / g.HG;
-  g.rope_off = L.rope_off; g.d_r = L.rope_dim; g.rope_style = L.rope_style; g.theta = L.rope_theta;
+  g.R = g.HG * g.G;
+  g.NT = (G + 7) / 8;
+  g.rope_off = L.rope_off; g.d_r = L.rope_dim; g.rope_style = L.rope_style;
   g.row_bytes = g.H * g.D * 2; g.slice_bytes = g.HG * g.D * 2;
   g.use_tma = c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers;
-  g.ncb = g.HG * g.D / 64; g.box_bytes = 2048 * g.ncb;
+  g.ncb = g.HG * g.D / 64;
   g.s_row = g.slice_bytes + 16;                                   // (s_row / 16) odd: ldmatrix rows never share a bank group
-  g.off_warp = 128;
-  g.warp_bytes = align_up(std::max(1, g.d_r / 2) * 8, 128);
-  if (g.use_tma) {                                                // two 16-token boxes for K, two for V, 1024-byte aligned
-    g.st_k = 0; g.st_v = 2 * g.box_bytes; g.st_hdr = 4 * g.box_bytes;
-    g.stage_bytes = align_up(g.st_hdr + 16, 1024);
-    g.off_stage0 = align_up(g.off_warp + g.HG * g.warp_bytes, 1024);
-  } else {
-    g.st_k = 0; g.st_v = kDecTT * g.s_row; g.st_hdr = 2 * kDecTT * g.s_row;
-    g.stage_bytes = align_up(g.st_hdr + 16, 128);
-    g.off_stage0 = align_up(g.off_warp + g.HG * g.warp_bytes, 128);
+  g.box_bytes = g.use_tma ? 2048 * g.ncb : (int)align_up_sz((size_t)kDecTile * g.s_row, 128);
+  g.off_hdr = 128; g.off_box0 = 1024;
+  // CTAs per SM x ring depth: 3 CTAs with 2 K + 2 V boxes each when that fits, else fewer CTAs with a deeper ring
+  const int sm_total = 227 * 1024;
+  int want = c->dec_ctas_per_sm > 0 ? c->dec_ctas_per_sm : 3;
+  for (; want >= 1; --want) {
+    const int budget = sm_total / want - 1024 - g.off_box0;
+    int nb = std::min(8, budget / g.box_bytes) & ~1;
+    if (c->dec_boxes > 0) nb = std::min(nb, c->dec_boxes & ~1);
+    if (nb < 2) continue;
+    if (nb < 4 && want > 1) continue;
+    g.n_boxes = nb;
+    g.smem_bytes = g.off_box0 + nb * g.box_bytes;
+    if (decode_occupancy(g) >= want) break;
   }
-  g.n_stages = std::min(6, (220 * 1024 - g.off_stage0) / g.stage_bytes);
-  if (g.n_stages < 2) return fail(c, KAM_ERR_UNSUPPORTED, "decode tile does not fit shared memory");
-  g.smem_bytes = g.off_stage0 + g.n_stages * g.stage_bytes;
+  if (want < 1) return fail(c, KAM_ERR_UNSUPPORTED, "decode tile does not fit shared memory");
+  g.n_ctas = c->sm_count * want;
   *out = g;
   return KAM_OK;
 }
 
-// workspace layout in c->d_ws
-struct WsLayout { size_t items, scalars, n_splits, part_lse, part_o, total; };
-WsLayout ws_layout(const DecodeGeom& g, int batch, int max_splits) {
+// workspace layout in c->d_ws: plan arrays first (chunks | rcb are what the window path uploads), then the partials
+struct WsLayout { size_t chunks, rcb, tile_pre, seg_base, cta_seg, segs, cs, part_lse, part_o, total; int max_segs; };
+WsLayout ws_layout(const DecodeGeom& g, int n_chunks, int batch) {
   WsLayout w{};
   size_t off = 0;
-  w.items = off; off += (size_t)batch * max_splits * sizeof(DecodeItem); off = (off + 255) & ~size_t(255);
-  w.scalars = off; off += 256;
-  w.n_splits = off; off += (size_t)batch * 4; off = (off + 255) & ~size_t(255);
-  w.part_lse = off; off += (size_t)batch * g.Hq * max_splits * 4; off = (off + 255) & ~size_t(255);
-  w.part_o = off; off += (size_t)batch * g.Hq * max_splits * g.Dv * 4;
+  auto take = [&](size_t bytes) { const size_t o = off; off = align_up_sz(off + bytes, 256); return o; };
+  w.max_segs = g.n_ctas + g.n_hg * n_chunks;
+  w.chunks = take((size_t)n_chunks * sizeof(DecChunk));
+  w.rcb = take((size_t)(batch + 1) * 4);
+  w.tile_pre = take((size_t)(n_chunks + 1) * 4);
+  w.seg_base = take(((size_t)g.n_hg * n_chunks + 1) * 4);
+  w.cta_seg = take((size_t)(g.n_ctas + 1) * 4);
+  w.segs = take((size_t)w.max_segs * sizeof(DecSeg));
+  w.cs = take((size_t)n_chunks * std::max(1, g.d_r / 2) * sizeof(float2));
+  w.part_lse = take((size_t)w.max_segs * g.R * 4);
+  w.part_o = take((size_t)w.max_segs * g.R * g.Dv * 4);
   w.total = off;
   return w;
 }
 
-int pick_split(const kam_ctx* c, const DecodeGeom& g, long long token_bound) {
-  // aim at >= 16 work units per SM; splits are powers of two between 256 and 4096 tokens
-  long long per = token_bound * g.n_hg / std::max(1, c->sm_count * 16);
-  int s = 256;
-  while (s < 4096 && s < per) s <<= 1;
-  return s;
+DecodePlan plan_of(kam_ctx* c, const WsLayout& w, int n_chunks, int batch) {
+  char* ws = static_cast<char*>(c->d_ws);
+  DecodePlan pl{};
+  pl.chunks = reinterpret_cast<DecChunk*>(ws + w.chunks);
+  pl.rcb = reinterpret_cast<int32_t*>(ws + w.rcb);
+  pl.tile_pre = reinterpret_cast<int32_t*>(ws + w.tile_pre);
+  pl.seg_base = reinterpret_cast<int32_t*>(ws + w.seg_base);
+  pl.cta_seg = reinterpret_cast<int32_t*>(ws + w.cta_seg);
+  pl.segs = reinterpret_cast<DecSeg*>(ws + w.segs);
+  pl.cs = reinterpret_cast<float2*>(ws + w.cs);
+  pl.inv_freq = c->d_inv_freq;
+  pl.n_chunks = n_chunks; pl.batch = batch; pl.max_segs = w.max_segs;
+  return pl;
+}
+
+kam_status grow_ws(kam_ctx* c, size_t bytes) {
+  if (c->ws_cap >= bytes) return KAM_OK;
+  c->winplan_epoch = ~0ull;                                       // the cached window plan lives in the old buffer
+  return grow_device(c, &c->d_ws, &c->ws_cap, bytes + bytes / 4, "cudaMalloc(decode workspace)");
 }
 
 }  // namespace
@@ -88,32 +112,30 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   if (patches) return fail(c, KAM_ERR_UNSUPPORTED, "on-read patching is not built yet; materialise the patch with kam_relocate_patch");
   if (batch == 0) return KAM_OK;
   if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
+  if ((long long)batch * max_chunks > (1ll << 24)) return fail(c, KAM_ERR_UNSUPPORTED, "batch * max_chunks too large");
   DecodeGeom g;
   if ((s = decode_geom(c, pool, &g)) != KAM_OK) return s;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
 
-  g.split_tokens = pick_split(c, g, (long long)batch * max_pages * g.P);
-  const int max_splits = max_chunks + (int)(((long long)max_pages * g.P + g.split_tokens - 1) / g.split_tokens);
-  const WsLayout w = ws_layout(g, batch, max_splits);
-  if ((s = grow_device(c, &c->d_ws, &c->ws_cap, w.total, "cudaMalloc(decode workspace)")) != KAM_OK) return s;
-  char* ws = static_cast<char*>(c->d_ws);
+  const int N = batch * max_chunks;
+  const WsLayout w = ws_layout(g, N, batch);
+  if ((s = grow_ws(c, w.total)) != KAM_OK) return s;
+  c->winplan_epoch = ~0ull;                                       // this call overwrites the plan area
 
   DecodeParams p{};
   p.q = q; p.pool_k_layers = pool->k_layers; p.pool_v_layers = pool->v_layers; p.layer = layer;
   p.block_tables = block_tables; p.tmaps = c->d_tmaps;
-  p.items = reinterpret_cast<DecodeItem*>(ws + w.items);
-  p.n_items = reinterpret_cast<int32_t*>(ws + w.scalars);
-  p.work_counter = reinterpret_cast<int32_t*>(ws + w.scalars) + 1;
-  p.patches = nullptr; p.max_chunks = max_chunks;
-  p.part_o = reinterpret_cast<float*>(ws + w.part_o); p.part_lse = reinterpret_cast<float*>(ws + w.part_lse);
-  p.n_splits = reinterpret_cast<int32_t*>(ws + w.n_splits); p.max_splits = max_splits;
-  p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.batch = batch;
+  p.plan = plan_of(c, w, N, batch);
+  p.patches = nullptr;
+  p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
+  p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
+  p.sm_scale = sm_scale; p.out = out; p.lse = lse;
 
-  launch_decode_plan(chunk_starts, reinterpret_cast<const long long*>(chunk_offsets), n_chunks, max_chunks, max_pages, batch,
-                     g.split_tokens, max_splits, reinterpret_cast<DecodeItem*>(ws + w.items),
-                     reinterpret_cast<int32_t*>(ws + w.scalars), reinterpret_cast<int32_t*>(ws + w.n_splits),
-                     reinterpret_cast<int32_t*>(ws + w.scalars) + 1, st);
-  launch_decode(g, p, c->sm_count, st);
+  DecodeCsr csr{};
+  csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
+  csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = 0;
+  launch_decode_plan(g, p.plan, csr, st);
+  launch_decode(g, p, st);
   launch_decode_merge(g, p, st);
   c->kernels_launched += 3;
   cudaError_t e = cudaGetLastError();
@@ -137,58 +159,61 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   if (s != KAM_OK) return s;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
 
-  long long tokens = 0;
-  for (int b = 0; b < batch; ++b) for (const ChunkRec& r : c->win->chunks(req_ids[b])) tokens += r.n_tokens;
-  g.split_tokens = pick_split(c, g, tokens);
-  // the host knows its own windows: the split list is built here (pending lazy deltas become on-read rotations)
-  std::vector<DecodeItem> items;
-  std::vector<int32_t> n_splits(batch);
-  int max_splits = 1;
-  for (int b = 0; b < batch; ++b) {
-    int64_t pos = c->win->window_base(req_ids[b]);
-    int sp = 0;
-    for (const ChunkRec& r : c->win->chunks(req_ids[b])) {
-      for (int o = 0; o < r.n_tokens; o += g.split_tokens) {
-        DecodeItem it{};
-        it.bt_off = (long long)r.slot * c->max_ppc; it.delta = pos - r.phase;
-        it.b = b; it.chunk = 0; it.tok0 = o; it.n_tok = std::min(g.split_tokens, r.n_tokens - o); it.split = sp++; it.ctok0 = o;
-        items.push_back(it);
-      }
-      pos += r.n_tokens;
-    }
-    n_splits[b] = sp;
-    max_splits = std::max(max_splits, sp);
+  // The plan (segments, cos/sin tables) depends only on the windows, not on the layer: it is rebuilt when a window
+  // changed (epoch) or the request list differs, and reused by the calls for the other layers of the same step.
+  const bool cached = c->winplan_epoch == c->win->epoch() && c->winplan_reqs.size() == (size_t)batch &&
+                      std::equal(c->winplan_reqs.begin(), c->winplan_reqs.end(), req_ids);
+  int N = c->winplan_chunks;
+  if (!cached) {
+    N = 0;
+    for (int b = 0; b < batch; ++b) N += (int)c->win->chunks(req_ids[b]).size();
   }
-  const WsLayout w = ws_layout(g, batch, max_splits);
-  if ((s = grow_device(c, &c->d_ws, &c->ws_cap, w.total, "cudaMalloc(decode workspace)")) != KAM_OK) return s;
-  char* ws = static_cast<char*>(c->d_ws);
-  // plan -> staging -> workspace (items | scalars | n_splits are contiguous at the front of the layout)
-  const size_t plan_bytes = w.n_splits + (size_t)batch * 4;
-  Staging* sg;
-  if ((s = staging_acquire(c, plan_bytes, &sg)) != KAM_OK) return s;
-  char* h = static_cast<char*>(sg->host);
-  memset(h, 0, plan_bytes);
-  if (!items.empty()) memcpy(h + w.items, items.data(), items.size() * sizeof(DecodeItem));
-  reinterpret_cast<int32_t*>(h + w.scalars)[0] = (int32_t)items.size();
-  reinterpret_cast<int32_t*>(h + w.scalars)[1] = 0;
-  memcpy(h + w.n_splits, n_splits.data(), (size_t)batch * 4);
-  cudaError_t e = cudaMemcpyAsync(ws, h, plan_bytes, cudaMemcpyHostToDevice, st);
-  staging_release(sg, st);
-  if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(window plan)");
-
+  const WsLayout w = ws_layout(g, N, batch);
+  if (!cached) {
+    if ((s = grow_ws(c, w.total)) != KAM_OK) return s;
+    // host -> device: the flat chunk list (pending lazy deltas become on-read rotations) and the request index
+    const size_t up_bytes = w.rcb + (size_t)(batch + 1) * 4;
+    Staging* sg;
+    if ((s = staging_acquire(c, up_bytes, &sg)) != KAM_OK) return s;
+    char* h = static_cast<char*>(sg->host);
+    DecChunk* hc = reinterpret_cast<DecChunk*>(h + w.chunks);
+    int32_t* hr = reinterpret_cast<int32_t*>(h + w.rcb);
+    int j = 0;
+    for (int b = 0; b < batch; ++b) {
+      hr[b] = j;
+      int64_t pos = c->win->window_base(req_ids[b]);
+      for (const ChunkRec& r : c->win->chunks(req_ids[b])) {
+        DecChunk ch{};
+        ch.bt_off = (long long)r.slot * c->max_ppc; ch.delta = pos - r.phase;
+        ch.b = b; ch.tok0 = 0; ch.n_tok = r.n_tokens; ch.patch = -1;
+        hc[j++] = ch;
+        pos += r.n_tokens;
+      }
+    }
+    hr[batch] = j;
+    cudaError_t e = cudaMemcpyAsync(c->d_ws, h, up_bytes, cudaMemcpyHostToDevice, st);
+    staging_release(sg, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(window plan)");
+  }
   DecodeParams p{};
   p.q = q; p.pool_k_layers = c->pool.k_layers; p.pool_v_layers = c->pool.v_layers; p.layer = layer;
   p.block_tables = c->d_slot_pages; p.tmaps = c->d_tmaps;
-  p.items = reinterpret_cast<DecodeItem*>(ws + w.items);
-  p.n_items = reinterpret_cast<int32_t*>(ws + w.scalars);
-  p.work_counter = reinterpret_cast<int32_t*>(ws + w.scalars) + 1;
-  p.part_o = reinterpret_cast<float*>(ws + w.part_o); p.part_lse = reinterpret_cast<float*>(ws + w.part_lse);
-  p.n_splits = reinterpret_cast<int32_t*>(ws + w.n_splits); p.max_splits = max_splits;
-  p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.batch = batch;
-  launch_decode(g, p, c->sm_count, st);
+  p.plan = plan_of(c, w, N, batch);
+  p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
+  p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
+  p.sm_scale = sm_scale; p.out = out; p.lse = lse;
+  if (!cached) {
+    DecodeCsr csr{};
+    launch_decode_plan(g, p.plan, csr, st);
+    ++c->kernels_launched;
+    c->winplan_epoch = c->win->epoch();
+    c->winplan_reqs.assign(req_ids, req_ids + batch);
+    c->winplan_chunks = N;
+  }
+  launch_decode(g, p, st);
   launch_decode_merge(g, p, st);
   c->kernels_launched += 2;
-  e = cudaGetLastError();
+  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(c, e, "decode launch");
   return KAM_OK;
 }

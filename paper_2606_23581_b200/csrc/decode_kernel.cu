@@ -1,19 +1,25 @@
 // kam_paged_decode_merge: fused-on-read paged decode attention with per-chunk LSE merge.
 //
-//   plan    (1 CTA)      device chunk metadata -> a flat list of splits (token ranges inside one chunk), so that
-//                        nothing about the batch has to be known on the host (CUDA-graph friendly)
-//   decode  (persistent) one CTA per SM pulls (split, KV-head-group) work units from an atomic counter.  A producer
-//                        warp resolves the block table and streams 32-token K and V tiles into shared memory with
-//                        1-D bulk async copies behind an mbarrier ring that runs ACROSS work units (no drain between
-//                        them); one compute warp per KV head runs QK^T and PV as m16n8k16 bf16 MMAs with the G query
-//                        heads of the group as the M dimension (online softmax in fp32, exp2 domain).
-//                        The cached keys are NOT rewritten: relocation is applied on read as q~ = R(-delta) q
-//                        (q.(R(delta)k) = (R(-delta)q).k), carried as a bf16 hi+lo pair so that the rotation costs
-//                        no precision; per (split, head) state (o, lse) goes to a partials buffer
-//   merge   (B*Hq CTAs)  lse = ln sum_s e^{lse_s}; out = sum_s e^{lse_s - lse} o_s   (the paper's state merge)
+//   plan    (1 + n CTAs)  device chunk metadata -> the flat list of 16-token tiles (head group x request x chunk x tile)
+//                         is cut into one equal contiguous range per persistent CTA; a range is a list of SEGMENTS (runs
+//                         of tiles inside one chunk).  Everything is computed on the device from device metadata, so a
+//                         call never needs the batch on the host (CUDA-graph friendly).  The other CTAs of the launch
+//                         write the per-chunk (cos, sin)(delta f_i) tables, fp64 sincos, once for all layers.
+//   decode  (persistent)  2-3 CTAs per SM, each = 1 producer warp + one compute warp per KV head of the head group.  The
+//                         producer resolves the block table and streams 16-token K and V boxes through a ring of
+//                         mbarrier-guarded shared-memory boxes with TMA tensor-map loads (cp.async.bulk.tensor, 128-byte
+//                         swizzle); the ring runs ACROSS segments.  A compute warp owns one KV head: S^T = K q~^T and
+//                         O^T += V^T P^T as m16n8k16 bf16 MMAs with the TOKENS / head-dim as the M dimension and the (<= 8)
+//                         query heads of the group as N - no MMA rows are wasted on padding and the accumulators of a
+//                         128-wide head are 32 registers.  Online softmax in fp32 (exp2 domain); P^T goes from the
+//                         accumulator layout to the B-operand layout with one movmatrix.trans per 8 tokens.
+//                         The cached keys are NOT rewritten: relocation is applied on read as q~ = R(-delta) q
+//                         (q.(R(delta)k) = (R(-delta)q).k), carried as a bf16 hi+lo pair so the rotation costs no
+//                         precision.  Per (segment, query head) state (o, lse) goes to a partials buffer.
+//   merge   (B*Hq CTAs)   lse = ln sum_s e^{lse_s}; out = sum_s e^{lse_s - lse} o_s   (the paper's state merge)
 //
-// Decode is HBM-bound: every K and V byte is read exactly once; MMA work is G flop/byte, far below the
-// legacy tensor pipe's rate, which is why mma.sync (not tcgen05/TMEM) carries it - see DESIGN.md.
+// Decode is HBM-bound: every K and V byte is read exactly once.  MMA work is 2 HMMA per 16 tokens x 16 dims, a few percent
+// of the legacy tensor pipe, which is why mma.sync (not tcgen05/TMEM, whose M is 64/128) carries it - see DESIGN.md.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
@@ -23,254 +29,329 @@
 namespace kam {
 
 // ---------------------------------------------------------------------------------------------------- plan
-__global__ void __launch_bounds__(1024) kam_decode_plan_kernel(const int32_t* __restrict__ chunk_starts,
-                                                               const long long* __restrict__ chunk_offsets,
-                                                               const int32_t* __restrict__ n_chunks, int max_chunks,
-                                                               int max_pages, int batch, int split_tokens, int max_splits,
-                                                               DecodeItem* items, int32_t* n_items, int32_t* n_splits,
-                                                               int32_t* work_counter) {
-  __shared__ int scan[1024];
-  __shared__ int carry;
-  const int tid = threadIdx.x;
-  if (tid == 0) carry = 0;
-  __syncthreads();
-  for (int base = 0; base < batch; base += 1024) {
-    const int b = base + tid;
-    int cnt = 0, nc = 0;
-    const int32_t* cs = nullptr;
-    if (b < batch) {
-      nc = min(n_chunks[b], max_chunks);
-      cs = chunk_starts + static_cast<size_t>(b) * (max_chunks + 1);
-      for (int c = 0; c < nc; ++c) cnt += (cs[c + 1] - cs[c] + split_tokens - 1) / split_tokens;
-      cnt = min(cnt, max_splits);
-    }
-    scan[tid] = cnt;
-    __syncthreads();
-    for (int off = 1; off < 1024; off <<= 1) {          // inclusive Hillis-Steele scan
-      const int v = tid >= off ? scan[tid - off] : 0;
-      __syncthreads();
-      scan[tid] += v;
-      __syncthreads();
-    }
-    int idx = carry + scan[tid] - cnt;
-    if (b < batch) {
-      n_splits[b] = cnt;
-      int sp = 0;
-      for (int c = 0; c < nc && sp < cnt; ++c) {
-        const int len = cs[c + 1] - cs[c];
-        for (int o = 0; o < len && sp < cnt; o += split_tokens) {
-          DecodeItem it;
-          it.bt_off = static_cast<long long>(b) * max_pages;
-          it.delta = chunk_offsets ? chunk_offsets[static_cast<size_t>(b) * max_chunks + c] : 0;
-          it.b = b; it.chunk = c;
-          it.tok0 = cs[c] - cs[0] + o;
-          it.n_tok = min(split_tokens, len - o);
-          it.split = sp++;
-          it.ctok0 = o;
-          items[idx++] = it;
-        }
-      }
-    }
-    __syncthreads();
-    if (tid == 1023) carry += scan[1023];
-    __syncthreads();
-  }
-  if (tid == 0) { *n_items = carry; *work_counter = 0; }
-}
-
-void launch_decode_plan(const int32_t* chunk_starts, const long long* chunk_offsets, const int32_t* n_chunks,
-                        int32_t max_chunks, int32_t max_pages, int32_t batch, int32_t split_tokens, int32_t max_splits,
-                        DecodeItem* items, int32_t* n_items, int32_t* n_splits, int32_t* work_counter, cudaStream_t st) {
-  kam_decode_plan_kernel<<<1, 1024, 0, st>>>(chunk_starts, chunk_offsets, n_chunks, max_chunks, max_pages, batch,
-                                             split_tokens, max_splits, items, n_items, n_splits, work_counter);
-}
-
-// ---------------------------------------------------------------------------------------------------- decode
 namespace {
-enum : int { HDR_FIRST = 1, HDR_LAST = 2 };
 
-__device__ __forceinline__ float quad_max(float v) {
-  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
-  return fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));
+// Exclusive prefix sum of data[0, M) in place; data[M] = total (also returned).  One block, any M.
+__device__ int block_excl_scan(int32_t* data, int M, int* sh) {
+  const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
+  const int per = (M + T - 1) / T;
+  const int lo = min(M, tid * per), hi = min(M, lo + per);
+  int local = 0;
+  for (int i = lo; i < hi; ++i) local += data[i];
+  int inc = local;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, inc, off);
+    if (lane >= off) inc += v;
+  }
+  if (lane == 31) sh[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    int v = lane < (T >> 5) ? sh[lane] : 0;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, v, off);
+      if (lane >= off) v += u;
+    }
+    sh[lane] = v;                                  // inclusive totals of the warps
+  }
+  __syncthreads();
+  int run = inc - local + (warp ? sh[warp - 1] : 0);
+  const int total = sh[(T >> 5) - 1];
+  for (int i = lo; i < hi; ++i) { const int v = data[i]; data[i] = run; run += v; }
+  if (tid == 0) data[M] = total;
+  __syncthreads();
+  return total;
 }
-__device__ __forceinline__ float quad_sum(float v) {
-  v += __shfl_xor_sync(0xffffffffu, v, 1);
-  return v + __shfl_xor_sync(0xffffffffu, v, 2);
+
+__device__ __forceinline__ long long ceil_div_ll(long long a, long long b) { return (a + b - 1) / b; }
+
+struct SegCut { long long g0, g1, i_lo; int nseg; };
+// Chunk j of head group hg covers global tiles [g0, g1); CTA i starts at tile s_i = i * total / n_eff.
+__device__ __forceinline__ SegCut seg_cut(int hg, int j, const int32_t* tile_pre, long long total_hg, long long total, long long n_eff) {
+  SegCut c;
+  c.g0 = hg * total_hg + tile_pre[j];
+  c.g1 = hg * total_hg + tile_pre[j + 1];
+  c.nseg = 0; c.i_lo = 0;
+  if (c.g1 > c.g0) {
+    c.i_lo = ceil_div_ll((c.g0 + 1) * n_eff, total);            // smallest i with s_i > g0
+    const long long i_hi = ceil_div_ll(c.g1 * n_eff, total);    // smallest i with s_i >= g1
+    c.nseg = 1 + static_cast<int>(max(0ll, i_hi - c.i_lo));
+  }
+  return c;
 }
+
 }  // namespace
 
-// KS = D / 16 (k-steps of QK^T; D = Dv).  TMA: pool pages arrive as swizzled 16-token tensor-map boxes.
-//
-// TMA path shared-memory layout of one box: [64-column block c][token r (16)][128 bytes], SWIZZLE_128B, i.e. the 16-byte
-// chunk j of (c, r) sits at (c*16 + r)*128 + ((j ^ (r & 7)) << 4): eight consecutive tokens of one chunk hit eight
-// different bank groups, so ldmatrix (K) and ldmatrix.trans (V) are conflict-free without padding.  Tiles are aligned
-// to 16 tokens of the page list (a box never straddles a page because P % 16 == 0); rows outside the split's token
-// range are masked in the softmax.
-template <int KS, bool TMA>
-__global__ void __launch_bounds__((kDecMaxHG + 1) * 32, 1)
-kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem);
-  uint64_t* empty_bar = full_bar + g.n_stages;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_threads = blockDim.x;
+__global__ void __launch_bounds__(kDecPlanThreads) kam_decode_plan_kernel(const __grid_constant__ DecodeGeom g,
+                                                                          const __grid_constant__ DecodePlan pl,
+                                                                          const __grid_constant__ DecodeCsr csr) {
+  __shared__ int sh[32];
+  const int tid = threadIdx.x;
+  const int N = pl.n_chunks;
 
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < g.n_stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], g.HG); }
-    mbar_fence_init();
-  }
-  // Rows beyond a tile's valid tokens are never copied; they must hold finite values (0 * NaN would poison PV).
-  for (int i = threadIdx.x * 16; i < g.n_stages * g.stage_bytes; i += n_threads * 16)
-    *reinterpret_cast<uint4*>(smem + g.off_stage0 + i) = make_uint4(0, 0, 0, 0);
-  fence_proxy_async();
-  __syncthreads();
-
-  const int total = *p.n_items * g.n_hg;
-
-  if (warp == g.HG) {
-    // ================================================================ producer warp: schedule, slot-map, copy
-    int stage = 0; uint32_t phase = 0;
-    const char* pk = static_cast<const char*>(p.pool_k_layers[p.layer]);
-    const char* pv = static_cast<const char*>(p.pool_v_layers[p.layer]);
-    while (true) {
-      int w = 0;
-      if (lane == 0) w = atomicAdd(p.work_counter, 1);
-      w = __shfl_sync(0xffffffffu, w, 0);
-      if (w >= total) {
-        mbar_wait(&empty_bar[stage], phase ^ 1);
-        if (lane == 0) {
-          *reinterpret_cast<int4*>(smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes + g.st_hdr) = make_int4(-1, 0, 0, 0);
-          mbar_arrive(&full_bar[stage]);
-        }
-        break;
+  if (blockIdx.x > 0) {
+    // ---- A2 for decode: (cos, sin)(delta f_i) per (chunk, frequency); the angle is formed in fp64 (R-18)
+    const int half = g.d_r >> 1;
+    const long long n = static_cast<long long>(N) * half;
+    for (long long idx = static_cast<long long>(blockIdx.x - 1) * blockDim.x + tid; idx < n; idx += static_cast<long long>(gridDim.x - 1) * blockDim.x) {
+      const int j = static_cast<int>(idx / half), i = static_cast<int>(idx - static_cast<long long>(j) * half);
+      long long delta;
+      if (csr.enabled) {
+        const int b = j / csr.max_chunks, c = j - b * csr.max_chunks;
+        delta = (csr.chunk_offsets && c < csr.n_chunks[b]) ? csr.chunk_offsets[j] : 0;
+      } else {
+        delta = pl.chunks[j].delta;
       }
-      const int item_idx = w / g.n_hg, hg = w - item_idx * g.n_hg;
-      const DecodeItem it = p.items[item_idx];
-      const int32_t* bt = p.block_tables + it.bt_off;
-      if constexpr (TMA) {
-        const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * 256;
-        const char* tm_v = tm_k + 128;
-        const int a0 = it.tok0 & ~15, end = it.tok0 + it.n_tok;
-        const int n_tiles = (end - a0 + kDecTT - 1) / kDecTT;
-        for (int t = 0; t < n_tiles; ++t) {
-          const int base = a0 + t * kDecTT;
-          const int n_box = min(2, (end - base + 15) >> 4);
-          int slot0 = 0;
-          if (lane < n_box) {
-            const int tok = base + lane * 16;
-            const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
-            slot0 = bt[pg] * g.P + (tok - pg * g.P);
-          }
-          const int slot1 = __shfl_sync(0xffffffffu, slot0, 1);
-          mbar_wait(&empty_bar[stage], phase ^ 1);
-          if (lane == 0) {
-            uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
-            const int lo = max(it.tok0 - base, 0), hi = min(end - base, kDecTT);
-            *reinterpret_cast<int4*>(st + g.st_hdr) = make_int4(w, t, lo | (hi << 16), (t == 0 ? HDR_FIRST : 0) | (t == n_tiles - 1 ? HDR_LAST : 0));
-            mbar_arrive_expect_tx(&full_bar[stage], static_cast<uint32_t>(n_box) * g.box_bytes * 2u);
-            tma_load_3d(st + g.st_k, tm_k, 0, slot0, hg * g.ncb, &full_bar[stage]);
-            tma_load_3d(st + g.st_v, tm_v, 0, slot0, hg * g.ncb, &full_bar[stage]);
-            if (n_box > 1) {
-              tma_load_3d(st + g.st_k + g.box_bytes, tm_k, 0, slot1, hg * g.ncb, &full_bar[stage]);
-              tma_load_3d(st + g.st_v + g.box_bytes, tm_v, 0, slot1, hg * g.ncb, &full_bar[stage]);
-            }
-          }
-          if (++stage == g.n_stages) { stage = 0; phase ^= 1; }
-        }
-        continue;
-      }
-      const int n_tiles = (it.n_tok + kDecTT - 1) / kDecTT;
-      const size_t off = static_cast<size_t>(hg) * g.slice_bytes;
-      for (int t = 0; t < n_tiles; ++t) {
-        // A1 slot mapping for the tile's 32 tokens, one per lane (issued before waiting for the stage)
-        const int rel = t * kDecTT + lane;
-        int slot = 0;
-        if (rel < it.n_tok) {
-          const int tok = it.tok0 + rel;
-          const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
-          slot = bt[pg] * g.P + (tok - pg * g.P);
-        }
-        const int nvalid = min(kDecTT, it.n_tok - t * kDecTT);
-        mbar_wait(&empty_bar[stage], phase ^ 1);
-        uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
-        if (lane == 0) {
-          *reinterpret_cast<int4*>(st + g.st_hdr) = make_int4(w, t, nvalid << 16, (t == 0 ? HDR_FIRST : 0) | (t == n_tiles - 1 ? HDR_LAST : 0));
-          mbar_arrive_expect_tx(&full_bar[stage], static_cast<uint32_t>(nvalid) * g.slice_bytes * 2u);
-        }
-        __syncwarp();
-        for (int r = 0; r < nvalid; ++r) {
-          const int s = __shfl_sync(0xffffffffu, slot, r);
-          if (lane == 0) {
-            const size_t row = static_cast<size_t>(s) * g.row_bytes + off;
-            bulk_g2s(st + g.st_k + r * g.s_row, pk + row, g.slice_bytes, &full_bar[stage]);
-            bulk_g2s(st + g.st_v + r * g.s_row, pv + row, g.slice_bytes, &full_bar[stage]);
-          }
-        }
-        if (++stage == g.n_stages) { stage = 0; phase ^= 1; }
+      if (delta != 0) {
+        double s, c;
+        sincos(static_cast<double>(delta) * pl.inv_freq[i], &s, &c);
+        pl.cs[idx] = make_float2(static_cast<float>(c), static_cast<float>(s));
       }
     }
     return;
   }
 
+  // ---- phase 0: chunk records of the stateless call (CSR token boundaries per request)
+  if (csr.enabled) {
+    for (int j = tid; j < N; j += blockDim.x) {
+      const int b = j / csr.max_chunks, c = j - b * csr.max_chunks;
+      const int32_t* cs = csr.chunk_starts + static_cast<size_t>(b) * (csr.max_chunks + 1);
+      const int nc = min(csr.n_chunks[b], csr.max_chunks);
+      DecChunk ch;
+      ch.bt_off = static_cast<long long>(b) * csr.max_pages;
+      ch.delta = 0; ch.b = b; ch.tok0 = 0; ch.n_tok = 0; ch.patch = -1;
+      if (c < nc) {
+        ch.tok0 = cs[c] - cs[0];
+        ch.n_tok = max(0, cs[c + 1] - cs[c]);
+        ch.delta = csr.chunk_offsets ? csr.chunk_offsets[j] : 0;
+        ch.patch = csr.has_patches ? j : -1;
+      }
+      pl.chunks[j] = ch;
+    }
+    for (int b = tid; b <= pl.batch; b += blockDim.x) pl.rcb[b] = b * csr.max_chunks;
+    __syncthreads();
+  }
+
+  // ---- phase 1: 16-token tiles per chunk (tiles are aligned to the page list, so a box never straddles a page)
+  for (int j = tid; j < N; j += blockDim.x) {
+    const DecChunk& ch = pl.chunks[j];
+    pl.tile_pre[j] = ch.n_tok > 0 ? ((ch.tok0 + ch.n_tok + kDecTile - 1) / kDecTile) - (ch.tok0 / kDecTile) : 0;
+  }
+  __syncthreads();
+  const long long total_hg = block_excl_scan(pl.tile_pre, N, sh);
+  const long long total = total_hg * g.n_hg;
+  const long long n_eff = min(static_cast<long long>(g.n_ctas), total);
+  const int M = g.n_hg * N;
+
+  // ---- phase 2: segments per (head group, chunk) = 1 + CTA cuts strictly inside it
+  for (int e = tid; e < M; e += blockDim.x) {
+    const int hg = e / N, j = e - hg * N;
+    pl.seg_base[e] = total ? seg_cut(hg, j, pl.tile_pre, total_hg, total, n_eff).nseg : 0;
+  }
+  __syncthreads();
+  const int n_segs = block_excl_scan(pl.seg_base, M, sh);
+
+  // ---- phase 3: emit the segments and each CTA's first segment
+  for (int i = tid; i <= g.n_ctas; i += blockDim.x)
+    if (i >= n_eff) pl.cta_seg[i] = n_segs;
+  for (int e = tid; e < M; e += blockDim.x) {
+    if (!total) break;
+    const int hg = e / N, j = e - hg * N;
+    const SegCut c = seg_cut(hg, j, pl.tile_pre, total_hg, total, n_eff);
+    if (c.nseg == 0) continue;
+    const DecChunk ch = pl.chunks[j];
+    const int base = pl.seg_base[e];
+    for (int k = 0; k < c.nseg; ++k) {
+      const long long start = k == 0 ? c.g0 : ((c.i_lo + k - 1) * total) / n_eff;
+      const long long end = k == c.nseg - 1 ? c.g1 : ((c.i_lo + k) * total) / n_eff;
+      DecSeg s;
+      s.bt_off = ch.bt_off; s.chunk = j; s.b = ch.b; s.hg = hg;
+      s.tile0 = ch.tok0 / kDecTile + static_cast<int>(start - c.g0);
+      s.n_tiles = static_cast<int>(end - start);
+      s.tok_lo = ch.tok0; s.tok_hi = ch.tok0 + ch.n_tok;
+      s.rotate = (ch.delta != 0) && g.d_r > 0;
+      s.patch = ch.patch; s.pad = 0;
+      pl.segs[base + k] = s;
+      const long long i = k == 0 ? ceil_div_ll(start * n_eff, total) : c.i_lo + k - 1;   // the CTA starting exactly here, if any
+      if (i < n_eff && (i * total) / n_eff == start) pl.cta_seg[i] = base + k;
+    }
+  }
+}
+
+void launch_decode_plan(const DecodeGeom& g, const DecodePlan& plan, const DecodeCsr& csr, cudaStream_t st) {
+  const long long n_cs = static_cast<long long>(plan.n_chunks) * (g.d_r / 2);
+  const int cs_blocks = static_cast<int>(min(64ll, (n_cs + kDecPlanThreads - 1) / kDecPlanThreads));
+  kam_decode_plan_kernel<<<1 + cs_blocks, kDecPlanThreads, 0, st>>>(g, plan, csr);
+}
+
+// ---------------------------------------------------------------------------------------------------- decode
+namespace {
+enum : int { HDR_FIRST = 1, HDR_LAST = 2, HDR_PARTIAL = 4 };
+
+__device__ __forceinline__ float ex2(float x) {                  // 2^x, ex2(-inf) = 0
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {   // 8x8 b16 transpose across the warp
+  uint32_t d;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
+  return d;
+}
+__device__ __forceinline__ float col_max(float v) {              // over the 8 lanes that share lane % 4
+  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 4));
+  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 8));
+  return fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 16));
+}
+__device__ __forceinline__ float col_sum(float v) {
+  v += __shfl_xor_sync(0xffffffffu, v, 4);
+  v += __shfl_xor_sync(0xffffffffu, v, 8);
+  return v + __shfl_xor_sync(0xffffffffu, v, 16);
+}
+}  // namespace
+
+// KS = D / 16 (k-steps of QK^T; D = Dv).  NT = ceil(G / 8) query-head tiles.  TMA: pool pages arrive as swizzled boxes.
+//
+// Box layout, TMA path: [64-column block c][token r (16)][128 bytes], SWIZZLE_128B: the 16-byte chunk j of (c, r) sits at
+// (c*16 + r)*128 + ((j ^ (r & 7)) << 4), so eight consecutive tokens of one chunk column hit eight different bank groups
+// and ldmatrix (K) / ldmatrix.trans (V) are conflict-free without padding.  Bulk-copy path: [token r][s_row bytes], s_row
+// padded so that (s_row / 16) is odd.  Tiles are aligned to 16 tokens of the page list (P % 16 == 0 on the TMA path, so a
+// box never straddles a page); rows outside the chunk's token range are masked in the softmax and zeroed in V.
+template <int KS, int NT, bool TMA>
+__global__ void __launch_bounds__((kDecMaxHG + 1) * 32, NT == 1 ? 3 : 1)
+kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem);
+  uint64_t* empty_bar = full_bar + g.n_boxes;
+  int4* hdrs = reinterpret_cast<int4*>(smem + g.off_hdr);
+  uint8_t* box0 = smem + g.off_box0;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < g.n_boxes; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], g.HG); }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  const int seg_begin = p.plan.cta_seg[blockIdx.x], seg_end = p.plan.cta_seg[blockIdx.x + 1];
+  if (seg_begin >= seg_end) return;
+
+  if (warp == g.HG) {
+    // ================================================================ producer warp: slot-map (A1), stream K / V boxes
+    int box = 0; uint32_t phase = 0;
+    const char* pk = static_cast<const char*>(p.pool_k_layers[p.layer]);
+    const char* pv = static_cast<const char*>(p.pool_v_layers[p.layer]);
+    const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * 256;
+    const char* tm_v = tm_k + 128;
+    for (int seg = seg_begin; seg < seg_end; ++seg) {
+      const DecSeg S = p.plan.segs[seg];
+      const int32_t* bt = p.block_tables + S.bt_off;
+      const size_t col_off = static_cast<size_t>(S.hg) * g.slice_bytes;
+      for (int t0 = 0; t0 < S.n_tiles; t0 += 32) {
+        int slot = 0;
+        if (t0 + lane < S.n_tiles) {                            // A1: page = block_table[tok / P], slot = page * P + tok % P
+          const int tok = (S.tile0 + t0 + lane) * kDecTile;
+          const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
+          slot = bt[pg] * g.P + (tok - pg * g.P);
+        }
+        const int nb = min(32, S.n_tiles - t0);
+        for (int i = 0; i < nb; ++i) {
+          const int s0 = __shfl_sync(0xffffffffu, slot, i);
+          const int tl = t0 + i;
+          const int tok = (S.tile0 + tl) * kDecTile;
+          const int row_lo = max(S.tok_lo - tok, 0), row_hi = min(S.tok_hi - tok, kDecTile);
+          int rslot = 0;
+          if constexpr (!TMA) {                                 // any page size: every row of the tile is slot-mapped
+            if (lane >= row_lo && lane < row_hi) {
+              const int tk = tok + lane;
+              const int pg = g.P_shift >= 0 ? (tk >> g.P_shift) : tk / g.P;
+              rslot = bt[pg] * g.P + (tk - pg * g.P);
+            }
+          }
+#pragma unroll
+          for (int kv = 0; kv < 2; ++kv) {
+            mbar_wait(&empty_bar[box], phase ^ 1);
+            uint8_t* dst = box0 + static_cast<size_t>(box) * g.box_bytes;
+            if (lane == 0) {
+              if (kv == 0) {
+                const int flags = (tl == 0 ? HDR_FIRST : 0) | (tl == S.n_tiles - 1 ? HDR_LAST : 0) |
+                                  ((row_lo > 0 || row_hi < kDecTile) ? HDR_PARTIAL : 0);
+                hdrs[box] = make_int4(seg, flags, row_lo | (row_hi << 8), tok - S.tok_lo);
+              }
+              if constexpr (TMA) {
+                mbar_arrive_expect_tx(&full_bar[box], static_cast<uint32_t>(g.box_bytes));
+                tma_load_3d(dst, kv ? tm_v : tm_k, 0, s0, S.hg * g.ncb, &full_bar[box]);
+              } else {
+                mbar_arrive_expect_tx(&full_bar[box], static_cast<uint32_t>(row_hi - row_lo) * g.slice_bytes);
+              }
+            }
+            if constexpr (!TMA) {
+              const char* src = (kv ? pv : pk) + col_off;
+              for (int r = row_lo; r < row_hi; ++r) {
+                const int sr = __shfl_sync(0xffffffffu, rslot, r);
+                if (lane == 0) bulk_g2s(dst + r * g.s_row, src + static_cast<size_t>(sr) * g.row_bytes, g.slice_bytes, &full_bar[box]);
+              }
+            }
+            if (++box == g.n_boxes) { box = 0; phase ^= 1; }
+          }
+        }
+      }
+    }
+    mbar_wait(&empty_bar[box], phase ^ 1);
+    if (lane == 0) { hdrs[box] = make_int4(-1, 0, 0, 0); mbar_arrive(&full_bar[box]); }
+    return;
+  }
+
   // ================================================================ compute warps: one KV head each
   const int gq = lane >> 2, t4 = lane & 3;
-  const int D = KS * 16;
-  float2* cs_w = reinterpret_cast<float2*>(smem + g.off_warp + warp * g.warp_bytes);
+  constexpr int D = KS * 16;
   const float scale_log2 = p.sm_scale * 1.4426950408889634f;
 
-  uint32_t qhi[KS][4], qlo[KS][4];
-  float O[2 * KS][4];
-  float m_run[2] = {-CUDART_INF_F, -CUDART_INF_F}, l_run[2] = {0.f, 0.f};
+  uint32_t qhi[NT][KS][2], qlo[NT][KS][2];
+  float O[NT][KS][4];
+  float m_run[NT][2], l_run[NT][2];
   bool use_lo = false;
-  int item_b = 0, item_split = 0, head = 0;
 
-  // ldmatrix lane addressing inside a stage (bytes relative to the K / V region)
-  //   K (non-trans): matrices = (tokens 0-7 | 8-15 of a 16-token block) x (first | second 16-byte chunk of the k-step)
-  //   V (trans):     matrices = (tokens 0-7 | 8-15) x (first | second d n-tile of the pair)
-  const int k_row = (lane & 7) + ((lane >> 4) & 1) * 8, k_hi = (lane >> 3) & 1;
-  const int v_row = (lane & 7) + ((lane >> 3) & 1) * 8, v_hi = (lane >> 4) & 1;
+  // ldmatrix lane addressing inside a box (bytes)
+  //   K (A operand, rows = tokens): matrices (tokens 0-7 | 8-15) x (first | second 16-byte chunk of the k-step)
+  //   V (A operand via .trans, rows = head dims): matrices (first | second d chunk) x (tokens 0-7 | 8-15)
+  const int k_row = (lane & 7) + ((lane >> 3) & 1) * 8, k_hi = lane >> 4;
+  const int v_row = (lane & 7) + (lane >> 4) * 8, v_hi = (lane >> 3) & 1;
   const uint32_t k_lane = TMA ? (warp * (D / 64) * 16 + k_row) * 128 : k_row * g.s_row + warp * D * 2 + k_hi * 16;
   const uint32_t v_lane = TMA ? (warp * (D / 64) * 16 + v_row) * 128 : v_row * g.s_row + warp * D * 2 + v_hi * 16;
-  const uint32_t k_sw = (k_hi ^ (lane & 7)) << 4, v_sw = (v_hi ^ (lane & 7)) << 4;   // swizzled chunk of k-step 0
-  const uint32_t blk16 = TMA ? g.box_bytes : 16 * g.s_row;                            // bytes between 16-token blocks
+  const uint32_t k_sw = (k_hi ^ (lane & 7)) << 4, v_sw = (v_hi ^ (lane & 7)) << 4;   // swizzled chunk of step 0
 
-  int stage = 0; uint32_t phase = 0;
+  int box = 0; uint32_t phase = 0;
+  int seg = 0;
   while (true) {
-    mbar_wait(&full_bar[stage], phase);
-    const uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
-    const int4 hdr = *reinterpret_cast<const int4*>(st + g.st_hdr);
+    mbar_wait(&full_bar[box], phase);
+    const int4 hdr = hdrs[box];
     if (hdr.x < 0) break;
-    const int row_lo = hdr.z & 0xffff, row_hi = hdr.z >> 16;        // valid token rows of this tile
+    const uint32_t kb = smem_u32(box0 + static_cast<size_t>(box) * g.box_bytes) + k_lane;
+    const int kbox = box;
+    if (++box == g.n_boxes) { box = 0; phase ^= 1; }
 
-    if (hdr.w & HDR_FIRST) {
-      // ---- new work unit: load the G query rows of this KV head, rotate them by -delta, split into bf16 hi + lo
-      const int item_idx = hdr.x / g.n_hg, hg = hdr.x - item_idx * g.n_hg;
-      const DecodeItem it = p.items[item_idx];
-      item_b = it.b; item_split = it.split;
-      head = hg * g.HG + warp;
-      use_lo = (it.delta != 0) && g.d_r > 0;
+    if (hdr.y & HDR_FIRST) {
+      // ---- new segment: the G query rows of this KV head, rotated by -delta (A8), split into bf16 hi + lo
+      seg = hdr.x;
+      const DecSeg S = p.plan.segs[seg];
+      const int head = S.hg * g.HG + warp;
+      use_lo = S.rotate;
       const int half = g.d_r >> 1;
-      if (use_lo) {
-        for (int i = lane; i < half; i += 32) {
-          const double f = pow(g.theta, -2.0 * i / g.d_r);
-          double s, c;
-          sincos(static_cast<double>(it.delta) * f, &s, &c);
-          cs_w[i] = make_float2(static_cast<float>(c), static_cast<float>(s));
-        }
-        __syncwarp();
-      }
-      const __nv_bfloat16* qb = static_cast<const __nv_bfloat16*>(p.q) + (static_cast<size_t>(it.b) * g.Hq + static_cast<size_t>(head) * g.G) * D;
+      const float2* cs = p.plan.cs + static_cast<size_t>(S.chunk) * half;
+      const __nv_bfloat16* qb = static_cast<const __nv_bfloat16*>(p.q) + (static_cast<size_t>(S.b) * g.Hq + static_cast<size_t>(head) * g.G) * D;
 #pragma unroll
-      for (int ks = 0; ks < KS; ++ks) {
+      for (int nt = 0; nt < NT; ++nt) {
+        const int row = nt * 8 + gq;                              // query head inside the group = column of S^T
+        const __nv_bfloat16* qr = qb + static_cast<size_t>(row) * D;
 #pragma unroll
-        for (int part = 0; part < 2; ++part) {
-          const int c0 = ks * 16 + part * 8 + 2 * t4;
+        for (int ks = 0; ks < KS; ++ks) {
 #pragma unroll
-          for (int rs = 0; rs < 2; ++rs) {
-            const int row = gq + rs * 8;
+          for (int part = 0; part < 2; ++part) {
+            const int c0 = ks * 16 + part * 8 + 2 * t4;
             float x0 = 0.f, x1 = 0.f;
             if (row < g.G) {
-              const __nv_bfloat16* qr = qb + static_cast<size_t>(row) * D;
               const uint32_t xv = *reinterpret_cast<const uint32_t*>(qr + c0);
               x0 = bf_lo(xv); x1 = bf_hi(xv);
               const int rel = c0 - g.rope_off;
@@ -279,122 +360,140 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
                 if (g.rope_style == KAM_ROPE_HALF) {
                   if (rel < half) {
                     const uint32_t yv = *reinterpret_cast<const uint32_t*>(qr + c0 + half);
-                    const float2 t0 = cs_w[rel], t1 = cs_w[rel + 1];
-                    x0 = fmaf(x0, t0.x, bf_lo(yv) * t0.y);
-                    x1 = fmaf(x1, t1.x, bf_hi(yv) * t1.y);
+                    const float2 u0 = cs[rel], u1 = cs[rel + 1];
+                    x0 = fmaf(x0, u0.x, bf_lo(yv) * u0.y);
+                    x1 = fmaf(x1, u1.x, bf_hi(yv) * u1.y);
                   } else {
                     const uint32_t yv = *reinterpret_cast<const uint32_t*>(qr + c0 - half);
-                    const float2 t0 = cs_w[rel - half], t1 = cs_w[rel - half + 1];
-                    x0 = fmaf(x0, t0.x, -bf_lo(yv) * t0.y);
-                    x1 = fmaf(x1, t1.x, -bf_hi(yv) * t1.y);
+                    const float2 u0 = cs[rel - half], u1 = cs[rel - half + 1];
+                    x0 = fmaf(x0, u0.x, -bf_lo(yv) * u0.y);
+                    x1 = fmaf(x1, u1.x, -bf_hi(yv) * u1.y);
                   }
                 } else {
-                  const float2 t0 = cs_w[rel >> 1];
+                  const float2 u0 = cs[rel >> 1];
                   const float a = x0, b = x1;
-                  x0 = fmaf(a, t0.x, b * t0.y);
-                  x1 = fmaf(b, t0.x, -a * t0.y);
+                  x0 = fmaf(a, u0.x, b * u0.y);
+                  x1 = fmaf(b, u0.x, -a * u0.y);
                 }
               }
             }
             const uint32_t hi = pack_bf16x2(x0, x1);
-            qhi[ks][part * 2 + rs] = hi;
-            qlo[ks][part * 2 + rs] = pack_bf16x2(x0 - bf_lo(hi), x1 - bf_hi(hi));
+            qhi[nt][ks][part] = hi;
+            qlo[nt][ks][part] = pack_bf16x2(x0 - bf_lo(hi), x1 - bf_hi(hi));
           }
         }
-      }
 #pragma unroll
-      for (int n = 0; n < 2 * KS; ++n) { O[n][0] = O[n][1] = O[n][2] = O[n][3] = 0.f; }
-      m_run[0] = m_run[1] = -CUDART_INF_F;
-      l_run[0] = l_run[1] = 0.f;
+        for (int n = 0; n < KS; ++n) { O[nt][n][0] = O[nt][n][1] = O[nt][n][2] = O[nt][n][3] = 0.f; }
+        m_run[nt][0] = m_run[nt][1] = -CUDART_INF_F;
+        l_run[nt][0] = l_run[nt][1] = 0.f;
+      }
     }
 
-    // ---- S = q~ K^T for 32 tokens (4 n-tiles)
-    float S[4][4];
+    // ---- S^T[16 tokens][8 heads] = K q~^T : two interleaved accumulator chains per head tile
+    float sa[NT][4], sb[NT][4];
 #pragma unroll
-    for (int n = 0; n < 4; ++n) { S[n][0] = S[n][1] = S[n][2] = S[n][3] = 0.f; }
-    const uint32_t kb = smem_u32(st + g.st_k) + k_lane;
+    for (int nt = 0; nt < NT; ++nt) { sa[nt][0] = sa[nt][1] = sa[nt][2] = sa[nt][3] = 0.f; sb[nt][0] = sb[nt][1] = sb[nt][2] = sb[nt][3] = 0.f; }
 #pragma unroll
     for (int ks = 0; ks < KS; ++ks) {
+      uint32_t a0, a1, a2, a3;
+      // chunk index of this k-step inside its 64-column block: (ks & 3) * 2 (+ k_hi), XOR-swizzled on the TMA path
+      ldmatrix_x4(a0, a1, a2, a3, TMA ? kb + (ks >> 2) * 2048 + (k_sw ^ ((ks & 3) << 5)) : kb + ks * 32);
 #pragma unroll
-      for (int np = 0; np < 2; ++np) {
-        uint32_t b0, b1, b2, b3;
-        // chunk index of this k-step inside its 64-column block: (ks & 3) * 2 (+ k_hi), XOR-swizzled on the TMA path
-        ldmatrix_x4(b0, b1, b2, b3, TMA ? kb + np * blk16 + (ks >> 2) * 2048 + (k_sw ^ ((ks & 3) << 5))
-                                        : kb + np * blk16 + ks * 32);
-        mma_bf16_16816(S[2 * np][0], S[2 * np][1], S[2 * np][2], S[2 * np][3], qhi[ks][0], qhi[ks][1], qhi[ks][2], qhi[ks][3], b0, b1);
-        mma_bf16_16816(S[2 * np + 1][0], S[2 * np + 1][1], S[2 * np + 1][2], S[2 * np + 1][3], qhi[ks][0], qhi[ks][1], qhi[ks][2], qhi[ks][3], b2, b3);
+      for (int nt = 0; nt < NT; ++nt) {
+        if (ks & 1) mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, qhi[nt][ks][0], qhi[nt][ks][1]);
+        else        mma_bf16_16816(sa[nt][0], sa[nt][1], sa[nt][2], sa[nt][3], a0, a1, a2, a3, qhi[nt][ks][0], qhi[nt][ks][1]);
         if (use_lo) {
-          mma_bf16_16816(S[2 * np][0], S[2 * np][1], S[2 * np][2], S[2 * np][3], qlo[ks][0], qlo[ks][1], qlo[ks][2], qlo[ks][3], b0, b1);
-          mma_bf16_16816(S[2 * np + 1][0], S[2 * np + 1][1], S[2 * np + 1][2], S[2 * np + 1][3], qlo[ks][0], qlo[ks][1], qlo[ks][2], qlo[ks][3], b2, b3);
+          if (ks & 1) mma_bf16_16816(sa[nt][0], sa[nt][1], sa[nt][2], sa[nt][3], a0, a1, a2, a3, qlo[nt][ks][0], qlo[nt][ks][1]);
+          else        mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, qlo[nt][ks][0], qlo[nt][ks][1]);
         }
-      }
-    }
-    // ---- online softmax (exp2 domain), rows gq and gq + 8
-    float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F;
-#pragma unroll
-    for (int n = 0; n < 4; ++n) {
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int tr = n * 8 + 2 * t4 + e;
-        const bool ok = tr >= row_lo && tr < row_hi;
-        S[n][e] = ok ? S[n][e] * scale_log2 : -CUDART_INF_F;
-        S[n][2 + e] = ok ? S[n][2 + e] * scale_log2 : -CUDART_INF_F;
-        mx0 = fmaxf(mx0, S[n][e]); mx1 = fmaxf(mx1, S[n][2 + e]);
-      }
-    }
-    mx0 = quad_max(mx0); mx1 = quad_max(mx1);
-    const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
-    const float ms0 = (mn0 == -CUDART_INF_F) ? 0.f : mn0, ms1 = (mn1 == -CUDART_INF_F) ? 0.f : mn1;
-    const float al0 = exp2f(m_run[0] - ms0), al1 = exp2f(m_run[1] - ms1);
-    m_run[0] = mn0; m_run[1] = mn1;
-    float ps0 = 0.f, ps1 = 0.f;
-#pragma unroll
-    for (int n = 0; n < 4; ++n) {
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        S[n][e] = exp2f(S[n][e] - ms0); ps0 += S[n][e];
-        S[n][2 + e] = exp2f(S[n][2 + e] - ms1); ps1 += S[n][2 + e];
-      }
-    }
-    l_run[0] = l_run[0] * al0 + ps0; l_run[1] = l_run[1] * al1 + ps1;
-#pragma unroll
-    for (int n = 0; n < 2 * KS; ++n) { O[n][0] *= al0; O[n][1] *= al0; O[n][2] *= al1; O[n][3] *= al1; }
-    // ---- O += P V
-    const uint32_t vb = smem_u32(st + g.st_v) + v_lane;
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-      const uint32_t pa0 = pack_bf16x2(S[2 * j][0], S[2 * j][1]), pa1 = pack_bf16x2(S[2 * j][2], S[2 * j][3]);
-      const uint32_t pa2 = pack_bf16x2(S[2 * j + 1][0], S[2 * j + 1][1]), pa3 = pack_bf16x2(S[2 * j + 1][2], S[2 * j + 1][3]);
-#pragma unroll
-      for (int dp = 0; dp < KS; ++dp) {
-        uint32_t v0, v1, v2, v3;
-        ldmatrix_x4_trans(v0, v1, v2, v3, TMA ? vb + j * blk16 + (dp >> 2) * 2048 + (v_sw ^ ((dp & 3) << 5))
-                                              : vb + j * blk16 + dp * 32);
-        mma_bf16_16816(O[2 * dp][0], O[2 * dp][1], O[2 * dp][2], O[2 * dp][3], pa0, pa1, pa2, pa3, v0, v1);
-        mma_bf16_16816(O[2 * dp + 1][0], O[2 * dp + 1][1], O[2 * dp + 1][2], O[2 * dp + 1][3], pa0, pa1, pa2, pa3, v2, v3);
       }
     }
     __syncwarp();
-    if (lane == 0) mbar_arrive(&empty_bar[stage]);          // the stage's shared memory is no longer read below
-    if (++stage == g.n_stages) { stage = 0; phase ^= 1; }
+    if (lane == 0) mbar_arrive(&empty_bar[kbox]);               // the K box is no longer read
 
-    if (hdr.w & HDR_LAST) {
-      // ---- per-(split, head) softmax state -> partials: o normalised, lse in natural log
-      const float l0 = quad_sum(l_run[0]), l1 = quad_sum(l_run[1]);
-      const float inv0 = l0 > 0.f ? 1.f / l0 : 0.f, inv1 = l1 > 0.f ? 1.f / l1 : 0.f;
+    // ---- online softmax (exp2 domain) per query head (column); thread holds tokens gq, gq+8 x heads 2*t4, 2*t4+1
+    const bool partial = hdr.y & HDR_PARTIAL;
+    const int row_lo = hdr.z & 0xff, row_hi = hdr.z >> 8;
+    const bool ok0 = !partial || (gq >= row_lo && gq < row_hi);
+    const bool ok1 = !partial || (gq + 8 >= row_lo && gq + 8 < row_hi);
+    uint32_t pb[NT][2];
+    float al[NT][2];
+    bool rescale = false;
 #pragma unroll
-      for (int rs = 0; rs < 2; ++rs) {
-        const int row = gq + rs * 8;
-        if (row < g.G) {
-          const size_t slot = (static_cast<size_t>(item_b) * g.Hq + static_cast<size_t>(head) * g.G + row) * p.max_splits + item_split;
-          float* po = p.part_o + slot * g.Dv + 2 * t4;
-          const float inv = rs ? inv1 : inv0;
+    for (int nt = 0; nt < NT; ++nt) {
+      float v[4];
 #pragma unroll
-          for (int n = 0; n < 2 * KS; ++n)
-            *reinterpret_cast<float2*>(po + n * 8) = make_float2(O[n][2 * rs] * inv, O[n][2 * rs + 1] * inv);
-          if (t4 == 0) {
-            const float l = rs ? l1 : l0, m = rs ? m_run[1] : m_run[0];
-            p.part_lse[slot] = l > 0.f ? (m + log2f(l)) * 0.6931471805599453f : -CUDART_INF_F;
+      for (int e = 0; e < 4; ++e) {
+        const float sv = (sa[nt][e] + sb[nt][e]) * scale_log2;
+        v[e] = ((e < 2) ? ok0 : ok1) ? sv : -CUDART_INF_F;
+      }
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const float mx = col_max(fmaxf(v[e], v[2 + e]));
+        const float mn = fmaxf(m_run[nt][e], mx);
+        const float ms = (mn == -CUDART_INF_F) ? 0.f : mn;
+        al[nt][e] = ex2(m_run[nt][e] - ms);
+        m_run[nt][e] = mn;
+        v[e] = ex2(v[e] - ms); v[2 + e] = ex2(v[2 + e] - ms);
+        l_run[nt][e] = fmaf(l_run[nt][e], al[nt][e], v[e] + v[2 + e]);
+        rescale |= (al[nt][e] != 1.f);
+      }
+      // P^T as the B operand: b0 = P[tokens 2t,2t+1][head g], b1 = P[tokens 2t+8,2t+9][head g]
+      pb[nt][0] = movmatrix_trans(pack_bf16x2(v[0], v[1]));
+      pb[nt][1] = movmatrix_trans(pack_bf16x2(v[2], v[3]));
+    }
+    if (__any_sync(0xffffffffu, rescale)) {
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int n = 0; n < KS; ++n) { O[nt][n][0] *= al[nt][0]; O[nt][n][1] *= al[nt][1]; O[nt][n][2] *= al[nt][0]; O[nt][n][3] *= al[nt][1]; }
+    }
+
+    // ---- O^T[d][head] += V^T P^T
+    mbar_wait(&full_bar[box], phase);
+    uint8_t* vbox = box0 + static_cast<size_t>(box) * g.box_bytes;
+    const int vboxi = box;
+    if (++box == g.n_boxes) { box = 0; phase ^= 1; }
+    if (partial) {
+      // rows outside the chunk may hold anything (another chunk's tokens, uninitialised pages): 0 * NaN must not reach O
+      for (int idx = lane; idx < 16 * (D / 8); idx += 32) {
+        const int r = idx / (D / 8), j = idx - r * (D / 8);       // token row, 16-byte chunk of this head's D columns
+        if (r < row_lo || r >= row_hi) {
+          uint8_t* dst = TMA ? vbox + ((warp * (D / 64) + (j >> 3)) * 16 + r) * 128 + (((j & 7) ^ (r & 7)) << 4)
+                             : vbox + r * g.s_row + warp * D * 2 + j * 16;
+          *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
+        }
+      }
+      __syncwarp();
+    }
+    const uint32_t vb = smem_u32(vbox) + v_lane;
+#pragma unroll
+    for (int dp = 0; dp < KS; ++dp) {
+      uint32_t a0, a1, a2, a3;
+      ldmatrix_x4_trans(a0, a1, a2, a3, TMA ? vb + (dp >> 2) * 2048 + (v_sw ^ ((dp & 3) << 5)) : vb + dp * 32);
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+        mma_bf16_16816(O[nt][dp][0], O[nt][dp][1], O[nt][dp][2], O[nt][dp][3], a0, a1, a2, a3, pb[nt][0], pb[nt][1]);
+    }
+    if (partial) fence_proxy_async();                           // the zeroed rows were generic-proxy writes; the next fill is TMA
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty_bar[vboxi]);
+
+    if (hdr.y & HDR_LAST) {
+      // ---- per-(segment, head) softmax state -> partials: o normalised, lse in natural log
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int hq = nt * 8 + 2 * t4 + e;
+          const float l = col_sum(l_run[nt][e]);
+          if (hq < g.G) {
+            const float inv = l > 0.f ? 1.f / l : 0.f;
+            const size_t row = static_cast<size_t>(seg) * g.R + warp * g.G + hq;
+            float* po = p.part_o + row * g.Dv + gq;
+#pragma unroll
+            for (int n = 0; n < KS; ++n) { po[n * 16] = O[nt][n][e] * inv; po[n * 16 + 8] = O[nt][n][2 + e] * inv; }
+            if (gq == 0) p.part_lse[row] = l > 0.f ? (m_run[nt][e] + log2f(l)) * 0.6931471805599453f : -CUDART_INF_F;
           }
         }
       }
@@ -402,26 +501,48 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
   }
 }
 
-void launch_decode(const DecodeGeom& g, const DecodeParams& p, int grid, cudaStream_t st) {
-  const int threads = (g.HG + 1) * 32;
-  auto go = [&](auto kern) {
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    kern<<<grid, threads, g.smem_bytes, st>>>(g, p);
-  };
-  if (g.D == 128) { if (g.use_tma) go(kam_paged_decode_kernel<8, true>); else go(kam_paged_decode_kernel<8, false>); }
-  else            { if (g.use_tma) go(kam_paged_decode_kernel<4, true>); else go(kam_paged_decode_kernel<4, false>); }
+namespace {
+template <typename F> void decode_dispatch(const DecodeGeom& g, F&& f) {
+  if (g.D == 128) {
+    if (g.NT == 1) { if (g.use_tma) f(kam_paged_decode_kernel<8, 1, true>); else f(kam_paged_decode_kernel<8, 1, false>); }
+    else           { if (g.use_tma) f(kam_paged_decode_kernel<8, 2, true>); else f(kam_paged_decode_kernel<8, 2, false>); }
+  } else {
+    if (g.NT == 1) { if (g.use_tma) f(kam_paged_decode_kernel<4, 1, true>); else f(kam_paged_decode_kernel<4, 1, false>); }
+    else           { if (g.use_tma) f(kam_paged_decode_kernel<4, 2, true>); else f(kam_paged_decode_kernel<4, 2, false>); }
+  }
+}
+}  // namespace
+
+int decode_occupancy(const DecodeGeom& g) {
+  int n = 0;
+  decode_dispatch(g, [&](auto kern) {
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, (g.HG + 1) * 32, g.smem_bytes) != cudaSuccess) { cudaGetLastError(); n = 0; }
+  });
+  return n;
+}
+
+void launch_decode(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st) {
+  decode_dispatch(g, [&](auto kern) {
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
+    kern<<<g.n_ctas, (g.HG + 1) * 32, g.smem_bytes, st>>>(g, p);
+  });
 }
 
 // ---------------------------------------------------------------------------------------------------- merge
-// A9: lse = ln sum_s e^{lse_s};  out = sum_s e^{lse_s - lse} o_s.  Fixed summation order => run-to-run deterministic.
+// A9: lse = ln sum_s e^{lse_s};  out = sum_s e^{lse_s - lse} o_s over the request's segments of this head's group.
+// Fixed summation order => run-to-run deterministic.
 __global__ void __launch_bounds__(128) kam_lse_merge_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
   const int bh = blockIdx.x;                      // b * Hq + hq
-  const int b = bh / g.Hq;
-  const int ns = p.n_splits[b];
-  const float* pl = p.part_lse + static_cast<size_t>(bh) * p.max_splits;
-  const float* po = p.part_o + static_cast<size_t>(bh) * p.max_splits * g.Dv;
+  const int b = bh / g.Hq, hq = bh - b * g.Hq;
+  const int hg = hq / g.R, r = hq - hg * g.R;
+  const int N = p.plan.n_chunks;
+  const int s0 = p.plan.seg_base[hg * N + p.plan.rcb[b]], s1 = p.plan.seg_base[hg * N + p.plan.rcb[b + 1]];
+  const float* pl = p.part_lse + r;
+  const float* po = p.part_o + static_cast<size_t>(r) * g.Dv;
+  const size_t so = static_cast<size_t>(g.R) * g.Dv;
   float m = -CUDART_INF_F;
-  for (int s = 0; s < ns; ++s) m = fmaxf(m, pl[s]);
+  for (int s = s0; s < s1; ++s) m = fmaxf(m, pl[static_cast<size_t>(s) * g.R]);
   __nv_bfloat16* out = static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(bh) * g.Dv;
   if (m == -CUDART_INF_F) {                       // no tokens at all: out = 0, lse = -inf, no NaN
     for (int c = threadIdx.x; c < g.Dv; c += blockDim.x) out[c] = __float2bfloat16_rn(0.f);
@@ -429,18 +550,18 @@ __global__ void __launch_bounds__(128) kam_lse_merge_kernel(const __grid_constan
     return;
   }
   float tot = 0.f;
-  for (int s = 0; s < ns; ++s) tot += __expf(pl[s] - m);
+  for (int s = s0; s < s1; ++s) tot += __expf(pl[static_cast<size_t>(s) * g.R] - m);
   const float inv = 1.f / tot;
   for (int c = threadIdx.x; c < g.Dv; c += blockDim.x) {
     float acc = 0.f;
-    for (int s = 0; s < ns; ++s) acc = fmaf(__expf(pl[s] - m), po[static_cast<size_t>(s) * g.Dv + c], acc);
+    for (int s = s0; s < s1; ++s) acc = fmaf(__expf(pl[static_cast<size_t>(s) * g.R] - m), po[s * so + c], acc);
     out[c] = __float2bfloat16_rn(acc * inv);
   }
   if (threadIdx.x == 0) p.lse[bh] = m + logf(tot);
 }
 
 void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st) {
-  kam_lse_merge_kernel<<<p.batch * g.Hq, 128, 0, st>>>(g, p);
+  kam_lse_merge_kernel<<<p.plan.batch * g.Hq, 128, 0, st>>>(g, p);
 }
 
 }  // namespace kam

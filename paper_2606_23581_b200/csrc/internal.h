@@ -89,31 +89,54 @@ void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, int grid, cu
 void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
 
 // ---------------------------------------------------------------- decode
-constexpr int kDecTT = 32;                 // tokens per pipeline stage
+constexpr int kDecTile = 16;               // tokens per pipeline box (one TMA box of K or of V)
 constexpr int kDecMaxHG = 4;               // KV heads (= compute warps) per CTA
+constexpr int kDecPlanThreads = 1024;
 
 struct DecodeGeom {
   int32_t Hq, H, G, D, Dv, P, P_shift;
-  int32_t HG, n_hg;              // KV heads per work unit, units per token row
+  int32_t HG, n_hg;              // KV heads per work unit (one compute warp each), units per token row
+  int32_t R;                     // query rows per unit = HG * G (rows of one partial)
+  int32_t NT;                    // 8-wide query-head tiles per KV head: ceil(G / 8)
   int32_t rope_off, d_r, rope_style;
-  int32_t row_bytes, slice_bytes, s_row;      // s_row: padded stride of a token's slice in shared memory ((s_row/16) odd)
-  int32_t n_stages, stage_bytes, st_k, st_v, st_uk, st_uv, st_hdr, su_row;
-  int32_t off_warp, off_stage0, smem_bytes;   // off_warp: per-warp scratch (sin/cos table, z / y staging)
-  int32_t warp_bytes;
-  int32_t split_tokens;
-  int32_t max_rank;              // 0: no on-read patch in this call
+  int32_t row_bytes, slice_bytes, s_row;      // s_row: padded stride of a token's slice in shared memory (bulk-copy path)
+  int32_t n_boxes, box_bytes;    // ring of boxes; K and V tiles alternate (even = K, odd = V)
+  int32_t off_hdr, off_box0, smem_bytes;
   int32_t use_tma;               // 1: pool pages arrive as 16-token swizzled TMA boxes; 0: one padded bulk copy per token
-  int32_t ncb, box_bytes;        // TMA path: 64-column blocks per slice, bytes of one 16-token box
-  double theta;
+  int32_t ncb;                   // TMA path: 64-column blocks per slice
+  int32_t n_ctas;                // persistent grid: sm_count * CTAs per SM
+  int32_t max_rank;              // 0: no on-read patch in this call
 };
 
-struct DecodeItem {              // one split = a contiguous token range inside ONE chunk of one request
-  long long bt_off;              // index of the page list's first entry in the block-table array
+struct DecChunk {                // plan input: one chunk of one request (flat, request-major)
+  long long bt_off;              // index of the chunk's page list (its first entry) in the block-table array
   long long delta;               // RoPE offset to apply on read
-  int32_t b, chunk;              // request index in the batch, chunk index in the request
+  int32_t b;                     // request index in the batch
   int32_t tok0, n_tok;           // tokens [tok0, tok0 + n_tok) of that page list
-  int32_t split;                 // partial slot within the request
-  int32_t ctok0;                 // first token relative to the chunk start (indexes U when patching on read)
+  int32_t patch;                 // index into the patch-ref array, or -1
+};
+
+struct DecSeg {                  // plan output: a run of 16-token tiles inside ONE chunk, owned by one CTA
+  long long bt_off;
+  int32_t chunk;                 // flat chunk index (row of the cos/sin table, patch lookup)
+  int32_t b, hg;
+  int32_t tile0, n_tiles;        // tiles [tile0, tile0 + n_tiles) of the page list, 16 tokens each
+  int32_t tok_lo, tok_hi;        // the chunk's tokens of that page list: rows outside are masked
+  int32_t rotate;                // 1: delta != 0, q is rotated by -delta on read
+  int32_t patch;                 // index into the patch-ref array, or -1
+  int32_t pad;
+};
+
+struct DecodePlan {              // device pointers into the workspace; filled by the plan kernel
+  DecChunk* chunks;              // [n_chunks]
+  int32_t* rcb;                  // [batch + 1] request -> first flat chunk
+  int32_t* tile_pre;             // [n_chunks + 1]
+  int32_t* seg_base;             // [n_hg * n_chunks + 1]
+  DecSeg* segs;                  // [max_segs]
+  int32_t* cta_seg;              // [n_ctas + 1]
+  float2* cs;                    // [n_chunks][d_r / 2] (cos, sin)(delta f_i)
+  const double* inv_freq;        // [d_r / 2] f_i = theta^(-2i/d_r), fp64, written at kam_create
+  int32_t n_chunks, batch, max_segs;
 };
 
 struct DecodeParams {
@@ -123,25 +146,32 @@ struct DecodeParams {
   int32_t layer;
   const int32_t* block_tables;
   const void* tmaps;             // device array of CUtensorMap [n_layers][2] over the context's pool (TMA path)
-  const DecodeItem* items;
-  const int32_t* n_items;        // device scalar
-  int32_t* work_counter;         // device scalar, zero on entry
-  const kam_patch_ref* patches;  // [B][max_chunks] or nullptr
-  int32_t max_chunks;
-  float* part_o;                 // [B][Hq][max_splits][Dv]
-  float* part_lse;               // [B][Hq][max_splits]
-  const int32_t* n_splits;       // [B]
-  int32_t max_splits;
+  DecodePlan plan;
+  const kam_patch_ref* patches;  // device array or nullptr
+  float* part_o;                 // [max_segs][R][Dv]
+  float* part_lse;               // [max_segs][R]
   float sm_scale;
   void* out;                     // [B][Hq][Dv] bf16
   float* lse;                    // [B][Hq]
-  int32_t batch;
 };
 
-void launch_decode_plan(const int32_t* chunk_starts, const long long* chunk_offsets, const int32_t* n_chunks,
-                        int32_t max_chunks, int32_t max_pages, int32_t batch, int32_t split_tokens, int32_t max_splits,
-                        DecodeItem* items, int32_t* n_items, int32_t* n_splits, int32_t* work_counter, cudaStream_t st);
-void launch_decode(const DecodeGeom& g, const DecodeParams& p, int grid, cudaStream_t st);
+struct DecodeCsr {               // front end of the plan kernel for the stateless call (device metadata)
+  const int32_t* chunk_starts;   // [B][max_chunks + 1]
+  const long long* chunk_offsets;  // [B][max_chunks] or nullptr
+  const int32_t* n_chunks;       // [B]
+  int32_t max_chunks, max_pages;
+  int32_t enabled;               // 0: plan.chunks / plan.rcb were uploaded by the host (window store)
+  int32_t has_patches;           // patch index of chunk (b, c) = b * max_chunks + c
+};
+
+// KV heads per decode work unit (= compute warps per CTA): the largest divisor of n_kv_heads <= kDecMaxHG.
+inline int decode_head_group(const kam_layout& L) {
+  for (int h = L.n_kv_heads < kDecMaxHG ? L.n_kv_heads : kDecMaxHG; h >= 1; --h) if (L.n_kv_heads % h == 0) return h;
+  return 1;
+}
+int decode_occupancy(const DecodeGeom& g);     // resident CTAs per SM of the decode kernel this geometry selects
+void launch_decode_plan(const DecodeGeom& g, const DecodePlan& plan, const DecodeCsr& csr, cudaStream_t st);
+void launch_decode(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st);
 void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st);
 
 }  // namespace kam
