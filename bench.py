@@ -8,7 +8,9 @@ A STEP is one pass of the whole hot path over one b
                                       patches into one request's pages, ONE launch           (A1-A5)   <- the headline metric
   phase B  kam_evict + kam_admit    : the request's window slides: oldest chunk out (its 7 survivors re-rotate in place by
                                       -1024), one evicted chunk recalled by relocate+patch      (A6, A7)
-  phase C  kam_window_decode        : fused paged decode over every request's 8192-token window, 28 layers, LSE merge (A8, A9)
+  phase C  kam_window_plan + 28 x kam_window_decode : fused paged decode over every request's 8192-token window, all
+                                      layers, LSE merge (A8, A9).  The 28 per-layer calls (2 kernels each) are captured once
+                                      into a CUDA graph and replayed; the plan is rebuilt eagerly every step (the window slid)
 Inputs are resident in HBM before the timed region; every step touches > 1 GB of fresh source and destination memory
 (the B200 L2 is 126 MB), and the request / canonical set rotate from step to step.
 
@@ -30,7 +32,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 CFG_ID = 2
-N_REQ = 8               # requests per GPU (decode batch; each owns an 8-chunk window)
+N_REQ = 32              # requests per GPU = decode batch (configs[1] names none; 32 is configs[3]'s); each owns an 8-chunk window
 N_SETS = 2              # canonical chunk sets cycled so that sources miss L2
 
 
@@ -87,7 +89,7 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------------------------------- the workload
 class Workload:
-    def __init__(self, device, rank):
+    def __init__(self, device, rank, use_graph=True):
         import numpy as np
         import torch
 
@@ -145,9 +147,25 @@ class Workload:
         self.bytes_c_layer = N_REQ * 2 * self.n_chunks * T * H * D * 2
         self.bytes_c = L * self.bytes_c_layer
         torch.cuda.synchronize()
+        # phase C as a CUDA graph: with a valid plan kam_window_decode launches exactly two kernels and nothing else
+        self.graph, self.graph_replays = None, 0
+        if use_graph:
+            self.ctx_b.kam_window_plan(self.req_ids)
+            self.decode_layers()                                   # eager once: workspace sized, kernels loaded
+            torch.cuda.synchronize()
+            self.graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(self.graph):
+                self.decode_layers()
+            torch.cuda.synchronize()
+
+    def decode_layers(self):
+        for l in range(self.cfg.n_layers):
+            self.ctx_b.kam_window_decode(self.q, self.req_ids, l, self.sm_scale, self.out, self.lse)
 
     def launches(self):
-        return self.ctx_a.kam_get_stats()["kernels_launched"] + self.ctx_b.kam_get_stats()["kernels_launched"]
+        """Kernels launched so far: the contexts' own counters + 2 per layer for every graph replay."""
+        return (self.ctx_a.kam_get_stats()["kernels_launched"] + self.ctx_b.kam_get_stats()["kernels_launched"]
+                + self.graph_replays * 2 * self.cfg.n_layers)
 
     def step(self, i, ev=None):
         cfg, B, T, m = self.cfg, self.B, self.cfg.chunk_tokens, self.cfg.rank
@@ -165,8 +183,12 @@ class Workload:
         self.ctx_b.kam_admit(r, B.KAM_BACK, ch, pa, m, 1)
         rec(2)
         # phase C: every request decodes one token over its window, all layers
-        for l in range(cfg.n_layers):
-            self.ctx_b.kam_window_decode(self.q, self.req_ids, l, self.sm_scale, self.out, self.lse)
+        self.ctx_b.kam_window_plan(self.req_ids)
+        if self.graph is not None:
+            self.graph.replay()
+            self.graph_replays += 1
+        else:
+            self.decode_layers()
         rec(3)
 
 
@@ -296,6 +318,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--profile-step", action="store_true",
+                    help="bracket the first timed step with cudaProfilerStart/Stop (for `ncu --profile-from-start off`)")
+    ap.add_argument("--no-graph", action="store_true", help="launch the per-layer decode calls eagerly instead of replaying a CUDA graph")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -313,7 +338,7 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=device)
 
-    wl = Workload(device, rank)
+    wl = Workload(device, rank, use_graph=not args.no_graph)
     peak, peak_src = peaks()
 
     def barrier():
@@ -332,7 +357,11 @@ def main():
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t_start.record()
     for i in range(args.steps):
+        if args.profile_step and i == 0:
+            torch.cuda.profiler.start()
         wl.step(args.warmup + i, ev[i])
+        if args.profile_step and i == 0:
+            torch.cuda.profiler.stop()
     t_end.record()
     barrier()
     clocks = sampler.stop() if rank == 0 else None
@@ -395,6 +424,7 @@ def main():
             "config": {"workload": "BASELINE.json configs[1]: GQA Qwen2-VL-7B-like, 28 layers, 28q/4kv heads, head_dim 128, theta 1e6, "
                                    "8 chunks x 1024 tokens per slide, rank-16 patch, page 16, offsets U[0,32768)",
                        "requests_per_gpu": N_REQ, "decode_batch": N_REQ, "window_tokens": wl.n_chunks * T,
+                       "decode_launch": "eager" if args.no_graph else "CUDA graph of 28 x (decode, merge), plan rebuilt eagerly per step",
                        "l2": "inputs larger than L2: each step streams >1 GB of fresh source and destination; request and canonical set rotate",
                        "parallelism": "requests sharded over ranks, no collective"},
             "phases_ms": {"relocate_patch_batch": ms_a, "window_slide": ms_b, "decode_all_layers": ms_c},

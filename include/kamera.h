@@ -202,7 +202,13 @@ kam_status kam_paged_decode_merge(kam_ctx *ctx, const void *q, const kam_pool *p
                                   int32_t max_pages, const int32_t *chunk_starts, const int64_t *chunk_offsets,
                                   const int32_t *n_chunks, int32_t max_chunks, const kam_patch_ref *patches,
                                   int32_t layer, int32_t batch, float sm_scale, void *out, float *lse, void *stream);
-/* Same, over the context's own windows: request ids req_ids[0..batch) (host).  Pending lazy deltas are applied on read. */
+/* Same, over the context's own windows: request ids req_ids[0..batch) (host).  Pending lazy deltas are applied on read.
+ * The work split of a step (which 16-token tiles each persistent CTA streams, the per-chunk cos/sin tables) depends on
+ * the windows only, not on the layer: kam_window_plan builds it (one small H2D copy + one kernel); kam_window_decode
+ * builds it itself when the windows or the request list changed since the last plan and otherwise launches exactly two
+ * kernels (decode, merge) and nothing else - in that state it may be captured into a CUDA graph.  A context serves one
+ * stream at a time: the plan and the partials live in its workspace. */
+kam_status kam_window_plan(kam_ctx *ctx, const int32_t *req_ids, int32_t batch, void *stream);
 kam_status kam_window_decode(kam_ctx *ctx, const void *q, const int32_t *req_ids, int32_t batch, int32_t layer,
                              float sm_scale, void *out, float *lse, void *stream);
 /* Same as kam_paged_decode_merge with q, out and lse in HOST memory (H2D / D2H on `stream`, then a stream sync). */

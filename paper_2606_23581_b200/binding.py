@@ -80,6 +80,7 @@ SIGNATURES = {
     "kam_get_stats": (i32, [vp, C.POINTER(kam_stats)]),
     "kam_paged_decode_merge": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
                                      vp, vp, vp]),
+    "kam_window_plan": (i32, [vp, C.POINTER(i32), i32, vp]),
     "kam_window_decode": (i32, [vp, vp, C.POINTER(i32), i32, i32, C.c_float, vp, vp, vp]),
     "kam_paged_decode_merge_host": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32,
                                           C.c_float, vp, vp, vp]),
@@ -276,6 +277,10 @@ class Context:
                                             max_pages, _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks),
                                             max_chunks, _ptr(patches), int(layer), batch, float(sm_scale), _ptr(out),
                                             _ptr(lse), _stream_ptr(stream)), self.h)
+
+    def kam_window_plan(self, req_ids, stream=None):
+        ids = (i32 * len(req_ids))(*req_ids)
+        _check(lib().kam_window_plan(self.h, ids, len(req_ids), _stream_ptr(stream)), self.h)
 
     def kam_window_decode(self, q, req_ids, layer, sm_scale, out, lse, stream=None):
         ids = (i32 * len(req_ids))(*req_ids)

@@ -398,6 +398,7 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
     build_pool_tensor_maps(c);
     if (const char* ev = getenv("KAM_DEC_CTAS_PER_SM")) c->dec_ctas_per_sm = atoi(ev);
     if (const char* ev = getenv("KAM_DEC_BOXES")) c->dec_boxes = atoi(ev);
+    if (const char* ev = getenv("KAM_NO_PDL")) c->use_pdl = (ev[0] == '0');
     if (layout->rope_dim > 0) {                // f_i = theta^(-2i/d_r) in fp64, once (R-2)
       std::vector<double> f((size_t)layout->rope_dim / 2);
       for (size_t i = 0; i < f.size(); ++i) f[i] = pow(layout->rope_theta, -2.0 * (double)i / layout->rope_dim);

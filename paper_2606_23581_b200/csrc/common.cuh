@@ -53,6 +53,11 @@ __device__ __forceinline__ void tma_load_3d(void* dst_smem, const void* tmap, in
 // Orders prior generic-proxy accesses of shared memory before later async-proxy (bulk copy) accesses.
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// Programmatic dependent launch: wait for the kernels this launch depends on (their memory is then visible) / allow the
+// dependent launch to start its prologue.  Both are no-ops for a launch without the attribute.
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }

@@ -56,6 +56,9 @@ struct kam_ctx {
   std::vector<int32_t> winplan_reqs;
   int32_t winplan_chunks = 0;
   double* d_inv_freq = nullptr;                // [rope_dim / 2] f_i = theta^(-2i/d_r), fp64
+  kam::DecodeGeom dec_geom[2];                 // cached geometry: [0] bulk-copy path, [1] TMA path over the context's pool
+  bool dec_geom_ok[2] = {false, false};
+  bool use_pdl = true;                         // programmatic dependent launch between decode and merge (KAM_NO_PDL=1 turns it off)
   int dec_ctas_per_sm = 0, dec_boxes = 0;      // tuning switches (KAM_DEC_CTAS_PER_SM, KAM_DEC_BOXES); 0 = automatic
   // device staging of host-resident chunks (kam_relocate_patch_host) and host-resident q/out (decode host variant)
   void* d_hstage = nullptr;

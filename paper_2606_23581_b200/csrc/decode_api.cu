@@ -14,6 +14,8 @@ inline size_t align_up_sz(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // Geometry of the decode kernel for this context's layout; `ctas_per_sm` = 0 picks the densest configuration that fits.
 kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
   const kam_layout& L = c->lay;
+  const int variant = (c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers) ? 1 : 0;
+  if (c->dec_geom_ok[variant]) { *out = c->dec_geom[variant]; return KAM_OK; }
   if (L.elem_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "decode needs a bf16 pool");
   if (!L.has_v) return fail(c, KAM_ERR_UNSUPPORTED, "decode over an MLA latent pool is not built yet (SURVEY.md 8(f) f1)");
   if (L.row_dim != 64 && L.row_dim != 128) return fail(c, KAM_ERR_UNSUPPORTED, "decode supports head_dim 64 or 128");
@@ -50,6 +52,7 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
   }
   if (want < 1) return fail(c, KAM_ERR_UNSUPPORTED, "decode tile does not fit shared memory");
   g.n_ctas = c->sm_count * want;
+  c->dec_geom[variant] = g; c->dec_geom_ok[variant] = true;
   *out = g;
   return KAM_OK;
 }
@@ -85,6 +88,7 @@ DecodePlan plan_of(kam_ctx* c, const WsLayout& w, int n_chunks, int batch) {
   pl.segs = reinterpret_cast<DecSeg*>(ws + w.segs);
   pl.cs = reinterpret_cast<float2*>(ws + w.cs);
   pl.inv_freq = c->d_inv_freq;
+  pl.block_tables = nullptr;                                      // set by the caller
   pl.n_chunks = n_chunks; pl.batch = batch; pl.max_segs = w.max_segs;
   return pl;
 }
@@ -126,6 +130,7 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   p.q = q; p.pool_k_layers = pool->k_layers; p.pool_v_layers = pool->v_layers; p.layer = layer;
   p.block_tables = block_tables; p.tmaps = c->d_tmaps;
   p.plan = plan_of(c, w, N, batch);
+  p.plan.block_tables = block_tables;
   p.patches = nullptr;
   p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
@@ -135,32 +140,26 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
   csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = 0;
   launch_decode_plan(g, p.plan, csr, st);
-  launch_decode(g, p, st);
-  launch_decode_merge(g, p, st);
+  launch_decode(g, p, false, st);                                 // reads the plan just written: plain stream order
+  launch_decode_merge(g, p, c->use_pdl, st);
   c->kernels_launched += 3;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(c, e, "decode launch");
   return KAM_OK;
 }
 
-kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, int32_t batch, int32_t layer, float sm_scale,
-                             void* out, float* lse, void* stream) {
-  if (!c) return KAM_ERR_INVALID_ARG;
+// The plan (segments, first slots, cos/sin tables) depends only on the windows, not on the layer or the query: it is
+// rebuilt when a window changed (epoch) or the request list differs, and reused by every layer of the same step.
+static kam_status window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch, cudaStream_t st, DecodeGeom* g_out,
+                              WsLayout* w_out, bool* was_cached) {
   if (!c->win) return fail(c, KAM_ERR_STATE, "context was created without a window store");
-  if (!c->has_pool || !c->cuda_ok) return fail(c, KAM_ERR_CUDA, "kam_window_decode needs a context with a pool on a CUDA device");
-  if (!q || !req_ids || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_window_decode: NULL argument");
-  if (layer < 0 || layer >= c->lay.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, c->lay.n_layers);
-  if (batch < 0) return fail(c, KAM_ERR_INVALID_ARG, "negative batch");
+  if (!c->has_pool || !c->cuda_ok) return fail(c, KAM_ERR_CUDA, "window decode needs a context with a pool on a CUDA device");
+  if (!req_ids || batch < 1) return fail(c, KAM_ERR_INVALID_ARG, "window decode: bad request list");
   for (int b = 0; b < batch; ++b)
     if (!c->win->is_open(req_ids[b])) return fail(c, KAM_ERR_STATE, "request %d is not open", req_ids[b]);
-  if (batch == 0) return KAM_OK;
   DecodeGeom g;
   kam_status s = decode_geom(c, &c->pool, &g);
   if (s != KAM_OK) return s;
-  cudaStream_t st = static_cast<cudaStream_t>(stream);
-
-  // The plan (segments, cos/sin tables) depends only on the windows, not on the layer: it is rebuilt when a window
-  // changed (epoch) or the request list differs, and reused by the calls for the other layers of the same step.
   const bool cached = c->winplan_epoch == c->win->epoch() && c->winplan_reqs.size() == (size_t)batch &&
                       std::equal(c->winplan_reqs.begin(), c->winplan_reqs.end(), req_ids);
   int N = c->winplan_chunks;
@@ -169,49 +168,72 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
     for (int b = 0; b < batch; ++b) N += (int)c->win->chunks(req_ids[b]).size();
   }
   const WsLayout w = ws_layout(g, N, batch);
-  if (!cached) {
-    if ((s = grow_ws(c, w.total)) != KAM_OK) return s;
-    // host -> device: the flat chunk list (pending lazy deltas become on-read rotations) and the request index
-    const size_t up_bytes = w.rcb + (size_t)(batch + 1) * 4;
-    Staging* sg;
-    if ((s = staging_acquire(c, up_bytes, &sg)) != KAM_OK) return s;
-    char* h = static_cast<char*>(sg->host);
-    DecChunk* hc = reinterpret_cast<DecChunk*>(h + w.chunks);
-    int32_t* hr = reinterpret_cast<int32_t*>(h + w.rcb);
-    int j = 0;
-    for (int b = 0; b < batch; ++b) {
-      hr[b] = j;
-      int64_t pos = c->win->window_base(req_ids[b]);
-      for (const ChunkRec& r : c->win->chunks(req_ids[b])) {
-        DecChunk ch{};
-        ch.bt_off = (long long)r.slot * c->max_ppc; ch.delta = pos - r.phase;
-        ch.b = b; ch.tok0 = 0; ch.n_tok = r.n_tokens; ch.patch = -1;
-        hc[j++] = ch;
-        pos += r.n_tokens;
-      }
+  *g_out = g; *w_out = w; *was_cached = cached;
+  if (cached) return KAM_OK;
+  if ((s = grow_ws(c, w.total)) != KAM_OK) return s;
+  // host -> device: the flat chunk list (pending lazy deltas become on-read rotations) and the request index
+  const size_t up_bytes = w.rcb + (size_t)(batch + 1) * 4;
+  Staging* sg;
+  if ((s = staging_acquire(c, up_bytes, &sg)) != KAM_OK) return s;
+  char* h = static_cast<char*>(sg->host);
+  DecChunk* hc = reinterpret_cast<DecChunk*>(h + w.chunks);
+  int32_t* hr = reinterpret_cast<int32_t*>(h + w.rcb);
+  int j = 0;
+  for (int b = 0; b < batch; ++b) {
+    hr[b] = j;
+    int64_t pos = c->win->window_base(req_ids[b]);
+    for (const ChunkRec& r : c->win->chunks(req_ids[b])) {
+      DecChunk ch{};
+      ch.bt_off = (long long)r.slot * c->max_ppc; ch.delta = pos - r.phase;
+      ch.b = b; ch.tok0 = 0; ch.n_tok = r.n_tokens; ch.patch = -1;
+      hc[j++] = ch;
+      pos += r.n_tokens;
     }
-    hr[batch] = j;
-    cudaError_t e = cudaMemcpyAsync(c->d_ws, h, up_bytes, cudaMemcpyHostToDevice, st);
-    staging_release(sg, st);
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(window plan)");
   }
+  hr[batch] = j;
+  cudaError_t e = cudaMemcpyAsync(c->d_ws, h, up_bytes, cudaMemcpyHostToDevice, st);
+  staging_release(sg, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(window plan)");
+  DecodePlan pl = plan_of(c, w, N, batch);
+  pl.block_tables = c->d_slot_pages;
+  DecodeCsr csr{};
+  launch_decode_plan(g, pl, csr, st);
+  ++c->kernels_launched;
+  if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(c, e, "decode plan launch");
+  c->winplan_epoch = c->win->epoch();
+  c->winplan_reqs.assign(req_ids, req_ids + batch);
+  c->winplan_chunks = N;
+  return KAM_OK;
+}
+
+kam_status kam_window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (batch == 0) return KAM_OK;
+  DecodeGeom g; WsLayout w; bool cached;
+  return window_plan(c, req_ids, batch, static_cast<cudaStream_t>(stream), &g, &w, &cached);
+}
+
+kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, int32_t batch, int32_t layer, float sm_scale,
+                             void* out, float* lse, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (batch == 0) return KAM_OK;
+  if (!q || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_window_decode: NULL argument");
+  if (layer < 0 || layer >= c->lay.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, c->lay.n_layers);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  DecodeGeom g; WsLayout w; bool cached;
+  kam_status s = window_plan(c, req_ids, batch, st, &g, &w, &cached);
+  if (s != KAM_OK) return s;
   DecodeParams p{};
   p.q = q; p.pool_k_layers = c->pool.k_layers; p.pool_v_layers = c->pool.v_layers; p.layer = layer;
   p.block_tables = c->d_slot_pages; p.tmaps = c->d_tmaps;
-  p.plan = plan_of(c, w, N, batch);
+  p.plan = plan_of(c, w, c->winplan_chunks, batch);
+  p.plan.block_tables = c->d_slot_pages;
   p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse;
-  if (!cached) {
-    DecodeCsr csr{};
-    launch_decode_plan(g, p.plan, csr, st);
-    ++c->kernels_launched;
-    c->winplan_epoch = c->win->epoch();
-    c->winplan_reqs.assign(req_ids, req_ids + batch);
-    c->winplan_chunks = N;
-  }
-  launch_decode(g, p, st);
-  launch_decode_merge(g, p, st);
+  // with a plan from an earlier call the decode prologue may overlap whatever precedes it on the stream (it only reads the plan)
+  launch_decode(g, p, cached && c->use_pdl, st);
+  launch_decode_merge(g, p, c->use_pdl, st);
   c->kernels_launched += 2;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(c, e, "decode launch");

@@ -171,7 +171,12 @@ __global__ void __launch_bounds__(kDecPlanThreads) kam_decode_plan_kernel(const 
       s.n_tiles = static_cast<int>(end - start);
       s.tok_lo = ch.tok0; s.tok_hi = ch.tok0 + ch.n_tok;
       s.rotate = (ch.delta != 0) && g.d_r > 0;
-      s.patch = ch.patch; s.pad = 0;
+      s.patch = ch.patch;
+      {
+        const int tok = s.tile0 * kDecTile;
+        const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
+        s.slot0 = pl.block_tables[ch.bt_off + pg] * g.P + (tok - pg * g.P);
+      }
       pl.segs[base + k] = s;
       const long long i = k == 0 ? ceil_div_ll(start * n_eff, total) : c.i_lo + k - 1;   // the CTA starting exactly here, if any
       if (i < n_eff && (i * total) / n_eff == start) pl.cta_seg[i] = base + k;
@@ -234,6 +239,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
   }
   __syncthreads();
 
+  grid_dep_launch();
   const int seg_begin = p.plan.cta_seg[blockIdx.x], seg_end = p.plan.cta_seg[blockIdx.x + 1];
   if (seg_begin >= seg_end) return;
 
@@ -244,20 +250,23 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
     const char* pv = static_cast<const char*>(p.pool_v_layers[p.layer]);
     const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * 256;
     const char* tm_v = tm_k + 128;
+    DecSeg S_next = p.plan.segs[seg_begin];
+    grid_dep_wait();                                            // nothing of the pool is read before the stream's earlier work is done
     for (int seg = seg_begin; seg < seg_end; ++seg) {
-      const DecSeg S = p.plan.segs[seg];
+      const DecSeg S = S_next;
+      if (seg + 1 < seg_end) S_next = p.plan.segs[seg + 1];     // in flight while this segment streams
       const int32_t* bt = p.block_tables + S.bt_off;
       const size_t col_off = static_cast<size_t>(S.hg) * g.slice_bytes;
       for (int t0 = 0; t0 < S.n_tiles; t0 += 32) {
         int slot = 0;
-        if (t0 + lane < S.n_tiles) {                            // A1: page = block_table[tok / P], slot = page * P + tok % P
+        if (t0 + lane < S.n_tiles && t0 + lane > 0) {           // A1: page = block_table[tok / P], slot = page * P + tok % P
           const int tok = (S.tile0 + t0 + lane) * kDecTile;
           const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
           slot = bt[pg] * g.P + (tok - pg * g.P);
         }
         const int nb = min(32, S.n_tiles - t0);
         for (int i = 0; i < nb; ++i) {
-          const int s0 = __shfl_sync(0xffffffffu, slot, i);
+          const int s0 = (t0 + i == 0) ? S.slot0 : __shfl_sync(0xffffffffu, slot, i);
           const int tl = t0 + i;
           const int tok = (S.tile0 + tl) * kDecTile;
           const int row_lo = max(S.tok_lo - tok, 0), row_hi = min(S.tok_hi - tok, kDecTile);
@@ -324,6 +333,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
 
   int box = 0; uint32_t phase = 0;
   int seg = 0;
+  grid_dep_wait();                                              // q and the partials buffer belong to earlier work until here
   while (true) {
     mbar_wait(&full_bar[box], phase);
     const int4 hdr = hdrs[box];
@@ -516,52 +526,109 @@ template <typename F> void decode_dispatch(const DecodeGeom& g, F&& f) {
 int decode_occupancy(const DecodeGeom& g) {
   int n = 0;
   decode_dispatch(g, [&](auto kern) {
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);   // the launch passes the real size
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, (g.HG + 1) * 32, g.smem_bytes) != cudaSuccess) { cudaGetLastError(); n = 0; }
   });
   return n;
 }
 
-void launch_decode(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st) {
-  decode_dispatch(g, [&](auto kern) {
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
-    kern<<<g.n_ctas, (g.HG + 1) * 32, g.smem_bytes, st>>>(g, p);
-  });
+namespace {
+template <typename K, typename... A>
+void launch_ex(K kern, int grid, int block, int smem, bool pdl, cudaStream_t st, const A&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kern, args...);
+}
+}  // namespace
+
+void launch_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st) {
+  decode_dispatch(g, [&](auto kern) { launch_ex(kern, g.n_ctas, (g.HG + 1) * 32, g.smem_bytes, pdl, st, g, p); });
 }
 
 // ---------------------------------------------------------------------------------------------------- merge
 // A9: lse = ln sum_s e^{lse_s};  out = sum_s e^{lse_s - lse} o_s over the request's segments of this head's group.
-// Fixed summation order => run-to-run deterministic.
-__global__ void __launch_bounds__(128) kam_lse_merge_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
+// One CTA per (request, query head); warp w folds segments s0 + w, s0 + w + 8, ... (four independent loads in flight per
+// lane), then the 8 warp states are folded in warp order.  Fixed assignment and order => run-to-run deterministic.
+constexpr int kMergeWarps = 8;
+constexpr int kMergeUnroll = 4;
+
+template <int CPL>   // columns per lane = Dv / 32
+__global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
+  __shared__ float sm_m[kMergeWarps], sm_l[kMergeWarps];
+  __shared__ float sm_acc[kMergeWarps][32 * CPL];
+  grid_dep_launch();
   const int bh = blockIdx.x;                      // b * Hq + hq
   const int b = bh / g.Hq, hq = bh - b * g.Hq;
   const int hg = hq / g.R, r = hq - hg * g.R;
   const int N = p.plan.n_chunks;
   const int s0 = p.plan.seg_base[hg * N + p.plan.rcb[b]], s1 = p.plan.seg_base[hg * N + p.plan.rcb[b + 1]];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  grid_dep_wait();                                // the partials are complete and visible from here
   const float* pl = p.part_lse + r;
-  const float* po = p.part_o + static_cast<size_t>(r) * g.Dv;
+  const float* po = p.part_o + static_cast<size_t>(r) * g.Dv + lane * CPL;
   const size_t so = static_cast<size_t>(g.R) * g.Dv;
-  float m = -CUDART_INF_F;
-  for (int s = s0; s < s1; ++s) m = fmaxf(m, pl[static_cast<size_t>(s) * g.R]);
+
+  float m = -CUDART_INF_F, l = 0.f, acc[CPL];
+#pragma unroll
+  for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
+  for (int base = s0 + warp; base < s1; base += kMergeWarps * kMergeUnroll) {
+    float ls[kMergeUnroll], o[kMergeUnroll][CPL];
+#pragma unroll
+    for (int u = 0; u < kMergeUnroll; ++u) {
+      const int s = base + u * kMergeWarps;
+      ls[u] = -CUDART_INF_F;
+#pragma unroll
+      for (int c = 0; c < CPL; ++c) o[u][c] = 0.f;
+      if (s < s1) {
+        ls[u] = pl[static_cast<size_t>(s) * g.R];
+        if constexpr (CPL == 4) { const float4 v = *reinterpret_cast<const float4*>(po + s * so); o[u][0] = v.x; o[u][1] = v.y; o[u][2] = v.z; o[u][3] = v.w; }
+        else { const float2 v = *reinterpret_cast<const float2*>(po + s * so); o[u][0] = v.x; o[u][1] = v.y; }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kMergeUnroll; ++u) {
+      if (ls[u] == -CUDART_INF_F) continue;
+      const float mn = fmaxf(m, ls[u]);
+      const float a = __expf(m - mn), w = __expf(ls[u] - mn);
+      l = fmaf(l, a, w);
+#pragma unroll
+      for (int c = 0; c < CPL; ++c) acc[c] = fmaf(acc[c], a, w * o[u][c]);
+      m = mn;
+    }
+  }
+  if (lane == 0) { sm_m[warp] = m; sm_l[warp] = l; }
+#pragma unroll
+  for (int c = 0; c < CPL; ++c) sm_acc[warp][lane * CPL + c] = acc[c];
+  __syncthreads();
+
+  float M = -CUDART_INF_F;
+#pragma unroll
+  for (int w = 0; w < kMergeWarps; ++w) M = fmaxf(M, sm_m[w]);
   __nv_bfloat16* out = static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(bh) * g.Dv;
-  if (m == -CUDART_INF_F) {                       // no tokens at all: out = 0, lse = -inf, no NaN
-    for (int c = threadIdx.x; c < g.Dv; c += blockDim.x) out[c] = __float2bfloat16_rn(0.f);
-    if (threadIdx.x == 0) p.lse[bh] = -CUDART_INF_F;
+  const int c = threadIdx.x;
+  if (M == -CUDART_INF_F) {                       // no tokens at all: out = 0, lse = -inf, no NaN
+    if (c < g.Dv) out[c] = __float2bfloat16_rn(0.f);
+    if (c == 0) p.lse[bh] = -CUDART_INF_F;
     return;
   }
-  float tot = 0.f;
-  for (int s = s0; s < s1; ++s) tot += __expf(pl[static_cast<size_t>(s) * g.R] - m);
-  const float inv = 1.f / tot;
-  for (int c = threadIdx.x; c < g.Dv; c += blockDim.x) {
-    float acc = 0.f;
-    for (int s = s0; s < s1; ++s) acc = fmaf(__expf(pl[static_cast<size_t>(s) * g.R] - m), po[s * so + c], acc);
-    out[c] = __float2bfloat16_rn(acc * inv);
+  float tot = 0.f, v = 0.f;
+#pragma unroll
+  for (int w = 0; w < kMergeWarps; ++w) {
+    const float e = sm_m[w] == -CUDART_INF_F ? 0.f : __expf(sm_m[w] - M);
+    tot = fmaf(sm_l[w], e, tot);
+    if (c < g.Dv) v = fmaf(sm_acc[w][c], e, v);
   }
-  if (threadIdx.x == 0) p.lse[bh] = m + logf(tot);
+  if (c < g.Dv) out[c] = __float2bfloat16_rn(v / tot);
+  if (c == 0) p.lse[bh] = M + logf(tot);
 }
 
-void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st) {
-  kam_lse_merge_kernel<<<p.plan.batch * g.Hq, 128, 0, st>>>(g, p);
+void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st) {
+  if (g.Dv == 128) launch_ex(kam_lse_merge_kernel<4>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
+  else             launch_ex(kam_lse_merge_kernel<2>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
 }
 
 }  // namespace kam

@@ -124,7 +124,7 @@ struct DecSeg {                  // plan output: a run of 16-token tiles inside 
   int32_t tok_lo, tok_hi;        // the chunk's tokens of that page list: rows outside are masked
   int32_t rotate;                // 1: delta != 0, q is rotated by -delta on read
   int32_t patch;                 // index into the patch-ref array, or -1
-  int32_t pad;
+  int32_t slot0;                 // pool slot of the segment's first tile (saves the producer one dependent load)
 };
 
 struct DecodePlan {              // device pointers into the workspace; filled by the plan kernel
@@ -136,6 +136,7 @@ struct DecodePlan {              // device pointers into the workspace; filled b
   int32_t* cta_seg;              // [n_ctas + 1]
   float2* cs;                    // [n_chunks][d_r / 2] (cos, sin)(delta f_i)
   const double* inv_freq;        // [d_r / 2] f_i = theta^(-2i/d_r), fp64, written at kam_create
+  const int32_t* block_tables;   // the call's block-table array (segments record their first slot)
   int32_t n_chunks, batch, max_segs;
 };
 
@@ -171,7 +172,9 @@ inline int decode_head_group(const kam_layout& L) {
 }
 int decode_occupancy(const DecodeGeom& g);     // resident CTAs per SM of the decode kernel this geometry selects
 void launch_decode_plan(const DecodeGeom& g, const DecodePlan& plan, const DecodeCsr& csr, cudaStream_t st);
-void launch_decode(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st);
-void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, cudaStream_t st);
+// pdl: launch with programmatic stream serialization - the kernel's prologue (plan reads, barrier setup) overlaps the
+// tail of the previous kernel on the stream; only legal when that kernel does not write the plan.
+void launch_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
+void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 
 }  // namespace kam
