@@ -287,6 +287,12 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------------- main
+def rank_requests(rank, world, per_gpu=N_REQ):
+    """Global request ids rank `rank` owns: the path partitions by request with no exchange; per-GPU
+    work is fixed as N grows (weak scaling), so the job serves world * per_gpu requests and rank r the r-th block of them."""
+    return list(range(rank * per_gpu, (rank + 1) * per_gpu))
+
+
 def max_over_ranks(x, world):
     """Largest value of x over all ranks (device timing is reduced this way; works on NCCL and gloo alike)."""
     if world == 1:
