@@ -87,14 +87,14 @@ bool build_head_blocks(kam_ctx* c) {
   return true;
 }
 
-bool build_reloc_geom(const kam_ctx* c, int max_rank, RelocGeom* out, std::string* why) {
+bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGeom* out, std::string* why) {
   const kam_layout& L = c->lay;
   RelocGeom g{};
   g.L = L.n_layers; g.H = L.n_kv_heads; g.D = L.row_dim; g.P = L.page_size;
   g.row_bytes = g.H * g.D * 2;
   g.P_shift = -1;
   for (int sft = 0; sft < 31; ++sft) if ((1 << sft) == g.P) g.P_shift = sft;
-  g.nkv = L.has_v ? 2 : 1;
+  g.nkv = (L.has_v && !inplace_only) ? 2 : 1;       // survivors are rotated in place: K only, V is never staged
   g.KT_max = max_rank / 16;
   g.rope_style = L.rope_style; g.d_r = L.rope_dim; g.half_groups = L.rope_dim / 64;
   g.theta = L.rope_theta;
@@ -110,7 +110,8 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, RelocGeom* out, std::strin
     t.contig = (HG == g.H) && c->contig_copies;
     // padded rows (== 64 mod 128) make the 128-bit row loads conflict-free; unpadded rows allow one copy per tile
     t.s_row = t.contig ? t.slice_bytes : t.slice_bytes + ((64 - t.slice_bytes % 128) + 128) % 128;
-    t.su_row = g.KT_max ? HG * max_rank * 2 + 16 : 0;                          // (su_row / 16) odd
+    // U rows: unpadded when a tile arrives as one copy (the one ldmatrix per slab tolerates the bank conflicts)
+    t.su_row = g.KT_max ? HG * max_rank * 2 + (t.contig ? 0 : 16) : 0;
     t.RB = std::min(4, std::max(1, (kRelocConsumerWarps + t.nkv * NB - 1) / (t.nkv * NB)));
     t.TT = 16 * t.RB;
     t.st_k = 0;
@@ -122,8 +123,8 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, RelocGeom* out, std::strin
     t.w_row = (g.D + 8) * 2;
     t.w_kv_stride = HG * max_rank * t.w_row;
     t.off_tab = 128;
-    t.off_cs = t.off_tab + 256 + align_up(NB * 16, 128);
-    t.off_w = t.off_cs + align_up(std::max(1, g.d_r / 2) * 8, 128);
+    t.off_cs = t.off_tab + align_up(2 * t.RB * NB * 16, 128);                    // slab table: one int4 per slab
+    t.off_w = t.off_cs + align_up(std::max(1, g.d_r / 2) * 12, 128);               // c | s | -s, planar fp32
     t.off_stage0 = align_up(t.off_w + t.nkv * t.w_kv_stride, 128);
     for (int i = 0; i < NB; ++i) {
       ColBlock b = c->head_blocks[i % c->blocks_per_head];
@@ -221,13 +222,14 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
   const int n = (int)hs.size();
   // ---- validate everything before touching anything
   int max_rank = 0, max_tokens = 0;
-  bool fast = c->fast_layout;
+  bool fast = c->fast_layout, inplace_only = true;
   for (int i = 0; i < n; ++i) {
     const HostReloc& h = hs[i];
     if (h.n_tokens < 0) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: n_tokens < 0", i);
     if (h.bt == nullptr) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: block_table is NULL", i);
     if (h.dst0 < 0) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: negative token start", i);
     const bool inplace = h.flags & FLAG_INPLACE;
+    inplace_only = inplace_only && inplace;
     if (!inplace && (h.k == nullptr || (L.has_v && h.v == nullptr)))
       return fail(c, KAM_ERR_INVALID_ARG, "desc %d: chunk layer-pointer arrays must not be NULL", i);
     kam_status vs = validate_patch(c, h.patch, h.rank, i);
@@ -245,16 +247,22 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
   if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
 
   RelocGeom g{};
-  if (fast) { std::string why; if (!build_reloc_geom(c, max_rank, &g, &why)) fast = false; }
+  if (fast) { std::string why; if (!build_reloc_geom(c, max_rank, inplace_only, &g, &why)) fast = false; }
 
+  // Small batches on the tiled kernel carry their descriptors in the kernel parameters; anything else is staged through
+  // pinned host memory and copied with one cudaMemcpyAsync on the caller's stream.
+  const bool inline_descs = fast && n <= kRelocInlineDescs;
   const size_t desc_bytes = (size_t)n * sizeof(RelocDescDev);
   const size_t prefix_off = (desc_bytes + 15) & ~size_t(15);
   const size_t total_bytes = prefix_off + (size_t)(n + 1) * sizeof(long long);
-  Staging* sg;
-  kam_status s = staging_acquire(c, total_bytes, &sg);
-  if (s != KAM_OK) return s;
-  RelocDescDev* dd = static_cast<RelocDescDev*>(sg->host);
-  long long* prefix = reinterpret_cast<long long*>(static_cast<char*>(sg->host) + prefix_off);
+  Staging* sg = nullptr;
+  std::unique_ptr<RelocInline> inl(new (std::nothrow) RelocInline());
+  if (!inl) return fail(c, KAM_ERR_STATE, "out of host memory");
+  memset(inl.get(), 0, sizeof(RelocInline));
+  kam_status s = KAM_OK;
+  if (!inline_descs && (s = staging_acquire(c, total_bytes, &sg)) != KAM_OK) return s;
+  RelocDescDev* dd = inline_descs ? inl->d : static_cast<RelocDescDev*>(sg->host);
+  long long* prefix = inline_descs ? inl->prefix : reinterpret_cast<long long*>(static_cast<char*>(sg->host) + prefix_off);
   long long acc = 0;
   for (int i = 0; i < n; ++i) {
     const HostReloc& h = hs[i];
@@ -273,17 +281,20 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
     if (fast) acc += (long long)L.n_layers * g.n_hg * ((h.n_tokens + g.TT - 1) / g.TT);
   }
   prefix[n] = acc;
-  if ((s = staging_commit(c, sg, total_bytes, st)) != KAM_OK) return s;
-  const RelocDescDev* d_descs = static_cast<const RelocDescDev*>(sg->dev);
+  const RelocDescDev* d_descs = nullptr;
+  if (!inline_descs) {
+    if ((s = staging_commit(c, sg, total_bytes, st)) != KAM_OK) return s;
+    d_descs = static_cast<const RelocDescDev*>(sg->dev);
+  }
 
   if (fast) {
     RelocParams p{};
     p.descs = d_descs;
-    p.tile_prefix = reinterpret_cast<const long long*>(static_cast<const char*>(sg->dev) + prefix_off);
+    p.tile_prefix = inline_descs ? nullptr : reinterpret_cast<const long long*>(static_cast<const char*>(sg->dev) + prefix_off);
     p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;
-    p.total_tiles = acc; p.n_descs = n;
+    p.total_tiles = acc; p.n_descs = n; p.inv_freq = c->d_inv_freq;
     const int grid = (int)std::min<long long>(c->sm_count, acc);
-    launch_relocate_fast(g, p, grid, st);
+    launch_relocate_fast(g, p, *inl, grid, st);
   } else {
     GenericParams p{};
     p.descs = d_descs; p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;
@@ -294,7 +305,7 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
   }
   ++c->kernels_launched;
   cudaError_t e = cudaGetLastError();
-  staging_release(sg, st);
+  if (sg) staging_release(sg, st);
   if (e != cudaSuccess) return cuda_fail(c, e, fast ? "kam_relocate_patch_kernel launch" : "kam_relocate_patch_generic_kernel launch");
   return KAM_OK;
 }
@@ -386,7 +397,7 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
   if (!c) return fail(nullptr, KAM_ERR_STATE, "out of host memory");
   c->lay = *layout;
   c->fast_layout = build_head_blocks(c);
-  if (const char* e = getenv("KAM_RELOC_CONTIG")) c->contig_copies = (e[0] != '0');
+  if (const char* e = getenv("KAM_RELOC_CONTIG")) c->contig_copies = (e[0] != '0');   // tuning switch, default on
   c->max_requests = max_requests; c->max_chunks = max_chunks_per_request; c->max_ppc = max_pages_per_chunk;
   if (pool) { c->pool = *pool; c->has_pool = true; }
   if (pool) {

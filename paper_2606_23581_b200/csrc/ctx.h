@@ -35,7 +35,7 @@ struct kam_ctx {
   bool fast_layout = false;
   std::string fast_layout_why;
   int blocks_per_head = 0;
-  bool contig_copies = false;                 // KAM_RELOC_CONTIG=1: one unpadded copy per tile when a slice is a whole row (tuning switch; measured no faster)
+  bool contig_copies = true;                  // one unpadded copy per tile when a slice is a whole token row (KAM_RELOC_CONTIG=0: padded per-row copies)
   kam::ColBlock head_blocks[kam::kMaxColBlocks];
 
   kam::Staging staging[kam::kStagingSlots];

@@ -67,11 +67,18 @@ struct RelocGeom {
   ColBlock blk[kMaxColBlocks];
 };
 
+constexpr int kRelocInlineDescs = 8;   // batches up to this size travel in the kernel parameters
+struct RelocInline {
+  RelocDescDev d[kRelocInlineDescs];
+  long long prefix[kRelocInlineDescs + 1];
+};
+
 struct RelocParams {
-  const RelocDescDev* descs;
+  const RelocDescDev* descs;     // device array, or nullptr => RelocInline
   const long long* tile_prefix;  // [n_descs + 1]
   void* const* pool_k;
   void* const* pool_v;
+  const double* inv_freq;        // [d_r / 2] f_i = theta^(-2i/d_r) in fp64 (written at kam_create), or nullptr
   long long total_tiles;
   int32_t n_descs;
 };
@@ -85,7 +92,7 @@ struct GenericParams {
   double theta;
 };
 
-void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, int grid, cudaStream_t st);
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, int grid, cudaStream_t st);
 void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
 
 // ---------------------------------------------------------------- decode

@@ -30,58 +30,86 @@ namespace {
 struct TileWalk {
   int d, l, hg, tt, n_tt, n_tokens;
   long long d_end;                       // first tile index of the next chunk
-  __device__ __forceinline__ void init(const RelocGeom& g, const RelocParams& p, long long tile) {
-    int lo = 0, hi = p.n_descs;          // largest d with prefix[d] <= tile
-    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (p.tile_prefix[mid] <= tile) lo = mid; else hi = mid; }
+  __device__ __forceinline__ void init(const RelocGeom& g, int n_descs, const RelocDescDev* descs, const long long* tile_prefix, long long tile) {
+    int lo = 0, hi = n_descs;            // largest d with prefix[d] <= tile
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (tile_prefix[mid] <= tile) lo = mid; else hi = mid; }
     d = lo;
-    while (p.tile_prefix[d + 1] <= tile) ++d;          // skip empty chunks
-    n_tokens = p.descs[d].n_tokens;
+    while (tile_prefix[d + 1] <= tile) ++d;            // skip empty chunks
+    n_tokens = descs[d].n_tokens;
     n_tt = (n_tokens + g.TT - 1) / g.TT;
-    d_end = p.tile_prefix[d + 1];
-    const int local = static_cast<int>(tile - p.tile_prefix[d]);
+    d_end = tile_prefix[d + 1];
+    const int local = static_cast<int>(tile - tile_prefix[d]);
     tt = local % n_tt;
     const int uu = local / n_tt;
     hg = uu % g.n_hg;
     l = uu / g.n_hg;
   }
-  __device__ __forceinline__ void next(const RelocGeom& g, const RelocParams& p, long long new_tile) {
+  __device__ __forceinline__ void next(const RelocGeom& g, const RelocDescDev* descs, const long long* tile_prefix, long long new_tile) {
     if (++tt < n_tt) return;
     tt = 0;
     if (++hg < g.n_hg) return;
     hg = 0;
     if (++l < g.L) return;
     l = 0;
-    do { ++d; } while (p.tile_prefix[d + 1] <= new_tile);
-    n_tokens = p.descs[d].n_tokens;
+    do { ++d; } while (tile_prefix[d + 1] <= new_tile);
+    n_tokens = descs[d].n_tokens;
     n_tt = (n_tokens + g.TT - 1) / g.TT;
-    d_end = p.tile_prefix[d + 1];
+    d_end = tile_prefix[d + 1];
   }
 };
 
-// Rotate 8 column pairs.  HALF: element e of `a` pairs with element e of `b` (columns i and i + d_r/2).
-__device__ __forceinline__ void rotate_half8(float* a, float* b, const float2* cs) {
+// ---- packed fp32 pairs (sm_100a FFMA2 / FMUL2): two fp32 lanes per 64-bit register pair
+__device__ __forceinline__ uint64_t pk2(float lo, float hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) { uint64_t r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) { uint64_t r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+// The (cos, sin) table of a chunk is planar in shared memory: c[half] | s[half] | -s[half]  (half = d_r / 2).
+// HALF: element e of `a` (column i) pairs with element e of `b` (column i + d_r/2); tab points at the thread's first
+// frequency.  a' = a c - b s ; b' = a s + b c, two pairs per packed instruction.
+__device__ __forceinline__ void rotate_half8(float* a, float* b, const float* tab, int half) {
+  const float4 c0 = *reinterpret_cast<const float4*>(tab), c1 = *reinterpret_cast<const float4*>(tab + 4);
+  const float4 s0 = *reinterpret_cast<const float4*>(tab + half), s1 = *reinterpret_cast<const float4*>(tab + half + 4);
+  const float4 n0 = *reinterpret_cast<const float4*>(tab + 2 * half), n1 = *reinterpret_cast<const float4*>(tab + 2 * half + 4);
+  const uint64_t C[4] = {pk2(c0.x, c0.y), pk2(c0.z, c0.w), pk2(c1.x, c1.y), pk2(c1.z, c1.w)};
+  const uint64_t S[4] = {pk2(s0.x, s0.y), pk2(s0.z, s0.w), pk2(s1.x, s1.y), pk2(s1.z, s1.w)};
+  const uint64_t N[4] = {pk2(n0.x, n0.y), pk2(n0.z, n0.w), pk2(n1.x, n1.y), pk2(n1.z, n1.w)};
 #pragma unroll
-  for (int e = 0; e < 8; e += 2) {
-    const float4 t = *reinterpret_cast<const float4*>(cs + e);   // (c0, s0, c1, s1)
-    float x = a[e], y = b[e];
-    a[e] = fmaf(x, t.x, -y * t.y);
-    b[e] = fmaf(x, t.y, y * t.x);
-    x = a[e + 1]; y = b[e + 1];
-    a[e + 1] = fmaf(x, t.z, -y * t.w);
-    b[e + 1] = fmaf(x, t.w, y * t.z);
+  for (int e = 0; e < 4; ++e) {
+    const uint64_t A = pk2(a[2 * e], a[2 * e + 1]), B = pk2(b[2 * e], b[2 * e + 1]);
+    upk2(fma2(B, N[e], mul2(A, C[e])), a[2 * e], a[2 * e + 1]);
+    upk2(fma2(A, S[e], mul2(B, C[e])), b[2 * e], b[2 * e + 1]);
   }
 }
-// INTERLEAVED: columns (2i, 2i+1) are adjacent inside one 8-vector.
-__device__ __forceinline__ void rotate_inter8(float* a, const float2* cs) {
+__device__ __forceinline__ void rotate_half8x2(float* a0, float* b0, float* a1, float* b1, const float* tab, int half) {
+  const float4 c0 = *reinterpret_cast<const float4*>(tab), c1 = *reinterpret_cast<const float4*>(tab + 4);
+  const float4 s0 = *reinterpret_cast<const float4*>(tab + half), s1 = *reinterpret_cast<const float4*>(tab + half + 4);
+  const float4 n0 = *reinterpret_cast<const float4*>(tab + 2 * half), n1 = *reinterpret_cast<const float4*>(tab + 2 * half + 4);
+  const uint64_t C[4] = {pk2(c0.x, c0.y), pk2(c0.z, c0.w), pk2(c1.x, c1.y), pk2(c1.z, c1.w)};
+  const uint64_t S[4] = {pk2(s0.x, s0.y), pk2(s0.z, s0.w), pk2(s1.x, s1.y), pk2(s1.z, s1.w)};
+  const uint64_t N[4] = {pk2(n0.x, n0.y), pk2(n0.z, n0.w), pk2(n1.x, n1.y), pk2(n1.z, n1.w)};
 #pragma unroll
-  for (int e = 0; e < 8; e += 4) {
-    const float4 t = *reinterpret_cast<const float4*>(cs + e / 2);
-    float x = a[e], y = a[e + 1];
-    a[e] = fmaf(x, t.x, -y * t.y);
-    a[e + 1] = fmaf(x, t.y, y * t.x);
-    x = a[e + 2]; y = a[e + 3];
-    a[e + 2] = fmaf(x, t.z, -y * t.w);
-    a[e + 3] = fmaf(x, t.w, y * t.z);
+  for (int e = 0; e < 4; ++e) {
+    uint64_t A = pk2(a0[2 * e], a0[2 * e + 1]), B = pk2(b0[2 * e], b0[2 * e + 1]);
+    upk2(fma2(B, N[e], mul2(A, C[e])), a0[2 * e], a0[2 * e + 1]);
+    upk2(fma2(A, S[e], mul2(B, C[e])), b0[2 * e], b0[2 * e + 1]);
+    A = pk2(a1[2 * e], a1[2 * e + 1]); B = pk2(b1[2 * e], b1[2 * e + 1]);
+    upk2(fma2(B, N[e], mul2(A, C[e])), a1[2 * e], a1[2 * e + 1]);
+    upk2(fma2(A, S[e], mul2(B, C[e])), b1[2 * e], b1[2 * e + 1]);
+  }
+}
+// INTERLEAVED: columns (2i, 2i+1) are adjacent inside one 8-vector; tab points at the thread's first frequency.
+__device__ __forceinline__ void rotate_inter8x2(float* a0, float* a1, const float* tab, int half) {
+  const float4 c = *reinterpret_cast<const float4*>(tab), s = *reinterpret_cast<const float4*>(tab + half);
+  const float cc[4] = {c.x, c.y, c.z, c.w}, ss[4] = {s.x, s.y, s.z, s.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float x = a0[2 * i], y = a0[2 * i + 1];
+    a0[2 * i] = fmaf(x, cc[i], -y * ss[i]);
+    a0[2 * i + 1] = fmaf(x, ss[i], y * cc[i]);
+    x = a1[2 * i]; y = a1[2 * i + 1];
+    a1[2 * i] = fmaf(x, cc[i], -y * ss[i]);
+    a1[2 * i + 1] = fmaf(x, ss[i], y * cc[i]);
   }
 }
 
@@ -93,20 +121,87 @@ __device__ __forceinline__ void mma_group(float* r0, float* r1, const uint32_t* 
   mma_bf16_16816(r0[6], r0[7], r1[6], r1[7], a[0], a[1], a[2], a[3], w23[2], w23[3]);
 }
 
+enum : int { ROPE_NONE = 0, ROPE_HALF = 1, ROPE_INTER = 2 };
+
+// What one consumer warp needs to process a slab (16 tokens x one column block), beyond the template parameters.
+struct SlabArgs {
+  const uint8_t* rows;       // this thread's first vector: token row (lane / 4), 16-byte column slot (lane % 4) of group 0
+  char* dst0;                // pool address of the same vector for token row lane/4, and for row lane/4 + 8
+  char* dst1;
+  const float* tab;          // the thread's first table entry for group 0 of the block (HALF: frequency; INTER: column / 2)
+  uint32_t wb;               // shared address of this lane's ldmatrix row of W (k-tile 0, group 0)
+  int s_row, w_row16, half;  // token stride in the stage; bytes of 16 k-rows of W; d_r / 2
+  int steps;                 // pairs of 32-column groups
+  bool ok0, ok1, canonical;
+};
+
+// A step = two 32-column groups (gA, gB) x 16 tokens: HALF pairs group sp with group sp + steps (column i with i + d_r/2).
+template <int KT, int ROPE, int STEPS>
+__device__ __forceinline__ void slab_steps(const SlabArgs& s, const uint32_t (*afr)[4]) {
+#pragma unroll
+  for (int sp = 0; sp < STEPS; ++sp) {                                          // independent steps: unrolled for ILP
+    const int offA = (ROPE == ROPE_HALF ? sp : 2 * sp) * 64;
+    const int offB = (ROPE == ROPE_HALF ? sp + STEPS : 2 * sp + 1) * 64;
+    float a0[8], a1[8], b0[8], b1[8];
+    unpack8(*reinterpret_cast<const uint4*>(s.rows + offA), a0);
+    unpack8(*reinterpret_cast<const uint4*>(s.rows + 8 * s.s_row + offA), a1);
+    unpack8(*reinterpret_cast<const uint4*>(s.rows + offB), b0);
+    unpack8(*reinterpret_cast<const uint4*>(s.rows + 8 * s.s_row + offB), b1);
+    auto rotate = [&]() {
+      if constexpr (ROPE == ROPE_HALF) {
+        rotate_half8x2(a0, b0, a1, b1, s.tab + (offA >> 1), s.half);            // 32 frequencies per group
+      } else if constexpr (ROPE == ROPE_INTER) {
+        rotate_inter8x2(a0, a1, s.tab + (offA >> 2), s.half);                   // 16 frequencies per group
+        rotate_inter8x2(b0, b1, s.tab + (offB >> 2), s.half);
+      }
+    };
+    if (ROPE != ROPE_NONE && !s.canonical) rotate();                            // Eq. 1: rotate, then add the patch
+#pragma unroll
+    for (int kt = 0; kt < KT; ++kt) {
+      uint32_t wA[8], wB[8];
+      const uint32_t base = s.wb + kt * s.w_row16;
+      ldmatrix_x4_trans(wA[0], wA[1], wA[2], wA[3], base + offA);
+      ldmatrix_x4_trans(wA[4], wA[5], wA[6], wA[7], base + offA + 32);
+      ldmatrix_x4_trans(wB[0], wB[1], wB[2], wB[3], base + offB);
+      ldmatrix_x4_trans(wB[4], wB[5], wB[6], wB[7], base + offB + 32);
+      mma_group(a0, a1, afr[kt], wA, wA + 4);
+      mma_group(b0, b1, afr[kt], wB, wB + 4);
+    }
+    if (ROPE != ROPE_NONE && s.canonical) rotate();                             // patch stored in the chunk's own frame (R-4)
+    if (s.ok0) { st_global_v4(s.dst0 + offA, pack8(a0)); st_global_v4(s.dst0 + offB, pack8(b0)); }
+    if (s.ok1) { st_global_v4(s.dst1 + offA, pack8(a1)); st_global_v4(s.dst1 + offB, pack8(b1)); }
+  }
+}
+
+template <int KT>
+__device__ __forceinline__ void slab_run(const SlabArgs& s, int rope, uint32_t ua) {
+  uint32_t afr[KT > 0 ? KT : 1][4];
+#pragma unroll
+  for (int kt = 0; kt < KT; ++kt) ldmatrix_x4(afr[kt][0], afr[kt][1], afr[kt][2], afr[kt][3], ua + kt * 32);
+  if (s.steps == 2) {
+    if (rope == ROPE_NONE) slab_steps<KT, ROPE_NONE, 2>(s, afr);
+    else if (rope == ROPE_HALF) slab_steps<KT, ROPE_HALF, 2>(s, afr);
+    else slab_steps<KT, ROPE_INTER, 2>(s, afr);
+  } else {
+    if (rope == ROPE_NONE) slab_steps<KT, ROPE_NONE, 1>(s, afr);
+    else if (rope == ROPE_HALF) slab_steps<KT, ROPE_HALF, 1>(s, afr);
+    else slab_steps<KT, ROPE_INTER, 1>(s, afr);
+  }
+}
+
 }  // namespace
 
-// Shared-memory map (dynamic): [0,128) mbarriers | slab table | column-block table | cs | W (column-permuted, padded
-// rows) | stages.  W in shared memory is [kv][head-in-group][k][D + 8] bf16 with the columns of every 32-group stored
-// in MMA order (position 8j + 2i + e holds column 8i + 2j + e), so that ldmatrix.trans yields B fragments whose
-// accumulator columns are 8 CONTIGUOUS columns per thread.
+// Shared-memory map (dynamic): [0,128) mbarriers | slab table | cos/sin table | W (column-permuted, padded rows) | stages.
+// W in shared memory is [kv][head-in-group][k][D + 8] bf16 with the columns of every 32-group stored in MMA order
+// (position 8j + 2i + e holds column 8i + 2j + e), so that ldmatrix.trans yields B fragments whose accumulator columns
+// are 8 CONTIGUOUS columns per thread.
 __global__ void __launch_bounds__(kRelocThreads, 1)
-kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_constant__ RelocParams p) {
+kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_constant__ RelocParams p, const __grid_constant__ RelocInline inl) {
   extern __shared__ __align__(128) uint8_t smem[];
   uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem);
   uint64_t* empty_bar = full_bar + g.n_stages;
-  uint32_t* slab_tab = reinterpret_cast<uint32_t*>(smem + g.off_tab);
-  int4* blk_tab = reinterpret_cast<int4*>(smem + g.off_tab + 256);
-  float2* cs = reinterpret_cast<float2*>(smem + g.off_cs);
+  int4* slab_tab = reinterpret_cast<int4*>(smem + g.off_tab);
+  float* tab = reinterpret_cast<float*>(smem + g.off_cs);
   uint8_t* wsm = smem + g.off_w;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -114,25 +209,31 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
     for (int s = 0; s < g.n_stages; ++s) { mbar_init(&full_bar[s], kRelocProducerWarps); mbar_init(&empty_bar[s], kRelocConsumerWarps); }
     mbar_fence_init();
   }
-  if (threadIdx.x < 2 * g.RB * g.n_blocks && threadIdx.x < 64) {     // slab s -> (kv, row block, column block); K slabs first
+  if (threadIdx.x < 2 * g.RB * g.n_blocks) {
+    // slab s -> (kv, row block, column block), K slabs first; everything a consumer needs, as byte offsets
     const int s = threadIdx.x, per = g.RB * g.n_blocks;
-    const int kv = s / per, rem = s - kv * per;
-    slab_tab[s] = kv | ((rem / g.n_blocks) << 8) | ((rem % g.n_blocks) << 16);
-  }
-  if (threadIdx.x >= 64 && threadIdx.x < 64 + g.n_blocks) {
-    const ColBlock cb = g.blk[threadIdx.x - 64];
-    blk_tab[threadIdx.x - 64] = make_int4(cb.col_off, cb.w_col_off | (cb.band_col0 << 16), cb.n_groups | (cb.fhead << 8) | (cb.rope << 16), 0);
+    const int kv = s / per, rem = s - kv * per, rb = rem / g.n_blocks;
+    const ColBlock cb = g.blk[rem % g.n_blocks];
+    const int rope = (kv == 0 && cb.rope) ? (g.rope_style == KAM_ROPE_HALF ? ROPE_HALF : ROPE_INTER) : ROPE_NONE;
+    const int tab_off = g.rope_style == KAM_ROPE_HALF ? cb.band_col0 : cb.band_col0 >> 1;       // first frequency of the block
+    slab_tab[s] = make_int4(kv | (rb << 4) | (cb.fhead << 8) | (rope << 16) | ((cb.n_groups >> 1) << 20),
+                            cb.col_off * 2, cb.w_col_off * 2, tab_off);
   }
   __syncthreads();
 
+  // small batches carry their descriptors in the kernel parameters (no H2D staging copy, no global loads to read them)
+  const RelocDescDev* descs = p.descs ? p.descs : inl.d;
+  const long long* tile_prefix = p.descs ? p.tile_prefix : inl.prefix;
   const long long t_begin = p.total_tiles * blockIdx.x / gridDim.x;
   const long long t_end = p.total_tiles * (blockIdx.x + 1) / gridDim.x;
   if (t_begin >= t_end) return;
   TileWalk w;
-  w.init(g, p, t_begin);
+  w.init(g, p.n_descs, descs, tile_prefix, t_begin);
 
   if (warp >= kRelocConsumerWarps) {
     // ================================================================ producer warps: K | V | U_k | U_v
+    // Copies are issued lane-parallel (lane r owns token row r, or the run of rows that starts at r); the block-table
+    // entries of a tile are loaded BEFORE the wait for a free stage, so their latency hides behind it.
     const int role = warp - kRelocConsumerWarps;
     int stage = 0; uint32_t phase = 0;
     int cur_d = -1, cur_l = -1;
@@ -143,86 +244,113 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
     for (long long tile = t_begin; tile < t_end; ++tile) {
       if (w.d != cur_d || w.l != cur_l) {
         cur_d = w.d; cur_l = w.l;
-        const RelocDescDev& desc = p.descs[w.d];
+        const RelocDescDev& desc = descs[w.d];
         flags = desc.flags; m = desc.rank_l[w.l]; bt = desc.block_table; dst0 = static_cast<int>(desc.dst_token_start);
         u_tok_stride = desc.u_token_stride; u_head_stride = desc.u_head_stride;
         const bool inplace = flags & FLAG_INPLACE;
-        const void* const* tab = role == 0 ? desc.k_src : role == 1 ? desc.v_src : role == 2 ? desc.Uk : desc.Uv;
+        const void* const* tab_l = role == 0 ? desc.k_src : role == 1 ? desc.v_src : role == 2 ? desc.Uk : desc.Uv;
         src = nullptr;
-        if (role == 0) src = inplace ? static_cast<const char*>(p.pool_k[w.l]) : static_cast<const char*>(tab[w.l]);
-        else if (role == 1) { if (!inplace && g.nkv == 2) src = static_cast<const char*>(tab[w.l]); }
-        else if (m && tab && !inplace && (role == 2 || g.nkv == 2)) src = static_cast<const char*>(tab[w.l]);
+        if (role == 0) src = inplace ? static_cast<const char*>(p.pool_k[w.l]) : static_cast<const char*>(tab_l[w.l]);
+        else if (role == 1) { if (!inplace && g.nkv == 2) src = static_cast<const char*>(tab_l[w.l]); }
+        else if (m && tab_l && !inplace && (role == 2 || g.nkv == 2)) src = static_cast<const char*>(tab_l[w.l]);
+        if (role >= 2 && src) {
+          // the consumers stage this (chunk, layer)'s W a few tiles from now: pull it into L2 ahead of them
+          const void* const* Wt = role == 2 ? desc.Wk : desc.Wv;
+          const size_t wbytes = static_cast<size_t>(g.HG) * m * g.D * 2;
+          const char* wp = static_cast<const char*>(Wt[w.l]) + static_cast<size_t>(w.hg) * wbytes;
+          for (size_t o = static_cast<size_t>(lane) * 128; o < wbytes; o += 32 * 128)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(wp + o));
+        }
       }
-      mbar_wait(&empty_bar[stage], phase ^ 1);
-      uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
       const int tok0 = w.tt * g.TT;
       const int nvalid = min(g.TT, w.n_tokens - tok0);
       const bool inplace = flags & FLAG_INPLACE;
+      // A1 slot mapping: g = dst_token_start + t -> page = block_table[g / P], slot = page * P + g % P   (TT <= 64: 2 rows per lane)
+      int slot_lo = -1, slot_hi = -1;
       if (role == 0) {
-        // A1 slot mapping: g = dst_token_start + t -> page = block_table[g / P], slot = page * P + g % P
-        int32_t* slots = reinterpret_cast<int32_t*>(st + g.st_slot);
-        for (int r = lane; r < g.TT; r += 32) {
-          int slot = -1;
-          if (r < nvalid) {
-            const int gt = dst0 + tok0 + r;
-            const int pg = g.P_shift >= 0 ? (gt >> g.P_shift) : gt / g.P;
-            slot = bt[pg] * g.P + (gt - pg * g.P);
-          }
-          slots[r] = slot;
+        if (lane < nvalid) {
+          const int gt = dst0 + tok0 + lane;
+          const int pg = g.P_shift >= 0 ? (gt >> g.P_shift) : gt / g.P;
+          slot_lo = __ldg(bt + pg) * g.P + (gt - pg * g.P);
         }
-        __syncwarp();
-        if (lane == 0) {
-          const uint32_t bytes = static_cast<uint32_t>(nvalid) * g.slice_bytes;
-          mbar_arrive_expect_tx(&full_bar[stage], bytes);
+        if (lane + 32 < nvalid) {
+          const int gt = dst0 + tok0 + lane + 32;
+          const int pg = g.P_shift >= 0 ? (gt >> g.P_shift) : gt / g.P;
+          slot_hi = __ldg(bt + pg) * g.P + (gt - pg * g.P);
+        }
+      }
+      mbar_wait(&empty_bar[stage], phase ^ 1);
+      uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
+      uint64_t* fb = &full_bar[stage];
+      if (role <= 1) {
+        if (role == 0) {
+          int32_t* slots = reinterpret_cast<int32_t*>(st + g.st_slot);
+          if (lane < g.TT) slots[lane] = slot_lo;
+          if (lane + 32 < g.TT) slots[lane + 32] = slot_hi;
+          __syncwarp();                              // every lane's slots are written before lane 0 arrives on the barrier
+        }
+        if (src == nullptr) {
+          if (lane == 0) mbar_arrive(fb);
+        } else {
+          if (lane == 0) mbar_arrive_expect_tx(fb, static_cast<uint32_t>(nvalid) * g.slice_bytes);
+          __syncwarp();
           const size_t off = static_cast<size_t>(w.hg) * g.slice_bytes;
-          uint8_t* dst = st + g.st_k;
+          uint8_t* dst = st + (role == 0 ? g.st_k : g.st_v);
           if (!inplace) {
             const char* s0 = src + static_cast<size_t>(tok0) * g.row_bytes + off;
-            if (g.contig) bulk_g2s(dst, s0, bytes, &full_bar[stage]);
-            else for (int r = 0; r < nvalid; ++r) bulk_g2s(dst + r * g.s_row, s0 + static_cast<size_t>(r) * g.row_bytes, g.slice_bytes, &full_bar[stage]);
-          } else if (g.contig) {                     // pool rows: contiguous inside a page -> one copy per run of slots
-            int r = 0;
-            while (r < nvalid) {
-              const int s_first = slots[r];
-              int n = 1;
-              while (r + n < nvalid && slots[r + n] == s_first + n) ++n;
-              bulk_g2s(dst + r * g.s_row, src + static_cast<size_t>(s_first) * g.row_bytes, n * g.slice_bytes, &full_bar[stage]);
-              r += n;
+            if (g.contig) { if (lane == 0) bulk_g2s(dst, s0, static_cast<uint32_t>(nvalid) * g.slice_bytes, fb); }
+            else for (int r = lane; r < nvalid; r += 32) bulk_g2s(dst + r * g.s_row, s0 + static_cast<size_t>(r) * g.row_bytes, g.slice_bytes, fb);
+          } else if (g.contig) {
+            // pool rows are contiguous inside a page: one copy per run of consecutive slots, issued by the run's first lane
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+              const int r = lane + 32 * hf;
+              const int mine = hf ? slot_hi : slot_lo;
+              const int prev = __shfl_up_sync(0xffffffffu, mine, 1);
+              const bool valid = r < nvalid;
+              const bool head = valid && (lane == 0 || mine != prev + 1);          // a run never spans the two halves
+              const uint32_t heads = __ballot_sync(0xffffffffu, head), valids = __ballot_sync(0xffffffffu, valid);
+              if (head) {
+                const uint32_t above = heads & ~((2u << lane) - 1u);                  // run heads after this lane
+                const int end = above ? __ffs(above) - 1 : __popc(valids);           // rows of this half are valid from lane 0 up
+                bulk_g2s(dst + r * g.s_row, src + static_cast<size_t>(mine) * g.row_bytes, static_cast<uint32_t>(end - lane) * g.slice_bytes, fb);
+              }
             }
           } else {
-            for (int r = 0; r < nvalid; ++r)
-              bulk_g2s(dst + r * g.s_row, src + static_cast<size_t>(slots[r]) * g.row_bytes + off, g.slice_bytes, &full_bar[stage]);
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+              const int r = lane + 32 * hf;
+              if (r < nvalid) bulk_g2s(dst + r * g.s_row, src + static_cast<size_t>(hf ? slot_hi : slot_lo) * g.row_bytes + off, g.slice_bytes, fb);
+            }
           }
         }
-      } else if (lane == 0) {
+      } else {
         if (src == nullptr) {
-          mbar_arrive(&full_bar[stage]);
-        } else if (role == 1) {
-          const uint32_t bytes = static_cast<uint32_t>(nvalid) * g.slice_bytes;
-          mbar_arrive_expect_tx(&full_bar[stage], bytes);
-          const char* s0 = src + static_cast<size_t>(tok0) * g.row_bytes + static_cast<size_t>(w.hg) * g.slice_bytes;
-          uint8_t* dst = st + g.st_v;
-          if (g.contig) bulk_g2s(dst, s0, bytes, &full_bar[stage]);
-          else for (int r = 0; r < nvalid; ++r) bulk_g2s(dst + r * g.s_row, s0 + static_cast<size_t>(r) * g.row_bytes, g.slice_bytes, &full_bar[stage]);
+          if (lane == 0) mbar_arrive(fb);
         } else {
-          // U rows of this tile: one run of (heads-in-slice * m) elements per token when the heads are adjacent
+          // U rows of this tile: one run of (heads-in-slice * m) elements per token when the heads are adjacent; the whole
+          // tile in ONE copy when the token runs are adjacent too and fill the shared-memory row exactly
           const int hf_n = (u_head_stride == 0) ? 1 : g.HG;
           const uint32_t u_run = static_cast<uint32_t>(m) * 2u, u_tok_bytes = u_run * hf_n;
-          mbar_arrive_expect_tx(&full_bar[stage], static_cast<uint32_t>(nvalid) * u_tok_bytes);
+          if (lane == 0) mbar_arrive_expect_tx(fb, static_cast<uint32_t>(nvalid) * u_tok_bytes);
+          __syncwarp();
           const long long h0 = (u_head_stride == 0) ? 0 : static_cast<long long>(w.hg) * g.HG;
           const char* s0 = src + (static_cast<long long>(tok0) * u_tok_stride + h0 * u_head_stride) * 2;
           uint8_t* dst = st + (role == 2 ? g.st_uk : g.st_uv);
-          if (hf_n == 1 || u_head_stride == m) {
-            for (int r = 0; r < nvalid; ++r) bulk_g2s(dst + r * g.su_row, s0 + r * u_tok_stride * 2, u_tok_bytes, &full_bar[stage]);
+          const bool heads_adjacent = hf_n == 1 || u_head_stride == m;
+          if (heads_adjacent && u_tok_stride * 2 == u_tok_bytes && static_cast<int>(u_tok_bytes) == g.su_row) {
+            if (lane == 0) bulk_g2s(dst, s0, static_cast<uint32_t>(nvalid) * u_tok_bytes, fb);
+          } else if (heads_adjacent) {
+            for (int r = lane; r < nvalid; r += 32) bulk_g2s(dst + r * g.su_row, s0 + r * u_tok_stride * 2, u_tok_bytes, fb);
           } else {
-            for (int r = 0; r < nvalid; ++r)
+            for (int r = lane; r < nvalid; r += 32)
               for (int h = 0; h < hf_n; ++h)
-                bulk_g2s(dst + r * g.su_row + h * u_run, s0 + (r * u_tok_stride + h * u_head_stride) * 2, u_run, &full_bar[stage]);
+                bulk_g2s(dst + r * g.su_row + h * u_run, s0 + (r * u_tok_stride + h * u_head_stride) * 2, u_run, fb);
           }
         }
       }
       if (++stage == g.n_stages) { stage = 0; phase ^= 1; }
-      if (tile + 1 < t_end) w.next(g, p, tile + 1);
+      if (tile + 1 < t_end) w.next(g, descs, tile_prefix, tile + 1);
     }
     return;
   }
@@ -232,7 +360,9 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   const int ctid = threadIdx.x;                                   // 0 .. 255
   int stage = 0; uint32_t phase = 0;
   int cur_d = -1, cur_l = -1, cur_hg = -1;
-  int m = 0, flags = 0; bool u_shared = false, has_uk = false, has_uv = false;
+  int m = 0, flags = 0, KT = 0; bool u_shared = false, has_uk = false, has_uv = false;
+  char* pool_k = nullptr; char* pool_v = nullptr;
+  const int half = g.d_r >> 1;
   // ldmatrix lane addressing
   const int a_row = lane & 15, a_koff = (lane >> 4) * 8;                       // A: rows of U, k offset
   const int b_k = (lane & 7) + ((lane >> 3) & 1) * 8, b_nt = lane >> 4;         // B: k row of W, n-tile 0/1 of the pair
@@ -242,35 +372,54 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
       // ---- new (chunk, layer, head group): rebuild the sin/cos table (new chunk) and stage W
       const bool new_chunk = (w.d != cur_d);
       cur_d = w.d; cur_l = w.l; cur_hg = w.hg;
-      const RelocDescDev& desc = p.descs[w.d];
-      flags = desc.flags; m = desc.rank_l[w.l];
+      const RelocDescDev& desc = descs[w.d];
+      flags = desc.flags; m = desc.rank_l[w.l]; KT = m >> 4;
       u_shared = desc.u_head_stride == 0;
       const bool inplace = flags & FLAG_INPLACE;
       has_uk = m && desc.Uk && !inplace; has_uv = m && desc.Uv && !inplace && g.nkv == 2;
+      pool_k = static_cast<char*>(p.pool_k[w.l]) + static_cast<size_t>(w.hg) * g.slice_bytes;
+      pool_v = g.nkv == 2 ? static_cast<char*>(p.pool_v[w.l]) + static_cast<size_t>(w.hg) * g.slice_bytes : nullptr;
       named_bar_sync(1, kRelocConsumerWarps * 32);                // everyone is done with the old tables
-      if (new_chunk && ctid < g.d_r / 2) {
+      if (new_chunk && ctid < half) {
         // A2: f_i = theta^(-2i/d_r); angle = delta * f_i in fp64 (positions reach 1e5: fp32 angles would cost 2 bf16 ulp)
-        const double f = pow(g.theta, -2.0 * ctid / g.d_r);
-        double s, c;
-        sincos(static_cast<double>(desc.delta) * f, &s, &c);
-        cs[ctid] = make_float2(static_cast<float>(c), static_cast<float>(s));
+        const double f = p.inv_freq ? p.inv_freq[ctid] : pow(g.theta, -2.0 * ctid / g.d_r);
+        double sn, cs;
+        sincos(static_cast<double>(desc.delta) * f, &sn, &cs);
+        tab[ctid] = static_cast<float>(cs);
+        tab[half + ctid] = static_cast<float>(sn);
+        tab[2 * half + ctid] = -static_cast<float>(sn);
       }
       if (has_uk) {
         // W[l] is [H][m][D]; copy this head group's rows, 16 bytes (8 columns = 4 pairs) per thread, scattering the pairs
         // to their MMA-order positions inside the 32-column group.
         const int vec_per_row = g.D >> 3;
         const int per_kv = g.HG * m * vec_per_row;
-        const int nkv_w = has_uv ? 2 : 1;
-        for (int e = ctid; e < nkv_w * per_kv; e += kRelocConsumerWarps * 32) {
-          const int kv = e >= per_kv;
-          int r = e - kv * per_kv;
-          const int v = r % vec_per_row; r /= vec_per_row;       // r = head-in-group * m + k
-          const void* const* Wl = kv ? desc.Wv : desc.Wk;
-          const uint4 x = __ldg(reinterpret_cast<const uint4*>(static_cast<const char*>(Wl[w.l]) +
-                                (static_cast<size_t>(w.hg) * g.HG * m + r) * g.D * 2) + v);
-          const int q = v >> 2, i = v & 3;                         // columns 32q + 8i .. +7 = pairs j = 0..3
-          uint32_t* dst = reinterpret_cast<uint32_t*>(wsm + static_cast<size_t>(kv) * g.w_kv_stride + static_cast<size_t>(r) * g.w_row) + q * 16 + i;
-          dst[0] = x.x; dst[4] = x.y; dst[8] = x.z; dst[12] = x.w; // pair j lands at 32-bit position 4j + i
+        const int n_vec = (has_uv ? 2 : 1) * per_kv;
+        constexpr int kCT = kRelocConsumerWarps * 32, kBatch = 8;      // 8 independent 16-byte loads in flight per thread
+        for (int e0 = ctid; e0 < n_vec; e0 += kCT * kBatch) {
+          uint4 x[kBatch];
+#pragma unroll
+          for (int u = 0; u < kBatch; ++u) {
+            const int e = e0 + u * kCT;
+            if (e < n_vec) {
+              const int kv = e >= per_kv;
+              const int r = e - kv * per_kv;
+              const void* const* Wl = kv ? desc.Wv : desc.Wk;
+              x[u] = __ldg(reinterpret_cast<const uint4*>(static_cast<const char*>(Wl[w.l]) + static_cast<size_t>(w.hg) * g.HG * m * g.D * 2) + r);
+            }
+          }
+#pragma unroll
+          for (int u = 0; u < kBatch; ++u) {
+            const int e = e0 + u * kCT;
+            if (e < n_vec) {
+              const int kv = e >= per_kv;
+              int r = e - kv * per_kv;
+              const int v = r % vec_per_row; r /= vec_per_row;     // r = head-in-group * m + k
+              const int q = v >> 2, i = v & 3;                       // columns 32q + 8i .. +7 = pairs j = 0..3
+              uint32_t* dst = reinterpret_cast<uint32_t*>(wsm + static_cast<size_t>(kv) * g.w_kv_stride + static_cast<size_t>(r) * g.w_row) + q * 16 + i;
+              dst[0] = x[u].x; dst[4] = x[u].y; dst[8] = x[u].z; dst[12] = x[u].w;   // pair j lands at 32-bit position 4j + i
+            }
+          }
         }
       }
       named_bar_sync(1, kRelocConsumerWarps * 32);
@@ -281,96 +430,48 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
     const uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
     const int32_t* slots = reinterpret_cast<const int32_t*>(st + g.st_slot);
     const bool inplace = flags & FLAG_INPLACE;
-    const bool canonical = flags & FLAG_CANONICAL_FRAME;
-    const int KT = m >> 4;
     const int n_slabs = ((g.nkv == 2 && !inplace) ? 2 : 1) * g.RB * g.n_blocks;
 
     for (int s = warp; s < n_slabs; s += kRelocConsumerWarps) {
-      const uint32_t se = slab_tab[s];
-      const int kv = se & 0xff, rb = (se >> 8) & 0xff, b = se >> 16;
-      const int4 cbv = blk_tab[b];
-      const int col_off = cbv.x, w_col_off = cbv.y & 0xffff, band_col0 = cbv.y >> 16;
-      const int n_groups = cbv.z & 0xff, fhead = (cbv.z >> 8) & 0xff;
-      const bool rope = (kv == 0) && ((cbv.z >> 16) & 1);
+      const int4 e = slab_tab[s];
+      const int kv = e.x & 0xf, rb = (e.x >> 4) & 0xf, fhead = (e.x >> 8) & 0xff, rope = (e.x >> 16) & 0xf;
       const int row0 = rb * 16 + gq;
       const int slot0 = slots[row0], slot1 = slots[row0 + 8];
-      char* pool = static_cast<char*>(kv ? p.pool_v[w.l] : p.pool_k[w.l]) + static_cast<size_t>(w.hg) * g.slice_bytes + col_off * 2 + t4 * 16;
-      char* dst0 = pool + static_cast<size_t>(slot0 < 0 ? 0 : slot0) * g.row_bytes;
-      char* dst1 = pool + static_cast<size_t>(slot1 < 0 ? 0 : slot1) * g.row_bytes;
-      const uint8_t* rows = st + (kv ? g.st_v : g.st_k) + row0 * g.s_row + col_off * 2 + t4 * 16;
-      const bool patched = KT > 0 && (kv ? has_uv : has_uk);
-
+      char* pool = (kv ? pool_v : pool_k) + e.y + t4 * 16;
+      SlabArgs a;
+      a.rows = st + (kv ? g.st_v : g.st_k) + row0 * g.s_row + e.y + t4 * 16;
+      a.dst0 = pool + static_cast<size_t>(slot0 < 0 ? 0 : slot0) * g.row_bytes;
+      a.dst1 = pool + static_cast<size_t>(slot1 < 0 ? 0 : slot1) * g.row_bytes;
+      a.tab = tab + e.w + (rope == ROPE_HALF ? 8 * t4 : 4 * t4);
+      a.s_row = g.s_row; a.w_row16 = 16 * g.w_row; a.half = half;
+      a.steps = e.x >> 20;
+      a.ok0 = slot0 >= 0; a.ok1 = slot1 >= 0; a.canonical = flags & FLAG_CANONICAL_FRAME;
+      a.wb = smem_u32(wsm + static_cast<size_t>(kv) * g.w_kv_stride + static_cast<size_t>(fhead * m + b_k) * g.w_row + e.z + b_nt * 16);
+      const int kt = (kv ? has_uv : has_uk) ? KT : 0;
       // A fragments of U for this slab's 16 tokens and head: one ldmatrix.x4 per 16 ranks
-      uint32_t afr[4][4];
-      if (patched) {
-        const int hf = u_shared ? 0 : fhead;
-        const uint32_t ua = smem_u32(st + (kv ? g.st_uv : g.st_uk) + (rb * 16 + a_row) * g.su_row + (hf * m + a_koff) * 2);
-#pragma unroll
-        for (int kt = 0; kt < 4; ++kt)
-          if (kt < KT) ldmatrix_x4(afr[kt][0], afr[kt][1], afr[kt][2], afr[kt][3], ua + kt * 32);
-      }
-      // B fragments come from W rows k of this head: address of (k = b_k, 32-bit position 0 of n-tile b_nt)
-      const uint32_t wb = smem_u32(wsm + static_cast<size_t>(kv) * g.w_kv_stride + static_cast<size_t>(fhead * m + b_k) * g.w_row + (w_col_off + b_nt * 8) * 2);
-
-      const bool half_rope = rope && g.rope_style == KAM_ROPE_HALF;
-      const int steps = n_groups >> 1;
-#pragma unroll 1
-      for (int sp = 0; sp < steps; ++sp) {
-        const int gA = half_rope ? sp : 2 * sp;
-        const int gB = half_rope ? sp + steps : 2 * sp + 1;
-        float a0[8], a1[8], b0[8], b1[8];
-        unpack8(*reinterpret_cast<const uint4*>(rows + gA * 64), a0);
-        unpack8(*reinterpret_cast<const uint4*>(rows + 8 * g.s_row + gA * 64), a1);
-        unpack8(*reinterpret_cast<const uint4*>(rows + gB * 64), b0);
-        unpack8(*reinterpret_cast<const uint4*>(rows + 8 * g.s_row + gB * 64), b1);
-
-        const float2* csA = cs;
-        const float2* csB = cs;
-        if (rope) {
-          if (half_rope) csA = cs + band_col0 + 32 * gA + 8 * t4;
-          else { csA = cs + ((band_col0 + 32 * gA + 8 * t4) >> 1); csB = cs + ((band_col0 + 32 * gB + 8 * t4) >> 1); }
-        }
-        if (rope && !canonical) {                                  // Eq. 1: rotate, then add the patch
-          if (half_rope) { rotate_half8(a0, b0, csA); rotate_half8(a1, b1, csA); }
-          else { rotate_inter8(a0, csA); rotate_inter8(a1, csA); rotate_inter8(b0, csB); rotate_inter8(b1, csB); }
-        }
-        if (patched) {
-#pragma unroll
-          for (int kt = 0; kt < 4; ++kt) {
-            if (kt < KT) {
-              uint32_t wA[8], wB[8];
-              const uint32_t base = wb + kt * 16 * g.w_row;
-              ldmatrix_x4_trans(wA[0], wA[1], wA[2], wA[3], base + gA * 64);
-              ldmatrix_x4_trans(wA[4], wA[5], wA[6], wA[7], base + gA * 64 + 32);
-              ldmatrix_x4_trans(wB[0], wB[1], wB[2], wB[3], base + gB * 64);
-              ldmatrix_x4_trans(wB[4], wB[5], wB[6], wB[7], base + gB * 64 + 32);
-              mma_group(a0, a1, afr[kt], wA, wA + 4);
-              mma_group(b0, b1, afr[kt], wB, wB + 4);
-            }
-          }
-        }
-        if (rope && canonical) {                                   // patch stored in the chunk's own frame (R-4)
-          if (half_rope) { rotate_half8(a0, b0, csA); rotate_half8(a1, b1, csA); }
-          else { rotate_inter8(a0, csA); rotate_inter8(a1, csA); rotate_inter8(b0, csB); rotate_inter8(b1, csB); }
-        }
-        if (slot0 >= 0) { st_global_v4(dst0 + gA * 64, pack8(a0)); st_global_v4(dst0 + gB * 64, pack8(b0)); }
-        if (slot1 >= 0) { st_global_v4(dst1 + gA * 64, pack8(a1)); st_global_v4(dst1 + gB * 64, pack8(b1)); }
+      const uint32_t ua = smem_u32(st + (kv ? g.st_uv : g.st_uk) + (rb * 16 + a_row) * g.su_row + ((u_shared ? 0 : fhead) * m + a_koff) * 2);
+      switch (kt) {
+        case 0: slab_run<0>(a, rope, ua); break;
+        case 1: slab_run<1>(a, rope, ua); break;
+        case 2: slab_run<2>(a, rope, ua); break;
+        case 3: slab_run<3>(a, rope, ua); break;
+        default: slab_run<4>(a, rope, ua); break;
       }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty_bar[stage]);
     if (++stage == g.n_stages) { stage = 0; phase ^= 1; }
-    if (tile + 1 < t_end) w.next(g, p, tile + 1);
+    if (tile + 1 < t_end) w.next(g, descs, tile_prefix, tile + 1);
   }
 }
 
-void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, int grid, cudaStream_t st) {
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, int grid, cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(kam_relocate_patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_set = true;
   }
-  kam_relocate_patch_kernel<<<grid, kRelocThreads, g.smem_bytes, st>>>(g, p);
+  kam_relocate_patch_kernel<<<grid, kRelocThreads, g.smem_bytes, st>>>(g, p, inl);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
