@@ -98,7 +98,8 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
   g.KT_max = max_rank / 16;
   g.rope_style = L.rope_style; g.d_r = L.rope_dim; g.half_groups = L.rope_dim / 64;
   g.theta = L.rope_theta;
-  const int limit = 220 * 1024;
+  const int limit = 226 * 1024;
+  const int ns_max = c->reloc_stages > 0 ? c->reloc_stages : 3;   // measured on B200: 3 x 37 KB in flight per SM beats 4 and 5
   RelocGeom best{}; bool have = false;
   for (int HG = std::min(g.H, 4); HG >= 1; --HG) {
     if (g.H % HG) continue;
@@ -113,6 +114,7 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
     // U rows: unpadded when a tile arrives as one copy (the one ldmatrix per slab tolerates the bank conflicts)
     t.su_row = g.KT_max ? HG * max_rank * 2 + (t.contig ? 0 : 16) : 0;
     t.RB = std::min(4, std::max(1, (kRelocConsumerWarps + t.nkv * NB - 1) / (t.nkv * NB)));
+    if (c->reloc_rb > 0) t.RB = std::min(4, c->reloc_rb);
     t.TT = 16 * t.RB;
     t.st_k = 0;
     t.st_v = t.st_k + t.TT * t.s_row;
@@ -132,10 +134,11 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
       b.fhead = (int8_t)h; b.col_off = (int16_t)(b.col_off + h * g.D);
       t.blk[i] = b;
     }
-    for (int NS = 4; NS >= 2; --NS) {
+    for (int NS = ns_max; NS >= 2; --NS) {
       t.n_stages = NS;
       t.smem_bytes = t.off_stage0 + NS * t.stage_bytes;
       if (t.smem_bytes > limit) continue;
+      t.load_hint = c->reloc_load_hint;
       if (NS >= 3) { *out = t; return true; }
       if (!have) { best = t; have = true; }
       break;
@@ -398,6 +401,9 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
   c->lay = *layout;
   c->fast_layout = build_head_blocks(c);
   if (const char* e = getenv("KAM_RELOC_CONTIG")) c->contig_copies = (e[0] != '0');   // tuning switch, default on
+  if (const char* e = getenv("KAM_RELOC_STAGES")) c->reloc_stages = atoi(e);
+  if (const char* e = getenv("KAM_RELOC_RB")) c->reloc_rb = atoi(e);
+  if (const char* e = getenv("KAM_RELOC_HINT")) c->reloc_load_hint = atoi(e);
   c->max_requests = max_requests; c->max_chunks = max_chunks_per_request; c->max_ppc = max_pages_per_chunk;
   if (pool) { c->pool = *pool; c->has_pool = true; }
   if (pool) {

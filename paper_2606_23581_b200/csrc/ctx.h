@@ -36,6 +36,7 @@ struct kam_ctx {
   std::string fast_layout_why;
   int blocks_per_head = 0;
   bool contig_copies = true;                  // one unpadded copy per tile when a slice is a whole token row (KAM_RELOC_CONTIG=0: padded per-row copies)
+  int reloc_stages = 0, reloc_load_hint = 1, reloc_rb = 0;  // tuning switches (KAM_RELOC_STAGES, KAM_RELOC_HINT, KAM_RELOC_RB)
   kam::ColBlock head_blocks[kam::kMaxColBlocks];
 
   kam::Staging staging[kam::kStagingSlots];

@@ -63,6 +63,7 @@ struct RelocGeom {
   int32_t st_k, st_v, st_uk, st_uv, st_slot;        // offsets inside a stage
   int32_t w_kv_stride;          // bytes of one of {K,V}'s fragment table
   int32_t smem_bytes;
+  int32_t load_hint;            // 1: canonical sources are read with L2 evict_first
   double theta;
   ColBlock blk[kMaxColBlocks];
 };

@@ -298,7 +298,12 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
           uint8_t* dst = st + (role == 0 ? g.st_k : g.st_v);
           if (!inplace) {
             const char* s0 = src + static_cast<size_t>(tok0) * g.row_bytes + off;
-            if (g.contig) { if (lane == 0) bulk_g2s(dst, s0, static_cast<uint32_t>(nvalid) * g.slice_bytes, fb); }
+            if (g.contig) {
+              if (lane == 0) {
+                if (g.load_hint) bulk_g2s_hint(dst, s0, static_cast<uint32_t>(nvalid) * g.slice_bytes, fb, make_policy_evict_first());
+                else bulk_g2s(dst, s0, static_cast<uint32_t>(nvalid) * g.slice_bytes, fb);
+              }
+            }
             else for (int r = lane; r < nvalid; r += 32) bulk_g2s(dst + r * g.s_row, s0 + static_cast<size_t>(r) * g.row_bytes, g.slice_bytes, fb);
           } else if (g.contig) {
             // pool rows are contiguous inside a page: one copy per run of consecutive slots, issued by the run's first lane
