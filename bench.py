@@ -34,6 +34,7 @@ sys.path.insert(0, ROOT)
 CFG_ID = 2
 N_REQ = 32              # requests per GPU = decode batch (configs[1] names none; 32 is configs[3]'s); each owns an 8-chunk window
 N_SETS = 2              # canonical chunk sets cycled so that sources miss L2
+CPU_SAMPLE_CHUNKS = 12  # cpu_baseline sample: ~10 s of oracle work on the GPU box's host
 
 
 def algorithmic_bytes_relocate(T, H, D, m, P, has_v=True):
@@ -57,11 +58,18 @@ class ClockSampler:
 
     def __init__(self, gpu_index):
         self.rows, self.proc, self.idx = [], None, gpu_index
+        self.t0 = self.t1 = None                      # host times bracketing the timed region: only samples inside count
+
+    def mark_begin(self):
+        self.t0 = time.time()
+
+    def mark_end(self):
+        self.t1 = time.time()
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
         except Exception:
@@ -69,7 +77,7 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            self.rows.append([x.strip() for x in line.split(",")] + [time.time()])
 
     def stop(self):
         if not self.proc:
@@ -79,10 +87,13 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
-        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        rows = [r for r in self.rows if len(r) >= 10 and r[1].replace(".", "").isdigit()]
+        if self.t0 is not None and self.t1 is not None:
+            rows = [r for r in rows if self.t0 <= r[-1] <= self.t1 + 0.02]
+        sm = [float(r[1]) for r in rows]
+        mx = [float(r[2]) for r in rows if r[2].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({n for r in self.rows if len(r) >= 9 for n, v in zip(names, r[5:9]) if v.lower().startswith("active")})
+        reasons = sorted({n for r in rows for n, v in zip(names, r[5:9]) if v.lower().startswith("active")})
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
                 "samples": len(sm)}
 
@@ -319,7 +330,7 @@ def sum_over_ranks(x, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
@@ -352,14 +363,15 @@ def main():
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()                              # already streaming when the timed region starts
     for i in range(args.warmup):
         wl.step(i)
     barrier()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
     l0 = wl.launches()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
+    sampler.mark_begin()
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t_start.record()
     for i in range(args.steps):
@@ -370,6 +382,7 @@ def main():
             torch.cuda.profiler.stop()
     t_end.record()
     barrier()
+    sampler.mark_end()
     clocks = sampler.stop() if rank == 0 else None
     launches = (wl.launches() - l0) // args.steps
     total_ms = max_over_ranks(t_start.elapsed_time(t_end), world)
@@ -418,9 +431,10 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        gbs, dt = oracle_sample(2, L)
+        gbs, dt = oracle_sample(CPU_SAMPLE_CHUNKS, L)
         cpu = {"value": gbs, "unit": "GB/s", "cores": cpu_threads(), "kind": "oracle", "seconds": dt,
-               "sample": "relocate+patch of 2 chunks x 28 layers of config 2 (of 8 chunks per step), oracle/reuse.py in numpy fp64"}
+               "sample": "relocate+patch of %d chunks x 28 layers of config 2 (1.5 steps' worth; a step has 8 chunks), "
+                         "oracle/reuse.py in numpy fp64" % CPU_SAMPLE_CHUNKS}
 
     if rank == 0:
         out = {
