@@ -106,12 +106,19 @@ typedef struct kam_reloc_desc {
   int32_t rank;
 } kam_reloc_desc;
 
-/* One layer's factors of one (request, chunk), for patching on read inside the decode kernel. */
+/* One layer's factors of one (request, chunk), for patching on read inside the decode kernel (Eq. 1 applied to
+ * the keys and values as they are read, the pool is never written).  Uk/Wk/Uv/Wv: device pointers to THIS layer's
+ * U [T][..] (token t of the chunk = row t, strides as in kam_patch) and W [H][rank][row_dim]; bf16.  rank: 0 or all
+ * pointers NULL => no patch for this chunk; otherwise a multiple of 16, <= the context's max patch rank
+ * (kam_decode_set_max_patch_rank), u_token_stride and u_head_stride multiples of 8, pointers 16-byte aligned.
+ * u_head_stride is either 0 (one U shared by all KV heads, R-6) or >= rank.  A ref that breaks these rules is ignored
+ * by the kernel and counted in kam_stats.device_errors.  MLA (has_v == 0): Uv/Wv are not read - the value patch is the
+ * first v_dim columns of the key patch. */
 typedef struct kam_patch_ref {
-  const void *Uk, *Wk, *Uv, *Wv;   /* device; this layer's U [T][..] and W [H][rank][row_dim]; all NULL => no patch */
+  const void *Uk, *Wk, *Uv, *Wv;
   int64_t u_token_stride, u_head_stride;
   int32_t rank;
-  int32_t reserved;
+  int32_t frame;                   /* kam_patch_frame of the K patch: TARGET (Eq. 1) or CANONICAL (R-4) */
 } kam_patch_ref;
 
 typedef struct kam_stats {
@@ -119,6 +126,7 @@ typedef struct kam_stats {
   int64_t table_entries_written;   /* page-table entries written since kam_create (O(1)-per-op evidence) */
   int64_t chunks_live;
   int64_t kernels_launched;        /* CUDA kernels this context has launched since kam_create */
+  int64_t device_errors;           /* malformed kam_patch_ref records the decode kernels ignored (reading it synchronises) */
 } kam_stats;
 
 /* ---- context -------------------------------------------------------------------------------------------------
@@ -186,6 +194,7 @@ kam_status kam_window_export(kam_ctx *ctx, int32_t req, int32_t *block_table_out
                              int64_t *slot_mapping_out, int64_t slot_mapping_cap, int32_t *chunk_starts_out,
                              int64_t *chunk_offsets_out, int32_t *chunk_handles_out, int32_t chunk_cap,
                              int32_t *n_pages_out, int32_t *n_chunks_out);
+/* Host counters; device_errors is copied back from the device, so this call waits for the context's earlier work. */
 kam_status kam_get_stats(kam_ctx *ctx, kam_stats *out);
 
 /* ---- fused-on-read paged decode with LSE merge (R-12) -----------------------------------------------------
@@ -195,9 +204,15 @@ kam_status kam_get_stats(kam_ctx *ctx, kam_stats *out);
  * q [batch][n_q_heads][row_dim] bf16 device.  block_tables device int32 [batch][max_pages].  chunk_starts device
  * int32 [batch][max_chunks+1] (CSR token boundaries; only differences to chunk_starts[b][0] are used).
  * chunk_offsets device int64 [batch][max_chunks] (delta to apply on read; 0 if materialised) or NULL (= all 0).
- * n_chunks device int32 [batch].  patches: NULL, or device kam_patch_ref [batch][max_chunks].
+ * n_chunks device int32 [batch].  patches: NULL, or device kam_patch_ref [batch][max_chunks]: the rank-m patch of Eq. 1
+ * is applied ON READ in O(m) per token, s_t += sm_scale * U_k[t,:].(W_k q) and o += (sum_t p_t U_v[t,:]) W_v, which is
+ * the same readout as attending over k_t + U_k W_k, v_t + U_v W_v (P:44 with Eq. 1 substituted).
  * out [batch][n_q_heads][Dv] bf16 (Dv = row_dim, or v_dim for MLA), lse [batch][n_q_heads] f32 (natural log, scale
  * inside).  A request with no tokens gives out = 0, lse = -inf.  Requires elem_dtype == KAM_BF16. */
+/* Largest rank a kam_patch_ref of later decode calls may carry: 16, 32 or 64 (default KAM_MAX_RANK).  The decode kernel
+ * is specialised for it (shared memory and registers per tile grow with it), so a caller whose patches are all rank 16
+ * should say so.  Errors: INVALID_ARG. */
+kam_status kam_decode_set_max_patch_rank(kam_ctx *ctx, int32_t max_rank);
 kam_status kam_paged_decode_merge(kam_ctx *ctx, const void *q, const kam_pool *pool, const int32_t *block_tables,
                                   int32_t max_pages, const int32_t *chunk_starts, const int64_t *chunk_offsets,
                                   const int32_t *n_chunks, int32_t max_chunks, const kam_patch_ref *patches,

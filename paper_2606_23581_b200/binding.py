@@ -51,12 +51,12 @@ class kam_reloc_desc(C.Structure):
 
 class kam_patch_ref(C.Structure):
     _fields_ = [("Uk", vp), ("Wk", vp), ("Uv", vp), ("Wv", vp), ("u_token_stride", i64), ("u_head_stride", i64),
-                ("rank", i32), ("reserved", i32)]
+                ("rank", i32), ("frame", i32)]
 
 
 class kam_stats(C.Structure):
     _fields_ = [(n, i64) for n in ("pages_free", "pages_total", "table_entries_written", "chunks_live",
-                                    "kernels_launched")]
+                                    "kernels_launched", "device_errors")]
 
 
 # name -> (restype, argtypes): every symbol include/kamera.h declares
@@ -80,6 +80,7 @@ SIGNATURES = {
     "kam_get_stats": (i32, [vp, C.POINTER(kam_stats)]),
     "kam_paged_decode_merge": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
                                      vp, vp, vp]),
+    "kam_decode_set_max_patch_rank": (i32, [vp, i32]),
     "kam_window_plan": (i32, [vp, C.POINTER(i32), i32, vp]),
     "kam_window_decode": (i32, [vp, vp, C.POINTER(i32), i32, i32, C.c_float, vp, vp, vp]),
     "kam_paged_decode_merge_host": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32,
@@ -278,6 +279,9 @@ class Context:
                                             max_chunks, _ptr(patches), int(layer), batch, float(sm_scale), _ptr(out),
                                             _ptr(lse), _stream_ptr(stream)), self.h)
 
+    def kam_decode_set_max_patch_rank(self, max_rank):
+        _check(lib().kam_decode_set_max_patch_rank(self.h, int(max_rank)), self.h)
+
     def kam_window_plan(self, req_ids, stream=None):
         ids = (i32 * len(req_ids))(*req_ids)
         _check(lib().kam_window_plan(self.h, ids, len(req_ids), _stream_ptr(stream)), self.h)
@@ -298,20 +302,22 @@ class Context:
                self.h)
 
 
-def patch_refs(refs, device):
-    """Device array of kam_patch_ref [batch][max_chunks] from nested lists of (Uk, Wk, Uv, Wv, rank) tensors or None."""
-    batch, max_chunks = len(refs), max(len(r) for r in refs)
+def patch_refs(refs, device, max_chunks=None):
+    """Device array of kam_patch_ref [batch][max_chunks] from nested lists of (Uk, Wk, Uv, Wv, rank[, frame]) or None."""
+    batch = len(refs)
+    max_chunks = max_chunks if max_chunks is not None else max(len(r) for r in refs)
     arr = (kam_patch_ref * (batch * max_chunks))()
     keep = []
     for b, row in enumerate(refs):
         for c, ref in enumerate(row):
             if ref is None:
                 continue
-            Uk, Wk, Uv, Wv, rank = ref
+            Uk, Wk, Uv, Wv, rank = ref[:5]
             a = arr[b * max_chunks + c]
             a.Uk, a.Wk, a.Uv, a.Wv = _ptr(Uk), _ptr(Wk), _ptr(Uv), _ptr(Wv)
             a.u_token_stride, a.u_head_stride = (Uk.stride(0), Uk.stride(1)) if Uk.dim() == 3 else (Uk.stride(0), 0)
             a.rank = int(rank)
+            a.frame = int(ref[5]) if len(ref) > 5 else KAM_PATCH_TARGET_FRAME
             keep.append(ref)
     raw = torch.frombuffer(bytearray(bytes(arr)), dtype=torch.uint8).to(device)
     raw._keep = keep

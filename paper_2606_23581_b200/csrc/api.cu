@@ -416,6 +416,9 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
     if (const char* ev = getenv("KAM_DEC_CTAS_PER_SM")) c->dec_ctas_per_sm = atoi(ev);
     if (const char* ev = getenv("KAM_DEC_BOXES")) c->dec_boxes = atoi(ev);
     if (const char* ev = getenv("KAM_NO_PDL")) c->use_pdl = (ev[0] == '0');
+    e = cudaMalloc(&c->d_err, sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemset(c->d_err, 0, sizeof(int32_t));
+    if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "kam_create: device error counter"); kam_destroy(c); return r; }
     if (layout->rope_dim > 0) {                // f_i = theta^(-2i/d_r) in fp64, once (R-2)
       std::vector<double> f((size_t)layout->rope_dim / 2);
       for (size_t i = 0; i < f.size(); ++i) f[i] = pow(layout->rope_theta, -2.0 * (double)i / layout->rope_dim);
@@ -452,6 +455,7 @@ kam_status kam_destroy(kam_ctx* c) {
     if (c->d_hstage2) cudaFree(c->d_hstage2);
     if (c->d_tmaps) cudaFree(c->d_tmaps);
     if (c->d_inv_freq) cudaFree(c->d_inv_freq);
+    if (c->d_err) cudaFree(c->d_err);
   }
   delete c;
   return KAM_OK;
@@ -465,6 +469,12 @@ kam_status kam_get_stats(kam_ctx* c, kam_stats* out) {
     s.table_entries_written = c->win->table_entries_written(); s.chunks_live = c->win->chunks_live();
   }
   s.kernels_launched = c->kernels_launched;
+  if (c->d_err) {
+    int32_t n = 0;
+    cudaError_t e = cudaMemcpy(&n, c->d_err, sizeof(n), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(device error counter)");
+    s.device_errors = n;
+  }
   *out = s;
   return KAM_OK;
 }

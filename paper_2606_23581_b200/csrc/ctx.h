@@ -57,8 +57,10 @@ struct kam_ctx {
   std::vector<int32_t> winplan_reqs;
   int32_t winplan_chunks = 0;
   double* d_inv_freq = nullptr;                // [rope_dim / 2] f_i = theta^(-2i/d_r), fp64
-  kam::DecodeGeom dec_geom[2];                 // cached geometry: [0] bulk-copy path, [1] TMA path over the context's pool
-  bool dec_geom_ok[2] = {false, false};
+  kam::DecodeGeom dec_geom[2][5];              // cached geometry: [bulk-copy path | TMA path over the context's pool][patch rank tiles KT]
+  bool dec_geom_ok[2][5] = {};
+  int32_t dec_max_rank = KAM_MAX_RANK;         // largest rank of an on-read patch (kam_decode_set_max_patch_rank)
+  int32_t* d_err = nullptr;                    // device counter: malformed kam_patch_ref records ignored by the decode kernel
   bool use_pdl = true;                         // programmatic dependent launch between decode and merge (KAM_NO_PDL=1 turns it off)
   int dec_ctas_per_sm = 0, dec_boxes = 0;      // tuning switches (KAM_DEC_CTAS_PER_SM, KAM_DEC_BOXES); 0 = automatic
   // device staging of host-resident chunks (kam_relocate_patch_host) and host-resident q/out (decode host variant)

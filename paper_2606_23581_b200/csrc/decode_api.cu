@@ -12,10 +12,11 @@ namespace {
 inline size_t align_up_sz(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // Geometry of the decode kernel for this context's layout; `ctas_per_sm` = 0 picks the densest configuration that fits.
-kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
+// kt: 16-wide rank tiles of the on-read patch the kernel is specialised for (0 = the call carries no patch refs).
+kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out) {
   const kam_layout& L = c->lay;
   const int variant = (c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers) ? 1 : 0;
-  if (c->dec_geom_ok[variant]) { *out = c->dec_geom[variant]; return KAM_OK; }
+  if (c->dec_geom_ok[variant][kt]) { *out = c->dec_geom[variant][kt]; return KAM_OK; }
   if (L.elem_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "decode needs a bf16 pool");
   if (!L.has_v) return fail(c, KAM_ERR_UNSUPPORTED, "decode over an MLA latent pool is not built yet (SURVEY.md 8(f) f1)");
   if (L.row_dim != 64 && L.row_dim != 128) return fail(c, KAM_ERR_UNSUPPORTED, "decode supports head_dim 64 or 128");
@@ -35,11 +36,19 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
   g.use_tma = c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers;
   g.ncb = g.HG * g.D / 64;
   g.s_row = g.slice_bytes + 16;                                   // (s_row / 16) odd: ldmatrix rows never share a bank group
-  g.box_bytes = g.use_tma ? 2048 * g.ncb : (int)align_up_sz((size_t)kDecTile * g.s_row, 128);
+  g.kv_bytes = g.use_tma ? 2048 * g.ncb : (int)align_up_sz((size_t)kDecTile * g.s_row, 128);
+  g.box_bytes = g.kv_bytes;
+  g.KT = kt;
+  if (kt > 0) {                                                   // the U tile rides behind the K / V rows of its box
+    g.u_off = g.kv_bytes;
+    g.su_row = g.HG * kt * 16 * 2;
+    if ((g.su_row / 16) % 2 == 0) g.su_row += 16;                 // (su_row / 16) odd: conflict-free ldmatrix over 8 token rows
+    g.box_bytes = (int)align_up_sz((size_t)g.kv_bytes + (size_t)kDecTile * g.su_row, g.use_tma ? 1024 : 128);
+  }
   g.off_hdr = 128; g.off_box0 = 1024;
   // CTAs per SM x ring depth: 3 CTAs with 2 K + 2 V boxes each when that fits, else fewer CTAs with a deeper ring
   const int sm_total = 227 * 1024;
-  int want = c->dec_ctas_per_sm > 0 ? c->dec_ctas_per_sm : 3;
+  int want = c->dec_ctas_per_sm > 0 ? c->dec_ctas_per_sm : (kt > 0 ? 2 : 3);
   for (; want >= 1; --want) {
     const int budget = sm_total / want - 1024 - g.off_box0;
     int nb = std::min(8, budget / g.box_bytes) & ~1;
@@ -52,7 +61,7 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, DecodeGeom* out) {
   }
   if (want < 1) return fail(c, KAM_ERR_UNSUPPORTED, "decode tile does not fit shared memory");
   g.n_ctas = c->sm_count * want;
-  c->dec_geom[variant] = g; c->dec_geom_ok[variant] = true;
+  c->dec_geom[variant][kt] = g; c->dec_geom_ok[variant][kt] = true;
   *out = g;
   return KAM_OK;
 }
@@ -113,12 +122,12 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   if (!q || !block_tables || !chunk_starts || !n_chunks || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge: NULL argument");
   if (layer < 0 || layer >= c->lay.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, c->lay.n_layers);
   if (batch < 0 || max_pages < 1 || max_chunks < 1) return fail(c, KAM_ERR_INVALID_ARG, "bad batch / max_pages / max_chunks");
-  if (patches) return fail(c, KAM_ERR_UNSUPPORTED, "on-read patching is not built yet; materialise the patch with kam_relocate_patch");
   if (batch == 0) return KAM_OK;
   if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
   if ((long long)batch * max_chunks > (1ll << 24)) return fail(c, KAM_ERR_UNSUPPORTED, "batch * max_chunks too large");
   DecodeGeom g;
-  if ((s = decode_geom(c, pool, &g)) != KAM_OK) return s;
+  const int kt = patches ? (c->dec_max_rank <= 16 ? 1 : c->dec_max_rank <= 32 ? 2 : 4) : 0;
+  if ((s = decode_geom(c, pool, kt, &g)) != KAM_OK) return s;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
 
   const int N = batch * max_chunks;
@@ -131,14 +140,14 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   p.block_tables = block_tables; p.tmaps = c->d_tmaps;
   p.plan = plan_of(c, w, N, batch);
   p.plan.block_tables = block_tables;
-  p.patches = nullptr;
+  p.patches = patches; p.err = c->d_err;
   p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse;
 
   DecodeCsr csr{};
   csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
-  csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = 0;
+  csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = patches ? 1 : 0;
   launch_decode_plan(g, p.plan, csr, st);
   launch_decode(g, p, false, st);                                 // reads the plan just written: plain stream order
   launch_decode_merge(g, p, c->use_pdl, st);
@@ -158,7 +167,7 @@ static kam_status window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch,
   for (int b = 0; b < batch; ++b)
     if (!c->win->is_open(req_ids[b])) return fail(c, KAM_ERR_STATE, "request %d is not open", req_ids[b]);
   DecodeGeom g;
-  kam_status s = decode_geom(c, &c->pool, &g);
+  kam_status s = decode_geom(c, &c->pool, 0, &g);
   if (s != KAM_OK) return s;
   const bool cached = c->winplan_epoch == c->win->epoch() && c->winplan_reqs.size() == (size_t)batch &&
                       std::equal(c->winplan_reqs.begin(), c->winplan_reqs.end(), req_ids);
@@ -206,6 +215,13 @@ static kam_status window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch,
   return KAM_OK;
 }
 
+kam_status kam_decode_set_max_patch_rank(kam_ctx* c, int32_t max_rank) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (max_rank != 16 && max_rank != 32 && max_rank != 64) return fail(c, KAM_ERR_INVALID_ARG, "max patch rank must be 16, 32 or 64 (got %d)", max_rank);
+  c->dec_max_rank = max_rank;
+  return KAM_OK;
+}
+
 kam_status kam_window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch, void* stream) {
   if (!c) return KAM_ERR_INVALID_ARG;
   if (batch == 0) return KAM_OK;
@@ -230,7 +246,7 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   p.plan.block_tables = c->d_slot_pages;
   p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
-  p.sm_scale = sm_scale; p.out = out; p.lse = lse;
+  p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.err = c->d_err;
   // with a plan from an earlier call the decode prologue may overlap whatever precedes it on the stream (it only reads the plan)
   launch_decode(g, p, cached && c->use_pdl, st);
   launch_decode_merge(g, p, c->use_pdl, st);

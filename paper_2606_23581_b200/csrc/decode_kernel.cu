@@ -214,6 +214,28 @@ __device__ __forceinline__ float col_sum(float v) {
   v += __shfl_xor_sync(0xffffffffu, v, 8);
   return v + __shfl_xor_sync(0xffffffffu, v, 16);
 }
+__device__ __forceinline__ uint32_t ldg_u32(const void* p) { return __ldg(reinterpret_cast<const unsigned int*>(p)); }
+__device__ __forceinline__ uint32_t ldg_u16(const void* p) { return __ldg(reinterpret_cast<const unsigned short*>(p)); }
+
+// On-read patch of one segment: rank of the chunk's kam_patch_ref if the record is well formed and the kernel is specialised
+// for it (KT rank tiles), else 0 (no patch; malformed records are counted once per segment by the producer warp).
+struct SegPatch { const char* Uk; const char* Uv; const __nv_bfloat16* Wk; const __nv_bfloat16* Wv; long long uts, uhs; int rank, frame; };
+__device__ __forceinline__ SegPatch seg_patch(const kam_patch_ref* refs, int idx, int KT, bool* malformed) {
+  SegPatch sp{};
+  *malformed = false;
+  if (!refs || idx < 0) return sp;
+  const kam_patch_ref r = refs[idx];
+  if (r.rank == 0 || (!r.Uk && !r.Wk && !r.Uv && !r.Wv)) return sp;
+  const bool ok = r.rank > 0 && r.rank % 16 == 0 && r.rank <= KT * 16 && r.Uk && r.Wk && r.Uv && r.Wv &&
+                  (r.u_token_stride & 7) == 0 && (r.u_head_stride & 7) == 0 && (r.u_head_stride == 0 || r.u_head_stride >= r.rank) &&
+                  ((reinterpret_cast<uintptr_t>(r.Uk) | reinterpret_cast<uintptr_t>(r.Uv) | reinterpret_cast<uintptr_t>(r.Wk) |
+                    reinterpret_cast<uintptr_t>(r.Wv)) & 15) == 0;
+  if (!ok) { *malformed = true; return sp; }
+  sp.Uk = static_cast<const char*>(r.Uk); sp.Uv = static_cast<const char*>(r.Uv);
+  sp.Wk = static_cast<const __nv_bfloat16*>(r.Wk); sp.Wv = static_cast<const __nv_bfloat16*>(r.Wv);
+  sp.uts = r.u_token_stride; sp.uhs = r.u_head_stride; sp.rank = r.rank; sp.frame = r.frame;
+  return sp;
+}
 }  // namespace
 
 // KS = D / 16 (k-steps of QK^T; D = Dv).  NT = ceil(G / 8) query-head tiles.  TMA: pool pages arrive as swizzled boxes.
@@ -223,8 +245,13 @@ __device__ __forceinline__ float col_sum(float v) {
 // and ldmatrix (K) / ldmatrix.trans (V) are conflict-free without padding.  Bulk-copy path: [token r][s_row bytes], s_row
 // padded so that (s_row / 16) is odd.  Tiles are aligned to 16 tokens of the page list (P % 16 == 0 on the TMA path, so a
 // box never straddles a page); rows outside the chunk's token range are masked in the softmax and zeroed in V.
-template <int KS, int NT, bool TMA>
-__global__ void __launch_bounds__((kDecMaxHG + 1) * 32, NT == 1 ? 3 : 1)
+//
+// KT > 0: on-read patch (Eq. 1 applied to what is read; the pool is never written).  Behind the K rows of a box rides the
+// tile's U_k rows, behind the V rows its U_v rows ([16 tokens][su_row bytes], one run of `rank` values per KV head).  With
+// wq = W_k q (per segment, m x G, carried as bf16 hi + lo):   s_t += U_k[t,:] . wq          (rank/16 MMAs per tile)
+// and z += U_v^T P^T accumulated like O (rank/16 MMAs per tile); at the end of the segment o += W_v^T z.
+template <int KS, int NT, bool TMA, int KT>
+__global__ void __launch_bounds__((kDecMaxHG + 1) * 32, (NT == 1 && KT == 0) ? 3 : (NT == 1 ? 2 : 1))
 kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
   uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem);
@@ -257,6 +284,21 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
       if (seg + 1 < seg_end) S_next = p.plan.segs[seg + 1];     // in flight while this segment streams
       const int32_t* bt = p.block_tables + S.bt_off;
       const size_t col_off = static_cast<size_t>(S.hg) * g.slice_bytes;
+      [[maybe_unused]] SegPatch sp{};
+      [[maybe_unused]] uint32_t u_row_bytes = 0, u_run_bytes = 0; [[maybe_unused]] int u_runs = 0;
+      if constexpr (KT > 0) {
+        bool bad;
+        sp = seg_patch(p.patches, S.patch, KT, &bad);
+        if (bad && lane == 0 && S.tile0 * kDecTile <= S.tok_lo && S.hg == 0) atomicAdd(p.err, 1);   // once per chunk
+        if (sp.rank) {
+          // a token's U run of this head group: HG heads x rank (one copy if the heads are contiguous), or rank (shared U)
+          const int nh = sp.uhs == 0 ? 1 : g.HG;
+          const bool one = nh == 1 || sp.uhs == sp.rank;
+          u_runs = one ? 1 : nh;
+          u_run_bytes = static_cast<uint32_t>((one ? nh : 1) * sp.rank * 2);
+          u_row_bytes = static_cast<uint32_t>(nh * sp.rank * 2);
+        }
+      }
       for (int t0 = 0; t0 < S.n_tiles; t0 += 32) {
         int slot = 0;
         if (t0 + lane < S.n_tiles && t0 + lane > 0) {           // A1: page = block_table[tok / P], slot = page * P + tok % P
@@ -282,6 +324,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
           for (int kv = 0; kv < 2; ++kv) {
             mbar_wait(&empty_bar[box], phase ^ 1);
             uint8_t* dst = box0 + static_cast<size_t>(box) * g.box_bytes;
+            const uint32_t u_bytes = static_cast<uint32_t>(row_hi - row_lo) * u_row_bytes;      // 0 without a patch
             if (lane == 0) {
               if (kv == 0) {
                 const int flags = (tl == 0 ? HDR_FIRST : 0) | (tl == S.n_tiles - 1 ? HDR_LAST : 0) |
@@ -289,10 +332,21 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
                 hdrs[box] = make_int4(seg, flags, row_lo | (row_hi << 8), tok - S.tok_lo);
               }
               if constexpr (TMA) {
-                mbar_arrive_expect_tx(&full_bar[box], static_cast<uint32_t>(g.box_bytes));
+                mbar_arrive_expect_tx(&full_bar[box], static_cast<uint32_t>(g.kv_bytes) + u_bytes);
                 tma_load_3d(dst, kv ? tm_v : tm_k, 0, s0, S.hg * g.ncb, &full_bar[box]);
               } else {
-                mbar_arrive_expect_tx(&full_bar[box], static_cast<uint32_t>(row_hi - row_lo) * g.slice_bytes);
+                mbar_arrive_expect_tx(&full_bar[box], static_cast<uint32_t>(row_hi - row_lo) * g.slice_bytes + u_bytes);
+              }
+            }
+            if constexpr (KT > 0) {
+              if (u_bytes) {                                       // lane r copies token row r's U run(s): chunk-local token tok - tok_lo + r
+                __syncwarp();
+                if (lane >= row_lo && lane < row_hi) {
+                  const char* src = (kv ? sp.Uv : sp.Uk) +
+                                    ((static_cast<long long>(tok - S.tok_lo + lane)) * sp.uts + static_cast<long long>(S.hg) * g.HG * sp.uhs) * 2;
+                  uint8_t* ud = dst + g.u_off + lane * g.su_row;
+                  for (int r = 0; r < u_runs; ++r) bulk_g2s(ud + r * sp.rank * 2, src + r * sp.uhs * 2, u_run_bytes, &full_bar[box]);
+                }
               }
             }
             if constexpr (!TMA) {
@@ -321,6 +375,12 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
   float O[NT][KS][4];
   float m_run[NT][2], l_run[NT][2];
   bool use_lo = false;
+  constexpr int KTA = KT > 0 ? KT : 1;
+  [[maybe_unused]] uint32_t wqh[NT][KTA][2], wql[NT][KTA][2];     // (W_k q)^T as the B operand of the score MMA, bf16 hi + lo
+  [[maybe_unused]] float Z[NT][KTA][4];                           // z^T[j][head] = sum_t p_t U_v[t][j]
+  [[maybe_unused]] int kt_seg = 0;                                // rank / 16 of this segment's patch (0: none)
+  [[maybe_unused]] const __nv_bfloat16* Wv_seg = nullptr;
+  [[maybe_unused]] uint32_t u_head_off = 0;                       // bytes: this warp's KV head inside a U row
 
   // ldmatrix lane addressing inside a box (bytes)
   //   K (A operand, rows = tokens): matrices (tokens 0-7 | 8-15) x (first | second 16-byte chunk of the k-step)
@@ -397,6 +457,53 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
         m_run[nt][0] = m_run[nt][1] = -CUDART_INF_F;
         l_run[nt][0] = l_run[nt][1] = 0.f;
       }
+      if constexpr (KT > 0) {
+        // ---- on-read patch of this segment: (W_k q)^T [rank][G] by MMA (A = W_k rows from global, B = the q fragments).
+        // TARGET frame (Eq. 1: rotate, then add) contracts W_k with the UNrotated q; CANONICAL with the rotated one.
+        bool bad;
+        const SegPatch sp = seg_patch(p.patches, S.patch, KT, &bad);
+        kt_seg = sp.rank >> 4;
+        if (kt_seg) {
+          const __nv_bfloat16* Wk = sp.Wk + static_cast<size_t>(head) * sp.rank * D;
+          Wv_seg = sp.Wv + static_cast<size_t>(head) * sp.rank * D;
+          u_head_off = sp.uhs ? static_cast<uint32_t>(warp * sp.rank * 2) : 0u;
+          const bool raw_q = use_lo && sp.frame != KAM_PATCH_CANONICAL_FRAME;
+#pragma unroll
+          for (int kt = 0; kt < KT; ++kt) {
+            if (kt < kt_seg) {
+              float acc[NT][4];
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+              const __nv_bfloat16* w0 = Wk + static_cast<size_t>(kt * 16 + gq) * D + 2 * t4;
+#pragma unroll
+              for (int ks = 0; ks < KS; ++ks) {
+                const uint32_t a0 = ldg_u32(w0 + ks * 16), a1 = ldg_u32(w0 + 8 * D + ks * 16);
+                const uint32_t a2 = ldg_u32(w0 + ks * 16 + 8), a3 = ldg_u32(w0 + 8 * D + ks * 16 + 8);
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                  uint32_t b0 = qhi[nt][ks][0], b1 = qhi[nt][ks][1];
+                  if (raw_q) {
+                    const int row = nt * 8 + gq;
+                    b0 = b1 = 0u;
+                    if (row < g.G) { const __nv_bfloat16* qr = qb + static_cast<size_t>(row) * D + ks * 16 + 2 * t4; b0 = ldg_u32(qr); b1 = ldg_u32(qr + 8); }
+                  }
+                  mma_bf16_16816(acc[nt][0], acc[nt][1], acc[nt][2], acc[nt][3], a0, a1, a2, a3, b0, b1);
+                  if (use_lo && !raw_q) mma_bf16_16816(acc[nt][0], acc[nt][1], acc[nt][2], acc[nt][3], a0, a1, a2, a3, qlo[nt][ks][0], qlo[nt][ks][1]);
+                }
+              }
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) {
+                const uint32_t h01 = pack_bf16x2(acc[nt][0], acc[nt][1]), h23 = pack_bf16x2(acc[nt][2], acc[nt][3]);
+                const uint32_t l01 = pack_bf16x2(acc[nt][0] - bf_lo(h01), acc[nt][1] - bf_hi(h01));
+                const uint32_t l23 = pack_bf16x2(acc[nt][2] - bf_lo(h23), acc[nt][3] - bf_hi(h23));
+                wqh[nt][kt][0] = movmatrix_trans(h01); wqh[nt][kt][1] = movmatrix_trans(h23);
+                wql[nt][kt][0] = movmatrix_trans(l01); wql[nt][kt][1] = movmatrix_trans(l23);
+                Z[nt][kt][0] = Z[nt][kt][1] = Z[nt][kt][2] = Z[nt][kt][3] = 0.f;
+              }
+            }
+          }
+        }
+      }
     }
 
     // ---- S^T[16 tokens][8 heads] = K q~^T : two interleaved accumulator chains per head tile
@@ -415,6 +522,23 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
         if (use_lo) {
           if (ks & 1) mma_bf16_16816(sa[nt][0], sa[nt][1], sa[nt][2], sa[nt][3], a0, a1, a2, a3, qlo[nt][ks][0], qlo[nt][ks][1]);
           else        mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, qlo[nt][ks][0], qlo[nt][ks][1]);
+        }
+      }
+    }
+    if constexpr (KT > 0) {
+      if (kt_seg) {                                             // s_t += U_k[t,:] . (W_k q): A = the tile's U_k rows (tokens x rank)
+        const uint32_t ub = kb - k_lane + g.u_off + k_row * g.su_row + u_head_off + k_hi * 16;
+#pragma unroll
+        for (int kt = 0; kt < KT; ++kt) {
+          if (kt < kt_seg) {
+            uint32_t a0, a1, a2, a3;
+            ldmatrix_x4(a0, a1, a2, a3, ub + kt * 32);
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              mma_bf16_16816(sa[nt][0], sa[nt][1], sa[nt][2], sa[nt][3], a0, a1, a2, a3, wqh[nt][kt][0], wqh[nt][kt][1]);
+              mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, wql[nt][kt][0], wql[nt][kt][1]);
+            }
+          }
         }
       }
     }
@@ -457,6 +581,12 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
       for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
         for (int n = 0; n < KS; ++n) { O[nt][n][0] *= al[nt][0]; O[nt][n][1] *= al[nt][1]; O[nt][n][2] *= al[nt][0]; O[nt][n][3] *= al[nt][1]; }
+      if constexpr (KT > 0) {
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+          for (int kt = 0; kt < KT; ++kt) { Z[nt][kt][0] *= al[nt][0]; Z[nt][kt][1] *= al[nt][1]; Z[nt][kt][2] *= al[nt][0]; Z[nt][kt][3] *= al[nt][1]; }
+      }
     }
 
     // ---- O^T[d][head] += V^T P^T
@@ -474,6 +604,15 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
           *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
         }
       }
+      if constexpr (KT > 0) {
+        if (kt_seg) {                                           // same for the U_v rows of this warp's head (2 chunks per rank tile)
+          const int cpr = kt_seg * 2;
+          for (int idx = lane; idx < 16 * cpr; idx += 32) {
+            const int r = idx / cpr, j = idx - r * cpr;
+            if (r < row_lo || r >= row_hi) *reinterpret_cast<uint4*>(vbox + g.u_off + r * g.su_row + u_head_off + j * 16) = make_uint4(0, 0, 0, 0);
+          }
+        }
+      }
       __syncwarp();
     }
     const uint32_t vb = smem_u32(vbox) + v_lane;
@@ -485,10 +624,56 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
       for (int nt = 0; nt < NT; ++nt)
         mma_bf16_16816(O[nt][dp][0], O[nt][dp][1], O[nt][dp][2], O[nt][dp][3], a0, a1, a2, a3, pb[nt][0], pb[nt][1]);
     }
+    if constexpr (KT > 0) {
+      if (kt_seg) {                                             // z^T[j][head] += U_v^T P^T: A = the tile's U_v rows, transposed on load
+        const uint32_t ub = smem_u32(vbox) + g.u_off + v_row * g.su_row + u_head_off + v_hi * 16;
+#pragma unroll
+        for (int kt = 0; kt < KT; ++kt) {
+          if (kt < kt_seg) {
+            uint32_t a0, a1, a2, a3;
+            ldmatrix_x4_trans(a0, a1, a2, a3, ub + kt * 32);
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt)
+              mma_bf16_16816(Z[nt][kt][0], Z[nt][kt][1], Z[nt][kt][2], Z[nt][kt][3], a0, a1, a2, a3, pb[nt][0], pb[nt][1]);
+          }
+        }
+      }
+    }
     if (partial) fence_proxy_async();                           // the zeroed rows were generic-proxy writes; the next fill is TMA
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty_bar[vboxi]);
 
+    if constexpr (KT > 0) {
+      if ((hdr.y & HDR_LAST) && kt_seg) {
+        // ---- o^T[d][head] += W_v^T[d][j] z^T[j][head]: A[d][j] = W_v[j][d] gathered from global, B = z^T as bf16 hi + lo
+#pragma unroll
+        for (int kt = 0; kt < KT; ++kt) {
+          if (kt < kt_seg) {
+            uint32_t bh[NT][2], bl[NT][2];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              const uint32_t h01 = pack_bf16x2(Z[nt][kt][0], Z[nt][kt][1]), h23 = pack_bf16x2(Z[nt][kt][2], Z[nt][kt][3]);
+              const uint32_t l01 = pack_bf16x2(Z[nt][kt][0] - bf_lo(h01), Z[nt][kt][1] - bf_hi(h01));
+              const uint32_t l23 = pack_bf16x2(Z[nt][kt][2] - bf_lo(h23), Z[nt][kt][3] - bf_hi(h23));
+              bh[nt][0] = movmatrix_trans(h01); bh[nt][1] = movmatrix_trans(h23);
+              bl[nt][0] = movmatrix_trans(l01); bl[nt][1] = movmatrix_trans(l23);
+            }
+            const __nv_bfloat16* w0 = Wv_seg + static_cast<size_t>(kt * 16 + 2 * t4) * D + gq;
+#pragma unroll
+            for (int dp = 0; dp < KS; ++dp) {
+              const __nv_bfloat16* w = w0 + dp * 16;
+              const uint32_t a0 = ldg_u16(w) | (ldg_u16(w + D) << 16), a1 = ldg_u16(w + 8) | (ldg_u16(w + D + 8) << 16);
+              const uint32_t a2 = ldg_u16(w + 8 * D) | (ldg_u16(w + 9 * D) << 16), a3 = ldg_u16(w + 8 * D + 8) | (ldg_u16(w + 9 * D + 8) << 16);
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) {
+                mma_bf16_16816(O[nt][dp][0], O[nt][dp][1], O[nt][dp][2], O[nt][dp][3], a0, a1, a2, a3, bh[nt][0], bh[nt][1]);
+                mma_bf16_16816(O[nt][dp][0], O[nt][dp][1], O[nt][dp][2], O[nt][dp][3], a0, a1, a2, a3, bl[nt][0], bl[nt][1]);
+              }
+            }
+          }
+        }
+      }
+    }
     if (hdr.y & HDR_LAST) {
       // ---- per-(segment, head) softmax state -> partials: o normalised, lse in natural log
 #pragma unroll
@@ -512,14 +697,26 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
 }
 
 namespace {
-template <typename F> void decode_dispatch(const DecodeGeom& g, F&& f) {
-  if (g.D == 128) {
-    if (g.NT == 1) { if (g.use_tma) f(kam_paged_decode_kernel<8, 1, true>); else f(kam_paged_decode_kernel<8, 1, false>); }
-    else           { if (g.use_tma) f(kam_paged_decode_kernel<8, 2, true>); else f(kam_paged_decode_kernel<8, 2, false>); }
+template <int KS, int NT, typename F> void decode_dispatch_kt(const DecodeGeom& g, F&& f) {
+  if (g.use_tma) {
+    switch (g.KT) {
+      case 0: f(kam_paged_decode_kernel<KS, NT, true, 0>); break;
+      case 1: f(kam_paged_decode_kernel<KS, NT, true, 1>); break;
+      case 2: f(kam_paged_decode_kernel<KS, NT, true, 2>); break;
+      default: f(kam_paged_decode_kernel<KS, NT, true, 4>); break;
+    }
   } else {
-    if (g.NT == 1) { if (g.use_tma) f(kam_paged_decode_kernel<4, 1, true>); else f(kam_paged_decode_kernel<4, 1, false>); }
-    else           { if (g.use_tma) f(kam_paged_decode_kernel<4, 2, true>); else f(kam_paged_decode_kernel<4, 2, false>); }
+    switch (g.KT) {
+      case 0: f(kam_paged_decode_kernel<KS, NT, false, 0>); break;
+      case 1: f(kam_paged_decode_kernel<KS, NT, false, 1>); break;
+      case 2: f(kam_paged_decode_kernel<KS, NT, false, 2>); break;
+      default: f(kam_paged_decode_kernel<KS, NT, false, 4>); break;
+    }
   }
+}
+template <typename F> void decode_dispatch(const DecodeGeom& g, F&& f) {
+  if (g.D == 128) { if (g.NT == 1) decode_dispatch_kt<8, 1>(g, f); else decode_dispatch_kt<8, 2>(g, f); }
+  else            { if (g.NT == 1) decode_dispatch_kt<4, 1>(g, f); else decode_dispatch_kt<4, 2>(g, f); }
 }
 }  // namespace
 

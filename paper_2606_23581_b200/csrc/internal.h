@@ -113,7 +113,9 @@ struct DecodeGeom {
   int32_t use_tma;               // 1: pool pages arrive as 16-token swizzled TMA boxes; 0: one padded bulk copy per token
   int32_t ncb;                   // TMA path: 64-column blocks per slice
   int32_t n_ctas;                // persistent grid: sm_count * CTAs per SM
-  int32_t max_rank;              // 0: no on-read patch in this call
+  int32_t KT;                    // on-read patch: 16-wide rank tiles the kernel is specialised for (0: no patch in this call)
+  int32_t kv_bytes;              // bytes of the K (or V) rows of a box; box_bytes = kv_bytes + the U tile (KT > 0)
+  int32_t u_off, su_row;         // U tile inside a box: [16 tokens][su_row bytes], (su_row / 16) odd
 };
 
 struct DecChunk {                // plan input: one chunk of one request (flat, request-major)
@@ -157,6 +159,7 @@ struct DecodeParams {
   const void* tmaps;             // device array of CUtensorMap [n_layers][2] over the context's pool (TMA path)
   DecodePlan plan;
   const kam_patch_ref* patches;  // device array or nullptr
+  int32_t* err;                  // device counter of malformed patch refs (kam_stats.device_errors)
   float* part_o;                 // [max_segs][R][Dv]
   float* part_lse;               // [max_segs][R]
   float sm_scale;

@@ -250,3 +250,151 @@ def test_window_store_slides_lazy_and_materialised_match_oracle():
         ctx.kam_window_close(1)
         assert ctx.kam_get_stats()["pages_free"] == n_pages
         ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ on-read patch (A8)
+def _run_patched(cfg, lens, deltas, ranks, seed, max_rank=None, shared_u=False, frame=reuse.TARGET_FRAME, other_pool=False,
+                 bad=None):
+    """Stateless decode with the rank-m patch applied ON READ: ranks[b][c] = rank of chunk (b, c) (0 = no patch).  The oracle
+    attends over k^ = R(delta) k + U_k W_k, v^ = v + U_v W_v formed in fp64 from the same pool bits and factor bits (O8).
+    bad = (b, c, rank): that ref is given a malformed rank; the kernel must ignore it and count it."""
+    rng = _rng(seed)
+    P, H, D = cfg.page_size, cfg.n_kv_heads, cfg.row_dim
+    batch = len(lens)
+    max_chunks = max(1, max(len(x) for x in lens))
+    max_pages = max(1, max((sum(x) + P - 1) // P for x in lens))
+    num_pages = batch * max_pages + 3
+    pool = _fill_pool(cfg, 1, num_pages, seed)
+    ctx_pool = _fill_pool(cfg, 1, 2, seed + 1) if other_pool else pool       # other_pool: the bulk-copy (non tensor-map) path
+    ctx = kam.Context(par.layout_of(cfg, 1), ctx_pool)
+    if max_rank:
+        ctx.kam_decode_set_max_patch_rank(max_rank)
+    perm = make_block_table(rng, batch * max_pages, num_pages).reshape(batch, max_pages)
+    starts = np.zeros((batch, max_chunks + 1), np.int32)
+    offs = np.zeros((batch, max_chunks), np.int64)
+    ncs = np.array([len(x) for x in lens], np.int32)
+    refs, host = [], {}
+    for b in range(batch):
+        row = []
+        for c, n in enumerate(lens[b]):
+            starts[b, c + 1] = starts[b, c] + n
+            offs[b, c] = deltas[b][c]
+            m = ranks[b][c]
+            if m == 0:
+                row.append(None)
+                continue
+            f = make_chunk(cfg.scaled(n_layers=1), rng, n_tokens=n, n_layers=1, rank=m)      # only the factors are used
+            Uk, Wk, Uv, Wv = f["Uk"][0], f["Wk"][0], f["Uv"][0], f["Wv"][0]
+            if shared_u:
+                Uk, Uv = Uk[:, 0, :].contiguous(), Uv[:, 0, :].contiguous()
+            host[(b, c)] = (Uk, Wk, Uv, Wv)
+            mm = bad[2] if bad is not None and bad[:2] == (b, c) else m
+            row.append((Uk.cuda(), Wk.cuda(), Uv.cuda(), Wv.cuda(), mm, frame))
+        starts[b, len(lens[b]) + 1:] = starts[b, len(lens[b])]
+        refs.append(row)
+    patches = B.patch_refs(refs, "cuda", max_chunks=max_chunks)
+    q = make_query(cfg, rng, batch)
+    out = torch.full((batch, cfg.n_q_heads, D), 7.0, dtype=torch.bfloat16, device="cuda")
+    lse = torch.full((batch, cfg.n_q_heads), 7.0, dtype=torch.float32, device="cuda")
+    scale = D ** -0.5
+    args = (q.cuda(), torch.from_numpy(perm).cuda(), torch.from_numpy(starts).cuda(), torch.from_numpy(offs).cuda(),
+            torch.from_numpy(ncs).cuda(), 0, scale)
+    ctx.kam_paged_decode_merge(*args, out, lse, patches=patches, pool=pool if other_pool else None)
+    out2, lse2 = torch.empty_like(out), torch.empty_like(lse)
+    ctx.kam_paged_decode_merge(*args, out2, lse2, patches=patches, pool=pool if other_pool else None)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2) and torch.equal(lse, lse2)                 # deterministic
+    out_g, lse_g = par.to_f64(out), par.to_f64(lse)
+    rope = dict(par.rope_kw(cfg), frame=frame)
+    for b in range(batch):
+        chunks, t0 = [], 0
+        for c, n in enumerate(lens[b]):
+            ch = {"k": par.pool_rows(pool.k_layers[0], perm[b], t0, n), "v": par.pool_rows(pool.v_layers[0], perm[b], t0, n),
+                  "delta": int(deltas[b][c])}
+            if (b, c) in host and not (bad is not None and bad[:2] == (b, c)):
+                Uk, Wk, Uv, Wv = [par.to_f64(x) for x in host[(b, c)]]
+                if shared_u:
+                    Uk = np.repeat(Uk[:, None, :], H, axis=1); Uv = np.repeat(Uv[:, None, :], H, axis=1)
+                ch.update(Uk=Uk, Wk=Wk, Uv=Uv, Wv=Wv)
+            chunks.append(ch)
+            t0 += n
+        o, l = att.attend_bruteforce(par.to_f64(q[b]), chunks, scale, rope)
+        check_attention(out_g[b], lse_g[b], o, l, "patched request %d" % b)
+    errs = ctx.kam_get_stats()["device_errors"]
+    ctx.close()
+    return errs
+
+
+def test_on_read_patch_config2_rank16_ragged_with_rotation():
+    """GQA 28/4, rank 16: ragged chunks (tiles that straddle chunk boundaries), pending offsets AND patches on read, one
+    chunk without a patch."""
+    lens = [[100, 1024, 37], [1024], [5, 16, 300, 700]]
+    deltas = [[0, 31000, -77], [12345], [0, 0, -1280, 99999]]
+    ranks = [[16, 16, 16], [16], [16, 0, 16, 16]]
+    assert _run_patched(CONFIGS[2], lens, deltas, ranks, 41, max_rank=16) == 0
+
+
+def test_on_read_patch_config5_rank32_mixed_ranks_two_head_groups():
+    """GQA 64/8 (two head groups of 4 KV heads): ranks 32 and 16 mixed in one call, kernel specialised for 32."""
+    rng = _rng(42)
+    lens = [[int(x) for x in rng.integers(40, 200, size=6)] for _ in range(2)]
+    deltas = [[int(x) for x in rng.integers(-131072, 131072, size=6)] for _ in range(2)]
+    ranks = [[32, 16, 32, 0, 32, 16], [16, 32, 32, 32, 0, 32]]
+    assert _run_patched(CONFIGS[5], lens, deltas, ranks, 42, max_rank=32) == 0
+
+
+def test_on_read_patch_rank64_default_max_rank_mha():
+    """MHA (config 4 shape, 32 heads): the rank-64 removal patch with the default specialisation (KAM_MAX_RANK)."""
+    assert _run_patched(CONFIGS[4], [[160, 96]], [[-1280, 0]], [[64, 48]], 43) == 0
+
+
+def test_on_read_patch_shared_u_and_canonical_frame():
+    """The paper's per-layer form (one U for all KV heads, R-6) and the CANONICAL frame R(delta)(k + U W) (R-4)."""
+    lens, deltas, ranks = [[200, 64]], [[777, -3]], [[16, 16]]
+    assert _run_patched(CONFIGS[2], lens, deltas, ranks, 44, max_rank=16, shared_u=True) == 0
+    assert _run_patched(CONFIGS[2], lens, deltas, ranks, 45, max_rank=16, frame=reuse.CANONICAL_FRAME) == 0
+
+
+def test_on_read_patch_head_dim_64_and_bulk_copy_path():
+    cfg = CONFIGS[1].scaled(elem_dtype="bf16", factor_dtype="bf16")
+    assert _run_patched(cfg, [[256, 40]], [[17, 4000]], [[16, 16]], 46, max_rank=16) == 0
+    assert _run_patched(CONFIGS[2], [[300, 33]], [[5, 0]], [[16, 16]], 47, max_rank=16, other_pool=True) == 0
+
+
+def test_on_read_patch_equals_materialised_patch():
+    """Patching on read and materialising the same patch with kam_relocate_patch give the same readout within the decode
+    tolerance (the materialised one rounds k^, v^ to bf16 once; the on-read one never rounds them)."""
+    cfg = CONFIGS[2]
+    rng = _rng(48)
+    T, P, m = 512, cfg.page_size, 16
+    ch = make_chunk(cfg, rng, n_tokens=T, n_layers=1, rank=m)
+    bt_h = make_block_table(rng, 2 * T // P, 2 * T // P + 2)
+    bt = torch.from_numpy(bt_h).cuda()
+    pool = par.make_pool(cfg, 1, 2 * T // P + 2, torch.bfloat16)
+    ctx = kam.Context(par.layout_of(cfg, 1), pool)
+    ctx.kam_decode_set_max_patch_rank(16)
+    chunk, patch = par.upload_chunk(ch)
+    p_t = 20000
+    ctx.kam_relocate_patch(bt, 0, chunk, p_t, patch, m)              # tokens [0, T): rotated + patched in the pool
+    ctx.kam_relocate_patch(bt, T, chunk, 0, None, 0)                 # tokens [T, 2T): the canonical rows, untouched
+    q = make_query(cfg, rng, 1).cuda()
+    nc = torch.tensor([1], dtype=torch.int32, device="cuda")
+    res = []
+    for on_read in (False, True):
+        out = torch.zeros((1, cfg.n_q_heads, cfg.row_dim), dtype=torch.bfloat16, device="cuda")
+        lse = torch.zeros((1, cfg.n_q_heads), dtype=torch.float32, device="cuda")
+        starts = torch.tensor([[0, T]], dtype=torch.int32, device="cuda")
+        table = (bt[T // P:] if on_read else bt[:T // P]).contiguous().reshape(1, -1)
+        offs = torch.tensor([[p_t if on_read else 0]], dtype=torch.int64, device="cuda")
+        pr = B.patch_refs([[(patch.t[0][0], patch.t[1][0], patch.t[2][0], patch.t[3][0], m)]], "cuda") if on_read else None
+        ctx.kam_paged_decode_merge(q, table, starts, offs, nc, 0, cfg.row_dim ** -0.5, out, lse, patches=pr)
+        torch.cuda.synchronize()
+        res.append((par.to_f64(out)[0], par.to_f64(lse)[0]))
+    check_attention(res[1][0], res[1][1], res[0][0], res[0][1], "on-read vs materialised patch")
+    ctx.close()
+
+
+def test_on_read_patch_malformed_ref_is_ignored_and_counted():
+    lens, deltas, ranks = [[64, 64]], [[0, 9]], [[16, 16]]
+    assert _run_patched(CONFIGS[2], lens, deltas, ranks, 49, max_rank=16, bad=(0, 1, 8)) == 2      # rank 8: not a multiple of 16; the helper calls decode twice
+    assert _run_patched(CONFIGS[2], lens, deltas, ranks, 50, max_rank=16, bad=(0, 0, 32)) == 2     # above the specialisation
