@@ -322,8 +322,10 @@ typedef CUresult (*PFN_tmapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuin
 void build_pool_tensor_maps(kam_ctx* c) {
   const kam_layout& L = c->lay;
   if (getenv("KAM_DECODE_NO_TMA")) { c->tmap_why = "disabled by KAM_DECODE_NO_TMA"; return; }
-  if (L.elem_dtype != KAM_BF16 || !L.has_v) { c->tmap_why = "needs a bf16 K/V pool"; return; }
-  if (L.page_size % 16 || (L.row_dim != 64 && L.row_dim != 128)) { c->tmap_why = "needs page_size % 16 == 0 and head_dim 64/128"; return; }
+  if (L.elem_dtype != KAM_BF16) { c->tmap_why = "needs a bf16 pool"; return; }
+  const bool mla = !L.has_v;
+  if (mla && (L.n_kv_heads != 1 || L.row_dim % 64)) { c->tmap_why = "MLA rows must be a multiple of 64 columns"; return; }
+  if (L.page_size % 16 || (!mla && L.row_dim != 64 && L.row_dim != 128)) { c->tmap_why = "needs page_size % 16 == 0 and head_dim 64/128"; return; }
   if (c->pool.num_pages < 1) { c->tmap_why = "empty pool"; return; }
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -333,17 +335,17 @@ void build_pool_tensor_maps(kam_ctx* c) {
   PFN_tmapEncodeTiled encode = reinterpret_cast<PFN_tmapEncodeTiled>(fn);
   std::vector<void*> kp(L.n_layers), vp(L.n_layers);
   if (cudaMemcpy(kp.data(), c->pool.k_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess ||
-      cudaMemcpy(vp.data(), c->pool.v_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess) {
+      (!mla && cudaMemcpy(vp.data(), c->pool.v_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess)) {
     cudaGetLastError(); c->tmap_why = "could not read the pool's layer pointers"; return;
   }
-  const int HG = decode_head_group(L);
+  const int HG = decode_head_group(L);                  // MLA: one "head" of row_dim columns, the whole row is one box
   const cuuint64_t gdim[3] = {64, (cuuint64_t)c->pool.num_pages * L.page_size, (cuuint64_t)L.n_kv_heads * L.row_dim / 64};
   const cuuint64_t gstride[2] = {(cuuint64_t)L.n_kv_heads * L.row_dim * 2, 128};
   const cuuint32_t box[3] = {64, 16, (cuuint32_t)(HG * L.row_dim / 64)};
   const cuuint32_t estr[3] = {1, 1, 1};
   std::vector<CUtensorMap> maps((size_t)2 * L.n_layers);
   for (int l = 0; l < L.n_layers; ++l)
-    for (int kv = 0; kv < 2; ++kv) {
+    for (int kv = 0; kv < (mla ? 1 : 2); ++kv) {
       CUresult r = encode(&maps[2 * l + kv], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv ? vp[l] : kp[l], gdim, gstride, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);

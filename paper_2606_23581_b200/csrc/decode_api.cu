@@ -18,7 +18,43 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
   const int variant = (c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers) ? 1 : 0;
   if (c->dec_geom_ok[variant][kt]) { *out = c->dec_geom[variant][kt]; return KAM_OK; }
   if (L.elem_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "decode needs a bf16 pool");
-  if (!L.has_v) return fail(c, KAM_ERR_UNSUPPORTED, "decode over an MLA latent pool is not built yet (SURVEY.md 8(f) f1)");
+  if (!L.has_v) {
+    // absorbed MLA decode: one latent+rope row per token, value = its first v_dim columns (decode_mla_kernel.cu)
+    if (L.n_kv_heads != 1 || L.row_dim != 576 || L.v_dim != 512 || L.rope_off != 512 || L.rope_dim != 64)
+      return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode is built for rows of 512 latent + 64 rope columns with v_dim 512");
+    if (!variant) return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode needs the context's own pool with page_size %% 16 == 0 (%s)", c->tmap_why.c_str());
+    DecodeGeom g{};
+    g.mla = 1;
+    g.Hq = L.n_q_heads; g.H = 1; g.D = 576; g.Dv = 512; g.P = L.page_size;
+    g.G = std::min(L.n_q_heads, kMlaHeads);
+    g.P_shift = -1;
+    for (int s = 0; s < 31; ++s) if ((1 << s) == g.P) g.P_shift = s;
+    g.HG = 1; g.n_hg = (L.n_q_heads + kMlaHeads - 1) / kMlaHeads; g.R = g.G; g.NT = 2;
+    g.rope_off = L.rope_off; g.d_r = L.rope_dim; g.rope_style = L.rope_style;
+    g.row_bytes = g.slice_bytes = 576 * 2; g.use_tma = 1; g.ncb = 9;
+    g.kv_bytes = 2048 * g.ncb; g.box_bytes = g.kv_bytes; g.KT = kt;
+    if (kt > 0) {
+      g.u_off = g.kv_bytes;
+      g.su_row = kt * 16 * 2 + 16;
+      g.box_bytes = (int)align_up_sz((size_t)g.kv_bytes + (size_t)kDecTile * g.su_row, 1024);
+    }
+    g.off_hdr = 128; g.off_xch = 1024; g.off_box0 = 1024 + 2 * kMlaWarps * 256 * 4;
+    int want = c->dec_ctas_per_sm > 0 ? std::min(c->dec_ctas_per_sm, 2) : 2;
+    for (; want >= 1; --want) {
+      const int budget = 227 * 1024 / want - 1024 - g.off_box0;
+      int nb = std::min(8, budget / g.box_bytes);
+      if (c->dec_boxes > 0) nb = std::min(nb, c->dec_boxes);
+      if (nb < 2) continue;
+      g.n_boxes = nb;
+      g.smem_bytes = g.off_box0 + nb * g.box_bytes;
+      if (mla_decode_occupancy(g) >= want) break;
+    }
+    if (want < 1) return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode tile does not fit shared memory");
+    g.n_ctas = c->sm_count * want;
+    c->dec_geom[variant][kt] = g; c->dec_geom_ok[variant][kt] = true;
+    *out = g;
+    return KAM_OK;
+  }
   if (L.row_dim != 64 && L.row_dim != 128) return fail(c, KAM_ERR_UNSUPPORTED, "decode supports head_dim 64 or 128");
   const int G = L.n_q_heads / L.n_kv_heads;
   if (G > 16) return fail(c, KAM_ERR_UNSUPPORTED, "decode supports up to 16 query heads per KV head");
@@ -149,7 +185,8 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
   csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = patches ? 1 : 0;
   launch_decode_plan(g, p.plan, csr, st);
-  launch_decode(g, p, false, st);                                 // reads the plan just written: plain stream order
+  if (g.mla) launch_mla_decode(g, p, false, st);
+  else launch_decode(g, p, false, st);                            // reads the plan just written: plain stream order
   launch_decode_merge(g, p, c->use_pdl, st);
   c->kernels_launched += 3;
   cudaError_t e = cudaGetLastError();
@@ -248,7 +285,8 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.err = c->d_err;
   // with a plan from an earlier call the decode prologue may overlap whatever precedes it on the stream (it only reads the plan)
-  launch_decode(g, p, cached && c->use_pdl, st);
+  if (g.mla) launch_mla_decode(g, p, cached && c->use_pdl, st);
+  else launch_decode(g, p, cached && c->use_pdl, st);
   launch_decode_merge(g, p, c->use_pdl, st);
   c->kernels_launched += 2;
   cudaError_t e = cudaGetLastError();
@@ -267,7 +305,8 @@ kam_status kam_paged_decode_merge_host(kam_ctx* c, const void* q_host, const kam
   if (batch == 0) return KAM_OK;
   if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
   const kam_layout& L = c->lay;
-  const size_t qb = (size_t)batch * L.n_q_heads * L.row_dim * 2, ob = qb, lb = (size_t)batch * L.n_q_heads * 4;
+  const size_t qb = (size_t)batch * L.n_q_heads * L.row_dim * 2, lb = (size_t)batch * L.n_q_heads * 4;
+  const size_t ob = L.has_v ? qb : (size_t)batch * L.n_q_heads * L.v_dim * 2;
   const size_t o_off = (qb + 255) & ~size_t(255), l_off = (o_off + ob + 255) & ~size_t(255);
   kam_status s = grow_device(c, &c->d_hstage2, &c->hstage2_cap, l_off + lb, "cudaMalloc(decode host staging)");
   if (s != KAM_OK) return s;

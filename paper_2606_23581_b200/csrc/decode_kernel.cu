@@ -24,6 +24,7 @@
 #include <math_constants.h>
 
 #include "common.cuh"
+#include "decode_common.cuh"
 #include "internal.h"
 
 namespace kam {
@@ -191,52 +192,6 @@ void launch_decode_plan(const DecodeGeom& g, const DecodePlan& plan, const Decod
 }
 
 // ---------------------------------------------------------------------------------------------------- decode
-namespace {
-enum : int { HDR_FIRST = 1, HDR_LAST = 2, HDR_PARTIAL = 4 };
-
-__device__ __forceinline__ float ex2(float x) {                  // 2^x, ex2(-inf) = 0
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {   // 8x8 b16 transpose across the warp
-  uint32_t d;
-  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
-  return d;
-}
-__device__ __forceinline__ float col_max(float v) {              // over the 8 lanes that share lane % 4
-  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 4));
-  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 8));
-  return fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 16));
-}
-__device__ __forceinline__ float col_sum(float v) {
-  v += __shfl_xor_sync(0xffffffffu, v, 4);
-  v += __shfl_xor_sync(0xffffffffu, v, 8);
-  return v + __shfl_xor_sync(0xffffffffu, v, 16);
-}
-__device__ __forceinline__ uint32_t ldg_u32(const void* p) { return __ldg(reinterpret_cast<const unsigned int*>(p)); }
-__device__ __forceinline__ uint32_t ldg_u16(const void* p) { return __ldg(reinterpret_cast<const unsigned short*>(p)); }
-
-// On-read patch of one segment: rank of the chunk's kam_patch_ref if the record is well formed and the kernel is specialised
-// for it (KT rank tiles), else 0 (no patch; malformed records are counted once per segment by the producer warp).
-struct SegPatch { const char* Uk; const char* Uv; const __nv_bfloat16* Wk; const __nv_bfloat16* Wv; long long uts, uhs; int rank, frame; };
-__device__ __forceinline__ SegPatch seg_patch(const kam_patch_ref* refs, int idx, int KT, bool* malformed) {
-  SegPatch sp{};
-  *malformed = false;
-  if (!refs || idx < 0) return sp;
-  const kam_patch_ref r = refs[idx];
-  if (r.rank == 0 || (!r.Uk && !r.Wk && !r.Uv && !r.Wv)) return sp;
-  const bool ok = r.rank > 0 && r.rank % 16 == 0 && r.rank <= KT * 16 && r.Uk && r.Wk && r.Uv && r.Wv &&
-                  (r.u_token_stride & 7) == 0 && (r.u_head_stride & 7) == 0 && (r.u_head_stride == 0 || r.u_head_stride >= r.rank) &&
-                  ((reinterpret_cast<uintptr_t>(r.Uk) | reinterpret_cast<uintptr_t>(r.Uv) | reinterpret_cast<uintptr_t>(r.Wk) |
-                    reinterpret_cast<uintptr_t>(r.Wv)) & 15) == 0;
-  if (!ok) { *malformed = true; return sp; }
-  sp.Uk = static_cast<const char*>(r.Uk); sp.Uv = static_cast<const char*>(r.Uv);
-  sp.Wk = static_cast<const __nv_bfloat16*>(r.Wk); sp.Wv = static_cast<const __nv_bfloat16*>(r.Wv);
-  sp.uts = r.u_token_stride; sp.uhs = r.u_head_stride; sp.rank = r.rank; sp.frame = r.frame;
-  return sp;
-}
-}  // namespace
 
 // KS = D / 16 (k-steps of QK^T; D = Dv).  NT = ceil(G / 8) query-head tiles.  TMA: pool pages arrive as swizzled boxes.
 //
@@ -288,7 +243,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
       [[maybe_unused]] uint32_t u_row_bytes = 0, u_run_bytes = 0; [[maybe_unused]] int u_runs = 0;
       if constexpr (KT > 0) {
         bool bad;
-        sp = seg_patch(p.patches, S.patch, KT, &bad);
+        sp = seg_patch(p.patches, S.patch, KT, true, &bad);
         if (bad && lane == 0 && S.tile0 * kDecTile <= S.tok_lo && S.hg == 0) atomicAdd(p.err, 1);   // once per chunk
         if (sp.rank) {
           // a token's U run of this head group: HG heads x rank (one copy if the heads are contiguous), or rank (shared U)
@@ -461,7 +416,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
         // ---- on-read patch of this segment: (W_k q)^T [rank][G] by MMA (A = W_k rows from global, B = the q fragments).
         // TARGET frame (Eq. 1: rotate, then add) contracts W_k with the UNrotated q; CANONICAL with the rotated one.
         bool bad;
-        const SegPatch sp = seg_patch(p.patches, S.patch, KT, &bad);
+        const SegPatch sp = seg_patch(p.patches, S.patch, KT, true, &bad);
         kt_seg = sp.rank >> 4;
         if (kt_seg) {
           const __nv_bfloat16* Wk = sp.Wk + static_cast<size_t>(head) * sp.rank * D;
@@ -729,18 +684,7 @@ int decode_occupancy(const DecodeGeom& g) {
   return n;
 }
 
-namespace {
-template <typename K, typename... A>
-void launch_ex(K kern, int grid, int block, int smem, bool pdl, cudaStream_t st, const A&... args) {
-  cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, kern, args...);
-}
-}  // namespace
+
 
 void launch_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st) {
   decode_dispatch(g, [&](auto kern) { launch_ex(kern, g.n_ctas, (g.HG + 1) * 32, g.smem_bytes, pdl, st, g, p); });
@@ -782,8 +726,13 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
       for (int c = 0; c < CPL; ++c) o[u][c] = 0.f;
       if (s < s1) {
         ls[u] = pl[static_cast<size_t>(s) * g.R];
-        if constexpr (CPL == 4) { const float4 v = *reinterpret_cast<const float4*>(po + s * so); o[u][0] = v.x; o[u][1] = v.y; o[u][2] = v.z; o[u][3] = v.w; }
-        else { const float2 v = *reinterpret_cast<const float2*>(po + s * so); o[u][0] = v.x; o[u][1] = v.y; }
+        if constexpr (CPL % 4 == 0) {
+#pragma unroll
+          for (int c4 = 0; c4 < CPL / 4; ++c4) {
+            const float4 v = *reinterpret_cast<const float4*>(po + s * so + c4 * 4);
+            o[u][c4 * 4] = v.x; o[u][c4 * 4 + 1] = v.y; o[u][c4 * 4 + 2] = v.z; o[u][c4 * 4 + 3] = v.w;
+          }
+        } else { const float2 v = *reinterpret_cast<const float2*>(po + s * so); o[u][0] = v.x; o[u][1] = v.y; }
       }
     }
 #pragma unroll
@@ -806,26 +755,30 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
 #pragma unroll
   for (int w = 0; w < kMergeWarps; ++w) M = fmaxf(M, sm_m[w]);
   __nv_bfloat16* out = static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(bh) * g.Dv;
-  const int c = threadIdx.x;
   if (M == -CUDART_INF_F) {                       // no tokens at all: out = 0, lse = -inf, no NaN
-    if (c < g.Dv) out[c] = __float2bfloat16_rn(0.f);
-    if (c == 0) p.lse[bh] = -CUDART_INF_F;
+    for (int c = threadIdx.x; c < g.Dv; c += kMergeWarps * 32) out[c] = __float2bfloat16_rn(0.f);
+    if (threadIdx.x == 0) p.lse[bh] = -CUDART_INF_F;
     return;
   }
-  float tot = 0.f, v = 0.f;
+  float tot = 0.f, ew[kMergeWarps];
 #pragma unroll
   for (int w = 0; w < kMergeWarps; ++w) {
-    const float e = sm_m[w] == -CUDART_INF_F ? 0.f : __expf(sm_m[w] - M);
-    tot = fmaf(sm_l[w], e, tot);
-    if (c < g.Dv) v = fmaf(sm_acc[w][c], e, v);
+    ew[w] = sm_m[w] == -CUDART_INF_F ? 0.f : __expf(sm_m[w] - M);
+    tot = fmaf(sm_l[w], ew[w], tot);
   }
-  if (c < g.Dv) out[c] = __float2bfloat16_rn(v / tot);
-  if (c == 0) p.lse[bh] = M + logf(tot);
+  for (int c = threadIdx.x; c < g.Dv; c += kMergeWarps * 32) {
+    float v = 0.f;
+#pragma unroll
+    for (int w = 0; w < kMergeWarps; ++w) v = fmaf(sm_acc[w][c], ew[w], v);
+    out[c] = __float2bfloat16_rn(v / tot);
+  }
+  if (threadIdx.x == 0) p.lse[bh] = M + logf(tot);
 }
 
 void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st) {
-  if (g.Dv == 128) launch_ex(kam_lse_merge_kernel<4>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
-  else             launch_ex(kam_lse_merge_kernel<2>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
+  if (g.Dv == 512)      launch_ex(kam_lse_merge_kernel<16>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
+  else if (g.Dv == 128) launch_ex(kam_lse_merge_kernel<4>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
+  else                  launch_ex(kam_lse_merge_kernel<2>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
 }
 
 }  // namespace kam
