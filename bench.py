@@ -297,6 +297,118 @@ def run_reference(args):
         "e2e": {"value": value, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
+
+# ------------------------------------------------------------------------------------------------------- extras (outside the step)
+def _time_ms(torch, fn, reps):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    fn(); torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record(); torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def extras(wl, device, peak):
+    """Measured after the timed region, NOT part of the step or of `value`: the paper's "rank-invariant in latency" claim
+     as a rank sweep of the relocate kernel on config 2's shape, the rank-m patch applied ON READ inside the decode
+    (row A8's second form), and the MLA instantiation (config 3's shape): relocate+patch and absorbed decode.  Every
+    figure is algorithmic bytes / device time, as a fraction of the measured HBM peak."""
+    import torch
+    kam, B, cfg = wl.kam, wl.B, wl.cfg
+    from synth import CONFIGS, randn_device
+    L, H, D, P, T, n = cfg.n_layers, cfg.n_kv_heads, cfg.row_dim, cfg.page_size, cfg.chunk_tokens, wl.n_chunks
+    out, seed = {}, [987654]
+
+    def rnd(shape, std=1.0):
+        seed[0] += 1
+        return randn_device(shape, seed[0], std, torch.bfloat16, device)
+
+    # ---- T11: rank sweep, one launch of 8 chunks x 28 layers per rank; sources/destinations rotate over 4 request slots
+    sweep = {}
+    for m in (0, 16, 32, 64):
+        pats = None
+        if m:
+            pats = [kam.Patch([rnd((T, H, m)) for _ in range(L)], [rnd((H, m, D), cfg.w_std) for _ in range(L)],
+                              [rnd((T, H, m)) for _ in range(L)], [rnd((H, m, D), cfg.w_std) for _ in range(L)]) for _ in range(n)]
+        it = [0]
+
+        def launch():
+            r, cs = it[0] % bench_slots, wl.sets[it[0] % N_SETS]
+            it[0] += 1
+            wl.ctx_a.kam_relocate_patch_batch([(wl.bt_a, (r * n + c) * T, cs[c][0], 1000 + 37 * c + it[0], pats[c] if pats else None, m) for c in range(n)])
+        bench_slots = N_REQ
+        ms = _time_ms(torch, launch, 10)
+        nbytes = n * L * algorithmic_bytes_relocate(T, H, D, m, P) if m else n * L * (2 * 2 * T * H * D * 2 + 4 * (T // P))
+        sweep["m=%d" % m] = {"ms": ms, "us_per_1024tok_chunk": 1e3 * ms / n, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
+        del pats
+    out["relocate_rank_sweep"] = sweep
+
+    # ---- A8, second form: decode with the rank-16 patch applied on read (stateless call: plan + decode + merge per layer)
+    Ld = 4
+    ppr = n * T // P
+    npages = N_REQ * ppr
+    bt = torch.randperm(npages, device=device, dtype=torch.int32).reshape(N_REQ, ppr)
+    starts = torch.arange(0, (n + 1) * T, T, dtype=torch.int32, device=device).repeat(N_REQ, 1)
+    offs = torch.full((N_REQ, n), 4321, dtype=torch.int64, device=device)
+    nc = torch.full((N_REQ,), n, dtype=torch.int32, device=device)
+    m = cfg.rank
+    wl.ctx_a.kam_decode_set_max_patch_rank(16)
+    refs = [B.patch_refs([[(rnd((T, H, m)), rnd((H, m, D), cfg.w_std), rnd((T, H, m)), rnd((H, m, D), cfg.w_std), m) for _ in range(n)]
+                          for _ in range(N_REQ)], device) for _ in range(Ld)]
+    for name, pr in (("decode_stateless_no_patch", None), ("decode_stateless_on_read_patch_m16", refs)):
+        it = [0]
+
+        def launch():
+            l = it[0] % Ld
+            it[0] += 1
+            wl.ctx_a.kam_paged_decode_merge(wl.q, bt, starts, offs, nc, l, wl.sm_scale, wl.out, wl.lse, patches=pr[l] if pr else None)
+        ms = _time_ms(torch, launch, 12)
+        nbytes = N_REQ * n * T * H * (2 * D + (2 * m if pr else 0)) * 2
+        out[name] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak,
+                     "bytes": "K + V" + (" + U_k + U_v" if pr else "") + " once; on-read rotation by a pending offset in both"}
+    del refs
+
+    # ---- MLA (config 3 shape): relocate+patch of 4 chunks x 27 layers in one launch; absorbed decode, batch 64 x 8192 tokens
+    c3 = CONFIGS[3]
+    L3, D3, P3, T3, m3 = c3.n_layers, c3.row_dim, c3.page_size, c3.chunk_tokens, c3.rank
+    lay3 = kam.make_layout(B.KAM_MLA, L3, c3.n_q_heads, 1, D3, c3.rope_off, c3.rope_dim, False, P3, c3.theta, v_dim=c3.v_dim)
+    nb3, nch3 = 64, 8
+    np3 = nb3 * nch3 * T3 // P3
+    pool3 = kam.Pool([rnd((np3, P3, 1, D3)) for _ in range(L3)], None)
+    ctx3 = kam.Context(lay3, pool3)
+    ch3 = [(kam.Chunk([rnd((T3, 1, D3)) for _ in range(L3)], None), kam.Patch([rnd((T3, 1, m3)) for _ in range(L3)], [rnd((1, m3, D3), c3.w_std) for _ in range(L3)]))
+           for _ in range(8)]
+    bt3 = torch.randperm(np3, device=device, dtype=torch.int32)
+    it = [0]
+
+    def launch():
+        i = it[0]
+        it[0] += 1
+        ctx3.kam_relocate_patch_batch([(bt3, ((4 * i + c) % (nb3 * nch3)) * T3, ch3[(4 * i + c) % 8][0], 1024 * c, ch3[(4 * i + c) % 8][1], m3) for c in range(4)])
+    ms = _time_ms(torch, launch, 10)
+    nbytes = 4 * L3 * algorithmic_bytes_relocate(T3, 1, D3, m3, P3, has_v=False)
+    out["mla_relocate_patch"] = {"ms": ms, "us_per_1024tok_chunk": 1e3 * ms / 4, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
+    q3 = rnd((nb3, c3.n_q_heads, D3))
+    o3 = torch.zeros((nb3, c3.n_q_heads, c3.v_dim), dtype=torch.bfloat16, device=device)
+    l3 = torch.zeros((nb3, c3.n_q_heads), dtype=torch.float32, device=device)
+    st3 = torch.arange(0, (nch3 + 1) * T3, T3, dtype=torch.int32, device=device).repeat(nb3, 1)
+    nc3 = torch.full((nb3,), nch3, dtype=torch.int32, device=device)
+    bt3b = bt3.reshape(nb3, -1)
+    it = [0]
+
+    def launch():
+        l = it[0] % L3
+        it[0] += 1
+        ctx3.kam_paged_decode_merge(q3, bt3b, st3, None, nc3, l, 192 ** -0.5, o3, l3)
+    ms = _time_ms(torch, launch, 27)
+    nbytes = nb3 * nch3 * T3 * D3 * 2
+    out["mla_decode_absorbed"] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak,
+                                  "bytes": "every latent+rope row once (it is both key and value)", "batch": nb3, "tokens": nch3 * T3,
+                                  "tflops": nb3 * nch3 * T3 * c3.n_q_heads * (D3 + c3.v_dim) * 2 / ms / 1e9}
+    ctx3.close()
+    return out
+
 # ------------------------------------------------------------------------------------------------------- main
 def rank_requests(rank, world, per_gpu=N_REQ):
     """Global request ids rank `rank` owns: the path partitions by request with no exchange; per-GPU
@@ -335,6 +447,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the measurements outside the step (rank sweep, on-read patch, MLA)")
     ap.add_argument("--profile-step", action="store_true",
                     help="bracket the first timed step with cudaProfilerStart/Stop (for `ncu --profile-from-start off`)")
     ap.add_argument("--no-graph", action="store_true", help="launch the per-layer decode calls eagerly instead of replaying a CUDA graph")
@@ -436,6 +549,10 @@ def main():
                "sample": "relocate+patch of %d chunks x 28 layers of config 2 (1.5 steps' worth; a step has 8 chunks), "
                          "oracle/reuse.py in numpy fp64" % CPU_SAMPLE_CHUNKS}
 
+    ex = None
+    if rank == 0 and world == 1 and not args.no_extras and not args.profile_step:
+        ex = extras(wl, device, peak)
+
     if rank == 0:
         out = {
             "metric": "relocate+patch GB/s", "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -453,6 +570,7 @@ def main():
             "decode_note": "attention only: batch / (per-layer attention time x 28 layers); projections and MLP are not part of the method",
             "step_gbs": sum_over_ranks(wl.bytes_a + wl.bytes_b + wl.bytes_c, world) / (total_ms / args.steps * 1e-3) / 1e9 if world == 1 else None,
             "roofline": roofline, "roofline_all": kernels, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "extras_outside_the_step": ex,
         }
         print(json.dumps(out))
     if world > 1:
