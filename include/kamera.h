@@ -217,6 +217,21 @@ kam_status kam_paged_decode_merge(kam_ctx *ctx, const void *q, const kam_pool *p
                                   int32_t max_pages, const int32_t *chunk_starts, const int64_t *chunk_offsets,
                                   const int32_t *n_chunks, int32_t max_chunks, const kam_patch_ref *patches,
                                   int32_t layer, int32_t batch, float sm_scale, void *out, float *lse, void *stream);
+/* ---- chunk-parallel decode across GPUs ("the log-sum-exp state merge already used by ... ring/star
+ * attention").  When a request's chunks are spread over several GPUs, each rank runs kam_paged_decode_state over the
+ * chunks IT holds - same arguments as kam_paged_decode_merge, but the result is the softmax STATE in fp32:
+ * o_state [batch][n_q_heads][Dv] (normalised readout over this rank's chunks), lse_state [batch][n_q_heads] (-inf if the
+ * rank holds none of the request's tokens).  The states of all ranks are exchanged (one all-gather of (Dv + 1) floats per
+ * query head, or peer-memory pointers) and kam_lse_merge_states applies the same merge over them in the fixed order
+ * 0 .. n_parts-1:   lse = ln sum_p e^{lse_p},  out = sum_p e^{lse_p - lse} o_p   -> out bf16 [batch][n_q_heads][Dv], lse f32.
+ * o_states / lse_states: HOST arrays [n_parts] of DEVICE pointers (they may point into peer GPUs' memory).
+ * n_parts <= 16.  Errors: INVALID_ARG, CUDA. */
+kam_status kam_paged_decode_state(kam_ctx *ctx, const void *q, const kam_pool *pool, const int32_t *block_tables,
+                                  int32_t max_pages, const int32_t *chunk_starts, const int64_t *chunk_offsets,
+                                  const int32_t *n_chunks, int32_t max_chunks, const kam_patch_ref *patches,
+                                  int32_t layer, int32_t batch, float sm_scale, float *o_state, float *lse_state, void *stream);
+kam_status kam_lse_merge_states(kam_ctx *ctx, int32_t n_parts, const float *const *o_states, const float *const *lse_states,
+                                int32_t batch, void *out, float *lse, void *stream);
 /* Same, over the context's own windows: request ids req_ids[0..batch) (host).  Pending lazy deltas are applied on read.
  * The work split of a step (which 16-token tiles each persistent CTA streams, the per-chunk cos/sin tables) depends on
  * the windows only, not on the layer: kam_window_plan builds it (one small H2D copy + one kernel); kam_window_decode

@@ -81,6 +81,9 @@ SIGNATURES = {
     "kam_paged_decode_merge": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
                                      vp, vp, vp]),
     "kam_decode_set_max_patch_rank": (i32, [vp, i32]),
+    "kam_paged_decode_state": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
+                                     vp, vp, vp]),
+    "kam_lse_merge_states": (i32, [vp, i32, C.POINTER(vp), C.POINTER(vp), i32, vp, vp, vp]),
     "kam_window_plan": (i32, [vp, C.POINTER(i32), i32, vp]),
     "kam_window_decode": (i32, [vp, vp, C.POINTER(i32), i32, i32, C.c_float, vp, vp, vp]),
     "kam_paged_decode_merge_host": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32,
@@ -278,6 +281,23 @@ class Context:
                                             max_pages, _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks),
                                             max_chunks, _ptr(patches), int(layer), batch, float(sm_scale), _ptr(out),
                                             _ptr(lse), _stream_ptr(stream)), self.h)
+
+    def kam_paged_decode_state(self, q, block_tables, chunk_starts, chunk_offsets, n_chunks, layer, sm_scale, o_state,
+                               lse_state, patches=None, pool=None, stream=None):
+        batch, max_pages = block_tables.shape
+        max_chunks = chunk_starts.shape[1] - 1
+        _check(lib().kam_paged_decode_state(self.h, _ptr(q), C.byref(pool.c) if pool else None, _ptr(block_tables),
+                                            max_pages, _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks),
+                                            max_chunks, _ptr(patches), int(layer), batch, float(sm_scale),
+                                            _ptr(o_state), _ptr(lse_state), _stream_ptr(stream)), self.h)
+
+    def kam_lse_merge_states(self, o_states, lse_states, batch, out, lse, stream=None):
+        """o_states / lse_states: lists of device tensors (one per part), or data pointers (peer memory)."""
+        ptr = lambda t: t.data_ptr() if hasattr(t, "data_ptr") else int(t)
+        n = len(o_states)
+        oa = (vp * n)(*[ptr(t) for t in o_states])
+        la = (vp * n)(*[ptr(t) for t in lse_states])
+        _check(lib().kam_lse_merge_states(self.h, n, oa, la, int(batch), _ptr(out), _ptr(lse), _stream_ptr(stream)), self.h)
 
     def kam_decode_set_max_patch_rank(self, max_rank):
         _check(lib().kam_decode_set_max_patch_rank(self.h, int(max_rank)), self.h)

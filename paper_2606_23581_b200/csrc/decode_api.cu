@@ -146,12 +146,10 @@ kam_status grow_ws(kam_ctx* c, size_t bytes) {
 
 }  // namespace
 
-extern "C" {
-
-kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables,
-                                  int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
-                                  const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, int32_t layer,
-                                  int32_t batch, float sm_scale, void* out, float* lse, void* stream) {
+static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables,
+                                   int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
+                                   const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, int32_t layer,
+                                   int32_t batch, float sm_scale, void* out, float* lse, bool out_f32, void* stream) {
   if (!c) return KAM_ERR_INVALID_ARG;
   kam_status s = check_pool(c, &pool);
   if (s != KAM_OK) return s;
@@ -179,7 +177,7 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   p.patches = patches; p.err = c->d_err;
   p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
-  p.sm_scale = sm_scale; p.out = out; p.lse = lse;
+  p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.out_f32 = out_f32 ? 1 : 0;
 
   DecodeCsr csr{};
   csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
@@ -193,6 +191,46 @@ kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* poo
   if (e != cudaSuccess) return cuda_fail(c, e, "decode launch");
   return KAM_OK;
 }
+
+extern "C" {
+
+kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables,
+                                  int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
+                                  const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, int32_t layer,
+                                  int32_t batch, float sm_scale, void* out, float* lse, void* stream) {
+  return decode_stateless(c, q, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, patches, layer,
+                          batch, sm_scale, out, lse, false, stream);
+}
+
+kam_status kam_paged_decode_state(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables,
+                                  int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
+                                  const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, int32_t layer,
+                                  int32_t batch, float sm_scale, float* o_state, float* lse_state, void* stream) {
+  return decode_stateless(c, q, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, patches, layer,
+                          batch, sm_scale, o_state, lse_state, true, stream);
+}
+
+kam_status kam_lse_merge_states(kam_ctx* c, int32_t n_parts, const float* const* o_states, const float* const* lse_states,
+                                int32_t batch, void* out, float* lse, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (n_parts < 1 || n_parts > kMaxStateParts) return fail(c, KAM_ERR_INVALID_ARG, "n_parts outside [1, %d]", kMaxStateParts);
+  if (!o_states || !lse_states || !out || !lse || batch < 0) return fail(c, KAM_ERR_INVALID_ARG, "kam_lse_merge_states: bad argument");
+  for (int i = 0; i < n_parts; ++i)
+    if (!o_states[i] || !lse_states[i]) return fail(c, KAM_ERR_INVALID_ARG, "kam_lse_merge_states: part %d is NULL", i);
+  if (batch == 0) return KAM_OK;
+  if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
+  StateMergeParams p{};
+  for (int i = 0; i < n_parts; ++i) { p.o[i] = o_states[i]; p.lse[i] = lse_states[i]; }
+  p.n_parts = n_parts; p.rows = batch * c->lay.n_q_heads; p.Dv = c->lay.has_v ? c->lay.row_dim : c->lay.v_dim;
+  p.out = out; p.lse_out = lse;
+  launch_state_merge(p, static_cast<cudaStream_t>(stream));
+  ++c->kernels_launched;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(c, e, "kam_state_merge_kernel launch");
+  return KAM_OK;
+}
+
+}  // extern "C"
 
 // The plan (segments, first slots, cos/sin tables) depends only on the windows, not on the layer or the query: it is
 // rebuilt when a window changed (epoch) or the request list differs, and reused by every layer of the same step.
@@ -251,6 +289,8 @@ static kam_status window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch,
   c->winplan_chunks = N;
   return KAM_OK;
 }
+
+extern "C" {
 
 kam_status kam_decode_set_max_patch_rank(kam_ctx* c, int32_t max_rank) {
   if (!c) return KAM_ERR_INVALID_ARG;

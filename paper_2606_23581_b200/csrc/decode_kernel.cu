@@ -755,8 +755,9 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
 #pragma unroll
   for (int w = 0; w < kMergeWarps; ++w) M = fmaxf(M, sm_m[w]);
   __nv_bfloat16* out = static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(bh) * g.Dv;
+  float* outf = static_cast<float*>(p.out) + static_cast<size_t>(bh) * g.Dv;
   if (M == -CUDART_INF_F) {                       // no tokens at all: out = 0, lse = -inf, no NaN
-    for (int c = threadIdx.x; c < g.Dv; c += kMergeWarps * 32) out[c] = __float2bfloat16_rn(0.f);
+    for (int c = threadIdx.x; c < g.Dv; c += kMergeWarps * 32) { if (p.out_f32) outf[c] = 0.f; else out[c] = __float2bfloat16_rn(0.f); }
     if (threadIdx.x == 0) p.lse[bh] = -CUDART_INF_F;
     return;
   }
@@ -770,9 +771,39 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
     float v = 0.f;
 #pragma unroll
     for (int w = 0; w < kMergeWarps; ++w) v = fmaf(sm_acc[w][c], ew[w], v);
-    out[c] = __float2bfloat16_rn(v / tot);
+    if (p.out_f32) outf[c] = v / tot; else out[c] = __float2bfloat16_rn(v / tot);
   }
   if (threadIdx.x == 0) p.lse[bh] = M + logf(tot);
+}
+
+// A9 across ranks (S 8(e), f4): the same state merge over n_parts (o_p, lse_p) pairs, fixed order p = 0, 1, ... (deterministic
+// and identical on every rank).  One CTA per query row; a part whose lse is -inf (a rank that held none of the request's
+// chunks) contributes nothing.
+__global__ void __launch_bounds__(128) kam_state_merge_kernel(const __grid_constant__ StateMergeParams p) {
+  const int row = blockIdx.x;
+  float M = -CUDART_INF_F;
+  for (int i = 0; i < p.n_parts; ++i) M = fmaxf(M, p.lse[i][row]);
+  __nv_bfloat16* out = static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(row) * p.Dv;
+  if (M == -CUDART_INF_F) {
+    for (int c = threadIdx.x; c < p.Dv; c += blockDim.x) out[c] = __float2bfloat16_rn(0.f);
+    if (threadIdx.x == 0) p.lse_out[row] = -CUDART_INF_F;
+    return;
+  }
+  float tot = 0.f;
+  for (int i = 0; i < p.n_parts; ++i) { const float l = p.lse[i][row]; tot += l == -CUDART_INF_F ? 0.f : __expf(l - M); }
+  for (int c = threadIdx.x; c < p.Dv; c += blockDim.x) {
+    float v = 0.f;
+    for (int i = 0; i < p.n_parts; ++i) {
+      const float l = p.lse[i][row];
+      if (l != -CUDART_INF_F) v = fmaf(p.o[i][static_cast<size_t>(row) * p.Dv + c], __expf(l - M), v);
+    }
+    out[c] = __float2bfloat16_rn(v / tot);
+  }
+  if (threadIdx.x == 0) p.lse_out[row] = M + logf(tot);
+}
+
+void launch_state_merge(const StateMergeParams& p, cudaStream_t st) {
+  kam_state_merge_kernel<<<p.rows, 128, 0, st>>>(p);
 }
 
 void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st) {

@@ -165,9 +165,22 @@ struct DecodeParams {
   float* part_o;                 // [max_segs][R][Dv]
   float* part_lse;               // [max_segs][R]
   float sm_scale;
-  void* out;                     // [B][Hq][Dv] bf16
+  void* out;                     // [B][Hq][Dv] bf16 (f32 when out_f32: a softmax STATE for a later cross-rank merge)
   float* lse;                    // [B][Hq]
+  int32_t out_f32;
 };
+
+// merge of n_parts softmax states (o_p f32 [rows][Dv], lse_p f32 [rows]) of the same queries, e.g. one per rank of a
+// chunk-parallel decode; the pointers may be peer memory.
+constexpr int kMaxStateParts = 16;
+struct StateMergeParams {
+  const float* o[kMaxStateParts];
+  const float* lse[kMaxStateParts];
+  int32_t n_parts, rows, Dv;
+  void* out;                     // [rows][Dv] bf16
+  float* lse_out;                // [rows]
+};
+void launch_state_merge(const StateMergeParams& p, cudaStream_t st);
 
 struct DecodeCsr {               // front end of the plan kernel for the stateless call (device metadata)
   const int32_t* chunk_starts;   // [B][max_chunks + 1]

@@ -1,0 +1,140 @@
+"""Chunk-parallel decode: the per-rank softmax states merged by the state merge of P:44.
+
+CPU (gloo, world size 2): the host logic - chunk sharding and the all-gather layout of paper_2606_23581_b200.chunk_parallel -
+with each rank's state computed by the oracle on its own chunks; the merged readout must equal brute-force softmax over all
+chunks.  GPU (one device): the two shards of every request run one after the other through kam_paged_decode_state (no
+kernel waits on another rank), then kam_lse_merge_states; compared with the oracle and with the single-call decode.
+"""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_shard_chunks_covers_every_chunk_once():
+    from paper_2606_23581_b200.chunk_parallel import shard_chunks
+    for n in (0, 1, 5, 32, 33):
+        for world in (1, 2, 3, 8):
+            got = [c for r in range(world) for c in shard_chunks(n, r, world)]
+            assert got == list(range(n))
+            sizes = [len(shard_chunks(n, r, world)) for r in range(world)]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def _gloo_worker(rank, world, port, q_out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+
+    from oracle import attention as att
+    from paper_2606_23581_b200.chunk_parallel import all_gather_states, shard_chunks
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    rng = np.random.Generator(np.random.PCG64(5))                    # same inputs on every rank
+    B, Hq, H, D, n_chunks = 3, 8, 2, 32, 5
+    rope = dict(theta=1e4, rope_off=0, d_r=D)
+    q = rng.standard_normal((B, Hq, D))
+    chunks = [[{"k": rng.standard_normal((int(rng.integers(0, 9)), H, D)), "v": None, "delta": int(rng.integers(-50, 50))}
+               for _ in range(n_chunks)] for _ in range(B)]
+    for row in chunks:
+        for ch in row:
+            ch["v"] = rng.standard_normal(ch["k"].shape)
+    chunks[2] = [dict(ch, k=ch["k"][:0], v=ch["v"][:0]) if i in shard_chunks(n_chunks, 1, world) else ch for i, ch in enumerate(chunks[2])]
+    mine = shard_chunks(n_chunks, rank, world)
+    o = np.zeros((B, Hq, D)); l = np.zeros((B, Hq))
+    for b in range(B):
+        o[b], l[b] = att.attend_chunks_merge(q[b], [chunks[b][c] for c in mine], 0.3, rope)     # this rank's state
+    o_all, l_all = all_gather_states(torch.from_numpy(o).float(), torch.from_numpy(l).float())
+    assert o_all.shape == (world, B, Hq, D) and l_all.shape == (world, B, Hq)
+    assert torch.equal(o_all[rank], torch.from_numpy(o).float()) and torch.equal(l_all[rank], torch.from_numpy(l).float())
+    worst = 0.0
+    for b in range(B):
+        om, lm = att.lse_merge(o_all[:, b].double().numpy(), l_all[:, b].double().numpy())
+        ob, lb = att.attend_bruteforce(q[b], chunks[b], 0.3, rope)
+        worst = max(worst, float(np.abs(om - ob).max()), float(np.abs(lm - lb).max()))
+    q_out.put((rank, worst))
+    dist.destroy_process_group()
+
+
+def test_world_size_2_gloo_gather_and_merge_equals_bruteforce():
+    import torch.multiprocessing as mp
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    ctx = mp.get_context("spawn")
+    q_out = ctx.Queue()
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q_out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q_out.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [r for r, _ in res] == [0, 1]
+    assert all(w < 1e-5 for _, w in res), res                        # states travel as fp32
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg_id,world", [(2, 2), (5, 4), (3, 2)])
+def test_gpu_states_of_virtual_ranks_merge_to_the_full_readout(cfg_id, world):
+    import paper_2606_23581_b200 as kam
+    from oracle import attention as att
+    from paper_2606_23581_b200.chunk_parallel import shard_chunks
+    from synth import CONFIGS, make_block_table, randn_device
+    from tests import parity as par
+    from tests.test_gpu_decode import check_attention
+    cfg = CONFIGS[cfg_id]
+    rng = np.random.Generator(np.random.PCG64(100 + cfg_id))
+    P, D, Hq, H = cfg.page_size, cfg.row_dim, cfg.n_q_heads, cfg.n_kv_heads
+    Dv = D if cfg.has_v else cfg.v_dim
+    B, n_chunks = 3, 7
+    lens = [[int(x) * P for x in rng.integers(1, 6, size=n_chunks)] for _ in range(B)]        # page-aligned chunks: a shard is a page range
+    lens[1][3] = 0
+    deltas = [[int(x) for x in rng.integers(-4000, 4000, size=n_chunks)] for _ in range(B)]
+    max_pages = max(sum(x) for x in lens) // P
+    num_pages = B * max_pages + 2
+    shape = (num_pages, P, H, D)
+    pool = kam.Pool([randn_device(shape, 7, 1.0, torch.bfloat16, "cuda")], [randn_device(shape, 8, 1.0, torch.bfloat16, "cuda")] if cfg.has_v else None)
+    ctx = kam.Context(par.layout_of(cfg, 1), pool)
+    perm = make_block_table(rng, B * max_pages, num_pages).reshape(B, max_pages)
+    q = torch.from_numpy(rng.standard_normal((B, Hq, D), dtype=np.float32)).to(torch.bfloat16).cuda()
+    scale = 0.09
+
+    def tables(chunk_ids):
+        """Block table / CSR of the given chunks only (what a rank holding just those chunks would pass)."""
+        bt = np.zeros((B, max_pages), np.int32); st = np.zeros((B, n_chunks + 1), np.int32); of = np.zeros((B, n_chunks), np.int64)
+        for b in range(B):
+            pg = 0
+            for i, c in enumerate(chunk_ids):
+                first = sum(lens[b][:c]) // P
+                n = lens[b][c] // P
+                bt[b, pg:pg + n] = perm[b, first:first + n]; pg += n
+                st[b, i + 1] = st[b, i] + lens[b][c]; of[b, i] = deltas[b][c]
+            st[b, len(chunk_ids) + 1:] = st[b, len(chunk_ids)]
+        nc = np.full(B, len(chunk_ids), np.int32)
+        return [torch.from_numpy(x).cuda() for x in (bt, st, of, nc)]
+
+    o_parts, l_parts = [], []
+    for r in range(world):
+        bt, st, of, nc = tables(shard_chunks(n_chunks, r, world))
+        o = torch.empty((B, Hq, Dv), dtype=torch.float32, device="cuda"); l = torch.empty((B, Hq), dtype=torch.float32, device="cuda")
+        ctx.kam_paged_decode_state(q, bt, st, of, nc, 0, scale, o, l)
+        o_parts.append(o); l_parts.append(l)
+    out = torch.zeros((B, Hq, Dv), dtype=torch.bfloat16, device="cuda"); lse = torch.zeros((B, Hq), dtype=torch.float32, device="cuda")
+    ctx.kam_lse_merge_states(o_parts, l_parts, B, out, lse)
+    bt, st, of, nc = tables(list(range(n_chunks)))
+    out1 = torch.zeros_like(out); lse1 = torch.zeros_like(lse)
+    ctx.kam_paged_decode_merge(q, bt, st, of, nc, 0, scale, out1, lse1)
+    torch.cuda.synchronize()
+    for b in range(B):
+        chunks, t0 = [], 0
+        for c in range(n_chunks):
+            chunks.append({"k": par.pool_rows(pool.k_layers[0], perm[b], t0, lens[b][c]),
+                           "v": par.pool_rows(pool.v_layers[0], perm[b], t0, lens[b][c]) if cfg.has_v else None, "delta": deltas[b][c]})
+            t0 += lens[b][c]
+        o, l = att.attend_bruteforce(par.to_f64(q[b]), chunks, scale, par.rope_kw(cfg), v_dim=cfg.v_dim or None)
+        check_attention(par.to_f64(out)[b], par.to_f64(lse)[b], o, l, "chunk-parallel request %d" % b)
+        check_attention(par.to_f64(out)[b], par.to_f64(lse)[b], par.to_f64(out1)[b], par.to_f64(lse1)[b], "vs single call %d" % b)
+    ctx.close()
