@@ -171,6 +171,21 @@ kam_status kam_relocate_patch_host(kam_ctx *ctx, const kam_pool *pool, const int
                                    const void *const *Uv_host, const void *const *Wv_host,
                                    int32_t rank, int32_t frame, void *stream);
 
+/* ---- compile side (P:189-193 `form_patch`; Eq. 2) -------------------------------------------------
+ * Forms the rank-m patch of ONE chunk from its conditioned rows:  Delta = KV(B|A) - R(delta) KV(B|0) per layer and KV head,
+ * top-m singular triplets, singular values folded into U (R-15):  U_out[l] [n_tokens][n_kv_heads][rank] = U_m S,
+ * W_out[l] [n_kv_heads][rank][row_dim] = V_m^T (both bf16, contiguous), sigma_out [n_layers][n_kv_heads][rank] f32 or NULL.
+ * kv_cond_layers / kv_solo_layers / U_out / W_out: DEVICE arrays [n_layers] of device pointers; rows [n_tokens][H][row_dim]
+ * bf16.  is_key = 1: the solo rows are relocated by delta on their rope band first (TARGET frame, Eq. 1); is_key = 0
+ * (values; or MLA with delta = 0): plain difference.  The conditioned forward that yields KV(B|A) is the caller's.
+ * Method: block subspace iteration on Delta^T Delta with 8 columns of oversampling + Rayleigh-Ritz, n_iter sweeps (0 = 6);
+ * exact for rank(Delta) <= rank + 8, otherwise the subspace error shrinks by (sigma_{m+9}/sigma_m)^2 per sweep.
+ * What is unique - U W, the best rank-m approximation, and sigma - is what tests compare (signs of U, W columns are free).
+ * Errors: INVALID_ARG, UNSUPPORTED (fp32 layouts; row_dim x rank too large for shared memory, e.g. MLA above rank 32), CUDA. */
+kam_status kam_form_patch(kam_ctx *ctx, const void *const *kv_cond_layers, const void *const *kv_solo_layers,
+                          int32_t n_tokens, int64_t delta, int32_t is_key, int32_t rank, int32_t n_iter,
+                          void *const *U_out, void *const *W_out, float *sigma_out, void *stream);
+
 /* ---- the window store as a deque (allocation policy R-13) ------------------------------------------
  * Per request: an ordered list of chunks; logical token order = list order; position of chunk i =
  * window_base + tokens before it.  Pages come from one LIFO free list (first pops give 0,1,2,...; admit pops in

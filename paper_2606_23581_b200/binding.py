@@ -70,6 +70,7 @@ SIGNATURES = {
     "kam_rotate_inplace": (i32, [vp, C.POINTER(kam_pool), vp, i64, i32, i64, vp]),
     "kam_relocate_patch_host": (i32, [vp, C.POINTER(kam_pool), vp, i64, i32, i64, i64, C.POINTER(vp), C.POINTER(vp),
                                       C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), i32, i32, vp]),
+    "kam_form_patch": (i32, [vp, vp, vp, i32, i64, i32, i32, i32, vp, vp, vp, vp]),
     "kam_window_open": (i32, [vp, i32, i64]),
     "kam_window_pin": (i32, [vp, i32, i32]),
     "kam_window_close": (i32, [vp, i32]),
@@ -228,6 +229,18 @@ class Context:
                                              int(dst_token_start), int(n_tokens), int(p_base), int(p_target),
                                              tab(k_host), tab(v_host), tab(Uk_host), tab(Wk_host), tab(Uv_host),
                                              tab(Wv_host), int(rank), int(frame), _stream_ptr(stream)), self.h)
+
+    def kam_form_patch(self, kv_cond_layers, kv_solo_layers, delta, is_key, rank, n_iter=0, sigma=None, stream=None):
+        """kv_*_layers: lists of per-layer device tensors [T, H, D].  Returns (U list [T, H, rank], W list [H, rank, D])."""
+        dev, T = kv_cond_layers[0].device, kv_cond_layers[0].shape[0]
+        H, D = self.layout.n_kv_heads, self.layout.row_dim
+        U = [torch.empty((T, H, rank), dtype=torch.bfloat16, device=dev) for _ in kv_cond_layers]
+        W = [torch.empty((H, rank, D), dtype=torch.bfloat16, device=dev) for _ in kv_cond_layers]
+        tabs = [_ptr_table(x, dev) for x in (kv_cond_layers, kv_solo_layers, U, W)]
+        _check(lib().kam_form_patch(self.h, _ptr(tabs[0]), _ptr(tabs[1]), T, int(delta), int(is_key), int(rank), int(n_iter),
+                                    _ptr(tabs[2]), _ptr(tabs[3]), _ptr(sigma), _stream_ptr(stream)), self.h)
+        torch.cuda.current_stream().synchronize() if stream is None else None      # the pointer tables must outlive the launch
+        return U, W
 
     # ---- window store
     def kam_window_open(self, req, window_base=0):

@@ -458,6 +458,7 @@ kam_status kam_destroy(kam_ctx* c) {
     if (c->d_tmaps) cudaFree(c->d_tmaps);
     if (c->d_inv_freq) cudaFree(c->d_inv_freq);
     if (c->d_err) cudaFree(c->d_err);
+    if (c->d_fp_ws) cudaFree(c->d_fp_ws);
   }
   delete c;
   return KAM_OK;
@@ -674,6 +675,41 @@ kam_status kam_window_export(kam_ctx* c, int32_t req, int32_t* bt_out, int32_t b
   if (starts_out) starts_out[nc] = (int32_t)tok;
   if (n_pages_out) *n_pages_out = n_pages;
   if (n_chunks_out) *n_chunks_out = nc;
+  return KAM_OK;
+}
+
+
+// ---- compile side: form the rank-m patch of one chunk ----------------------------------------------------
+kam_status kam_form_patch(kam_ctx* c, const void* const* kv_cond_layers, const void* const* kv_solo_layers, int32_t n_tokens,
+                          int64_t delta, int32_t is_key, int32_t rank, int32_t n_iter, void* const* U_out, void* const* W_out,
+                          float* sigma_out, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (!kv_cond_layers || !kv_solo_layers || !U_out || !W_out) return fail(c, KAM_ERR_INVALID_ARG, "kam_form_patch: NULL argument");
+  if (n_tokens < 1 || rank < 1 || rank > KAM_MAX_RANK || n_iter < 0 || n_iter > 64) return fail(c, KAM_ERR_INVALID_ARG, "kam_form_patch: bad n_tokens / rank / n_iter");
+  const kam_layout& L = c->lay;
+  if (L.elem_dtype != KAM_BF16 || L.factor_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "kam_form_patch needs bf16 rows and factors");
+  if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
+  FormPatchParams p{};
+  p.cond = kv_cond_layers; p.solo = kv_solo_layers; p.U_out = U_out; p.W_out = W_out; p.sigma_out = sigma_out;
+  p.inv_freq = c->d_inv_freq; p.delta = delta;
+  p.L = L.n_layers; p.H = L.n_kv_heads; p.T = n_tokens; p.D = L.row_dim; p.m = rank;
+  p.b = std::min(rank + 8, std::min(L.row_dim, n_tokens));
+  if (p.b < rank) return fail(c, KAM_ERR_INVALID_ARG, "rank %d exceeds min(row_dim, n_tokens)", rank);
+  p.ldq = p.b | 1;
+  p.n_iter = n_iter ? n_iter : 6;
+  p.rope_off = L.rope_off; p.d_r = L.rope_dim; p.rope_style = L.rope_style; p.rotate = (is_key && L.rope_dim > 0 && delta != 0) ? 1 : 0;
+  const size_t fl = (size_t)2 * p.D * p.ldq + (size_t)16 * p.D + (size_t)16 * p.b + (size_t)2 * p.b * (p.b + 1) + p.b + 8 + p.b;
+  p.smem_bytes = (int)(fl * 4 + 64);
+  if (p.smem_bytes > 227 * 1024) return fail(c, KAM_ERR_UNSUPPORTED, "row_dim %d x rank %d does not fit the subspace block in shared memory", p.D, rank);
+  const size_t dws = (size_t)p.L * p.H * p.T * p.D * 4, bws = (size_t)p.L * p.H * p.T * p.b * 4;
+  kam_status s = grow_device(c, &c->d_fp_ws, &c->fp_ws_cap, dws + bws + 256, "cudaMalloc(form_patch workspace)");
+  if (s != KAM_OK) return s;
+  p.delta_ws = static_cast<float*>(c->d_fp_ws);
+  p.b_ws = reinterpret_cast<float*>(static_cast<char*>(c->d_fp_ws) + ((dws + 255) & ~size_t(255)));
+  launch_form_patch(p, static_cast<cudaStream_t>(stream));
+  c->kernels_launched += 2;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(c, e, "kam_form_patch launch");
   return KAM_OK;
 }
 

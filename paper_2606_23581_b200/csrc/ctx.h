@@ -68,6 +68,8 @@ struct kam_ctx {
   size_t hstage_cap = 0;
   void* d_hstage2 = nullptr;
   size_t hstage2_cap = 0;
+  void* d_fp_ws = nullptr;                     // kam_form_patch: Delta and B workspaces (fp32)
+  size_t fp_ws_cap = 0;
 };
 
 namespace kam {

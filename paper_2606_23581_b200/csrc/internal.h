@@ -208,4 +208,21 @@ constexpr int kMlaHeads = 16;              // query heads per work unit (two 8-w
 int mla_decode_occupancy(const DecodeGeom& g);
 void launch_mla_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 
+// ---------------------------------------------------------------- form_patch (compile side, form_patch.cu)
+struct FormPatchParams {
+  const void* const* cond;       // device array [L] -> KV(B|A) rows [T][H][D] bf16, at the target position
+  const void* const* solo;       // device array [L] -> canonical KV(B|0) rows [T][H][D] bf16
+  void* const* U_out;            // device array [L] -> [T][H][m] bf16  (U_m S)
+  void* const* W_out;            // device array [L] -> [H][m][D] bf16  (V_m^T)
+  float* sigma_out;              // [L][H][m] or nullptr
+  float* delta_ws;               // [L][H][T][D] fp32
+  float* b_ws;                   // [L][H][T][b] fp32
+  const double* inv_freq;        // [d_r / 2]
+  long long delta;               // p_target - p_base
+  int32_t L, H, T, D, m, b, ldq, n_iter;
+  int32_t rope_off, d_r, rope_style, rotate;   // rotate = 0 for V
+  int32_t smem_bytes;
+};
+void launch_form_patch(const FormPatchParams& p, cudaStream_t st);
+
 }  // namespace kam
