@@ -519,7 +519,9 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const float mx = col_max(fmaxf(v[e], v[2 + e]));
-        const float mn = fmaxf(m_run[nt][e], mx);
+        // lazy rescale: the running reference only moves when the tile's max exceeds it by more than 2^8 (p stays <= 256, exact
+        // enough in bf16 / fp32; l and lse are relative to the reference, so the result is unchanged) - O is rarely rescaled
+        const float mn = mx > m_run[nt][e] + 8.f ? mx : m_run[nt][e];
         const float ms = (mn == -CUDART_INF_F) ? 0.f : mn;
         al[nt][e] = ex2(m_run[nt][e] - ms);
         m_run[nt][e] = mn;

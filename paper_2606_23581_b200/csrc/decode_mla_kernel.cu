@@ -256,15 +256,21 @@ kam_mla_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constan
     float sa[2][4], sb[2][4];
 #pragma unroll
     for (int nt = 0; nt < 2; ++nt) { sa[nt][0] = sa[nt][1] = sa[nt][2] = sa[nt][3] = 0.f; sb[nt][0] = sb[nt][1] = sb[nt][2] = sb[nt][3] = 0.f; }
+    {
+      // the asm statements are volatile (ordered as written): fragments are fetched two steps ahead of the MMAs that use them
+      uint32_t a[3][4];
+      ldmatrix_x4(a[0][0], a[0][1], a[0][2], a[0][3], k_addr(bb, step_col(0)));
+      ldmatrix_x4(a[1][0], a[1][1], a[1][2], a[1][3], k_addr(bb, step_col(1)));
 #pragma unroll
-    for (int i = 0; i < kSteps; ++i) {
-      uint32_t a0, a1, a2, a3;
-      ldmatrix_x4(a0, a1, a2, a3, k_addr(bb, step_col(i)));
+      for (int i = 0; i < kSteps; ++i) {
+        if (i + 2 < kSteps) ldmatrix_x4(a[(i + 2) % 3][0], a[(i + 2) % 3][1], a[(i + 2) % 3][2], a[(i + 2) % 3][3], k_addr(bb, step_col(i + 2)));
+        const uint32_t a0 = a[i % 3][0], a1 = a[i % 3][1], a2 = a[i % 3][2], a3 = a[i % 3][3];
 #pragma unroll
-      for (int nt = 0; nt < 2; ++nt) {
-        if (i & 1) mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, qhi[nt][i][0], qhi[nt][i][1]);
-        else       mma_bf16_16816(sa[nt][0], sa[nt][1], sa[nt][2], sa[nt][3], a0, a1, a2, a3, qhi[nt][i][0], qhi[nt][i][1]);
-        if (i == kLatSteps && use_lo) mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, qlo[nt][0], qlo[nt][1]);
+        for (int nt = 0; nt < 2; ++nt) {
+          if (i & 1) mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, qhi[nt][i][0], qhi[nt][i][1]);
+          else       mma_bf16_16816(sa[nt][0], sa[nt][1], sa[nt][2], sa[nt][3], a0, a1, a2, a3, qhi[nt][i][0], qhi[nt][i][1]);
+          if (i == kLatSteps && use_lo) mma_bf16_16816(sb[nt][0], sb[nt][1], sb[nt][2], sb[nt][3], a0, a1, a2, a3, qlo[nt][0], qlo[nt][1]);
+        }
       }
     }
     if constexpr (KT > 0) {
@@ -314,7 +320,9 @@ kam_mla_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constan
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const float mx = col_max(fmaxf(v[e], v[2 + e]));
-        const float mn = fmaxf(m_run[nt][e], mx);
+        // lazy rescale: the running reference only moves when the tile's max exceeds it by more than 2^8 (p stays <= 256, exact
+        // enough in bf16 / fp32; l and lse are relative to the reference, so the result is unchanged) - O is rarely rescaled
+        const float mn = mx > m_run[nt][e] + 8.f ? mx : m_run[nt][e];
         const float ms = (mn == -CUDART_INF_F) ? 0.f : mn;
         al[nt][e] = ex2(m_run[nt][e] - ms);
         m_run[nt][e] = mn;
@@ -357,13 +365,17 @@ kam_mla_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constan
       }
       __syncwarp();
     }
+    {
+      uint32_t a[3][4];
+      ldmatrix_x4_trans(a[0][0], a[0][1], a[0][2], a[0][3], v_addr(bb, warp * 128));
+      ldmatrix_x4_trans(a[1][0], a[1][1], a[1][2], a[1][3], v_addr(bb, warp * 128 + 16));
 #pragma unroll
-    for (int dp = 0; dp < kDvTiles; ++dp) {
-      uint32_t a0, a1, a2, a3;
-      ldmatrix_x4_trans(a0, a1, a2, a3, v_addr(bb, warp * 128 + dp * 16));
+      for (int dp = 0; dp < kDvTiles; ++dp) {
+        if (dp + 2 < kDvTiles) ldmatrix_x4_trans(a[(dp + 2) % 3][0], a[(dp + 2) % 3][1], a[(dp + 2) % 3][2], a[(dp + 2) % 3][3], v_addr(bb, warp * 128 + (dp + 2) * 16));
 #pragma unroll
-      for (int nt = 0; nt < 2; ++nt)
-        mma_bf16_16816(O[nt][dp][0], O[nt][dp][1], O[nt][dp][2], O[nt][dp][3], a0, a1, a2, a3, pb[nt][0], pb[nt][1]);
+        for (int nt = 0; nt < 2; ++nt)
+          mma_bf16_16816(O[nt][dp][0], O[nt][dp][1], O[nt][dp][2], O[nt][dp][3], a[dp % 3][0], a[dp % 3][1], a[dp % 3][2], a[dp % 3][3], pb[nt][0], pb[nt][1]);
+      }
     }
     if constexpr (KT > 0) {
       if (kt_seg) {                                             // z^T[j][head] += U^T P^T (every warp keeps the whole z: it is tiny)
