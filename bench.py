@@ -450,6 +450,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the measurements outside the step (rank sweep, on-read patch, MLA)")
     ap.add_argument("--profile-step", action="store_true",
                     help="bracket the first timed step with cudaProfilerStart/Stop (for `ncu --profile-from-start off`)")
+    ap.add_argument("--profile-extras", action="store_true",
+                    help="bracket the extras leg with cudaProfilerStart/Stop instead of a timed step")
     ap.add_argument("--no-graph", action="store_true", help="launch the per-layer decode calls eagerly instead of replaying a CUDA graph")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -551,7 +553,11 @@ def main():
 
     ex = None
     if rank == 0 and world == 1 and not args.no_extras and not args.profile_step:
+        if args.profile_extras:
+            torch.cuda.profiler.start()
         ex = extras(wl, device, peak)
+        if args.profile_extras:
+            torch.cuda.profiler.stop()
 
     if rank == 0:
         out = {
