@@ -256,23 +256,25 @@ def oracle_sample(n_chunks, n_layers, seed=1):
     f = lambda t: t.to(torch.float64).numpy()
     pool_k = np.zeros((T // P, P, H, D), np.uint16); pool_v = np.zeros_like(pool_k)
     bt = rng.permutation(T // P).astype(np.int32)
-    t0 = time.perf_counter()
+    t0, c0 = time.perf_counter(), time.process_time()
     for ch in chunks:
         p = int(rng.integers(0, cfg.max_pos))
         for l in range(n_layers):
             reuse.relocate_patch_layer(pool_k, pool_v, bt, 0, f(ch["K"][l]), f(ch["V"][l]), p, f(ch["Uk"][l]), f(ch["Wk"][l]),
                                        f(ch["Uv"][l]), f(ch["Wv"][l]), theta=cfg.theta, rope_off=cfg.rope_off, d_r=cfg.rope_dim)
     dt = time.perf_counter() - t0
+    global _ORACLE_CORES
+    _ORACLE_CORES = max(1, int(round((time.process_time() - c0) / dt)))       # threads the oracle actually kept busy
     nbytes = n_chunks * n_layers * algorithmic_bytes_relocate(T, H, D, m, P)
     return nbytes / dt / 1e9, dt
 
 
+_ORACLE_CORES = 1
+
+
 def cpu_threads():
-    try:
-        import torch
-        return int(torch.get_num_threads())
-    except Exception:
-        return os.cpu_count() or 1
+    """Cores the last oracle_sample() actually used: process CPU time / wall time (the numpy fp64 oracle is mostly one thread)."""
+    return _ORACLE_CORES
 
 
 def run_reference(args):
@@ -547,7 +549,7 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         gbs, dt = oracle_sample(CPU_SAMPLE_CHUNKS, L)
-        cpu = {"value": gbs, "unit": "GB/s", "cores": cpu_threads(), "kind": "oracle", "seconds": dt,
+        cpu = {"value": gbs, "unit": "GB/s", "cores": cpu_threads(), "host_cores": os.cpu_count(), "kind": "oracle", "seconds": dt,
                "sample": "relocate+patch of %d chunks x 28 layers of config 2 (1.5 steps' worth; a step has 8 chunks), "
                          "oracle/reuse.py in numpy fp64" % CPU_SAMPLE_CHUNKS}
 
