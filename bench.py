@@ -159,10 +159,12 @@ class Workload:
         self.bytes_c = L * self.bytes_c_layer
         torch.cuda.synchronize()
         # phase C as a CUDA graph: with a valid plan kam_window_decode launches exactly two kernels and nothing else
-        self.graph, self.graph_replays = None, 0
+        self.graph, self.graph_replays, self.launches_per_replay = None, 0, 0
         if use_graph:
             self.ctx_b.kam_window_plan(self.req_ids)
+            k0 = self.ctx_b.kam_get_stats()["kernels_launched"]
             self.decode_layers()                                   # eager once: workspace sized, kernels loaded
+            self.launches_per_replay = self.ctx_b.kam_get_stats()["kernels_launched"] - k0     # what one graph replay launches
             torch.cuda.synchronize()
             self.graph = torch.cuda.CUDAGraph()
             with torch.cuda.graph(self.graph):
@@ -174,9 +176,9 @@ class Workload:
             self.ctx_b.kam_window_decode(self.q, self.req_ids, l, self.sm_scale, self.out, self.lse)
 
     def launches(self):
-        """Kernels launched so far: the contexts' own counters + 2 per layer for every graph replay."""
+        """Kernels launched so far: the contexts' own counters + what every graph replay launches (counted on the eager pass)."""
         return (self.ctx_a.kam_get_stats()["kernels_launched"] + self.ctx_b.kam_get_stats()["kernels_launched"]
-                + self.graph_replays * 2 * self.cfg.n_layers)
+                + self.graph_replays * self.launches_per_replay)
 
     def step(self, i, ev=None):
         cfg, B, T, m = self.cfg, self.B, self.cfg.chunk_tokens, self.cfg.rank
