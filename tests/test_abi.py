@@ -55,6 +55,15 @@ def test_compute_entries_fail_loudly_without_cuda():
     assert st == B.KAM_ERR_INVALID_ARG
     st = kam.lib().kam_rotate_inplace(ctx.h, None, None, 0, 16, 5, None)
     assert st == B.KAM_ERR_INVALID_ARG and b"pool" in kam.lib().kam_last_error(ctx.h)
+    # the newer entries too: valid-looking arguments, but no device -> KAM_ERR_CUDA (never a CPU computation)
+    fake = (B.vp * 1)(0x1000)
+    st = kam.lib().kam_form_patch(ctx.h, C.cast(fake, B.vp), C.cast(fake, B.vp), 16, 0, 1, 16, 0, C.cast(fake, B.vp), C.cast(fake, B.vp), None, None)
+    assert st == B.KAM_ERR_CUDA and b"no CPU fallback" in kam.lib().kam_last_error(ctx.h)
+    st = kam.lib().kam_lse_merge_states(ctx.h, 1, fake, fake, 2, B.vp(0x1000), B.vp(0x1000), None)
+    assert st == B.KAM_ERR_CUDA
+    assert kam.lib().kam_lse_merge_states(ctx.h, 17, fake, fake, 2, B.vp(0x1000), B.vp(0x1000), None) == B.KAM_ERR_INVALID_ARG
+    assert kam.lib().kam_decode_set_max_patch_rank(ctx.h, 48) == B.KAM_ERR_INVALID_ARG
+    assert kam.lib().kam_decode_set_max_patch_rank(ctx.h, 32) == B.KAM_OK
 
 
 def _chunk(n):
