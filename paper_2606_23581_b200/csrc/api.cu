@@ -345,7 +345,16 @@ void build_pool_tensor_maps(kam_ctx* c) {
   const cuuint32_t estr[3] = {1, 1, 1};
   std::vector<CUtensorMap> maps((size_t)2 * L.n_layers);
   for (int l = 0; l < L.n_layers; ++l)
-    for (int kv = 0; kv < (mla ? 1 : 2); ++kv) {
+    for (int kv = 0; kv < 2; ++kv) {
+      // MLA: map 0 = the whole row as one box (mma.sync kernel), map 1 = one 64-column block x 16 tokens (tcgen05 kernel)
+      const cuuint32_t box1[3] = {64, 16, 1};
+      if (mla && kv == 1) {
+        CUresult r1 = encode(&maps[2 * l + 1], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kp[l], gdim, gstride, box1, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r1 != CUDA_SUCCESS) { c->tmap_why = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r1); return; }
+        continue;
+      }
       CUresult r = encode(&maps[2 * l + kv], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv ? vp[l] : kp[l], gdim, gstride, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);

@@ -116,7 +116,7 @@ struct DecodeGeom {
   int32_t KT;                    // on-read patch: 16-wide rank tiles the kernel is specialised for (0: no patch in this call)
   int32_t kv_bytes;              // bytes of the K (or V) rows of a box; box_bytes = kv_bytes + the U tile (KT > 0)
   int32_t u_off, su_row;         // U tile inside a box: [16 tokens][su_row bytes], (su_row / 16) odd
-  int32_t mla;                   // 1: absorbed MLA decode (one latent+rope row per token, value = its first Dv columns)
+  int32_t mla;                   // 1: absorbed MLA decode, mma.sync kernel; 2: tcgen05 kernel (no on-read patch) (one latent+rope row per token, value = its first Dv columns)
   int32_t off_xch;               // MLA: shared-memory offset of the partial-score exchange buffer
 };
 
@@ -206,6 +206,9 @@ void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, bool pdl, c
 constexpr int kMlaWarps = 4;               // compute warps: each owns 1/4 of the contraction and 1/4 of the value columns
 constexpr int kMlaHeads = 16;              // query heads per work unit (two 8-wide MMA n-tiles)
 int mla_decode_occupancy(const DecodeGeom& g);
+// tcgen05 / tensor-memory formulation (decode_mla_tc_kernel.cu): g.mla == 2, one CTA per SM
+int mla_tc_smem_bytes();
+void launch_mla_tc_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 void launch_mla_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 
 // ---------------------------------------------------------------- form_patch (compile side, form_patch.cu)
