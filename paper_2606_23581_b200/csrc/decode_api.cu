@@ -39,7 +39,10 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
       g.su_row = kt * 16 * 2 + 16;
       g.box_bytes = (int)align_up_sz((size_t)g.kv_bytes + (size_t)kDecTile * g.su_row, 1024);
     }
-    if (kt == 0 && !getenv("KAM_MLA_NO_TC")) {                    // tensor-memory kernel: one persistent CTA per SM
+    // tensor-memory kernel, opt-in (KAM_MLA_TC=1): correct, but with only 16 query heads (N = 16) each tcgen05.mma re-reads a
+    // 4 KB A tile from shared memory for 8 cycles of math - measured slower than the mma.sync kernel (decode_mla_tc_kernel.cu)
+    const char* tc_env = getenv("KAM_MLA_TC");
+    if (kt == 0 && tc_env && tc_env[0] == '1') {
       g.mla = 2;
       g.smem_bytes = mla_tc_smem_bytes();
       g.n_ctas = c->sm_count;

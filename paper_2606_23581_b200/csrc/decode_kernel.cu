@@ -230,7 +230,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
     int box = 0; uint32_t phase = 0;
     const char* pk = static_cast<const char*>(p.pool_k_layers[p.layer]);
     const char* pv = static_cast<const char*>(p.pool_v_layers[p.layer]);
-    const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * 256;
+    const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * kTmapLayerBytes;
     const char* tm_v = tm_k + 128;
     DecSeg S_next = p.plan.segs[seg_begin];
     grid_dep_wait();                                            // nothing of the pool is read before the stream's earlier work is done

@@ -53,7 +53,7 @@ kam_mla_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constan
   if (warp == kMlaWarps) {
     // ================================================================ producer warp: slot-map (A1), one box per tile
     int box = 0; uint32_t phase = 0;
-    const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * 256;
+    const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * kTmapLayerBytes;
     DecSeg S_next = p.plan.segs[seg_begin];
     grid_dep_wait();
     for (int seg = seg_begin; seg < seg_end; ++seg) {

@@ -5,15 +5,25 @@
 // mma.sync formulation is bound by its own instruction chain at 61 % of the HBM roofline (profiles/ncu_extras_r01.md).  With
 // the TOKENS as the M = 128 dimension one tile costs 36 + 32 tcgen05.mma of 8 cycles against a 6640-cycle HBM budget.
 //
-//   S^T[128 tokens][16 heads] = K[128 x 576] q~^T        A = the tile (K-major, 128-byte swizzle, straight from TMA), B = q~ in smem
+//   S^T[tokens][16 heads]     = K[tile x 576] q~^T          A = the tile (K-major, 128-byte swizzle, straight from TMA), B = q~ in smem
 //   O^T[512][16 heads]       += V^T[512 x 128] P^T        A = the SAME tile read MN-major (no second copy), B = P^T written by softmax
 // S and O live in tensor memory (16 + 4 x 16 columns).  CTA = 4 softmax warps (thread = token row: tcgen05.ld, exp2, P^T to
 // smem, lazy O rescale, epilogue), 1 TMA producer warp, 1 MMA-issuing warp.  One CTA per SM, persistent over the plan's
-// segments.  The tile arrives as 16-token TMA boxes (a box never straddles a page) into two rings: 5 slots of a PAIR of
-// 64-column blocks (2 x 16 KB: one M = 128 block of V^T) and 2 slots of the rope block (16 KB).  A pair is released by the
+// segments.  A tile is 64 tokens (2.6 tiles fit the rings, so the loads run ahead of the softmax; the M = 128 score MMA simply
+// has 64 don't-care rows).  It arrives as 16-token TMA boxes (a box never straddles a page) into two rings: 10 slots of a PAIR
+// of 64-column blocks (2 x 8 KB: one M = 128 block of V^T) and 3 slots of the rope block (8 KB).  A pair is released by the
 // tcgen05.commit of the PV block that read it.
 //
 // Not covered here (the mma.sync kernel takes those calls): the on-read patch.
+//
+// STATUS (round 1): parity-green (tests/test_gpu_decode_mla.py::test_tcgen05_kernel_matches_the_oracle) but OPT-IN
+// (KAM_MLA_TC=1), because it is slower than the mma.sync kernel on the 16-head shape: 2.5 TB/s with 64-token tiles, 3.2 TB/s
+// with 128-token tiles (first version, git history) against 3.9 TB/s.  ncu: sm__pipe_tc_cycles_active 45 % at 34 % DRAM - the
+// tensor pipe is busy but each M = 128, N = 16, K = 16 instruction takes ~69 cycles, not the 8 of the M*N/256 pacing law: in
+// SS mode it re-reads its 4 KB A operand (128 token rows x 32 B) from shared memory, so with N = 16 the tile is streamed from
+// shared memory twice (QK^T, PV) at ~60 B/cycle for 8 cycles of math per 4 KB.  The formulation pays off from N >= 64 query
+// heads per work unit (DeepSeek-V2/V3: 128 heads), where the same A read feeds 4-8x the math; for 16 heads the next step is
+// the swapped form (heads, padded, as M from tensor memory; tokens as N), which changes the softmax ownership.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
@@ -24,10 +34,10 @@
 namespace kam {
 
 namespace {
-constexpr int kTcTok = 128;                         // tokens per tile = M of the score MMA
+constexpr int kTcTok = 64;                          // tokens per tile (the score MMA is M = 128: its upper 64 rows are don't-care)
 constexpr int kTcGroups = kTcTok / kDecTile;        // 16-token TMA boxes per column block
-constexpr int kTcPairSlots = 5, kTcRopeSlots = 2, kTcHdrs = 4;
-constexpr int kBlkBytes = kTcTok * 128;             // one 64-column block of a tile: 128 rows x 128 B
+constexpr int kTcPairSlots = 10, kTcRopeSlots = 3, kTcHdrs = 8;
+constexpr int kBlkBytes = kTcTok * 128;             // one 64-column block of a tile: 64 rows x 128 B
 constexpr int kPairBytes = 2 * kBlkBytes;
 // shared-memory map (bytes)
 constexpr int kOffBar = 0;                          // mbarriers
@@ -36,13 +46,14 @@ constexpr int kOffHdr = 1024;                       // int4[kTcHdrs]
 constexpr int kOffRed = 1280;                       // float[4][16] cross-warp reductions
 constexpr int kOffQhi = 2048;                       // q~ hi: 9 blocks x [16 heads][128 B]
 constexpr int kOffQlo = kOffQhi + 9 * 2048;         // q~ lo of the rope block
-constexpr int kOffP = kOffQlo + 2048;               // P^T: 2 token halves x [16 heads][128 B]
+constexpr int kOffP = kOffQlo + 2048;               // P^T: [16 heads][64 tokens = 128 B] (+ 2 KB spare)
 constexpr int kOffRope = kOffP + 4096;              // 26624 = 26 x 1024
 constexpr int kOffPair = kOffRope + kTcRopeSlots * kBlkBytes;
-constexpr int kTcSmem = kOffPair + kTcPairSlots * kPairBytes;     // 223232 bytes
+// + one block of padding: the M = 128 score MMA reads 128 rows from a 64-row block (the extra rows only feed S rows nobody uses)
+constexpr int kTcSmem = kOffPair + kTcPairSlots * kPairBytes + kBlkBytes;     // 223232 bytes
 static_assert(kOffRope % 1024 == 0 && kTcSmem <= 227 * 1024, "shared-memory map");
-enum : int { BAR_FULL_PAIR = 0, BAR_EMPTY_PAIR = 5, BAR_FULL_ROPE = 10, BAR_EMPTY_ROPE = 12, BAR_S_FULL = 14, BAR_P_FULL = 15,
-             BAR_O_DONE = 16, BAR_Q_FULL = 17, BAR_HDR = 18, BAR_COUNT = 19 };
+enum : int { BAR_FULL_PAIR = 0, BAR_EMPTY_PAIR = 10, BAR_FULL_ROPE = 20, BAR_EMPTY_ROPE = 23, BAR_S_FULL = 26, BAR_P_FULL = 27,
+             BAR_O_DONE = 28, BAR_Q_FULL = 29, BAR_HDR = 30, BAR_COUNT = 31 };
 constexpr uint32_t kTmemCols = 128;                 // S: columns [0, 16); O block b: columns [32 + 16 b, 48 + 16 b)
 
 // ---- tcgen05 wrappers (PTX as documented in the Blackwell guide / CUTLASS cute/arch/mma_sm100_umma.hpp)
@@ -131,46 +142,58 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
   grid_dep_launch();
 
   if (warp == 4) {
-    // ================================================================ producer: slot-map (A1) + 72 TMA boxes per 128-token tile
-    const char* tm = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * 256 + 128;     // the (64 x 16 x 1) box map
+    // ================================================================ producer: slot-map (A1) + 36 TMA boxes per 64-token tile
+    const char* tm = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * kTmapLayerBytes + 128;   // (64 col x 16 tok x 1)
+    const char* tm_pair = tm + 128;                               // (64 x 64 x 2): a whole pair slot in one copy
+    const char* tm_blk = tm + 256;                                // (64 x 64 x 1): the rope block in one copy
+    const bool big = g.P % kTcTok == 0;                           // a 64-aligned run of 64 tokens of the page list is one page run
     int pair_slot = 0, rope_slot = 0; uint32_t pair_phase = 0, rope_phase = 0; int hdr_i = 0;
     grid_dep_wait();
     for (int seg = seg_begin; seg < seg_end; ++seg) {
       const DecSeg S = p.plan.segs[seg];
       const int32_t* bt = p.block_tables + S.bt_off;
-      for (int t0 = 0; t0 < S.n_tiles; t0 += kTcGroups) {
-        const int ng = min(kTcGroups, S.n_tiles - t0);            // 16-token groups of this tile
+      // tiles are cut at multiples of 64 tokens of the page list, so every inner tile is one page run (first / last may be short)
+      for (int t0 = 0; t0 < S.n_tiles;) {
+        const int gpos = S.tile0 + t0;                            // 16-token index in the page list
+        const int ng = min(kTcGroups - (gpos % kTcGroups), S.n_tiles - t0);
         int slot = 0;                                             // lane i < ng: pool slot of group i
         if (lane < ng) {
-          const int tok = (S.tile0 + t0 + lane) * kDecTile;
+          const int tok = (gpos + lane) * kDecTile;
           const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
           slot = bt[pg] * g.P + (tok - pg * g.P);
         }
-        const int tok0 = (S.tile0 + t0) * kDecTile;
+        const int slot0 = __shfl_sync(0xffffffffu, slot, 0);
+        const bool one = big && ng == kTcGroups;                  // full, aligned tile: 5 copies instead of 36
+        const int tok0 = gpos * kDecTile;
         const int row_lo = max(S.tok_lo - tok0, 0), row_hi = min(S.tok_hi - tok0, ng * kDecTile);
         // rope block first (its slot also publishes the tile header)
         mbar_wait(&bars[BAR_EMPTY_ROPE + rope_slot], rope_phase ^ 1);
         if (lane == 0) {
-          const int flags = (t0 == 0 ? HDR_FIRST : 0) | (t0 + kTcGroups >= S.n_tiles ? HDR_LAST : 0) |
+          const int flags = (t0 == 0 ? HDR_FIRST : 0) | (t0 + ng >= S.n_tiles ? HDR_LAST : 0) |
                             ((row_lo > 0 || row_hi < kTcTok) ? HDR_PARTIAL : 0);
           hdrs[hdr_i] = make_int4(seg, flags, row_lo | (row_hi << 16), ng);
           mbar_arrive_expect_tx(&bars[BAR_FULL_ROPE + rope_slot], static_cast<uint32_t>(ng) * 2048u);
+          if (one) tma_load_3d(smem + kOffRope + rope_slot * kBlkBytes, tm_blk, 0, slot0, 8, &bars[BAR_FULL_ROPE + rope_slot]);
         }
         __syncwarp();
-        if (lane < ng) tma_load_3d(smem + kOffRope + rope_slot * kBlkBytes + lane * 2048, tm, 0, slot, 8, &bars[BAR_FULL_ROPE + rope_slot]);
+        if (!one && lane < ng) tma_load_3d(smem + kOffRope + rope_slot * kBlkBytes + lane * 2048, tm, 0, slot, 8, &bars[BAR_FULL_ROPE + rope_slot]);
         if (++rope_slot == kTcRopeSlots) { rope_slot = 0; rope_phase ^= 1; }
         hdr_i = (hdr_i + 1) % kTcHdrs;
         for (int b = 0; b < 4; ++b) {                             // the four pairs of latent blocks
           mbar_wait(&bars[BAR_EMPTY_PAIR + pair_slot], pair_phase ^ 1);
-          if (lane == 0) mbar_arrive_expect_tx(&bars[BAR_FULL_PAIR + pair_slot], static_cast<uint32_t>(ng) * 4096u);
+          uint8_t* dst0 = smem + kOffPair + pair_slot * kPairBytes;
+          if (lane == 0) {
+            mbar_arrive_expect_tx(&bars[BAR_FULL_PAIR + pair_slot], static_cast<uint32_t>(ng) * 4096u);
+            if (one) tma_load_3d(dst0, tm_pair, 0, slot0, 2 * b, &bars[BAR_FULL_PAIR + pair_slot]);
+          }
           __syncwarp();
-          if (lane < ng) {
-            uint8_t* dst = smem + kOffPair + pair_slot * kPairBytes + lane * 2048;
-            tma_load_3d(dst, tm, 0, slot, 2 * b, &bars[BAR_FULL_PAIR + pair_slot]);
-            tma_load_3d(dst + kBlkBytes, tm, 0, slot, 2 * b + 1, &bars[BAR_FULL_PAIR + pair_slot]);
+          if (!one && lane < ng) {
+            tma_load_3d(dst0 + lane * 2048, tm, 0, slot, 2 * b, &bars[BAR_FULL_PAIR + pair_slot]);
+            tma_load_3d(dst0 + lane * 2048 + kBlkBytes, tm, 0, slot, 2 * b + 1, &bars[BAR_FULL_PAIR + pair_slot]);
           }
           if (++pair_slot == kTcPairSlots) { pair_slot = 0; pair_phase ^= 1; }
         }
+        t0 += ng;
       }
     }
     mbar_wait(&bars[BAR_EMPTY_ROPE + rope_slot], rope_phase ^ 1);
@@ -223,8 +246,8 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
         int ps = my_pair0;
         for (int b = 0; b < 4; ++b) {
           const uint32_t base = sm0 + kOffPair + ps * kPairBytes;
-          for (int j = 0; j < 8; ++j)                             // 16 tokens per k-step: A advances 16 rows, B 32 bytes (second token half: +2048)
-            tc_mma(tmem + 32 + 16 * b, tc_desc(base + j * 2048, kBlkBytes, 1024), tc_desc(sm0 + kOffP + (j >> 2) * 2048 + (j & 3) * 32, 16, 1024),
+          for (int j = 0; j < kTcGroups; ++j)                     // 16 tokens per k-step: A advances 16 rows, B 32 bytes
+            tc_mma(tmem + 32 + 16 * b, tc_desc(base + j * 2048, kBlkBytes, 1024), tc_desc(sm0 + kOffP + j * 32, 16, 1024),
                    idesc_pv, (!first || j > 0) ? 1u : 0u);
           tc_commit(&bars[BAR_EMPTY_PAIR + ps]);                 // the pair returns to the producer when this block's MMAs are done
           if (++ps == kTcPairSlots) ps = 0;
@@ -342,17 +365,17 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
       }
       // ---- P^T[head][token] in bf16 as the B operand of the PV MMA: 2 token halves x [16 heads][128 B], swizzled
       {
-        uint8_t* pbase = smem + kOffP + (tid >> 6) * 2048;
+        uint8_t* pbase = smem + kOffP;
         const int c = tid & 63;
 #pragma unroll
         for (int h = 0; h < 16; ++h) {
           const float ms = m_ref[h] == -CUDART_INF_F ? 0.f : m_ref[h];
           const float pv = ex2(v[h] - ms);
           l_sum[h] += pv;
-          *reinterpret_cast<__nv_bfloat16*>(pbase + sw_off(h, c)) = __float2bfloat16_rn(pv);
+          if (tid < kTcTok) *reinterpret_cast<__nv_bfloat16*>(pbase + sw_off(h, c)) = __float2bfloat16_rn(pv);
         }
       }
-      if ((hdr.y & HDR_PARTIAL) && !valid) {
+      if ((hdr.y & HDR_PARTIAL) && !valid && tid < kTcTok) {
         // this token row is outside the chunk: whatever it holds (a neighbouring chunk, an unwritten page) must not reach O as 0 * NaN
         int ps = pair_slot;
         for (int b = 0; b < 4; ++b) {

@@ -97,6 +97,7 @@ void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocI
 void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
 
 // ---------------------------------------------------------------- decode
+constexpr int kTmapLayerBytes = 4 * 128;   // tensor maps per layer: K | V (MLA: 16-token block) | MLA page pair | MLA page block
 constexpr int kDecTile = 16;               // tokens per pipeline box (one TMA box of K or of V)
 constexpr int kDecMaxHG = 4;               // KV heads (= compute warps) per CTA
 constexpr int kDecPlanThreads = 1024;

@@ -161,3 +161,16 @@ def test_window_decode_over_mla_pool_lazy_slides():
     o, l = att.attend_bruteforce(par.to_f64(q[0]), chunks, scale, par.rope_kw(cfg), v_dim=cfg.v_dim)
     check_attention(par.to_f64(out)[0], par.to_f64(lse)[0], o, l, "MLA window")
     ctx.close()
+
+
+def test_tcgen05_kernel_matches_the_oracle(monkeypatch):
+    """The tensor-memory formulation (csrc/decode_mla_tc_kernel.cu; opt-in with KAM_MLA_TC=1, read when a context first decodes):
+    ragged chunks, partial tiles, pending rotations, more and fewer heads than one tile, both pair layouts."""
+    monkeypatch.setenv("KAM_MLA_TC", "1")
+    _run(CONFIGS[3], [[100, 1024, 37], [1024], [5, 16, 300, 700]], [[0, 3100, -77], [1024], [0, 0, -1024, 2048]], 81)
+    _run(CONFIGS[3], [[1024] * 4, [1024] * 4], [[0, 1024, 2048, 3072], [3072, 0, 1024, 2048]], 82, L=2, layer=1)
+    _run(CONFIGS[3].scaled(n_q_heads=32), [[200, 64]], [[17, 0]], 83)
+    _run(CONFIGS[3].scaled(n_q_heads=8), [[70], [130, 3]], [[-5], [0, 999]], 84)
+    _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 85, style=reuse.INTERLEAVED)
+    _run(CONFIGS[3], [[], [0, 1], [16, 0, 16], [1]], [[], [5, 7], [0, 3, -3], [4000]], 86)
+    _run(CONFIGS[3].scaled(page_size=16), [[100, 500], [77]], [[9, -9], [0]], 87)          # no page-sized boxes: 16-token copies only
