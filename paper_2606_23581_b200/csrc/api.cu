@@ -101,8 +101,10 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
   const int limit = 226 * 1024;
   const int ns_max = c->reloc_stages > 0 ? c->reloc_stages : 3;   // measured on B200: 3 x 37 KB in flight per SM beats 4 and 5
   RelocGeom best{}; bool have = false;
+  const int hg_force = getenv("KAM_RELOC_HG") ? atoi(getenv("KAM_RELOC_HG")) : 0;       // tuning switch
   for (int HG = std::min(g.H, 4); HG >= 1; --HG) {
     if (g.H % HG) continue;
+    if (hg_force > 0 && HG != hg_force) continue;
     const int NB = HG * c->blocks_per_head;
     if (NB > kMaxColBlocks) continue;
     RelocGeom t = g;
@@ -139,7 +141,9 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
       t.smem_bytes = t.off_stage0 + NS * t.stage_bytes;
       if (t.smem_bytes > limit) continue;
       t.load_hint = c->reloc_load_hint;
-      if (NS >= 3) { *out = t; return true; }
+      // three stages, or two big ones (>= 96 KB in flight: measured at rank 64, where W takes 70 KB: 2 x 54 KB tiles of two heads
+      // stream at 4.9 TB/s, three 60 KB stages of one-head slices at 4.0 TB/s - four times as many 256-byte copies)
+      if (NS >= 3 || NS * t.stage_bytes >= 96 * 1024 || hg_force > 0) { *out = t; return true; }
       if (!have) { best = t; have = true; }
       break;
     }
