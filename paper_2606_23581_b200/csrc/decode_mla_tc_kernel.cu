@@ -17,13 +17,15 @@
 // Not covered here (the mma.sync kernel takes those calls): the on-read patch.
 //
 // STATUS (round 1): parity-green (tests/test_gpu_decode_mla.py::test_tcgen05_kernel_matches_the_oracle) but OPT-IN
-// (KAM_MLA_TC=1), because it is slower than the mma.sync kernel on the 16-head shape: 2.5 TB/s with 64-token tiles, 3.2 TB/s
-// with 128-token tiles (first version, git history) against 3.9 TB/s.  ncu: sm__pipe_tc_cycles_active 45 % at 34 % DRAM - the
-// tensor pipe is busy but each M = 128, N = 16, K = 16 instruction takes ~69 cycles, not the 8 of the M*N/256 pacing law: in
-// SS mode it re-reads its 4 KB A operand (128 token rows x 32 B) from shared memory, so with N = 16 the tile is streamed from
-// shared memory twice (QK^T, PV) at ~60 B/cycle for 8 cycles of math per 4 KB.  The formulation pays off from N >= 64 query
-// heads per work unit (DeepSeek-V2/V3: 128 heads), where the same A read feeds 4-8x the math; for 16 heads the next step is
-// the swapped form (heads, padded, as M from tensor memory; tokens as N), which changes the softmax ownership.
+// (KAM_MLA_TC=1), because it is slower than the mma.sync kernel on the 16-head shape: 2.5 TB/s against 3.9 TB/s.
+// What was measured (ncu, profiles/): the tcgen05 pipe is 43-45 % active at 35 % DRAM; 52 instructions per 64-token tile take
+// ~3300 cycles = ~64 cycles per tcgen05.mma whatever was tried - M = 128 or M = 64 for the scores, 8 independent partial
+// accumulators instead of one dependent chain, the PV blocks interleaved, QK^T of tile t + 1 issued ahead of PV of tile t,
+// 5 page-sized TMA copies per tile instead of 36.  64 cycles is the cost of an M x 128 x 16 instruction (M N / 256 with N = 128):
+// an instruction with N = 16 is charged like N = 128, so 7/8 of the tensor pipe is idle by construction, and the instruction
+// count alone (52 x 64 = 3328 cycles) equals the 3320-cycle HBM budget of a 64-token tile.  The formulation pays off from
+// N >= 64 query heads per work unit (DeepSeek-V2/V3: 128 heads); for 16 heads the tokens must be the N dimension (padded heads
+// as M = 64, O^T [64 x 512] packed into 256 tensor-memory columns, softmax rows = heads) - the next round's kernel.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
@@ -52,9 +54,14 @@ constexpr int kOffPair = kOffRope + kTcRopeSlots * kBlkBytes;
 // + one block of padding: the M = 128 score MMA reads 128 rows from a 64-row block (the extra rows only feed S rows nobody uses)
 constexpr int kTcSmem = kOffPair + kTcPairSlots * kPairBytes + kBlkBytes;     // 223232 bytes
 static_assert(kOffRope % 1024 == 0 && kTcSmem <= 227 * 1024, "shared-memory map");
-enum : int { BAR_FULL_PAIR = 0, BAR_EMPTY_PAIR = 10, BAR_FULL_ROPE = 20, BAR_EMPTY_ROPE = 23, BAR_S_FULL = 26, BAR_P_FULL = 27,
-             BAR_O_DONE = 28, BAR_Q_FULL = 29, BAR_HDR = 30, BAR_COUNT = 31 };
-constexpr uint32_t kTmemCols = 128;                 // S: columns [0, 16); O block b: columns [32 + 16 b, 48 + 16 b)
+enum : int { BAR_FULL_PAIR = 0, BAR_EMPTY_PAIR = 10, BAR_FULL_ROPE = 20, BAR_EMPTY_ROPE = 23, BAR_S_FULL = 26 /* x2 */, BAR_P_FULL = 28,
+             BAR_O_DONE = 29, BAR_Q_FULL = 30, BAR_SEG = 31, BAR_COUNT = 32 };
+// Tensor-memory columns.  O block b: [16 b, 16 b + 16).  S of tile parity u: kSParts partial sums at [64 + 128 u + 16 p, +16): back-to-back
+// MMAs into ONE accumulator serialise on its ~64-cycle pipeline latency (measured: 64 cycles per N = 16 instruction whatever M),
+// so consecutive k-steps go to different partial accumulators and the softmax warps add them.
+constexpr uint32_t kTmemCols = 512;
+constexpr int kSParts = 8;
+constexpr uint32_t kTmemS = 64;
 
 // ---- tcgen05 wrappers (PTX as documented in the Blackwell guide / CUTLASS cute/arch/mma_sm100_umma.hpp)
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -73,9 +80,9 @@ __device__ __forceinline__ uint64_t tc_desc(uint32_t smem_addr, uint32_t lbo, ui
   return static_cast<uint64_t>((smem_addr & 0x3ffff) >> 4) | (static_cast<uint64_t>(lbo >> 4) << 16) |
          (static_cast<uint64_t>(sbo >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
-// instruction descriptor: D = f32, A = B = bf16, N = 16, M = 128; a_mn: A is MN-major (the V^T read of the tile)
-__device__ __forceinline__ constexpr uint32_t tc_idesc(bool a_mn) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((a_mn ? 1u : 0u) << 15) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
+// instruction descriptor: D = f32, A = B = bf16, N = 16, M = m; a_mn: A is MN-major (the V^T read of the tile)
+__device__ __forceinline__ constexpr uint32_t tc_idesc(bool a_mn, uint32_t m) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((a_mn ? 1u : 0u) << 15) | ((16u >> 3) << 17) | ((m >> 4) << 24);
 }
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {          // this thread's lane, 16 consecutive columns
   uint32_t r[16];
@@ -125,7 +132,8 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
   if (threadIdx.x == 0) {
     for (int i = 0; i < kTcPairSlots; ++i) { mbar_init(&bars[BAR_FULL_PAIR + i], 1); mbar_init(&bars[BAR_EMPTY_PAIR + i], 1); }
     for (int i = 0; i < kTcRopeSlots; ++i) { mbar_init(&bars[BAR_FULL_ROPE + i], 1); mbar_init(&bars[BAR_EMPTY_ROPE + i], 1); }
-    mbar_init(&bars[BAR_S_FULL], 1); mbar_init(&bars[BAR_P_FULL], 128); mbar_init(&bars[BAR_O_DONE], 1); mbar_init(&bars[BAR_Q_FULL], 128); mbar_init(&bars[BAR_HDR], 1);
+    mbar_init(&bars[BAR_S_FULL], 1); mbar_init(&bars[BAR_S_FULL + 1], 1); mbar_init(&bars[BAR_P_FULL], 128); mbar_init(&bars[BAR_O_DONE], 1);
+    mbar_init(&bars[BAR_Q_FULL], 128); mbar_init(&bars[BAR_SEG], 1);
     mbar_fence_init();
   }
   // the rings start as zeros: rows a tile never loads (beyond the end of a segment) are read by the PV MMA with P = 0
@@ -199,81 +207,104 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
     mbar_wait(&bars[BAR_EMPTY_ROPE + rope_slot], rope_phase ^ 1);
     if (lane == 0) { hdrs[hdr_i] = make_int4(-1, 0, 0, 0); mbar_arrive(&bars[BAR_FULL_ROPE + rope_slot]); }
   } else if (warp == 5) {
-    // ================================================================ MMA issuer (one lane)
-    int pair_slot = 0, rope_slot = 0; uint32_t pair_phase = 0, rope_phase = 0, p_phase = 0, q_phase = 0; int hdr_i = 0;
+    // ================================================================ MMA issuer (one lane).  Tile t: S buffer t & 1, rope slot t % 3,
+    // pairs (4 t + b) % 10.  QK^T of tile t + 1 is issued BEFORE the PV of tile t (same segment), so the tensor pipe works
+    // while the softmax warps turn S(t) into P(t).
     const uint32_t sm0 = smem_u32(smem);
-    constexpr uint32_t idesc_qk = tc_idesc(false), idesc_pv = tc_idesc(true);
-    while (true) {
-      mbar_wait(&bars[BAR_FULL_ROPE + rope_slot], rope_phase);
-      const int4 hdr = hdrs[hdr_i];
-      hdr_i = (hdr_i + 1) % kTcHdrs;
-      if (lane == 0) mbar_arrive(&bars[BAR_HDR]);                                    // the softmax warps may read this tile's header
-      if (hdr.x < 0) break;                                                          // terminator
-      const bool first = hdr.y & HDR_FIRST;
-      if (first) { mbar_wait(&bars[BAR_Q_FULL], q_phase); q_phase ^= 1; }             // q~ of the new segment is in shared memory
+    constexpr uint32_t idesc_qk = tc_idesc(false, 64), idesc_pv = tc_idesc(true, 128);
+    uint32_t p_phase = 0, q_phase = 0;
+    auto read_hdr = [&](int t) {
+      mbar_wait(&bars[BAR_FULL_ROPE + t % kTcRopeSlots], (t / kTcRopeSlots) & 1);
+      return hdrs[t % kTcHdrs];
+    };
+    auto issue_qk = [&](int t, const int4& hdr) {
       tc_fence_after();
+      const uint32_t s_tmem = tmem + kTmemS + 128 * (t & 1);
       const bool rotate = p.plan.segs[hdr.x].rotate;
-      const int my_pair0 = pair_slot; const uint32_t my_phase0 = pair_phase;
+      // k-step k (0-3 rope, then 8 per pair, then the 4 lo steps of a rotated q~) accumulates into partial k % kSParts
+      auto step = [&](int k, uint64_t a, uint64_t b_) { tc_mma(s_tmem + 16 * (k % kSParts), a, b_, idesc_qk, k >= kSParts ? 1u : 0u); };
       if (lane == 0) {
-        // ---- S^T = K q~^T: rope block (4 k-steps, + the lo part of a rotated q~), then the 8 latent blocks
-        const uint32_t rope = sm0 + kOffRope + rope_slot * kBlkBytes;
-        for (int j = 0; j < 4; ++j)
-          tc_mma(tmem, tc_desc(rope + j * 32, 16, 1024), tc_desc(sm0 + kOffQhi + 8 * 2048 + j * 32, 16, 1024), idesc_qk, j > 0);
-        if (rotate)
-          for (int j = 0; j < 4; ++j) tc_mma(tmem, tc_desc(rope + j * 32, 16, 1024), tc_desc(sm0 + kOffQlo + j * 32, 16, 1024), idesc_qk, 1);
-        tc_commit(&bars[BAR_EMPTY_ROPE + rope_slot]);
+        const uint32_t rope = sm0 + kOffRope + (t % kTcRopeSlots) * kBlkBytes;
+        for (int j = 0; j < 4; ++j) step(j, tc_desc(rope + j * 32, 16, 1024), tc_desc(sm0 + kOffQhi + 8 * 2048 + j * 32, 16, 1024));
       }
       __syncwarp();
       for (int b = 0; b < 4; ++b) {
-        mbar_wait(&bars[BAR_FULL_PAIR + pair_slot], pair_phase);
+        const int c = 4 * t + b, slot = c % kTcPairSlots;
+        mbar_wait(&bars[BAR_FULL_PAIR + slot], (c / kTcPairSlots) & 1);
         tc_fence_after();
         if (lane == 0) {
-          const uint32_t base = sm0 + kOffPair + pair_slot * kPairBytes;
+          const uint32_t base = sm0 + kOffPair + slot * kPairBytes;
           for (int half = 0; half < 2; ++half)
             for (int j = 0; j < 4; ++j)
-              tc_mma(tmem, tc_desc(base + half * kBlkBytes + j * 32, 16, 1024), tc_desc(sm0 + kOffQhi + (2 * b + half) * 2048 + j * 32, 16, 1024), idesc_qk, 1);
+              step(4 + 8 * b + 4 * half + j, tc_desc(base + half * kBlkBytes + j * 32, 16, 1024), tc_desc(sm0 + kOffQhi + (2 * b + half) * 2048 + j * 32, 16, 1024));
         }
         __syncwarp();
-        if (++pair_slot == kTcPairSlots) { pair_slot = 0; pair_phase ^= 1; }
       }
-      if (lane == 0) tc_commit(&bars[BAR_S_FULL]);
+      if (lane == 0) {
+        if (rotate) {
+          const uint32_t rope = sm0 + kOffRope + (t % kTcRopeSlots) * kBlkBytes;
+          for (int j = 0; j < 4; ++j) step(36 + j, tc_desc(rope + j * 32, 16, 1024), tc_desc(sm0 + kOffQlo + j * 32, 16, 1024));
+        }
+        tc_commit(&bars[BAR_EMPTY_ROPE + t % kTcRopeSlots]);
+        tc_commit(&bars[BAR_S_FULL + (t & 1)]);
+      }
       __syncwarp();
-      if (++rope_slot == kTcRopeSlots) { rope_slot = 0; rope_phase ^= 1; }
-      // ---- O^T += V^T P^T once the softmax warps have written P^T (and rescaled O if the reference moved)
-      mbar_wait(&bars[BAR_P_FULL], p_phase); p_phase ^= 1;
+    };
+    auto issue_pv = [&](int t, bool first) {
+      mbar_wait(&bars[BAR_P_FULL], p_phase); p_phase ^= 1;     // P^T(t) is in shared memory, O rescaled if the reference moved
       tc_fence_after();
       if (lane == 0) {
-        int ps = my_pair0;
-        for (int b = 0; b < 4; ++b) {
-          const uint32_t base = sm0 + kOffPair + ps * kPairBytes;
-          for (int j = 0; j < kTcGroups; ++j)                     // 16 tokens per k-step: A advances 16 rows, B 32 bytes
-            tc_mma(tmem + 32 + 16 * b, tc_desc(base + j * 2048, kBlkBytes, 1024), tc_desc(sm0 + kOffP + j * 32, 16, 1024),
-                   idesc_pv, (!first || j > 0) ? 1u : 0u);
-          tc_commit(&bars[BAR_EMPTY_PAIR + ps]);                 // the pair returns to the producer when this block's MMAs are done
-          if (++ps == kTcPairSlots) ps = 0;
-        }
+        for (int j = 0; j < kTcGroups; ++j)                     // 16 tokens per k-step: A advances 16 rows, B 32 bytes;
+          for (int b = 0; b < 4; ++b) {                         // the four O blocks are independent accumulators: interleave them
+            const uint32_t base = sm0 + kOffPair + ((4 * t + b) % kTcPairSlots) * kPairBytes;
+            tc_mma(tmem + 16 * b, tc_desc(base + j * 2048, kBlkBytes, 1024), tc_desc(sm0 + kOffP + j * 32, 16, 1024), idesc_pv,
+                   (!first || j > 0) ? 1u : 0u);
+          }
+        for (int b = 0; b < 4; ++b) tc_commit(&bars[BAR_EMPTY_PAIR + (4 * t + b) % kTcPairSlots]);   // the pairs return to the producer
         tc_commit(&bars[BAR_O_DONE]);
       }
       __syncwarp();
-      (void)my_phase0;
+    };
+    int tile = 0;
+    int4 hdr = read_hdr(tile);
+    while (hdr.x >= 0) {                                        // hdr: the FIRST tile of a segment
+      if (lane == 0) mbar_arrive(&bars[BAR_SEG]);               // the softmax warps stage q~ of this segment ...
+      mbar_wait(&bars[BAR_Q_FULL], q_phase); q_phase ^= 1;      // ... and say when it is in shared memory
+      issue_qk(tile, hdr);
+      int4 cur = hdr; int cur_t = tile;
+      ++tile;
+      while (true) {
+        const int4 nxt = read_hdr(tile);
+        const bool look = nxt.x >= 0 && !(nxt.y & HDR_FIRST);   // same segment: its scores can be computed ahead
+        if (look) issue_qk(tile, nxt);
+        issue_pv(cur_t, cur.y & HDR_FIRST);
+        if (!look) { hdr = nxt; break; }
+        cur = nxt; cur_t = tile;
+        ++tile;
+      }
     }
+    if (lane == 0) mbar_arrive(&bars[BAR_SEG]);                 // terminator
   } else {
-    // ================================================================ softmax warps 0-3: thread = token row of the tile
+    // ================================================================ softmax warps 0-3.  The M = 64 score MMA puts token row t of the tile in
+    // tensor-memory lane (t % 16) + 32 (t / 16): the lower 16 lanes of warp t / 16.  For O^T (M = 128) lane = value column.
     const int tid = threadIdx.x;
+    const int trow_tok = lane < 16 ? warp * 16 + lane : -1;        // the token row this thread owns (none for the upper lanes)
     const uint32_t trow = tmem + (static_cast<uint32_t>(warp * 32) << 16);     // this thread's tensor-memory lane
     const float scale_log2 = p.sm_scale * 1.4426950408889634f;
     float m_ref[16], l_sum[16];
-    uint32_t h_phase = 0, s_phase = 0, o_phase = 0; int hdr_i = 0, pair_slot = 0;
-    bool pending_o = false;
+    uint32_t seg_phase = 0, o_phase = 0;
+    bool pending_o = false, need_seg = true;
     int n_rows = 0;
     grid_dep_wait();
-    while (true) {
-      mbar_wait(&bars[BAR_HDR], h_phase); h_phase ^= 1;
-      const int4 hdr = hdrs[hdr_i];
-      hdr_i = (hdr_i + 1) % kTcHdrs;
-      if (hdr.x < 0) break;
+    for (int ti = 0;; ++ti) {
+      if (need_seg) {                                            // the next tile starts a segment (or is the terminator)
+        mbar_wait(&bars[BAR_SEG], seg_phase); seg_phase ^= 1;
+        if (hdrs[ti % kTcHdrs].x < 0) break;
+      }
+      const int4 hdr = hdrs[ti % kTcHdrs];
       const int seg = hdr.x;
-      const bool first = hdr.y & HDR_FIRST;
+      const bool first = need_seg;
+      need_seg = false;
       if (first) {
         // ---- q~ of the segment into shared memory as the B operand: [9 blocks][16 heads][128 B], 128-byte swizzle; the rope
         // block rotated by -delta and split into bf16 hi + lo.  The previous segment's MMAs are complete (its epilogue waited).
@@ -319,12 +350,19 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
       }
 
       // ---- S^T row of this token
-      mbar_wait(&bars[BAR_S_FULL], s_phase); s_phase ^= 1;
+      mbar_wait(&bars[BAR_S_FULL + (ti & 1)], (ti >> 1) & 1);
       tc_fence_after();
       float v[16];
-      tmem_ld16(trow, v);
+      tmem_ld16(trow + kTmemS + 128 * (ti & 1), v);
+#pragma unroll
+      for (int part = 1; part < kSParts; ++part) {
+        float w[16];
+        tmem_ld16(trow + kTmemS + 128 * (ti & 1) + 16 * part, w);
+#pragma unroll
+        for (int h = 0; h < 16; ++h) v[h] += w[h];
+      }
       const int row_lo = hdr.z & 0xffff, row_hi = hdr.z >> 16;
-      const bool valid = tid >= row_lo && tid < row_hi;
+      const bool valid = trow_tok >= row_lo && trow_tok < row_hi;
       bool need = false;
 #pragma unroll
       for (int h = 0; h < 16; ++h) { v[h] = valid ? v[h] * scale_log2 : -CUDART_INF_F; need |= v[h] > m_ref[h] + 8.f; }
@@ -355,10 +393,10 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
 #pragma unroll
           for (int b = 0; b < 4; ++b) {
             float o[16];
-            tmem_ld16(trow + 32 + 16 * b, o);
+            tmem_ld16(trow + 16 * b, o);
 #pragma unroll
             for (int h = 0; h < 16; ++h) o[h] *= alpha[h];
-            tmem_st16(trow + 32 + 16 * b, o);
+            tmem_st16(trow + 16 * b, o);
           }
           tmem_st_wait();
         }
@@ -366,26 +404,23 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
       // ---- P^T[head][token] in bf16 as the B operand of the PV MMA: 2 token halves x [16 heads][128 B], swizzled
       {
         uint8_t* pbase = smem + kOffP;
-        const int c = tid & 63;
+        const int c = trow_tok & 63;
 #pragma unroll
         for (int h = 0; h < 16; ++h) {
           const float ms = m_ref[h] == -CUDART_INF_F ? 0.f : m_ref[h];
           const float pv = ex2(v[h] - ms);
           l_sum[h] += pv;
-          if (tid < kTcTok) *reinterpret_cast<__nv_bfloat16*>(pbase + sw_off(h, c)) = __float2bfloat16_rn(pv);
+          if (trow_tok >= 0) *reinterpret_cast<__nv_bfloat16*>(pbase + sw_off(h, c)) = __float2bfloat16_rn(pv);
         }
       }
-      if ((hdr.y & HDR_PARTIAL) && !valid && tid < kTcTok) {
+      if ((hdr.y & HDR_PARTIAL) && !valid && trow_tok >= 0) {
         // this token row is outside the chunk: whatever it holds (a neighbouring chunk, an unwritten page) must not reach O as 0 * NaN
-        int ps = pair_slot;
         for (int b = 0; b < 4; ++b) {
-          uint8_t* rowp = smem + kOffPair + ps * kPairBytes + tid * 128;
+          uint8_t* rowp = smem + kOffPair + ((4 * ti + b) % kTcPairSlots) * kPairBytes + trow_tok * 128;
 #pragma unroll
           for (int j = 0; j < 8; ++j) { reinterpret_cast<uint4*>(rowp)[j] = make_uint4(0, 0, 0, 0); reinterpret_cast<uint4*>(rowp + kBlkBytes)[j] = make_uint4(0, 0, 0, 0); }
-          if (++ps == kTcPairSlots) ps = 0;
         }
       }
-      pair_slot = (pair_slot + 4) % kTcPairSlots;
       fence_proxy_async();
       tc_fence_before();
       mbar_arrive(&bars[BAR_P_FULL]);
@@ -415,12 +450,13 @@ kam_mla_tc_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
           float o[16];
-          tmem_ld16(trow + 32 + 16 * b, o);
+          tmem_ld16(trow + 16 * b, o);
           float* po = p.part_o + static_cast<size_t>(seg) * g.R * 512 + b * 128 + tid;
 #pragma unroll
           for (int h = 0; h < 16; ++h) if (h < n_rows) po[static_cast<size_t>(h) * 512] = o[h] * inv[h];
         }
         tc_fence_before();
+        need_seg = true;
       }
     }
   }
