@@ -562,11 +562,21 @@ kam_status kam_relocate_patch_host(kam_ctx* c, const kam_pool* pool, const int32
   const void** tabs = static_cast<const void**>(sg->host);
   char* d = static_cast<char*>(c->d_hstage);
   cudaError_t e = cudaSuccess;
+  // Copies whose source AND staging destination continue the previous one are merged: a canonical store that keeps a chunk as
+  // one slab in this order (per layer: K, V, U_k, W_k, U_v, W_v) crosses PCIe in ONE transfer instead of 6 per layer.
+  const char* run_src = nullptr; char* run_dst = nullptr; size_t run_bytes = 0;
+  auto flush = [&]() {
+    if (run_bytes && e == cudaSuccess) e = cudaMemcpyAsync(run_dst, run_src, run_bytes, cudaMemcpyHostToDevice, st);
+    run_bytes = 0;
+  };
   auto put = [&](int which, int l, const void* const* src, size_t bytes, size_t& off) {
     tabs[which * L.n_layers + l] = nullptr;
     if (!src || bytes == 0) return;
     tabs[which * L.n_layers + l] = d + off;
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d + off, src[l], bytes, cudaMemcpyHostToDevice, st);
+    const char* sp = static_cast<const char*>(src[l]);
+    if (run_bytes && sp == run_src + run_bytes && d + off == run_dst + run_bytes) { run_bytes += bytes; return; }
+    flush();
+    run_src = sp; run_dst = d + off; run_bytes = bytes;
   };
   for (int l = 0; l < L.n_layers; ++l) {
     size_t off = per_layer * l;
@@ -579,6 +589,7 @@ kam_status kam_relocate_patch_host(kam_ctx* c, const kam_pool* pool, const int32
       put(5, l, rank ? Wv_host : nullptr, (size_t)L.n_kv_heads * rank * L.row_dim * fb, off);
     } else { tabs[4 * L.n_layers + l] = nullptr; tabs[5 * L.n_layers + l] = nullptr; }
   }
+  flush();
   if (e != cudaSuccess) { staging_release(sg, st); return cuda_fail(c, e, "cudaMemcpyAsync(host chunk)"); }
   if ((s = staging_commit(c, sg, (size_t)6 * L.n_layers * sizeof(void*), st)) != KAM_OK) return s;
   staging_release(sg, st);          // NOTE: the tables stay valid until this staging slot is reused (8 calls later)
