@@ -163,7 +163,8 @@ kam_status kam_rotate_inplace(kam_ctx *ctx, const kam_pool *pool, const int32_t 
 /* Same operator with the canonical chunk and its factors in HOST memory (a chunk recalled from an off-device
  * canonical store): every k/v/U/W array is a HOST array [n_layers] of HOST pointers with the layouts above
  * (U contiguous [T][H][rank]).  The library copies them to device staging it owns (H2D on `stream`), then runs
- * kam_relocate_patch.  Pinned host memory makes the copies asynchronous. */
+ * kam_relocate_patch.  Pinned host memory makes the copies asynchronous.  Copies whose host source continues the previous
+ * one are merged: a chunk kept as ONE slab in the order (per layer: K, V, U_k, W_k, U_v, W_v) crosses PCIe in one transfer. */
 kam_status kam_relocate_patch_host(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_table /* device */,
                                    int64_t dst_token_start, int32_t n_tokens, int64_t p_base, int64_t p_target,
                                    const void *const *k_host, const void *const *v_host,
@@ -223,7 +224,9 @@ kam_status kam_get_stats(kam_ctx *ctx, kam_stats *out);
  * is applied ON READ in O(m) per token, s_t += sm_scale * U_k[t,:].(W_k q) and o += (sum_t p_t U_v[t,:]) W_v, which is
  * the same readout as attending over k_t + U_k W_k, v_t + U_v W_v (P:44 with Eq. 1 substituted).
  * out [batch][n_q_heads][Dv] bf16 (Dv = row_dim, or v_dim for MLA), lse [batch][n_q_heads] f32 (natural log, scale
- * inside).  A request with no tokens gives out = 0, lse = -inf.  Requires elem_dtype == KAM_BF16. */
+ * inside).  A request with no tokens gives out = 0, lse = -inf.  Requires elem_dtype == KAM_BF16; head_dim 64 or 128 and at most
+ * 16 query heads per KV head (MHA/GQA); MLA in absorbed form: row_dim 576 = 512 latent + 64 rope, v_dim 512, q rows of 576,
+ * the context's own pool with page_size % 16 == 0 (any number of query heads).  Otherwise KAM_ERR_UNSUPPORTED. */
 /* Largest rank a kam_patch_ref of later decode calls may carry: 16, 32 or 64 (default KAM_MAX_RANK).  The decode kernel
  * is specialised for it (shared memory and registers per tile grow with it), so a caller whose patches are all rank 16
  * should say so.  Errors: INVALID_ARG. */
