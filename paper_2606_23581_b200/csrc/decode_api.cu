@@ -50,6 +50,17 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
       *out = g;
       return KAM_OK;
     }
+    // calls without an on-read patch run the token-split kernel (decode_mla_ts_kernel.cu: one CTA per SM, 64-token iterations);
+    // KAM_MLA_KSPLIT=1 keeps them on the k-split kernel below (the one that carries the patch)
+    const char* ks_env = getenv("KAM_MLA_KSPLIT");
+    if (kt == 0 && !(ks_env && ks_env[0] == '1')) {
+      g.mla = 3;
+      g.smem_bytes = mla_ts_smem_bytes();
+      g.n_ctas = c->sm_count;
+      c->dec_geom[variant][kt] = g; c->dec_geom_ok[variant][kt] = true;
+      *out = g;
+      return KAM_OK;
+    }
     g.off_hdr = 128; g.off_xch = 1024; g.off_box0 = 1024 + 2 * kMlaWarps * 256 * 4;
     int want = c->dec_ctas_per_sm > 0 ? std::min(c->dec_ctas_per_sm, 2) : 2;
     for (; want >= 1; --want) {
@@ -195,7 +206,8 @@ static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* po
   csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
   csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = patches ? 1 : 0;
   launch_decode_plan(g, p.plan, csr, st);
-  if (g.mla == 2) launch_mla_tc_decode(g, p, false, st);
+  if (g.mla == 3) launch_mla_ts_decode(g, p, false, st);
+  else if (g.mla == 2) launch_mla_tc_decode(g, p, false, st);
   else if (g.mla) launch_mla_decode(g, p, false, st);
   else launch_decode(g, p, false, st);                            // reads the plan just written: plain stream order
   launch_decode_merge(g, p, c->use_pdl, st);
@@ -338,7 +350,8 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.err = c->d_err;
   // with a plan from an earlier call the decode prologue may overlap whatever precedes it on the stream (it only reads the plan)
-  if (g.mla == 2) launch_mla_tc_decode(g, p, cached && c->use_pdl, st);
+  if (g.mla == 3) launch_mla_ts_decode(g, p, cached && c->use_pdl, st);
+  else if (g.mla == 2) launch_mla_tc_decode(g, p, cached && c->use_pdl, st);
   else if (g.mla) launch_mla_decode(g, p, cached && c->use_pdl, st);
   else launch_decode(g, p, cached && c->use_pdl, st);
   launch_decode_merge(g, p, c->use_pdl, st);

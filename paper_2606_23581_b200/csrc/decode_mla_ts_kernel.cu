@@ -1,0 +1,459 @@
+// kam_mla_ts_decode_kernel: absorbed MLA decode, TOKEN-split form.  Same operation, plan, partials
+// and merge as decode_mla_kernel.cu (which still takes the calls that carry an on-read patch); this is the kernel the
+// patch-free calls run.
+//
+// Why a second mma.sync formulation: decode_mla_kernel.cu splits the 576-deep contraction over four warps, so every 16-token
+// tile costs a shared-memory exchange of partial scores, a CTA barrier and a softmax repeated in all four warps - ncu
+// (profiles/ncu_extras_r01.md) shows ~600 instructions per warp and tile and a kernel bound by that chain (tensor pipe 29 %,
+// issue slots 42 %, DRAM 58 %).  Here one ITERATION is 64 tokens (four 16-token TMA boxes) and the work is split by TOKENS:
+//
+//   warp w of 8:  tg = w & 3 (which box), hh = w >> 2 (which 8 of the 16 query heads)
+//   S^T[16 tokens][8 heads] = K_box q~^T   : all 36 k-steps in this one warp (q~ fragments live in 72 registers), so the
+//                                           scores are complete - no exchange; softmax values are computed once, not 4x
+//   P^T (bf16) -> shared memory [64 tokens][16 heads] (48-byte rows: conflict-free stores and ldmatrix.trans)
+//   ONE barrier per iteration (barrier.red.or: also tells whether any score ran 2^8 past its head's reference)
+//   O^T[64 w .. 64 w + 64][16 heads] += V^T P^T over the iteration's 64 tokens: warp w owns 64-column block w of every box
+//
+// The reference of the lazy softmax (decode_kernel.cu) is common to the CTA and moves only through a slow path (two more
+// barriers: tile maxima -> new references, rescale factors -> O), taken on the first iteration of a segment and then rarely.
+// Per warp and 64 tokens: 68 HMMA, 56 LDSM, ~250 instructions in all (the k-split kernel: ~1200).
+// CTA = 8 compute warps + 1 producer warp (slot mapping A1 + one TMA box [9 x 64 columns][16 tokens][128 B swizzled] per
+// tile), one CTA per SM, flat ring of 11 boxes (an iteration takes the next 1-4 slots).
+//
+// The compute warps never load from global memory.  Measured on B200: with ~200 KB of bulk copies in flight per SM, a demand
+// load from the same SM waits microseconds (it queues behind them), and two dependent ones per segment (the segment record,
+// then q) cost 28 of 133 us.  So the producer also stages q (16 rows x 1152 B, one bulk copy) and the chunk's (cos, sin) row
+// into shared memory IN the stream, right before the segment's first box, and the segment's fields ride in the box header.
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+#include "common.cuh"
+#include "decode_common.cuh"
+#include "internal.h"
+
+namespace kam {
+
+namespace {
+constexpr int kTsWarps = 8;                 // compute warps
+constexpr int kTsThreads = kTsWarps * 32;   // threads at the compute warps' named barriers
+constexpr int kTsBlock = 384;               // 2 compute warpgroups + 1 warpgroup whose first warp is the producer (registers move
+                                            // between warpgroups: 12 warps launch at 168 registers, the compute warps take 232, the producer keeps 40)
+constexpr int kTsIter = 4;                  // boxes (16-token tiles) per full iteration
+constexpr int kTsSlots = 11;                // ring of boxes
+constexpr int kTsSteps = 36;                // 16-column k-steps of a 576-wide row (32 latent + 4 rope)
+constexpr int kTsBox = kDecTile * 576 * 2;  // 18432 bytes
+constexpr int kTsPRow = 48;                 // bytes of one token's row of P^T (16 heads x bf16 + 16 bytes of padding)
+constexpr int kTsPBuf = kTsIter * kDecTile * kTsPRow;
+// shared-memory map (bytes)
+constexpr int kTsOffHdr = 256;              // int4[11]
+constexpr int kTsOffRed = 512;              // float[8 warps][8 heads]: tile maxima (slow path)
+constexpr int kTsOffAlpha = 768;            // float[16 heads]: rescale factors (slow path)
+constexpr int kTsOffLsum = 1024;            // float[8 warps][8 heads]: softmax masses at the end of a segment
+constexpr int kTsOffCs = 1280;              // float2[32]: (cos, sin)(delta f_i) of the segment's chunk
+constexpr int kTsOffP = 2048;               // 2 x kTsPBuf
+constexpr int kTsOffQ = 8192;               // q of the segment: [16 heads][1152 B], as in global memory
+constexpr int kTsOffBox = kTsOffQ + kTsBox; // 26624 = 26 x 1024
+constexpr int kTsSmem = kTsOffBox + kTsSlots * kTsBox;      // 229376
+static_assert(kTsOffP + 2 * kTsPBuf <= kTsOffQ && kTsOffBox % 1024 == 0 && kTsSmem <= 227 * 1024, "shared-memory map");
+enum : int { HDR_ROTATE = 8 };              // header flags beyond decode_common.cuh's; bits 16+ of the flags word: head group
+
+__device__ __forceinline__ bool bar_or(int id, bool pred) {      // barrier over the compute warps + OR of pred
+  uint32_t out;
+  asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.b32 q, %2, 0;\n\tbarrier.cta.red.or.pred p, %1, %3, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(out) : "r"(id), "r"(static_cast<uint32_t>(pred)), "n"(kTsThreads) : "memory");
+  return out != 0;
+}
+// 4 x 4 transpose of 32-bit words across a quad (lanes t4 = 0-3): in, lane r holds row r = (x, y, z, w); out, lane c holds
+// column c.  Two butterfly stages (xor 2, xor 1), two shuffles each.
+__device__ __forceinline__ void quad_transpose(uint4& v, int t4) {
+  const bool h2 = t4 & 2, h1 = t4 & 1;
+  uint32_t s0 = h2 ? v.x : v.z, s1 = h2 ? v.y : v.w;
+  s0 = __shfl_xor_sync(0xffffffffu, s0, 2); s1 = __shfl_xor_sync(0xffffffffu, s1, 2);
+  if (h2) { v.x = s0; v.y = s1; } else { v.z = s0; v.w = s1; }
+  s0 = h1 ? v.x : v.y; s1 = h1 ? v.z : v.w;
+  s0 = __shfl_xor_sync(0xffffffffu, s0, 1); s1 = __shfl_xor_sync(0xffffffffu, s1, 1);
+  if (h1) { v.x = s0; v.z = s1; } else { v.y = s0; v.w = s1; }
+}
+}  // namespace
+
+__global__ void __launch_bounds__(kTsBlock, 1)
+kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem);
+  uint64_t* empty_bar = full_bar + kTsSlots;
+  uint64_t* q_full = empty_bar + kTsSlots;                       // q (+ cos/sin) of a segment staged / read into registers by all warps
+  uint64_t* q_empty = q_full + 1;
+  int4* hdrs = reinterpret_cast<int4*>(smem + kTsOffHdr);
+  float* red = reinterpret_cast<float*>(smem + kTsOffRed);
+  float* alpha_s = reinterpret_cast<float*>(smem + kTsOffAlpha);
+  float* lsum = reinterpret_cast<float*>(smem + kTsOffLsum);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kTsSlots; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], kTsWarps); }
+    mbar_init(q_full, 1); mbar_init(q_empty, kTsWarps);
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  grid_dep_launch();
+  const int seg_begin = p.plan.cta_seg[blockIdx.x], seg_end = p.plan.cta_seg[blockIdx.x + 1];
+  if (seg_begin >= seg_end) return;
+
+  if (warp >= kTsWarps) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    if (warp > kTsWarps) return;                                 // the rest of the producer warpgroup only gives its registers away
+    // ================================================================ producer warp: lanes 0-3 issue the boxes of an iteration
+    int slot = 0; uint32_t phase = 0, q_phase = 0;
+    const char* tm_k = static_cast<const char*>(p.tmaps) + static_cast<size_t>(p.layer) * kTmapLayerBytes;
+    auto tile_slot = [&](const DecSeg& S, const int32_t* bt, int tl) {       // pool slot of tile tl of the segment (A1)
+      if (tl == 0) return S.slot0;
+      const int tok = (S.tile0 + tl) * kDecTile;
+      const int pg = g.P_shift >= 0 ? (tok >> g.P_shift) : tok / g.P;
+      return bt[pg] * g.P + (tok - pg * g.P);
+    };
+    grid_dep_wait();
+    DecSeg S_next = p.plan.segs[seg_begin];
+    for (int seg = seg_begin; seg < seg_end; ++seg) {
+      const DecSeg S = S_next;
+      if (seg + 1 < seg_end) S_next = p.plan.segs[seg + 1];        // in flight while this segment streams
+      const int32_t* bt = p.block_tables + S.bt_off;
+      const int n_rows = min(kMlaHeads, g.Hq - S.hg * kMlaHeads);
+      if (lane == 0) {
+        // q and the cos/sin row travel in the stream, ahead of the segment's first box
+        mbar_wait(q_empty, q_phase ^ 1);
+        mbar_arrive_expect_tx(q_full, static_cast<uint32_t>(n_rows * 1152 + (S.rotate ? 256 : 0)));
+        bulk_g2s(smem + kTsOffQ, static_cast<const char*>(p.q) + (static_cast<size_t>(S.b) * g.Hq + static_cast<size_t>(S.hg) * kMlaHeads) * 1152,
+                 static_cast<uint32_t>(n_rows * 1152), q_full);
+        if (S.rotate) bulk_g2s(smem + kTsOffCs, p.plan.cs + static_cast<size_t>(S.chunk) * 32, 256, q_full);
+      }
+      q_phase ^= 1;
+      int my_next = (lane < S.n_tiles) ? tile_slot(S, bt, lane) : 0;          // slots of tiles t0 + lane, one batch ahead
+      for (int t0 = 0; t0 < S.n_tiles; t0 += 32) {
+        const int my_slot = my_next;
+        if (t0 + 32 + lane < S.n_tiles) my_next = tile_slot(S, bt, t0 + 32 + lane);
+        const int nbatch = min(32, S.n_tiles - t0);
+        for (int i0 = 0; i0 < nbatch; i0 += kTsIter) {
+          const int nb = min(kTsIter, nbatch - i0);
+          const int s0 = __shfl_sync(0xffffffffu, my_slot, i0 + (lane & 3));
+          if (lane < nb) {
+            int sl = slot + lane; uint32_t ph = phase;
+            if (sl >= kTsSlots) { sl -= kTsSlots; ph ^= 1; }
+            mbar_wait(&empty_bar[sl], ph ^ 1);
+            const int tl = t0 + i0 + lane;
+            const int tok = (S.tile0 + tl) * kDecTile;
+            const int row_lo = max(S.tok_lo - tok, 0), row_hi = min(S.tok_hi - tok, kDecTile);
+            const int flags = ((lane == 0 && tl == 0) ? HDR_FIRST : 0) | ((lane == 0 && t0 + i0 + nb >= S.n_tiles) ? HDR_LAST : 0) |
+                              ((row_lo > 0 || row_hi < kDecTile) ? HDR_PARTIAL : 0) | (S.rotate ? HDR_ROTATE : 0) | (S.hg << 16);
+            hdrs[sl] = make_int4(seg, flags, row_lo | (row_hi << 8), nb);
+            mbar_arrive_expect_tx(&full_bar[sl], static_cast<uint32_t>(kTsBox));
+            tma_load_3d(smem + kTsOffBox + sl * kTsBox, tm_k, 0, s0, 0, &full_bar[sl]);
+          }
+          __syncwarp();
+          slot += nb;
+          if (slot >= kTsSlots) { slot -= kTsSlots; phase ^= 1; }
+        }
+      }
+    }
+    if (lane == 0) {
+      mbar_wait(&empty_bar[slot], phase ^ 1);
+      hdrs[slot] = make_int4(-1, 0, 0, 0);
+      mbar_arrive(&full_bar[slot]);
+    }
+    return;
+  }
+
+  // ================================================================ compute warps
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+  const int tg = warp & 3, hh = warp >> 2;
+  const int gq = lane >> 2, t4 = lane & 3;
+  const float scale_log2 = p.sm_scale * 1.4426950408889634f;
+  constexpr float kLn2 = 0.6931471805599453f;
+
+  // lane offsets inside a box: K rows through ldmatrix (A of S^T), V^T through ldmatrix.trans (A of O^T); 128-byte swizzle
+  const int k_row = (lane & 7) + ((lane >> 3) & 1) * 8, k_hi = lane >> 4;
+  const int v_row = (lane & 7) + (lane >> 4) * 8, v_hi = (lane >> 3) & 1;
+  uint32_t koff[4], voff[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    koff[j] = static_cast<uint32_t>(k_row * 128) + ((static_cast<uint32_t>(k_hi ^ (lane & 7)) << 4) ^ (static_cast<uint32_t>(j) << 5));
+    voff[j] = static_cast<uint32_t>(warp * 2048 + v_row * 128) + ((static_cast<uint32_t>(v_hi ^ (lane & 7)) << 4) ^ (static_cast<uint32_t>(j) << 5));
+  }
+  const uint32_t sm0 = smem_u32(smem);
+  // P^T: this lane's stores (token rows gq and gq + 8 of box tg, heads hh * 8 + 2 t4, +1) and its ldmatrix.trans rows
+  const uint32_t p_st = static_cast<uint32_t>(kTsOffP + (tg * kDecTile + gq) * kTsPRow + hh * 16 + t4 * 4);
+  const uint32_t p_ld = sm0 + static_cast<uint32_t>(kTsOffP + ((lane & 7) + ((lane >> 3) & 1) * 8) * kTsPRow + (lane >> 4) * 16);
+
+  uint32_t qf[kTsSteps][2], ql[4][2];
+  float O[2][4][4];
+  float m_ref[2] = {-CUDART_INF_F, -CUDART_INF_F}, l_run[2] = {0.f, 0.f};
+  bool use_lo = false;
+  int n_rows = 0, seg = 0;
+  int slot = 0, pbuf = 0; uint32_t phase = 0, q_phase = 0;
+  // ring slot j of the current iteration (slots slot .. slot + 3, wrapping) and its mbarrier parity
+  auto slot_of = [&](int j) { const int sl = slot + j; return sl >= kTsSlots ? sl - kTsSlots : sl; };
+  auto phase_of = [&](int j) { return slot + j >= kTsSlots ? (phase ^ 1u) : phase; };
+  while (true) {
+    const int leader = slot;
+    mbar_wait(&full_bar[leader], phase);
+    const int4 hdr = hdrs[leader];
+    if (hdr.x < 0) break;
+    const int nb = hdr.w;
+    const bool first = hdr.y & HDR_FIRST;
+
+    if (first) {
+      // ---- new segment: q~ fragments of this warp's 8 heads for all 36 k-steps; the rope band rotated by -delta (hi + lo)
+      seg = hdr.x;
+      use_lo = hdr.y & HDR_ROTATE;
+      n_rows = min(kMlaHeads, g.Hq - (hdr.y >> 16) * kMlaHeads);
+      mbar_wait(q_full, q_phase); q_phase ^= 1;
+      const float2* cs = reinterpret_cast<const float2*>(smem + kTsOffCs);
+      // lane (gq, t4) reads 16-byte chunks 4 j + t4 of row hh * 8 + gq of the staged q; a 4 x 4
+      // transpose of 32-bit words across the quad turns four chunks into the B fragments of k-steps 2 j and 2 j + 1
+      const int row = hh * 8 + gq;
+      const uint4* qr = reinterpret_cast<const uint4*>(smem + kTsOffQ + row * 1152) + t4;
+      const bool live = row < n_rows;
+      const uint4 zero4 = make_uint4(0, 0, 0, 0);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        uint4 w = live ? qr[4 * j] : zero4;
+        quad_transpose(w, t4);
+        qf[2 * j][0] = w.x; qf[2 * j][1] = w.y; qf[2 * j + 1][0] = w.z; qf[2 * j + 1][1] = w.w;
+      }
+      {
+        // rope band: chunk 64 + t4 holds columns rel = 8 t4 .. + 7, chunk 68 + t4 their HALF-style partners rel + 32
+        uint4 wx = live ? qr[64] : zero4, wy = live ? qr[68] : zero4;
+        uint4 lx = zero4, ly = zero4;
+        if (use_lo) {                                              // q~ = R(-delta) q, carried as bf16 hi + lo
+          float x[8], y[8], rx[8], ry[8];
+          unpack8(wx, x); unpack8(wy, y);
+          if (g.rope_style == KAM_ROPE_HALF) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+              const float2 u = cs[8 * t4 + e];
+              rx[e] = fmaf(x[e], u.x, y[e] * u.y);
+              ry[e] = fmaf(y[e], u.x, -x[e] * u.y);
+            }
+          } else {
+#pragma unroll
+            for (int e = 0; e < 8; e += 2) {
+              const float2 u = cs[4 * t4 + (e >> 1)], v = cs[16 + 4 * t4 + (e >> 1)];
+              rx[e] = fmaf(x[e], u.x, x[e + 1] * u.y); rx[e + 1] = fmaf(x[e + 1], u.x, -x[e] * u.y);
+              ry[e] = fmaf(y[e], v.x, y[e + 1] * v.y); ry[e + 1] = fmaf(y[e + 1], v.x, -y[e] * v.y);
+            }
+          }
+          wx = pack8(rx); wy = pack8(ry);
+          unpack8(wx, x); unpack8(wy, y);
+#pragma unroll
+          for (int e = 0; e < 8; ++e) { rx[e] -= x[e]; ry[e] -= y[e]; }
+          lx = pack8(rx); ly = pack8(ry);
+        }
+        quad_transpose(wx, t4); quad_transpose(wy, t4); quad_transpose(lx, t4); quad_transpose(ly, t4);
+        qf[32][0] = wx.x; qf[32][1] = wx.y; qf[33][0] = wx.z; qf[33][1] = wx.w;
+        qf[34][0] = wy.x; qf[34][1] = wy.y; qf[35][0] = wy.z; qf[35][1] = wy.w;
+        ql[0][0] = lx.x; ql[0][1] = lx.y; ql[1][0] = lx.z; ql[1][1] = lx.w;
+        ql[2][0] = ly.x; ql[2][1] = ly.y; ql[3][0] = ly.z; ql[3][1] = ly.w;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(q_empty);                       // the staging buffers may take the next segment's q
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int n = 0; n < 4; ++n) O[nt][n][0] = O[nt][n][1] = O[nt][n][2] = O[nt][n][3] = 0.f;
+      m_ref[0] = m_ref[1] = -CUDART_INF_F;
+      l_run[0] = l_run[1] = 0.f;
+    }
+
+    // ---- S^T[16 tokens of box tg][this warp's 8 heads], complete
+    float s[4] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
+    const int my_box = slot_of(tg);
+    if (tg < nb) {
+      if (tg) mbar_wait(&full_bar[my_box], phase_of(tg));
+      const int4 h2 = hdrs[my_box];
+      const uint32_t kb = sm0 + static_cast<uint32_t>(kTsOffBox + my_box * kTsBox);
+      // a 64-column block = 4 k-steps: the fragments of block c + 1 are fetched while the MMAs of block c run, and k-step k
+      // accumulates into chain k & 3 (a dependent HMMA would wait out the previous one's latency)
+      float sc[4][4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) sc[c][0] = sc[c][1] = sc[c][2] = sc[c][3] = 0.f;
+      {
+        uint32_t a[2][4][4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) ldmatrix_x4(a[0][k][0], a[0][k][1], a[0][k][2], a[0][k][3], kb + koff[k]);
+#pragma unroll
+        for (int c = 0; c < 9; ++c) {
+          if (c + 1 < 9) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              ldmatrix_x4(a[(c + 1) & 1][k][0], a[(c + 1) & 1][k][1], a[(c + 1) & 1][k][2], a[(c + 1) & 1][k][3], kb + koff[k] + (c + 1) * 2048);
+          }
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const uint32_t* f = a[c & 1][k];
+            mma_bf16_16816(sc[k][0], sc[k][1], sc[k][2], sc[k][3], f[0], f[1], f[2], f[3], qf[4 * c + k][0], qf[4 * c + k][1]);
+            if (c == 8 && use_lo) mma_bf16_16816(sc[(k + 2) & 3][0], sc[(k + 2) & 3][1], sc[(k + 2) & 3][2], sc[(k + 2) & 3][3], f[0], f[1], f[2], f[3], ql[k][0], ql[k][1]);
+          }
+        }
+      }
+      float sa[4], sb[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { sa[e] = sc[0][e] + sc[1][e]; sb[e] = sc[2][e] + sc[3][e]; }
+      const bool partial = h2.y & HDR_PARTIAL;
+      const int row_lo = h2.z & 0xff, row_hi = h2.z >> 8;
+      const bool ok0 = !partial || (gq >= row_lo && gq < row_hi);
+      const bool ok1 = !partial || (gq + 8 >= row_lo && gq + 8 < row_hi);
+      s[0] = ok0 ? (sa[0] + sb[0]) * scale_log2 : -CUDART_INF_F;
+      s[1] = ok0 ? (sa[1] + sb[1]) * scale_log2 : -CUDART_INF_F;
+      s[2] = ok1 ? (sa[2] + sb[2]) * scale_log2 : -CUDART_INF_F;
+      s[3] = ok1 ? (sa[3] + sb[3]) * scale_log2 : -CUDART_INF_F;
+      if (partial) {
+        // rows outside the chunk may hold anything (a neighbouring chunk, an unwritten page): 0 * NaN must not reach O.  The two
+        // warps of this box clear the latent columns of those rows (4 blocks each); the other warp's score MMAs may still read
+        // them - its scores of those rows are masked too.
+        uint8_t* bptr = smem + kTsOffBox + my_box * kTsBox + hh * 4 * 2048;
+        for (int idx = lane; idx < 16 * 32; idx += 32) {
+          const int r = idx >> 5, j = idx & 31;                  // token row, 16-byte chunk of this warp's 4 blocks
+          if (r < row_lo || r >= row_hi) *reinterpret_cast<uint4*>(bptr + (j >> 3) * 2048 + r * 128 + ((j & 7) << 4)) = make_uint4(0, 0, 0, 0);
+        }
+        fence_proxy_async();
+      }
+    }
+
+    // ---- P^T with the current references; one barrier publishes it and tells whether a reference must move
+    bool need = false;
+    float pv[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      need |= s[e] > m_ref[e & 1] + 8.f;
+      pv[e] = ex2(s[e] - (m_ref[e & 1] == -CUDART_INF_F ? 0.f : m_ref[e & 1]));
+    }
+    uint8_t* pb = smem + pbuf * kTsPBuf;
+    if (tg < nb) {
+      *reinterpret_cast<uint32_t*>(pb + p_st) = pack_bf16x2(pv[0], pv[1]);
+      *reinterpret_cast<uint32_t*>(pb + p_st + 8 * kTsPRow) = pack_bf16x2(pv[2], pv[3]);
+    }
+    if (bar_or(1, need)) {
+      // ---- slow path (first iteration of a segment, then rare): tile maxima -> new references -> P again, O rescaled
+      float mx0 = fmaxf(s[0], s[2]), mx1 = fmaxf(s[1], s[3]);
+      mx0 = col_max(mx0); mx1 = col_max(mx1);
+      if (gq == 0) { red[warp * 8 + 2 * t4] = mx0; red[warp * 8 + 2 * t4 + 1] = mx1; }
+      named_bar_sync(2, kTsThreads);
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const float* r0 = red + hh * 32 + 2 * t4 + e;
+        const float tm = fmaxf(fmaxf(r0[0], r0[8]), fmaxf(r0[16], r0[24]));
+        const float mn = tm > m_ref[e] + 8.f ? tm : m_ref[e];
+        const float al = mn == m_ref[e] ? 1.f : ex2(m_ref[e] - mn);
+        l_run[e] *= al;
+        m_ref[e] = mn;
+        if (tg == 0 && gq == 0) alpha_s[hh * 8 + 2 * t4 + e] = al;
+      }
+#pragma unroll
+      for (int e = 0; e < 4; ++e) pv[e] = ex2(s[e] - (m_ref[e & 1] == -CUDART_INF_F ? 0.f : m_ref[e & 1]));
+      if (tg < nb) {
+        *reinterpret_cast<uint32_t*>(pb + p_st) = pack_bf16x2(pv[0], pv[1]);
+        *reinterpret_cast<uint32_t*>(pb + p_st + 8 * kTsPRow) = pack_bf16x2(pv[2], pv[3]);
+      }
+      named_bar_sync(2, kTsThreads);
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+        const float a0 = alpha_s[nt * 8 + 2 * t4], a1 = alpha_s[nt * 8 + 2 * t4 + 1];
+#pragma unroll
+        for (int n = 0; n < 4; ++n) { O[nt][n][0] *= a0; O[nt][n][1] *= a1; O[nt][n][2] *= a0; O[nt][n][3] *= a1; }
+      }
+    }
+    l_run[0] += pv[0] + pv[2];
+    l_run[1] += pv[1] + pv[3];
+
+    // ---- O^T[this warp's 64 value columns][16 heads] += V^T P^T over the iteration's boxes; a box returns to the producer
+    // as soon as this warp's MMAs on it are issued (they consumed its fragments)
+    {
+      const uint32_t pl = p_ld + static_cast<uint32_t>(pbuf * kTsPBuf);
+      const uint32_t box0 = sm0 + static_cast<uint32_t>(kTsOffBox);
+      if (nb == kTsIter) {
+        // full iteration, straight-line: every box landed (its owner waited before the barrier; this wait orders OUR reads),
+        // P^T fragments of all four k-steps up front, V^T fragments of box j + 1 fetched under the MMAs of box j
+        uint32_t vb[kTsIter];
+#pragma unroll
+        for (int j = 0; j < kTsIter; ++j) {
+          if (j != tg) mbar_wait(&full_bar[slot_of(j)], phase_of(j));
+          vb[j] = box0 + static_cast<uint32_t>(slot_of(j) * kTsBox);
+        }
+        uint32_t b[kTsIter][4];
+#pragma unroll
+        for (int j = 0; j < kTsIter; ++j) ldmatrix_x4_trans(b[j][0], b[j][1], b[j][2], b[j][3], pl + j * (kDecTile * kTsPRow));
+        uint32_t a[2][4][4];
+#pragma unroll
+        for (int n = 0; n < 4; ++n) ldmatrix_x4_trans(a[0][n][0], a[0][n][1], a[0][n][2], a[0][n][3], vb[0] + voff[n]);
+#pragma unroll
+        for (int j = 0; j < kTsIter; ++j) {
+          if (j + 1 < kTsIter) {
+#pragma unroll
+            for (int n = 0; n < 4; ++n)
+              ldmatrix_x4_trans(a[(j + 1) & 1][n][0], a[(j + 1) & 1][n][1], a[(j + 1) & 1][n][2], a[(j + 1) & 1][n][3], vb[j + 1] + voff[n]);
+          }
+#pragma unroll
+          for (int n = 0; n < 4; ++n) {
+            const uint32_t* f = a[j & 1][n];
+            mma_bf16_16816(O[0][n][0], O[0][n][1], O[0][n][2], O[0][n][3], f[0], f[1], f[2], f[3], b[j][0], b[j][1]);
+            mma_bf16_16816(O[1][n][0], O[1][n][1], O[1][n][2], O[1][n][3], f[0], f[1], f[2], f[3], b[j][2], b[j][3]);
+          }
+          if (lane == 0) mbar_arrive(&empty_bar[slot_of(j)]);
+        }
+      } else {
+        // short iteration at the end of a segment
+        for (int j = 0; j < nb; ++j) {
+          const int sl = slot_of(j);
+          if (j != tg) mbar_wait(&full_bar[sl], phase_of(j));
+          const uint32_t vbj = box0 + static_cast<uint32_t>(sl * kTsBox);
+          uint32_t b[4];
+          ldmatrix_x4_trans(b[0], b[1], b[2], b[3], pl + j * (kDecTile * kTsPRow));
+#pragma unroll
+          for (int n = 0; n < 4; ++n) {
+            uint32_t f[4];
+            ldmatrix_x4_trans(f[0], f[1], f[2], f[3], vbj + voff[n]);
+            mma_bf16_16816(O[0][n][0], O[0][n][1], O[0][n][2], O[0][n][3], f[0], f[1], f[2], f[3], b[0], b[1]);
+            mma_bf16_16816(O[1][n][0], O[1][n][1], O[1][n][2], O[1][n][3], f[0], f[1], f[2], f[3], b[2], b[3]);
+          }
+          if (lane == 0) mbar_arrive(&empty_bar[sl]);
+        }
+      }
+    }
+    pbuf ^= 1;
+    slot += nb;
+    if (slot >= kTsSlots) { slot -= kTsSlots; phase ^= 1; }
+
+    if (hdr.y & HDR_LAST) {
+      // ---- the segment's softmax state -> partials: o normalised, lse in natural log
+      const float l0 = col_sum(l_run[0]), l1 = col_sum(l_run[1]);
+      if (gq == 0) { lsum[warp * 8 + 2 * t4] = l0; lsum[warp * 8 + 2 * t4 + 1] = l1; }
+      named_bar_sync(2, kTsThreads);
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const float* r0 = lsum + nt * 32 + 2 * t4 + e;
+          const float tot = (r0[0] + r0[8]) + (r0[16] + r0[24]);
+          const int hq = nt * 8 + 2 * t4 + e;
+          if (hq < n_rows) {
+            const float inv = tot > 0.f ? 1.f / tot : 0.f;
+            const size_t row = static_cast<size_t>(seg) * g.R + hq;
+            float* po = p.part_o + row * 512 + warp * 64 + gq;
+#pragma unroll
+            for (int n = 0; n < 4; ++n) { po[n * 16] = O[nt][n][e] * inv; po[n * 16 + 8] = O[nt][n][2 + e] * inv; }
+            if (nt == hh && tg == 0 && gq == 0) p.part_lse[row] = tot > 0.f ? (m_ref[e] + log2f(tot)) * kLn2 : -CUDART_INF_F;
+          }
+        }
+      }
+    }
+  }
+}
+
+int mla_ts_smem_bytes() { return kTsSmem; }
+
+void launch_mla_ts_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st) {
+  cudaFuncSetAttribute(kam_mla_ts_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTsSmem);
+  launch_ex(kam_mla_ts_decode_kernel, g.n_ctas, kTsBlock, kTsSmem, pdl, st, g, p);
+}
+
+}  // namespace kam

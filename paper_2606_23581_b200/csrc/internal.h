@@ -117,7 +117,7 @@ struct DecodeGeom {
   int32_t KT;                    // on-read patch: 16-wide rank tiles the kernel is specialised for (0: no patch in this call)
   int32_t kv_bytes;              // bytes of the K (or V) rows of a box; box_bytes = kv_bytes + the U tile (KT > 0)
   int32_t u_off, su_row;         // U tile inside a box: [16 tokens][su_row bytes], (su_row / 16) odd
-  int32_t mla;                   // 1: absorbed MLA decode, mma.sync kernel; 2: tcgen05 kernel (no on-read patch) (one latent+rope row per token, value = its first Dv columns)
+  int32_t mla;                   // 1: absorbed MLA decode, k-split mma.sync kernel; 2: tcgen05 kernel; 3: token-split mma.sync kernel (2, 3: no on-read patch) (one latent+rope row per token, value = its first Dv columns)
   int32_t off_xch;               // MLA: shared-memory offset of the partial-score exchange buffer
 };
 
@@ -211,6 +211,9 @@ int mla_decode_occupancy(const DecodeGeom& g);
 int mla_tc_smem_bytes();
 void launch_mla_tc_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 void launch_mla_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
+// token-split mma.sync formulation (decode_mla_ts_kernel.cu): g.mla == 3, one CTA per SM, calls without an on-read patch
+int mla_ts_smem_bytes();
+void launch_mla_ts_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 
 // ---------------------------------------------------------------- form_patch (compile side, form_patch.cu)
 struct FormPatchParams {

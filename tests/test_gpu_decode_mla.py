@@ -174,3 +174,15 @@ def test_tcgen05_kernel_matches_the_oracle(monkeypatch):
     _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 85, style=reuse.INTERLEAVED)
     _run(CONFIGS[3], [[], [0, 1], [16, 0, 16], [1]], [[], [5, 7], [0, 3, -3], [4000]], 86)
     _run(CONFIGS[3].scaled(page_size=16), [[100, 500], [77]], [[9, -9], [0]], 87)          # no page-sized boxes: 16-token copies only
+
+
+def test_k_split_kernel_without_a_patch_matches_the_oracle(monkeypatch):
+    """Patch-free calls run the token-split kernel (csrc/decode_mla_ts_kernel.cu) by default, so every other test of this file
+    that carries no patch checks THAT kernel; KAM_MLA_KSPLIT=1 keeps such calls on the k-split kernel (csrc/decode_mla_kernel.cu,
+    the one the patched calls always use) - same cases as the tensor-memory test above."""
+    monkeypatch.setenv("KAM_MLA_KSPLIT", "1")
+    _run(CONFIGS[3], [[100, 1024, 37], [1024], [5, 16, 300, 700]], [[0, 3100, -77], [1024], [0, 0, -1024, 2048]], 91)
+    _run(CONFIGS[3].scaled(n_q_heads=32), [[200, 64]], [[17, 0]], 93)
+    _run(CONFIGS[3].scaled(n_q_heads=8), [[70], [130, 3]], [[-5], [0, 999]], 94)
+    _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 95, style=reuse.INTERLEAVED)
+    _run(CONFIGS[3], [[], [0, 1], [16, 0, 16], [1]], [[], [5, 7], [0, 3, -3], [4000]], 96)
