@@ -27,6 +27,8 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
+#include <type_traits>
+
 #include "common.cuh"
 #include "decode_common.cuh"
 #include "internal.h"
@@ -42,7 +44,7 @@ constexpr int kTsIter = 4;                  // boxes (16-token tiles) per full i
 constexpr int kTsSlots = 11;                // ring of boxes
 constexpr int kTsSteps = 36;                // 16-column k-steps of a 576-wide row (32 latent + 4 rope)
 constexpr int kTsBox = kDecTile * 576 * 2;  // 18432 bytes
-constexpr int kTsPRow = 48;                 // bytes of one token's row of P^T (16 heads x bf16 + 16 bytes of padding)
+constexpr int kTsPRow = 32;                 // bytes of one token's row of P^T: 16 heads x bf16, 16-byte halves swapped in rows 4-7 of 8
 constexpr int kTsPBuf = kTsIter * kDecTile * kTsPRow;
 // shared-memory map (bytes)
 constexpr int kTsOffHdr = 256;              // int4[11]
@@ -51,10 +53,11 @@ constexpr int kTsOffAlpha = 768;            // float[16 heads]: rescale factors 
 constexpr int kTsOffLsum = 1024;            // float[8 warps][8 heads]: softmax masses at the end of a segment
 constexpr int kTsOffCs = 1280;              // float2[32]: (cos, sin)(delta f_i) of the segment's chunk
 constexpr int kTsOffP = 2048;               // 2 x kTsPBuf
-constexpr int kTsOffQ = 8192;               // q of the segment: [16 heads][1152 B], as in global memory
-constexpr int kTsOffBox = kTsOffQ + kTsBox; // 26624 = 26 x 1024
-constexpr int kTsSmem = kTsOffBox + kTsSlots * kTsBox;      // 229376
-static_assert(kTsOffP + 2 * kTsPBuf <= kTsOffQ && kTsOffBox % 1024 == 0 && kTsSmem <= 227 * 1024, "shared-memory map");
+constexpr int kTsOffXch = kTsOffP + 2 * kTsPBuf;            // float[8 warps][4][32 lanes]: partial scores between the k-halves
+constexpr int kTsOffQ = kTsOffXch + 4096;   // q of the segment: [16 heads][1152 B], as in global memory
+constexpr int kTsOffBox = kTsOffQ + kTsBox; // 28672 = 28 x 1024
+constexpr int kTsSmem = kTsOffBox + kTsSlots * kTsBox;      // 231424
+static_assert(kTsOffBox % 1024 == 0 && kTsSmem <= 227 * 1024, "shared-memory map");
 enum : int { HDR_ROTATE = 8 };              // header flags beyond decode_common.cuh's; bits 16+ of the flags word: head group
 
 __device__ __forceinline__ bool bar_or(int id, bool pred) {      // barrier over the compute warps + OR of pred
@@ -165,7 +168,8 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
 
   // ================================================================ compute warps
   asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
-  const int tg = warp & 3, hh = warp >> 2;
+  const int tg = warp & 3, kh = warp >> 2;   // box of the iteration; k-half of the scores = head half of the softmax
+  const int hh = kh;
   const int gq = lane >> 2, t4 = lane & 3;
   const float scale_log2 = p.sm_scale * 1.4426950408889634f;
   constexpr float kLn2 = 0.6931471805599453f;
@@ -180,11 +184,15 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
     voff[j] = static_cast<uint32_t>(warp * 2048 + v_row * 128) + ((static_cast<uint32_t>(v_hi ^ (lane & 7)) << 4) ^ (static_cast<uint32_t>(j) << 5));
   }
   const uint32_t sm0 = smem_u32(smem);
-  // P^T: this lane's stores (token rows gq and gq + 8 of box tg, heads hh * 8 + 2 t4, +1) and its ldmatrix.trans rows
-  const uint32_t p_st = static_cast<uint32_t>(kTsOffP + (tg * kDecTile + gq) * kTsPRow + hh * 16 + t4 * 4);
-  const uint32_t p_ld = sm0 + static_cast<uint32_t>(kTsOffP + ((lane & 7) + ((lane >> 3) & 1) * 8) * kTsPRow + (lane >> 4) * 16);
+  // P^T [token][16 heads]: this lane's stores (token rows gq and gq + 8 of box tg, heads hh * 8 + 2 t4, +1) and its
+  // ldmatrix.trans rows; the two 16-byte halves of a row are swapped in rows 4-7 of every 8, so that eight rows cover all banks
+  const uint32_t p_st = static_cast<uint32_t>(kTsOffP + (tg * kDecTile + gq) * kTsPRow + ((hh ^ ((gq >> 2) & 1)) << 4) + t4 * 4);
+  const int p_row = (lane & 7) + ((lane >> 3) & 1) * 8;
+  const uint32_t p_ld = sm0 + static_cast<uint32_t>(kTsOffP + p_row * kTsPRow + (((lane >> 4) ^ ((p_row >> 2) & 1)) << 4));
+  float* xch_w = reinterpret_cast<float*>(smem + kTsOffXch) + warp * 128 + lane;          // this warp's partial scores out
+  const float* xch_r = reinterpret_cast<const float*>(smem + kTsOffXch) + (warp ^ 4) * 128 + lane;   // the other k-half's in
 
-  uint32_t qf[kTsSteps][2], ql[4][2];
+  uint32_t qf[kTsSteps / 2][2][2], ql[4][2][2];      // [k-step of this half][head tile][b0, b1]; lo: the rope k-steps (k-half 1)
   float O[2][4][4];
   float m_ref[2] = {-CUDART_INF_F, -CUDART_INF_F}, l_run[2] = {0.f, 0.f};
   bool use_lo = false;
@@ -202,29 +210,30 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
     const bool first = hdr.y & HDR_FIRST;
 
     if (first) {
-      // ---- new segment: q~ fragments of this warp's 8 heads for all 36 k-steps; the rope band rotated by -delta (hi + lo)
+      // ---- new segment: q~ fragments of all 16 heads for this warp's 18 k-steps; the rope band rotated by -delta (hi + lo)
       seg = hdr.x;
       use_lo = hdr.y & HDR_ROTATE;
       n_rows = min(kMlaHeads, g.Hq - (hdr.y >> 16) * kMlaHeads);
       mbar_wait(q_full, q_phase); q_phase ^= 1;
       const float2* cs = reinterpret_cast<const float2*>(smem + kTsOffCs);
-      // lane (gq, t4) reads 16-byte chunks 4 j + t4 of row hh * 8 + gq of the staged q; a 4 x 4
-      // transpose of 32-bit words across the quad turns four chunks into the B fragments of k-steps 2 j and 2 j + 1
-      const int row = hh * 8 + gq;
-      const uint4* qr = reinterpret_cast<const uint4*>(smem + kTsOffQ + row * 1152) + t4;
-      const bool live = row < n_rows;
+      // lane (gq, t4) reads 16-byte chunks 36 kh + 4 j + t4 (j < 9: this k-half's 18 k-steps) of rows gq and gq + 8 of the staged
+      // q; a 4 x 4 transpose of 32-bit words across the quad turns four chunks into the B fragments of k-steps 2 j and 2 j + 1.
+      // In k-half 1, j = 7 holds rope columns rel = 8 t4 .. + 7 and j = 8 their HALF-style partners rel + 32.
       const uint4 zero4 = make_uint4(0, 0, 0, 0);
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        uint4 w = live ? qr[4 * j] : zero4;
-        quad_transpose(w, t4);
-        qf[2 * j][0] = w.x; qf[2 * j][1] = w.y; qf[2 * j + 1][0] = w.z; qf[2 * j + 1][1] = w.w;
-      }
-      {
-        // rope band: chunk 64 + t4 holds columns rel = 8 t4 .. + 7, chunk 68 + t4 their HALF-style partners rel + 32
-        uint4 wx = live ? qr[64] : zero4, wy = live ? qr[68] : zero4;
+      for (int nt = 0; nt < 2; ++nt) {
+        const int row = nt * 8 + gq;
+        const uint4* qr = reinterpret_cast<const uint4*>(smem + kTsOffQ + row * 1152) + 36 * kh + t4;
+        const bool live = row < n_rows;
+#pragma unroll
+        for (int j = 0; j < 7; ++j) {
+          uint4 w = live ? qr[4 * j] : zero4;
+          quad_transpose(w, t4);
+          qf[2 * j][nt][0] = w.x; qf[2 * j][nt][1] = w.y; qf[2 * j + 1][nt][0] = w.z; qf[2 * j + 1][nt][1] = w.w;
+        }
+        uint4 wx = live ? qr[28] : zero4, wy = live ? qr[32] : zero4;
         uint4 lx = zero4, ly = zero4;
-        if (use_lo) {                                              // q~ = R(-delta) q, carried as bf16 hi + lo
+        if (kh == 1 && use_lo) {                                   // q~ = R(-delta) q, carried as bf16 hi + lo
           float x[8], y[8], rx[8], ry[8];
           unpack8(wx, x); unpack8(wy, y);
           if (g.rope_style == KAM_ROPE_HALF) {
@@ -249,10 +258,10 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
           lx = pack8(rx); ly = pack8(ry);
         }
         quad_transpose(wx, t4); quad_transpose(wy, t4); quad_transpose(lx, t4); quad_transpose(ly, t4);
-        qf[32][0] = wx.x; qf[32][1] = wx.y; qf[33][0] = wx.z; qf[33][1] = wx.w;
-        qf[34][0] = wy.x; qf[34][1] = wy.y; qf[35][0] = wy.z; qf[35][1] = wy.w;
-        ql[0][0] = lx.x; ql[0][1] = lx.y; ql[1][0] = lx.z; ql[1][1] = lx.w;
-        ql[2][0] = ly.x; ql[2][1] = ly.y; ql[3][0] = ly.z; ql[3][1] = ly.w;
+        qf[14][nt][0] = wx.x; qf[14][nt][1] = wx.y; qf[15][nt][0] = wx.z; qf[15][nt][1] = wx.w;
+        qf[16][nt][0] = wy.x; qf[16][nt][1] = wy.y; qf[17][nt][0] = wy.z; qf[17][nt][1] = wy.w;
+        ql[0][nt][0] = lx.x; ql[0][nt][1] = lx.y; ql[1][nt][0] = lx.z; ql[1][nt][1] = lx.w;
+        ql[2][nt][0] = ly.x; ql[2][nt][1] = ly.y; ql[3][nt][0] = ly.z; ql[3][nt][1] = ly.w;
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(q_empty);                       // the staging buffers may take the next segment's q
@@ -264,40 +273,64 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
       l_run[0] = l_run[1] = 0.f;
     }
 
-    // ---- S^T[16 tokens of box tg][this warp's 8 heads], complete
+    // ---- S^T[16 tokens of box tg][16 heads] over this warp's 18 k-steps; the two k-halves of a box swap the head half the
+    // other one owns (4 values per lane through shared memory, one 64-thread barrier): complete scores of 8 heads per warp
     float s[4] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
     const int my_box = slot_of(tg);
     if (tg < nb) {
       if (tg) mbar_wait(&full_bar[my_box], phase_of(tg));
       const int4 h2 = hdrs[my_box];
       const uint32_t kb = sm0 + static_cast<uint32_t>(kTsOffBox + my_box * kTsBox);
-      // a 64-column block = 4 k-steps: the fragments of block c + 1 are fetched while the MMAs of block c run, and k-step k
-      // accumulates into chain k & 3 (a dependent HMMA would wait out the previous one's latency)
-      float sc[4][4];
+      float sc[2][2][4];                                           // [head tile][chain: k-step parity]
 #pragma unroll
-      for (int c = 0; c < 4; ++c) sc[c][0] = sc[c][1] = sc[c][2] = sc[c][3] = 0.f;
-      {
-        uint32_t a[2][4][4];
+      for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
-        for (int k = 0; k < 4; ++k) ldmatrix_x4(a[0][k][0], a[0][k][1], a[0][k][2], a[0][k][3], kb + koff[k]);
+        for (int c = 0; c < 2; ++c) sc[nt][c][0] = sc[nt][c][1] = sc[nt][c][2] = sc[nt][c][3] = 0.f;
+      auto qk_half = [&](auto KH) {
+        constexpr int H = decltype(KH)::value;                     // compile-time k-half: every ldmatrix address is base + immediate
+        constexpr int NB6 = 3;                                     // 18 k-steps in 3 batches of 6: batch c + 1 is fetched under the MMAs of batch c
+        uint32_t a[2][6][4];
 #pragma unroll
-        for (int c = 0; c < 9; ++c) {
-          if (c + 1 < 9) {
+        for (int k = 0; k < 6; ++k) {
+          const int c = 18 * H + k;
+          ldmatrix_x4(a[0][k][0], a[0][k][1], a[0][k][2], a[0][k][3], kb + koff[c & 3] + (c >> 2) * 2048);
+        }
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-              ldmatrix_x4(a[(c + 1) & 1][k][0], a[(c + 1) & 1][k][1], a[(c + 1) & 1][k][2], a[(c + 1) & 1][k][3], kb + koff[k] + (c + 1) * 2048);
+        for (int bt6 = 0; bt6 < NB6; ++bt6) {
+          if (bt6 + 1 < NB6) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) {
+              const int c = 18 * H + 6 * (bt6 + 1) + k;
+              ldmatrix_x4(a[(bt6 + 1) & 1][k][0], a[(bt6 + 1) & 1][k][1], a[(bt6 + 1) & 1][k][2], a[(bt6 + 1) & 1][k][3], kb + koff[c & 3] + (c >> 2) * 2048);
+            }
           }
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const uint32_t* f = a[c & 1][k];
-            mma_bf16_16816(sc[k][0], sc[k][1], sc[k][2], sc[k][3], f[0], f[1], f[2], f[3], qf[4 * c + k][0], qf[4 * c + k][1]);
-            if (c == 8 && use_lo) mma_bf16_16816(sc[(k + 2) & 3][0], sc[(k + 2) & 3][1], sc[(k + 2) & 3][2], sc[(k + 2) & 3][3], f[0], f[1], f[2], f[3], ql[k][0], ql[k][1]);
+          for (int k = 0; k < 6; ++k) {
+            const int i = 6 * bt6 + k;
+            const uint32_t* f = a[bt6 & 1][k];
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) {
+              mma_bf16_16816(sc[nt][i & 1][0], sc[nt][i & 1][1], sc[nt][i & 1][2], sc[nt][i & 1][3], f[0], f[1], f[2], f[3], qf[i][nt][0], qf[i][nt][1]);
+              if (H == 1 && i >= 14 && use_lo)
+                mma_bf16_16816(sc[nt][(i & 1) ^ 1][0], sc[nt][(i & 1) ^ 1][1], sc[nt][(i & 1) ^ 1][2], sc[nt][(i & 1) ^ 1][3], f[0], f[1], f[2], f[3], ql[i - 14][nt][0], ql[i - 14][nt][1]);
+            }
           }
         }
+      };
+      if (kh) qk_half(std::integral_constant<int, 1>{}); else qk_half(std::integral_constant<int, 0>{});
+      float own[4], oth[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const float s0 = sc[0][0][e] + sc[0][1][e], s1 = sc[1][0][e] + sc[1][1][e];
+        own[e] = kh ? s1 : s0;
+        oth[e] = kh ? s0 : s1;
       }
+#pragma unroll
+      for (int e = 0; e < 4; ++e) xch_w[e * 32] = oth[e];
+      named_bar_sync(4 + tg, 64);
       float sa[4], sb[4];
 #pragma unroll
-      for (int e = 0; e < 4; ++e) { sa[e] = sc[0][e] + sc[1][e]; sb[e] = sc[2][e] + sc[3][e]; }
+      for (int e = 0; e < 4; ++e) { sa[e] = own[e]; sb[e] = xch_r[e * 32]; }
       const bool partial = h2.y & HDR_PARTIAL;
       const int row_lo = h2.z & 0xff, row_hi = h2.z >> 8;
       const bool ok0 = !partial || (gq >= row_lo && gq < row_hi);
