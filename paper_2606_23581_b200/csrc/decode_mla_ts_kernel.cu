@@ -146,9 +146,13 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
             const int tl = t0 + i0 + lane;
             const int tok = (S.tile0 + tl) * kDecTile;
             const int row_lo = max(S.tok_lo - tok, 0), row_hi = min(S.tok_hi - tok, kDecTile);
-            const int flags = ((lane == 0 && tl == 0) ? HDR_FIRST : 0) | ((lane == 0 && t0 + i0 + nb >= S.n_tiles) ? HDR_LAST : 0) |
+            const int flags = ((t0 + i0 == 0) ? HDR_FIRST : 0) | ((t0 + i0 + nb >= S.n_tiles) ? HDR_LAST : 0) |     // of the ITERATION, in all its headers
                               ((row_lo > 0 || row_hi < kDecTile) ? HDR_PARTIAL : 0) | (S.rotate ? HDR_ROTATE : 0) | (S.hg << 16);
-            hdrs[sl] = make_int4(seg, flags, row_lo | (row_hi << 8), nb);
+            // .w: boxes of this iteration | boxes of the NEXT one << 8 (0: the CTA's work ends) - the compute warps then know which
+            // barriers to look at before any header of that iteration is readable (the plan emits no empty segment)
+            const int rem = S.n_tiles - (t0 + i0 + nb);
+            const int nb_next = rem > 0 ? min(kTsIter, rem) : (seg + 1 < seg_end ? min(kTsIter, S_next.n_tiles) : 0);
+            hdrs[sl] = make_int4(seg, flags, row_lo | (row_hi << 8), nb | (nb_next << 8));
             mbar_arrive_expect_tx(&full_bar[sl], static_cast<uint32_t>(kTsBox));
             tma_load_3d(smem + kTsOffBox + sl * kTsBox, tm_k, 0, s0, 0, &full_bar[sl]);
           }
@@ -157,11 +161,6 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
           if (slot >= kTsSlots) { slot -= kTsSlots; phase ^= 1; }
         }
       }
-    }
-    if (lane == 0) {
-      mbar_wait(&empty_bar[slot], phase ^ 1);
-      hdrs[slot] = make_int4(-1, 0, 0, 0);
-      mbar_arrive(&full_bar[slot]);
     }
     return;
   }
@@ -201,12 +200,15 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
   // ring slot j of the current iteration (slots slot .. slot + 3, wrapping) and its mbarrier parity
   auto slot_of = [&](int j) { const int sl = slot + j; return sl >= kTsSlots ? sl - kTsSlots : sl; };
   auto phase_of = [&](int j) { return slot + j >= kTsSlots ? (phase ^ 1u) : phase; };
-  while (true) {
-    const int leader = slot;
-    mbar_wait(&full_bar[leader], phase);
-    const int4 hdr = hdrs[leader];
-    if (hdr.x < 0) break;
-    const int nb = hdr.w;
+  mbar_wait(&full_bar[0], 0);                                    // bootstrap: the first iteration's header tells its own size
+  int nb = hdrs[0].w & 0xff;
+  while (nb > 0) {
+    // a try_wait costs ~100+ cycles even when the phase is long complete, so a warp waits ONCE here: for its own box, whose
+    // header repeats the iteration's fields (a warp without a box in a short iteration waits for the first one)
+    const int my_box = slot_of(tg < nb ? tg : 0);
+    mbar_wait(&full_bar[my_box], phase_of(tg < nb ? tg : 0));
+    const int4 hdr = hdrs[my_box];
+    const int nb_next = (hdr.w >> 8) & 0xff;
     const bool first = hdr.y & HDR_FIRST;
 
     if (first) {
@@ -276,10 +278,8 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
     // ---- S^T[16 tokens of box tg][16 heads] over this warp's 18 k-steps; the two k-halves of a box swap the head half the
     // other one owns (4 values per lane through shared memory, one 64-thread barrier): complete scores of 8 heads per warp
     float s[4] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
-    const int my_box = slot_of(tg);
     if (tg < nb) {
-      if (tg) mbar_wait(&full_bar[my_box], phase_of(tg));
-      const int4 h2 = hdrs[my_box];
+      const int4 h2 = hdr;
       const uint32_t kb = sm0 + static_cast<uint32_t>(kTsOffBox + my_box * kTsBox);
       float sc[2][2][4];                                           // [head tile][chain: k-step parity]
 #pragma unroll
@@ -404,14 +404,15 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
       const uint32_t pl = p_ld + static_cast<uint32_t>(pbuf * kTsPBuf);
       const uint32_t box0 = sm0 + static_cast<uint32_t>(kTsOffBox);
       if (nb == kTsIter) {
-        // full iteration, straight-line: every box landed (its owner waited before the barrier; this wait orders OUR reads),
+        // full iteration, straight-line,
         // P^T fragments of all four k-steps up front, V^T fragments of box j + 1 fetched under the MMAs of box j
+        // the other boxes: their owners waited for them before the barrier above, this look orders OUR reads - lanes 0-3 take one
+        // barrier each (one pass instead of three waits in a row), __syncwarp orders the other lanes behind them
+        if (lane < kTsIter && lane != tg) mbar_wait(&full_bar[slot_of(lane)], phase_of(lane));
+        __syncwarp();
         uint32_t vb[kTsIter];
 #pragma unroll
-        for (int j = 0; j < kTsIter; ++j) {
-          if (j != tg) mbar_wait(&full_bar[slot_of(j)], phase_of(j));
-          vb[j] = box0 + static_cast<uint32_t>(slot_of(j) * kTsBox);
-        }
+        for (int j = 0; j < kTsIter; ++j) vb[j] = box0 + static_cast<uint32_t>(slot_of(j) * kTsBox);
         uint32_t b[kTsIter][4];
 #pragma unroll
         for (int j = 0; j < kTsIter; ++j) ldmatrix_x4_trans(b[j][0], b[j][1], b[j][2], b[j][3], pl + j * (kDecTile * kTsPRow));
@@ -455,6 +456,7 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
     pbuf ^= 1;
     slot += nb;
     if (slot >= kTsSlots) { slot -= kTsSlots; phase ^= 1; }
+    nb = nb_next;
 
     if (hdr.y & HDR_LAST) {
       // ---- the segment's softmax state -> partials: o normalised, lse in natural log
