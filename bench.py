@@ -420,6 +420,7 @@ def extras(wl, device, peak):
     nbytes = nb3 * nch3 * T3 * D3 * 2
     out["mla_decode_absorbed"] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak,
                                   "bytes": "every latent+rope row once (it is both key and value)", "batch": nb3, "tokens": nch3 * T3,
+                                  "what": "stateless call = plan + kam_mla_ts_decode_kernel (token-split) + merge",
                                   "tflops": nb3 * nch3 * T3 * c3.n_q_heads * (D3 + c3.v_dim) * 2 / ms / 1e9}
     ctx3.close()
     return out

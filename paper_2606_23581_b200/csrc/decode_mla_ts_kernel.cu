@@ -2,28 +2,38 @@
 // and merge as decode_mla_kernel.cu (which still takes the calls that carry an on-read patch); this is the kernel the
 // patch-free calls run.
 //
-// Why a second mma.sync formulation: decode_mla_kernel.cu splits the 576-deep contraction over four warps, so every 16-token
-// tile costs a shared-memory exchange of partial scores, a CTA barrier and a softmax repeated in all four warps - ncu
-// (profiles/ncu_extras_r01.md) shows ~600 instructions per warp and tile and a kernel bound by that chain (tensor pipe 29 %,
-// issue slots 42 %, DRAM 58 %).  Here one ITERATION is 64 tokens (four 16-token TMA boxes) and the work is split by TOKENS:
+// Why a second mma.sync formulation: decode_mla_kernel.cu splits the 576-deep contraction over four warps for EVERY 16-token
+// tile, so each tile costs a shared-memory exchange of partial scores, a CTA barrier and a softmax repeated in all four
+// warps - ncu (profiles/ncu_extras_r01.md) shows ~600 instructions per warp and tile.  Here one ITERATION is 64 tokens (four
+// 16-token TMA boxes) and the work is split by TOKENS first:
 //
-//   warp w of 8:  tg = w & 3 (which box), hh = w >> 2 (which 8 of the 16 query heads)
-//   S^T[16 tokens][8 heads] = K_box q~^T   : all 36 k-steps in this one warp (q~ fragments live in 72 registers), so the
-//                                           scores are complete - no exchange; softmax values are computed once, not 4x
-//   P^T (bf16) -> shared memory [64 tokens][16 heads] (48-byte rows: conflict-free stores and ldmatrix.trans)
-//   ONE barrier per iteration (barrier.red.or: also tells whether any score ran 2^8 past its head's reference)
+//   warp w of 8:  tg = w & 3 (which box of the iteration), kh = w >> 2 (which half of the contraction / of the heads)
+//   S^T[16 tokens of box tg][16 heads] over k-steps [18 kh, 18 kh + 18): 18 ldmatrix + 36 HMMA, q~ fragments in 72 registers;
+//     the two warps of a box swap the head half the other one owns (4 floats per lane, one 64-thread barrier), so each warp
+//     ends with COMPLETE scores of 8 heads x 16 tokens and every softmax value is computed once
+//   P^T (bf16) -> shared memory [64 tokens][16 heads]
+//   ONE CTA barrier per iteration (barrier.red.or: it also tells whether any score ran 2^8 past its head's reference)
 //   O^T[64 w .. 64 w + 64][16 heads] += V^T P^T over the iteration's 64 tokens: warp w owns 64-column block w of every box
 //
 // The reference of the lazy softmax (decode_kernel.cu) is common to the CTA and moves only through a slow path (two more
 // barriers: tile maxima -> new references, rescale factors -> O), taken on the first iteration of a segment and then rarely.
-// Per warp and 64 tokens: 68 HMMA, 56 LDSM, ~250 instructions in all (the k-split kernel: ~1200).
+// Per warp and 64 tokens: 68 HMMA, 38 LDSM, ~250 instructions in all (the k-split kernel: ~1200).
 // CTA = 8 compute warps + 1 producer warp (slot mapping A1 + one TMA box [9 x 64 columns][16 tokens][128 B swizzled] per
-// tile), one CTA per SM, flat ring of 11 boxes (an iteration takes the next 1-4 slots).
+// tile) inside a third warpgroup that gives its registers away (setmaxnreg: 12 warps launch at 168 registers, the compute
+// warps run at 232, the producer at 40).  One CTA per SM, flat ring of 11 boxes (an iteration takes the next 1-4 slots).
 //
-// The compute warps never load from global memory.  Measured on B200: with ~200 KB of bulk copies in flight per SM, a demand
-// load from the same SM waits microseconds (it queues behind them), and two dependent ones per segment (the segment record,
-// then q) cost 28 of 133 us.  So the producer also stages q (16 rows x 1152 B, one bulk copy) and the chunk's (cos, sin) row
-// into shared memory IN the stream, right before the segment's first box, and the segment's fields ride in the box header.
+// Two things measured on B200 while building this (both shaped the code, both are in DESIGN.md 7.2):
+//  * With ~200 KB of bulk copies in flight per SM, a DEMAND load from the same SM waits microseconds (it queues behind them);
+//    two dependent ones per segment (the segment record, then q) cost 28 of 133 us.  So the compute warps never load from
+//    global memory: the producer stages q (16 rows x 1152 B, one bulk copy) and the chunk's (cos, sin) row into shared memory
+//    IN the copy stream, right before the segment's first box, and the segment's fields ride in the box headers.
+//  * mbarrier.try_wait costs 100+ cycles even on a phase that completed long ago.  Three of them in a row before PV (the boxes
+//    of the other warps) cost 11 of 123 us; so a warp waits ONCE per iteration (its own box, whose header repeats the
+//    iteration's fields and the next iteration's size) and lanes 0-3 check the other boxes' barriers in one pass before PV.
+//    (Doing that one-pass check where the data may really be late - at the top of the iteration - is slow: the lanes spin
+//    one after the other.)
+// Measured and rejected: computing the next iteration's scores inside this iteration's PV (two independent ldmatrix -> HMMA
+// streams per warp): 123 -> 133 us, whether or not it waited for the next boxes.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
