@@ -217,7 +217,8 @@ kam_status kam_get_stats(kam_ctx *ctx, kam_stats *out);
  * For request b, query head hq (KV head h = hq / G), over all chunks c of the request:
  *     k^_t = R(chunk_offsets[b][c]) k_t (+ U_k W_k)   v^_t = v_t (+ U_v W_v)          read from the pool, never written
  *     s_t = sm_scale * q . k^_t ;  per chunk (o_c, lse_c) ;  lse = ln sum_c e^{lse_c} ;  out = sum_c e^{lse_c - lse} o_c
- * q [batch][n_q_heads][row_dim] bf16 device.  block_tables device int32 [batch][max_pages].  chunk_starts device
+ * q [batch][n_q_heads][row_dim] bf16 device, 16-byte aligned like out (q rows travel as bulk copies; else INVALID_ARG).
+ * block_tables device int32 [batch][max_pages].  chunk_starts device
  * int32 [batch][max_chunks+1] (CSR token boundaries; only differences to chunk_starts[b][0] are used).
  * chunk_offsets device int64 [batch][max_chunks] (delta to apply on read; 0 if materialised) or NULL (= all 0).
  * n_chunks device int32 [batch].  patches: NULL, or device kam_patch_ref [batch][max_chunks]: the rank-m patch of Eq. 1

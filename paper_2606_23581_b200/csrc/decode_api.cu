@@ -177,6 +177,7 @@ static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* po
   kam_status s = check_pool(c, &pool);
   if (s != KAM_OK) return s;
   if (!q || !block_tables || !chunk_starts || !n_chunks || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge: NULL argument");
+  if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge: q and out must be 16-byte aligned");
   if (layer < 0 || layer >= c->lay.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, c->lay.n_layers);
   if (batch < 0 || max_pages < 1 || max_chunks < 1) return fail(c, KAM_ERR_INVALID_ARG, "bad batch / max_pages / max_chunks");
   if (batch == 0) return KAM_OK;
@@ -336,6 +337,7 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   if (!c) return KAM_ERR_INVALID_ARG;
   if (batch == 0) return KAM_OK;
   if (!q || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_window_decode: NULL argument");
+  if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(c, KAM_ERR_INVALID_ARG, "kam_window_decode: q and out must be 16-byte aligned");
   if (layer < 0 || layer >= c->lay.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, c->lay.n_layers);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   DecodeGeom g; WsLayout w; bool cached;

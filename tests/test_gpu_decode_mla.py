@@ -186,3 +186,32 @@ def test_k_split_kernel_without_a_patch_matches_the_oracle(monkeypatch):
     _run(CONFIGS[3].scaled(n_q_heads=8), [[70], [130, 3]], [[-5], [0, 999]], 94)
     _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 95, style=reuse.INTERLEAVED)
     _run(CONFIGS[3], [[], [0, 1], [16, 0, 16], [1]], [[], [5, 7], [0, 3, -3], [4000]], 96)
+
+
+def test_token_split_kernel_shapes_its_iterations_do_not_divide():
+    """Shapes that stress the token-split kernel's own structure (64-token iterations over a ring of 11 boxes, q staged per
+    segment): a second head tile with 8 live rows of 16, 16-token pages (every box its own page), and runs of segments
+    shorter than one iteration - the producer then stages the next q while the previous segment's boxes are still unread."""
+    _run(CONFIGS[3].scaled(n_q_heads=24), [[200, 64, 1000], [333]], [[17, 0, -4], [5]], 101)
+    _run(CONFIGS[3].scaled(page_size=16), [[100, 500, 64, 48], [77]], [[9, -9, 0, 3], [0]], 102)
+    tiny = [[16, 33, 48, 7, 64, 20, 16, 95, 1, 40] * 3, [48] * 12]
+    _run(CONFIGS[3], tiny, [[(7 * i) % 5 - 2 for i in range(30)], [0] * 12], 103)
+    _run(CONFIGS[3], [[4096 + 50], [3000, 3000]], [[123], [0, -3000]], 104)          # long segments: many ring wraps
+
+
+def test_misaligned_query_is_refused():
+    """q rows travel as 16-byte-granular bulk copies: a query pointer off a 16-byte boundary is INVALID_ARG, not a fault."""
+    cfg = CONFIGS[3]
+    pool = _latent_pool(cfg, 1, 4, 7)
+    ctx = kam.Context(par.layout_of(cfg, 1), pool)
+    qbuf = torch.zeros(cfg.n_q_heads * cfg.row_dim + 8, dtype=torch.bfloat16, device="cuda")
+    q = qbuf[1:1 + cfg.n_q_heads * cfg.row_dim].view(1, cfg.n_q_heads, cfg.row_dim)      # 2 bytes off
+    bt = torch.zeros((1, 4), dtype=torch.int32, device="cuda")
+    st = torch.tensor([[0, 64]], dtype=torch.int32, device="cuda")
+    nc = torch.ones(1, dtype=torch.int32, device="cuda")
+    out = torch.zeros((1, cfg.n_q_heads, cfg.v_dim), dtype=torch.bfloat16, device="cuda")
+    lse = torch.zeros((1, cfg.n_q_heads), dtype=torch.float32, device="cuda")
+    with pytest.raises(B.KameraError) as e:
+        ctx.kam_paged_decode_merge(q, bt, st, None, nc, 0, 0.1, out, lse)
+    assert e.value.status == B.KAM_ERR_INVALID_ARG
+    ctx.close()
