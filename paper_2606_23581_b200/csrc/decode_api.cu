@@ -207,10 +207,13 @@ static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* po
   csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
   csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = patches ? 1 : 0;
   launch_decode_plan(g, p.plan, csr, st);
-  if (g.mla == 3) launch_mla_ts_decode(g, p, false, st);
+  // the decode kernels read the plan just written: with programmatic dependent launch only their prologue (barrier setup,
+  // shared-memory carve-up, launch latency) overlaps the plan kernel - plan_fresh makes them wait before the first plan read
+  p.plan_fresh = 1;
+  if (g.mla == 3) launch_mla_ts_decode(g, p, c->use_pdl, st);
   else if (g.mla == 2) launch_mla_tc_decode(g, p, false, st);
-  else if (g.mla) launch_mla_decode(g, p, false, st);
-  else launch_decode(g, p, false, st);                            // reads the plan just written: plain stream order
+  else if (g.mla) launch_mla_decode(g, p, c->use_pdl, st);
+  else launch_decode(g, p, c->use_pdl, st);
   launch_decode_merge(g, p, c->use_pdl, st);
   c->kernels_launched += 3;
   cudaError_t e = cudaGetLastError();

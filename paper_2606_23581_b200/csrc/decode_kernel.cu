@@ -90,6 +90,7 @@ __global__ void __launch_bounds__(kDecPlanThreads) kam_decode_plan_kernel(const 
   __shared__ int sh[32];
   const int tid = threadIdx.x;
   const int N = pl.n_chunks;
+  grid_dep_launch();                                            // the decode kernel may set itself up while this one runs
 
   if (blockIdx.x > 0) {
     // ---- A2 for decode: (cos, sin)(delta f_i) per (chunk, frequency); the angle is formed in fp64 (R-18)
@@ -222,6 +223,7 @@ kam_paged_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_const
   __syncthreads();
 
   grid_dep_launch();
+  if (p.plan_fresh) grid_dep_wait();                             // the plan comes from the kernel right before this one
   const int seg_begin = p.plan.cta_seg[blockIdx.x], seg_end = p.plan.cta_seg[blockIdx.x + 1];
   if (seg_begin >= seg_end) return;
 
@@ -704,6 +706,9 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
   __shared__ float sm_m[kMergeWarps], sm_l[kMergeWarps];
   __shared__ float sm_acc[kMergeWarps][32 * CPL];
   grid_dep_launch();
+  // stateless call: the decode kernel before this one may itself have started under the plan kernel (it signals its dependents
+  // at once), so the plan is only safe to read once the decode kernel - and with it the plan kernel - has completed
+  if (p.plan_fresh) grid_dep_wait();
   const int bh = blockIdx.x;                      // b * Hq + hq
   const int b = bh / g.Hq, hq = bh - b * g.Hq;
   const int hg = hq / g.R, r = hq - hg * g.R;

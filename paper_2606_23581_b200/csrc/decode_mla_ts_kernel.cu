@@ -110,6 +110,7 @@ kam_mla_ts_decode_kernel(const __grid_constant__ DecodeGeom g, const __grid_cons
   __syncthreads();
 
   grid_dep_launch();
+  if (p.plan_fresh) grid_dep_wait();                             // the plan comes from the kernel right before this one
   const int seg_begin = p.plan.cta_seg[blockIdx.x], seg_end = p.plan.cta_seg[blockIdx.x + 1];
   if (seg_begin >= seg_end) return;
 

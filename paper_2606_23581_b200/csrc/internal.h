@@ -169,6 +169,8 @@ struct DecodeParams {
   void* out;                     // [B][Hq][Dv] bf16 (f32 when out_f32: a softmax STATE for a later cross-rank merge)
   float* lse;                    // [B][Hq]
   int32_t out_f32;
+  int32_t plan_fresh;            // 1: the plan is written by the kernel just before this one on the stream (stateless call):
+                                 // nothing of it may be read before griddepcontrol.wait
 };
 
 // merge of n_parts softmax states (o_p f32 [rows][Dv], lse_p f32 [rows]) of the same queries, e.g. one per rank of a
