@@ -327,7 +327,8 @@ def _time_ms(torch, fn, reps):
 def extras(wl, device, peak):
     """Measured after the timed region, NOT part of the step or of `value`: the paper's "rank-invariant in latency" claim
      as a rank sweep of the relocate kernel on config 2's shape, the rank-m patch applied ON READ inside the decode
-    (row A8's second form), and the MLA instantiation (config 3's shape): relocate+patch and absorbed decode.  Every
+    (row A8's second form), the decode on the shapes of configs 4 and 5 (2.3 / 4.3 GB per layer instead of config 2's 0.54 GB),
+    and the MLA instantiation (config 3's shape): relocate+patch and absorbed decode.  Every
     figure is algorithmic bytes / device time, as a fraction of the measured HBM peak."""
     import torch
     kam, B, cfg = wl.kam, wl.B, wl.cfg
@@ -383,6 +384,31 @@ def extras(wl, device, peak):
         out[name] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak,
                      "bytes": "K + V" + (" + U_k + U_v" if pr else "") + " once; on-read rotation by a pending offset in both"}
     del refs
+
+    # ---- the decode kernel on the other configs' shapes (stateless call, no patch, two resident layers): a layer of config 2 is
+    # 0.54 GB, so plan / ramp / merge weigh ~15 %; configs 4 and 5 read 2.3 and 4.3 GB per layer
+    for name, cid, nreq, nch, Tc in (("decode_config4_shape_b32_4352tok", 4, 32, 4, 1088), ("decode_config5_shape_b64_16384tok", 5, 64, 8, 2048)):
+        cx = CONFIGS[cid]
+        Hx, Dx, Px, Lx = cx.n_kv_heads, cx.row_dim, cx.page_size, 2
+        pprx = nch * Tc // Px
+        poolx = kam.Pool([rnd((nreq * pprx, Px, Hx, Dx)) for _ in range(Lx)], [rnd((nreq * pprx, Px, Hx, Dx)) for _ in range(Lx)])
+        ctxx = kam.Context(kam.make_layout(B.KAM_MHA if cx.n_q_heads == Hx else B.KAM_GQA, Lx, cx.n_q_heads, Hx, Dx, 0, Dx, True, Px, cx.theta), poolx)
+        btx = torch.randperm(nreq * pprx, device=device, dtype=torch.int32).reshape(nreq, pprx)
+        stx = torch.arange(0, (nch + 1) * Tc, Tc, dtype=torch.int32, device=device).repeat(nreq, 1)
+        ncx = torch.full((nreq,), nch, dtype=torch.int32, device=device)
+        qx = rnd((nreq, cx.n_q_heads, Dx))
+        ox, lx = torch.zeros_like(qx), torch.zeros((nreq, cx.n_q_heads), dtype=torch.float32, device=device)
+        it = [0]
+
+        def launch():
+            it[0] += 1
+            ctxx.kam_paged_decode_merge(qx, btx, stx, None, ncx, it[0] % Lx, Dx ** -0.5, ox, lx)
+        ms = _time_ms(torch, launch, 6)
+        nbytes = nreq * nch * Tc * Hx * 2 * Dx * 2
+        out[name] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak, "bytes": "K + V once",
+                     "what": "stateless call = plan + kam_paged_decode_kernel + merge; %d q / %d kv heads" % (cx.n_q_heads, Hx)}
+        ctxx.close()
+        del poolx, ctxx, btx, qx, ox
 
     # ---- MLA (config 3 shape): relocate+patch of 4 chunks x 27 layers in one launch; absorbed decode, batch 64 x 8192 tokens
     c3 = CONFIGS[3]
