@@ -698,14 +698,14 @@ void launch_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStr
 // A9: lse = ln sum_s e^{lse_s};  out = sum_s e^{lse_s - lse} o_s over the request's segments of this head's group.
 // One CTA per (request, query head); warp w folds segments s0 + w, s0 + w + 8, ... (four independent loads in flight per
 // lane), then the 8 warp states are folded in warp order.  Fixed assignment and order => run-to-run deterministic.
-constexpr int kMergeWarps = 8;
-constexpr int kMergeUnroll = 4;
 
-template <int CPL>   // columns per lane = Dv / 32
-__global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
-  __shared__ float sm_m[kMergeWarps], sm_l[kMergeWarps];
-  __shared__ float sm_acc[kMergeWarps][32 * CPL];
-  grid_dep_launch();
+// CPL: columns per lane = Dv / 32.  WARPS x UNROLL segments are in flight per CTA; the three instantiations are sized so that
+// the whole grid (one CTA per query head) is resident at once: a second wave would repeat the kernel's latency chain (plan read
+// -> partials read -> reduce -> write), which is all this kernel's time (measured: 896 CTAs at 5 per SM = 2 waves, 9.7 us).
+template <int CPL, int WARPS, int UNROLL, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) kam_lse_merge_kernel(const __grid_constant__ DecodeGeom g, const __grid_constant__ DecodeParams p) {
+  __shared__ float sm_m[WARPS], sm_l[WARPS];
+  __shared__ float sm_acc[WARPS][32 * CPL];
   // stateless call: the decode kernel before this one may itself have started under the plan kernel (it signals its dependents
   // at once), so the plan is only safe to read once the decode kernel - and with it the plan kernel - has completed
   if (p.plan_fresh) grid_dep_wait();
@@ -716,6 +716,10 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
   const int s0 = p.plan.seg_base[hg * N + p.plan.rcb[b]], s1 = p.plan.seg_base[hg * N + p.plan.rcb[b + 1]];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   grid_dep_wait();                                // the partials are complete and visible from here
+  // the next kernel on the stream (the next layer's decode) is released only now: released at the top of this kernel its CTAs
+  // become resident during the TAIL of the decode before this merge and hold SM slots its last CTAs' merge needs - measured
+  // with the whole merge grid resident at once: 28 layers 3.08 ms instead of 2.71 ms
+  grid_dep_launch();
   const float* pl = p.part_lse + r;
   const float* po = p.part_o + static_cast<size_t>(r) * g.Dv + lane * CPL;
   const size_t so = static_cast<size_t>(g.R) * g.Dv;
@@ -723,11 +727,11 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
   float m = -CUDART_INF_F, l = 0.f, acc[CPL];
 #pragma unroll
   for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
-  for (int base = s0 + warp; base < s1; base += kMergeWarps * kMergeUnroll) {
-    float ls[kMergeUnroll], o[kMergeUnroll][CPL];
+  for (int base = s0 + warp; base < s1; base += WARPS * UNROLL) {
+    float ls[UNROLL], o[UNROLL][CPL];
 #pragma unroll
-    for (int u = 0; u < kMergeUnroll; ++u) {
-      const int s = base + u * kMergeWarps;
+    for (int u = 0; u < UNROLL; ++u) {
+      const int s = base + u * WARPS;
       ls[u] = -CUDART_INF_F;
 #pragma unroll
       for (int c = 0; c < CPL; ++c) o[u][c] = 0.f;
@@ -743,7 +747,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
       }
     }
 #pragma unroll
-    for (int u = 0; u < kMergeUnroll; ++u) {
+    for (int u = 0; u < UNROLL; ++u) {
       if (ls[u] == -CUDART_INF_F) continue;
       const float mn = fmaxf(m, ls[u]);
       const float a = __expf(m - mn), w = __expf(ls[u] - mn);
@@ -760,24 +764,24 @@ __global__ void __launch_bounds__(kMergeWarps * 32) kam_lse_merge_kernel(const _
 
   float M = -CUDART_INF_F;
 #pragma unroll
-  for (int w = 0; w < kMergeWarps; ++w) M = fmaxf(M, sm_m[w]);
+  for (int w = 0; w < WARPS; ++w) M = fmaxf(M, sm_m[w]);
   __nv_bfloat16* out = static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(bh) * g.Dv;
   float* outf = static_cast<float*>(p.out) + static_cast<size_t>(bh) * g.Dv;
   if (M == -CUDART_INF_F) {                       // no tokens at all: out = 0, lse = -inf, no NaN
-    for (int c = threadIdx.x; c < g.Dv; c += kMergeWarps * 32) { if (p.out_f32) outf[c] = 0.f; else out[c] = __float2bfloat16_rn(0.f); }
+    for (int c = threadIdx.x; c < g.Dv; c += WARPS * 32) { if (p.out_f32) outf[c] = 0.f; else out[c] = __float2bfloat16_rn(0.f); }
     if (threadIdx.x == 0) p.lse[bh] = -CUDART_INF_F;
     return;
   }
-  float tot = 0.f, ew[kMergeWarps];
+  float tot = 0.f, ew[WARPS];
 #pragma unroll
-  for (int w = 0; w < kMergeWarps; ++w) {
+  for (int w = 0; w < WARPS; ++w) {
     ew[w] = sm_m[w] == -CUDART_INF_F ? 0.f : __expf(sm_m[w] - M);
     tot = fmaf(sm_l[w], ew[w], tot);
   }
-  for (int c = threadIdx.x; c < g.Dv; c += kMergeWarps * 32) {
+  for (int c = threadIdx.x; c < g.Dv; c += WARPS * 32) {
     float v = 0.f;
 #pragma unroll
-    for (int w = 0; w < kMergeWarps; ++w) v = fmaf(sm_acc[w][c], ew[w], v);
+    for (int w = 0; w < WARPS; ++w) v = fmaf(sm_acc[w][c], ew[w], v);
     if (p.out_f32) outf[c] = v / tot; else out[c] = __float2bfloat16_rn(v / tot);
   }
   if (threadIdx.x == 0) p.lse[bh] = M + logf(tot);
@@ -814,9 +818,10 @@ void launch_state_merge(const StateMergeParams& p, cudaStream_t st) {
 }
 
 void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st) {
-  if (g.Dv == 512)      launch_ex(kam_lse_merge_kernel<16>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
-  else if (g.Dv == 128) launch_ex(kam_lse_merge_kernel<4>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
-  else                  launch_ex(kam_lse_merge_kernel<2>, p.plan.batch * g.Hq, kMergeWarps * 32, 0, pdl, st, g, p);
+  const int grid = p.plan.batch * g.Hq;
+  if (g.Dv == 512)      launch_ex(kam_lse_merge_kernel<16, 4, 2, 7>, grid, 128, 0, pdl, st, g, p);
+  else if (g.Dv == 128) launch_ex(kam_lse_merge_kernel<4, 4, 4, 8>, grid, 128, 0, pdl, st, g, p);
+  else                  launch_ex(kam_lse_merge_kernel<2, 4, 4, 8>, grid, 128, 0, pdl, st, g, p);
 }
 
 }  // namespace kam
