@@ -6,6 +6,8 @@
 // so every cached byte is read ONCE and serves both QK^T and PV.  Relocation on read touches only q_pe (q~ = R(-delta) q on
 // the rope band, bf16 hi + lo); the rank-m patch on read is one U (the key's): s_t += U[t,:].(W q),  o += (sum_t p_t U[t,:]) W[:, 0:512].
 //
+// This k-split kernel carries the calls WITH an on-read patch (and KAM_MLA_KSPLIT=1); patch-free calls run the token-split kernel
+// (decode_mla_ts_kernel.cu), which is faster (0.129 vs 0.152 ms per layer at batch 64 x 8192 tokens).
 // Same plan, partials and merge as the GQA kernel (decode_kernel.cu).  Work unit = (16 query heads, run of 16-token tiles of
 // one chunk).  CTA = 1 producer warp (slot mapping A1 + one TMA box [9 x 64 columns][16 tokens][128 B, swizzled] per tile) +
 // 4 compute warps.  30 flop per byte is ~35 % of the mma.sync rate at the HBM roofline, so nothing may be computed twice:
