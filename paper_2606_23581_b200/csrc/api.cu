@@ -347,24 +347,11 @@ void build_pool_tensor_maps(kam_ctx* c) {
   const cuuint64_t gstride[2] = {(cuuint64_t)L.n_kv_heads * L.row_dim * 2, 128};
   const cuuint32_t box[3] = {64, 16, (cuuint32_t)(HG * L.row_dim / 64)};
   const cuuint32_t estr[3] = {1, 1, 1};
-  std::vector<CUtensorMap> maps((size_t)4 * L.n_layers);
+  std::vector<CUtensorMap> maps((size_t)2 * L.n_layers);
   memset(maps.data(), 0, maps.size() * sizeof(CUtensorMap));
   for (int l = 0; l < L.n_layers; ++l)
-    for (int kv = 0; kv < 2; ++kv) {
-      // MLA: map 0 = the whole row as one box (mma.sync kernel), map 1 = one 64-column block x 16 tokens (tcgen05 kernel)
-      if (mla && kv == 1) {
-        // tcgen05 kernel: [1] one 64-column block x 16 tokens; and, when a 64-token tile is one page run (page_size % 64 == 0),
-        // [2] a PAIR of blocks x 64 tokens (lands as [2][64][128 B] = one pair slot) and [3] one block x 64 tokens (the rope block)
-        const cuuint32_t boxes[3][3] = {{64, 16, 1}, {64, 64, 2}, {64, 64, 1}};
-        for (int k = 0; k < (L.page_size % 64 == 0 ? 3 : 1); ++k) {
-          CUresult r1 = encode(&maps[4 * l + 1 + k], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kp[l], gdim, gstride, boxes[k], estr,
-                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-          if (r1 != CUDA_SUCCESS) { c->tmap_why = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r1); return; }
-        }
-        continue;
-      }
-      CUresult r = encode(&maps[4 * l + kv], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv ? vp[l] : kp[l], gdim, gstride, box, estr,
+    for (int kv = 0; kv < (mla ? 1 : 2); ++kv) {             // MLA: one map, the whole latent+rope row x 16 tokens is one box
+      CUresult r = encode(&maps[2 * l + kv], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv ? vp[l] : kp[l], gdim, gstride, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
       if (r != CUDA_SUCCESS) { c->tmap_why = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r); return; }

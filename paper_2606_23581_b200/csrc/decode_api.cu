@@ -20,10 +20,11 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
   if (c->dec_geom_ok[variant][kt]) { *out = c->dec_geom[variant][kt]; return KAM_OK; }
   if (L.elem_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "decode needs a bf16 pool");
   if (!L.has_v) {
-    // absorbed MLA decode: one latent+rope row per token, value = its first v_dim columns (decode_mla_kernel.cu)
+    // absorbed MLA decode: one latent+rope row per token, value = its first v_dim columns
     if (L.n_kv_heads != 1 || L.row_dim != 576 || L.v_dim != 512 || L.rope_off != 512 || L.rope_dim != 64)
       return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode is built for rows of 512 latent + 64 rope columns with v_dim 512");
     if (!variant) return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode needs the context's own pool with page_size %% 16 == 0 (%s)", c->tmap_why.c_str());
+    // token-split kernel (decode_mla_ts_kernel.cu): one CTA per SM, 64-token iterations, the on-read patch rides in the ring
     DecodeGeom g{};
     g.mla = 1;
     g.Hq = L.n_q_heads; g.H = 1; g.D = 576; g.Dv = 512; g.P = L.page_size;
@@ -34,46 +35,8 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
     g.rope_off = L.rope_off; g.d_r = L.rope_dim; g.rope_style = L.rope_style;
     g.row_bytes = g.slice_bytes = 576 * 2; g.use_tma = 1; g.ncb = 9;
     g.kv_bytes = 2048 * g.ncb; g.box_bytes = g.kv_bytes; g.KT = kt;
-    if (kt > 0) {
-      g.u_off = g.kv_bytes;
-      g.su_row = kt * 16 * 2 + 16;
-      g.box_bytes = (int)align_up_sz((size_t)g.kv_bytes + (size_t)kDecTile * g.su_row, 1024);
-    }
-    // tensor-memory kernel, opt-in (KAM_MLA_TC=1): correct, but with only 16 query heads (N = 16) each tcgen05.mma re-reads a
-    // 4 KB A tile from shared memory for 8 cycles of math - measured slower than the mma.sync kernel (decode_mla_tc_kernel.cu)
-    const char* tc_env = getenv("KAM_MLA_TC");
-    if (kt == 0 && tc_env && tc_env[0] == '1') {
-      g.mla = 2;
-      g.smem_bytes = mla_tc_smem_bytes();
-      g.n_ctas = c->sm_count;
-      c->dec_geom[variant][kt] = g; c->dec_geom_ok[variant][kt] = true;
-      *out = g;
-      return KAM_OK;
-    }
-    // calls without an on-read patch run the token-split kernel (decode_mla_ts_kernel.cu: one CTA per SM, 64-token iterations);
-    // KAM_MLA_KSPLIT=1 keeps them on the k-split kernel below (the one that carries the patch)
-    const char* ks_env = getenv("KAM_MLA_KSPLIT");
-    if (kt == 0 && !(ks_env && ks_env[0] == '1')) {
-      g.mla = 3;
-      g.smem_bytes = mla_ts_smem_bytes();
-      g.n_ctas = c->sm_count;
-      c->dec_geom[variant][kt] = g; c->dec_geom_ok[variant][kt] = true;
-      *out = g;
-      return KAM_OK;
-    }
-    g.off_hdr = 128; g.off_xch = 1024; g.off_box0 = 1024 + 2 * kMlaWarps * 256 * 4;
-    int want = c->dec_ctas_per_sm > 0 ? std::min(c->dec_ctas_per_sm, 2) : 2;
-    for (; want >= 1; --want) {
-      const int budget = 227 * 1024 / want - 1024 - g.off_box0;
-      int nb = std::min(8, budget / g.box_bytes);
-      if (c->dec_boxes > 0) nb = std::min(nb, c->dec_boxes);
-      if (nb < 2) continue;
-      g.n_boxes = nb;
-      g.smem_bytes = g.off_box0 + nb * g.box_bytes;
-      if (mla_decode_occupancy(g) >= want) break;
-    }
-    if (want < 1) return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode tile does not fit shared memory");
-    g.n_ctas = c->sm_count * want;
+    g.smem_bytes = mla_ts_smem_bytes(kt);
+    g.n_ctas = c->sm_count;
     c->dec_geom[variant][kt] = g; c->dec_geom_ok[variant][kt] = true;
     *out = g;
     return KAM_OK;
@@ -210,9 +173,7 @@ static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* po
   // the decode kernels read the plan just written: with programmatic dependent launch only their prologue (barrier setup,
   // shared-memory carve-up, launch latency) overlaps the plan kernel - plan_fresh makes them wait before the first plan read
   p.plan_fresh = 1;
-  if (g.mla == 3) launch_mla_ts_decode(g, p, c->use_pdl, st);
-  else if (g.mla == 2) launch_mla_tc_decode(g, p, false, st);
-  else if (g.mla) launch_mla_decode(g, p, c->use_pdl, st);
+  if (g.mla) launch_mla_ts_decode(g, p, c->use_pdl, st);
   else launch_decode(g, p, c->use_pdl, st);
   launch_decode_merge(g, p, c->use_pdl, st);
   c->kernels_launched += 3;
@@ -355,9 +316,7 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.err = c->d_err;
   // with a plan from an earlier call the decode prologue may overlap whatever precedes it on the stream (it only reads the plan)
-  if (g.mla == 3) launch_mla_ts_decode(g, p, cached && c->use_pdl, st);
-  else if (g.mla == 2) launch_mla_tc_decode(g, p, cached && c->use_pdl, st);
-  else if (g.mla) launch_mla_decode(g, p, cached && c->use_pdl, st);
+  if (g.mla) launch_mla_ts_decode(g, p, cached && c->use_pdl, st);
   else launch_decode(g, p, cached && c->use_pdl, st);
   launch_decode_merge(g, p, c->use_pdl, st);
   c->kernels_launched += 2;

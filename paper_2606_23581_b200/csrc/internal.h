@@ -97,7 +97,7 @@ void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocI
 void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
 
 // ---------------------------------------------------------------- decode
-constexpr int kTmapLayerBytes = 4 * 128;   // tensor maps per layer: K | V (MLA: 16-token block) | MLA page pair | MLA page block
+constexpr int kTmapLayerBytes = 2 * 128;   // tensor maps per layer: K | V (MLA: one map, the whole 576-wide row x 16 tokens)
 constexpr int kDecTile = 16;               // tokens per pipeline box (one TMA box of K or of V)
 constexpr int kDecMaxHG = 4;               // KV heads (= compute warps) per CTA
 constexpr int kDecPlanThreads = 1024;
@@ -117,8 +117,7 @@ struct DecodeGeom {
   int32_t KT;                    // on-read patch: 16-wide rank tiles the kernel is specialised for (0: no patch in this call)
   int32_t kv_bytes;              // bytes of the K (or V) rows of a box; box_bytes = kv_bytes + the U tile (KT > 0)
   int32_t u_off, su_row;         // U tile inside a box: [16 tokens][su_row bytes], (su_row / 16) odd
-  int32_t mla;                   // 1: absorbed MLA decode, k-split mma.sync kernel; 2: tcgen05 kernel; 3: token-split mma.sync kernel (2, 3: no on-read patch) (one latent+rope row per token, value = its first Dv columns)
-  int32_t off_xch;               // MLA: shared-memory offset of the partial-score exchange buffer
+  int32_t mla;                   // 1: absorbed MLA decode (one latent+rope row per token, value = its first Dv columns)
 };
 
 struct DecChunk {                // plan input: one chunk of one request (flat, request-major)
@@ -205,16 +204,9 @@ void launch_decode_plan(const DecodeGeom& g, const DecodePlan& plan, const Decod
 // tail of the previous kernel on the stream; only legal when that kernel does not write the plan.
 void launch_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 void launch_decode_merge(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
-// absorbed MLA decode (decode_mla_kernel.cu): same plan, same partials, same merge
-constexpr int kMlaWarps = 4;               // compute warps: each owns 1/4 of the contraction and 1/4 of the value columns
+// absorbed MLA decode (decode_mla_ts_kernel.cu: token-split mma.sync kernel, one CTA per SM): same plan, same partials, same merge
 constexpr int kMlaHeads = 16;              // query heads per work unit (two 8-wide MMA n-tiles)
-int mla_decode_occupancy(const DecodeGeom& g);
-// tcgen05 / tensor-memory formulation (decode_mla_tc_kernel.cu): g.mla == 2, one CTA per SM
-int mla_tc_smem_bytes();
-void launch_mla_tc_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
-void launch_mla_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
-// token-split mma.sync formulation (decode_mla_ts_kernel.cu): g.mla == 3, one CTA per SM, calls without an on-read patch
-int mla_ts_smem_bytes();
+int mla_ts_smem_bytes(int kt);             // kt: rank tiles of the on-read patch the instantiation carries (0, 1, 2, 4)
 void launch_mla_ts_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 
 // ---------------------------------------------------------------- form_patch (compile side, form_patch.cu)

@@ -28,7 +28,7 @@ def _latent_pool(cfg, L, num_pages, seed):
     return kam.Pool([randn_device(shape, seed + l, 1.0, torch.bfloat16, "cuda") for l in range(L)], None)
 
 
-def _run(cfg, lens, deltas, seed, ranks=None, frame=reuse.TARGET_FRAME, style=reuse.HALF, layer=0, L=1):
+def _run(cfg, lens, deltas, seed, ranks=None, frame=reuse.TARGET_FRAME, style=reuse.HALF, layer=0, L=1, u_pad=0):
     rng = _rng(seed)
     P, D, Dv, Hq = cfg.page_size, cfg.row_dim, cfg.v_dim, cfg.n_q_heads
     batch = len(lens)
@@ -54,7 +54,12 @@ def _run(cfg, lens, deltas, seed, ranks=None, frame=reuse.TARGET_FRAME, style=re
             f = make_chunk(cfg.scaled(n_layers=1), rng, n_tokens=n, n_layers=1, rank=m)
             Uk, Wk = f["Uk"][0], f["Wk"][0]
             host[(b, c)] = (Uk, Wk)
-            row.append((Uk.cuda(), Wk.cuda(), None, None, m, frame))
+            Ud = Uk.cuda()
+            if u_pad:                                            # token stride m + u_pad: the U rows of a tile are not one run
+                wide = torch.zeros((n, 1, m + u_pad), dtype=Ud.dtype, device="cuda")
+                wide[:, :, :m] = Ud
+                Ud = wide[:, :, :m]
+            row.append((Ud, Wk.cuda(), None, None, m, frame))
         starts[b, len(lens[b]) + 1:] = starts[b, len(lens[b])]
         refs.append(row)
     patches = None
@@ -163,29 +168,21 @@ def test_window_decode_over_mla_pool_lazy_slides():
     ctx.close()
 
 
-def test_tcgen05_kernel_matches_the_oracle(monkeypatch):
-    """The tensor-memory formulation (csrc/decode_mla_tc_kernel.cu; opt-in with KAM_MLA_TC=1, read when a context first decodes):
-    ragged chunks, partial tiles, pending rotations, more and fewer heads than one tile, both pair layouts."""
-    monkeypatch.setenv("KAM_MLA_TC", "1")
-    _run(CONFIGS[3], [[100, 1024, 37], [1024], [5, 16, 300, 700]], [[0, 3100, -77], [1024], [0, 0, -1024, 2048]], 81)
-    _run(CONFIGS[3], [[1024] * 4, [1024] * 4], [[0, 1024, 2048, 3072], [3072, 0, 1024, 2048]], 82, L=2, layer=1)
-    _run(CONFIGS[3].scaled(n_q_heads=32), [[200, 64]], [[17, 0]], 83)
-    _run(CONFIGS[3].scaled(n_q_heads=8), [[70], [130, 3]], [[-5], [0, 999]], 84)
-    _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 85, style=reuse.INTERLEAVED)
-    _run(CONFIGS[3], [[], [0, 1], [16, 0, 16], [1]], [[], [5, 7], [0, 3, -3], [4000]], 86)
-    _run(CONFIGS[3].scaled(page_size=16), [[100, 500], [77]], [[9, -9], [0]], 87)          # no page-sized boxes: 16-token copies only
-
-
-def test_k_split_kernel_without_a_patch_matches_the_oracle(monkeypatch):
-    """Patch-free calls run the token-split kernel (csrc/decode_mla_ts_kernel.cu) by default, so every other test of this file
-    that carries no patch checks THAT kernel; KAM_MLA_KSPLIT=1 keeps such calls on the k-split kernel (csrc/decode_mla_kernel.cu,
-    the one the patched calls always use) - same cases as the tensor-memory test above."""
-    monkeypatch.setenv("KAM_MLA_KSPLIT", "1")
-    _run(CONFIGS[3], [[100, 1024, 37], [1024], [5, 16, 300, 700]], [[0, 3100, -77], [1024], [0, 0, -1024, 2048]], 91)
-    _run(CONFIGS[3].scaled(n_q_heads=32), [[200, 64]], [[17, 0]], 93)
-    _run(CONFIGS[3].scaled(n_q_heads=8), [[70], [130, 3]], [[-5], [0, 999]], 94)
-    _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 95, style=reuse.INTERLEAVED)
-    _run(CONFIGS[3], [[], [0, 1], [16, 0, 16], [1]], [[], [5, 7], [0, 3, -3], [4000]], 96)
+def test_on_read_patch_shapes_that_stress_the_ring():
+    """The patch rides in the token-split kernel's box ring (W iterations around every patched segment, U rows behind their
+    boxes): mixed ranks and unpatched chunks in one call, chunks shorter than one iteration, 16-token pages, more and fewer
+    heads than one tile, long segments (many ring wraps), both pair layouts, U rows that are not one run per tile."""
+    _run(CONFIGS[3], [[16, 33, 48, 7, 64, 20, 16, 95, 1, 40] * 2, [48] * 6], [[(7 * i) % 5 - 2 for i in range(20)], [0, 3] * 3], 110,
+         ranks=[[16, 0, 32, 16, 0, 16, 48, 16, 16, 64] * 2, [16] * 6])
+    _run(CONFIGS[3].scaled(page_size=16), [[100, 500, 64, 48], [77]], [[9, -9, 0, 3], [0]], 111, ranks=[[16, 16, 0, 16], [16]])
+    _run(CONFIGS[3].scaled(n_q_heads=32), [[200, 64]], [[17, 0]], 112, ranks=[[16, 32]])
+    _run(CONFIGS[3].scaled(n_q_heads=24), [[70], [130, 3]], [[-5], [0, 999]], 113, ranks=[[16], [16, 16]])
+    _run(CONFIGS[3].scaled(n_q_heads=8), [[70], [130, 3]], [[-5], [0, 999]], 114, ranks=[[32], [16, 64]])
+    _run(CONFIGS[3], [[4096 + 50], [3000, 3000]], [[123], [0, -3000]], 115, ranks=[[16], [16, 16]])
+    _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 116, ranks=[[16, 16]], style=reuse.INTERLEAVED)
+    _run(CONFIGS[3], [[256, 31]], [[1234, -1]], 117, ranks=[[32, 16]], style=reuse.INTERLEAVED, frame=reuse.CANONICAL_FRAME)
+    _run(CONFIGS[3], [[300, 100, 37]], [[5, 0, -9]], 118, ranks=[[16, 32, 16]], u_pad=8)
+    _run(CONFIGS[3], [[], [0, 1], [16, 0, 16], [1]], [[], [5, 7], [0, 3, -3], [4000]], 119, ranks=[[], [16, 16], [16, 16, 0], [16]])
 
 
 def test_token_split_kernel_shapes_its_iterations_do_not_divide():
