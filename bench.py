@@ -6,8 +6,8 @@
 A STEP is one pass of the whole hot path over one batch of synthetic input:
   phase A  kam_relocate_patch_batch : 8 chunks x 1024 tokens x 28 layers relocated to p ~ U[0, 32768) with their rank-16
                                       patches into one request's pages, ONE launch           (A1-A5)   <- the headline metric
-  phase B  kam_evict + kam_admit    : the request's window slides: oldest chunk out (its 7 survivors re-rotate in place by
-                                      -1024), one evicted chunk recalled by relocate+patch      (A6, A7)
+  phase B  kam_slide                : the request's window slides: oldest chunk out (its 7 survivors re-rotate in place by
+                                      -1024), one evicted chunk recalled by relocate+patch, ONE launch (A6, A7)
   phase C  kam_window_plan + 28 x kam_window_decode : fused paged decode over every request's 8192-token window, all
                                       layers, LSE merge (A8, A9).  The 28 per-layer calls (2 kernels each) are captured once
                                       into a CUDA graph and replayed; the plan is rebuilt eagerly every step (the window slid)
@@ -191,9 +191,8 @@ class Workload:
         self.ctx_a.kam_relocate_patch_batch([(self.bt_a, base + c * T, cs[c][0], int(p[c]), cs[c][1], m) for c in range(self.n_chunks)])
         rec(1)
         # phase B: the window of request r slides by one chunk
-        self.ctx_b.kam_evict(r, B.KAM_FRONT, 1)
         ch, pa = cs[i % self.n_chunks]
-        self.ctx_b.kam_admit(r, B.KAM_BACK, ch, pa, m, 1)
+        self.ctx_b.kam_slide(r, B.KAM_FRONT, B.KAM_BACK, ch, pa, m, 1)
         rec(2)
         # phase C: every request decodes one token over its window, all layers
         self.ctx_b.kam_window_plan(self.req_ids)
@@ -571,7 +570,7 @@ def main():
     kernels = {
         "kam_relocate_patch_kernel": {"bound": "hbm", "achieved": gb(wl.bytes_a, ms[0]), "bytes_per_launch": wl.bytes_a, "ms_per_launch": ms[0],
                                       "share_of_step": ms[0] / (ms[0] + ms[1] + ms[2])},
-        "window_slide(evict+admit)": {"bound": "hbm", "achieved": gb(wl.bytes_b, ms[1]), "bytes_per_launch": wl.bytes_b / 2, "ms_per_launch": ms[1] / 2,
+        "window_slide(kam_slide)": {"bound": "hbm", "achieved": gb(wl.bytes_b, ms[1]), "bytes_per_launch": wl.bytes_b, "ms_per_launch": ms[1],
                                       "share_of_step": ms[1] / (ms[0] + ms[1] + ms[2])},
         "kam_paged_decode_kernel(+merge)": {"bound": "hbm", "achieved": gb(wl.bytes_c, ms[2]), "bytes_per_launch": wl.bytes_c_layer, "ms_per_launch": ms[2] / L,
                                             "share_of_step": ms[2] / (ms[0] + ms[1] + ms[2])},

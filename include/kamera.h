@@ -19,9 +19,15 @@
  *  - Every call that takes a `stream` (a cudaStream_t passed as void*; NULL = legacy default stream) enqueues
  *    its work on that stream and returns without synchronising.  Host bookkeeping (windows, free list) is
  *    applied immediately; device effects are stream-ordered.
- *  - Errors: every function returns a kam_status; nothing throws or aborts.  Arguments are validated before
- *    any state changes, so a failed call leaves the context as it was.  kam_last_error() gives the reason.
+ *  - A context serves ONE stream at a time: its staging buffers, descriptor rings, decode plans and partials are
+ *    reused from call to call and ordered by that stream only.  Use one context per concurrently used stream.
+ *  - Errors: every function returns a kam_status; nothing throws or aborts.  Arguments, window state and page
+ *    supply are validated before any state changes, so a call that fails with INVALID_ARG / STATE / NO_PAGES /
+ *    UNSUPPORTED leaves the context as it was.  KAM_ERR_CUDA reports a failure of the CUDA runtime itself (a
+ *    launch, a copy): device state is then undefined as after any CUDA error, and the context should be
+ *    destroyed.  kam_last_error() gives the reason.
  *  - There is no CPU fallback: without a CUDA device every compute entry returns KAM_ERR_CUDA.
+ *  - The library never reads the process environment; what is tunable goes through kam_set_option.
  */
 #ifndef KAMERA_H_
 #define KAMERA_H_
@@ -126,18 +132,33 @@ typedef struct kam_stats {
   int64_t table_entries_written;   /* page-table entries written since kam_create (O(1)-per-op evidence) */
   int64_t chunks_live;
   int64_t kernels_launched;        /* CUDA kernels this context has launched since kam_create */
-  int64_t device_errors;           /* malformed kam_patch_ref records the decode kernels ignored (reading it synchronises) */
+  int64_t device_errors;           /* malformed kam_patch_ref records the decode kernels ignored + block-table entries outside
+                                      [0, num_pages) the relocate kernels skipped (reading it synchronises) */
+  int64_t generic_launches;        /* of kernels_launched: launches of the element-wise fallback relocate kernel (fp32 tensors,
+                                      row regions that are not multiples of 64 columns, U strides bulk copies cannot address);
+                                      every bf16 rank in [0, KAM_MAX_RANK] runs on the tiled kernel */
 } kam_stats;
 
 /* ---- context -------------------------------------------------------------------------------------------------
  * pool == NULL creates a bookkeeping-only context: window calls update and export host state but launch nothing
- * (used to test the host logic without a GPU); every stateless compute entry then needs an explicit pool.
- * max_requests / max_chunks_per_request / max_pages_per_chunk size the window store. */
+ * (used to test the host logic without a GPU); its compute entries return KAM_ERR_CUDA.
+ * max_requests / max_chunks_per_request / max_pages_per_chunk size the window store: page lists are kept per chunk
+ * ([max_requests * max_chunks_per_request][max_pages_per_chunk] int32, host + device mirror), which is what makes an
+ * admit / evict touch only that chunk's entries.  (SURVEY.md 8(b) sketched one max_pages_per_request; the
+ * per-chunk table needs the two factors separately.) */
 kam_status kam_create(const kam_layout *layout, const kam_pool *pool, int32_t max_requests,
                       int32_t max_chunks_per_request, int32_t max_pages_per_chunk, kam_ctx **out);
 kam_status kam_destroy(kam_ctx *ctx);
 const char *kam_last_error(const kam_ctx *ctx);     /* ctx may be NULL: error of the last failed kam_create */
 const char *kam_version(void);
+/* Tunables, per context; the defaults are the measured choices and nothing reads the environment.  Keys:
+ *   reloc_stages 0..8 (0 = automatic)   reloc_head_group 0..4   reloc_kv_split 0 never / 1 automatic / 2 always
+ *   reloc_contig 0/1   reloc_row_blocks 0..4   reloc_evict_first 0/1   reloc_patch_cost_pct 50..200
+ *   decode_ctas_per_sm 0..8   decode_boxes 0..16
+ *   decode_pdl 0/1   decode_tma 0/1   host_copy_overlap 0/1   host_entries_sync 0/1
+ * Setting any of them drops cached decode plans; CUDA graphs captured over this context's calls must be re-captured.
+ * Errors: INVALID_ARG (unknown key, value out of range). */
+kam_status kam_set_option(kam_ctx *ctx, const char *key, int64_t value);
 
 /* ---- stateless operator: Eq. 1 written into the paged pool (`apply_reuse`) --------------------
  * For every layer l, token t, head h:
@@ -147,11 +168,17 @@ const char *kam_version(void);
  * dst_token_start need not be page aligned.  patch == NULL or rank == 0 => pure rotation (survivors).
  * p_target is a RoPE phase (any int64; M-RoPE positions are not sequence indices); dst_token_start is the
  * logical index inside the block table - two different things on purpose.
+ * A block-table entry outside [0, pool->num_pages) is never dereferenced: its tokens are skipped and the entry is counted
+ * once in kam_stats.device_errors.  rank: any value in [0, KAM_MAX_RANK] (ranks that are not multiples of 16 are padded
+ * with zeros in shared memory, never in HBM).
+ * layout: north_star's `layout = {MHA, GQA, MLA}` argument.  A context is created for ONE layout (kernel geometry, the
+ * frequency table and the tensor maps hang off it), so this is a check, not a dispatch: NULL = the context's layout, else it
+ * must equal it field by field (INVALID_ARG otherwise).
  * pool == NULL => the context's pool.  Errors: INVALID_ARG (null/misaligned pointers, rank < 0 or > KAM_MAX_RANK,
- * n_tokens < 0), UNSUPPORTED (layout the kernels do not cover), CUDA. */
+ * n_tokens < 0, dst_token_start + n_tokens > 2^31 - 1), UNSUPPORTED (layout the kernels do not cover), CUDA. */
 kam_status kam_relocate_patch(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_table,
                               int64_t dst_token_start, const kam_chunk *chunk, int64_t p_target,
-                              const kam_patch *patch, int32_t rank, void *stream);
+                              const kam_patch *patch, int32_t rank, const kam_layout *layout, void *stream);
 kam_status kam_relocate_patch_batch(kam_ctx *ctx, const kam_pool *pool, int32_t n,
                                     const kam_reloc_desc *descs /* host array [n] */, void *stream);
 
@@ -164,7 +191,10 @@ kam_status kam_rotate_inplace(kam_ctx *ctx, const kam_pool *pool, const int32_t 
  * canonical store): every k/v/U/W array is a HOST array [n_layers] of HOST pointers with the layouts above
  * (U contiguous [T][H][rank]).  The library copies them to device staging it owns (H2D on `stream`), then runs
  * kam_relocate_patch.  Pinned host memory makes the copies asynchronous.  Copies whose host source continues the previous
- * one are merged: a chunk kept as ONE slab in the order (per layer: K, V, U_k, W_k, U_v, W_v) crosses PCIe in one transfer. */
+ * one are merged: a chunk kept as ONE slab in the order (per layer: K, V, U_k, W_k, U_v, W_v) crosses PCIe in one transfer.
+ * The copies run on a stream of the library's own into one of two staging buffers, so the transfer of one call overlaps the
+ * kernel of the previous one; the kernel is ordered behind its copies on `stream` as usual (option host_copy_overlap = 0:
+ * one buffer, everything on `stream`).  The host arrays must stay valid until `stream` has passed this call. */
 kam_status kam_relocate_patch_host(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_table /* device */,
                                    int64_t dst_token_start, int32_t n_tokens, int64_t p_base, int64_t p_target,
                                    const void *const *k_host, const void *const *v_host,
@@ -196,6 +226,11 @@ kam_status kam_form_patch(kam_ctx *ctx, const void *const *kv_cond_layers, const
  *   kam_evict  returns the chunk's pages.
  * Chunks whose position moved (FRONT ops): materialize = 1 rotates them in place now (delta = position - phase);
  * materialize = 0 touches nothing - the pending delta is applied on read by kam_window_decode.
+ * kam_slide = kam_evict(evict_end, lazy) + kam_admit(admit_end, materialize) as ONE call and ONE kernel launch ("as the
+ * oldest frame leaves, survivors re-rotate by the slide offset and a later recall rehydrates the dropped frame"): the
+ * survivors' in-place rotations (by their NET displacement, rounded once) and the admitted chunk's Eq. 1 ride in the same
+ * descriptor list.  kam_admit alone likewise launches once for its survivors and its chunk.  A slide whose admission cannot
+ * succeed (pages, sizes) fails before anything is evicted.
  * Errors: INVALID_ARG, STATE (request not open / already open / window empty / too many chunks), NO_PAGES. */
 kam_status kam_window_open(kam_ctx *ctx, int32_t req, int64_t window_base);
 kam_status kam_window_pin(kam_ctx *ctx, int32_t req, int32_t n_front_chunks);
@@ -204,8 +239,12 @@ kam_status kam_admit(kam_ctx *ctx, int32_t req, int32_t end /* kam_end */, const
                      const kam_patch *patch, int32_t rank, int32_t materialize, int32_t *chunk_handle_out,
                      void *stream);
 kam_status kam_evict(kam_ctx *ctx, int32_t req, int32_t end /* kam_end */, int32_t materialize, void *stream);
+kam_status kam_slide(kam_ctx *ctx, int32_t req, int32_t evict_end /* kam_end */, int32_t admit_end /* kam_end */,
+                     const kam_chunk *chunk, const kam_patch *patch, int32_t rank, int32_t materialize,
+                     int32_t *chunk_handle_out, void *stream);
 /* Linear host view of one request, for bit-exact checks.  Any output pointer may be NULL.  Capacities are in
- * entries; too small => INVALID_ARG.  chunk_starts_out gets n_chunks + 1 entries. */
+ * entries; too small => INVALID_ARG.  chunk_cap counts the entries of EACH chunk array that is not NULL; chunk_starts_out gets
+ * n_chunks + 1 entries, so with chunk_starts_out != NULL chunk_cap must be >= n_chunks + 1. */
 kam_status kam_window_export(kam_ctx *ctx, int32_t req, int32_t *block_table_out, int32_t block_table_cap,
                              int64_t *slot_mapping_out, int64_t slot_mapping_cap, int32_t *chunk_starts_out,
                              int64_t *chunk_offsets_out, int32_t *chunk_handles_out, int32_t chunk_cap,
@@ -227,7 +266,11 @@ kam_status kam_get_stats(kam_ctx *ctx, kam_stats *out);
  * out [batch][n_q_heads][Dv] bf16 (Dv = row_dim, or v_dim for MLA), lse [batch][n_q_heads] f32 (natural log, scale
  * inside).  A request with no tokens gives out = 0, lse = -inf.  Requires elem_dtype == KAM_BF16; head_dim 64 or 128 and at most
  * 16 query heads per KV head (MHA/GQA); MLA in absorbed form: row_dim 576 = 512 latent + 64 rope, v_dim 512, q rows of 576,
- * the context's own pool with page_size % 16 == 0 (any number of query heads).  Otherwise KAM_ERR_UNSUPPORTED. */
+ * page_size % 16 == 0 (any number of query heads).  Otherwise KAM_ERR_UNSUPPORTED.
+ * pool: NULL = the context's, or any pool of the context's layout.  Pool pages travel as TMA tensor-map boxes; the maps are
+ * built per pool and cached (keyed by the pool's pointer-array addresses and page count): the FIRST decode call that names a
+ * new pool reads its layer pointers back, which synchronises; a caller that re-fills a pointer array in place must pass it
+ * under a new address. */
 /* Largest rank a kam_patch_ref of later decode calls may carry: 16, 32 or 64 (default KAM_MAX_RANK).  The decode kernel
  * is specialised for it (shared memory and registers per tile grow with it), so a caller whose patches are all rank 16
  * should say so.  Errors: INVALID_ARG. */
@@ -236,6 +279,17 @@ kam_status kam_paged_decode_merge(kam_ctx *ctx, const void *q, const kam_pool *p
                                   int32_t max_pages, const int32_t *chunk_starts, const int64_t *chunk_offsets,
                                   const int32_t *n_chunks, int32_t max_chunks, const kam_patch_ref *patches,
                                   int32_t layer, int32_t batch, float sm_scale, void *out, float *lse, void *stream);
+/* The work split of a decode call (which 16-token tiles each persistent CTA streams, each segment's first pool slot, the
+ * per-chunk cos/sin rows) depends on the paging metadata only - not on the layer, the query or the factors.  By default
+ * kam_paged_decode_merge rebuilds it on every call (one small kernel).  kam_paged_decode_plan builds it once and PINS it:
+ * every later kam_paged_decode_merge / _state / _merge_host call on this context that names the same block_tables,
+ * chunk_starts, chunk_offsets, n_chunks arrays, the same pool, max_pages, max_chunks, batch and the same `patches != NULL`
+ * reuses the pinned plan (all layers of a decode step share one plan, as kam_window_decode's do).  The caller must call
+ * kam_paged_decode_plan again when the CONTENT of those arrays changed; a call with different arrays or sizes rebuilds its own
+ * plan and drops the pin; batch == 0 or block_tables == NULL just drops it. */
+kam_status kam_paged_decode_plan(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_tables, int32_t max_pages,
+                                 const int32_t *chunk_starts, const int64_t *chunk_offsets, const int32_t *n_chunks,
+                                 int32_t max_chunks, int32_t has_patches, int32_t batch, void *stream);
 /* ---- chunk-parallel decode across GPUs ("the log-sum-exp state merge already used by ... ring/star
  * attention").  When a request's chunks are spread over several GPUs, each rank runs kam_paged_decode_state over the
  * chunks IT holds - same arguments as kam_paged_decode_merge, but the result is the softmax STATE in fp32:
@@ -255,12 +309,17 @@ kam_status kam_lse_merge_states(kam_ctx *ctx, int32_t n_parts, const float *cons
  * The work split of a step (which 16-token tiles each persistent CTA streams, the per-chunk cos/sin tables) depends on
  * the windows only, not on the layer: kam_window_plan builds it (one small H2D copy + one kernel); kam_window_decode
  * builds it itself when the windows or the request list changed since the last plan and otherwise launches exactly two
- * kernels (decode, merge) and nothing else - in that state it may be captured into a CUDA graph.  A context serves one
- * stream at a time: the plan and the partials live in its workspace. */
+ * kernels (decode, merge) and nothing else - in that state it may be captured into a CUDA graph.  The window workspace is
+ * laid out once for the largest plan the store can produce (max_requests x max_chunks_per_request chunks) and never moves,
+ * and the kernels read the plan's sizes from it: a captured graph stays valid when the windows slide, grow or shrink (re-plan
+ * eagerly, then replay).  It is tied, like any graph, to its q / out / lse pointers, its batch size and the options. */
 kam_status kam_window_plan(kam_ctx *ctx, const int32_t *req_ids, int32_t batch, void *stream);
 kam_status kam_window_decode(kam_ctx *ctx, const void *q, const int32_t *req_ids, int32_t batch, int32_t layer,
                              float sm_scale, void *out, float *lse, void *stream);
-/* Same as kam_paged_decode_merge with q, out and lse in HOST memory (H2D / D2H on `stream`, then a stream sync). */
+/* Same as kam_paged_decode_merge with q, out and lse in HOST memory: H2D of q, the kernels, D2H of out and lse, all enqueued on
+ * `stream`; like every other entry it returns without synchronising - out_host / lse_host are valid once `stream` has passed
+ * this call (one synchronise per decode step, not per layer).  Each layer has its own device staging, so the calls of a step do
+ * not wait for each other.  Option host_entries_sync = 1 restores a cudaStreamSynchronize at the end of every call. */
 kam_status kam_paged_decode_merge_host(kam_ctx *ctx, const void *q_host, const kam_pool *pool,
                                        const int32_t *block_tables, int32_t max_pages, const int32_t *chunk_starts,
                                        const int64_t *chunk_offsets, const int32_t *n_chunks, int32_t max_chunks,

@@ -56,7 +56,7 @@ class kam_patch_ref(C.Structure):
 
 class kam_stats(C.Structure):
     _fields_ = [(n, i64) for n in ("pages_free", "pages_total", "table_entries_written", "chunks_live",
-                                    "kernels_launched", "device_errors")]
+                                    "kernels_launched", "device_errors", "generic_launches")]
 
 
 # name -> (restype, argtypes): every symbol include/kamera.h declares
@@ -65,7 +65,9 @@ SIGNATURES = {
     "kam_destroy": (i32, [vp]),
     "kam_last_error": (C.c_char_p, [vp]),
     "kam_version": (C.c_char_p, []),
-    "kam_relocate_patch": (i32, [vp, C.POINTER(kam_pool), vp, i64, C.POINTER(kam_chunk), i64, C.POINTER(kam_patch), i32, vp]),
+    "kam_set_option": (i32, [vp, C.c_char_p, i64]),
+    "kam_relocate_patch": (i32, [vp, C.POINTER(kam_pool), vp, i64, C.POINTER(kam_chunk), i64, C.POINTER(kam_patch), i32,
+                                 C.POINTER(kam_layout), vp]),
     "kam_relocate_patch_batch": (i32, [vp, C.POINTER(kam_pool), i32, C.POINTER(kam_reloc_desc), vp]),
     "kam_rotate_inplace": (i32, [vp, C.POINTER(kam_pool), vp, i64, i32, i64, vp]),
     "kam_relocate_patch_host": (i32, [vp, C.POINTER(kam_pool), vp, i64, i32, i64, i64, C.POINTER(vp), C.POINTER(vp),
@@ -76,11 +78,13 @@ SIGNATURES = {
     "kam_window_close": (i32, [vp, i32]),
     "kam_admit": (i32, [vp, i32, i32, C.POINTER(kam_chunk), C.POINTER(kam_patch), i32, i32, C.POINTER(i32), vp]),
     "kam_evict": (i32, [vp, i32, i32, i32, vp]),
+    "kam_slide": (i32, [vp, i32, i32, i32, C.POINTER(kam_chunk), C.POINTER(kam_patch), i32, i32, C.POINTER(i32), vp]),
     "kam_window_export": (i32, [vp, i32, C.POINTER(i32), i32, C.POINTER(i64), i64, C.POINTER(i32), C.POINTER(i64),
                                 C.POINTER(i32), i32, C.POINTER(i32), C.POINTER(i32)]),
     "kam_get_stats": (i32, [vp, C.POINTER(kam_stats)]),
     "kam_paged_decode_merge": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
                                      vp, vp, vp]),
+    "kam_paged_decode_plan": (i32, [vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, i32, i32, vp]),
     "kam_decode_set_max_patch_rank": (i32, [vp, i32]),
     "kam_paged_decode_state": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
                                      vp, vp, vp]),
@@ -193,18 +197,21 @@ class Context:
         self.h = h
 
     def close(self):
-        if getattr(self, "h", None):
-            lib().kam_destroy(self.h)
-            self.h = None
+        if getattr(self, "h", None) and _lib is not None:      # at interpreter shutdown the module globals may be gone already
+            _lib.kam_destroy(self.h)
+        self.h = None
 
     __del__ = close
 
+    def kam_set_option(self, key, value):
+        _check(lib().kam_set_option(self.h, key.encode(), int(value)), self.h)
+
     def kam_relocate_patch(self, block_table, dst_token_start, chunk, p_target, patch=None, rank=0, pool=None,
-                           stream=None):
+                           layout=None, stream=None):
         _check(lib().kam_relocate_patch(self.h, C.byref(pool.c) if pool else None, _ptr(block_table),
                                         int(dst_token_start), C.byref(chunk.c), int(p_target),
                                         C.byref(patch.c) if patch is not None else None, int(rank),
-                                        _stream_ptr(stream)), self.h)
+                                        C.byref(layout) if layout is not None else None, _stream_ptr(stream)), self.h)
 
     def kam_relocate_patch_batch(self, descs, pool=None, stream=None):
         """descs: list of (block_table, dst_token_start, chunk, p_target, patch or None, rank)."""
@@ -264,6 +271,14 @@ class Context:
         sp = _stream_ptr(stream) if torch.cuda.is_available() else vp(None)
         _check(lib().kam_evict(self.h, req, end, int(materialize), sp), self.h)
 
+    def kam_slide(self, req, evict_end, admit_end, chunk, patch=None, rank=0, materialize=1, stream=None):
+        handle = i32(-1)
+        sp = _stream_ptr(stream) if torch.cuda.is_available() else vp(None)
+        _check(lib().kam_slide(self.h, req, evict_end, admit_end, C.byref(chunk.c if hasattr(chunk, "c") else chunk),
+                               C.byref(patch.c) if patch is not None else None, int(rank), int(materialize),
+                               C.byref(handle), sp), self.h)
+        return handle.value
+
     def kam_window_export(self, req):
         n_pages, n_chunks = i32(), i32()
         _check(lib().kam_window_export(self.h, req, None, 0, None, 0, None, None, None, 0, C.byref(n_pages),
@@ -272,10 +287,10 @@ class Context:
         bt = (i32 * max(1, n_pages.value))()
         sm = (i64 * max(1, n_pages.value * P))()
         st = (i32 * (n_chunks.value + 1))()
-        of = (i64 * max(1, n_chunks.value))()
-        hd = (i32 * max(1, n_chunks.value))()
+        of = (i64 * (n_chunks.value + 1))()
+        hd = (i32 * (n_chunks.value + 1))()
         _check(lib().kam_window_export(self.h, req, bt, n_pages.value, sm, n_pages.value * P, st, of, hd,
-                                       n_chunks.value, C.byref(n_pages), C.byref(n_chunks)), self.h)
+                                       n_chunks.value + 1, C.byref(n_pages), C.byref(n_chunks)), self.h)
         nc, npg = n_chunks.value, n_pages.value
         return {"block_table": list(bt[:npg]), "slot_mapping": list(sm[:npg * P]), "chunk_starts": list(st[:nc + 1]),
                 "chunk_offsets": list(of[:nc]), "handles": list(hd[:nc])}
@@ -294,6 +309,18 @@ class Context:
                                             max_pages, _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks),
                                             max_chunks, _ptr(patches), int(layer), batch, float(sm_scale), _ptr(out),
                                             _ptr(lse), _stream_ptr(stream)), self.h)
+
+    def kam_paged_decode_plan(self, block_tables, chunk_starts, chunk_offsets, n_chunks, has_patches=False, pool=None,
+                              stream=None):
+        """Pins the plan of these metadata arrays (None block_tables releases it)."""
+        if block_tables is None:
+            _check(lib().kam_paged_decode_plan(self.h, None, None, 0, None, None, None, 0, 0, 0, _stream_ptr(stream)), self.h)
+            return
+        batch, max_pages = block_tables.shape
+        max_chunks = chunk_starts.shape[1] - 1
+        _check(lib().kam_paged_decode_plan(self.h, C.byref(pool.c) if pool else None, _ptr(block_tables), max_pages,
+                                           _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks), max_chunks,
+                                           int(bool(has_patches)), batch, _stream_ptr(stream)), self.h)
 
     def kam_paged_decode_state(self, q, block_tables, chunk_starts, chunk_offsets, n_chunks, layer, sm_scale, o_state,
                                lse_state, patches=None, pool=None, stream=None):

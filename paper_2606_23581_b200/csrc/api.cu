@@ -37,12 +37,17 @@ kam_status cuda_fail(kam_ctx* ctx, cudaError_t e, const char* what) {
   return fail(ctx, KAM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
-kam_status grow_device(kam_ctx* c, void** buf, size_t* cap, size_t bytes, const char* what) {
+// Grows a library-owned device buffer.  The outgrown buffer may still be read by work already enqueued, and cudaFree would
+// synchronise the whole device inside a call documented to return without synchronising: it is parked and freed by
+// kam_destroy.  Capacities grow geometrically, so the parked buffers add up to less than the live one.
+kam_status grow_device(kam_ctx* c, void** buf, size_t* cap, size_t bytes, const char* what, cudaStream_t) {
   if (*cap >= bytes) return KAM_OK;
-  cudaError_t e;
-  if (*buf) { cudaDeviceSynchronize(); cudaFree(*buf); *buf = nullptr; *cap = 0; }
-  if ((e = cudaMalloc(buf, bytes)) != cudaSuccess) return cuda_fail(c, e, what);
-  *cap = bytes;
+  void* fresh = nullptr;
+  const size_t want = std::max(bytes, *cap + *cap / 2);
+  cudaError_t e = cudaMalloc(&fresh, want);
+  if (e != cudaSuccess) return cuda_fail(c, e, what);
+  if (*buf) c->graveyard.push_back(*buf);
+  *buf = fresh; *cap = want;
   return KAM_OK;
 }
 
@@ -87,6 +92,10 @@ bool build_head_blocks(kam_ctx* c) {
   return true;
 }
 
+// Shared-memory geometry of the tiled kernel for a call whose largest rank is max_rank.  Candidates, best first:
+// whole-row slices (one copy per tile) with three stages; if the resident W_k + W_v leave no room for that (ranks 48 / 64:
+// 139 KB for four heads of 128 columns), the kv-split form - a tile carries K rows or V rows, so only one of the two W tables
+// is resident and three 48 KB stages fit again; last, fewer heads per slice or two big stages (the round-1 geometry).
 bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGeom* out, std::string* why) {
   const kam_layout& L = c->lay;
   RelocGeom g{};
@@ -95,62 +104,92 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
   g.P_shift = -1;
   for (int sft = 0; sft < 31; ++sft) if ((1 << sft) == g.P) g.P_shift = sft;
   g.nkv = (L.has_v && !inplace_only) ? 2 : 1;       // survivors are rotated in place: K only, V is never staged
-  g.KT_max = max_rank / 16;
+  g.KT_max = (max_rank + 15) / 16;
+  const int m_pad = g.KT_max * 16;                  // ranks are padded to a multiple of 16 in shared memory only
   g.rope_style = L.rope_style; g.d_r = L.rope_dim; g.half_groups = L.rope_dim / 64;
   g.theta = L.rope_theta;
   const int limit = 226 * 1024;
-  const int ns_max = c->reloc_stages > 0 ? c->reloc_stages : 3;   // measured on B200: 3 x 37 KB in flight per SM beats 4 and 5
-  RelocGeom best{}; bool have = false;
-  const int hg_force = getenv("KAM_RELOC_HG") ? atoi(getenv("KAM_RELOC_HG")) : 0;       // tuning switch
-  for (int HG = std::min(g.H, 4); HG >= 1; --HG) {
-    if (g.H % HG) continue;
-    if (hg_force > 0 && HG != hg_force) continue;
+  const int ns_max = c->opt.reloc_stages > 0 ? c->opt.reloc_stages : 3;   // measured on B200: 3 x 37 KB in flight per SM beats 4 and 5
+  const int hg_force = c->opt.reloc_hg;                                   // kam_set_option("reloc_head_group")
+  // one candidate: `HG` heads per slice, plain or kv-split; fills *t with the deepest pipeline (<= ns_max stages) that fits
+  auto candidate = [&](bool split, int HG, RelocGeom* out_t) -> bool {
+    if (g.H % HG) return false;
     const int NB = HG * c->blocks_per_head;
-    if (NB > kMaxColBlocks) continue;
+    if (NB > kMaxColBlocks) return false;
     RelocGeom t = g;
+    t.kv_split = split ? 1 : 0;
+    const int nkv_tile = split ? 1 : g.nkv;           // row sets (K, V) a tile holds
     t.HG = HG; t.n_hg = g.H / HG; t.n_blocks = NB;
     t.slice_bytes = HG * g.D * 2;
-    t.contig = (HG == g.H) && c->contig_copies;
+    t.contig = (HG == g.H) && c->opt.reloc_contig;
     // padded rows (== 64 mod 128) make the 128-bit row loads conflict-free; unpadded rows allow one copy per tile
     t.s_row = t.contig ? t.slice_bytes : t.slice_bytes + ((64 - t.slice_bytes % 128) + 128) % 128;
     // U rows: unpadded when a tile arrives as one copy (the one ldmatrix per slab tolerates the bank conflicts)
-    t.su_row = g.KT_max ? HG * max_rank * 2 + (t.contig ? 0 : 16) : 0;
-    t.RB = std::min(4, std::max(1, (kRelocConsumerWarps + t.nkv * NB - 1) / (t.nkv * NB)));
-    if (c->reloc_rb > 0) t.RB = std::min(4, c->reloc_rb);
+    t.su_row = g.KT_max ? align_up(HG * max_rank * 2, 16) + (t.contig ? 0 : 16) : 0;
+    t.RB = std::min(4, std::max(1, (kRelocConsumerWarps + nkv_tile * NB - 1) / (nkv_tile * NB)));
+    if (c->opt.reloc_rb > 0) t.RB = std::min(4, c->opt.reloc_rb);
     t.TT = 16 * t.RB;
     t.st_k = 0;
     t.st_v = t.st_k + t.TT * t.s_row;
-    t.st_uk = t.st_v + (t.nkv == 2 ? t.TT * t.s_row : 0);
+    t.st_uk = t.st_v + (nkv_tile == 2 ? t.TT * t.s_row : 0);
     t.st_uv = t.st_uk + t.TT * t.su_row;
-    t.st_slot = t.st_uv + (t.nkv == 2 ? t.TT * t.su_row : 0);
-    t.stage_bytes = align_up(t.st_slot + t.TT * 4, 128);
+    t.st_slot = t.st_uv + (nkv_tile == 2 ? t.TT * t.su_row : 0);
+    t.stage_bytes = align_up(t.st_slot + 2 * t.TT * 4, 128);                     // slots: 2 TT (the in-place x2 tile form)
     t.w_row = (g.D + 8) * 2;
-    t.w_kv_stride = HG * max_rank * t.w_row;
+    t.w_kv_stride = HG * m_pad * t.w_row;
     t.off_tab = 128;
     t.off_cs = t.off_tab + align_up(2 * t.RB * NB * 16, 128);                    // slab table: one int4 per slab
     t.off_w = t.off_cs + align_up(std::max(1, g.d_r / 2) * 12, 128);               // c | s | -s, planar fp32
-    t.off_stage0 = align_up(t.off_w + t.nkv * t.w_kv_stride, 128);
+    t.off_stage0 = align_up(t.off_w + nkv_tile * t.w_kv_stride, 128);
     for (int i = 0; i < NB; ++i) {
       ColBlock b = c->head_blocks[i % c->blocks_per_head];
       const int h = i / c->blocks_per_head;
       b.fhead = (int8_t)h; b.col_off = (int16_t)(b.col_off + h * g.D);
       t.blk[i] = b;
     }
+    t.load_hint = c->opt.reloc_load_hint;
     for (int NS = ns_max; NS >= 2; --NS) {
       t.n_stages = NS;
       t.smem_bytes = t.off_stage0 + NS * t.stage_bytes;
-      if (t.smem_bytes > limit) continue;
-      t.load_hint = c->reloc_load_hint;
-      // three stages, or two big ones (>= 96 KB in flight: measured at rank 64, where W takes 70 KB: 2 x 54 KB tiles of two heads
-      // stream at 4.9 TB/s, three 60 KB stages of one-head slices at 4.0 TB/s - four times as many 256-byte copies)
-      if (NS >= 3 || NS * t.stage_bytes >= 96 * 1024 || hg_force > 0) { *out = t; return true; }
-      if (!have) { best = t; have = true; }
-      break;
+      if (t.smem_bytes <= limit) { *out_t = t; return true; }
     }
+    return false;
+  };
+  int hg_max = 1;
+  for (int HG = std::min(g.H, 4); HG >= 1; --HG) if (g.H % HG == 0) { hg_max = HG; break; }
+  const bool may_split = g.nkv == 2 && c->opt.reloc_kv_split != 0, must_split = g.nkv == 2 && c->opt.reloc_kv_split == 2;
+  RelocGeom t{};
+  if (hg_force > 0) {
+    if (candidate(must_split, hg_force, &t)) { *out = t; return true; }
+    *why = "forced head group does not fit";
+    return false;
   }
+  // 1. the widest slice with three stages, plain; 2. the same, kv-split
+  if (!must_split && candidate(false, hg_max, &t) && t.n_stages >= 3) { *out = t; return true; }
+  if (may_split && candidate(true, hg_max, &t) && (t.n_stages >= 3 || must_split)) { *out = t; return true; }
+  // 3. round 1's order: narrower slices, three stages or two big ones (>= 96 KB in flight: measured at rank 64 before the
+  //    kv-split form existed - two 54 KB stages of two heads 4.9 TB/s, three 60 KB stages of one-head slices 4.0 TB/s)
+  RelocGeom best{}; bool have = false;
+  for (int pass = must_split ? 1 : 0; pass < (may_split ? 2 : 1); ++pass)
+    for (int HG = hg_max; HG >= 1; --HG) {
+      if (!candidate(pass == 1, HG, &t)) continue;
+      if (t.n_stages >= 3 || t.n_stages * t.stage_bytes >= 96 * 1024) { *out = t; return true; }
+      if (!have) { best = t; have = true; }
+    }
   if (have) { *out = best; return true; }
   *why = "no shared-memory configuration fits";
   return false;
+}
+
+// Can the tiled kernel stream this U layout?  Its producer moves U with bulk copies: 16-byte aligned sources and sizes, unless
+// the whole tile is one contiguous run of the caller's array (then a ragged tail of < 16 bytes is handled separately).
+bool u_layout_fast(const RelocGeom& g, int r, long long uts, long long uhs) {
+  if (uts * 2 <= g.su_row && (uhs == 0 || g.n_hg == 1)) return true;        // native form: one copy per tile (u_native in the kernel)
+  const int hf_n = uhs == 0 ? 1 : g.HG;
+  const bool heads_adjacent = hf_n == 1 || uhs == r;
+  const long long tok_bytes = (long long)hf_n * r * 2;
+  if ((uts * 2) % 16 || ((long long)g.HG * uhs * 2) % 16) return false;
+  return heads_adjacent ? tok_bytes % 16 == 0 : (r * 2) % 16 == 0 && (uhs * 2) % 16 == 0;
 }
 
 }  // namespace
@@ -207,6 +246,9 @@ struct HostReloc {
   const void* const* k; const void* const* v;
   const kam_patch* patch; int32_t rank; int32_t n_tokens; int32_t flags;
 };
+// The page list of a chunk being admitted to a window (descriptor `desc` of the call): host copy in a staging slot, device
+// mirror row.  The tiled kernel takes it in its parameters; otherwise it is copied to the mirror ahead of the launch.
+struct AdmitPages { int desc; int32_t n; Staging* sg; int32_t* d_mirror; };
 
 // Checked before any state changes, by the stateless entries and by kam_admit alike.
 kam_status validate_patch(kam_ctx* c, const kam_patch* p, int32_t rank, int idx) {
@@ -224,7 +266,7 @@ kam_status validate_patch(kam_ctx* c, const kam_patch* p, int32_t rank, int idx)
   return KAM_OK;
 }
 
-kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostReloc>& hs, cudaStream_t st) {
+kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostReloc>& hs, cudaStream_t st, const AdmitPages* ap = nullptr) {
   const kam_layout& L = c->lay;
   const int n = (int)hs.size();
   // ---- validate everything before touching anything
@@ -233,8 +275,9 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
   for (int i = 0; i < n; ++i) {
     const HostReloc& h = hs[i];
     if (h.n_tokens < 0) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: n_tokens < 0", i);
-    if (h.bt == nullptr) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: block_table is NULL", i);
+    if (h.bt == nullptr && !(ap && ap->desc == i)) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: block_table is NULL", i);
     if (h.dst0 < 0) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: negative token start", i);
+    if (h.dst0 + h.n_tokens > (int64_t)INT32_MAX) return fail(c, KAM_ERR_INVALID_ARG, "desc %d: token range beyond 2^31 - 1", i);
     const bool inplace = h.flags & FLAG_INPLACE;
     inplace_only = inplace_only && inplace;
     if (!inplace && (h.k == nullptr || (L.has_v && h.v == nullptr)))
@@ -243,25 +286,36 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
     if (vs != KAM_OK) return vs;
     max_tokens = std::max(max_tokens, h.n_tokens);
     const kam_patch* p = (h.patch && h.rank > 0) ? h.patch : nullptr;
-    for (int l = 0; l < L.n_layers && p; ++l) {
-      const int r = p->rank_per_layer ? p->rank_per_layer[l] : h.rank;
-      max_rank = std::max(max_rank, r);
-      if (r % 16) fast = false;
-    }
-    if (p && (p->u_token_stride % 8 || p->u_head_stride % 8)) fast = false;
+    for (int l = 0; l < L.n_layers && p; ++l) max_rank = std::max(max_rank, p->rank_per_layer ? p->rank_per_layer[l] : h.rank);
   }
   if (n == 0 || max_tokens == 0) return KAM_OK;
   if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
 
   RelocGeom g{};
   if (fast) { std::string why; if (!build_reloc_geom(c, max_rank, inplace_only, &g, &why)) fast = false; }
+  // any rank <= KAM_MAX_RANK runs on the tiled kernel (padded to a multiple of 16 in shared memory); what can still send a
+  // call to the element-wise kernel is a U layout the bulk copies cannot address (see u_layout_fast)
+  for (int i = 0; i < n && fast; ++i) {
+    const kam_patch* p = (hs[i].patch && hs[i].rank > 0) ? hs[i].patch : nullptr;
+    for (int l = 0; l < L.n_layers && p && fast; ++l) {
+      const int r = p->rank_per_layer ? p->rank_per_layer[l] : hs[i].rank;
+      if (r > 0 && !u_layout_fast(g, r, p->u_token_stride, p->u_head_stride)) fast = false;
+    }
+  }
 
+  // the admitted chunk's page list: in the kernel parameters when it fits, else one small copy ahead of the launch
+  const bool inline_pages = ap && fast && ap->n <= kRelocInlinePages;
+  if (ap && !inline_pages) {
+    cudaError_t e = cudaMemcpyAsync(ap->d_mirror, ap->sg->host, (size_t)ap->n * 4, cudaMemcpyHostToDevice, st);
+    staging_release(ap->sg, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(page list)");
+  }
   // Small batches on the tiled kernel carry their descriptors in the kernel parameters; anything else is staged through
   // pinned host memory and copied with one cudaMemcpyAsync on the caller's stream.
   const bool inline_descs = fast && n <= kRelocInlineDescs;
   const size_t desc_bytes = (size_t)n * sizeof(RelocDescDev);
   const size_t prefix_off = (desc_bytes + 15) & ~size_t(15);
-  const size_t total_bytes = prefix_off + (size_t)(n + 1) * sizeof(long long);
+  const size_t total_bytes = prefix_off + (size_t)2 * (n + 1) * sizeof(long long);      // tile prefix | weight prefix
   Staging* sg = nullptr;
   std::unique_ptr<RelocInline> inl(new (std::nothrow) RelocInline());
   if (!inl) return fail(c, KAM_ERR_STATE, "out of host memory");
@@ -270,7 +324,8 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
   if (!inline_descs && (s = staging_acquire(c, total_bytes, &sg)) != KAM_OK) return s;
   RelocDescDev* dd = inline_descs ? inl->d : static_cast<RelocDescDev*>(sg->host);
   long long* prefix = inline_descs ? inl->prefix : reinterpret_cast<long long*>(static_cast<char*>(sg->host) + prefix_off);
-  long long acc = 0;
+  long long* wprefix = inline_descs ? inl->wprefix : prefix + (n + 1);
+  long long acc = 0, wacc = 0;
   for (int i = 0; i < n; ++i) {
     const HostReloc& h = hs[i];
     RelocDescDev d{};
@@ -278,16 +333,31 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
     d.k_src = h.k; d.v_src = h.v;
     d.Uk = p ? p->Uk : nullptr; d.Wk = p ? p->Wk : nullptr;
     d.Uv = (p && L.has_v) ? p->Uv : nullptr; d.Wv = (p && L.has_v) ? p->Wv : nullptr;
-    d.block_table = h.bt; d.dst_token_start = h.dst0; d.delta = h.delta;
+    d.block_table = (ap && ap->desc == i) ? ap->d_mirror : h.bt; d.dst_token_start = h.dst0; d.delta = h.delta;
     d.u_token_stride = p ? p->u_token_stride : 0; d.u_head_stride = p ? p->u_head_stride : 0;
     d.n_tokens = h.n_tokens;
-    d.flags = h.flags | ((p && p->frame == KAM_PATCH_CANONICAL_FRAME) ? FLAG_CANONICAL_FRAME : 0);
+    d.flags = h.flags | ((p && p->frame == KAM_PATCH_CANONICAL_FRAME) ? FLAG_CANONICAL_FRAME : 0) |
+              ((inline_pages && ap->desc == i) ? FLAG_INLINE_PAGES : 0);
     for (int l = 0; l < L.n_layers; ++l) d.rank_l[l] = (uint8_t)(p ? (p->rank_per_layer ? p->rank_per_layer[l] : h.rank) : 0);
+    prefix[i] = acc; wprefix[i] = wacc;
+    d.tile_weight = 1;
+    if (fast) {                                              // the same tile forms as TileWalk::set_desc in the kernel
+      const bool inplace = h.flags & FLAG_INPLACE;
+      const int tile_tok = (inplace && g.nkv == 2 && !g.kv_split) ? 2 * g.TT : g.TT;
+      const int n_kv = (g.kv_split && g.nkv == 2 && !inplace) ? 2 : 1;
+      const long long tiles = (long long)L.n_layers * g.n_hg * n_kv * ((h.n_tokens + tile_tok - 1) / tile_tok);
+      // weight of a tile: the bytes it moves (rows read + written, U read), in 64-byte units; tiles that also run the patch
+      // (W staging, MMAs) cost "reloc_patch_cost_pct" of their bytes (measured: 1.72 vs 1.50 us for 68 vs 64 KB)
+      const int row_sets = (inplace || g.kv_split) ? 1 : g.nkv;
+      const int u_heads = (p && p->u_head_stride) ? g.HG : 1;
+      long long bytes = (long long)row_sets * 2 * tile_tok * g.slice_bytes + (p ? (long long)row_sets * g.TT * u_heads * h.rank * 2 : 0);
+      if (p) bytes = bytes * c->opt.reloc_patch_cost_pct / 100;
+      d.tile_weight = (int32_t)std::max<long long>(1, bytes / 64);
+      acc += tiles; wacc += tiles * d.tile_weight;
+    }
     dd[i] = d;
-    prefix[i] = acc;
-    if (fast) acc += (long long)L.n_layers * g.n_hg * ((h.n_tokens + g.TT - 1) / g.TT);
   }
-  prefix[n] = acc;
+  prefix[n] = acc; wprefix[n] = wacc;
   const RelocDescDev* d_descs = nullptr;
   if (!inline_descs) {
     if ((s = staging_commit(c, sg, total_bytes, st)) != KAM_OK) return s;
@@ -298,17 +368,29 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
     RelocParams p{};
     p.descs = d_descs;
     p.tile_prefix = inline_descs ? nullptr : reinterpret_cast<const long long*>(static_cast<const char*>(sg->dev) + prefix_off);
+    p.w_prefix = inline_descs ? nullptr : p.tile_prefix + (n + 1);
+    p.total_weight = wacc;
     p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;
     p.total_tiles = acc; p.n_descs = n; p.inv_freq = c->d_inv_freq;
+    p.num_pages = pool->num_pages; p.err = c->d_err;
     const int grid = (int)std::min<long long>(c->sm_count, acc);
-    launch_relocate_fast(g, p, *inl, grid, st);
+    std::unique_ptr<RelocPages> pg(new (std::nothrow) RelocPages());
+    if (!pg) return fail(c, KAM_ERR_STATE, "out of host memory");
+    pg->mirror_dst = nullptr; pg->n = 0;
+    if (inline_pages) {
+      memcpy(pg->pages, ap->sg->host, (size_t)ap->n * 4);
+      pg->mirror_dst = ap->d_mirror; pg->n = ap->n;
+    }
+    launch_relocate_fast(g, p, *inl, *pg, grid, st);
   } else {
     GenericParams p{};
     p.descs = d_descs; p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;
     p.n_descs = n; p.L = L.n_layers; p.H = L.n_kv_heads; p.D = L.row_dim; p.P = L.page_size;
     p.rope_off = L.rope_off; p.d_r = L.rope_dim; p.rope_style = L.rope_style; p.has_v = L.has_v;
     p.elem_f32 = L.elem_dtype == KAM_F32; p.factor_f32 = L.factor_dtype == KAM_F32; p.theta = L.rope_theta;
+    p.num_pages = pool->num_pages; p.err = c->d_err;
     launch_relocate_generic(p, max_tokens, st);
+    ++c->generic_launches;
   }
   ++c->kernels_launched;
   cudaError_t e = cudaGetLastError();
@@ -323,27 +405,27 @@ typedef CUresult (*PFN_tmapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuin
                                         const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                         CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-void build_pool_tensor_maps(kam_ctx* c) {
+// Builds the maps of one pool; returns the device array or nullptr (c->tmap_why says why).
+void* build_pool_tensor_maps(kam_ctx* c, const kam_pool& pool) {
   const kam_layout& L = c->lay;
-  if (getenv("KAM_DECODE_NO_TMA")) { c->tmap_why = "disabled by KAM_DECODE_NO_TMA"; return; }
-  if (L.elem_dtype != KAM_BF16) { c->tmap_why = "needs a bf16 pool"; return; }
+  if (L.elem_dtype != KAM_BF16) { c->tmap_why = "needs a bf16 pool"; return nullptr; }
   const bool mla = !L.has_v;
-  if (mla && (L.n_kv_heads != 1 || L.row_dim % 64)) { c->tmap_why = "MLA rows must be a multiple of 64 columns"; return; }
-  if (L.page_size % 16 || (!mla && L.row_dim != 64 && L.row_dim != 128)) { c->tmap_why = "needs page_size % 16 == 0 and head_dim 64/128"; return; }
-  if (c->pool.num_pages < 1) { c->tmap_why = "empty pool"; return; }
+  if (mla && (L.n_kv_heads != 1 || L.row_dim % 64)) { c->tmap_why = "MLA rows must be a multiple of 64 columns"; return nullptr; }
+  if (L.page_size % 16 || (!mla && L.row_dim != 64 && L.row_dim != 128)) { c->tmap_why = "needs page_size % 16 == 0 and head_dim 64/128"; return nullptr; }
+  if (pool.num_pages < 1) { c->tmap_why = "empty pool"; return nullptr; }
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
-    cudaGetLastError(); c->tmap_why = "cuTensorMapEncodeTiled not available"; return;
+    cudaGetLastError(); c->tmap_why = "cuTensorMapEncodeTiled not available"; return nullptr;
   }
   PFN_tmapEncodeTiled encode = reinterpret_cast<PFN_tmapEncodeTiled>(fn);
   std::vector<void*> kp(L.n_layers), vp(L.n_layers);
-  if (cudaMemcpy(kp.data(), c->pool.k_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess ||
-      (!mla && cudaMemcpy(vp.data(), c->pool.v_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess)) {
-    cudaGetLastError(); c->tmap_why = "could not read the pool's layer pointers"; return;
+  if (cudaMemcpy(kp.data(), pool.k_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess ||
+      (!mla && cudaMemcpy(vp.data(), pool.v_layers, sizeof(void*) * L.n_layers, cudaMemcpyDeviceToHost) != cudaSuccess)) {
+    cudaGetLastError(); c->tmap_why = "could not read the pool's layer pointers"; return nullptr;
   }
   const int HG = decode_head_group(L);                  // MLA: one "head" of row_dim columns, the whole row is one box
-  const cuuint64_t gdim[3] = {64, (cuuint64_t)c->pool.num_pages * L.page_size, (cuuint64_t)L.n_kv_heads * L.row_dim / 64};
+  const cuuint64_t gdim[3] = {64, (cuuint64_t)pool.num_pages * L.page_size, (cuuint64_t)L.n_kv_heads * L.row_dim / 64};
   const cuuint64_t gstride[2] = {(cuuint64_t)L.n_kv_heads * L.row_dim * 2, 128};
   const cuuint32_t box[3] = {64, 16, (cuuint32_t)(HG * L.row_dim / 64)};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -354,16 +436,43 @@ void build_pool_tensor_maps(kam_ctx* c) {
       CUresult r = encode(&maps[2 * l + kv], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv ? vp[l] : kp[l], gdim, gstride, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      if (r != CUDA_SUCCESS) { c->tmap_why = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r); return; }
+      if (r != CUDA_SUCCESS) { c->tmap_why = "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r); return nullptr; }
     }
   static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
-  if (cudaMalloc(&c->d_tmaps, maps.size() * sizeof(CUtensorMap)) != cudaSuccess ||
-      cudaMemcpy(c->d_tmaps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess) {
+  void* d = nullptr;
+  if (cudaMalloc(&d, maps.size() * sizeof(CUtensorMap)) != cudaSuccess ||
+      cudaMemcpy(d, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess) {
     cudaGetLastError();
-    if (c->d_tmaps) { cudaFree(c->d_tmaps); c->d_tmaps = nullptr; }
+    if (d) cudaFree(d);
     c->tmap_why = "could not upload tensor maps";
+    return nullptr;
   }
+  return d;
 }
+
+}  // namespace
+
+namespace kam {
+// Tensor maps are a property of a pool (its layer base pointers and page count), so they are cached per pool: the context's
+// own (built at kam_create) and up to kMaxTmapSets caller pools, keyed by the pool's pointer arrays.  The first decode call
+// with a new pool reads its layer pointers back (a synchronous copy); a pool whose arrays are re-filled in place must not
+// keep the same array addresses (the header says so).
+const void* tmaps_for_pool(kam_ctx* c, const kam_pool* pool) {
+  for (TmapSet& t : c->tmap_sets)
+    if (t.k_layers == pool->k_layers && t.v_layers == pool->v_layers && t.num_pages == pool->num_pages) { t.stamp = ++c->tmap_clock; return t.d_tmaps; }
+  void* d = build_pool_tensor_maps(c, *pool);               // nullptr is cached too: the reason does not change
+  if (c->tmap_sets.size() >= (size_t)kMaxTmapSets) {
+    size_t victim = 1;                                          // entry 0 is the context's own pool
+    for (size_t i = 2; i < c->tmap_sets.size(); ++i) if (c->tmap_sets[i].stamp < c->tmap_sets[victim].stamp) victim = i;
+    if (c->tmap_sets[victim].d_tmaps) c->graveyard.push_back(c->tmap_sets[victim].d_tmaps);    // may still be read by queued work
+    c->tmap_sets.erase(c->tmap_sets.begin() + victim);
+  }
+  c->tmap_sets.push_back(TmapSet{pool->k_layers, pool->v_layers, pool->num_pages, d, ++c->tmap_clock});
+  return d;
+}
+}  // namespace kam
+
+namespace {
 
 kam_status validate_layout(const kam_layout* L) {
   if (!L) return fail(nullptr, KAM_ERR_INVALID_ARG, "layout is NULL");
@@ -407,10 +516,6 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
   if (!c) return fail(nullptr, KAM_ERR_STATE, "out of host memory");
   c->lay = *layout;
   c->fast_layout = build_head_blocks(c);
-  if (const char* e = getenv("KAM_RELOC_CONTIG")) c->contig_copies = (e[0] != '0');   // tuning switch, default on
-  if (const char* e = getenv("KAM_RELOC_STAGES")) c->reloc_stages = atoi(e);
-  if (const char* e = getenv("KAM_RELOC_RB")) c->reloc_rb = atoi(e);
-  if (const char* e = getenv("KAM_RELOC_HINT")) c->reloc_load_hint = atoi(e);
   c->max_requests = max_requests; c->max_chunks = max_chunks_per_request; c->max_ppc = max_pages_per_chunk;
   if (pool) { c->pool = *pool; c->has_pool = true; }
   if (pool) {
@@ -419,10 +524,14 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "kam_create: no usable CUDA device"); delete c; return r; }
     c->cuda_ok = true;
-    build_pool_tensor_maps(c);
-    if (const char* ev = getenv("KAM_DEC_CTAS_PER_SM")) c->dec_ctas_per_sm = atoi(ev);
-    if (const char* ev = getenv("KAM_DEC_BOXES")) c->dec_boxes = atoi(ev);
-    if (const char* ev = getenv("KAM_NO_PDL")) c->use_pdl = (ev[0] == '0');
+    tmaps_for_pool(c, &c->pool);                   // entry 0 of the cache: the context's own pool
+    // the library's own copy stream + events (kam_relocate_patch_host); without them the host entry runs on the caller's stream
+    if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->copy_stream = nullptr; }
+    for (int i = 0; i < 2 && c->copy_stream; ++i)
+      if (cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming) != cudaSuccess ||
+          cudaEventCreateWithFlags(&c->ev_consumed[i], cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError(); cudaStreamDestroy(c->copy_stream); c->copy_stream = nullptr;
+      }
     e = cudaMalloc(&c->d_err, sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemset(c->d_err, 0, sizeof(int32_t));
     if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "kam_create: device error counter"); kam_destroy(c); return r; }
@@ -440,7 +549,7 @@ kam_status kam_create(const kam_layout* layout, const kam_pool* pool, int32_t ma
     if (c->cuda_ok) {
       const size_t bytes = (size_t)max_requests * max_chunks_per_request * max_pages_per_chunk * sizeof(int32_t);
       cudaError_t e = cudaMalloc(&c->d_slot_pages, bytes);
-      if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "cudaMalloc(page lists)"); delete c; return r; }
+      if (e != cudaSuccess) { kam_status r = cuda_fail(nullptr, e, "cudaMalloc(page lists)"); kam_destroy(c); return r; }
     }
   }
   *out = c;
@@ -458,12 +567,19 @@ kam_status kam_destroy(kam_ctx* c) {
     }
     if (c->d_slot_pages) cudaFree(c->d_slot_pages);
     if (c->d_ws) cudaFree(c->d_ws);
-    if (c->d_hstage) cudaFree(c->d_hstage);
+    if (c->d_ws_win) cudaFree(c->d_ws_win);
+    for (int i = 0; i < 2; ++i) {
+      if (c->d_hstage[i]) cudaFree(c->d_hstage[i]);
+      if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
+      if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]);
+    }
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->d_hstage2) cudaFree(c->d_hstage2);
-    if (c->d_tmaps) cudaFree(c->d_tmaps);
+    for (TmapSet& t : c->tmap_sets) if (t.d_tmaps) cudaFree(t.d_tmaps);
     if (c->d_inv_freq) cudaFree(c->d_inv_freq);
     if (c->d_err) cudaFree(c->d_err);
     if (c->d_fp_ws) cudaFree(c->d_fp_ws);
+    for (void* p : c->graveyard) cudaFree(p);
   }
   delete c;
   return KAM_OK;
@@ -477,6 +593,7 @@ kam_status kam_get_stats(kam_ctx* c, kam_stats* out) {
     s.table_entries_written = c->win->table_entries_written(); s.chunks_live = c->win->chunks_live();
   }
   s.kernels_launched = c->kernels_launched;
+  s.generic_launches = c->generic_launches;
   if (c->d_err) {
     int32_t n = 0;
     cudaError_t e = cudaMemcpy(&n, c->d_err, sizeof(n), cudaMemcpyDeviceToHost);
@@ -503,8 +620,21 @@ kam_status kam_relocate_patch_batch(kam_ctx* c, const kam_pool* pool, int32_t n,
   return run_reloc(c, pool, hs, static_cast<cudaStream_t>(stream));
 }
 
+// north_star's signature carries `layout = {MHA, GQA, MLA}`; the context was created for one layout (its kernels' geometry,
+// frequency table and tensor maps hang off it), so the argument is checked, not dispatched on: NULL = the context's.
+static bool same_layout(const kam_layout& a, const kam_layout& b) {
+  return a.kind == b.kind && a.n_layers == b.n_layers && a.n_q_heads == b.n_q_heads && a.n_kv_heads == b.n_kv_heads &&
+         a.row_dim == b.row_dim && a.rope_off == b.rope_off && a.rope_dim == b.rope_dim && a.has_v == b.has_v &&
+         a.v_dim == b.v_dim && a.page_size == b.page_size && a.rope_style == b.rope_style && a.elem_dtype == b.elem_dtype &&
+         a.factor_dtype == b.factor_dtype && a.rope_theta == b.rope_theta;
+}
+
 kam_status kam_relocate_patch(kam_ctx* c, const kam_pool* pool, const int32_t* block_table, int64_t dst_token_start,
-                              const kam_chunk* chunk, int64_t p_target, const kam_patch* patch, int32_t rank, void* stream) {
+                              const kam_chunk* chunk, int64_t p_target, const kam_patch* patch, int32_t rank,
+                              const kam_layout* layout, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (layout && !same_layout(*layout, c->lay))
+    return fail(c, KAM_ERR_INVALID_ARG, "kam_relocate_patch: layout differs from the one this context was created for");
   kam_reloc_desc d{block_table, dst_token_start, chunk, p_target, patch, rank};
   return kam_relocate_patch_batch(c, pool, 1, &d, stream);
 }
@@ -542,18 +672,28 @@ kam_status kam_relocate_patch_host(kam_ctx* c, const kam_pool* pool, const int32
   const size_t wb = ((size_t)L.n_kv_heads * rank * L.row_dim * fb + 255) & ~size_t(255);
   const int nkv = L.has_v ? 2 : 1;
   const size_t per_layer = nkv * (rows + ub + wb);
-  if ((s = grow_device(c, &c->d_hstage, &c->hstage_cap, per_layer * L.n_layers, "cudaMalloc(host-chunk staging)")) != KAM_OK) return s;
+  // Two staging buffers and a copy stream of the library's own: the H2D copy of this chunk runs under the kernel of the
+  // previous call (which reads the OTHER buffer).  copy stream: wait until the kernel that last read this buffer is done ->
+  // copies -> event; caller's stream: wait for that event -> kernel -> event "consumed".   ("host_copy_overlap" = 0: one
+  // buffer, everything on the caller's stream.)
+  const bool overlap = c->opt.host_copy_overlap && c->copy_stream;
+  const int hb = overlap ? c->hstage_next : 0;
+  if (overlap) c->hstage_next ^= 1;
+  if ((s = grow_device(c, &c->d_hstage[hb], &c->hstage_cap[hb], per_layer * L.n_layers, "cudaMalloc(host-chunk staging)", st)) != KAM_OK) return s;
+  cudaStream_t cs = overlap ? c->copy_stream : st;
+  cudaError_t e = cudaSuccess;
+  if (overlap && c->hstage_used[hb]) e = cudaStreamWaitEvent(cs, c->ev_consumed[hb], 0);
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamWaitEvent(staging buffer)");
   // device pointer tables for the staged copy: [k | v | Uk | Wk | Uv | Wv][n_layers]
   Staging* sg;
   if ((s = staging_acquire(c, (size_t)6 * L.n_layers * sizeof(void*), &sg)) != KAM_OK) return s;
   const void** tabs = static_cast<const void**>(sg->host);
-  char* d = static_cast<char*>(c->d_hstage);
-  cudaError_t e = cudaSuccess;
+  char* d = static_cast<char*>(c->d_hstage[hb]);
   // Copies whose source AND staging destination continue the previous one are merged: a canonical store that keeps a chunk as
   // one slab in this order (per layer: K, V, U_k, W_k, U_v, W_v) crosses PCIe in ONE transfer instead of 6 per layer.
   const char* run_src = nullptr; char* run_dst = nullptr; size_t run_bytes = 0;
   auto flush = [&]() {
-    if (run_bytes && e == cudaSuccess) e = cudaMemcpyAsync(run_dst, run_src, run_bytes, cudaMemcpyHostToDevice, st);
+    if (run_bytes && e == cudaSuccess) e = cudaMemcpyAsync(run_dst, run_src, run_bytes, cudaMemcpyHostToDevice, cs);
     run_bytes = 0;
   };
   auto put = [&](int which, int l, const void* const* src, size_t bytes, size_t& off) {
@@ -577,16 +717,22 @@ kam_status kam_relocate_patch_host(kam_ctx* c, const kam_pool* pool, const int32
     } else { tabs[4 * L.n_layers + l] = nullptr; tabs[5 * L.n_layers + l] = nullptr; }
   }
   flush();
-  if (e != cudaSuccess) { staging_release(sg, st); return cuda_fail(c, e, "cudaMemcpyAsync(host chunk)"); }
-  if ((s = staging_commit(c, sg, (size_t)6 * L.n_layers * sizeof(void*), st)) != KAM_OK) return s;
-  staging_release(sg, st);          // NOTE: the tables stay valid until this staging slot is reused (8 calls later)
+  if (e != cudaSuccess) { staging_release(sg, cs); return cuda_fail(c, e, "cudaMemcpyAsync(host chunk)"); }
+  if ((s = staging_commit(c, sg, (size_t)6 * L.n_layers * sizeof(void*), cs)) != KAM_OK) { staging_release(sg, cs); return s; }
+  if (overlap) {
+    if ((e = cudaEventRecord(c->ev_copied[hb], cs)) == cudaSuccess) e = cudaStreamWaitEvent(st, c->ev_copied[hb], 0);
+    if (e != cudaSuccess) { staging_release(sg, cs); return cuda_fail(c, e, "cudaEventRecord / cudaStreamWaitEvent(host chunk)"); }
+  }
   const void* const* dt = static_cast<const void* const*>(sg->dev);
   kam_chunk ch{dt, L.has_v ? dt + L.n_layers : nullptr, n_tokens, p_base};
   kam_patch pa{dt + 2 * L.n_layers, dt + 3 * L.n_layers, L.has_v ? dt + 4 * L.n_layers : nullptr,
                L.has_v ? dt + 5 * L.n_layers : nullptr, (int64_t)L.n_kv_heads * rank, rank, nullptr, frame};
   std::vector<HostReloc> hs(1);
   hs[0] = HostReloc{block_table, dst_token_start, p_target - p_base, ch.k_layers, ch.v_layers, rank ? &pa : nullptr, rank, n_tokens, 0};
-  return run_reloc(c, pool, hs, st);
+  s = run_reloc(c, pool, hs, st);
+  staging_release(sg, st);          // the pointer tables are released behind the kernel that reads them
+  if (overlap && cudaEventRecord(c->ev_consumed[hb], st) == cudaSuccess) c->hstage_used[hb] = true;
+  return s;
 }
 
 // ---- window store ---------------------------------------------------------------------------------------------------
@@ -616,44 +762,54 @@ kam_status kam_window_close(kam_ctx* c, int32_t req) {
   return win_status(c, c->win->close(req), "kam_window_close");
 }
 
-static kam_status rotate_survivors(kam_ctx* c, const std::vector<Rotation>& rot, cudaStream_t st) {
-  if (rot.empty() || !c->cuda_ok) return KAM_OK;
-  std::vector<HostReloc> hs(rot.size());
-  for (size_t i = 0; i < rot.size(); ++i)
-    hs[i] = HostReloc{c->d_slot_pages + (size_t)rot[i].slot * c->max_ppc, 0, rot[i].delta, nullptr, nullptr, nullptr, 0,
-                      rot[i].n_tokens, FLAG_INPLACE};
+static void survivors_to_descs(kam_ctx* c, const std::vector<Rotation>& rot, std::vector<HostReloc>* hs) {
+  for (const Rotation& r : rot)
+    hs->push_back(HostReloc{c->d_slot_pages + (size_t)r.slot * c->max_ppc, 0, r.delta, nullptr, nullptr, nullptr, 0, r.n_tokens, FLAG_INPLACE});
+}
+
+// What kam_admit and kam_slide share.  Everything that can fail for a reason of the caller's (arguments, window state, pages)
+// or of the host (staging memory) is checked BEFORE the window store changes; `evict_end` < 0 = no eviction.  The survivors'
+// in-place rotations and the admitted chunk's Eq. 1 travel in ONE kam_relocate_patch_kernel launch (they touch disjoint pages).
+static kam_status admit_core(kam_ctx* c, int32_t req, int evict_end, int admit_end, const kam_chunk* chunk, const kam_patch* patch,
+                             int32_t rank, int32_t materialize, int32_t* handle_out, cudaStream_t st, const char* what) {
+  if (!chunk) return fail(c, KAM_ERR_INVALID_ARG, "%s: chunk is NULL", what);
+  { kam_status vs = validate_patch(c, patch, rank, 0); if (vs != KAM_OK) return vs; }
+  if (c->cuda_ok && (!chunk->k_layers || (c->lay.has_v && !chunk->v_layers)))
+    return fail(c, KAM_ERR_INVALID_ARG, "%s: chunk layer-pointer arrays must not be NULL", what);
+  kam_status s = win_status(c, c->win->can_admit(req, evict_end, admit_end, chunk->n_tokens), what);
+  if (s != KAM_OK) return s;
+  const int32_t np = chunk->n_tokens / c->lay.page_size;
+  Staging* sg = nullptr;
+  if (c->cuda_ok && (s = staging_acquire(c, (size_t)np * 4, &sg)) != KAM_OK) return s;
+  // ---- commit: from here on only CUDA runtime failures can interrupt (reported as KAM_ERR_CUDA; the window then lists the
+  // chunk although its pages were not written - the context should be destroyed, as after any CUDA error)
+  ChunkRec rec; int64_t p_target = 0; std::vector<Rotation> rot;
+  if (evict_end >= 0) c->win->evict(req, evict_end, false, nullptr, nullptr);
+  c->win->admit(req, admit_end, chunk->n_tokens, materialize != 0, &rec, &p_target, &rot);
+  if (handle_out) *handle_out = rec.handle;
+  if (!c->cuda_ok) return KAM_OK;                     // bookkeeping-only context
+  // device mirror of the chunk's page list: exactly n_tokens / P entries are written (O(1) in the window length)
+  int32_t* d_pages = c->d_slot_pages + (size_t)rec.slot * c->max_ppc;
+  memcpy(sg->host, c->win->pages_of(rec.slot), (size_t)np * 4);
+  std::vector<HostReloc> hs;
+  survivors_to_descs(c, rot, &hs);
+  hs.push_back(HostReloc{nullptr, 0, p_target - chunk->p_base, chunk->k_layers, chunk->v_layers, patch, rank, chunk->n_tokens, 0});
+  const AdmitPages ap{(int)hs.size() - 1, np, sg, d_pages};
   const kam_pool* pool = &c->pool;
-  return run_reloc(c, pool, hs, st);
+  return run_reloc(c, pool, hs, st, &ap);
 }
 
 kam_status kam_admit(kam_ctx* c, int32_t req, int32_t end, const kam_chunk* chunk, const kam_patch* patch, int32_t rank,
                      int32_t materialize, int32_t* handle_out, void* stream) {
   KAM_NEED_WIN(c);
-  if (!chunk) return fail(c, KAM_ERR_INVALID_ARG, "chunk is NULL");
-  { kam_status vs = validate_patch(c, patch, rank, 0); if (vs != KAM_OK) return vs; }
-  if (c->cuda_ok && (!chunk->k_layers || (c->lay.has_v && !chunk->v_layers)))
-    return fail(c, KAM_ERR_INVALID_ARG, "chunk layer-pointer arrays must not be NULL");
-  cudaStream_t st = static_cast<cudaStream_t>(stream);
-  ChunkRec rec; int64_t p_target = 0; std::vector<Rotation> rot;
-  kam_status s = win_status(c, c->win->admit(req, end, chunk->n_tokens, materialize != 0, &rec, &p_target, &rot), "kam_admit");
-  if (s != KAM_OK) return s;
-  if (handle_out) *handle_out = rec.handle;
-  if (!c->cuda_ok) return KAM_OK;                     // bookkeeping-only context
-  // device mirror of the chunk's page list: exactly n_tokens / P entries are written (O(1) in the window length)
-  const int32_t np = rec.n_tokens / c->lay.page_size;
-  int32_t* d_pages = c->d_slot_pages + (size_t)rec.slot * c->max_ppc;
-  Staging* sg;
-  if ((s = staging_acquire(c, (size_t)np * 4, &sg)) != KAM_OK) return s;
-  memcpy(sg->host, c->win->pages_of(rec.slot), (size_t)np * 4);
-  cudaError_t e = cudaMemcpyAsync(d_pages, sg->host, (size_t)np * 4, cudaMemcpyHostToDevice, st);
-  staging_release(sg, st);
-  if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(page list)");
-  // survivors first (they only touch their own pages), then Eq. 1 for the admitted chunk
-  if ((s = rotate_survivors(c, rot, st)) != KAM_OK) return s;
-  std::vector<HostReloc> hs(1);
-  hs[0] = HostReloc{d_pages, 0, p_target - chunk->p_base, chunk->k_layers, chunk->v_layers, patch, rank, chunk->n_tokens, 0};
-  const kam_pool* pool = &c->pool;
-  return run_reloc(c, pool, hs, st);
+  return admit_core(c, req, -1, end, chunk, patch, rank, materialize, handle_out, static_cast<cudaStream_t>(stream), "kam_admit");
+}
+
+kam_status kam_slide(kam_ctx* c, int32_t req, int32_t evict_end, int32_t admit_end, const kam_chunk* chunk, const kam_patch* patch,
+                     int32_t rank, int32_t materialize, int32_t* handle_out, void* stream) {
+  KAM_NEED_WIN(c);
+  if (evict_end != KAM_FRONT && evict_end != KAM_BACK) return fail(c, KAM_ERR_INVALID_ARG, "kam_slide: bad evict end");
+  return admit_core(c, req, evict_end, admit_end, chunk, patch, rank, materialize, handle_out, static_cast<cudaStream_t>(stream), "kam_slide");
 }
 
 kam_status kam_evict(kam_ctx* c, int32_t req, int32_t end, int32_t materialize, void* stream) {
@@ -661,7 +817,11 @@ kam_status kam_evict(kam_ctx* c, int32_t req, int32_t end, int32_t materialize, 
   std::vector<Rotation> rot;
   kam_status s = win_status(c, c->win->evict(req, end, materialize != 0, nullptr, &rot), "kam_evict");
   if (s != KAM_OK) return s;
-  return rotate_survivors(c, rot, static_cast<cudaStream_t>(stream));
+  if (rot.empty() || !c->cuda_ok) return KAM_OK;
+  std::vector<HostReloc> hs;
+  survivors_to_descs(c, rot, &hs);
+  const kam_pool* pool = &c->pool;
+  return run_reloc(c, pool, hs, static_cast<cudaStream_t>(stream));
 }
 
 kam_status kam_window_export(kam_ctx* c, int32_t req, int32_t* bt_out, int32_t bt_cap, int64_t* sm_out, int64_t sm_cap,
@@ -674,8 +834,8 @@ kam_status kam_window_export(kam_ctx* c, int32_t req, int32_t* bt_out, int32_t b
   int64_t n_tok = 0; int32_t n_pages = 0;
   for (const ChunkRec& r : ch) { n_tok += r.n_tokens; n_pages += r.n_tokens / P; }
   const int32_t nc = (int32_t)ch.size();
-  if ((bt_out && bt_cap < n_pages) || (sm_out && sm_cap < n_tok) ||
-      ((starts_out || offs_out || handles_out) && chunk_cap < nc))
+  if ((bt_out && bt_cap < n_pages) || (sm_out && sm_cap < n_tok) || ((offs_out || handles_out) && chunk_cap < nc) ||
+      (starts_out && chunk_cap < nc + 1))                       // chunk_starts_out takes n_chunks + 1 entries
     return fail(c, KAM_ERR_INVALID_ARG, "kam_window_export: output capacity too small");
   int64_t pos = c->win->window_base(req), tok = 0; int32_t pg = 0, i = 0;
   for (const ChunkRec& r : ch) {
@@ -694,6 +854,32 @@ kam_status kam_window_export(kam_ctx* c, int32_t req, int32_t* bt_out, int32_t b
   return KAM_OK;
 }
 
+// ---- tunables ---------------------------------------------------------------------------------------------------------
+kam_status kam_set_option(kam_ctx* c, const char* key, int64_t value) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  if (!key) return fail(c, KAM_ERR_INVALID_ARG, "kam_set_option: key is NULL");
+  struct Opt { const char* name; int* field; int lo, hi; };
+  Options& o = c->opt;
+  const Opt opts[] = {
+      {"reloc_stages", &o.reloc_stages, 0, 8},       {"reloc_head_group", &o.reloc_hg, 0, 4},
+      {"reloc_kv_split", &o.reloc_kv_split, 0, 2},   {"reloc_contig", &o.reloc_contig, 0, 1},
+      {"reloc_row_blocks", &o.reloc_rb, 0, 4},       {"reloc_evict_first", &o.reloc_load_hint, 0, 1},
+      {"decode_ctas_per_sm", &o.dec_ctas_per_sm, 0, 8}, {"decode_boxes", &o.dec_boxes, 0, 16},
+      {"decode_pdl", &o.use_pdl, 0, 1},              {"decode_tma", &o.dec_tma, 0, 1},
+      {"host_copy_overlap", &o.host_copy_overlap, 0, 1}, {"host_entries_sync", &o.host_sync, 0, 1},
+      {"reloc_patch_cost_pct", &o.reloc_patch_cost_pct, 50, 200},
+  };
+  for (const Opt& op : opts)
+    if (strcmp(op.name, key) == 0) {
+      if (value < op.lo || value > op.hi) return fail(c, KAM_ERR_INVALID_ARG, "kam_set_option: %s = %lld outside [%d, %d]", key, (long long)value, op.lo, op.hi);
+      *op.field = (int)value;
+      for (auto& row : c->dec_geom_ok) for (bool& ok : row) ok = false;      // cached decode geometries depend on the options
+      c->winplan_epoch = ~0ull;
+      c->decplan_valid = false;
+      return KAM_OK;
+    }
+  return fail(c, KAM_ERR_INVALID_ARG, "kam_set_option: unknown key '%s'", key);
+}
 
 // ---- compile side: form the rank-m patch of one chunk ----------------------------------------------------
 kam_status kam_form_patch(kam_ctx* c, const void* const* kv_cond_layers, const void* const* kv_solo_layers, int32_t n_tokens,
@@ -718,7 +904,7 @@ kam_status kam_form_patch(kam_ctx* c, const void* const* kv_cond_layers, const v
   p.smem_bytes = (int)(fl * 4 + 64);
   if (p.smem_bytes > 227 * 1024) return fail(c, KAM_ERR_UNSUPPORTED, "row_dim %d x rank %d does not fit the subspace block in shared memory", p.D, rank);
   const size_t dws = (size_t)p.L * p.H * p.T * p.D * 4, bws = (size_t)p.L * p.H * p.T * p.b * 4;
-  kam_status s = grow_device(c, &c->d_fp_ws, &c->fp_ws_cap, dws + bws + 256, "cudaMalloc(form_patch workspace)");
+  kam_status s = grow_device(c, &c->d_fp_ws, &c->fp_ws_cap, dws + bws + 256, "cudaMalloc(form_patch workspace)", static_cast<cudaStream_t>(stream));
   if (s != KAM_OK) return s;
   p.delta_ws = static_cast<float*>(c->d_fp_ws);
   p.b_ws = reinterpret_cast<float*>(static_cast<char*>(c->d_fp_ws) + ((dws + 255) & ~size_t(255)));

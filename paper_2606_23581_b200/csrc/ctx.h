@@ -20,6 +20,26 @@ struct Staging {                 // pinned host + device buffer pair, reused rou
 };
 constexpr int kStagingSlots = 8;
 
+struct TmapSet { const void* k_layers; const void* v_layers; int32_t num_pages; void* d_tmaps; uint64_t stamp; };
+constexpr int kMaxTmapSets = 8;
+
+// Tunables behind kam_set_option(ctx, key, value).  Nothing in the library reads the process environment.
+struct Options {
+  int reloc_stages = 0;        // "reloc_stages": pipeline stages of the relocate kernel (0 = automatic: 3)
+  int reloc_hg = 0;            // "reloc_head_group": KV heads per slice (0 = automatic)
+  int reloc_kv_split = 1;      // "reloc_kv_split": 1 = automatic (when W_k + W_v crowd out the third stage), 0 = never, 2 = always
+  int reloc_contig = 1;        // "reloc_contig": one unpadded copy per tile when a slice is a whole token row
+  int reloc_rb = 0;            // "reloc_row_blocks": 16-token row blocks per tile (0 = automatic)
+  int reloc_load_hint = 1;     // "reloc_evict_first": canonical sources are read with an L2 evict-first hint
+  int reloc_patch_cost_pct = 108;  // "reloc_patch_cost_pct": cost of a tile that runs the patch, in % of its bytes (work split)
+  int dec_ctas_per_sm = 0;     // "decode_ctas_per_sm" (0 = automatic)
+  int dec_boxes = 0;           // "decode_boxes": ring depth of the decode kernel (0 = automatic)
+  int use_pdl = 1;             // "decode_pdl": programmatic dependent launch between plan, decode and merge
+  int dec_tma = 1;             // "decode_tma": pool pages arrive as TMA tensor-map boxes (0: per-token bulk copies)
+  int host_copy_overlap = 1;   // "host_copy_overlap": kam_relocate_patch_host copies chunk c+1 under the kernel of chunk c
+  int host_sync = 0;           // "host_entries_sync": kam_paged_decode_merge_host ends with a stream synchronise
+};
+
 }  // namespace kam
 
 struct kam_ctx {
@@ -35,8 +55,7 @@ struct kam_ctx {
   bool fast_layout = false;
   std::string fast_layout_why;
   int blocks_per_head = 0;
-  bool contig_copies = true;                  // one unpadded copy per tile when a slice is a whole token row (KAM_RELOC_CONTIG=0: padded per-row copies)
-  int reloc_stages = 0, reloc_load_hint = 1, reloc_rb = 0;  // tuning switches (KAM_RELOC_STAGES, KAM_RELOC_HINT, KAM_RELOC_RB)
+  kam::Options opt;                           // kam_set_option; the defaults are the measured choices
   kam::ColBlock head_blocks[kam::kMaxColBlocks];
 
   kam::Staging staging[kam::kStagingSlots];
@@ -47,12 +66,17 @@ struct kam_ctx {
   int32_t max_requests = 0, max_chunks = 0, max_ppc = 0;
   int32_t* d_slot_pages = nullptr;            // device mirror [n_slots][max_ppc]
 
-  // decode: TMA tensor maps over the context's pool ([n_layers][K,V], 128 bytes each, device memory)
-  void* d_tmaps = nullptr;
+  // decode: TMA tensor maps per pool ([n_layers][K,V], 128 bytes each, device memory); entry 0 = the context's own pool
+  std::vector<kam::TmapSet> tmap_sets;
+  uint64_t tmap_clock = 0;
   std::string tmap_why;                        // why the TMA path is off, if it is
   // decode: workspace (grown on demand); the plan of the window store stays cached in it between layers
-  void* d_ws = nullptr;
+  void* d_ws = nullptr;                        // stateless calls
   size_t ws_cap = 0;
+  bool decplan_valid = false;                  // a plan pinned by kam_paged_decode_plan sits in d_ws
+  alignas(8) unsigned char decplan_key[64] = {};
+  void* d_ws_win = nullptr;                    // window calls: laid out once for max_requests x max_chunks (graph-stable)
+  size_t ws_win_cap = 0;
   uint64_t winplan_epoch = ~0ull;              // window epoch the plan in d_ws was built for (~0 = none)
   std::vector<int32_t> winplan_reqs;
   int32_t winplan_chunks = 0;
@@ -61,11 +85,15 @@ struct kam_ctx {
   bool dec_geom_ok[2][5] = {};
   int32_t dec_max_rank = KAM_MAX_RANK;         // largest rank of an on-read patch (kam_decode_set_max_patch_rank)
   int32_t* d_err = nullptr;                    // device counter: malformed kam_patch_ref records ignored by the decode kernel
-  bool use_pdl = true;                         // programmatic dependent launch between decode and merge (KAM_NO_PDL=1 turns it off)
-  int dec_ctas_per_sm = 0, dec_boxes = 0;      // tuning switches (KAM_DEC_CTAS_PER_SM, KAM_DEC_BOXES); 0 = automatic
+  int64_t generic_launches = 0;                // launches of the element-wise fallback kernel (kam_stats.generic_launches)
   // device staging of host-resident chunks (kam_relocate_patch_host) and host-resident q/out (decode host variant)
-  void* d_hstage = nullptr;
-  size_t hstage_cap = 0;
+  void* d_hstage[2] = {nullptr, nullptr};      // two buffers: the copy of one chunk overlaps the kernel that reads the other
+  size_t hstage_cap[2] = {0, 0};
+  int hstage_next = 0;
+  bool hstage_used[2] = {false, false};
+  cudaStream_t copy_stream = nullptr;          // the library's own H2D stream (kam_relocate_patch_host)
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
+  std::vector<void*> graveyard;                // outgrown device buffers, freed by kam_destroy (see grow_device)
   void* d_hstage2 = nullptr;
   size_t hstage2_cap = 0;
   void* d_fp_ws = nullptr;                     // kam_form_patch: Delta and B workspaces (fp32)
@@ -79,5 +107,6 @@ kam_status staging_acquire(kam_ctx* c, size_t bytes, Staging** out);
 kam_status staging_commit(kam_ctx* c, Staging* s, size_t bytes, cudaStream_t st);
 void staging_release(Staging* s, cudaStream_t st);
 kam_status check_pool(kam_ctx* c, const kam_pool** pool);
-kam_status grow_device(kam_ctx* c, void** buf, size_t* cap, size_t bytes, const char* what);
+const void* tmaps_for_pool(kam_ctx* c, const kam_pool* pool);
+kam_status grow_device(kam_ctx* c, void** buf, size_t* cap, size_t bytes, const char* what, cudaStream_t st);
 }  // namespace kam

@@ -14,16 +14,19 @@ inline size_t align_up_sz(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // Geometry of the decode kernel for this context's layout; `ctas_per_sm` = 0 picks the densest configuration that fits.
 // kt: 16-wide rank tiles of the on-read patch the kernel is specialised for (0 = the call carries no patch refs).
-kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out) {
+kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out, const void** tmaps_out) {
   const kam_layout& L = c->lay;
-  const int variant = (c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers) ? 1 : 0;
+  // TMA tensor maps exist per pool (cached; the first call with a new pool reads its layer pointers back, which synchronises)
+  const void* tmaps = c->opt.dec_tma ? tmaps_for_pool(c, pool) : nullptr;
+  *tmaps_out = tmaps;
+  const int variant = tmaps ? 1 : 0;
   if (c->dec_geom_ok[variant][kt]) { *out = c->dec_geom[variant][kt]; return KAM_OK; }
   if (L.elem_dtype != KAM_BF16) return fail(c, KAM_ERR_UNSUPPORTED, "decode needs a bf16 pool");
   if (!L.has_v) {
     // absorbed MLA decode: one latent+rope row per token, value = its first v_dim columns
     if (L.n_kv_heads != 1 || L.row_dim != 576 || L.v_dim != 512 || L.rope_off != 512 || L.rope_dim != 64)
       return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode is built for rows of 512 latent + 64 rope columns with v_dim 512");
-    if (!variant) return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode needs the context's own pool with page_size %% 16 == 0 (%s)", c->tmap_why.c_str());
+    if (!variant) return fail(c, KAM_ERR_UNSUPPORTED, "MLA decode needs TMA tensor maps over the pool: page_size %% 16 == 0, option decode_tma = 1 (%s)", c->tmap_why.c_str());
     // token-split kernel (decode_mla_ts_kernel.cu): one CTA per SM, 64-token iterations, the on-read patch rides in the ring
     DecodeGeom g{};
     g.mla = 1;
@@ -55,7 +58,7 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
   g.NT = (G + 7) / 8;
   g.rope_off = L.rope_off; g.d_r = L.rope_dim; g.rope_style = L.rope_style;
   g.row_bytes = g.H * g.D * 2; g.slice_bytes = g.HG * g.D * 2;
-  g.use_tma = c->d_tmaps != nullptr && pool->k_layers == c->pool.k_layers && pool->v_layers == c->pool.v_layers;
+  g.use_tma = variant;
   g.ncb = g.HG * g.D / 64;
   g.s_row = g.slice_bytes + 16;                                   // (s_row / 16) odd: ldmatrix rows never share a bank group
   g.kv_bytes = g.use_tma ? 2048 * g.ncb : (int)align_up_sz((size_t)kDecTile * g.s_row, 128);
@@ -70,11 +73,11 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
   g.off_hdr = 128; g.off_box0 = 1024;
   // CTAs per SM x ring depth: 3 CTAs with 2 K + 2 V boxes each when that fits, else fewer CTAs with a deeper ring
   const int sm_total = 227 * 1024;
-  int want = c->dec_ctas_per_sm > 0 ? c->dec_ctas_per_sm : (kt > 0 ? 2 : 3);
+  int want = c->opt.dec_ctas_per_sm > 0 ? c->opt.dec_ctas_per_sm : (kt > 0 ? 2 : 3);
   for (; want >= 1; --want) {
     const int budget = sm_total / want - 1024 - g.off_box0;
     int nb = std::min(8, budget / g.box_bytes) & ~1;
-    if (c->dec_boxes > 0) nb = std::min(nb, c->dec_boxes & ~1);
+    if (c->opt.dec_boxes > 0) nb = std::min(nb, c->opt.dec_boxes & ~1);
     if (nb < 2) continue;
     if (nb < 4 && want > 1) continue;
     g.n_boxes = nb;
@@ -88,8 +91,8 @@ kam_status decode_geom(kam_ctx* c, const kam_pool* pool, int kt, DecodeGeom* out
   return KAM_OK;
 }
 
-// workspace layout in c->d_ws: plan arrays first (chunks | rcb are what the window path uploads), then the partials
-struct WsLayout { size_t chunks, rcb, tile_pre, seg_base, cta_seg, segs, cs, part_lse, part_o, total; int max_segs; };
+// workspace layout: plan arrays first (chunks | rcb are what the window path uploads), then the partials
+struct WsLayout { size_t chunks, rcb, dyn, tile_pre, seg_base, cta_seg, segs, cs, part_lse, part_o, total; int max_segs; };
 WsLayout ws_layout(const DecodeGeom& g, int n_chunks, int batch) {
   WsLayout w{};
   size_t off = 0;
@@ -97,6 +100,7 @@ WsLayout ws_layout(const DecodeGeom& g, int n_chunks, int batch) {
   w.max_segs = g.n_ctas + g.n_hg * n_chunks;
   w.chunks = take((size_t)n_chunks * sizeof(DecChunk));
   w.rcb = take((size_t)(batch + 1) * 4);
+  w.dyn = take(16);
   w.tile_pre = take((size_t)(n_chunks + 1) * 4);
   w.seg_base = take(((size_t)g.n_hg * n_chunks + 1) * 4);
   w.cta_seg = take((size_t)(g.n_ctas + 1) * 4);
@@ -108,11 +112,12 @@ WsLayout ws_layout(const DecodeGeom& g, int n_chunks, int batch) {
   return w;
 }
 
-DecodePlan plan_of(kam_ctx* c, const WsLayout& w, int n_chunks, int batch) {
-  char* ws = static_cast<char*>(c->d_ws);
+DecodePlan plan_of(kam_ctx* c, void* base, const WsLayout& w, int n_chunks, int batch) {
+  char* ws = static_cast<char*>(base);
   DecodePlan pl{};
   pl.chunks = reinterpret_cast<DecChunk*>(ws + w.chunks);
   pl.rcb = reinterpret_cast<int32_t*>(ws + w.rcb);
+  pl.dyn = reinterpret_cast<int32_t*>(ws + w.dyn);
   pl.tile_pre = reinterpret_cast<int32_t*>(ws + w.tile_pre);
   pl.seg_base = reinterpret_cast<int32_t*>(ws + w.seg_base);
   pl.cta_seg = reinterpret_cast<int32_t*>(ws + w.cta_seg);
@@ -124,59 +129,87 @@ DecodePlan plan_of(kam_ctx* c, const WsLayout& w, int n_chunks, int batch) {
   return pl;
 }
 
-kam_status grow_ws(kam_ctx* c, size_t bytes) {
-  if (c->ws_cap >= bytes) return KAM_OK;
-  c->winplan_epoch = ~0ull;                                       // the cached window plan lives in the old buffer
-  return grow_device(c, &c->d_ws, &c->ws_cap, bytes + bytes / 4, "cudaMalloc(decode workspace)");
+struct PlanKey {                 // what a stateless plan was built from (kam_paged_decode_plan)
+  const void *bt, *starts, *offs, *nc, *pool_k;
+  int32_t max_pages, max_chunks, batch, kt;
+  bool operator==(const PlanKey& o) const {
+    return bt == o.bt && starts == o.starts && offs == o.offs && nc == o.nc && pool_k == o.pool_k && max_pages == o.max_pages &&
+           max_chunks == o.max_chunks && batch == o.batch && kt == o.kt;
+  }
+};
+static_assert(sizeof(PlanKey) <= sizeof(((kam_ctx*)nullptr)->decplan_key), "plan key storage");
+
+inline int patch_tiles(const kam_ctx* c, bool has_patches) {
+  return has_patches ? (c->dec_max_rank <= 16 ? 1 : c->dec_max_rank <= 32 ? 2 : 4) : 0;
 }
 
 }  // namespace
 
+// plan_only: build and pin the plan, launch nothing else.  q == NULL is only legal then.
 static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables,
                                    int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
-                                   const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, int32_t layer,
-                                   int32_t batch, float sm_scale, void* out, float* lse, bool out_f32, void* stream) {
+                                   const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, bool has_patches,
+                                   int32_t layer, int32_t batch, float sm_scale, void* out, float* lse, bool out_f32,
+                                   bool plan_only, void* stream) {
   if (!c) return KAM_ERR_INVALID_ARG;
   kam_status s = check_pool(c, &pool);
   if (s != KAM_OK) return s;
-  if (!q || !block_tables || !chunk_starts || !n_chunks || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge: NULL argument");
-  if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge: q and out must be 16-byte aligned");
-  if (layer < 0 || layer >= c->lay.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, c->lay.n_layers);
+  if (!block_tables || !chunk_starts || !n_chunks) return fail(c, KAM_ERR_INVALID_ARG, "decode: NULL metadata argument");
+  if (!plan_only) {
+    if (!q || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge: NULL argument");
+    if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge: q and out must be 16-byte aligned");
+    if (layer < 0 || layer >= c->lay.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, c->lay.n_layers);
+  }
   if (batch < 0 || max_pages < 1 || max_chunks < 1) return fail(c, KAM_ERR_INVALID_ARG, "bad batch / max_pages / max_chunks");
   if (batch == 0) return KAM_OK;
   if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
   if ((long long)batch * max_chunks > (1ll << 24)) return fail(c, KAM_ERR_UNSUPPORTED, "batch * max_chunks too large");
-  DecodeGeom g;
-  const int kt = patches ? (c->dec_max_rank <= 16 ? 1 : c->dec_max_rank <= 32 ? 2 : 4) : 0;
-  if ((s = decode_geom(c, pool, kt, &g)) != KAM_OK) return s;
+  DecodeGeom g; const void* tmaps = nullptr;
+  const int kt = patch_tiles(c, has_patches);
+  if ((s = decode_geom(c, pool, kt, &g, &tmaps)) != KAM_OK) return s;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
 
   const int N = batch * max_chunks;
   const WsLayout w = ws_layout(g, N, batch);
-  if ((s = grow_ws(c, w.total)) != KAM_OK) return s;
-  c->winplan_epoch = ~0ull;                                       // this call overwrites the plan area
+  if (c->ws_cap < w.total) {
+    c->decplan_valid = false;                                     // a pinned plan lives in the old buffer
+    if ((s = grow_device(c, &c->d_ws, &c->ws_cap, w.total + w.total / 4, "cudaMalloc(decode workspace)", st)) != KAM_OK) return s;
+  }
+  // The plan depends on the paging metadata only, not on the layer or the query: a plan pinned by kam_paged_decode_plan is
+  // reused by every call that names the same arrays and sizes (the caller re-plans when their CONTENT changes).
+  PlanKey key{block_tables, chunk_starts, chunk_offsets, n_chunks, pool->k_layers, max_pages, max_chunks, batch, kt};
+  const bool reuse = !plan_only && c->decplan_valid && key == *reinterpret_cast<const PlanKey*>(c->decplan_key);
 
   DecodeParams p{};
   p.q = q; p.pool_k_layers = pool->k_layers; p.pool_v_layers = pool->v_layers; p.layer = layer;
-  p.block_tables = block_tables; p.tmaps = c->d_tmaps;
-  p.plan = plan_of(c, w, N, batch);
+  p.block_tables = block_tables; p.tmaps = tmaps;
+  p.plan = plan_of(c, c->d_ws, w, N, batch);
   p.plan.block_tables = block_tables;
   p.patches = patches; p.err = c->d_err;
   p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.out_f32 = out_f32 ? 1 : 0;
 
-  DecodeCsr csr{};
-  csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
-  csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = patches ? 1 : 0;
-  launch_decode_plan(g, p.plan, csr, st);
-  // the decode kernels read the plan just written: with programmatic dependent launch only their prologue (barrier setup,
-  // shared-memory carve-up, launch latency) overlaps the plan kernel - plan_fresh makes them wait before the first plan read
-  p.plan_fresh = 1;
-  if (g.mla) launch_mla_ts_decode(g, p, c->use_pdl, st);
-  else launch_decode(g, p, c->use_pdl, st);
-  launch_decode_merge(g, p, c->use_pdl, st);
-  c->kernels_launched += 3;
+  const bool pdl = c->opt.use_pdl != 0;
+  if (!reuse) {
+    DecodeCsr csr{};
+    csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
+    csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = has_patches ? 1 : 0;
+    launch_decode_plan(g, p.plan, csr, st);
+    ++c->kernels_launched;
+    c->decplan_valid = plan_only;
+    if (plan_only) memcpy(c->decplan_key, &key, sizeof key);
+  }
+  if (!plan_only) {
+    // a plan written by the kernel just before this one: with programmatic dependent launch only the decode kernel's prologue
+    // (barrier setup, shared-memory carve-up, launch latency) overlaps the plan kernel - plan_fresh makes it wait before the
+    // first plan read.  A reused plan is older than anything on the stream that could still be writing it.
+    p.plan_fresh = reuse ? 0 : 1;
+    if (g.mla) launch_mla_ts_decode(g, p, pdl, st);
+    else launch_decode(g, p, pdl, st);
+    launch_decode_merge(g, p, pdl, st);
+    c->kernels_launched += 2;
+  }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(c, e, "decode launch");
   return KAM_OK;
@@ -184,20 +217,30 @@ static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* po
 
 extern "C" {
 
+kam_status kam_paged_decode_plan(kam_ctx* c, const kam_pool* pool, const int32_t* block_tables, int32_t max_pages,
+                                 const int32_t* chunk_starts, const int64_t* chunk_offsets, const int32_t* n_chunks,
+                                 int32_t max_chunks, int32_t has_patches, int32_t batch, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  c->decplan_valid = false;
+  if (batch == 0 || !block_tables) return KAM_OK;                  // release
+  return decode_stateless(c, nullptr, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, nullptr,
+                          has_patches != 0, 0, batch, 0.f, nullptr, nullptr, false, true, stream);
+}
+
 kam_status kam_paged_decode_merge(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables,
                                   int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
                                   const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, int32_t layer,
                                   int32_t batch, float sm_scale, void* out, float* lse, void* stream) {
-  return decode_stateless(c, q, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, patches, layer,
-                          batch, sm_scale, out, lse, false, stream);
+  return decode_stateless(c, q, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, patches,
+                          patches != nullptr, layer, batch, sm_scale, out, lse, false, false, stream);
 }
 
 kam_status kam_paged_decode_state(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables,
                                   int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
                                   const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches, int32_t layer,
                                   int32_t batch, float sm_scale, float* o_state, float* lse_state, void* stream) {
-  return decode_stateless(c, q, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, patches, layer,
-                          batch, sm_scale, o_state, lse_state, true, stream);
+  return decode_stateless(c, q, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, patches,
+                          patches != nullptr, layer, batch, sm_scale, o_state, lse_state, true, false, stream);
 }
 
 kam_status kam_lse_merge_states(kam_ctx* c, int32_t n_parts, const float* const* o_states, const float* const* lse_states,
@@ -224,27 +267,30 @@ kam_status kam_lse_merge_states(kam_ctx* c, int32_t n_parts, const float* const*
 
 // The plan (segments, first slots, cos/sin tables) depends only on the windows, not on the layer or the query: it is
 // rebuilt when a window changed (epoch) or the request list differs, and reused by every layer of the same step.
+// The window path has a workspace of its own, laid out ONCE for the largest plan the window store can produce
+// (max_requests x max_chunks_per_request chunks): the addresses a decode launch carries never depend on how many chunks the
+// windows hold right now, so a CUDA graph captured over kam_window_decode stays valid while windows grow, shrink and slide.
 static kam_status window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch, cudaStream_t st, DecodeGeom* g_out,
                               WsLayout* w_out, bool* was_cached) {
   if (!c->win) return fail(c, KAM_ERR_STATE, "context was created without a window store");
   if (!c->has_pool || !c->cuda_ok) return fail(c, KAM_ERR_CUDA, "window decode needs a context with a pool on a CUDA device");
-  if (!req_ids || batch < 1) return fail(c, KAM_ERR_INVALID_ARG, "window decode: bad request list");
+  if (!req_ids || batch < 1 || batch > c->max_requests) return fail(c, KAM_ERR_INVALID_ARG, "window decode: bad request list");
   for (int b = 0; b < batch; ++b)
     if (!c->win->is_open(req_ids[b])) return fail(c, KAM_ERR_STATE, "request %d is not open", req_ids[b]);
-  DecodeGeom g;
-  kam_status s = decode_geom(c, &c->pool, 0, &g);
+  DecodeGeom g; const void* tmaps = nullptr;
+  kam_status s = decode_geom(c, &c->pool, 0, &g, &tmaps);
   if (s != KAM_OK) return s;
   const bool cached = c->winplan_epoch == c->win->epoch() && c->winplan_reqs.size() == (size_t)batch &&
                       std::equal(c->winplan_reqs.begin(), c->winplan_reqs.end(), req_ids);
-  int N = c->winplan_chunks;
-  if (!cached) {
-    N = 0;
-    for (int b = 0; b < batch; ++b) N += (int)c->win->chunks(req_ids[b]).size();
-  }
-  const WsLayout w = ws_layout(g, N, batch);
+  const int n_max = c->max_requests * c->max_chunks;
+  const WsLayout w = ws_layout(g, n_max, c->max_requests);
   *g_out = g; *w_out = w; *was_cached = cached;
   if (cached) return KAM_OK;
-  if ((s = grow_ws(c, w.total)) != KAM_OK) return s;
+  // (re)allocation happens on the first plan only - or after kam_set_option changed the kernel's geometry, which invalidates
+  // captured graphs anyway (kamera.h)
+  if ((s = grow_device(c, &c->d_ws_win, &c->ws_win_cap, w.total, "cudaMalloc(window decode workspace)", st)) != KAM_OK) return s;
+  int N = 0;
+  for (int b = 0; b < batch; ++b) N += (int)c->win->chunks(req_ids[b]).size();
   // host -> device: the flat chunk list (pending lazy deltas become on-read rotations) and the request index
   const size_t up_bytes = w.rcb + (size_t)(batch + 1) * 4;
   Staging* sg;
@@ -265,10 +311,13 @@ static kam_status window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch,
     }
   }
   hr[batch] = j;
-  cudaError_t e = cudaMemcpyAsync(c->d_ws, h, up_bytes, cudaMemcpyHostToDevice, st);
+  // two copies: the chunk records are N entries, the request index sits at its fixed offset behind room for n_max of them
+  cudaError_t e = cudaMemcpyAsync(c->d_ws_win, h, (size_t)N * sizeof(DecChunk), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(static_cast<char*>(c->d_ws_win) + w.rcb, h + w.rcb, (size_t)(batch + 1) * 4, cudaMemcpyHostToDevice, st);
   staging_release(sg, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(window plan)");
-  DecodePlan pl = plan_of(c, w, N, batch);
+  DecodePlan pl = plan_of(c, c->d_ws_win, w, N, batch);
   pl.block_tables = c->d_slot_pages;
   DecodeCsr csr{};
   launch_decode_plan(g, pl, csr, st);
@@ -286,6 +335,7 @@ kam_status kam_decode_set_max_patch_rank(kam_ctx* c, int32_t max_rank) {
   if (!c) return KAM_ERR_INVALID_ARG;
   if (max_rank != 16 && max_rank != 32 && max_rank != 64) return fail(c, KAM_ERR_INVALID_ARG, "max patch rank must be 16, 32 or 64 (got %d)", max_rank);
   c->dec_max_rank = max_rank;
+  c->decplan_valid = false;
   return KAM_OK;
 }
 
@@ -309,16 +359,19 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   if (s != KAM_OK) return s;
   DecodeParams p{};
   p.q = q; p.pool_k_layers = c->pool.k_layers; p.pool_v_layers = c->pool.v_layers; p.layer = layer;
-  p.block_tables = c->d_slot_pages; p.tmaps = c->d_tmaps;
-  p.plan = plan_of(c, w, c->winplan_chunks, batch);
+  p.block_tables = c->d_slot_pages; p.tmaps = c->opt.dec_tma ? tmaps_for_pool(c, &c->pool) : nullptr;
+  // the one plan size a kernel needs (the chunk count, in the merge) is read from the workspace (DecodePlan::dyn), so the
+  // parameters a captured graph replays stay right when the windows change
+  p.plan = plan_of(c, c->d_ws_win, w, c->winplan_chunks, batch);
   p.plan.block_tables = c->d_slot_pages;
-  p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_o);
-  p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws) + w.part_lse);
+  p.part_o = reinterpret_cast<float*>(static_cast<char*>(c->d_ws_win) + w.part_o);
+  p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws_win) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.err = c->d_err;
+  const bool pdl = c->opt.use_pdl != 0;
   // with a plan from an earlier call the decode prologue may overlap whatever precedes it on the stream (it only reads the plan)
-  if (g.mla) launch_mla_ts_decode(g, p, cached && c->use_pdl, st);
-  else launch_decode(g, p, cached && c->use_pdl, st);
-  launch_decode_merge(g, p, c->use_pdl, st);
+  if (g.mla) launch_mla_ts_decode(g, p, cached && pdl, st);
+  else launch_decode(g, p, cached && pdl, st);
+  launch_decode_merge(g, p, pdl, st);
   c->kernels_launched += 2;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(c, e, "decode launch");
@@ -339,10 +392,12 @@ kam_status kam_paged_decode_merge_host(kam_ctx* c, const void* q_host, const kam
   const size_t qb = (size_t)batch * L.n_q_heads * L.row_dim * 2, lb = (size_t)batch * L.n_q_heads * 4;
   const size_t ob = L.has_v ? qb : (size_t)batch * L.n_q_heads * L.v_dim * 2;
   const size_t o_off = (qb + 255) & ~size_t(255), l_off = (o_off + ob + 255) & ~size_t(255);
-  kam_status s = grow_device(c, &c->d_hstage2, &c->hstage2_cap, l_off + lb, "cudaMalloc(decode host staging)");
-  if (s != KAM_OK) return s;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  char* d = static_cast<char*>(c->d_hstage2);
+  // one staging region per layer (q | out | lse): the calls of a step do not wait for one another's D2H copies
+  const size_t per = (l_off + lb + 255) & ~size_t(255);
+  kam_status s = grow_device(c, &c->d_hstage2, &c->hstage2_cap, per * L.n_layers, "cudaMalloc(decode host staging)", st);
+  if (s != KAM_OK) return s;
+  char* d = static_cast<char*>(c->d_hstage2) + per * (layer >= 0 && layer < L.n_layers ? layer : 0);
   cudaError_t e = cudaMemcpyAsync(d, q_host, qb, cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(q)");
   s = kam_paged_decode_merge(c, d, pool, block_tables, max_pages, chunk_starts, chunk_offsets, n_chunks, max_chunks, patches,
@@ -350,7 +405,7 @@ kam_status kam_paged_decode_merge_host(kam_ctx* c, const void* q_host, const kam
   if (s != KAM_OK) return s;
   if ((e = cudaMemcpyAsync(out_host, d + o_off, ob, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(out)");
   if ((e = cudaMemcpyAsync(lse_host, d + l_off, lb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(lse)");
-  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+  if (c->opt.host_sync && (e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
   return KAM_OK;
 }
 

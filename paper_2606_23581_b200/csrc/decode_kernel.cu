@@ -114,6 +114,7 @@ __global__ void __launch_bounds__(kDecPlanThreads) kam_decode_plan_kernel(const 
     return;
   }
 
+  if (tid == 0) pl.dyn[0] = N;
   // ---- phase 0: chunk records of the stateless call (CSR token boundaries per request)
   if (csr.enabled) {
     for (int j = tid; j < N; j += blockDim.x) {
@@ -712,7 +713,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) kam_lse_merge_kernel(const _
   const int bh = blockIdx.x;                      // b * Hq + hq
   const int b = bh / g.Hq, hq = bh - b * g.Hq;
   const int hg = hq / g.R, r = hq - hg * g.R;
-  const int N = p.plan.n_chunks;
+  const int N = p.plan.dyn[0];                    // see DecodePlan::dyn
   const int s0 = p.plan.seg_base[hg * N + p.plan.rcb[b]], s1 = p.plan.seg_base[hg * N + p.plan.rcb[b + 1]];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   grid_dep_wait();                                // the partials are complete and visible from here

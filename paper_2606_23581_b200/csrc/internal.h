@@ -23,9 +23,11 @@ struct RelocDescDev {
   long long u_head_stride;       // elements; 0 => U shared by all heads
   int32_t n_tokens;
   int32_t flags;
+  int32_t tile_weight;           // relative cost of one tile of this chunk (the CTAs' shares are cut by weight, not by count)
   uint8_t rank_l[KAM_MAX_LAYERS];
 };
-enum : int32_t { FLAG_INPLACE = 1, FLAG_CANONICAL_FRAME = 2 };
+enum : int32_t { FLAG_INPLACE = 1, FLAG_CANONICAL_FRAME = 2,
+                 FLAG_INLINE_PAGES = 4 };   // the chunk's page list is RelocPages in the kernel parameters, not block_table
 
 // A column block of a token's slice: what one warp processes for 16 tokens (up to 4 groups of 32 columns).
 struct ColBlock {
@@ -55,7 +57,9 @@ struct RelocGeom {
   int32_t RB, TT;               // 16-token row blocks per tile; TT = 16 * RB tokens
   int32_t nkv;                  // 2 with a V pool, 1 for MLA
   int32_t n_blocks;
-  int32_t KT_max;               // max rank / 16 over the call
+  int32_t KT_max;               // 16-wide rank tiles of the largest rank of the call: ceil(max rank / 16)
+  int32_t kv_split;             // 1: a tile carries K rows OR V rows (the tile list gets a kv level): only one of W_k / W_v is
+                                //    resident at a time, which is what lets three stages fit at ranks 48 / 64
   int32_t rope_style, d_r, half_groups;   // half_groups = d_r / 64 for HALF
   int32_t n_stages;
   int32_t off_tab, off_cs, off_w, off_stage0, stage_bytes;   // byte offsets in dynamic shared memory
@@ -72,16 +76,29 @@ constexpr int kRelocInlineDescs = 8;   // batches up to this size travel in the 
 struct RelocInline {
   RelocDescDev d[kRelocInlineDescs];
   long long prefix[kRelocInlineDescs + 1];
+  long long wprefix[kRelocInlineDescs + 1];
+};
+// The page list of a chunk admitted to a window travels in the kernel parameters too: the kernel maps its slots from here and
+// CTA 0 writes the list to the device mirror of the window's page lists - a slide is one launch and no copy.
+constexpr int kRelocInlinePages = 256;
+struct RelocPages {
+  int32_t pages[kRelocInlinePages];
+  int32_t* mirror_dst;           // device mirror row of the chunk's slot, or nullptr (no inline page list in this launch)
+  int32_t n;
 };
 
 struct RelocParams {
   const RelocDescDev* descs;     // device array, or nullptr => RelocInline
   const long long* tile_prefix;  // [n_descs + 1]
+  const long long* w_prefix;     // [n_descs + 1] cumulative tile weights
+  long long total_weight;
   void* const* pool_k;
   void* const* pool_v;
   const double* inv_freq;        // [d_r / 2] f_i = theta^(-2i/d_r) in fp64 (written at kam_create), or nullptr
   long long total_tiles;
   int32_t n_descs;
+  int32_t num_pages;             // block-table entries outside [0, num_pages) are skipped and counted in *err
+  int32_t* err;                  // device counter (kam_stats.device_errors)
 };
 
 // generic (any dtype / rank / width) element-wise path
@@ -90,10 +107,12 @@ struct GenericParams {
   void* const* pool_k;
   void* const* pool_v;
   int32_t n_descs, L, H, D, P, rope_off, d_r, rope_style, has_v, elem_f32, factor_f32;
+  int32_t num_pages;
+  int32_t* err;
   double theta;
 };
 
-void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, int grid, cudaStream_t st);
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages& pages, int grid, cudaStream_t st);
 void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
 
 // ---------------------------------------------------------------- decode
@@ -149,6 +168,9 @@ struct DecodePlan {              // device pointers into the workspace; filled b
   float2* cs;                    // [n_chunks][d_r / 2] (cos, sin)(delta f_i)
   const double* inv_freq;        // [d_r / 2] f_i = theta^(-2i/d_r), fp64, written at kam_create
   const int32_t* block_tables;   // the call's block-table array (segments record their first slot)
+  int32_t* dyn;                  // [0] = n_chunks as the plan kernel saw it.  The merge kernel reads it from HERE, not from its
+                                 // parameters: a CUDA graph captured over kam_window_decode replays stale parameters after
+                                 // the windows' chunk count changed, the workspace is always current
   int32_t n_chunks, batch, max_segs;
 };
 

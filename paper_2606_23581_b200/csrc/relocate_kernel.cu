@@ -26,37 +26,53 @@ namespace kam {
 
 namespace {
 
-// Incremental (division-free) walk over the flat tile list: chunk d -> layer l -> head group hg -> token tile tt.
+// Incremental (division-free) walk over the flat tile list: chunk d -> layer l -> head group hg -> kv -> token tile tt.
+// kv level: only in kv-split geometry (a tile carries K rows or V rows), and only for chunks that have V rows to write.
+// Survivors rotated in place inside a K+V launch use the V half of a stage for K rows too: their tiles hold 2 * TT tokens.
 struct TileWalk {
-  int d, l, hg, tt, n_tt, n_tokens;
+  int d, l, hg, kv, tt, n_tt, n_kv, n_tokens, tile_tok;
   long long d_end;                       // first tile index of the next chunk
+  __device__ __forceinline__ void set_desc(const RelocGeom& g, const RelocDescDev& desc) {
+    n_tokens = desc.n_tokens;
+    const bool inplace = desc.flags & FLAG_INPLACE;
+    tile_tok = (inplace && g.nkv == 2 && !g.kv_split) ? 2 * g.TT : g.TT;
+    n_tt = (n_tokens + tile_tok - 1) / tile_tok;
+    n_kv = (g.kv_split && g.nkv == 2 && !inplace) ? 2 : 1;
+  }
   __device__ __forceinline__ void init(const RelocGeom& g, int n_descs, const RelocDescDev* descs, const long long* tile_prefix, long long tile) {
     int lo = 0, hi = n_descs;            // largest d with prefix[d] <= tile
     while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (tile_prefix[mid] <= tile) lo = mid; else hi = mid; }
     d = lo;
     while (tile_prefix[d + 1] <= tile) ++d;            // skip empty chunks
-    n_tokens = descs[d].n_tokens;
-    n_tt = (n_tokens + g.TT - 1) / g.TT;
+    set_desc(g, descs[d]);
     d_end = tile_prefix[d + 1];
     const int local = static_cast<int>(tile - tile_prefix[d]);
     tt = local % n_tt;
-    const int uu = local / n_tt;
+    int uu = local / n_tt;
+    kv = uu % n_kv; uu /= n_kv;
     hg = uu % g.n_hg;
     l = uu / g.n_hg;
   }
   __device__ __forceinline__ void next(const RelocGeom& g, const RelocDescDev* descs, const long long* tile_prefix, long long new_tile) {
     if (++tt < n_tt) return;
     tt = 0;
+    if (++kv < n_kv) return;
+    kv = 0;
     if (++hg < g.n_hg) return;
     hg = 0;
     if (++l < g.L) return;
     l = 0;
     do { ++d; } while (tile_prefix[d + 1] <= new_tile);
-    n_tokens = descs[d].n_tokens;
-    n_tt = (n_tokens + g.TT - 1) / g.TT;
+    set_desc(g, descs[d]);
     d_end = tile_prefix[d + 1];
   }
 };
+
+// U of a (chunk, layer) travels in its native form - one contiguous run per tile, the caller's strides kept in shared memory -
+// when a token's U row fits the stage's U area and the slice holds all heads of the row (or U is shared by all heads).
+__device__ __forceinline__ bool u_native(const RelocGeom& g, long long u_tok_stride, long long u_head_stride) {
+  return u_tok_stride * 2 <= g.su_row && (u_head_stride == 0 || g.n_hg == 1);
+}
 
 // ---- packed fp32 pairs (sm_100a FFMA2 / FMUL2): two fp32 lanes per 64-bit register pair
 __device__ __forceinline__ uint64_t pk2(float lo, float hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
@@ -133,6 +149,11 @@ struct SlabArgs {
   int s_row, w_row16, half;  // token stride in the stage; bytes of 16 k-rows of W; d_r / 2
   int steps;                 // pairs of 32-column groups
   bool ok0, ok1, canonical;
+  // ranks that are not a multiple of 16: the A fragments are gathered element by element, columns >= m_rag read as zero
+  // (the W rows behind them are zero in shared memory too, so the padded products vanish exactly)
+  const uint8_t* ug;         // U[token row lane/4][head][0] of this slab in the stage
+  int su;                    // token stride of U in the stage (bytes)
+  int m_rag;                 // 0: rank is a multiple of 16 (ldmatrix path); else the rank
 };
 
 // A step = two 32-column groups (gA, gB) x 16 tokens: HALF pairs group sp with group sp + steps (column i with i + d_r/2).
@@ -176,8 +197,21 @@ __device__ __forceinline__ void slab_steps(const SlabArgs& s, const uint32_t (*a
 template <int KT>
 __device__ __forceinline__ void slab_run(const SlabArgs& s, int rope, uint32_t ua) {
   uint32_t afr[KT > 0 ? KT : 1][4];
+  if (KT > 0 && s.m_rag) {
+    const int t4 = threadIdx.x & 3;
 #pragma unroll
-  for (int kt = 0; kt < KT; ++kt) ldmatrix_x4(afr[kt][0], afr[kt][1], afr[kt][2], afr[kt][3], ua + kt * 32);
+    for (int kt = 0; kt < KT; ++kt)
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const int k0 = kt * 16 + 2 * t4 + (r >> 1) * 8;
+        const uint16_t* row = reinterpret_cast<const uint16_t*>(s.ug + (r & 1) * 8 * s.su);
+        const uint32_t lo = k0 < s.m_rag ? row[k0] : 0u, hi = k0 + 1 < s.m_rag ? row[k0 + 1] : 0u;
+        afr[kt][r] = lo | (hi << 16);
+      }
+  } else {
+#pragma unroll
+    for (int kt = 0; kt < KT; ++kt) ldmatrix_x4(afr[kt][0], afr[kt][1], afr[kt][2], afr[kt][3], ua + kt * 32);
+  }
   if (s.steps == 2) {
     if (rope == ROPE_NONE) slab_steps<KT, ROPE_NONE, 2>(s, afr);
     else if (rope == ROPE_HALF) slab_steps<KT, ROPE_HALF, 2>(s, afr);
@@ -192,11 +226,17 @@ __device__ __forceinline__ void slab_run(const SlabArgs& s, int rope, uint32_t u
 }  // namespace
 
 // Shared-memory map (dynamic): [0,128) mbarriers | slab table | cos/sin table | W (column-permuted, padded rows) | stages.
-// W in shared memory is [kv][head-in-group][k][D + 8] bf16 with the columns of every 32-group stored in MMA order
-// (position 8j + 2i + e holds column 8i + 2j + e), so that ldmatrix.trans yields B fragments whose accumulator columns
-// are 8 CONTIGUOUS columns per thread.
+// W in shared memory is [kv][head-in-group][k < 16 * KT][D + 8] bf16 (rows k >= m are zero: the rank is padded to a multiple of
+// 16 there, never in HBM) with the columns of every 32-group stored in MMA order (position 8j + 2i + e holds column
+// 8i + 2j + e), so that ldmatrix.trans yields B fragments whose accumulator columns are 8 CONTIGUOUS columns per thread.
+// A stage is [K rows | V rows | U_k | U_v | slots]; three tile forms share it:
+//   K+V tile     (a chunk with V, plain geometry)   : TT tokens, K rows and V rows of the same tokens
+//   in-place x2  (a survivor inside a K+V launch)   : 2 * TT tokens of K; the second half lands in the V area, so a slide's
+//                                                     survivors keep a full stage of bytes in flight beside the recalled chunk
+//   kv-split     (ranks 48 / 64)                    : TT tokens of K or of V in the K area, its U in the U_k area
 __global__ void __launch_bounds__(kRelocThreads, 1)
-kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_constant__ RelocParams p, const __grid_constant__ RelocInline inl) {
+kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_constant__ RelocParams p, const __grid_constant__ RelocInline inl,
+                          const __grid_constant__ RelocPages pages) {
   extern __shared__ __align__(128) uint8_t smem[];
   uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem);
   uint64_t* empty_bar = full_bar + g.n_stages;
@@ -210,11 +250,12 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
     mbar_fence_init();
   }
   if (threadIdx.x < 2 * g.RB * g.n_blocks) {
-    // slab s -> (kv, row block, column block), K slabs first; everything a consumer needs, as byte offsets
+    // slab s -> (half, row block, column block); everything a consumer needs, as byte offsets.  half = 1: the V rows of a
+    // K+V tile, or the second TT tokens of an in-place x2 tile.  The rope kind is the block's; V slabs ignore it.
     const int s = threadIdx.x, per = g.RB * g.n_blocks;
     const int kv = s / per, rem = s - kv * per, rb = rem / g.n_blocks;
     const ColBlock cb = g.blk[rem % g.n_blocks];
-    const int rope = (kv == 0 && cb.rope) ? (g.rope_style == KAM_ROPE_HALF ? ROPE_HALF : ROPE_INTER) : ROPE_NONE;
+    const int rope = cb.rope ? (g.rope_style == KAM_ROPE_HALF ? ROPE_HALF : ROPE_INTER) : ROPE_NONE;
     const int tab_off = g.rope_style == KAM_ROPE_HALF ? cb.band_col0 : cb.band_col0 >> 1;       // first frequency of the block
     slab_tab[s] = make_int4(kv | (rb << 4) | (cb.fhead << 8) | (rope << 16) | ((cb.n_groups >> 1) << 20),
                             cb.col_off * 2, cb.w_col_off * 2, tab_off);
@@ -224,11 +265,28 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   // small batches carry their descriptors in the kernel parameters (no H2D staging copy, no global loads to read them)
   const RelocDescDev* descs = p.descs ? p.descs : inl.d;
   const long long* tile_prefix = p.descs ? p.tile_prefix : inl.prefix;
-  const long long t_begin = p.total_tiles * blockIdx.x / gridDim.x;
-  const long long t_end = p.total_tiles * (blockIdx.x + 1) / gridDim.x;
+  const long long* w_prefix = p.descs ? p.w_prefix : inl.wprefix;
+  // the page list of a chunk just admitted to a window: CTA 0 publishes it to the device mirror (read by later launches only)
+  if (pages.mirror_dst && blockIdx.x == 0)
+    for (int i = threadIdx.x; i < pages.n; i += blockDim.x) pages.mirror_dst[i] = pages.pages[i];
+  // CTA i owns the tiles whose cumulative WEIGHT falls in [W i / n, W (i+1) / n): tiles of one chunk weigh the same, tiles of
+  // different chunks do not (a survivor rotated in place moves K only and runs no MMA; a recalled chunk moves K, V, U and runs
+  // the patch) - equal COUNTS left the CTAs of a slide 13 % apart (profiles/ncu_slide_r02.md)
+  auto cut = [&](unsigned i) -> long long {
+    if (i >= gridDim.x) return p.total_tiles;
+    const long long b = p.total_weight * i / gridDim.x;
+    int lo = 0, hi = p.n_descs;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (w_prefix[mid] <= b) lo = mid; else hi = mid; }
+    while (lo + 1 < p.n_descs && w_prefix[lo + 1] <= b) ++lo;
+    const int tw = descs[lo].tile_weight;
+    const long long t = tile_prefix[lo] + (tw > 0 ? (b - w_prefix[lo]) / tw : 0);
+    return t < tile_prefix[lo + 1] ? t : tile_prefix[lo + 1];
+  };
+  const long long t_begin = cut(blockIdx.x), t_end = cut(blockIdx.x + 1);
   if (t_begin >= t_end) return;
   TileWalk w;
   w.init(g, p.n_descs, descs, tile_prefix, t_begin);
+  const bool split = g.kv_split;
 
   if (warp >= kRelocConsumerWarps) {
     // ================================================================ producer warps: K | V | U_k | U_v
@@ -236,60 +294,77 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
     // entries of a tile are loaded BEFORE the wait for a free stage, so their latency hides behind it.
     const int role = warp - kRelocConsumerWarps;
     int stage = 0; uint32_t phase = 0;
-    int cur_d = -1, cur_l = -1;
-    // per (chunk, layer) state
+    int cur_d = -1, cur_l = -1, cur_kv = -1;
+    // per (chunk, layer[, kv]) state
     const char* src = nullptr; const int32_t* bt = nullptr;
     long long u_tok_stride = 0, u_head_stride = 0;
     int dst0 = 0, m = 0, flags = 0;
+    bool dbl = false;                      // in-place x2 tile form
     for (long long tile = t_begin; tile < t_end; ++tile) {
-      if (w.d != cur_d || w.l != cur_l) {
-        cur_d = w.d; cur_l = w.l;
+      if (w.d != cur_d || w.l != cur_l || w.kv != cur_kv) {
+        cur_d = w.d; cur_l = w.l; cur_kv = w.kv;
         const RelocDescDev& desc = descs[w.d];
-        flags = desc.flags; m = desc.rank_l[w.l]; bt = desc.block_table; dst0 = static_cast<int>(desc.dst_token_start);
+        flags = desc.flags; m = desc.rank_l[w.l]; dst0 = static_cast<int>(desc.dst_token_start);
+        bt = (flags & FLAG_INLINE_PAGES) ? pages.pages : desc.block_table;
         u_tok_stride = desc.u_token_stride; u_head_stride = desc.u_head_stride;
         const bool inplace = flags & FLAG_INPLACE;
-        const void* const* tab_l = role == 0 ? desc.k_src : role == 1 ? desc.v_src : role == 2 ? desc.Uk : desc.Uv;
+        dbl = inplace && g.nkv == 2 && !split;
+        // what this warp streams for this (chunk, layer, kv): sel 0 = K rows, 1 = V rows, 2 = U_k, 3 = U_v, -1 = nothing
+        int sel = role;
+        if (split) sel = (role & 1) ? -1 : role + w.kv;
         src = nullptr;
-        if (role == 0) src = inplace ? static_cast<const char*>(p.pool_k[w.l]) : static_cast<const char*>(tab_l[w.l]);
-        else if (role == 1) { if (!inplace && g.nkv == 2) src = static_cast<const char*>(tab_l[w.l]); }
-        else if (m && tab_l && !inplace && (role == 2 || g.nkv == 2)) src = static_cast<const char*>(tab_l[w.l]);
-        if (role >= 2 && src) {
-          // the consumers stage this (chunk, layer)'s W a few tiles from now: pull it into L2 ahead of them
-          const void* const* Wt = role == 2 ? desc.Wk : desc.Wv;
-          const size_t wbytes = static_cast<size_t>(g.HG) * m * g.D * 2;
-          const char* wp = static_cast<const char*>(Wt[w.l]) + static_cast<size_t>(w.hg) * wbytes;
-          for (size_t o = static_cast<size_t>(lane) * 128; o < wbytes; o += 32 * 128)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(wp + o));
+        if (sel == 0) src = inplace ? static_cast<const char*>(p.pool_k[w.l]) : static_cast<const char*>(desc.k_src[w.l]);
+        else if (sel == 1) {
+          if (dbl) src = static_cast<const char*>(p.pool_k[w.l]);
+          else if (!inplace && g.nkv == 2) src = static_cast<const char*>(desc.v_src[w.l]);
+        } else if (sel >= 2) {
+          const void* const* tab_l = sel == 2 ? desc.Uk : desc.Uv;
+          if (m && tab_l && !inplace && (sel == 2 || g.nkv == 2)) src = static_cast<const char*>(tab_l[w.l]);
+          if (src) {
+            // the consumers stage this (chunk, layer)'s W a few tiles from now: pull it into L2 ahead of them
+            const void* const* Wt = sel == 2 ? desc.Wk : desc.Wv;
+            const size_t wbytes = static_cast<size_t>(g.HG) * m * g.D * 2;
+            const char* wp = static_cast<const char*>(Wt[w.l]) + static_cast<size_t>(w.hg) * wbytes;
+            for (size_t o = static_cast<size_t>(lane) * 128; o < wbytes; o += 32 * 128)
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(wp + o));
+          }
         }
       }
-      const int tok0 = w.tt * g.TT;
-      const int nvalid = min(g.TT, w.n_tokens - tok0);
       const bool inplace = flags & FLAG_INPLACE;
+      const bool rows_role = role <= 1;
+      const bool second = dbl && role == 1;                      // this warp streams tokens [TT, 2 TT) of the tile
+      const int tok0 = w.tt * w.tile_tok + (second ? g.TT : 0);
+      const int nvalid = max(0, min(g.TT, w.n_tokens - tok0));
       // A1 slot mapping: g = dst_token_start + t -> page = block_table[g / P], slot = page * P + g % P   (TT <= 64: 2 rows per lane)
-      int slot_lo = -1, slot_hi = -1;
-      if (role == 0) {
-        if (lane < nvalid) {
-          const int gt = dst0 + tok0 + lane;
-          const int pg = g.P_shift >= 0 ? (gt >> g.P_shift) : gt / g.P;
-          slot_lo = __ldg(bt + pg) * g.P + (gt - pg * g.P);
-        }
-        if (lane + 32 < nvalid) {
-          const int gt = dst0 + tok0 + lane + 32;
-          const int pg = g.P_shift >= 0 ? (gt >> g.P_shift) : gt / g.P;
-          slot_hi = __ldg(bt + pg) * g.P + (gt - pg * g.P);
+      // A page outside the pool is never written (slot -1) and never read (row 0 stands in); it is counted once per table entry.
+      int slot_lo = -1, slot_hi = -1, rd_lo = 0, rd_hi = 0;
+      if (role == 0 || second) {
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+          const int r = lane + 32 * hf;
+          if (r < nvalid) {
+            const int gt = dst0 + tok0 + r;
+            const int pg = g.P_shift >= 0 ? (gt >> g.P_shift) : gt / g.P;
+            const int in_pg = gt - pg * g.P;
+            const int page = bt[pg];             // generic load: the list may sit in the kernel parameters
+            int slot = -1, rd = 0;
+            if (static_cast<unsigned>(page) < static_cast<unsigned>(p.num_pages)) { slot = page * g.P + in_pg; rd = slot; }
+            else if (p.err && w.l == 0 && w.hg == 0 && w.kv == 0 && (in_pg == 0 || tok0 + r == 0)) atomicAdd(p.err, 1);
+            if (hf) { slot_hi = slot; rd_hi = rd; } else { slot_lo = slot; rd_lo = rd; }
+          }
         }
       }
       mbar_wait(&empty_bar[stage], phase ^ 1);
       uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
       uint64_t* fb = &full_bar[stage];
-      if (role <= 1) {
-        if (role == 0) {
-          int32_t* slots = reinterpret_cast<int32_t*>(st + g.st_slot);
+      if (rows_role) {
+        if (role == 0 || second) {
+          int32_t* slots = reinterpret_cast<int32_t*>(st + g.st_slot) + (second ? g.TT : 0);
           if (lane < g.TT) slots[lane] = slot_lo;
           if (lane + 32 < g.TT) slots[lane + 32] = slot_hi;
           __syncwarp();                              // every lane's slots are written before lane 0 arrives on the barrier
         }
-        if (src == nullptr) {
+        if (src == nullptr || nvalid == 0) {
           if (lane == 0) mbar_arrive(fb);
         } else {
           if (lane == 0) mbar_arrive_expect_tx(fb, static_cast<uint32_t>(nvalid) * g.slice_bytes);
@@ -310,7 +385,7 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {
               const int r = lane + 32 * hf;
-              const int mine = hf ? slot_hi : slot_lo;
+              const int mine = hf ? rd_hi : rd_lo;
               const int prev = __shfl_up_sync(0xffffffffu, mine, 1);
               const bool valid = r < nvalid;
               const bool head = valid && (lane == 0 || mine != prev + 1);          // a run never spans the two halves
@@ -325,32 +400,42 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {
               const int r = lane + 32 * hf;
-              if (r < nvalid) bulk_g2s(dst + r * g.s_row, src + static_cast<size_t>(hf ? slot_hi : slot_lo) * g.row_bytes + off, g.slice_bytes, fb);
+              if (r < nvalid) bulk_g2s(dst + r * g.s_row, src + static_cast<size_t>(hf ? rd_hi : rd_lo) * g.row_bytes + off, g.slice_bytes, fb);
             }
           }
         }
       } else {
-        if (src == nullptr) {
+        if (src == nullptr || nvalid == 0) {
           if (lane == 0) mbar_arrive(fb);
         } else {
-          // U rows of this tile: one run of (heads-in-slice * m) elements per token when the heads are adjacent; the whole
-          // tile in ONE copy when the token runs are adjacent too and fill the shared-memory row exactly
+          // U rows of this tile.  Native form: the tile's rows are one contiguous run of the caller's array ([T][..] with its own
+          // token stride, all heads of the row in this slice) - ONE copy, and the consumers index it with the caller's strides.
+          // Otherwise one run of (heads-in-slice * m) elements per token when the heads are adjacent, else one run per head.
           const int hf_n = (u_head_stride == 0) ? 1 : g.HG;
           const uint32_t u_run = static_cast<uint32_t>(m) * 2u, u_tok_bytes = u_run * hf_n;
-          if (lane == 0) mbar_arrive_expect_tx(fb, static_cast<uint32_t>(nvalid) * u_tok_bytes);
-          __syncwarp();
           const long long h0 = (u_head_stride == 0) ? 0 : static_cast<long long>(w.hg) * g.HG;
           const char* s0 = src + (static_cast<long long>(tok0) * u_tok_stride + h0 * u_head_stride) * 2;
           uint8_t* dst = st + (role == 2 ? g.st_uk : g.st_uv);
           const bool heads_adjacent = hf_n == 1 || u_head_stride == m;
-          if (heads_adjacent && u_tok_stride * 2 == u_tok_bytes && static_cast<int>(u_tok_bytes) == g.su_row) {
-            if (lane == 0) bulk_g2s(dst, s0, static_cast<uint32_t>(nvalid) * u_tok_bytes, fb);
-          } else if (heads_adjacent) {
-            for (int r = lane; r < nvalid; r += 32) bulk_g2s(dst + r * g.su_row, s0 + r * u_tok_stride * 2, u_tok_bytes, fb);
+          if (u_native(g, u_tok_stride, u_head_stride)) {
+            if (lane == 0) {
+              // a ragged rank can leave < 16 bytes at the end of a chunk's last tile: those travel as plain 2-byte accesses
+              const uint32_t total = static_cast<uint32_t>(nvalid) * static_cast<uint32_t>(u_tok_stride) * 2u, bulk = total & ~15u;
+              for (uint32_t o = bulk; o < total; o += 2)
+                *reinterpret_cast<uint16_t*>(dst + o) = __ldg(reinterpret_cast<const uint16_t*>(s0 + o));
+              if (bulk) { mbar_arrive_expect_tx(fb, bulk); bulk_g2s(dst, s0, bulk, fb); }
+              else mbar_arrive(fb);
+            }
           } else {
-            for (int r = lane; r < nvalid; r += 32)
-              for (int h = 0; h < hf_n; ++h)
-                bulk_g2s(dst + r * g.su_row + h * u_run, s0 + (r * u_tok_stride + h * u_head_stride) * 2, u_run, fb);
+            if (lane == 0) mbar_arrive_expect_tx(fb, static_cast<uint32_t>(nvalid) * u_tok_bytes);
+            __syncwarp();
+            if (heads_adjacent) {
+              for (int r = lane; r < nvalid; r += 32) bulk_g2s(dst + r * g.su_row, s0 + r * u_tok_stride * 2, u_tok_bytes, fb);
+            } else {
+              for (int r = lane; r < nvalid; r += 32)
+                for (int h = 0; h < hf_n; ++h)
+                  bulk_g2s(dst + r * g.su_row + h * u_run, s0 + (r * u_tok_stride + h * u_head_stride) * 2, u_run, fb);
+            }
           }
         }
       }
@@ -364,8 +449,8 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   const int gq = lane >> 2, t4 = lane & 3;
   const int ctid = threadIdx.x;                                   // 0 .. 255
   int stage = 0; uint32_t phase = 0;
-  int cur_d = -1, cur_l = -1, cur_hg = -1;
-  int m = 0, flags = 0, KT = 0; bool u_shared = false, has_uk = false, has_uv = false;
+  int cur_d = -1, cur_l = -1, cur_hg = -1, cur_kv = -1;
+  int m = 0, m_pad = 0, flags = 0, KT = 0, su = 0, uhs = 0; bool u_shared = false, has_uk = false, has_uv = false;
   char* pool_k = nullptr; char* pool_v = nullptr;
   const int half = g.d_r >> 1;
   // ldmatrix lane addressing
@@ -373,15 +458,19 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   const int b_k = (lane & 7) + ((lane >> 3) & 1) * 8, b_nt = lane >> 4;         // B: k row of W, n-tile 0/1 of the pair
 
   for (long long tile = t_begin; tile < t_end; ++tile) {
-    if (w.d != cur_d || w.l != cur_l || w.hg != cur_hg) {
-      // ---- new (chunk, layer, head group): rebuild the sin/cos table (new chunk) and stage W
+    if (w.d != cur_d || w.l != cur_l || w.hg != cur_hg || w.kv != cur_kv) {
+      // ---- new (chunk, layer, head group[, kv]): rebuild the sin/cos table (new chunk) and stage W
       const bool new_chunk = (w.d != cur_d);
-      cur_d = w.d; cur_l = w.l; cur_hg = w.hg;
+      cur_d = w.d; cur_l = w.l; cur_hg = w.hg; cur_kv = w.kv;
       const RelocDescDev& desc = descs[w.d];
-      flags = desc.flags; m = desc.rank_l[w.l]; KT = m >> 4;
+      flags = desc.flags; m = desc.rank_l[w.l]; KT = (m + 15) >> 4; m_pad = KT << 4;
       u_shared = desc.u_head_stride == 0;
       const bool inplace = flags & FLAG_INPLACE;
       has_uk = m && desc.Uk && !inplace; has_uv = m && desc.Uv && !inplace && g.nkv == 2;
+      // strides of U in the stage: the caller's own when the tile arrived as one copy (see the producer), else padded rows of
+      // head runs of m elements
+      if (u_native(g, desc.u_token_stride, desc.u_head_stride)) { su = static_cast<int>(desc.u_token_stride) * 2; uhs = static_cast<int>(desc.u_head_stride); }
+      else { su = g.su_row; uhs = m; }
       pool_k = static_cast<char*>(p.pool_k[w.l]) + static_cast<size_t>(w.hg) * g.slice_bytes;
       pool_v = g.nkv == 2 ? static_cast<char*>(p.pool_v[w.l]) + static_cast<size_t>(w.hg) * g.slice_bytes : nullptr;
       named_bar_sync(1, kRelocConsumerWarps * 32);                // everyone is done with the old tables
@@ -394,23 +483,32 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
         tab[half + ctid] = static_cast<float>(sn);
         tab[2 * half + ctid] = -static_cast<float>(sn);
       }
-      if (has_uk) {
+      // which of W_k / W_v go to shared memory now: both (plain geometry) or the one of this tile's kv (kv-split)
+      const int kv_lo = split ? w.kv : 0;
+      const int kv_n = split ? ((w.kv ? has_uv : has_uk) ? 1 : 0) : (has_uk ? (has_uv ? 2 : 1) : 0);
+      if (kv_n) {
         // W[l] is [H][m][D]; copy this head group's rows, 16 bytes (8 columns = 4 pairs) per thread, scattering the pairs
-        // to their MMA-order positions inside the 32-column group.
+        // to their MMA-order positions inside the 32-column group; rows m .. m_pad-1 of every head are written as zeros.
         const int vec_per_row = g.D >> 3;
-        const int per_kv = g.HG * m * vec_per_row;
-        const int n_vec = (has_uv ? 2 : 1) * per_kv;
+        const int per_kv = g.HG * m_pad * vec_per_row;
+        const int n_vec = kv_n * per_kv;
         constexpr int kCT = kRelocConsumerWarps * 32, kBatch = 8;      // 8 independent 16-byte loads in flight per thread
         for (int e0 = ctid; e0 < n_vec; e0 += kCT * kBatch) {
           uint4 x[kBatch];
 #pragma unroll
           for (int u = 0; u < kBatch; ++u) {
             const int e = e0 + u * kCT;
+            x[u] = make_uint4(0u, 0u, 0u, 0u);
             if (e < n_vec) {
               const int kv = e >= per_kv;
-              const int r = e - kv * per_kv;
-              const void* const* Wl = kv ? desc.Wv : desc.Wk;
-              x[u] = __ldg(reinterpret_cast<const uint4*>(static_cast<const char*>(Wl[w.l]) + static_cast<size_t>(w.hg) * g.HG * m * g.D * 2) + r);
+              int r = e - kv * per_kv;
+              const int v = r % vec_per_row; r /= vec_per_row;     // r = head-in-group * m_pad + k
+              const int hd = r / m_pad, k = r - hd * m_pad;
+              if (k < m) {
+                const void* const* Wl = (kv_lo + kv) ? desc.Wv : desc.Wk;
+                x[u] = __ldg(reinterpret_cast<const uint4*>(static_cast<const char*>(Wl[w.l]) +
+                                                            (static_cast<size_t>(w.hg) * g.HG + hd) * m * g.D * 2 + static_cast<size_t>(k) * g.D * 2) + v);
+              }
             }
           }
 #pragma unroll
@@ -419,7 +517,7 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
             if (e < n_vec) {
               const int kv = e >= per_kv;
               int r = e - kv * per_kv;
-              const int v = r % vec_per_row; r /= vec_per_row;     // r = head-in-group * m + k
+              const int v = r % vec_per_row; r /= vec_per_row;     // r = head-in-group * m_pad + k
               const int q = v >> 2, i = v & 3;                       // columns 32q + 8i .. +7 = pairs j = 0..3
               uint32_t* dst = reinterpret_cast<uint32_t*>(wsm + static_cast<size_t>(kv) * g.w_kv_stride + static_cast<size_t>(r) * g.w_row) + q * 16 + i;
               dst[0] = x[u].x; dst[4] = x[u].y; dst[8] = x[u].z; dst[12] = x[u].w;   // pair j lands at 32-bit position 4j + i
@@ -435,26 +533,34 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
     const uint8_t* st = smem + g.off_stage0 + static_cast<size_t>(stage) * g.stage_bytes;
     const int32_t* slots = reinterpret_cast<const int32_t*>(st + g.st_slot);
     const bool inplace = flags & FLAG_INPLACE;
-    const int n_slabs = ((g.nkv == 2 && !inplace) ? 2 : 1) * g.RB * g.n_blocks;
+    const bool dbl = inplace && g.nkv == 2 && !split;
+    const int n_slabs = ((g.nkv == 2 && !split && (!inplace || dbl)) ? 2 : 1) * g.RB * g.n_blocks;
 
     for (int s = warp; s < n_slabs; s += kRelocConsumerWarps) {
       const int4 e = slab_tab[s];
-      const int kv = e.x & 0xf, rb = (e.x >> 4) & 0xf, fhead = (e.x >> 8) & 0xff, rope = (e.x >> 16) & 0xf;
+      const int hf = e.x & 0xf, rb = (e.x >> 4) & 0xf, fhead = (e.x >> 8) & 0xff;
+      const int kv = split ? w.kv : (dbl ? 0 : hf);                // what the rows are: 0 = keys, 1 = values
+      const int rope = kv ? ROPE_NONE : (e.x >> 16) & 0xf;
       const int row0 = rb * 16 + gq;
-      const int slot0 = slots[row0], slot1 = slots[row0 + 8];
+      const int srow = row0 + (dbl && hf ? g.TT : 0);
+      const int slot0 = slots[srow], slot1 = slots[srow + 8];
       char* pool = (kv ? pool_v : pool_k) + e.y + t4 * 16;
       SlabArgs a;
-      a.rows = st + (kv ? g.st_v : g.st_k) + row0 * g.s_row + e.y + t4 * 16;
+      a.rows = st + (hf ? g.st_v : g.st_k) + row0 * g.s_row + e.y + t4 * 16;
       a.dst0 = pool + static_cast<size_t>(slot0 < 0 ? 0 : slot0) * g.row_bytes;
       a.dst1 = pool + static_cast<size_t>(slot1 < 0 ? 0 : slot1) * g.row_bytes;
       a.tab = tab + e.w + (rope == ROPE_HALF ? 8 * t4 : 4 * t4);
       a.s_row = g.s_row; a.w_row16 = 16 * g.w_row; a.half = half;
       a.steps = e.x >> 20;
       a.ok0 = slot0 >= 0; a.ok1 = slot1 >= 0; a.canonical = flags & FLAG_CANONICAL_FRAME;
-      a.wb = smem_u32(wsm + static_cast<size_t>(kv) * g.w_kv_stride + static_cast<size_t>(fhead * m + b_k) * g.w_row + e.z + b_nt * 16);
+      const int wkv = split ? 0 : kv;                               // which resident W table
+      a.wb = smem_u32(wsm + static_cast<size_t>(wkv) * g.w_kv_stride + static_cast<size_t>(fhead * m_pad + b_k) * g.w_row + e.z + b_nt * 16);
       const int kt = (kv ? has_uv : has_uk) ? KT : 0;
       // A fragments of U for this slab's 16 tokens and head: one ldmatrix.x4 per 16 ranks
-      const uint32_t ua = smem_u32(st + (kv ? g.st_uv : g.st_uk) + (rb * 16 + a_row) * g.su_row + ((u_shared ? 0 : fhead) * m + a_koff) * 2);
+      const uint8_t* ubase = st + ((kv && !split) ? g.st_uv : g.st_uk) + ((u_shared ? 0 : fhead) * uhs) * 2;
+      const uint32_t ua = smem_u32(ubase + (rb * 16 + a_row) * su + a_koff * 2);
+      // ldmatrix needs 16-byte aligned rows of 16 k-values; anything else is gathered element by element
+      a.ug = ubase + row0 * su; a.su = su; a.m_rag = ((m | (su >> 1) | uhs) & 7 || (m & 15)) ? m : 0;
       switch (kt) {
         case 0: slab_run<0>(a, rope, ua); break;
         case 1: slab_run<1>(a, rope, ua); break;
@@ -470,19 +576,20 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   }
 }
 
-void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, int grid, cudaStream_t st) {
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages& pages, int grid, cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(kam_relocate_patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_set = true;
   }
-  kam_relocate_patch_kernel<<<grid, kRelocThreads, g.smem_bytes, st>>>(g, p, inl);
+  kam_relocate_patch_kernel<<<grid, kRelocThreads, g.smem_bytes, st>>>(g, p, inl, pages);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // Generic element-wise path: any element / factor dtype, any rank <= KAM_MAX_RANK, any even rope band.  One thread
-// owns a non-rotated column or BOTH columns of a rope pair (in-place safe).  Correctness path for small or odd
-// shapes (config 1's fp32 tensors and rank 4); the tiled kernel above is the one the roofline is quoted on.
+// owns a non-rotated column or BOTH columns of a rope pair (in-place safe).  Correctness path for fp32 tensors (config 1
+// as written), row regions that are not multiples of 64 columns and U layouts bulk copies cannot address; every bf16
+// rank <= KAM_MAX_RANK runs on the tiled kernel above, which is the one the roofline is quoted on.
 template <typename T> __device__ __forceinline__ float ld_as_float(const void* p, size_t i);
 template <> __device__ __forceinline__ float ld_as_float<float>(const void* p, size_t i) { return static_cast<const float*>(p)[i]; }
 template <> __device__ __forceinline__ float ld_as_float<__nv_bfloat16>(const void* p, size_t i) {
@@ -522,7 +629,12 @@ __global__ void __launch_bounds__(256) kam_relocate_patch_generic_kernel(const _
     if (t >= desc.n_tokens) continue;
     const long long gt = desc.dst_token_start + t;
     const long long pg = gt / p.P;
-    const size_t slot = static_cast<size_t>(desc.block_table[pg]) * p.P + static_cast<size_t>(gt - pg * p.P);
+    const int page = desc.block_table[pg];
+    if (static_cast<unsigned>(page) >= static_cast<unsigned>(p.num_pages)) {      // a page outside the pool: skipped, counted once
+      if (p.err && l == 0 && h == 0 && wc == 0 && (gt == pg * p.P || t == 0)) atomicAdd(p.err, 1);
+      continue;
+    }
+    const size_t slot = static_cast<size_t>(page) * p.P + static_cast<size_t>(gt - pg * p.P);
     const size_t dst_row = (slot * p.H + h) * p.D;
     const size_t src_row = inplace ? dst_row : (static_cast<size_t>(t) * p.H + h) * p.D;
     const void* ksrc = inplace ? static_cast<const void*>(pk) : desc.k_src[l];

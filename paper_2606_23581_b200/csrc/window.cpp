@@ -62,6 +62,25 @@ void WindowStore::settle(Request& r, bool materialize, std::vector<Rotation>* ro
   }
 }
 
+WindowStore::Result WindowStore::can_admit(int32_t req, int evict_end, int admit_end, int32_t n_tokens) const {
+  if (!is_open(req)) return BAD_STATE;
+  if ((admit_end != 0 && admit_end != 1) || evict_end > 1) return BAD_ARG;
+  if (n_tokens <= 0 || n_tokens % P_ != 0) return BAD_ARG;
+  const int32_t need = n_tokens / P_;
+  if (need > max_ppc_) return BAD_ARG;
+  const Request& r = reqs_[req];
+  int32_t n_chunks = (int32_t)r.chunks.size(), freed = 0;
+  if (evict_end >= 0) {
+    if (n_chunks <= r.pinned) return BAD_STATE;
+    const ChunkRec& c = (evict_end == 0) ? r.chunks[r.pinned] : r.chunks.back();
+    freed = c.n_tokens / P_;
+    --n_chunks;
+  }
+  if (n_chunks >= max_chunks_ || (free_slots_.empty() && evict_end < 0)) return BAD_STATE;
+  if (need > (int32_t)free_.size() + freed) return NO_PAGES;
+  return OK;
+}
+
 WindowStore::Result WindowStore::admit(int32_t req, int end, int32_t n_tokens, bool materialize, ChunkRec* rec,
                                        int64_t* p_target, std::vector<Rotation>* rotations) {
   if (!is_open(req)) return BAD_STATE;

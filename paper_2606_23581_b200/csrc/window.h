@@ -33,6 +33,8 @@ class WindowStore {
   Result admit(int32_t req, int end, int32_t n_tokens, bool materialize, ChunkRec* rec, int64_t* p_target,
                std::vector<Rotation>* rotations);
   Result evict(int32_t req, int end, bool materialize, ChunkRec* rec, std::vector<Rotation>* rotations);
+  // Would evict(req, evict_end) [skipped when evict_end < 0] followed by admit(req, admit_end, n_tokens) succeed?  Changes nothing.
+  Result can_admit(int32_t req, int evict_end, int admit_end, int32_t n_tokens) const;
 
   bool is_open(int32_t req) const { return req >= 0 && req < (int32_t)reqs_.size() && reqs_[req].open; }
   const std::deque<ChunkRec>& chunks(int32_t req) const { return reqs_[req].chunks; }

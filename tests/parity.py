@@ -98,8 +98,9 @@ def compare_f32(g, o, S, m, what=""):
     return {"n": int(ok.size), "fail": 0}
 
 
-def upload_chunk(ch, device="cuda", shared_u=False):
-    """synth.make_chunk output -> kam.Chunk / kam.Patch over per-layer device tensors."""
+def upload_chunk(ch, device="cuda", shared_u=False, rank_per_layer=None):
+    """synth.make_chunk output -> kam.Chunk / kam.Patch over per-layer device tensors.  rank_per_layer: layer l uses the first
+    r_l columns of its stored U (strides unchanged) and a contiguous W[l] of r_l rows (kamera.h: W[l] is [H][rank_l][D])."""
     L = ch["K"].shape[0]
     K = [ch["K"][l].to(device).contiguous() for l in range(L)]
     V = [ch["V"][l].to(device).contiguous() for l in range(L)] if ch["V"] is not None else None
@@ -112,7 +113,10 @@ def upload_chunk(ch, device="cuda", shared_u=False):
             return [(x[l][:, 0, :] if shared_u else x[l]).to(device).contiguous() for l in range(L)]
 
         def W(x):
-            return [x[l].to(device).contiguous() for l in range(L)] if x is not None else None
+            if x is None:
+                return None
+            r = rank_per_layer if rank_per_layer is not None else [x.shape[2]] * L
+            return [x[l][:, :max(1, r[l])].to(device).contiguous() for l in range(L)]
         patch = kam.Patch(U(ch["Uk"]), W(ch["Wk"]), U(ch["Uv"]), W(ch["Wv"]))
     return chunk, patch
 
@@ -123,6 +127,10 @@ def oracle_layer(cfg, ch, l, delta, style=reuse.HALF, frame=reuse.TARGET_FRAME, 
     use = ch["Uk"] is not None and ch["Uk"].shape[-1] > 0 and (rank is None or rank > 0)
     Uk = to_f64(ch["Uk"][l]) if use else None; Wk = to_f64(ch["Wk"][l]) if use else None
     Uv = to_f64(ch["Uv"][l]) if use and v is not None else None; Wv = to_f64(ch["Wv"][l]) if use and v is not None else None
+    if use and rank is not None:                     # a layer whose rank is below the stored one: leading columns / rows
+        Uk, Wk = Uk[..., :rank], Wk[:, :rank]
+        if Uv is not None:
+            Uv, Wv = Uv[..., :rank], Wv[:, :rank]
     if use and shared_u:
         Uk = np.repeat(Uk[:, :1, :], Uk.shape[1], axis=1)
         if Uv is not None:

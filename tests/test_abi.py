@@ -5,6 +5,7 @@ import ctypes as C
 import os
 import random
 import re
+import subprocess
 
 import pytest
 
@@ -33,10 +34,37 @@ def test_every_declared_symbol_is_exported_and_bound():
     assert b"sm_100a" in lib.kam_version()
 
 
-def test_struct_sizes_match_the_header_layout():
-    assert C.sizeof(B.kam_layout) == 13 * 4 + 4 + 8          # 13 int32, padding, double
-    assert C.sizeof(B.kam_pool) == 24 and C.sizeof(B.kam_chunk) == 32
-    assert C.sizeof(B.kam_patch) == 64 and C.sizeof(B.kam_reloc_desc) == 48 and C.sizeof(B.kam_patch_ref) == 56
+def test_c_program_against_the_header_agrees_with_the_ctypes_mirror(tmp_path):
+    """tests/abi_check.c is compiled with `cc -I include` and linked against libkamera.so: every struct size and field offset
+    the C compiler derives from include/kamera.h must equal binding.py's ctypes mirror, the constants must agree, and the
+    bookkeeping-only entries (create / set_option / window open / admit / export / slide / stats / destroy) work through the
+    header's own prototypes."""
+    lib_path = kam.build.build()
+    exe = str(tmp_path / "abi_check")
+    cc = subprocess.run(["cc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), os.path.join(ROOT, "tests", "abi_check.c"),
+                         "-o", exe, lib_path, "-Wl,-rpath," + os.path.dirname(lib_path)], capture_output=True, text=True)
+    assert cc.returncode == 0, cc.stdout + cc.stderr
+    run = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert run.returncode == 0 and run.stdout.strip().endswith("OK"), run.stdout + run.stderr
+    lines = [l.split() for l in run.stdout.splitlines()]
+    structs = {n: getattr(B, n) for n in ("kam_layout", "kam_pool", "kam_chunk", "kam_patch", "kam_reloc_desc", "kam_patch_ref", "kam_stats")}
+    seen = {n: set() for n in structs}
+    for l in lines:
+        if l[0] == "sizeof":
+            assert C.sizeof(structs[l[1]]) == int(l[2]), l
+        elif l[0] == "offsetof":
+            assert getattr(structs[l[1]], l[2]).offset == int(l[3]), l
+            seen[l[1]].add(l[2])
+        elif l[0] in ("const", "enum"):
+            assert getattr(B, l[1]) == int(l[2]), l
+    for n, st in structs.items():                                   # the C program lists every field the mirror has
+        assert seen[n] == {f[0] for f in st._fields_}, n
+    exp = [l for l in lines if l[0] == "export"][0]
+    # front-admitted 48-token chunk (pages 2,3,4) precedes the 32-token one (pages 0,1); lazily admitted, so the older chunk
+    # carries a pending offset of +48
+    assert exp[1:] == "n_pages 5 n_chunks 2 bt 2 3 4 0 1 starts 0 48 80 offs 0 48 handles 1 0".split()
+    st = [l for l in lines if l[0] == "stats"][0]
+    assert st[1:] == "free 61 total 64 written 6 live 2 launched 0".split()
 
 
 def test_create_rejects_bad_layouts():
@@ -51,7 +79,7 @@ def test_compute_entries_fail_loudly_without_cuda():
     ctx = kam.Context(_layout(), None, 2, 4, 8)
     # no pool, no device: the stateless operator must refuse, not fall back
     ch = B.kam_chunk(None, None, 16, 0)
-    st = kam.lib().kam_relocate_patch(ctx.h, None, None, 0, C.byref(ch), 0, None, 0, None)
+    st = kam.lib().kam_relocate_patch(ctx.h, None, None, 0, C.byref(ch), 0, None, 0, None, None)
     assert st == B.KAM_ERR_INVALID_ARG
     st = kam.lib().kam_rotate_inplace(ctx.h, None, None, 0, 16, 5, None)
     assert st == B.KAM_ERR_INVALID_ARG and b"pool" in kam.lib().kam_last_error(ctx.h)
@@ -64,6 +92,18 @@ def test_compute_entries_fail_loudly_without_cuda():
     assert kam.lib().kam_lse_merge_states(ctx.h, 17, fake, fake, 2, B.vp(0x1000), B.vp(0x1000), None) == B.KAM_ERR_INVALID_ARG
     assert kam.lib().kam_decode_set_max_patch_rank(ctx.h, 48) == B.KAM_ERR_INVALID_ARG
     assert kam.lib().kam_decode_set_max_patch_rank(ctx.h, 32) == B.KAM_OK
+    # a layout argument that differs from the context's is refused (north_star's `layout` is a check, not a dispatch)
+    other = _layout(row_dim=64, rope_dim=64)
+    st = kam.lib().kam_relocate_patch(ctx.h, None, None, 0, C.byref(ch), 0, None, 0, C.byref(other), None)
+    assert st == B.KAM_ERR_INVALID_ARG and b"layout" in kam.lib().kam_last_error(ctx.h)
+    # options: known keys in range only; the library reads no environment variable
+    ctx.kam_set_option("reloc_kv_split", 2)
+    for key, val in (("reloc_kv_split", 3), ("nonsense", 1)):
+        with pytest.raises(kam.KameraError) as e:
+            ctx.kam_set_option(key, val)
+        assert e.value.status == B.KAM_ERR_INVALID_ARG
+    srcs = "".join(open(os.path.join(ROOT, "paper_2606_23581_b200", "csrc", f)).read() for f in os.listdir(os.path.join(ROOT, "paper_2606_23581_b200", "csrc")))
+    assert "getenv" not in srcs
 
 
 def _chunk(n):
@@ -129,7 +169,21 @@ def test_window_matches_oracle_model_bit_for_bit_and_is_O1():
     for step in range(1500):
         r, end, mat = rnd.randrange(R), rnd.choice((FRONT, BACK)), rnd.randrange(2)
         before = ctx.kam_get_stats()["table_entries_written"]
-        if live[r] > ws.req[r]["pinned"] and (rnd.random() < 0.45 or live[r] == CH):
+        if live[r] > ws.req[r]["pinned"] and rnd.random() < 0.25:
+            # kam_slide = evict (lazy) + admit (materialize) as one call; fails as a whole, before evicting, when it cannot admit
+            end2, n = rnd.choice((FRONT, BACK)), P * rnd.randrange(1, PPC + 2)
+            if n > P * PPC:
+                with pytest.raises(kam.KameraError) as e:
+                    ctx.kam_slide(r, end, end2, _chunk(n), materialize=mat)
+                assert e.value.status == B.KAM_ERR_INVALID_ARG
+                assert ctx.kam_get_stats()["table_entries_written"] == before
+            else:
+                h = ctx.kam_slide(r, end, end2, _chunk(n), materialize=mat)
+                ws.evict(r, end, 0)
+                h2, _, _, _ = ws.admit(r, end2, n, mat)
+                assert h == h2
+                assert ctx.kam_get_stats()["table_entries_written"] - before == n // P
+        elif live[r] > ws.req[r]["pinned"] and (rnd.random() < 0.45 or live[r] == CH):
             ctx.kam_evict(r, end, mat); ws.evict(r, end, mat)
             live[r] -= 1
             assert ctx.kam_get_stats()["table_entries_written"] == before

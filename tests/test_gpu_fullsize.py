@@ -207,9 +207,12 @@ def test_config4_full_size_sliding_window_sampled():
                 w = ws.export(r)
                 before = {l: par.pool_rows(pool.k_layers[l], w["block_table"], w["chunk_starts"][2], 2 * T) for l in sample_layers}
                 v_before = par.pool_rows(pool.v_layers[0], w["block_table"], w["chunk_starts"][2], 2 * T)
-            ctx.kam_evict(r, FRONT, 1); ws.evict(r, FRONT, 1)
             ci = (r + 3 + s) % NCAN
-            ctx.kam_admit(r, BACK, canon[ci][0], canon[ci][1], m, 1); ws.admit(r, BACK, T, 1)
+            if s % 2:                                            # the two-call form ...
+                ctx.kam_evict(r, FRONT, 1); ws.evict(r, FRONT, 1)
+                ctx.kam_admit(r, BACK, canon[ci][0], canon[ci][1], m, 1); ws.admit(r, BACK, T, 1)
+            else:                                                # ... and the slide as ONE call and ONE launch
+                ctx.kam_slide(r, FRONT, BACK, canon[ci][0], canon[ci][1], m, 1); ws.evict(r, FRONT, 0); ws.admit(r, BACK, T, 1)
             if probe:
                 torch.cuda.synchronize()
                 w = ws.export(r)

@@ -30,8 +30,9 @@ def _bt(rng, n_pages, num_pages):
 
 
 def _run_single(cfg, L, T, m, dst0=0, style=B.KAM_ROPE_HALF, frame=B.KAM_PATCH_TARGET_FRAME, delta=None, salt=0,
-                shared_u=False, rank_per_layer=None, elem=None, factor=None):
-    """One stateless kam_relocate_patch call, everything verified.  Returns the comparison stats."""
+                shared_u=False, rank_per_layer=None, elem=None, factor=None, options=None):
+    """One stateless kam_relocate_patch call, everything verified.  Returns the comparison stats (+ the context's launch
+    counters: "generic_launches" says whether the element-wise fallback kernel ran)."""
     rng = _rng(cfg, salt)
     c = cfg.scaled(elem_dtype=elem or cfg.elem_dtype, factor_dtype=factor or cfg.factor_dtype)
     ch = make_chunk(c, rng, n_tokens=T, n_layers=L, rank=m)
@@ -42,16 +43,21 @@ def _run_single(cfg, L, T, m, dst0=0, style=B.KAM_ROPE_HALF, frame=B.KAM_PATCH_T
     dt = torch.bfloat16 if c.elem_dtype == "bf16" else torch.float32
     pool = par.make_pool(c, L, num_pages, dt)
     ctx = kam.Context(par.layout_of(c, L, style), pool)
-    chunk, patch = par.upload_chunk(ch, shared_u=shared_u)
+    for key, val in (options or {}).items():
+        ctx.kam_set_option(key, val)
+    chunk, patch = par.upload_chunk(ch, shared_u=shared_u, rank_per_layer=rank_per_layer)
     if patch is not None:
         patch.c.frame = frame
         if rank_per_layer is not None:
             patch._rpl = (B.i32 * L)(*rank_per_layer)
             patch.c.rank_per_layer = patch._rpl
-    ctx.kam_relocate_patch(bt_d, dst0, chunk, p_target, patch, m)
+    ctx.kam_relocate_patch(bt_d, dst0, chunk, p_target, patch, m, layout=ctx.layout)
     torch.cuda.synchronize()
     st = par.check_relocated(c, pool, ch, bt_h, dst0, p_target, m, style=style, frame=frame,
                              rank_per_layer=rank_per_layer, shared_u=shared_u, elem=c.elem_dtype)
+    stats = ctx.kam_get_stats()
+    st["generic_launches"], st["device_errors"] = stats["generic_launches"], stats["device_errors"]
+    assert stats["kernels_launched"] == 1 and stats["device_errors"] == 0
     assert par.untouched_pages_intact(pool, bt_h, L)
     # rows of the first/last page outside [dst0, dst0+T) must still hold the sentinel (slot mapping is exact)
     P = c.page_size
@@ -68,9 +74,10 @@ def _run_single(cfg, L, T, m, dst0=0, style=B.KAM_ROPE_HALF, frame=B.KAM_PATCH_T
 
 # ---------------------------------------------------------------------------------------------- config 1 (tiny MHA)
 def test_config1_fp32_as_written():
-    """BASELINE.json configs[0]: fp32 K/V/U/W, rank 4, one chunk of 256 tokens, p uniform in [0, 4096)."""
+    """BASELINE.json configs[0]: fp32 K/V/U/W, rank 4, one chunk of 256 tokens, p uniform in [0, 4096).  fp32 tensors are the
+    element-wise kernel's job (the tiled kernel moves bf16)."""
     st = _run_single(CONFIGS[1], 1, 256, 4)
-    assert st["fail"] == 0
+    assert st["fail"] == 0 and st["generic_launches"] == 1
 
 
 def test_config1_bf16_elements():
@@ -78,9 +85,10 @@ def test_config1_bf16_elements():
     assert st["fail"] == 0 and st["within_1ulp"] >= 0.999 * st["n"]
 
 
-def test_config1_all_bf16_rank4_uses_generic_kernel():
+def test_config1_all_bf16_rank4_runs_on_the_tiled_kernel():
+    """Rank 4 is padded to one 16-wide rank tile in shared memory (zero U columns, zero W rows): no fallback kernel."""
     st = _run_single(CONFIGS[1], 1, 256, 4, elem="bf16", factor="bf16")
-    assert st["fail"] == 0
+    assert st["fail"] == 0 and st["generic_launches"] == 0
 
 
 # ---------------------------------------------------------------------------------------------- config 2 (GQA)
@@ -128,11 +136,73 @@ def test_zero_tokens_is_a_noop():
     ctx.close()
 
 
-@pytest.mark.parametrize("m", [0, 16, 32, 48, 64, 8, 24])
+@pytest.mark.parametrize("m", [0, 16, 32, 48, 64, 4, 8, 24, 40, 5, 63, 1])
 def test_rank_sweep(m):
-    """m in {0,16,..,64}: tensor-core tiled kernel; 8 and 24: generic kernel (rank not a multiple of 16)."""
-    st = _run_single(CONFIGS[2], 2, 320, m, salt=m)
-    assert st["fail"] == 0
+    """Every rank in [0, 64] runs on the tensor-core tiled kernel ("rank-invariant in latency"; P:216 / P:297 free-form
+    ranks per layer): multiples of 16 directly, anything else padded to the next multiple in shared memory.  323 tokens: a
+    ragged last tile, whose U rows of an odd rank end off a 16-byte boundary."""
+    st = _run_single(CONFIGS[2], 2, 323, m, salt=m)
+    assert st["fail"] == 0 and st["generic_launches"] == 0
+
+
+@pytest.mark.parametrize("m,kw", [(16, {}), (32, dict(style=B.KAM_ROPE_INTERLEAVED)), (40, dict(frame=B.KAM_PATCH_CANONICAL_FRAME)),
+                                  (64, dict(shared_u=True)), (64, dict(rank_per_layer=[64, 0, 24])), (0, {})])
+def test_kv_split_geometry(m, kw):
+    """The tile form ranks 48 / 64 select on their own (a tile carries K rows OR V rows, so only one of W_k / W_v is resident),
+    forced here for every rank, both pair styles, both frames, shared U and mixed per-layer ranks; ragged tail, unaligned start."""
+    L = 3 if "rank_per_layer" in kw else 2
+    st = _run_single(CONFIGS[2], L, 1000, m, dst0=7, salt=100 + m, options={"reloc_kv_split": 2}, **kw)
+    assert st["fail"] == 0 and st["generic_launches"] == 0
+    if m >= 48:                                                  # and with the head group forced down: slices of one head
+        st = _run_single(CONFIGS[2], L, 200, m, salt=300 + m, options={"reloc_kv_split": 2, "reloc_head_group": 1}, **kw)
+        assert st["fail"] == 0
+
+
+def test_free_form_ranks_shared_u_and_mha():
+    cfg = CONFIGS[2]
+    assert _run_single(cfg, 2, 200, 4, shared_u=True, salt=41)["generic_launches"] == 0       # [T][4] bf16: 8 bytes per token
+    assert _run_single(cfg, 4, 200, 24, rank_per_layer=[4, 8, 24, 0], salt=42)["generic_launches"] == 0
+    assert _run_single(CONFIGS[4], 1, 100, 4, salt=43)["generic_launches"] == 0              # MHA 32 heads: 4-head slices of U
+    assert _run_single(CONFIGS[3], 2, 300, 12, salt=44)["generic_launches"] == 0             # MLA, one latent head
+
+
+def test_block_table_entry_outside_the_pool_is_skipped_and_counted():
+    """A block-table entry >= num_pages (or negative) is never dereferenced: its 16 tokens are skipped in every layer, the
+    other pages are written as usual, no page outside the table is touched, and kam_stats.device_errors counts the entry once.
+    Tiled kernel (stateless and in place) and the element-wise kernel (fp32 layout)."""
+    for elem, factor in (("bf16", "bf16"), ("f32", "f32")):
+        cfg = CONFIGS[2].scaled(elem_dtype=elem, factor_dtype=factor)
+        L, T, m = 2, 96, 16
+        rng = _rng(cfg, 77)
+        ch = make_chunk(cfg, rng, n_tokens=T, n_layers=L, rank=m)
+        n_pages = T // cfg.page_size
+        bt_h, _ = _bt(rng, n_pages, 16)
+        bad = bt_h.copy()
+        bad[2] = 16 if elem == "bf16" else -3                       # one entry outside [0, 16)
+        pool = par.make_pool(cfg, L, 16, torch.bfloat16 if elem == "bf16" else torch.float32)
+        ctx = kam.Context(par.layout_of(cfg, L), pool)
+        chunk, patch = par.upload_chunk(ch)
+        ctx.kam_relocate_patch(torch.from_numpy(bad).cuda(), 0, chunk, 999, patch, m)
+        torch.cuda.synchronize()
+        st = ctx.kam_get_stats()
+        assert st["device_errors"] == 1 and st["generic_launches"] == (0 if elem == "bf16" else 1)
+        good_pages = [int(p) for i, p in enumerate(bt_h) if i != 2]
+        assert par.untouched_pages_intact(pool, good_pages, L)      # incl. the page the valid table would have named
+        for l in range(L):                                          # the five good pages hold Eq. 1
+            ko, vo, Sk, Sv = par.oracle_layer(cfg, ch, l, 999)
+            rows = np.r_[0:32, 48:96]
+            got = np.concatenate([par.pool_rows(pool.k_layers[l], bt_h, 0, 32), par.pool_rows(pool.k_layers[l], bt_h, 48, 48)])
+            cmp = par.compare_bf16 if elem == "bf16" else par.compare_f32
+            assert cmp(got, ko[rows], Sk[rows], m, "K")["fail"] == 0
+        if elem == "bf16":                                          # in place over the same table: the bad page is skipped again
+            before = par.pool_rows(pool.k_layers[0], bt_h, 0, 32)
+            ctx.kam_rotate_inplace(torch.from_numpy(bad).cuda(), 0, T, -7)
+            torch.cuda.synchronize()
+            assert ctx.kam_get_stats()["device_errors"] == 2
+            want = reuse.relocate(before, -7, **par.rope_kw(cfg))
+            assert par.compare_bf16(par.pool_rows(pool.k_layers[0], bt_h, 0, 32), want, par.abs_sum_k(before, -7, None, None, cfg), 0, "in place")["fail"] == 0
+            assert par.untouched_pages_intact(pool, good_pages, L)
+        ctx.close()
 
 
 @pytest.mark.parametrize("delta", [0, 1, -1280, 131071, -131071, 32767])
@@ -283,6 +353,12 @@ def test_invalid_arguments_are_rejected_before_any_launch():
         ctx.kam_relocate_patch(None, 0, chunk, 0, patch, 16)
     with pytest.raises(kam.KameraError):
         ctx.kam_relocate_patch(bt, -1, chunk, 0, patch, 16)
+    with pytest.raises(kam.KameraError) as e:                     # token range beyond int32
+        ctx.kam_relocate_patch(bt, 2 ** 31 - 8, chunk, 0, patch, 16)
+    assert e.value.status == B.KAM_ERR_INVALID_ARG
+    with pytest.raises(kam.KameraError) as e:                     # a layout that is not the context's
+        ctx.kam_relocate_patch(bt, 0, chunk, 0, patch, 16, layout=par.layout_of(CONFIGS[5], 1))
+    assert e.value.status == B.KAM_ERR_INVALID_ARG
     assert ctx.kam_get_stats()["kernels_launched"] == 0
     assert par.untouched_pages_intact(pool, [], 1)
     ctx.close()
