@@ -124,8 +124,7 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
     t.contig = (HG == g.H) && c->opt.reloc_contig;
     // padded rows (== 64 mod 128) make the 128-bit row loads conflict-free; unpadded rows allow one copy per tile
     t.s_row = t.contig ? t.slice_bytes : t.slice_bytes + ((64 - t.slice_bytes % 128) + 128) % 128;
-    // U rows: unpadded when a tile arrives as one copy (the one ldmatrix per slab tolerates the bank conflicts)
-    t.su_row = g.KT_max ? align_up(HG * max_rank * 2, 16) + (t.contig ? 0 : 16) : 0;
+    t.su_row = g.KT_max ? align_up(HG * max_rank * 2, 32) + 16 : 0;          // (su_row / 16) odd: conflict-free ldmatrix over 8 token rows
     t.RB = std::min(4, std::max(1, (kRelocConsumerWarps + nkv_tile * NB - 1) / (nkv_tile * NB)));
     if (c->opt.reloc_rb > 0) t.RB = std::min(4, c->opt.reloc_rb);
     t.TT = 16 * t.RB;
@@ -179,17 +178,6 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
   if (have) { *out = best; return true; }
   *why = "no shared-memory configuration fits";
   return false;
-}
-
-// Can the tiled kernel stream this U layout?  Its producer moves U with bulk copies: 16-byte aligned sources and sizes, unless
-// the whole tile is one contiguous run of the caller's array (then a ragged tail of < 16 bytes is handled separately).
-bool u_layout_fast(const RelocGeom& g, int r, long long uts, long long uhs) {
-  if (uts * 2 <= g.su_row && (uhs == 0 || g.n_hg == 1)) return true;        // native form: one copy per tile (u_native in the kernel)
-  const int hf_n = uhs == 0 ? 1 : g.HG;
-  const bool heads_adjacent = hf_n == 1 || uhs == r;
-  const long long tok_bytes = (long long)hf_n * r * 2;
-  if ((uts * 2) % 16 || ((long long)g.HG * uhs * 2) % 16) return false;
-  return heads_adjacent ? tok_bytes % 16 == 0 : (r * 2) % 16 == 0 && (uhs * 2) % 16 == 0;
 }
 
 }  // namespace
@@ -294,12 +282,12 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
   RelocGeom g{};
   if (fast) { std::string why; if (!build_reloc_geom(c, max_rank, inplace_only, &g, &why)) fast = false; }
   // any rank <= KAM_MAX_RANK runs on the tiled kernel (padded to a multiple of 16 in shared memory); what can still send a
-  // call to the element-wise kernel is a U layout the bulk copies cannot address (see u_layout_fast)
+  // call to the element-wise kernel is a U layout the bulk copies cannot address (u_form in internal.h)
   for (int i = 0; i < n && fast; ++i) {
     const kam_patch* p = (hs[i].patch && hs[i].rank > 0) ? hs[i].patch : nullptr;
     for (int l = 0; l < L.n_layers && p && fast; ++l) {
       const int r = p->rank_per_layer ? p->rank_per_layer[l] : hs[i].rank;
-      if (r > 0 && !u_layout_fast(g, r, p->u_token_stride, p->u_head_stride)) fast = false;
+      if (r > 0 && u_form(g.su_row, g.HG, g.n_hg, r, p->u_token_stride, p->u_head_stride) == U_NONE) fast = false;
     }
   }
 

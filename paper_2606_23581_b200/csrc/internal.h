@@ -72,6 +72,26 @@ struct RelocGeom {
   ColBlock blk[kMaxColBlocks];
 };
 
+// How the U rows of a (chunk, layer) of rank m travel to shared memory (producer and consumers of the kernel and the host's
+// eligibility check all ask this one function).  NATIVE: the tile's rows are one contiguous run of the caller's array - one
+// copy, the caller's strides kept in shared memory (ldmatrix then sees rows at a power-of-two stride: 8-way bank conflicts,
+// tolerable for the ONE ldmatrix per slab of rank <= 16, and the only form that can carry ranks whose runs are not multiples
+// of 16 bytes).  ROWS: one copy per token (heads adjacent) or per (token, head) into rows padded to an odd multiple of 16
+// bytes - conflict-free, what ranks > 16 use when their runs are 16-byte multiples.  NONE: the element-wise kernel.
+#ifndef KAM_U_NATIVE_BELOW
+#define KAM_U_NATIVE_BELOW 17
+#endif
+enum : int { U_NONE = 0, U_NATIVE = 1, U_ROWS = 2 };
+__host__ __device__ inline int u_form(int su_row, int HG, int n_hg, int m, long long uts, long long uhs) {
+  const bool native_ok = uts * 2 <= su_row - 16 && (uhs == 0 || n_hg == 1);
+  const int hf_n = uhs == 0 ? 1 : HG;
+  const bool heads_adjacent = hf_n == 1 || uhs == m;
+  const bool rows_ok = (uts * 2) % 16 == 0 && ((long long)HG * uhs * 2) % 16 == 0 &&
+                       (heads_adjacent ? ((long long)hf_n * m * 2) % 16 == 0 : (m * 2) % 16 == 0 && (uhs * 2) % 16 == 0);
+  if (native_ok && (m < KAM_U_NATIVE_BELOW || !rows_ok)) return U_NATIVE;
+  return rows_ok ? U_ROWS : U_NONE;
+}
+
 constexpr int kRelocInlineDescs = 8;   // batches up to this size travel in the kernel parameters
 struct RelocInline {
   RelocDescDev d[kRelocInlineDescs];

@@ -68,12 +68,6 @@ struct TileWalk {
   }
 };
 
-// U of a (chunk, layer) travels in its native form - one contiguous run per tile, the caller's strides kept in shared memory -
-// when a token's U row fits the stage's U area and the slice holds all heads of the row (or U is shared by all heads).
-__device__ __forceinline__ bool u_native(const RelocGeom& g, long long u_tok_stride, long long u_head_stride) {
-  return u_tok_stride * 2 <= g.su_row && (u_head_stride == 0 || g.n_hg == 1);
-}
-
 // ---- packed fp32 pairs (sm_100a FFMA2 / FMUL2): two fp32 lanes per 64-bit register pair
 __device__ __forceinline__ uint64_t pk2(float lo, float hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ void upk2(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
@@ -197,7 +191,11 @@ __device__ __forceinline__ void slab_steps(const SlabArgs& s, const uint32_t (*a
 template <int KT>
 __device__ __forceinline__ void slab_run(const SlabArgs& s, int rope, uint32_t ua) {
   uint32_t afr[KT > 0 ? KT : 1][4];
+#ifdef KAM_VAR_NORAG
+  if (false) {
+#else
   if (KT > 0 && s.m_rag) {
+#endif
     const int t4 = threadIdx.x & 3;
 #pragma unroll
     for (int kt = 0; kt < KT; ++kt)
@@ -346,7 +344,11 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
             const int gt = dst0 + tok0 + r;
             const int pg = g.P_shift >= 0 ? (gt >> g.P_shift) : gt / g.P;
             const int in_pg = gt - pg * g.P;
+#ifdef KAM_VAR_LDG
+            const int page = (flags & FLAG_INLINE_PAGES) ? bt[pg] : __ldg(bt + pg);
+#else
             const int page = bt[pg];             // generic load: the list may sit in the kernel parameters
+#endif
             int slot = -1, rd = 0;
             if (static_cast<unsigned>(page) < static_cast<unsigned>(p.num_pages)) { slot = page * g.P + in_pg; rd = slot; }
             else if (p.err && w.l == 0 && w.hg == 0 && w.kv == 0 && (in_pg == 0 || tok0 + r == 0)) atomicAdd(p.err, 1);
@@ -417,7 +419,7 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
           const char* s0 = src + (static_cast<long long>(tok0) * u_tok_stride + h0 * u_head_stride) * 2;
           uint8_t* dst = st + (role == 2 ? g.st_uk : g.st_uv);
           const bool heads_adjacent = hf_n == 1 || u_head_stride == m;
-          if (u_native(g, u_tok_stride, u_head_stride)) {
+          if (u_form(g.su_row, g.HG, g.n_hg, m, u_tok_stride, u_head_stride) == U_NATIVE) {
             if (lane == 0) {
               // a ragged rank can leave < 16 bytes at the end of a chunk's last tile: those travel as plain 2-byte accesses
               const uint32_t total = static_cast<uint32_t>(nvalid) * static_cast<uint32_t>(u_tok_stride) * 2u, bulk = total & ~15u;
@@ -469,7 +471,7 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
       has_uk = m && desc.Uk && !inplace; has_uv = m && desc.Uv && !inplace && g.nkv == 2;
       // strides of U in the stage: the caller's own when the tile arrived as one copy (see the producer), else padded rows of
       // head runs of m elements
-      if (u_native(g, desc.u_token_stride, desc.u_head_stride)) { su = static_cast<int>(desc.u_token_stride) * 2; uhs = static_cast<int>(desc.u_head_stride); }
+      if (u_form(g.su_row, g.HG, g.n_hg, m, desc.u_token_stride, desc.u_head_stride) == U_NATIVE) { su = static_cast<int>(desc.u_token_stride) * 2; uhs = static_cast<int>(desc.u_head_stride); }
       else { su = g.su_row; uhs = m; }
       pool_k = static_cast<char*>(p.pool_k[w.l]) + static_cast<size_t>(w.hg) * g.slice_bytes;
       pool_v = g.nkv == 2 ? static_cast<char*>(p.pool_v[w.l]) + static_cast<size_t>(w.hg) * g.slice_bytes : nullptr;
