@@ -16,8 +16,10 @@ Inputs are resident in HBM before the timed region; every step touches > 1 GB of
 
 metric = relocate+patch GB/s: ALGORITHMIC bytes of phase A (page read + page write + U + W + block table)
 divided by the device time of phase A.  The other two headline figures (us per 1024-token chunk, decode tokens/s) and all
-three kernels' roofline fractions ride along in the same line.  N > 1: requests are sharded over ranks, no data-path
-collective (the path partitions by request), time = max over ranks, value = all ranks' bytes / that.
+three kernels' roofline fractions ride along in the same line.  N > 1: requests are sharded over ranks (rank_requests),
+no data-path collective (the path partitions by request), time = max over ranks, value = all ranks'
+bytes / that.  The rank-aware part (timed loop, reductions, the rank-0 line) is `run()`; tests/test_multirank.py drives it
+with a stub workload over gloo.
 """
 import argparse
 import json
@@ -52,21 +54,30 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    """SM clock and throttle reasons sampled DURING the timed region: NVML polled from a thread every ~2 ms (a 60 ms region
+    still yields tens of samples); `nvidia-smi -lms 20` as the fallback when the NVML binding is missing."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, gpu_index):
         self.rows, self.proc, self.idx = [], None, gpu_index
         self.t0 = self.t1 = None                      # host times bracketing the timed region: only samples inside count
-
-    def mark_begin(self):
-        self.t0 = time.time()
-
-    def mark_end(self):
-        self.t1 = time.time()
+        self.nvml, self.stop_flag, self.sm_max = None, False, None
 
     def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[self.idx]) if vis and all(x.strip().isdigit() for x in vis.split(",")) else self.idx
+            h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            self.nvml = (pynvml, h)
+            self.th = threading.Thread(target=self._poll, daemon=True)
+            self.th.start()
+            return
+        except Exception:
+            self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
                                           "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
@@ -75,11 +86,32 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
+    def _poll(self):
+        pynvml, h = self.nvml
+        bits = {"hw_slowdown": pynvml.nvmlClocksEventReasonHwSlowdown, "hw_thermal_slowdown": pynvml.nvmlClocksEventReasonHwThermalSlowdown,
+                "sw_thermal_slowdown": pynvml.nvmlClocksEventReasonSwThermalSlowdown, "sw_power_cap": pynvml.nvmlClocksEventReasonSwPowerCap}
+        while not self.stop_flag:
+            try:
+                sm = pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
+                rs = pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+                self.rows.append((time.time(), float(sm), [n for n, b in bits.items() if rs & b]))
+            except Exception:
+                pass
+            time.sleep(0.002)
+
     def _read(self):
         for line in self.proc.stdout:
             self.rows.append([x.strip() for x in line.split(",")] + [time.time()])
 
     def stop(self):
+        inside = lambda t: self.t0 is None or self.t1 is None or self.t0 <= t <= self.t1 + 0.02
+        if self.nvml:
+            self.stop_flag = True
+            self.th.join(timeout=1)
+            rows = [r for r in self.rows if inside(r[0])]
+            sm = [r[1] for r in rows]
+            return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": self.sm_max, "reasons": sorted({n for r in rows for n in r[2]}),
+                    "samples": len(sm), "how": "NVML polled every ~2 ms inside the timed region"}
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -87,20 +119,36 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        rows = [r for r in self.rows if len(r) >= 10 and r[1].replace(".", "").isdigit()]
-        if self.t0 is not None and self.t1 is not None:
-            rows = [r for r in rows if self.t0 <= r[-1] <= self.t1 + 0.02]
+        rows = [r for r in self.rows if len(r) >= 10 and r[1].replace(".", "").isdigit() and inside(r[-1])]
         sm = [float(r[1]) for r in rows]
         mx = [float(r[2]) for r in rows if r[2].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = sorted({n for r in rows for n, v in zip(names, r[5:9]) if v.lower().startswith("active")})
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
-                "samples": len(sm)}
+                "samples": len(sm), "how": "nvidia-smi -lms 20"}
 
 
 # ------------------------------------------------------------------------------------------------------- the workload
+class DeviceClock:
+    """Phase boundaries as CUDA events on the launching stream (torch's current stream, which the binding passes on)."""
+
+    def __init__(self, torch):
+        self.torch = torch
+
+    def mark(self):
+        e = self.torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
+
+    def ms(self, a, b):
+        return a.elapsed_time(b)
+
+    def sync(self):
+        self.torch.cuda.synchronize()
+
+
 class Workload:
-    def __init__(self, device, rank, use_graph=True):
+    def __init__(self, device, rank, use_graph=True, world=1):
         import numpy as np
         import torch
 
@@ -111,6 +159,9 @@ class Workload:
         cfg = self.cfg = CONFIGS[CFG_ID]
         L, H, D, P, T, m = cfg.n_layers, cfg.n_kv_heads, cfg.row_dim, cfg.page_size, cfg.chunk_tokens, cfg.rank
         self.n_chunks = cfg.chunks_per_step
+        # the job serves world * N_REQ requests; this rank owns the block rank_requests() names.  A request's content (which
+        # canonical set it recalls from) follows its GLOBAL id, so the ranks do different work of the same shape.
+        self.global_ids = rank_requests(rank, world)
         self.rng = np.random.Generator(np.random.PCG64(cfg.seed + 1000 * rank))
         seed = [cfg.seed * 100003 + 7919 * rank]
 
@@ -145,7 +196,7 @@ class Workload:
         for r in range(N_REQ):
             self.ctx_b.kam_window_open(r, 0)
             for c in range(self.n_chunks):
-                ch, pa = self.sets[r % N_SETS][c]
+                ch, pa = self.sets[self.global_ids[r] % N_SETS][c]
                 self.ctx_b.kam_admit(r, B.KAM_BACK, ch, pa, m, 1)
         self.q = rnd((N_REQ, cfg.n_q_heads, D), 1.0)
         self.out = torch.zeros((N_REQ, cfg.n_q_heads, D), dtype=torch.bfloat16, device=device)
@@ -180,10 +231,11 @@ class Workload:
         return (self.ctx_a.kam_get_stats()["kernels_launched"] + self.ctx_b.kam_get_stats()["kernels_launched"]
                 + self.graph_replays * self.launches_per_replay)
 
-    def step(self, i, ev=None):
+    def step(self, i, mark=None):
+        """One pass of the hot path.  mark(k): phase boundary k (0 .. 3), recorded by the caller's clock."""
         cfg, B, T, m = self.cfg, self.B, self.cfg.chunk_tokens, self.cfg.rank
-        r, cs = i % N_REQ, self.sets[i % N_SETS]
-        rec = (lambda k: ev[k].record()) if ev is not None else (lambda k: None)
+        r, cs = i % N_REQ, self.sets[(i + self.global_ids[0]) % N_SETS]
+        rec = mark if mark is not None else (lambda k: None)
         rec(0)
         # phase A: 8 chunks relocated+patched to random offsets, one launch
         p = self.rng.integers(0, cfg.max_pos, size=self.n_chunks)
@@ -207,7 +259,10 @@ class Workload:
 class E2E:
     """The same path through the C-ABI entries that take HOST buffers: canonical chunks and factors live in pinned host
     memory (an off-device canonical store), H2D inside kam_relocate_patch_host; the decode query comes from the host
-    and out / lse go back to it inside kam_paged_decode_merge_host."""
+    and out / lse go back to it inside kam_paged_decode_merge_host.  Pipelined (the library's default): the copy of chunk
+    c + 1 runs on the library's copy stream under the kernel of chunk c, the 28 decode calls share one pinned plan and the
+    step ends with ONE synchronise, after which the host reads out / lse.  Serial (options host_copy_overlap = 0,
+    host_entries_sync = 1): round 1's behaviour, every decode call synchronises."""
 
     def __init__(self, wl, device):
         torch = wl.torch
@@ -238,22 +293,39 @@ class E2E:
         self.starts = torch.arange(0, (wl.n_chunks + 1) * T, T, dtype=torch.int32, device=device).reshape(1, -1)
         self.nc = torch.tensor([wl.n_chunks], dtype=torch.int32, device=device)
         self.q_h = wl.q[:1].to("cpu").pin_memory()
-        self.out_h = torch.zeros((1, cfg.n_q_heads, cfg.row_dim), dtype=torch.bfloat16).pin_memory()
-        self.lse_h = torch.zeros((1, cfg.n_q_heads), dtype=torch.float32).pin_memory()
+        self.out_h = torch.zeros((L, 1, cfg.n_q_heads, cfg.row_dim), dtype=torch.bfloat16).pin_memory()
+        self.lse_h = torch.zeros((L, 1, cfg.n_q_heads), dtype=torch.float32).pin_memory()
         self.h2d += L * self.q_h.numel() * 2
-        self.d2h = L * (self.out_h.numel() * 2 + self.lse_h.numel() * 4)
+        self.d2h = self.out_h.numel() * 2 + self.lse_h.numel() * 4
 
-    def step(self, i):
+    def step(self, i, pipelined=True):
         wl, cfg = self.wl, self.wl.cfg
         T, m = cfg.chunk_tokens, cfg.rank
         p = wl.rng.integers(0, cfg.max_pos, size=wl.n_chunks)
         for c, (k, v, uk, wk, uv, wv, _slab) in enumerate(self.chunks):
             wl.ctx_a.kam_relocate_patch_host(self.bt.reshape(-1), c * T, T, 0, int(p[c]), k, v, uk, wk, uv, wv, m)
+        if pipelined:
+            wl.ctx_a.kam_paged_decode_plan(self.bt, self.starts, None, self.nc)
         for l in range(cfg.n_layers):
-            wl.ctx_a.kam_paged_decode_merge_host(self.q_h, self.bt, self.starts, None, self.nc, l, wl.sm_scale, self.out_h, self.lse_h)
+            wl.ctx_a.kam_paged_decode_merge_host(self.q_h, self.bt, self.starts, None, self.nc, l, wl.sm_scale, self.out_h[l], self.lse_h[l])
+        wl.torch.cuda.synchronize()                  # the step's result (out, lse of every layer) is now readable on the host
+        return float(self.lse_h[-1, 0, 0])
 
 
 # ------------------------------------------------------------------------------------------------------- CPU oracle legs
+_ORACLE_CORES = 1
+
+
+def _timed_oracle(fn):
+    """Runs fn() once; returns (seconds, cores it kept busy = process CPU time / wall time)."""
+    global _ORACLE_CORES
+    t0, c0 = time.perf_counter(), time.process_time()
+    fn()
+    dt = time.perf_counter() - t0
+    _ORACLE_CORES = max(1, int(round((time.process_time() - c0) / dt)))
+    return dt, _ORACLE_CORES
+
+
 def oracle_sample(n_chunks, n_layers, seed=1):
     """Times oracle/reuse.py (as it stands) on n_chunks x n_layers (chunk, layer) units of config 2.  Returns (GB/s, seconds)."""
     import numpy as np
@@ -268,24 +340,63 @@ def oracle_sample(n_chunks, n_layers, seed=1):
     f = lambda t: t.to(torch.float64).numpy()
     pool_k = np.zeros((T // P, P, H, D), np.uint16); pool_v = np.zeros_like(pool_k)
     bt = rng.permutation(T // P).astype(np.int32)
-    t0, c0 = time.perf_counter(), time.process_time()
-    for ch in chunks:
-        p = int(rng.integers(0, cfg.max_pos))
-        for l in range(n_layers):
-            reuse.relocate_patch_layer(pool_k, pool_v, bt, 0, f(ch["K"][l]), f(ch["V"][l]), p, f(ch["Uk"][l]), f(ch["Wk"][l]),
-                                       f(ch["Uv"][l]), f(ch["Wv"][l]), theta=cfg.theta, rope_off=cfg.rope_off, d_r=cfg.rope_dim)
-    dt = time.perf_counter() - t0
-    global _ORACLE_CORES
-    _ORACLE_CORES = max(1, int(round((time.process_time() - c0) / dt)))       # threads the oracle actually kept busy
+
+    def work():
+        for ch in chunks:
+            p = int(rng.integers(0, cfg.max_pos))
+            for l in range(n_layers):
+                reuse.relocate_patch_layer(pool_k, pool_v, bt, 0, f(ch["K"][l]), f(ch["V"][l]), p, f(ch["Uk"][l]), f(ch["Wk"][l]),
+                                           f(ch["Uv"][l]), f(ch["Wv"][l]), theta=cfg.theta, rope_off=cfg.rope_off, d_r=cfg.rope_dim)
+    dt, _ = _timed_oracle(work)
     nbytes = n_chunks * n_layers * algorithmic_bytes_relocate(T, H, D, m, P)
     return nbytes / dt / 1e9, dt
 
 
-_ORACLE_CORES = 1
+def oracle_inplace_sample(n_chunks, n_layers, seed=2):
+    """oracle/reuse.rotate_inplace_layer (row A6) on n_chunks x n_layers survivors of config 2's shape.  (GB/s, seconds, cores)."""
+    import numpy as np
+
+    from oracle import reuse
+    from synth import CONFIGS
+    cfg = CONFIGS[CFG_ID]
+    rng = np.random.Generator(np.random.PCG64(seed))
+    T, H, D, P = cfg.chunk_tokens, cfg.n_kv_heads, cfg.row_dim, cfg.page_size
+    pools = [rng.integers(0x3c00, 0x4000, size=(T // P, P, H, D)).astype(np.uint16) for _ in range(n_layers)]     # bf16 bits in [~0.008, 2)
+    bt = rng.permutation(T // P).astype(np.int32)
+
+    def work():
+        for _ in range(n_chunks):
+            for l in range(n_layers):
+                reuse.rotate_inplace_layer(pools[l], bt, 0, T, -T, theta=cfg.theta, rope_off=cfg.rope_off, d_r=cfg.rope_dim)
+    dt, cores = _timed_oracle(work)
+    return n_chunks * n_layers * (2 * T * H * D * 2) / dt / 1e9, dt, cores
+
+
+def oracle_decode_sample(n_layers, seed=3):
+    """oracle/attention.attend_bruteforce (rows A8 + A9 by their definition) for ONE request of config 2 (8 chunks x 1024 tokens,
+    28 query heads) over n_layers layers.  (GB/s of K+V read, tokens/s for a batch of 1, seconds, cores)."""
+    import numpy as np
+
+    from oracle import attention as att
+    from synth import CONFIGS
+    cfg = CONFIGS[CFG_ID]
+    rng = np.random.Generator(np.random.PCG64(seed))
+    T, H, D, n = cfg.chunk_tokens, cfg.n_kv_heads, cfg.row_dim, cfg.chunks_per_step
+    layers = [[{"k": rng.standard_normal((T, H, D)), "v": rng.standard_normal((T, H, D)), "delta": int(rng.integers(-4096, 4096))} for _ in range(n)]
+              for _ in range(n_layers)]
+    q = rng.standard_normal((cfg.n_q_heads, D))
+    rope = dict(theta=cfg.theta, rope_off=cfg.rope_off, d_r=cfg.rope_dim)
+
+    def work():
+        for chunks in layers:
+            att.attend_bruteforce(q, chunks, D ** -0.5, rope)
+    dt, cores = _timed_oracle(work)
+    nbytes = n_layers * n * T * H * 2 * D * 2
+    return nbytes / dt / 1e9, 1.0 / (dt / n_layers * cfg.n_layers), dt, cores
 
 
 def cpu_threads():
-    """Cores the last oracle_sample() actually used: process CPU time / wall time (the numpy fp64 oracle is mostly one thread)."""
+    """Cores the last oracle leg actually used: process CPU time / wall time (the numpy fp64 oracle is mostly one thread)."""
     return _ORACLE_CORES
 
 
@@ -311,7 +422,6 @@ def run_reference(args):
         "e2e": {"value": value, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
-
 # ------------------------------------------------------------------------------------------------------- extras (outside the step)
 def _time_ms(torch, fn, reps):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -324,11 +434,15 @@ def _time_ms(torch, fn, reps):
 
 
 def extras(wl, device, peak):
-    """Measured after the timed region, NOT part of the step or of `value`: the paper's "rank-invariant in latency" claim
-     as a rank sweep of the relocate kernel on config 2's shape, the rank-m patch applied ON READ inside the decode
-    (row A8's second form), the decode on the shapes of configs 4 and 5 (2.3 / 4.3 GB per layer instead of config 2's 0.54 GB),
-    and the MLA instantiation (config 3's shape): relocate+patch and absorbed decode.  Every
-    figure is algorithmic bytes / device time, as a fraction of the measured HBM peak."""
+    """Measured after the timed region, NOT part of the step or of `value`.  Every figure is algorithmic bytes / device time
+    (CUDA events around back-to-back launches) as a fraction of the measured HBM peak:
+      * the paper's "rank-invariant in latency" claim as a rank sweep m in {0, 4, 16, 32, 48, 64} of the relocate kernel
+        on config 2's shape (SURVEY.md 8(d) T11), and kam_rotate_inplace alone (row A6);
+      * relocate+patch on the shapes of configs 4 (MHA-32, m = 16, T = 1280) and 5 (GQA-8, m = 32, T = 2048), every launch
+        reading sources no other launch of the loop reads (no L2 reuse), and config 3's stated launch of 96 relocations;
+      * the stateless decode call (plan + decode + merge per call; with the plan pinned once for all layers; with the rank-16
+        patch applied ON READ, row A8's second form) and the decode on the shapes of configs 4 and 5;
+      * the MLA instantiation (config 3's shape): relocate+patch, absorbed decode without and with the on-read patch."""
     import torch
     kam, B, cfg = wl.kam, wl.B, wl.cfg
     from synth import CONFIGS, randn_device
@@ -339,9 +453,14 @@ def extras(wl, device, peak):
         seed[0] += 1
         return randn_device(shape, seed[0], std, torch.bfloat16, device)
 
-    # ---- T11: rank sweep, one launch of 8 chunks x 28 layers per rank; sources/destinations rotate over 4 request slots
+    def entry(nbytes, ms, **kw):
+        d = {"ms": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
+        d.update(kw)
+        return d
+
+    # ---- T11: rank sweep, one launch of 8 chunks x 28 layers per rank; sources/destinations rotate over the request slots
     sweep = {}
-    for m in (0, 16, 32, 64):
+    for m in (0, 4, 16, 32, 48, 64):
         pats = None
         if m:
             pats = [kam.Patch([rnd((T, H, m)) for _ in range(L)], [rnd((H, m, D), cfg.w_std) for _ in range(L)],
@@ -349,17 +468,54 @@ def extras(wl, device, peak):
         it = [0]
 
         def launch():
-            r, cs = it[0] % bench_slots, wl.sets[it[0] % N_SETS]
+            r, cs = it[0] % N_REQ, wl.sets[it[0] % N_SETS]
             it[0] += 1
             wl.ctx_a.kam_relocate_patch_batch([(wl.bt_a, (r * n + c) * T, cs[c][0], 1000 + 37 * c + it[0], pats[c] if pats else None, m) for c in range(n)])
-        bench_slots = N_REQ
+        g0 = wl.ctx_a.kam_get_stats()["generic_launches"]
         ms = _time_ms(torch, launch, 10)
         nbytes = n * L * algorithmic_bytes_relocate(T, H, D, m, P) if m else n * L * (2 * 2 * T * H * D * 2 + 4 * (T // P))
-        sweep["m=%d" % m] = {"ms": ms, "us_per_1024tok_chunk": 1e3 * ms / n, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
+        sweep["m=%d" % m] = entry(nbytes, ms, us_per_1024tok_chunk=1e3 * ms / n, tiled_kernel=wl.ctx_a.kam_get_stats()["generic_launches"] == g0)
         del pats
     out["relocate_rank_sweep"] = sweep
 
-    # ---- A8, second form: decode with the rank-16 patch applied on read (stateless call: plan + decode + merge per layer)
+    # ---- row A6 alone: kam_rotate_inplace over one request's 8 chunks (8192 tokens x 28 layers, K only), rotating requests
+    it = [0]
+
+    def launch():
+        r = it[0] % N_REQ
+        it[0] += 1
+        wl.ctx_a.kam_rotate_inplace(wl.bt_a, r * n * T, n * T, -T)
+    ms = _time_ms(torch, launch, 10)
+    out["rotate_inplace_alone"] = entry(n * L * 2 * T * H * D * 2, ms, bytes="K rows read + written, V untouched")
+
+    # ---- relocate+patch on the shapes of configs 4 and 5: a few resident layers, distinct sources and destinations per launch
+    for name, cid, Lx, n_src, per_launch in (("relocate_config4_shape_mha32_m16_T1280", 4, 4, 16, 4), ("relocate_config5_shape_gqa8_m32_T2048", 5, 4, 32, 8)):
+        cx = CONFIGS[cid]
+        Hx, Dx, Px, Tx, mx = cx.n_kv_heads, cx.row_dim, cx.page_size, cx.chunk_tokens, cx.rank
+        srcs = [(kam.Chunk([rnd((Tx, Hx, Dx)) for _ in range(Lx)], [rnd((Tx, Hx, Dx)) for _ in range(Lx)]),
+                 kam.Patch([rnd((Tx, Hx, mx)) for _ in range(Lx)], [rnd((Hx, mx, Dx), cx.w_std) for _ in range(Lx)],
+                           [rnd((Tx, Hx, mx)) for _ in range(Lx)], [rnd((Hx, mx, Dx), cx.w_std) for _ in range(Lx)])) for _ in range(n_src)]
+        npx = n_src * Tx // Px
+        poolx = kam.Pool([torch.zeros((npx, Px, Hx, Dx), dtype=torch.bfloat16, device=device) for _ in range(Lx)],
+                         [torch.zeros((npx, Px, Hx, Dx), dtype=torch.bfloat16, device=device) for _ in range(Lx)])
+        ctxx = kam.Context(kam.make_layout(B.KAM_MHA if cx.n_q_heads == Hx else B.KAM_GQA, Lx, cx.n_q_heads, Hx, Dx, 0, Dx, True, Px, cx.theta), poolx)
+        btx = torch.randperm(npx, device=device, dtype=torch.int32)
+        it = [0]
+
+        def launch():
+            i0 = (it[0] * per_launch) % n_src
+            it[0] += 1
+            ctxx.kam_relocate_patch_batch([(btx, (i0 + c) * Tx, srcs[i0 + c][0], 777 + 1000 * c + it[0], srcs[i0 + c][1], mx) for c in range(per_launch)])
+        reps = n_src // per_launch - 1                       # warm-up launch + reps launches = every source exactly once
+        ms = _time_ms(torch, launch, reps)
+        nbytes = per_launch * Lx * algorithmic_bytes_relocate(Tx, Hx, Dx, mx, Px)
+        out[name] = entry(nbytes, ms, us_per_1024tok_chunk=1e3 * ms / per_launch * 1024 / Tx * cx.n_layers / Lx, layers_resident=Lx,
+                          chunks_per_launch=per_launch, note="us per 1024 tokens scaled to the config's %d layers; every launch reads sources no other timed launch reads" % cx.n_layers,
+                          tiled_kernel=ctxx.kam_get_stats()["generic_launches"] == 0)
+        ctxx.close()
+        del srcs, poolx, ctxx, btx
+
+    # ---- A8: the stateless decode call on config 2's shape: per-call plan | plan pinned once | rank-16 patch on read
     Ld = 4
     ppr = n * T // P
     npages = N_REQ * ppr
@@ -371,8 +527,10 @@ def extras(wl, device, peak):
     wl.ctx_a.kam_decode_set_max_patch_rank(16)
     refs = [B.patch_refs([[(rnd((T, H, m)), rnd((H, m, D), cfg.w_std), rnd((T, H, m)), rnd((H, m, D), cfg.w_std), m) for _ in range(n)]
                           for _ in range(N_REQ)], device) for _ in range(Ld)]
-    for name, pr in (("decode_stateless_no_patch", None), ("decode_stateless_on_read_patch_m16", refs)):
+    for name, pr, pin in (("decode_stateless_no_patch", None, False), ("decode_stateless_pinned_plan", None, True),
+                          ("decode_stateless_on_read_patch_m16", refs, False), ("decode_stateless_on_read_patch_m16_pinned_plan", refs, True)):
         it = [0]
+        wl.ctx_a.kam_paged_decode_plan(bt if pin else None, starts, offs, nc, has_patches=pr is not None)
 
         def launch():
             l = it[0] % Ld
@@ -380,8 +538,9 @@ def extras(wl, device, peak):
             wl.ctx_a.kam_paged_decode_merge(wl.q, bt, starts, offs, nc, l, wl.sm_scale, wl.out, wl.lse, patches=pr[l] if pr else None)
         ms = _time_ms(torch, launch, 12)
         nbytes = N_REQ * n * T * H * (2 * D + (2 * m if pr else 0)) * 2
-        out[name] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak,
-                     "bytes": "K + V" + (" + U_k + U_v" if pr else "") + " once; on-read rotation by a pending offset in both"}
+        out[name] = entry(nbytes, ms, bytes="K + V" + (" + U_k + U_v" if pr else "") + " once; on-read rotation by a pending offset in both",
+                          what="kam_paged_decode_plan once, then decode + merge per layer" if pin else "plan + decode + merge per call")
+    wl.ctx_a.kam_paged_decode_plan(None, None, None, None)
     del refs
 
     # ---- the decode kernel on the other configs' shapes (stateless call, no patch, two resident layers): a layer of config 2 is
@@ -404,12 +563,12 @@ def extras(wl, device, peak):
             ctxx.kam_paged_decode_merge(qx, btx, stx, None, ncx, it[0] % Lx, Dx ** -0.5, ox, lx)
         ms = _time_ms(torch, launch, 6)
         nbytes = nreq * nch * Tc * Hx * 2 * Dx * 2
-        out[name] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak, "bytes": "K + V once",
-                     "what": "stateless call = plan + kam_paged_decode_kernel + merge; %d q / %d kv heads" % (cx.n_q_heads, Hx)}
+        out[name] = entry(nbytes, ms, bytes="K + V once", what="stateless call = plan + kam_paged_decode_kernel + merge; %d q / %d kv heads" % (cx.n_q_heads, Hx))
         ctxx.close()
         del poolx, ctxx, btx, qx, ox
 
-    # ---- MLA (config 3 shape): relocate+patch of 4 chunks x 27 layers in one launch; absorbed decode, batch 64 x 8192 tokens
+    # ---- MLA (config 3 shape): relocate+patch - 4 chunks x 27 layers, and config 3's stated launch (every ordering of the 4
+    # cached chunks = 96 relocations, one launch); absorbed decode, batch 64 x 8192 tokens, without and with the on-read patch
     c3 = CONFIGS[3]
     L3, D3, P3, T3, m3 = c3.n_layers, c3.row_dim, c3.page_size, c3.chunk_tokens, c3.rank
     lay3 = kam.make_layout(B.KAM_MLA, L3, c3.n_q_heads, 1, D3, c3.rope_off, c3.rope_dim, False, P3, c3.theta, v_dim=c3.v_dim)
@@ -427,28 +586,61 @@ def extras(wl, device, peak):
         it[0] += 1
         ctx3.kam_relocate_patch_batch([(bt3, ((4 * i + c) % (nb3 * nch3)) * T3, ch3[(4 * i + c) % 8][0], 1024 * c, ch3[(4 * i + c) % 8][1], m3) for c in range(4)])
     ms = _time_ms(torch, launch, 10)
-    nbytes = 4 * L3 * algorithmic_bytes_relocate(T3, 1, D3, m3, P3, has_v=False)
-    out["mla_relocate_patch"] = {"ms": ms, "us_per_1024tok_chunk": 1e3 * ms / 4, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
+    out["mla_relocate_patch"] = entry(4 * L3 * algorithmic_bytes_relocate(T3, 1, D3, m3, P3, has_v=False), ms, us_per_1024tok_chunk=1e3 * ms / 4)
+    import itertools
+    perms = list(itertools.permutations(range(4)))
+    it = [0]
+
+    def launch():
+        base = (it[0] % 5) * 96
+        it[0] += 1
+        ctx3.kam_relocate_patch_batch([(bt3, (base + 4 * pi + slot) * T3, ch3[c][0], 1024 * slot, ch3[c][1], m3)
+                                       for pi, perm in enumerate(perms) for slot, c in enumerate(perm)])
+    ms = _time_ms(torch, launch, 5)
+    out["mla_config3_96_relocations_one_launch"] = entry(96 * L3 * algorithmic_bytes_relocate(T3, 1, D3, m3, P3, has_v=False), ms, us_per_1024tok_chunk=1e3 * ms / 96,
+                                                         note="BASELINE.json configs[2] as stated: 4 cached chunks in all 24 orders; each source is read 24 times per launch, "
+                                                              "so most source reads hit L2 - an algorithmic rate, the DRAM traffic is the 3.1 GB of page writes")
     q3 = rnd((nb3, c3.n_q_heads, D3))
     o3 = torch.zeros((nb3, c3.n_q_heads, c3.v_dim), dtype=torch.bfloat16, device=device)
     l3 = torch.zeros((nb3, c3.n_q_heads), dtype=torch.float32, device=device)
     st3 = torch.arange(0, (nch3 + 1) * T3, T3, dtype=torch.int32, device=device).repeat(nb3, 1)
     nc3 = torch.full((nb3,), nch3, dtype=torch.int32, device=device)
     bt3b = bt3.reshape(nb3, -1)
-    it = [0]
+    ctx3.kam_decode_set_max_patch_rank(16)
+    Lr = 2
+    refs3 = [B.patch_refs([[(rnd((T3, 1, m3)), rnd((1, m3, D3), c3.w_std), None, None, m3) for _ in range(nch3)] for _ in range(nb3)], device) for _ in range(Lr)]
+    for name, pr in (("mla_decode_absorbed", None), ("mla_decode_on_read_patch_m16", refs3)):
+        it = [0]
 
-    def launch():
-        l = it[0] % L3
-        it[0] += 1
-        ctx3.kam_paged_decode_merge(q3, bt3b, st3, None, nc3, l, 192 ** -0.5, o3, l3)
-    ms = _time_ms(torch, launch, 27)
-    nbytes = nb3 * nch3 * T3 * D3 * 2
-    out["mla_decode_absorbed"] = {"ms_per_layer": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak,
-                                  "bytes": "every latent+rope row once (it is both key and value)", "batch": nb3, "tokens": nch3 * T3,
-                                  "what": "stateless call = plan + kam_mla_ts_decode_kernel (token-split) + merge",
-                                  "tflops": nb3 * nch3 * T3 * c3.n_q_heads * (D3 + c3.v_dim) * 2 / ms / 1e9}
+        def launch():
+            l = it[0] % L3
+            it[0] += 1
+            ctx3.kam_paged_decode_merge(q3, bt3b, st3, None, nc3, l, 192 ** -0.5, o3, l3, patches=pr[l % Lr] if pr else None)
+        ms = _time_ms(torch, launch, 27)
+        nbytes = nb3 * nch3 * T3 * (D3 + (m3 if pr else 0)) * 2
+        out[name] = entry(nbytes, ms, bytes="every latent+rope row once (it is both key and value)" + (" + its U row" if pr else ""), batch=nb3, tokens=nch3 * T3,
+                          what="stateless call = plan + kam_mla_ts_decode_kernel (token-split) + merge",
+                          tflops=nb3 * nch3 * T3 * c3.n_q_heads * (D3 + c3.v_dim) * 2 / ms / 1e9)
     ctx3.close()
     return out
+
+
+# ------------------------------------------------------------------------------------------------------- ncu evidence
+NCU_SUMMARY = "profiles/ncu_step_r02.json"
+
+
+def ncu_evidence(kernel_key):
+    """DRAM bytes per launch and ncu's own dram__throughput % for the named kernel, from the committed summary of ONE
+    `ncu --set full` capture of a bench step (profiles/ncu_step_r02.md names the command and the commit).  None if absent."""
+    path = os.path.join(ROOT, NCU_SUMMARY)
+    if not os.path.exists(path):
+        return None
+    d = json.load(open(path))
+    k = d.get("kernels", {}).get(kernel_key)
+    if k is None:
+        return None
+    return {"traffic": k.get("dram_bytes"), "ncu_dram_pct": k.get("dram_throughput_pct"), "source": "%s (%s)" % (NCU_SUMMARY, d.get("capture", ""))}
+
 
 # ------------------------------------------------------------------------------------------------------- main
 def rank_requests(rank, world, per_gpu=N_REQ):
@@ -457,27 +649,129 @@ def rank_requests(rank, world, per_gpu=N_REQ):
     return list(range(rank * per_gpu, (rank + 1) * per_gpu))
 
 
-def max_over_ranks(x, world):
-    """Largest value of x over all ranks (device timing is reduced this way; works on NCCL and gloo alike)."""
+def _reduce(x, world, op):
     if world == 1:
         return x
     import torch
     import torch.distributed as dist
     dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
     t = torch.tensor([x], dtype=torch.float64, device=dev)
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(t, op=getattr(dist.ReduceOp, op))
     return float(t.item())
+
+
+def max_over_ranks(x, world):
+    """Largest value of x over all ranks (device timing is reduced this way; works on NCCL and gloo alike)."""
+    return _reduce(x, world, "MAX")
 
 
 def sum_over_ranks(x, world):
-    if world == 1:
-        return x
-    import torch
-    import torch.distributed as dist
-    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
-    t = torch.tensor([x], dtype=torch.float64, device=dev)
-    dist.all_reduce(t, op=dist.ReduceOp.SUM)
-    return float(t.item())
+    return _reduce(x, world, "SUM")
+
+
+def barrier(world, clock):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    clock.sync()
+
+
+def timed_steps(wl, steps, warmup, world, clock, profile=None):
+    """W untimed warm-up steps, then EXACTLY `steps` steps bracketed by barrier + synchronise on both sides; device time of
+    the whole region and of each phase, each the MAX over ranks; bytes summed over ranks.  wl needs step(i, mark),
+    launches(), bytes_a / bytes_b / bytes_c.  clock: DeviceClock (CUDA events) - or a host clock in the gloo test."""
+    for i in range(warmup):
+        wl.step(i)
+    barrier(world, clock)
+    marks = [[None] * 4 for _ in range(steps)]
+    l0 = wl.launches()
+    t_host0 = time.time()
+    t_start = clock.mark()
+    for i in range(steps):
+        if profile and i == 0:
+            profile(True)
+        wl.step(warmup + i, lambda k, row=marks[i]: row.__setitem__(k, clock.mark()))
+        if profile and i == 0:
+            profile(False)
+    t_end = clock.mark()
+    barrier(world, clock)
+    t_host1 = time.time()
+    ms_local = [sum(clock.ms(m[k], m[k + 1]) for m in marks) / steps for k in range(3)]
+    return {
+        "total_ms": max_over_ranks(clock.ms(t_start, t_end), world),
+        "phase_ms": [max_over_ranks(x, world) for x in ms_local], "phase_ms_local": ms_local,
+        "launches_per_step": (wl.launches() - l0) // steps,
+        "bytes": [sum_over_ranks(b, world) for b in (wl.bytes_a, wl.bytes_b, wl.bytes_c)],
+        "host_window": (t_host0, t_host1),
+    }
+
+
+def assemble_line(args, world, tm, peak, peak_src, wl_info, cpu=None, e2e=None, clocks=None, ex=None):
+    """The one JSON line rank 0 prints.  value = ALL ranks' relocate+patch bytes / the slowest rank's device time."""
+    steps = args.steps
+    ms_a, ms_b, ms_c = tm["phase_ms"]
+    by_a, by_b, by_c = tm["bytes"]
+    la, lb, lc = tm["phase_ms_local"]
+    gb = lambda b, t_ms: b / (t_ms * 1e-3) / 1e9
+    L, n_req = wl_info["n_layers"], wl_info["n_req"]
+    tot = la + lb + lc
+    kernels = {
+        "kam_relocate_patch_kernel": {"bound": "hbm", "achieved": gb(wl_info["bytes_a"], la), "bytes_per_launch": wl_info["bytes_a"], "ms_per_launch": la, "share_of_step": la / tot},
+        "window_slide(kam_slide)": {"bound": "hbm", "achieved": gb(wl_info["bytes_b"], lb), "bytes_per_launch": wl_info["bytes_b"], "ms_per_launch": lb, "share_of_step": lb / tot},
+        "kam_paged_decode_kernel(+merge)": {"bound": "hbm", "achieved": gb(wl_info["bytes_c"], lc), "bytes_per_launch": wl_info["bytes_c"] / L, "ms_per_launch": lc / L, "share_of_step": lc / tot},
+    }
+    for name, k in kernels.items():
+        k.update({"peak": peak, "unit": "GB/s", "frac": k["achieved"] / peak})
+        ev = ncu_evidence(name)
+        if ev:
+            k.update({"traffic": ev["traffic"], "ncu_dram_pct": ev["ncu_dram_pct"], "traffic_source": ev["source"]})
+    dom = max(kernels, key=lambda k: kernels[k]["share_of_step"])
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["achieved"], "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": kernels[dom].get("traffic"), "ncu_dram_pct": kernels[dom].get("ncu_dram_pct"),
+                "traffic_source": kernels[dom].get("traffic_source", "no ncu summary committed: traffic is null"),
+                "denominators": "frac = achieved / MEASURED_PEAKS.json hbm_gbs (a copy: read + write); ncu_dram_pct = ncu's "
+                                "dram__throughput.avg.pct_of_peak_sustained_elapsed of the same kernel (BASELINE.json's 'per ncu')"}
+    return {
+        "metric": "relocate+patch GB/s", "value": by_a / (ms_a * 1e-3) / 1e9, "unit": "GB/s", "n_gpus": world, "steps": steps, "warmup": args.warmup,
+        "ms_per_step": tm["total_ms"] / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[1]: GQA Qwen2-VL-7B-like, 28 layers, 28q/4kv heads, head_dim 128, theta 1e6, "
+                               "8 chunks x 1024 tokens per slide, rank-16 patch, page 16, offsets U[0,32768)",
+                   "requests_per_gpu": n_req, "decode_batch": n_req, "window_tokens": wl_info["window_tokens"],
+                   "decode_launch": wl_info["decode_launch"],
+                   "l2": "inputs larger than L2: each step streams >1 GB of fresh source and destination; request and canonical set rotate",
+                   "parallelism": "requests sharded over ranks (rank r serves global requests [r*%d, (r+1)*%d)), no collective" % (n_req, n_req)},
+        "phases_ms": {"relocate_patch_batch": ms_a, "window_slide": ms_b, "decode_all_layers": ms_c},
+        "us_per_1024tok_chunk": 1e3 * ms_a / wl_info["n_chunks"],
+        "decode_tok_per_s": world * n_req / (ms_c * 1e-3),
+        "decode_note": "attention only: batch / (per-layer attention time x 28 layers); projections and MLP are not part of the method",
+        "step_gbs": (by_a + by_b + by_c) / (tm["total_ms"] / steps * 1e-3) / 1e9,
+        "roofline": roofline, "roofline_all": kernels, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": tm["launches_per_step"], "clocks": clocks,
+        "extras_outside_the_step": ex,
+    }
+
+
+def run(args, world, rank, wl, clock, wl_info, sampler=None, after=None):
+    """The rank-aware part of the bench: timed region (barrier + sync on both sides, max over ranks), then rank 0 assembles and
+    prints the line.  `after(tm)` (rank 0, single GPU) returns the extra legs measured outside the timed region."""
+    prof = None
+    if getattr(args, "profile_step", False):
+        import torch
+        prof = lambda on: torch.cuda.profiler.start() if on else torch.cuda.profiler.stop()
+    if sampler is not None and rank == 0:
+        sampler.start()                              # already streaming when the timed region starts
+    tm = timed_steps(wl, args.steps, args.warmup, world, clock, prof)
+    clocks = None
+    if sampler is not None and rank == 0:
+        sampler.t0, sampler.t1 = tm["host_window"]
+        clocks = sampler.stop()
+    legs = after(tm) if after is not None else {}
+    line = None
+    if rank == 0:
+        peak, peak_src = peaks()
+        line = assemble_line(args, world, tm, peak, peak_src, wl_info, cpu=legs.get("cpu"), e2e=legs.get("e2e"), clocks=clocks, ex=legs.get("extras"))
+        print(json.dumps(line))
+    return line
 
 
 def main():
@@ -511,115 +805,60 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=device)
 
-    wl = Workload(device, rank, use_graph=not args.no_graph)
-    peak, peak_src = peaks()
-
-    def barrier():
-        if world > 1:
-            torch.distributed.barrier()
-        torch.cuda.synchronize()
-
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()                              # already streaming when the timed region starts
-    for i in range(args.warmup):
-        wl.step(i)
-    barrier()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
-    l0 = wl.launches()
-    sampler.mark_begin()
-    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_start.record()
-    for i in range(args.steps):
-        if args.profile_step and i == 0:
-            torch.cuda.profiler.start()
-        wl.step(args.warmup + i, ev[i])
-        if args.profile_step and i == 0:
-            torch.cuda.profiler.stop()
-    t_end.record()
-    barrier()
-    sampler.mark_end()
-    clocks = sampler.stop() if rank == 0 else None
-    launches = (wl.launches() - l0) // args.steps
-    total_ms = max_over_ranks(t_start.elapsed_time(t_end), world)
-    ms = {k: sum(e[k].elapsed_time(e[k + 1]) for e in ev) / args.steps for k in range(3)}
-    ms_a = max_over_ranks(ms[0], world); ms_b = max_over_ranks(ms[1], world); ms_c = max_over_ranks(ms[2], world)
-    n_ranks_bytes_a = sum_over_ranks(wl.bytes_a, world)
-    value = n_ranks_bytes_a / (ms_a * 1e-3) / 1e9
-
-    # e2e: same path through the host-buffer entries
-    e2e = None
-    if not args.no_e2e:
-        ee = E2E(wl, device)
-        for i in range(2):
-            ee.step(i)
-        barrier()
-        n_e = max(2, min(args.steps, 5))
-        t0 = time.perf_counter()
-        for i in range(n_e):
-            ee.step(i)
-        torch.cuda.synchronize()
-        dt = max_over_ranks((time.perf_counter() - t0) / n_e, world)
-        e2e = {"value": sum_over_ranks(wl.bytes_a, world) / dt / 1e9, "unit": "GB/s", "h2d_bytes_per_step": ee.h2d, "d2h_bytes_per_step": ee.d2h,
-               "ms_per_step": dt * 1e3, "what": "8 x kam_relocate_patch_host (one pinned host slab per chunk: rows + factors of 28 layers -> one merged H2D -> kernel) + 28 x "
-               "kam_paged_decode_merge_host (q H2D, out/lse D2H) per step; relocate+patch bytes / whole region"}
-
+    wl = Workload(device, rank, use_graph=not args.no_graph, world=world)
+    peak, _ = peaks()
     cfg = wl.cfg
-    L, T = cfg.n_layers, cfg.chunk_tokens
-    gb = lambda b, t_ms: b / (t_ms * 1e-3) / 1e9
-    kernels = {
-        "kam_relocate_patch_kernel": {"bound": "hbm", "achieved": gb(wl.bytes_a, ms[0]), "bytes_per_launch": wl.bytes_a, "ms_per_launch": ms[0],
-                                      "share_of_step": ms[0] / (ms[0] + ms[1] + ms[2])},
-        "window_slide(kam_slide)": {"bound": "hbm", "achieved": gb(wl.bytes_b, ms[1]), "bytes_per_launch": wl.bytes_b, "ms_per_launch": ms[1],
-                                      "share_of_step": ms[1] / (ms[0] + ms[1] + ms[2])},
-        "kam_paged_decode_kernel(+merge)": {"bound": "hbm", "achieved": gb(wl.bytes_c, ms[2]), "bytes_per_launch": wl.bytes_c_layer, "ms_per_launch": ms[2] / L,
-                                            "share_of_step": ms[2] / (ms[0] + ms[1] + ms[2])},
-    }
-    for k in kernels.values():
-        k.update({"peak": peak, "unit": "GB/s", "frac": k["achieved"] / peak})
-    dom = max(kernels, key=lambda k: kernels[k]["share_of_step"])
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic_r01.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(dom.split("(")[0])
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["achieved"], "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-                "frac": kernels[dom]["frac"], "traffic": traffic}
+    wl_info = {"n_layers": cfg.n_layers, "n_req": N_REQ, "n_chunks": wl.n_chunks, "window_tokens": wl.n_chunks * cfg.chunk_tokens,
+               "bytes_a": wl.bytes_a, "bytes_b": wl.bytes_b, "bytes_c": wl.bytes_c,
+               "decode_launch": "eager" if args.no_graph else "CUDA graph of 28 x (decode, merge), plan rebuilt eagerly per step"}
+    clock = DeviceClock(torch)
 
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu:
-        gbs, dt = oracle_sample(CPU_SAMPLE_CHUNKS, L)
-        cpu = {"value": gbs, "unit": "GB/s", "cores": cpu_threads(), "host_cores": os.cpu_count(), "kind": "oracle", "seconds": dt,
-               "sample": "relocate+patch of %d chunks x 28 layers of config 2 (1.5 steps' worth; a step has 8 chunks), "
-                         "oracle/reuse.py in numpy fp64" % CPU_SAMPLE_CHUNKS}
+    def after(tm):
+        legs = {}
+        # e2e: the same path through the host-buffer entries, H2D and D2H inside the timed region
+        if not args.no_e2e:
+            ee = E2E(wl, device)
+            res = {}
+            for mode, pipelined in (("serial", False), ("pipelined", True)):
+                wl.ctx_a.kam_set_option("host_copy_overlap", int(pipelined))
+                wl.ctx_a.kam_set_option("host_entries_sync", int(not pipelined))
+                for i in range(2):
+                    ee.step(i, pipelined)
+                barrier(world, clock)
+                n_e = max(2, min(args.steps, 5))
+                t0 = time.perf_counter()
+                for i in range(n_e):
+                    ee.step(i, pipelined)
+                torch.cuda.synchronize()
+                res[mode] = max_over_ranks((time.perf_counter() - t0) / n_e, world)
+            by = sum_over_ranks(wl.bytes_a, world)
+            legs["e2e"] = {"value": by / res["pipelined"] / 1e9, "unit": "GB/s", "h2d_bytes_per_step": ee.h2d, "d2h_bytes_per_step": ee.d2h,
+                           "ms_per_step": res["pipelined"] * 1e3, "serial_value": by / res["serial"] / 1e9, "serial_ms_per_step": res["serial"] * 1e3,
+                           "what": "8 x kam_relocate_patch_host (one pinned host slab per chunk: rows + factors of 28 layers -> one merged H2D on the "
+                                   "library's copy stream -> kernel; the copy of chunk c+1 runs under the kernel of chunk c) + kam_paged_decode_plan + 28 x "
+                                   "kam_paged_decode_merge_host (q H2D, out/lse D2H) + ONE synchronise per step, after which the host reads out/lse; "
+                                   "relocate+patch bytes / whole region.  serial_*: options host_copy_overlap=0, host_entries_sync=1 (a synchronise per decode call)"}
+        if rank == 0 and world == 1 and not args.no_cpu:
+            gbs, dt = oracle_sample(CPU_SAMPLE_CHUNKS, cfg.n_layers)
+            cores = cpu_threads()
+            ig, idt, icores = oracle_inplace_sample(4, cfg.n_layers)
+            dg, dtok, ddt, dcores = oracle_decode_sample(4)
+            legs["cpu"] = {"value": gbs, "unit": "GB/s", "cores": cores, "host_cores": os.cpu_count(), "kind": "oracle", "seconds": dt,
+                           "sample": "relocate+patch of %d chunks x 28 layers of config 2 (1.5 steps' worth; a step has 8 chunks), "
+                                     "oracle/reuse.py in numpy fp64" % CPU_SAMPLE_CHUNKS,
+                           "legs": {"rotate_inplace": {"value": ig, "unit": "GB/s", "seconds": idt, "cores": icores,
+                                                       "sample": "oracle/reuse.rotate_inplace_layer on 4 survivors x 28 layers (a slide has 7)"},
+                                    "decode_bruteforce": {"value": dg, "unit": "GB/s", "tok_per_s_batch1_28_layers": dtok, "seconds": ddt, "cores": dcores,
+                                                          "sample": "oracle/attention.attend_bruteforce for ONE request (8 x 1024 tokens, 28 query heads) x 4 layers (a step has 32 requests x 28 layers)"}}}
+        if rank == 0 and world == 1 and not args.no_extras and not args.profile_step:
+            if args.profile_extras:
+                torch.cuda.profiler.start()
+            legs["extras"] = extras(wl, device, peak)
+            if args.profile_extras:
+                torch.cuda.profiler.stop()
+        return legs
 
-    ex = None
-    if rank == 0 and world == 1 and not args.no_extras and not args.profile_step:
-        if args.profile_extras:
-            torch.cuda.profiler.start()
-        ex = extras(wl, device, peak)
-        if args.profile_extras:
-            torch.cuda.profiler.stop()
-
-    if rank == 0:
-        out = {
-            "metric": "relocate+patch GB/s", "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-            "data": "synthetic",
-            "config": {"workload": "BASELINE.json configs[1]: GQA Qwen2-VL-7B-like, 28 layers, 28q/4kv heads, head_dim 128, theta 1e6, "
-                                   "8 chunks x 1024 tokens per slide, rank-16 patch, page 16, offsets U[0,32768)",
-                       "requests_per_gpu": N_REQ, "decode_batch": N_REQ, "window_tokens": wl.n_chunks * T,
-                       "decode_launch": "eager" if args.no_graph else "CUDA graph of 28 x (decode, merge), plan rebuilt eagerly per step",
-                       "l2": "inputs larger than L2: each step streams >1 GB of fresh source and destination; request and canonical set rotate",
-                       "parallelism": "requests sharded over ranks, no collective"},
-            "phases_ms": {"relocate_patch_batch": ms_a, "window_slide": ms_b, "decode_all_layers": ms_c},
-            "us_per_1024tok_chunk": 1e3 * ms_a / wl.n_chunks,
-            "decode_tok_per_s": world * N_REQ / (ms_c * 1e-3),
-            "decode_note": "attention only: batch / (per-layer attention time x 28 layers); projections and MLP are not part of the method",
-            "step_gbs": sum_over_ranks(wl.bytes_a + wl.bytes_b + wl.bytes_c, world) / (total_ms / args.steps * 1e-3) / 1e9 if world == 1 else None,
-            "roofline": roofline, "roofline_all": kernels, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-            "extras_outside_the_step": ex,
-        }
-        print(json.dumps(out))
+    run(args, world, rank, wl, clock, wl_info, sampler=ClockSampler(local), after=after)
     if world > 1:
         torch.distributed.destroy_process_group()
 

@@ -369,7 +369,7 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
       memcpy(pg->pages, ap->sg->host, (size_t)ap->n * 4);
       pg->mirror_dst = ap->d_mirror; pg->n = ap->n;
     }
-    launch_relocate_fast(g, p, *inl, *pg, grid, st);
+    launch_relocate_fast(g, p, *inl, *pg, grid, c->opt.reloc_pdl != 0, st);
   } else {
     GenericParams p{};
     p.descs = d_descs; p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;
@@ -855,7 +855,7 @@ kam_status kam_set_option(kam_ctx* c, const char* key, int64_t value) {
       {"decode_ctas_per_sm", &o.dec_ctas_per_sm, 0, 8}, {"decode_boxes", &o.dec_boxes, 0, 16},
       {"decode_pdl", &o.use_pdl, 0, 1},              {"decode_tma", &o.dec_tma, 0, 1},
       {"host_copy_overlap", &o.host_copy_overlap, 0, 1}, {"host_entries_sync", &o.host_sync, 0, 1},
-      {"reloc_patch_cost_pct", &o.reloc_patch_cost_pct, 50, 200},
+      {"reloc_patch_cost_pct", &o.reloc_patch_cost_pct, 50, 200}, {"reloc_pdl", &o.reloc_pdl, 0, 1},
   };
   for (const Opt& op : opts)
     if (strcmp(op.name, key) == 0) {

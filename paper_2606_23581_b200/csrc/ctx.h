@@ -32,6 +32,7 @@ struct Options {
   int reloc_rb = 0;            // "reloc_row_blocks": 16-token row blocks per tile (0 = automatic)
   int reloc_load_hint = 1;     // "reloc_evict_first": canonical sources are read with an L2 evict-first hint
   int reloc_patch_cost_pct = 108;  // "reloc_patch_cost_pct": cost of a tile that runs the patch, in % of its bytes (work split)
+  int reloc_pdl = 1;           // "reloc_pdl": the relocate kernel is launched with programmatic stream serialization
   int dec_ctas_per_sm = 0;     // "decode_ctas_per_sm" (0 = automatic)
   int dec_boxes = 0;           // "decode_boxes": ring depth of the decode kernel (0 = automatic)
   int use_pdl = 1;             // "decode_pdl": programmatic dependent launch between plan, decode and merge

@@ -259,6 +259,12 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
                             cb.col_off * 2, cb.w_col_off * 2, tab_off);
   }
   __syncthreads();
+  // Programmatic dependent launch: everything above (barrier init, slab table) may run under the tail of the previous kernel on
+  // the stream; nothing below - the first global read or write - starts before that kernel has completed.  The next kernel is
+  // released at once: its prologue then hides under this kernel's tail in the same way (one CTA per SM and ~220 KB of shared
+  // memory: it cannot become resident before a CTA of this kernel has left).
+  grid_dep_wait();
+  grid_dep_launch();
 
   // small batches carry their descriptors in the kernel parameters (no H2D staging copy, no global loads to read them)
   const RelocDescDev* descs = p.descs ? p.descs : inl.d;
@@ -578,13 +584,19 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   }
 }
 
-void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages& pages, int grid, cudaStream_t st) {
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages& pages, int grid, bool pdl, cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(kam_relocate_patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_set = true;
   }
-  kam_relocate_patch_kernel<<<grid, kRelocThreads, g.smem_bytes, st>>>(g, p, inl, pages);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kRelocThreads); cfg.dynamicSmemBytes = g.smem_bytes; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kam_relocate_patch_kernel, g, p, inl, pages);
 }
 
 // ---------------------------------------------------------------------------------------------------------------

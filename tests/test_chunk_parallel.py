@@ -56,6 +56,29 @@ def _gloo_worker(rank, world, port, q_out):
         om, lm = att.lse_merge(o_all[:, b].double().numpy(), l_all[:, b].double().numpy())
         ob, lb = att.attend_bruteforce(q[b], chunks[b], 0.3, rope)
         worst = max(worst, float(np.abs(om - ob).max()), float(np.abs(lm - lb).max()))
+    # the REAL decode_chunk_parallel (state call -> one all-gather -> merge call), driven over gloo with CPU tensors: the two C
+    # entries are stood in for by the oracle (this rank's state over ITS chunks; the P:44 merge in the order the parts arrive)
+    from paper_2606_23581_b200.chunk_parallel import decode_chunk_parallel
+    calls = []
+
+    class OracleCtx:
+        def kam_paged_decode_state(self, q_t, bt, starts, offs, ncs, layer, scale, o_state, l_state, patches=None):
+            calls.append(("state", tuple(o_state.shape), o_state.dtype))
+            for b in range(B):
+                ob_, lb_ = att.attend_chunks_merge(q_t[b].double().numpy(), [chunks[b][c] for c in mine], scale, rope)
+                o_state[b] = torch.from_numpy(ob_).float(); l_state[b] = torch.from_numpy(lb_).float()
+
+        def kam_lse_merge_states(self, o_parts, l_parts, batch, out_t, lse_t):
+            calls.append(("merge", len(o_parts), batch))
+            for b in range(batch):
+                om_, lm_ = att.lse_merge(np.stack([p[b].double().numpy() for p in o_parts]), np.stack([p[b].double().numpy() for p in l_parts]))
+                out_t[b] = torch.from_numpy(om_).float(); lse_t[b] = torch.from_numpy(lm_).float()
+    out_t = torch.zeros((B, Hq, D)); lse_t = torch.zeros((B, Hq))
+    decode_chunk_parallel(OracleCtx(), torch.from_numpy(q).float(), None, None, None, None, 0, 0.3, out_t, lse_t)
+    assert calls == [("state", (B, Hq, D), torch.float32), ("merge", world, B)]
+    for b in range(B):
+        ob, lb = att.attend_bruteforce(q[b], chunks[b], 0.3, rope)
+        worst = max(worst, float(np.abs(out_t[b].double().numpy() - ob).max()), float(np.abs(lse_t[b].double().numpy() - lb).max()))
     q_out.put((rank, worst))
     dist.destroy_process_group()
 
