@@ -14,13 +14,15 @@ Modules
 bf16       round-to-nearest-even fp64 -> bf16, bit packing, ulp          ("one bf16 ULP")
 reuse      Eq. 1: RoPE re-rotation R(delta), rank-m patch, paged scatter
 window     the position-free window store as a deque + page free list
-attention  brute-force softmax attention; per-chunk partials + LSE merge
+attention  brute-force softmax attention; per-chunk partials + LSE merge; the same readout for a block of
+           query rows with a causal mask over the appended tokens
 storage    byte accounting of the stored factors
 
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): every function below is pinned to
 something other than itself - closed forms, the identities the paper states
 (R(d)R(p)=R(p+d), rank-0 = rotation, exact rank-m reconstruction, LSE merge =
 softmax over the concatenation), an independent textbook RoPE restatement, torch's
-own bf16 cast, Eckart-Young, brute-force list rebuilds, and the storage ratios the
+own bf16 cast, Eckart-Young, brute-force list rebuilds, a dense masked score matrix and torch's
+scaled_dot_product_attention (multi-query readout), and the storage ratios the
 paper prints (tests/golden/).  No function is "parity unpinned".
 """

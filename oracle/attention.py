@@ -20,6 +20,15 @@ If v is None (MLA, absorbed form) the value of a token is the first `v_dim` colu
 
 Conventions (reading R-12): natural log, sm_scale inside the exponent, query head hq reads KV
 head hq // G with G = Hq // H, no mask (the decode query is the newest token).
+
+Multi-query readout ("chunked-prefill (multi-query) attention over relocated
+chunks"; the TTFT path of P:105 / P:349: after `apply_reuse` has placed the recalled
+chunks, the appended text turn is prefilled over them):
+  attend_prefill_bruteforce   the same readout for Tq query rows.  With causal=True the
+                              query rows ARE the last Tq cached tokens (reading R-19 in DESIGN.md):
+                              row t sees cached token j iff j <= N - Tq + t, N = all cached tokens
+                              of the request.  It is the single-query definition applied row by
+                              row to the visible prefix - nothing else.
 """
 import numpy as np
 
@@ -127,3 +136,28 @@ def attend_on_read_factorized(q, chunks, sm_scale, rope, v_dim=None):
             oc[hq], lc[hq] = acc / lsum, m + np.log(lsum)
         o.append(oc); l.append(lc)
     return lse_merge(np.stack(o), np.stack(l))
+
+
+def attend_prefill_bruteforce(q, chunks, sm_scale, rope, causal=True, v_dim=None):
+    """q [Tq, Hq, D] -> out [Tq, Hq, Dv], lse [Tq, Hq].  Row t = attend_bruteforce(q[t]) over the cached tokens it may see:
+    all N of them (causal=False), or tokens 0 .. N - Tq + t (causal=True: the rows are the last Tq cached tokens, each
+    seeing the recalled context, the appended tokens before it, and itself).  A row that sees nothing (Tq > N, its index
+    before the first cached token) gives out = 0, lse = -inf."""
+    q = np.asarray(q, np.float64)
+    Tq = q.shape[0]
+    N = sum(c["k"].shape[0] for c in chunks)
+    outs, lses = [], []
+    for t in range(Tq):
+        n_vis = N if not causal else N - Tq + t + 1
+        vis, left = [], max(n_vis, 0)
+        for c in chunks:                                      # the visible prefix, chunk by chunk (a chunk may be cut)
+            take = min(left, c["k"].shape[0])
+            cut = dict(c, k=c["k"][:take], v=None if c.get("v") is None else c["v"][:take])
+            for name in ("Uk", "Uv"):
+                if c.get(name) is not None:
+                    cut[name] = np.asarray(c[name])[:take]
+            vis.append(cut)
+            left -= take
+        o, l = attend_bruteforce(q[t], vis, sm_scale, rope, v_dim)
+        outs.append(o); lses.append(l)
+    return np.stack(outs), np.stack(lses)

@@ -120,3 +120,93 @@ def test_mla_absorbed_form_value_is_the_latent():
     assert np.max(np.abs(o1 - o2)) < 1e-12 and np.max(np.abs(l1 - l2)) < 1e-12
     # GQA head mapping: with H = 1 every query head reads the same keys; different q => different out
     assert not np.allclose(o1[0], o1[1])
+
+
+# ---------------------------------------------------------------------------------------- multi-query readout (f4)
+def _dense_masked_attention(q, K, V, G, sm_scale, causal):
+    """An independent formulation: the full [Tq, N] score matrix per head, a triangular -inf mask, row softmax."""
+    Tq, Hq, _ = q.shape
+    N = K.shape[0]
+    out = np.zeros((Tq, Hq, V.shape[2])); lse = np.zeros((Tq, Hq))
+    for hq in range(Hq):
+        S = sm_scale * np.einsum("td,nd->tn", q[:, hq], K[:, hq // G])
+        if causal:
+            S = np.where(np.arange(N)[None, :] <= (N - Tq + np.arange(Tq))[:, None], S, -np.inf)
+        m = S.max(axis=1, keepdims=True)
+        W = np.exp(S - m)
+        out[:, hq] = (W / W.sum(axis=1, keepdims=True)) @ V[:, hq // G]
+        lse[:, hq] = m[:, 0] + np.log(W.sum(axis=1))
+    return out, lse
+
+
+@pytest.mark.parametrize("causal", [True, False])
+def test_prefill_equals_a_dense_masked_score_matrix(causal):
+    """Row-by-row definition vs the matrix formulation with a triangular mask; chunks with pending offsets (applied to the keys
+    by hand here, through reuse.relocate) and one empty chunk."""
+    H, Hq, D, Tq = 2, 6, 64, 5
+    ch = _chunks(3, 4, H, D, deltas=[0, 37, -5])
+    ch.insert(1, {"k": np.zeros((0, H, D)), "v": np.zeros((0, H, D)), "delta": 9})
+    q = RNG.standard_normal((Tq, Hq, D))
+    out, lse = att.attend_prefill_bruteforce(q, ch, 0.11, ROPE, causal=causal)
+    K = np.concatenate([reuse.relocate(c["k"], c["delta"], **ROPE) for c in ch]); V = np.concatenate([c["v"] for c in ch])
+    want_o, want_l = _dense_masked_attention(q, K, V, Hq // H, 0.11, causal)
+    assert np.allclose(out, want_o, atol=1e-12) and np.allclose(lse, want_l, atol=1e-12)
+
+
+def test_prefill_rows_against_the_single_query_readout_and_closed_forms():
+    H, Hq, D = 1, 2, 64
+    ch = _chunks(2, 6, H, D)
+    N, Tq = 12, 4
+    q = RNG.standard_normal((Tq, Hq, D))
+    out, lse = att.attend_prefill_bruteforce(q, ch, 0.2, ROPE, causal=True)
+    # the LAST row sees every cached token: it is the decode readout (P:44)
+    o_last, l_last = att.attend_bruteforce(q[-1], ch, 0.2, ROPE)
+    assert np.allclose(out[-1], o_last, atol=1e-13) and np.allclose(lse[-1], l_last, atol=1e-13)
+    # without a mask every row is the decode readout of its own query
+    out_nc, lse_nc = att.attend_prefill_bruteforce(q, ch, 0.2, ROPE, causal=False)
+    for t in range(Tq):
+        o, l = att.attend_bruteforce(q[t], ch, 0.2, ROPE)
+        assert np.allclose(out_nc[t], o, atol=1e-13) and np.allclose(lse_nc[t], l, atol=1e-13)
+    # pure self-attention (Tq = N): row 0 sees only token 0 -> out = v_0, lse = scale * q_0 . k_0
+    qq = RNG.standard_normal((N, Hq, D))
+    o_s, l_s = att.attend_prefill_bruteforce(qq, ch, 0.2, ROPE, causal=True)
+    assert np.allclose(o_s[0, 0], ch[0]["v"][0, 0], atol=1e-13) and np.isclose(l_s[0, 1], 0.2 * qq[0, 1] @ ch[0]["k"][0, 0], atol=1e-12)
+    # uniform keys: row t averages the values it sees; lse = ln(count) + s
+    k1 = np.tile(RNG.standard_normal((1, H, D)), (N, 1, 1))
+    uni = [{"k": k1[:7], "v": ch[0]["v"][:6].repeat(2, axis=0)[:7], "delta": 0}, {"k": k1[7:], "v": ch[1]["v"][:5], "delta": 0}]
+    Vall = np.concatenate([c["v"] for c in uni])
+    o_u, l_u = att.attend_prefill_bruteforce(q, uni, 0.2, ROPE, causal=True)
+    for t in range(Tq):
+        n_vis = N - Tq + t + 1
+        assert np.allclose(o_u[t, 0], Vall[:n_vis, 0].mean(axis=0), atol=1e-12)
+        assert np.isclose(l_u[t, 0], np.log(n_vis) + 0.2 * q[t, 0] @ k1[0, 0], atol=1e-12)
+    # more query rows than cached tokens: the rows before the first cached token see nothing
+    o_e, l_e = att.attend_prefill_bruteforce(RNG.standard_normal((N + 2, Hq, D)), ch, 0.2, ROPE, causal=True)
+    assert np.all(o_e[:2] == 0) and np.all(np.isneginf(l_e[:2])) and np.all(np.isfinite(l_e[2:]))
+
+
+def test_prefill_matches_torch_sdpa_for_causal_self_attention():
+    """The special case a library routine covers: Tq = N, one chunk, no pending offset -> torch's scaled_dot_product_attention
+    with is_causal=True (fp64, CPU); GQA by repeating the KV heads."""
+    import torch
+    import torch.nn.functional as F
+    H, Hq, D, N = 2, 4, 64, 9
+    ch = _chunks(1, N, H, D)
+    q = RNG.standard_normal((N, Hq, D))
+    out, _ = att.attend_prefill_bruteforce(q, ch, D ** -0.5, ROPE, causal=True)
+    tq = torch.from_numpy(q).permute(1, 0, 2)[None]                                  # [1, Hq, N, D]
+    tk = torch.from_numpy(ch[0]["k"]).permute(1, 0, 2).repeat_interleave(Hq // H, dim=0)[None]
+    tv = torch.from_numpy(ch[0]["v"]).permute(1, 0, 2).repeat_interleave(Hq // H, dim=0)[None]
+    want = F.scaled_dot_product_attention(tq, tk, tv, is_causal=True)[0].permute(1, 0, 2).numpy()
+    assert np.allclose(out, want, atol=1e-12)
+
+
+def test_prefill_with_patch_on_read_and_mla_value_is_the_latent():
+    """The rows carry Eq. 1 like the decode readout does: pending patch factors cut with their chunk; MLA: value = latent."""
+    H, Hq, D, Tq = 1, 2, 64, 3
+    ch = _chunks(2, 4, H, D, m=2, deltas=[5, 0], with_v=False)
+    q = RNG.standard_normal((Tq, Hq, D))
+    out, lse = att.attend_prefill_bruteforce(q, ch, 0.3, ROPE, causal=True, v_dim=48)
+    K = np.concatenate([reuse.reuse_k(c["k"], c["delta"], c["Uk"], c["Wk"], **ROPE) for c in ch])
+    want_o, want_l = _dense_masked_attention(q, K, K[..., :48], Hq // H, 0.3, True)
+    assert out.shape == (Tq, Hq, 48) and np.allclose(out, want_o, atol=1e-12) and np.allclose(lse, want_l, atol=1e-12)
