@@ -290,6 +290,24 @@ kam_status kam_paged_decode_merge(kam_ctx *ctx, const void *q, const kam_pool *p
 kam_status kam_paged_decode_plan(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_tables, int32_t max_pages,
                                  const int32_t *chunk_starts, const int64_t *chunk_offsets, const int32_t *n_chunks,
                                  int32_t max_chunks, int32_t has_patches, int32_t batch, void *stream);
+/* ---- the same readout for a BLOCK of query rows: chunked prefill over relocated chunks (the TTFT path of
+ * P:105 / P:349: after `apply_reuse` has placed the recalled chunks, the appended text turn is prefilled over them).
+ * q [batch][n_q_tokens][n_q_heads][row_dim] bf16 device (RoPE already applied at the rows' own positions), out the same shape,
+ * lse [batch][n_q_tokens][n_q_heads] f32 (natural log, scale inside).  Paging arguments as kam_paged_decode_merge: the request's
+ * cached tokens are the logical tokens [0, N_b) of its block-table row, cut into chunks by chunk_starts; chunk_offsets (or NULL)
+ * are applied ON READ, by rotating the query block once per chunk (the pool is never written).
+ *   causal = 0: every row sees all N_b cached tokens.
+ *   causal = 1: the rows ARE the last n_q_tokens cached tokens (their keys and values were appended to the pool before this
+ *               call): row t sees cached token j iff j <= N_b - n_q_tokens + t (reading R-19).  A row that sees nothing
+ *               (n_q_tokens > N_b) gives out = 0, lse = -inf.
+ * The per-chunk softmax states are merged in registers by the same log-sum-exp state merge as the decode, online.
+ * No on-read patch here: on this path the patches were materialised by kam_relocate_patch / kam_admit.
+ * Requires a bf16 MHA / GQA pool, head_dim 64 or 128 rotated over the whole head; else KAM_ERR_UNSUPPORTED.
+ * Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+kam_status kam_paged_prefill_merge(kam_ctx *ctx, const void *q, const kam_pool *pool, const int32_t *block_tables,
+                                   int32_t max_pages, const int32_t *chunk_starts, const int64_t *chunk_offsets,
+                                   const int32_t *n_chunks, int32_t max_chunks, int32_t layer, int32_t batch,
+                                   int32_t n_q_tokens, int32_t causal, float sm_scale, void *out, float *lse, void *stream);
 /* ---- chunk-parallel decode across GPUs ("the log-sum-exp state merge already used by ... ring/star
  * attention").  When a request's chunks are spread over several GPUs, each rank runs kam_paged_decode_state over the
  * chunks IT holds - same arguments as kam_paged_decode_merge, but the result is the softmax STATE in fp32:

@@ -138,8 +138,8 @@ def attend_on_read_factorized(q, chunks, sm_scale, rope, v_dim=None):
     return lse_merge(np.stack(o), np.stack(l))
 
 
-def attend_prefill_bruteforce(q, chunks, sm_scale, rope, causal=True, v_dim=None):
-    """q [Tq, Hq, D] -> out [Tq, Hq, Dv], lse [Tq, Hq].  Row t = attend_bruteforce(q[t]) over the cached tokens it may see:
+def attend_prefill_bruteforce(q, chunks, sm_scale, rope, causal=True, v_dim=None, rows=None):
+    """q [Tq, Hq, D] -> out [Tq, Hq, Dv], lse [Tq, Hq] (rows: evaluate only these query rows, in this order).  Row t = attend_bruteforce(q[t]) over the cached tokens it may see:
     all N of them (causal=False), or tokens 0 .. N - Tq + t (causal=True: the rows are the last Tq cached tokens, each
     seeing the recalled context, the appended tokens before it, and itself).  A row that sees nothing (Tq > N, its index
     before the first cached token) gives out = 0, lse = -inf."""
@@ -147,7 +147,7 @@ def attend_prefill_bruteforce(q, chunks, sm_scale, rope, causal=True, v_dim=None
     Tq = q.shape[0]
     N = sum(c["k"].shape[0] for c in chunks)
     outs, lses = [], []
-    for t in range(Tq):
+    for t in (range(Tq) if rows is None else rows):
         n_vis = N if not causal else N - Tq + t + 1
         vis, left = [], max(n_vis, 0)
         for c in chunks:                                      # the visible prefix, chunk by chunk (a chunk may be cut)

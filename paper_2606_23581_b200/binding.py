@@ -85,6 +85,7 @@ SIGNATURES = {
     "kam_paged_decode_merge": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
                                      vp, vp, vp]),
     "kam_paged_decode_plan": (i32, [vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, i32, i32, vp]),
+    "kam_paged_prefill_merge": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, i32, i32, i32, i32, C.c_float, vp, vp, vp]),
     "kam_decode_set_max_patch_rank": (i32, [vp, i32]),
     "kam_paged_decode_state": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32, C.c_float,
                                      vp, vp, vp]),
@@ -321,6 +322,16 @@ class Context:
         _check(lib().kam_paged_decode_plan(self.h, C.byref(pool.c) if pool else None, _ptr(block_tables), max_pages,
                                            _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks), max_chunks,
                                            int(bool(has_patches)), batch, _stream_ptr(stream)), self.h)
+
+    def kam_paged_prefill_merge(self, q, block_tables, chunk_starts, chunk_offsets, n_chunks, layer, causal, sm_scale, out, lse,
+                                pool=None, stream=None):
+        """q, out: [batch, n_q_tokens, Hq, D] bf16; lse [batch, n_q_tokens, Hq] f32."""
+        batch, max_pages = block_tables.shape
+        max_chunks = chunk_starts.shape[1] - 1
+        _check(lib().kam_paged_prefill_merge(self.h, _ptr(q), C.byref(pool.c) if pool else None, _ptr(block_tables), max_pages,
+                                             _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks), max_chunks, int(layer), batch,
+                                             int(q.shape[1]), int(bool(causal)), float(sm_scale), _ptr(out), _ptr(lse),
+                                             _stream_ptr(stream)), self.h)
 
     def kam_paged_decode_state(self, q, block_tables, chunk_starts, chunk_offsets, n_chunks, layer, sm_scale, o_state,
                                lse_state, patches=None, pool=None, stream=None):

@@ -378,6 +378,40 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   return KAM_OK;
 }
 
+// The readout for a block of query rows: arithmetic in prefill_kernel.cu.
+kam_status kam_paged_prefill_merge(kam_ctx* c, const void* q, const kam_pool* pool, const int32_t* block_tables, int32_t max_pages,
+                                   const int32_t* chunk_starts, const int64_t* chunk_offsets, const int32_t* n_chunks,
+                                   int32_t max_chunks, int32_t layer, int32_t batch, int32_t n_q_tokens, int32_t causal,
+                                   float sm_scale, void* out, float* lse, void* stream) {
+  if (!c) return KAM_ERR_INVALID_ARG;
+  kam_status s = check_pool(c, &pool);
+  if (s != KAM_OK) return s;
+  if (!q || !block_tables || !chunk_starts || !n_chunks || !out || !lse) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_prefill_merge: NULL argument");
+  if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_prefill_merge: q and out must be 16-byte aligned");
+  const kam_layout& L = c->lay;
+  if (layer < 0 || layer >= L.n_layers) return fail(c, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, L.n_layers);
+  if (batch < 0 || n_q_tokens < 0 || max_pages < 1 || max_chunks < 1 || (causal != 0 && causal != 1))
+    return fail(c, KAM_ERR_INVALID_ARG, "kam_paged_prefill_merge: bad batch / n_q_tokens / max_pages / max_chunks / causal");
+  if (batch > 65535 || L.n_kv_heads > 65535) return fail(c, KAM_ERR_UNSUPPORTED, "kam_paged_prefill_merge: batch or KV heads beyond 65535");
+  if (batch == 0 || n_q_tokens == 0) return KAM_OK;
+  if (L.elem_dtype != KAM_BF16 || !L.has_v || (L.row_dim != 64 && L.row_dim != 128) || L.rope_off != 0 || L.rope_dim != L.row_dim)
+    return fail(c, KAM_ERR_UNSUPPORTED, "kam_paged_prefill_merge covers bf16 MHA / GQA pools with head_dim 64 or 128 rotated over the whole head");
+  if (!c->cuda_ok) return fail(c, KAM_ERR_CUDA, "no CUDA device: libkamera has no CPU fallback");
+  PrefillParams p{};
+  p.q = q; p.out = out; p.lse = lse; p.pool_k_layers = pool->k_layers; p.pool_v_layers = pool->v_layers;
+  p.block_tables = block_tables; p.chunk_starts = chunk_starts; p.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets);
+  p.n_chunks = n_chunks; p.inv_freq = c->d_inv_freq;
+  p.layer = layer; p.batch = batch; p.Tq = n_q_tokens; p.Hq = L.n_q_heads; p.H = L.n_kv_heads; p.G = L.n_q_heads / L.n_kv_heads;
+  p.P = L.page_size; p.P_shift = -1;
+  for (int sft = 0; sft < 31; ++sft) if ((1 << sft) == p.P) p.P_shift = sft;
+  p.max_pages = max_pages; p.max_chunks = max_chunks; p.causal = causal; p.rope_style = L.rope_style; p.sm_scale = sm_scale;
+  launch_prefill(p, L.row_dim, static_cast<cudaStream_t>(stream));
+  ++c->kernels_launched;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(c, e, "kam_paged_prefill_kernel launch");
+  return KAM_OK;
+}
+
 kam_status kam_paged_decode_merge_host(kam_ctx* c, const void* q_host, const kam_pool* pool, const int32_t* block_tables,
                                        int32_t max_pages, const int32_t* chunk_starts, const int64_t* chunk_offsets,
                                        const int32_t* n_chunks, int32_t max_chunks, const kam_patch_ref* patches,

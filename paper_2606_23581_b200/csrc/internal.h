@@ -251,6 +251,23 @@ constexpr int kMlaHeads = 16;              // query heads per work unit (two 8-w
 int mla_ts_smem_bytes(int kt);             // kt: rank tiles of the on-read patch the instantiation carries (0, 1, 2, 4)
 void launch_mla_ts_decode(const DecodeGeom& g, const DecodeParams& p, bool pdl, cudaStream_t st);
 
+// ---------------------------------------------------------------- multi-query readout (prefill_kernel.cu)
+struct PrefillParams {
+  const void* q;                 // [B][Tq][Hq][D] bf16
+  void* out;                     // [B][Tq][Hq][D] bf16
+  float* lse;                    // [B][Tq][Hq]
+  void* const* pool_k_layers;    // device arrays of per-layer page bases
+  void* const* pool_v_layers;
+  const int32_t* block_tables;   // [B][max_pages]
+  const int32_t* chunk_starts;   // [B][max_chunks + 1]
+  const long long* chunk_offsets;  // [B][max_chunks] or nullptr
+  const int32_t* n_chunks;       // [B]
+  const double* inv_freq;        // [D / 2]
+  int32_t layer, batch, Tq, Hq, H, G, P, P_shift, max_pages, max_chunks, causal, rope_style;
+  float sm_scale;
+};
+void launch_prefill(const PrefillParams& p, int D, cudaStream_t st);
+
 // ---------------------------------------------------------------- form_patch (compile side, form_patch.cu)
 struct FormPatchParams {
   const void* const* cond;       // device array [L] -> KV(B|A) rows [T][H][D] bf16, at the target position

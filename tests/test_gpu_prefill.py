@@ -1,0 +1,121 @@
+"""GPU parity of kam_paged_prefill_merge (the P:44 readout for a block of query rows over relocated chunks)
+against oracle.attention.attend_prefill_bruteforce.  Bar as for the decode (BASELINE.json; reading R-11): per (row, head)
+max-abs <= 2e-2, ||g-o||inf / ||o||inf <= 1e-2, |lse_g - lse_o| <= 1e-3.  The oracle reads the SAME pool bits the kernel reads.
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_23581_b200 as kam
+from oracle import attention as att
+from oracle import reuse
+from paper_2606_23581_b200 import binding as B
+from synth import CONFIGS, make_block_table
+from tests import parity as par
+from tests.test_gpu_decode import _fill_pool, check_attention
+
+pytestmark = pytest.mark.gpu
+
+
+def _run(cfg, lens, deltas, Tq, causal, seed, style=reuse.HALF, rows=None, layer=0, L=1):
+    """lens[b]: chunk lengths of request b (its cached tokens, the appended block included when causal); every request gets a
+    block of Tq query rows.  rows: the query rows the oracle evaluates (None = all)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    P, D, Hq = cfg.page_size, cfg.row_dim, cfg.n_q_heads
+    batch = len(lens)
+    max_chunks = max(1, max(len(x) for x in lens))
+    max_pages = max(1, max((sum(x) + P - 1) // P for x in lens))
+    num_pages = batch * max_pages + 3
+    pool = _fill_pool(cfg, L, num_pages, seed)
+    ctx = kam.Context(par.layout_of(cfg, L, B.KAM_ROPE_HALF if style == reuse.HALF else B.KAM_ROPE_INTERLEAVED), pool)
+    perm = make_block_table(rng, batch * max_pages, num_pages).reshape(batch, max_pages)
+    starts = np.zeros((batch, max_chunks + 1), np.int32)
+    offs = np.zeros((batch, max_chunks), np.int64)
+    base = rng.integers(0, 40, size=batch)
+    for b in range(batch):
+        starts[b, 0] = base[b]
+        for c, n in enumerate(lens[b]):
+            starts[b, c + 1] = starts[b, c] + n
+            offs[b, c] = deltas[b][c]
+        starts[b, len(lens[b]) + 1:] = starts[b, len(lens[b])]
+    ncs = torch.tensor([len(x) for x in lens], dtype=torch.int32, device="cuda")
+    q = torch.from_numpy(rng.standard_normal((batch, Tq, Hq, D), dtype=np.float32)).to(torch.bfloat16)
+    out = torch.full((batch, Tq, Hq, D), 7.0, dtype=torch.bfloat16, device="cuda")
+    lse = torch.full((batch, Tq, Hq), 7.0, dtype=torch.float32, device="cuda")
+    scale = D ** -0.5
+    args = (q.cuda(), torch.from_numpy(perm).cuda(), torch.from_numpy(starts).cuda(), torch.from_numpy(offs).cuda(), ncs, layer, causal, scale)
+    ctx.kam_paged_prefill_merge(*args, out, lse)
+    out2, lse2 = torch.empty_like(out), torch.empty_like(lse)
+    ctx.kam_paged_prefill_merge(*args, out2, lse2)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2) and torch.equal(lse, lse2)            # run-to-run deterministic
+    assert ctx.kam_get_stats()["kernels_launched"] == 2
+    out_g, lse_g = par.to_f64(out), par.to_f64(lse)
+    worst = (0.0, 0.0)
+    sel = list(range(Tq)) if rows is None else rows
+    for b in range(batch):
+        chunks, t0 = [], 0
+        for c, n in enumerate(lens[b]):
+            chunks.append({"k": par.pool_rows(pool.k_layers[layer], perm[b], t0, n), "v": par.pool_rows(pool.v_layers[layer], perm[b], t0, n),
+                           "delta": int(deltas[b][c])})
+            t0 += n
+        if not chunks:
+            chunks = [{"k": np.zeros((0, cfg.n_kv_heads, D)), "v": np.zeros((0, cfg.n_kv_heads, D))}]
+        o, l = att.attend_prefill_bruteforce(par.to_f64(q[b]), chunks, scale, par.rope_kw(cfg, style), causal=bool(causal), rows=sel)
+        for i, t in enumerate(sel):
+            r = check_attention(out_g[b, t], lse_g[b, t], o[i], l[i], "request %d row %d" % (b, t))
+            worst = (max(worst[0], r[0]), max(worst[1], r[1]))
+    ctx.close()
+    return worst
+
+
+def test_config2_gqa_64_rows_over_relocated_chunks():
+    """GQA 28 / 4: the appended 64-token turn (last chunk, offset 0) over recalled chunks read at pending offsets; ragged chunk
+    lengths, tiles cut by chunk ends, 64 x 7 = 448 rows per KV head = 7 row tiles."""
+    cfg = CONFIGS[2]
+    _run(cfg, [[300, 1024, 37, 64], [100, 64]], [[3100, -77, 5, 0], [0, 0]], 64, 1, 501)
+
+
+def test_config2_gqa_512_rows_sampled():
+    """A 512-token text turn (P:105 TTFT path) over three recalled chunks; the oracle evaluates 40 of the 512 rows."""
+    cfg = CONFIGS[2]
+    rows = sorted(set([0, 1, 63, 64, 255, 256, 510, 511] + list(range(5, 512, 16))))
+    _run(cfg, [[1024, 700, 200, 512]], [[-20000, 1, 32767, 0]], 512, 1, 502, rows=rows)
+
+
+def test_config4_mha_64_and_512_rows():
+    """MHA (G = 1: one row tile per 64 tokens and head), config 4's window + prefix shape scaled to 8 heads."""
+    cfg = CONFIGS[4].scaled(n_layers=2, n_q_heads=8, n_kv_heads=8)
+    _run(cfg, [[512, 1280, 64]], [[0, -1280, 0]], 64, 1, 503, layer=1, L=2)
+    _run(cfg, [[160, 1280, 512]], [[0, 4096, 0]], 512, 1, 504, rows=[0, 7, 100, 300, 511], layer=0, L=2)
+
+
+def test_not_causal_every_row_is_the_decode_readout():
+    cfg = CONFIGS[2].scaled(n_q_heads=8, n_kv_heads=4)
+    _run(cfg, [[130, 70], [16]], [[9, -9], [123]], 24, 0, 505)
+
+
+def test_edge_cases():
+    """Rows x G not a multiple of the 64-row tile; more query rows than cached tokens (the first rows see nothing: out = 0,
+    lse = -inf); a request with no cached tokens; single-token chunks; an empty chunk in the middle."""
+    cfg = CONFIGS[2].scaled(n_q_heads=12, n_kv_heads=4)           # G = 3
+    _run(cfg, [[5, 0, 1, 30], [3], []], [[7, 0, -1, 0], [0], []], 10, 1, 506)
+    _run(cfg, [[17]], [[0]], 1, 1, 507)                          # one query row = a decode step
+
+
+def test_head_dim_64_and_interleaved_pairs():
+    cfg = CONFIGS[1].scaled(elem_dtype="bf16", factor_dtype="bf16", n_layers=1)      # MHA 4 heads, head_dim 64
+    _run(cfg, [[200, 64]], [[1000, 0]], 64, 1, 508)
+    _run(CONFIGS[2].scaled(n_q_heads=8, n_kv_heads=4), [[90, 40]], [[-555, 0]], 40, 1, 509, style=reuse.INTERLEAVED)
+
+
+def test_unsupported_and_invalid_arguments():
+    cfg = CONFIGS[3]                                              # MLA: not covered by the multi-query kernel
+    pool = kam.Pool([torch.zeros((4, cfg.page_size, 1, cfg.row_dim), dtype=torch.bfloat16, device="cuda")], None)
+    ctx = kam.Context(par.layout_of(cfg, 1), pool)
+    z = lambda *s, dt=torch.int32: torch.zeros(s, dtype=dt, device="cuda")
+    q = torch.zeros((1, 4, cfg.n_q_heads, cfg.row_dim), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(kam.KameraError) as e:
+        ctx.kam_paged_prefill_merge(q, z(1, 4), z(1, 2), None, z(1), 0, 1, 0.1, torch.zeros_like(q), z(1, 4, cfg.n_q_heads, dt=torch.float32))
+    assert e.value.status == B.KAM_ERR_UNSUPPORTED and ctx.kam_get_stats()["kernels_launched"] == 0
+    ctx.close()
