@@ -129,6 +129,15 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------------- the workload
+def tensor_peak():
+    """Dense bf16 tensor peak in TFLOP/s: the sustained cuBLAS figure of MEASURED_PEAKS.json, else the profiling guide's nominal."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d.get("bf16_tflops_sustained") or d.get("bf16_tflops") or 2250.0)
+    return 2250.0
+
+
 class DeviceClock:
     """Phase boundaries as CUDA events on the launching stream (torch's current stream, which the binding passes on)."""
 
@@ -566,6 +575,37 @@ def extras(wl, device, peak):
         out[name] = entry(nbytes, ms, bytes="K + V once", what="stateless call = plan + kam_paged_decode_kernel + merge; %d q / %d kv heads" % (cx.n_q_heads, Hx))
         ctxx.close()
         del poolx, ctxx, btx, qx, ox
+
+    # ---- f4: chunked prefill - a 512-token text turn of 8 requests over their 8192-token recalled windows (config 2's shape,
+    # the TTFT path of P:105 / P:349), causal over the appended tokens, recalled chunks read at a pending offset
+    nbp, Tq = 8, 512
+    Lp = 2
+    pprp = (n * T + Tq) // P
+    poolp = kam.Pool([rnd((nbp * pprp, P, H, D)) for _ in range(Lp)], [rnd((nbp * pprp, P, H, D)) for _ in range(Lp)])
+    ctxp = kam.Context(kam.make_layout(B.KAM_GQA, Lp, cfg.n_q_heads, H, D, 0, D, True, P, cfg.theta), poolp)
+    btp = torch.randperm(nbp * pprp, device=device, dtype=torch.int32).reshape(nbp, pprp)
+    stp = torch.tensor([[c * T for c in range(n + 1)] + [n * T + Tq]] * nbp, dtype=torch.int32, device=device)
+    ofp = torch.tensor([[4321] * n + [0]] * nbp, dtype=torch.int64, device=device)
+    ncp = torch.full((nbp,), n + 1, dtype=torch.int32, device=device)
+    qp = rnd((nbp, Tq, cfg.n_q_heads, D))
+    op, lp = torch.zeros_like(qp), torch.zeros((nbp, Tq, cfg.n_q_heads), dtype=torch.float32, device=device)
+    it = [0]
+
+    def launch():
+        it[0] += 1
+        ctxp.kam_paged_prefill_merge(qp, btp, stp, ofp, ncp, it[0] % Lp, 1, wl.sm_scale, op, lp)
+    ms = _time_ms(torch, launch, 6)
+    Nkv = n * T + Tq
+    flops = 4.0 * nbp * cfg.n_q_heads * D * (Tq * (Nkv - Tq) + Tq * (Tq + 1) / 2)          # visible (row, token) pairs x 4 D
+    flops_issued = flops * 2 * (n * T) / Nkv + flops * Tq / Nkv                               # rotated chunks run the q~ lo products too
+    tf_peak = tensor_peak()
+    out["prefill_config2_shape_b8_512rows_over_8192"] = {
+        "ms": ms, "tflops": flops / ms / 1e9, "frac_of_dense_bf16_peak": flops / ms / 1e9 / tf_peak, "tflops_issued": flops_issued / ms / 1e9,
+        "tensor_peak_tflops": tf_peak, "GB/s": nbp * Nkv * H * 2 * D * 2 / ms / 1e6, "frac_of_hbm_peak": nbp * Nkv * H * 2 * D * 2 / ms / 1e6 / peak,
+        "bound": "tensor", "what": "kam_paged_prefill_kernel<128> (mma.sync m16n8k16, FlashAttention-2 shape); flops = 4 D per visible (row, token) "
+        "pair; tflops_issued counts the second (lo) QK^T product of chunks read at a pending offset; bytes = K + V once per request"}
+    ctxp.close()
+    del poolp, ctxp, btp, qp, op
 
     # ---- MLA (config 3 shape): relocate+patch - 4 chunks x 27 layers, and config 3's stated launch (every ordering of the 4
     # cached chunks = 96 relocations, one launch); absorbed decode, batch 64 x 8192 tokens, without and with the on-read patch

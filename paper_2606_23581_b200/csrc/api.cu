@@ -362,14 +362,14 @@ kam_status run_reloc(kam_ctx* c, const kam_pool* pool, const std::vector<HostRel
     p.total_tiles = acc; p.n_descs = n; p.inv_freq = c->d_inv_freq;
     p.num_pages = pool->num_pages; p.err = c->d_err;
     const int grid = (int)std::min<long long>(c->sm_count, acc);
-    std::unique_ptr<RelocPages> pg(new (std::nothrow) RelocPages());
-    if (!pg) return fail(c, KAM_ERR_STATE, "out of host memory");
-    pg->mirror_dst = nullptr; pg->n = 0;
+    std::unique_ptr<RelocPages> pg;
     if (inline_pages) {
+      pg.reset(new (std::nothrow) RelocPages());
+      if (!pg) return fail(c, KAM_ERR_STATE, "out of host memory");
       memcpy(pg->pages, ap->sg->host, (size_t)ap->n * 4);
       pg->mirror_dst = ap->d_mirror; pg->n = ap->n;
     }
-    launch_relocate_fast(g, p, *inl, *pg, grid, c->opt.reloc_pdl != 0, st);
+    launch_relocate_fast(g, p, *inl, pg.get(), grid, c->opt.reloc_pdl != 0, st);
   } else {
     GenericParams p{};
     p.descs = d_descs; p.pool_k = pool->k_layers; p.pool_v = pool->v_layers;

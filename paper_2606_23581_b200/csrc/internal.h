@@ -132,7 +132,7 @@ struct GenericParams {
   double theta;
 };
 
-void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages& pages, int grid, bool pdl, cudaStream_t st);
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages* pages /* or nullptr */, int grid, bool pdl, cudaStream_t st);
 void launch_relocate_generic(const GenericParams& p, int max_tokens, cudaStream_t st);
 
 // ---------------------------------------------------------------- decode

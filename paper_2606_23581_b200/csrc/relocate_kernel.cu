@@ -232,9 +232,9 @@ __device__ __forceinline__ void slab_run(const SlabArgs& s, int rope, uint32_t u
 //   in-place x2  (a survivor inside a K+V launch)   : 2 * TT tokens of K; the second half lands in the V area, so a slide's
 //                                                     survivors keep a full stage of bytes in flight beside the recalled chunk
 //   kv-split     (ranks 48 / 64)                    : TT tokens of K or of V in the K area, its U in the U_k area
-__global__ void __launch_bounds__(kRelocThreads, 1)
-kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_constant__ RelocParams p, const __grid_constant__ RelocInline inl,
-                          const __grid_constant__ RelocPages pages) {
+namespace {
+// pages: the page list of a chunk being admitted to a window, or nullptr (the stateless calls: their kernel has no such parameter)
+__device__ __forceinline__ void relocate_body(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages* pages) {
   extern __shared__ __align__(128) uint8_t smem[];
   uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem);
   uint64_t* empty_bar = full_bar + g.n_stages;
@@ -271,8 +271,8 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   const long long* tile_prefix = p.descs ? p.tile_prefix : inl.prefix;
   const long long* w_prefix = p.descs ? p.w_prefix : inl.wprefix;
   // the page list of a chunk just admitted to a window: CTA 0 publishes it to the device mirror (read by later launches only)
-  if (pages.mirror_dst && blockIdx.x == 0)
-    for (int i = threadIdx.x; i < pages.n; i += blockDim.x) pages.mirror_dst[i] = pages.pages[i];
+  if (pages && blockIdx.x == 0)
+    for (int i = threadIdx.x; i < pages->n; i += blockDim.x) pages->mirror_dst[i] = pages->pages[i];
   // CTA i owns the tiles whose cumulative WEIGHT falls in [W i / n, W (i+1) / n): tiles of one chunk weigh the same, tiles of
   // different chunks do not (a survivor rotated in place moves K only and runs no MMA; a recalled chunk moves K, V, U and runs
   // the patch) - equal COUNTS left the CTAs of a slide 13 % apart (profiles/ncu_slide_r02.md)
@@ -309,7 +309,7 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
         cur_d = w.d; cur_l = w.l; cur_kv = w.kv;
         const RelocDescDev& desc = descs[w.d];
         flags = desc.flags; m = desc.rank_l[w.l]; dst0 = static_cast<int>(desc.dst_token_start);
-        bt = (flags & FLAG_INLINE_PAGES) ? pages.pages : desc.block_table;
+        bt = (pages && (flags & FLAG_INLINE_PAGES)) ? pages->pages : desc.block_table;
         u_tok_stride = desc.u_token_stride; u_head_stride = desc.u_head_stride;
         const bool inplace = flags & FLAG_INPLACE;
         dbl = inplace && g.nkv == 2 && !split;
@@ -584,10 +584,24 @@ kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
   }
 }
 
-void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages& pages, int grid, bool pdl, cudaStream_t st) {
+}  // namespace
+
+__global__ void __launch_bounds__(kRelocThreads, 1)
+kam_relocate_patch_kernel(const __grid_constant__ RelocGeom g, const __grid_constant__ RelocParams p, const __grid_constant__ RelocInline inl) {
+  relocate_body(g, p, inl, nullptr);
+}
+// the same kernel with the admitted chunk's page list as a fourth parameter (kam_admit / kam_slide)
+__global__ void __launch_bounds__(kRelocThreads, 1)
+kam_relocate_admit_kernel(const __grid_constant__ RelocGeom g, const __grid_constant__ RelocParams p, const __grid_constant__ RelocInline inl,
+                          const __grid_constant__ RelocPages pages) {
+  relocate_body(g, p, inl, &pages);
+}
+
+void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages* pages, int grid, bool pdl, cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(kam_relocate_patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaFuncSetAttribute(kam_relocate_admit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_set = true;
   }
   cudaLaunchConfig_t cfg{};
@@ -596,7 +610,8 @@ void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocI
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, kam_relocate_patch_kernel, g, p, inl, pages);
+  if (pages) cudaLaunchKernelEx(&cfg, kam_relocate_admit_kernel, g, p, inl, *pages);
+  else cudaLaunchKernelEx(&cfg, kam_relocate_patch_kernel, g, p, inl);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
