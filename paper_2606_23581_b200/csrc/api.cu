@@ -154,8 +154,11 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
     }
     return false;
   };
+  // widest slice tried first: up to 8 heads (a whole 8-head row is one contiguous copy per tile; with W of 8 heads only the
+  // kv-split form leaves room for three stages), else the largest divisor of H up to 4
+  const int hg_cap = c->opt.reloc_hg_cap;
   int hg_max = 1;
-  for (int HG = std::min(g.H, 4); HG >= 1; --HG) if (g.H % HG == 0) { hg_max = HG; break; }
+  for (int HG = std::min(g.H, hg_cap); HG >= 1; --HG) if (g.H % HG == 0 && HG * c->blocks_per_head <= kMaxColBlocks) { hg_max = HG; break; }
   const bool may_split = g.nkv == 2 && c->opt.reloc_kv_split != 0, must_split = g.nkv == 2 && c->opt.reloc_kv_split == 2;
   RelocGeom t{};
   if (hg_force > 0) {
@@ -164,8 +167,12 @@ bool build_reloc_geom(const kam_ctx* c, int max_rank, bool inplace_only, RelocGe
     return false;
   }
   // 1. the widest slice with three stages, plain; 2. the same, kv-split
-  if (!must_split && candidate(false, hg_max, &t) && t.n_stages >= 3) { *out = t; return true; }
-  if (may_split && candidate(true, hg_max, &t) && (t.n_stages >= 3 || must_split)) { *out = t; return true; }
+  for (int HG = hg_max; HG >= std::min(hg_max, 4); --HG) {
+    if (g.H % HG) continue;
+    if (!must_split && candidate(false, HG, &t) && t.n_stages >= 3) { *out = t; return true; }
+    if (may_split && candidate(true, HG, &t) && (t.n_stages >= 3 || must_split)) { *out = t; return true; }
+  }
+  hg_max = std::min(hg_max, 4);
   // 3. round 1's order: narrower slices, three stages or two big ones (>= 96 KB in flight: measured at rank 64 before the
   //    kv-split form existed - two 54 KB stages of two heads 4.9 TB/s, three 60 KB stages of one-head slices 4.0 TB/s)
   RelocGeom best{}; bool have = false;
@@ -856,6 +863,7 @@ kam_status kam_set_option(kam_ctx* c, const char* key, int64_t value) {
       {"decode_pdl", &o.use_pdl, 0, 1},              {"decode_tma", &o.dec_tma, 0, 1},
       {"host_copy_overlap", &o.host_copy_overlap, 0, 1}, {"host_entries_sync", &o.host_sync, 0, 1},
       {"reloc_patch_cost_pct", &o.reloc_patch_cost_pct, 50, 200}, {"reloc_pdl", &o.reloc_pdl, 0, 1},
+      {"reloc_head_group_cap", &o.reloc_hg_cap, 1, 8},
   };
   for (const Opt& op : opts)
     if (strcmp(op.name, key) == 0) {

@@ -27,6 +27,7 @@ constexpr int kMaxTmapSets = 8;
 struct Options {
   int reloc_stages = 0;        // "reloc_stages": pipeline stages of the relocate kernel (0 = automatic: 3)
   int reloc_hg = 0;            // "reloc_head_group": KV heads per slice (0 = automatic)
+  int reloc_hg_cap = 4;        // "reloc_head_group_cap": widest slice the automatic choice tries (8-head slices measured within 2 % either way)
   int reloc_kv_split = 1;      // "reloc_kv_split": 1 = automatic (when W_k + W_v crowd out the third stage), 0 = never, 2 = always
   int reloc_contig = 1;        // "reloc_contig": one unpadded copy per tile when a slice is a whole token row
   int reloc_rb = 0;            // "reloc_row_blocks": 16-token row blocks per tile (0 = automatic)
