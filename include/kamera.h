@@ -155,7 +155,7 @@ const char *kam_version(void);
  *   reloc_stages 0..8 (0 = automatic)   reloc_head_group 0..4   reloc_head_group_cap 1..8   reloc_kv_split 0 never / 1 automatic / 2 always
  *   reloc_contig 0/1   reloc_row_blocks 0..4   reloc_evict_first 0/1   reloc_patch_cost_pct 50..200   reloc_pdl 0/1
  *   decode_ctas_per_sm 0..8   decode_boxes 0..16
- *   decode_pdl 0/1   decode_tma 0/1   host_copy_overlap 0/1   host_entries_sync 0/1
+ *   decode_pdl 0/1   decode_tma 0/1   prefill_tcgen05 0/1   host_copy_overlap 0/1   host_entries_sync 0/1
  * Setting any of them drops cached decode plans; CUDA graphs captured over this context's calls must be re-captured.
  * Errors: INVALID_ARG (unknown key, value out of range). */
 kam_status kam_set_option(kam_ctx *ctx, const char *key, int64_t value);

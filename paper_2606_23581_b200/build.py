@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkamera.so")
-SOURCES = ["api.cu", "decode_api.cu", "relocate_kernel.cu", "decode_kernel.cu", "decode_mla_ts_kernel.cu", "prefill_kernel.cu", "form_patch.cu", "window.cpp"]
+SOURCES = ["api.cu", "decode_api.cu", "relocate_kernel.cu", "decode_kernel.cu", "decode_mla_ts_kernel.cu", "prefill_kernel.cu", "prefill_tc_kernel.cu", "form_patch.cu", "window.cpp"]
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "--expt-relaxed-constexpr", "-shared", "--threads", "0"]
 

@@ -863,7 +863,7 @@ kam_status kam_set_option(kam_ctx* c, const char* key, int64_t value) {
       {"decode_pdl", &o.use_pdl, 0, 1},              {"decode_tma", &o.dec_tma, 0, 1},
       {"host_copy_overlap", &o.host_copy_overlap, 0, 1}, {"host_entries_sync", &o.host_sync, 0, 1},
       {"reloc_patch_cost_pct", &o.reloc_patch_cost_pct, 50, 200}, {"reloc_pdl", &o.reloc_pdl, 0, 1},
-      {"reloc_head_group_cap", &o.reloc_hg_cap, 1, 8},
+      {"reloc_head_group_cap", &o.reloc_hg_cap, 1, 8}, {"prefill_tcgen05", &o.prefill_tc, 0, 1},
   };
   for (const Opt& op : opts)
     if (strcmp(op.name, key) == 0) {

@@ -38,6 +38,7 @@ struct Options {
   int dec_boxes = 0;           // "decode_boxes": ring depth of the decode kernel (0 = automatic)
   int use_pdl = 1;             // "decode_pdl": programmatic dependent launch between plan, decode and merge
   int dec_tma = 1;             // "decode_tma": pool pages arrive as TMA tensor-map boxes (0: per-token bulk copies)
+  int prefill_tc = 1;          // "prefill_tcgen05": the multi-query readout runs on tcgen05 / tensor memory (0: the mma.sync kernel)
   int host_copy_overlap = 1;   // "host_copy_overlap": kam_relocate_patch_host copies chunk c+1 under the kernel of chunk c
   int host_sync = 0;           // "host_entries_sync": kam_paged_decode_merge_host ends with a stream synchronise
 };

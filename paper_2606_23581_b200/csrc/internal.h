@@ -266,7 +266,8 @@ struct PrefillParams {
   int32_t layer, batch, Tq, Hq, H, G, P, P_shift, max_pages, max_chunks, causal, rope_style;
   float sm_scale;
 };
-void launch_prefill(const PrefillParams& p, int D, cudaStream_t st);
+void launch_prefill(const PrefillParams& p, int D, cudaStream_t st);        // mma.sync formulation (prefill_kernel.cu)
+void launch_prefill_tc(const PrefillParams& p, int D, cudaStream_t st);     // tcgen05 / tensor-memory formulation (prefill_tc_kernel.cu)
 
 // ---------------------------------------------------------------- form_patch (compile side, form_patch.cu)
 struct FormPatchParams {
