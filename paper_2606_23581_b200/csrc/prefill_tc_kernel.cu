@@ -35,7 +35,6 @@ constexpr int kTcTile = 64;                // cached tokens per tile
 constexpr int kTcStages = 4;
 constexpr int kTcLoaders = 4;              // loader warps: each takes a quarter of a tile's rows
 constexpr int kTcThreads = (5 + kTcLoaders) * 32;   // 4 softmax warps + MMA warp + loader warps
-constexpr int kTcLag = 2;                  // tiles a loader keeps in flight beyond the one it publishes (<= kTcStages - 2, see below)
 enum : int { BAR_KV_FULL = 0, BAR_KV_EMPTY = kTcStages, BAR_S_FULL = 2 * kTcStages /* x2 */, BAR_P_FULL = 2 * kTcStages + 2, BAR_O_DONE = 2 * kTcStages + 3,
              BAR_Q_READY = 2 * kTcStages + 4, BAR_COUNT = 2 * kTcStages + 5 };
 
@@ -155,7 +154,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
   bool more = cur.enter(0);
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < kTcStages; ++i) { mbar_init(&bars[BAR_KV_FULL + i], kTcLoaders); mbar_init(&bars[BAR_KV_EMPTY + i], 1); }
+    for (int i = 0; i < kTcStages; ++i) { mbar_init(&bars[BAR_KV_FULL + i], kTcLoaders * 32); mbar_init(&bars[BAR_KV_EMPTY + i], 1); }
     mbar_init(&bars[BAR_S_FULL], 1); mbar_init(&bars[BAR_S_FULL + 1], 1);
     mbar_init(&bars[BAR_P_FULL], 128); mbar_init(&bars[BAR_O_DONE], 1); mbar_init(&bars[BAR_Q_READY], 128);
     mbar_fence_init();
@@ -182,13 +181,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
     constexpr int RPW = kTcTile / kTcLoaders;               // rows per loader warp
     const int lc = lane % CPR, lr0 = (warp - 5) * RPW + lane / CPR;
     const uint32_t dst_c = static_cast<uint32_t>((lc >> 3) * (kTcTile * 128));       // the chunk's 64-column block
-    int issued = 0, signalled = 0;
-    auto signal_upto = [&](int n) {                         // tiles [signalled, n) have landed: publish them
-      fence_proxy_async();                                  // cp.async wrote through the generic proxy; tcgen05.mma reads through the async one
-      __syncwarp();
-      if (lane == 0) for (int t = signalled; t < n; ++t) mbar_arrive(&bars[BAR_KV_FULL + t % kTcStages]);
-      signalled = n;
-    };
+    int issued = 0;
     while (more) {
       const int st = issued % kTcStages;
       if (issued >= kTcStages) mbar_wait(&bars[BAR_KV_EMPTY + st], ((issued / kTcStages) - 1) & 1);
@@ -207,17 +200,12 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
         cp_async_16z(kd + d, pool_k + src, valid);
         cp_async_16z(vd + d, pool_v + src, valid);
       }
-      asm volatile("cp.async.commit_group;" ::: "memory");
+      // the tile's barrier hears from this thread when ITS copies have landed (no wait here: up to kTcStages tiles stay in flight)
+      asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(&bars[BAR_KV_FULL + st])) : "memory");
       ++issued;
-      // a loader holds back the last kTcLag tiles it issued (they are in flight).  The MMA warp issues QK^T of tile t + 1 BEFORE
-      // PV of tile t, and the stage of tile t + kTcStages is only free after that PV: holding back more than kTcStages - 2 tiles
-      // would close that cycle
-      static_assert(kTcLag <= kTcStages - 2, "loader lag");
-      if (issued - signalled > kTcLag) { asm volatile("cp.async.wait_group %0;" ::"n"(kTcLag) : "memory"); signal_upto(issued - kTcLag); }
       more = cur.next();
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    signal_upto(issued);
+    asm volatile("cp.async.wait_all;" ::: "memory");
   } else if (warp == 4) {
     // ================================================================ MMA issuer (lane 0 issues; the warp stays converged for dealloc)
     constexpr uint32_t idesc_qk = tc_idesc(kTcRows, kTcTile, false), idesc_pv = tc_idesc(kTcRows, D, true);
@@ -227,6 +215,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
     auto issue_qk = [&](int t) {
       const int st = t % kTcStages;
       mbar_wait(&bars[BAR_KV_FULL + st], (t / kTcStages) & 1);
+      fence_proxy_async();                                  // the tile was written by cp.async (generic proxy), tcgen05.mma reads through the async proxy
       tcf_after();
       if (lane == 0) {
         const uint32_t kb = sm0 + OFF_KV + st * 2 * KVB;
