@@ -405,7 +405,7 @@ kam_status kam_paged_prefill_merge(kam_ctx* c, const void* q, const kam_pool* po
   p.P = L.page_size; p.P_shift = -1;
   for (int sft = 0; sft < 31; ++sft) if ((1 << sft) == p.P) p.P_shift = sft;
   p.max_pages = max_pages; p.max_chunks = max_chunks; p.causal = causal; p.rope_style = L.rope_style; p.sm_scale = sm_scale;
-  if (c->opt.prefill_tc) launch_prefill_tc(p, L.row_dim, static_cast<cudaStream_t>(stream));
+  if (c->opt.prefill_tc && sm_scale > 0.f) launch_prefill_tc(p, L.row_dim, static_cast<cudaStream_t>(stream));
   else launch_prefill(p, L.row_dim, static_cast<cudaStream_t>(stream));
   ++c->kernels_launched;
   cudaError_t e = cudaGetLastError();

@@ -35,8 +35,8 @@ constexpr int kTcTile = 64;                // cached tokens per tile
 constexpr int kTcStages = 4;
 constexpr int kTcLoaders = 4;              // loader warps: each takes a quarter of a tile's rows
 constexpr int kTcThreads = (5 + kTcLoaders) * 32;   // 4 softmax warps + MMA warp + loader warps
-enum : int { BAR_KV_FULL = 0, BAR_KV_EMPTY = kTcStages, BAR_S_FULL = 2 * kTcStages /* x2 */, BAR_P_FULL = 2 * kTcStages + 2, BAR_O_DONE = 2 * kTcStages + 3,
-             BAR_Q_READY = 2 * kTcStages + 4, BAR_COUNT = 2 * kTcStages + 5 };
+enum : int { BAR_KV_FULL = 0, BAR_KV_EMPTY = kTcStages, BAR_S_FULL = 2 * kTcStages /* x2 */, BAR_P_FULL = 2 * kTcStages + 2 /* x2 */, BAR_O_DONE = 2 * kTcStages + 4,
+             BAR_Q_READY = 2 * kTcStages + 5, BAR_COUNT = 2 * kTcStages + 6 };
 
 __device__ __forceinline__ void tcf_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tcf_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -128,9 +128,9 @@ template <int D>
 __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(const __grid_constant__ PrefillParams p) {
   constexpr int DB = D / 64;                               // 64-column blocks of a row
   constexpr int QBYTES = kTcRows * D * 2;                  // one q~ operand (hi or lo): [DB][128 rows][128 B]
-  constexpr int PBYTES = kTcRows * kTcTile * 2;            // P: [128 rows][128 B]
+  constexpr int PBYTES = kTcRows * kTcTile * 2;            // P: [128 rows][128 B], two buffers
   constexpr int KVB = kTcTile * D * 2;                     // one K (or V) tile: [DB][64 tokens][128 B]
-  constexpr int OFF_Q = 1024, OFF_QLO = OFF_Q + QBYTES, OFF_P = OFF_QLO + QBYTES, OFF_KV = OFF_P + PBYTES;
+  constexpr int OFF_Q = 1024, OFF_QLO = OFF_Q + QBYTES, OFF_P = OFF_QLO + QBYTES, OFF_KV = OFF_P + 2 * PBYTES;
   constexpr uint32_t TM_S = 0, TM_O = 2 * kTcTile, TM_COLS = (TM_O + D <= 256) ? 256 : 512;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
   if (threadIdx.x == 0) {
     for (int i = 0; i < kTcStages; ++i) { mbar_init(&bars[BAR_KV_FULL + i], kTcLoaders * 32); mbar_init(&bars[BAR_KV_EMPTY + i], 1); }
     mbar_init(&bars[BAR_S_FULL], 1); mbar_init(&bars[BAR_S_FULL + 1], 1);
-    mbar_init(&bars[BAR_P_FULL], 128); mbar_init(&bars[BAR_O_DONE], 1); mbar_init(&bars[BAR_Q_READY], 128);
+    mbar_init(&bars[BAR_P_FULL], 128); mbar_init(&bars[BAR_P_FULL + 1], 128); mbar_init(&bars[BAR_O_DONE], 1); mbar_init(&bars[BAR_Q_READY], 128);
     mbar_fence_init();
   }
   if (warp == 4) {                                          // one warp allocates the tensor memory and owns the deallocation
@@ -179,26 +179,35 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
     constexpr int CPR = D / 8;                              // 16-byte chunks per row
     constexpr int RPP = 32 / CPR;                           // rows per pass of the warp (2 at D = 128, 4 at D = 64)
     constexpr int RPW = kTcTile / kTcLoaders;               // rows per loader warp
-    const int lc = lane % CPR, lr0 = (warp - 5) * RPW + lane / CPR;
+    const int lc = lane % CPR;
+    static_assert(RPW == 16, "one slot per lane of a half warp");
     const uint32_t dst_c = static_cast<uint32_t>((lc >> 3) * (kTcTile * 128));       // the chunk's 64-column block
     int issued = 0;
+    const char* kbase = pool_k + head_off + lc * 16;
+    const char* vbase = pool_v + head_off + lc * 16;
+    const int wrow0 = (warp - 5) * RPW;                     // this warp's first row of a tile
     while (more) {
       const int st = issued % kTcStages;
-      if (issued >= kTcStages) mbar_wait(&bars[BAR_KV_EMPTY + st], ((issued / kTcStages) - 1) & 1);
-      const uint32_t kd = sm0 + OFF_KV + st * 2 * KVB, vd = kd + KVB;
-#pragma unroll 4
-      for (int i = 0; i < RPW / RPP; ++i) {
-        const int r = lr0 + i * RPP;
-        const int tok = cur.pos + r;
-        const bool valid = tok < cur.hi;
-        size_t src = 0;
-        if (valid) {
+      // A1 slot mapping, once per row: lane l < RPW maps row wrow0 + l; the copy loop below takes it by shuffle
+      int myslot = -1;
+      {
+        const int tok = cur.pos + wrow0 + (lane & (RPW - 1));
+        if (tok < cur.hi) {
           const int pg = p.P_shift >= 0 ? (tok >> p.P_shift) : tok / p.P;
-          src = (static_cast<size_t>(bt[pg]) * p.P + (tok - pg * p.P)) * tok_bytes + head_off + lc * 16;      // A1 slot mapping
+          myslot = bt[pg] * p.P + (tok - pg * p.P);
         }
-        const uint32_t d = dst_c + sw_chunk(r, lc & 7);
-        cp_async_16z(kd + d, pool_k + src, valid);
-        cp_async_16z(vd + d, pool_v + src, valid);
+      }
+      if (issued >= kTcStages) mbar_wait(&bars[BAR_KV_EMPTY + st], ((issued / kTcStages) - 1) & 1);
+      const uint32_t kd = sm0 + OFF_KV + st * 2 * KVB + dst_c, vd = kd + KVB;
+#pragma unroll
+      for (int i = 0; i < RPW / RPP; ++i) {
+        const int rr = lane / CPR + i * RPP;                  // row inside the warp's RPW rows
+        const int slot = __shfl_sync(0xffffffffu, myslot, rr);
+        const bool valid = slot >= 0;                          // rows beyond the chunk are zero-filled
+        const size_t off = valid ? static_cast<size_t>(slot) * tok_bytes : 0;
+        const uint32_t d = sw_chunk(wrow0 + rr, lc & 7);
+        cp_async_16z(kd + d, kbase + off, valid);
+        cp_async_16z(vd + d, vbase + off, valid);
       }
       // the tile's barrier hears from this thread when ITS copies have landed (no wait here: up to kTcStages tiles stay in flight)
       asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(&bars[BAR_KV_FULL + st])) : "memory");
@@ -209,7 +218,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
   } else if (warp == 4) {
     // ================================================================ MMA issuer (lane 0 issues; the warp stays converged for dealloc)
     constexpr uint32_t idesc_qk = tc_idesc(kTcRows, kTcTile, false), idesc_pv = tc_idesc(kTcRows, D, true);
-    uint32_t q_phase = 0, p_phase = 0;
+    uint32_t q_phase = 0;
     int cur_chunk = -1;
     bool use_lo = false;
     auto issue_qk = [&](int t) {
@@ -235,14 +244,14 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       __syncwarp();
     };
     auto issue_pv = [&](int t) {
-      mbar_wait(&bars[BAR_P_FULL], p_phase); p_phase ^= 1;   // P(t) is in shared memory, O rescaled if a reference moved
+      mbar_wait(&bars[BAR_P_FULL + (t & 1)], (t >> 1) & 1);   // P(t) is in shared memory, O rescaled if a reference moved
       tcf_after();
       if (lane == 0) {
         const int st = t % kTcStages;
         const uint32_t vb = sm0 + OFF_KV + st * 2 * KVB + KVB;
 #pragma unroll
         for (int kk = 0; kk < kTcTile / 16; ++kk)
-          tc_mma(tmem + TM_O, tc_desc(sm0 + OFF_P + kk * 32, 16, 1024), tc_desc(vb + kk * 2048, kTcTile * 128, 1024), idesc_pv,
+          tc_mma(tmem + TM_O, tc_desc(sm0 + OFF_P + (t & 1) * PBYTES + kk * 32, 16, 1024), tc_desc(vb + kk * 2048, kTcTile * 128, 1024), idesc_pv,
                  (t > 0 || kk > 0) ? 1u : 0u);
         tc_commit(&bars[BAR_KV_EMPTY + st]);                // the stage returns to the loader
         tc_commit(&bars[BAR_O_DONE]);
@@ -350,20 +359,23 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       for (int j = 0; j < kTcTile / 32; ++j) tmem_ld32_nowait(trow + TM_S + kTcTile * (t & 1) + 32 * j, s + 32 * j);
       tmem_ld_wait();
       const int tile_hi = min(cur.pos + kTcTile, cur.hi) - 1;
-      const bool masked = (cur.pos + kTcTile > cur.hi) || (tile_hi > cta_lim_lo);
-      const int last = min(tile_hi, lim) - cur.pos;          // last visible column of this row in the tile (may be < 0)
-      float mx = -CUDART_INF_F;
+      const bool masked = (cur.pos + kTcTile > cur.hi) || (tile_hi > cta_lim_lo);      // CTA-uniform
+      if (masked) {                                           // only where the chunk ends inside the tile or the diagonal crosses it
+        const int last = min(tile_hi, lim) - cur.pos;         // last visible column of this row in the tile (may be < 0)
 #pragma unroll
-      for (int j = 0; j < kTcTile; ++j) {
-        float v = s[j] * scale_log2;
-        if (masked && j > last) v = -CUDART_INF_F;
-        s[j] = v;
-        mx = fmaxf(mx, v);
+        for (int j = 0; j < kTcTile; ++j) if (j > last) s[j] = -CUDART_INF_F;
       }
+      float mx = s[0];
+#pragma unroll
+      for (int j = 1; j < kTcTile; ++j) mx = fmaxf(mx, s[j]);
+      mx *= scale_log2;                                       // sm_scale > 0: the scaled maximum is the maximum of the scaled scores
       const bool need = mx > m_ref + 8.f;                     // lazy reference: moves only when a score runs 2^8 past it
-      // O and the P buffer are ours once PV(t - 1) has completed
-      if (t > 0) { mbar_wait(&bars[BAR_O_DONE], o_phase); o_phase ^= 1; tcf_after(); }
+      // P has two buffers: P(t) may be written while PV(t - 1) still runs (PV(t - 2), the last reader of this buffer, was seen
+      // complete during tile t - 1).  Only a rescale of O must wait for PV(t - 1) first; otherwise that wait moves behind the
+      // P write, where it has long been satisfied.
+      bool o_pending = t > 0;
       if (__any_sync(0xffffffffu, need)) {
+        if (o_pending) { mbar_wait(&bars[BAR_O_DONE], o_phase); o_phase ^= 1; tcf_after(); o_pending = false; }
         const float mn = need ? mx : m_ref;
         const float alpha = (mn == m_ref) ? 1.f : ex2a(m_ref - mn);     // m_ref = -inf -> 0
         l_sum *= alpha;
@@ -381,17 +393,21 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
         }
       }
       // ---- P row (bf16) as the A operand of PV: [128 rows][128 B], swizzled
-      const float ref = m_ref == -CUDART_INF_F ? 0.f : m_ref;
+      const float nref = m_ref == -CUDART_INF_F ? 0.f : -m_ref;
+      float ls0 = 0.f, ls1 = 0.f;
 #pragma unroll
       for (int c = 0; c < kTcTile / 8; ++c) {
         float pv[8];
 #pragma unroll
-        for (int e = 0; e < 8; ++e) { pv[e] = ex2a(s[8 * c + e] - ref); l_sum += pv[e]; }
-        *reinterpret_cast<uint4*>(smem + OFF_P + sw_chunk(r, c)) = pack8(pv);
+        for (int e = 0; e < 8; ++e) pv[e] = ex2a(fmaf(s[8 * c + e], scale_log2, nref));     // e^{s - m}: -inf -> 0
+        ls0 += (pv[0] + pv[1]) + (pv[2] + pv[3]); ls1 += (pv[4] + pv[5]) + (pv[6] + pv[7]);
+        *reinterpret_cast<uint4*>(smem + OFF_P + (t & 1) * PBYTES + sw_chunk(r, c)) = pack8(pv);
       }
+      l_sum += ls0 + ls1;
       fence_proxy_async();
       tcf_before();
-      mbar_arrive(&bars[BAR_P_FULL]);
+      mbar_arrive(&bars[BAR_P_FULL + (t & 1)]);
+      if (o_pending) { mbar_wait(&bars[BAR_O_DONE], o_phase); o_phase ^= 1; tcf_after(); }
       more = cur.next();
       ++t;
     }
@@ -420,7 +436,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
   if (warp == 4) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TM_COLS) : "memory");
 }
 
-int prefill_tc_smem_bytes(int D) { return 1024 + 2 * kTcRows * D * 2 + kTcRows * kTcTile * 2 + kTcStages * 2 * kTcTile * D * 2; }
+int prefill_tc_smem_bytes(int D) { return 1024 + 2 * kTcRows * D * 2 + 2 * kTcRows * kTcTile * 2 + kTcStages * 2 * kTcTile * D * 2; }
 
 void launch_prefill_tc(const PrefillParams& p, int D, cudaStream_t st) {
   const int smem = prefill_tc_smem_bytes(D);
