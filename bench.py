@@ -595,6 +595,9 @@ def extras(wl, device, peak):
         it[0] += 1
         ctxp.kam_paged_prefill_merge(qp, btp, stp, ofp, ncp, it[0] % Lp, 1, wl.sm_scale, op, lp)
     ms = _time_ms(torch, launch, 6)
+    ctxp.kam_set_option("prefill_tcgen05", 0)
+    ms_legacy = _time_ms(torch, launch, 4)
+    ctxp.kam_set_option("prefill_tcgen05", 1)
     Nkv = n * T + Tq
     flops = 4.0 * nbp * cfg.n_q_heads * D * (Tq * (Nkv - Tq) + Tq * (Tq + 1) / 2)          # visible (row, token) pairs x 4 D
     flops_issued = flops * 2 * (n * T) / Nkv + flops * Tq / Nkv                               # rotated chunks run the q~ lo products too
@@ -602,7 +605,8 @@ def extras(wl, device, peak):
     out["prefill_config2_shape_b8_512rows_over_8192"] = {
         "ms": ms, "tflops": flops / ms / 1e9, "frac_of_dense_bf16_peak": flops / ms / 1e9 / tf_peak, "tflops_issued": flops_issued / ms / 1e9,
         "tensor_peak_tflops": tf_peak, "GB/s": nbp * Nkv * H * 2 * D * 2 / ms / 1e6, "frac_of_hbm_peak": nbp * Nkv * H * 2 * D * 2 / ms / 1e6 / peak,
-        "bound": "tensor", "what": "kam_paged_prefill_kernel<128> (mma.sync m16n8k16, FlashAttention-2 shape); flops = 4 D per visible (row, token) "
+        "bound": "tensor", "mma_sync_kernel": {"ms": ms_legacy, "tflops": flops / ms_legacy / 1e9, "what": "option prefill_tcgen05 = 0: kam_paged_prefill_kernel<128>, FlashAttention-2 shape on mma.sync"},
+        "what": "kam_paged_prefill_tc_kernel<128> (tcgen05.mma M128 N64/128 K16, S and O in tensor memory); flops = 4 D per visible (row, token) "
         "pair; tflops_issued counts the second (lo) QK^T product of chunks read at a pending offset; bytes = K + V once per request"}
     ctxp.close()
     del poolp, ctxp, btp, qp, op

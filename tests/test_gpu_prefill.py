@@ -17,7 +17,10 @@ from tests.test_gpu_decode import _fill_pool, check_attention
 pytestmark = pytest.mark.gpu
 
 
-def _run(cfg, lens, deltas, Tq, causal, seed, style=reuse.HALF, rows=None, layer=0, L=1):
+KERNELS = {"tcgen05": 1, "mma.sync": 0}       # option prefill_tcgen05: both formulations must meet the same bar
+
+
+def _run(cfg, lens, deltas, Tq, causal, seed, style=reuse.HALF, rows=None, layer=0, L=1, kernel="tcgen05"):
     """lens[b]: chunk lengths of request b (its cached tokens, the appended block included when causal); every request gets a
     block of Tq query rows.  rows: the query rows the oracle evaluates (None = all)."""
     rng = np.random.Generator(np.random.PCG64(seed))
@@ -28,6 +31,7 @@ def _run(cfg, lens, deltas, Tq, causal, seed, style=reuse.HALF, rows=None, layer
     num_pages = batch * max_pages + 3
     pool = _fill_pool(cfg, L, num_pages, seed)
     ctx = kam.Context(par.layout_of(cfg, L, B.KAM_ROPE_HALF if style == reuse.HALF else B.KAM_ROPE_INTERLEAVED), pool)
+    ctx.kam_set_option("prefill_tcgen05", KERNELS[kernel])
     perm = make_block_table(rng, batch * max_pages, num_pages).reshape(batch, max_pages)
     starts = np.zeros((batch, max_chunks + 1), np.int32)
     offs = np.zeros((batch, max_chunks), np.int64)
@@ -69,44 +73,50 @@ def _run(cfg, lens, deltas, Tq, causal, seed, style=reuse.HALF, rows=None, layer
     return worst
 
 
-def test_config2_gqa_64_rows_over_relocated_chunks():
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_config2_gqa_64_rows_over_relocated_chunks(kernel):
     """GQA 28 / 4: the appended 64-token turn (last chunk, offset 0) over recalled chunks read at pending offsets; ragged chunk
     lengths, tiles cut by chunk ends, 64 x 7 = 448 rows per KV head = 7 row tiles."""
     cfg = CONFIGS[2]
-    _run(cfg, [[300, 1024, 37, 64], [100, 64]], [[3100, -77, 5, 0], [0, 0]], 64, 1, 501)
+    _run(cfg, [[300, 1024, 37, 64], [100, 64]], [[3100, -77, 5, 0], [0, 0]], 64, 1, 501, kernel=kernel)
 
 
-def test_config2_gqa_512_rows_sampled():
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_config2_gqa_512_rows_sampled(kernel):
     """A 512-token text turn (P:105 TTFT path) over three recalled chunks; the oracle evaluates 40 of the 512 rows."""
     cfg = CONFIGS[2]
     rows = sorted(set([0, 1, 63, 64, 255, 256, 510, 511] + list(range(5, 512, 16))))
-    _run(cfg, [[1024, 700, 200, 512]], [[-20000, 1, 32767, 0]], 512, 1, 502, rows=rows)
+    _run(cfg, [[1024, 700, 200, 512]], [[-20000, 1, 32767, 0]], 512, 1, 502, rows=rows, kernel=kernel)
 
 
-def test_config4_mha_64_and_512_rows():
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_config4_mha_64_and_512_rows(kernel):
     """MHA (G = 1: one row tile per 64 tokens and head), config 4's window + prefix shape scaled to 8 heads."""
     cfg = CONFIGS[4].scaled(n_layers=2, n_q_heads=8, n_kv_heads=8)
-    _run(cfg, [[512, 1280, 64]], [[0, -1280, 0]], 64, 1, 503, layer=1, L=2)
-    _run(cfg, [[160, 1280, 512]], [[0, 4096, 0]], 512, 1, 504, rows=[0, 7, 100, 300, 511], layer=0, L=2)
+    _run(cfg, [[512, 1280, 64]], [[0, -1280, 0]], 64, 1, 503, layer=1, L=2, kernel=kernel)
+    _run(cfg, [[160, 1280, 512]], [[0, 4096, 0]], 512, 1, 504, rows=[0, 7, 100, 300, 511], layer=0, L=2, kernel=kernel)
 
 
-def test_not_causal_every_row_is_the_decode_readout():
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_not_causal_every_row_is_the_decode_readout(kernel):
     cfg = CONFIGS[2].scaled(n_q_heads=8, n_kv_heads=4)
-    _run(cfg, [[130, 70], [16]], [[9, -9], [123]], 24, 0, 505)
+    _run(cfg, [[130, 70], [16]], [[9, -9], [123]], 24, 0, 505, kernel=kernel)
 
 
-def test_edge_cases():
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_edge_cases(kernel):
     """Rows x G not a multiple of the 64-row tile; more query rows than cached tokens (the first rows see nothing: out = 0,
     lse = -inf); a request with no cached tokens; single-token chunks; an empty chunk in the middle."""
     cfg = CONFIGS[2].scaled(n_q_heads=12, n_kv_heads=4)           # G = 3
-    _run(cfg, [[5, 0, 1, 30], [3], []], [[7, 0, -1, 0], [0], []], 10, 1, 506)
-    _run(cfg, [[17]], [[0]], 1, 1, 507)                          # one query row = a decode step
+    _run(cfg, [[5, 0, 1, 30], [3], []], [[7, 0, -1, 0], [0], []], 10, 1, 506, kernel=kernel)
+    _run(cfg, [[17]], [[0]], 1, 1, 507, kernel=kernel)           # one query row = a decode step
 
 
-def test_head_dim_64_and_interleaved_pairs():
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_head_dim_64_and_interleaved_pairs(kernel):
     cfg = CONFIGS[1].scaled(elem_dtype="bf16", factor_dtype="bf16", n_layers=1)      # MHA 4 heads, head_dim 64
-    _run(cfg, [[200, 64]], [[1000, 0]], 64, 1, 508)
-    _run(CONFIGS[2].scaled(n_q_heads=8, n_kv_heads=4), [[90, 40]], [[-555, 0]], 40, 1, 509, style=reuse.INTERLEAVED)
+    _run(cfg, [[200, 64]], [[1000, 0]], 64, 1, 508, kernel=kernel)
+    _run(CONFIGS[2].scaled(n_q_heads=8, n_kv_heads=4), [[90, 40]], [[-555, 0]], 40, 1, 509, style=reuse.INTERLEAVED, kernel=kernel)
 
 
 def test_unsupported_and_invalid_arguments():
