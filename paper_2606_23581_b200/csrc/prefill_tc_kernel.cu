@@ -40,14 +40,21 @@ enum : int { BAR_KV_FULL = 0, BAR_KV_EMPTY = kTcStages, BAR_S_FULL = 2 * kTcStag
 
 __device__ __forceinline__ void tcf_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tcf_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint64_t* bar) {     // arrives on bar when all MMAs issued so far by this thread are done
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+// The MMA warp runs CONVERGED with warp-uniform operands; the single issuing lane is elected INSIDE each asm block.  (An
+// `if (lane == 0)` around tcgen05 instructions makes the compiler wrap every one of them in an ELECT / BRA.U.ANY loop and rebuild
+// its descriptors with ~16 uniform-datapath instructions: ~420 instructions per tile in the issuing warp - measured with clock64:
+// the warp spent 2 270 of 2 460 cycles per tile ISSUING, not waiting.)
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {     // arrives on bar when all MMAs issued so far by the elected lane are done
+  asm volatile("{\n\t.reg .pred e;\n\telect.sync _|e, 0xffffffff;\n\t"
+               "@e tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+// descriptors travel as (low word, high word): the low word is base + (byte offset >> 4), the high word a constant
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi, uint32_t idesc, uint32_t accumulate) {
   asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+      "{\n\t.reg .pred p, e;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 p, %6, 0;\n\tmov.b64 da, {%1, %2};\n\tmov.b64 db, {%3, %4};\n\t"
+      "elect.sync _|e, 0xffffffff;\n\t"
+      "@e tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %5, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate) : "memory");
 }
 // shared-memory matrix descriptor, 128-byte swizzle (layout type 2), version 1; offsets in bytes.  K-major operand: lbo unused
 // (16), sbo = stride between 8-row groups.  MN-major operand: lbo = stride between 64-element blocks along MN, sbo = stride
@@ -215,48 +222,58 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       more = cur.next();
     }
     asm volatile("cp.async.wait_all;" ::: "memory");
+#if defined(PF_DIAG) && (PF_DIAG & 8)
+    asm volatile("bar.sync 7, %0;" ::"n"(kTcThreads) : "memory");
+#endif
   } else if (warp == 4) {
     // ================================================================ MMA issuer (lane 0 issues; the warp stays converged for dealloc)
     constexpr uint32_t idesc_qk = tc_idesc(kTcRows, kTcTile, false), idesc_pv = tc_idesc(kTcRows, D, true);
     uint32_t q_phase = 0;
     int cur_chunk = -1;
     bool use_lo = false;
+#if defined(PF_DIAG) && (PF_DIAG & 8)
+    long long dbg_kv = 0, dbg_p = 0, dbg_t0 = clock64();
+#define DBG_T(acc, stmt) { const long long c0_ = clock64(); stmt; acc += clock64() - c0_; }
+#else
+#define DBG_T(acc, stmt) { stmt; }
+    long long dbg_kv = 0, dbg_p = 0;
+#endif
+    // descriptor words: hi = (sbo >> 4) | version 1 << 14 | swizzle-128B << 29 (+ the lbo field in the low word's upper half)
+    constexpr uint32_t kHiK = (1024u >> 4) | (1u << 14) | (2u << 29);
+    constexpr uint32_t kLoK = (16u >> 4) << 16;                                   // K-major operands: lbo unused (16)
+    constexpr uint32_t kLoV = ((kTcTile * 128u) >> 4) << 16;                      // the V tile, MN-major: lbo = stride between 64-column blocks
+    const uint32_t q_lo = kLoK | ((sm0 + OFF_Q) >> 4), ql_lo = kLoK | ((sm0 + OFF_QLO) >> 4), p_lo = kLoK | ((sm0 + OFF_P) >> 4);
+    const uint32_t kv_lo = (sm0 + OFF_KV) >> 4;
     auto issue_qk = [&](int t) {
       const int st = t % kTcStages;
-      mbar_wait(&bars[BAR_KV_FULL + st], (t / kTcStages) & 1);
+      DBG_T(dbg_kv, mbar_wait(&bars[BAR_KV_FULL + st], (t / kTcStages) & 1));
       fence_proxy_async();                                  // the tile was written by cp.async (generic proxy), tcgen05.mma reads through the async proxy
       tcf_after();
-      if (lane == 0) {
-        const uint32_t kb = sm0 + OFF_KV + st * 2 * KVB;
-        const uint32_t s_t = tmem + TM_S + kTcTile * (t & 1);
+      const uint32_t k_lo = kLoK | (kv_lo + st * (2 * KVB >> 4));
+      const uint32_t s_t = tmem + TM_S + kTcTile * (t & 1);
+#pragma unroll
+      for (int ks = 0; ks < D / 16; ++ks)
+        tc_mma(s_t, q_lo + (((ks >> 2) * (kTcRows * 128) + (ks & 3) * 32) >> 4), kHiK,
+               k_lo + (((ks >> 2) * (kTcTile * 128) + (ks & 3) * 32) >> 4), kHiK, idesc_qk, ks > 0 ? 1u : 0u);
+      if (use_lo) {
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks)
-          tc_mma(s_t, tc_desc(sm0 + OFF_Q + (ks >> 2) * (kTcRows * 128) + (ks & 3) * 32, 16, 1024),
-                 tc_desc(kb + (ks >> 2) * (kTcTile * 128) + (ks & 3) * 32, 16, 1024), idesc_qk, ks > 0 ? 1u : 0u);
-        if (use_lo) {
-#pragma unroll
-          for (int ks = 0; ks < D / 16; ++ks)
-            tc_mma(s_t, tc_desc(sm0 + OFF_QLO + (ks >> 2) * (kTcRows * 128) + (ks & 3) * 32, 16, 1024),
-                   tc_desc(kb + (ks >> 2) * (kTcTile * 128) + (ks & 3) * 32, 16, 1024), idesc_qk, 1u);
-        }
-        tc_commit(&bars[BAR_S_FULL + (t & 1)]);
+          tc_mma(s_t, ql_lo + (((ks >> 2) * (kTcRows * 128) + (ks & 3) * 32) >> 4), kHiK,
+                 k_lo + (((ks >> 2) * (kTcTile * 128) + (ks & 3) * 32) >> 4), kHiK, idesc_qk, 1u);
       }
-      __syncwarp();
+      tc_commit(&bars[BAR_S_FULL + (t & 1)]);
     };
     auto issue_pv = [&](int t) {
-      mbar_wait(&bars[BAR_P_FULL + (t & 1)], (t >> 1) & 1);   // P(t) is in shared memory, O rescaled if a reference moved
+      DBG_T(dbg_p, mbar_wait(&bars[BAR_P_FULL + (t & 1)], (t >> 1) & 1));   // P(t) is in shared memory, O rescaled if a reference moved
       tcf_after();
-      if (lane == 0) {
-        const int st = t % kTcStages;
-        const uint32_t vb = sm0 + OFF_KV + st * 2 * KVB + KVB;
+      const int st = t % kTcStages;
+      const uint32_t v_lo = kLoV | (kv_lo + ((st * 2 * KVB + KVB) >> 4));
+      const uint32_t pa_lo = p_lo + (t & 1) * (PBYTES >> 4);
 #pragma unroll
-        for (int kk = 0; kk < kTcTile / 16; ++kk)
-          tc_mma(tmem + TM_O, tc_desc(sm0 + OFF_P + (t & 1) * PBYTES + kk * 32, 16, 1024), tc_desc(vb + kk * 2048, kTcTile * 128, 1024), idesc_pv,
-                 (t > 0 || kk > 0) ? 1u : 0u);
-        tc_commit(&bars[BAR_KV_EMPTY + st]);                // the stage returns to the loader
-        tc_commit(&bars[BAR_O_DONE]);
-      }
-      __syncwarp();
+      for (int kk = 0; kk < kTcTile / 16; ++kk)
+        tc_mma(tmem + TM_O, pa_lo + ((kk * 32) >> 4), kHiK, v_lo + ((kk * 2048) >> 4), kHiK, idesc_pv, (t > 0 || kk > 0) ? 1u : 0u);
+      tc_commit(&bars[BAR_KV_EMPTY + st]);                  // the stage returns to the loader
+      tc_commit(&bars[BAR_O_DONE]);
     };
     auto enter_chunk = [&]() {                               // q~ of the tile's chunk is staged by the softmax threads
       if (cur.c != cur_chunk) {
@@ -271,13 +288,26 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
     while (more) {
       TcTiles nxt = cur;
       const bool has_next = nxt.next();
+#if defined(PF_DIAG) && (PF_DIAG & 2)
+      const bool look = false;
+#else
       const bool look = has_next && nxt.c == cur.c;          // same chunk: its scores are computed ahead of this tile's PV
+#endif
       if (look) issue_qk(t + 1);
       issue_pv(t);
       cur = nxt; more = has_next;
       if (has_next && !look) { enter_chunk(); issue_qk(t + 1); }
       ++t;
     }
+#if defined(PF_DIAG) && (PF_DIAG & 8)
+    __syncwarp();
+    asm volatile("bar.sync 7, %0;" ::"n"(kTcThreads) : "memory");          // everyone's results are written: the debug words go on top
+    if (lane == 0 && blockIdx.x == 3) {
+      float* dbg = p.lse + (static_cast<size_t>(b) * p.Tq + 55) * p.Hq + h * G;
+      dbg[0] = static_cast<float>(clock64() - dbg_t0); dbg[1] = static_cast<float>(dbg_kv); dbg[2] = static_cast<float>(dbg_p); dbg[3] = static_cast<float>(t);
+    }
+#endif
+    (void)dbg_kv; (void)dbg_p;
   } else {
     // ================================================================ softmax threads: thread = row = tensor-memory lane
     const int r = threadIdx.x;                               // 0 .. 127
@@ -292,6 +322,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
     float m_ref = -CUDART_INF_F, l_sum = 0.f;
     uint32_t o_phase = 0;
     int cur_chunk = -1, t = 0;
+    [[maybe_unused]] long long dbg_s = 0, dbg_s0 = clock64();
     while (more) {
       if (cur.c != cur_chunk) {
         // ---- new chunk: q~ = R(-delta) q of this thread's row into the A operand (hi, and lo when rotated).  Every MMA that
@@ -352,7 +383,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       }
 
       // ---- this row of S(t)
+#if defined(PF_DIAG) && (PF_DIAG & 8)
+      { const long long c0_ = clock64(); mbar_wait(&bars[BAR_S_FULL + (t & 1)], (t >> 1) & 1); dbg_s += clock64() - c0_; }
+#else
       mbar_wait(&bars[BAR_S_FULL + (t & 1)], (t >> 1) & 1);
+#endif
       tcf_after();
       float s[kTcTile];
 #pragma unroll
@@ -399,7 +434,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       for (int c = 0; c < kTcTile / 8; ++c) {
         float pv[8];
 #pragma unroll
+#if defined(PF_DIAG) && (PF_DIAG & 1)
+        for (int e = 0; e < 8; ++e) pv[e] = s[8 * c + e];
+#else
         for (int e = 0; e < 8; ++e) pv[e] = ex2a(fmaf(s[8 * c + e], scale_log2, nref));     // e^{s - m}: -inf -> 0
+#endif
         ls0 += (pv[0] + pv[1]) + (pv[2] + pv[3]); ls1 += (pv[4] + pv[5]) + (pv[6] + pv[7]);
         *reinterpret_cast<uint4*>(smem + OFF_P + (t & 1) * PBYTES + sw_chunk(r, c)) = pack8(pv);
       }
@@ -429,6 +468,14 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       if (live) { op[2 * j] = pack8(o); op[2 * j + 1] = pack8(o + 8); }
     }
     if (live) p.lse[orow] = l_sum > 0.f ? m_ref * 0.6931471805599453f + logf(l_sum) : -CUDART_INF_F;
+#if defined(PF_DIAG) && (PF_DIAG & 8)
+    const long long dbg_tot = clock64() - dbg_s0;
+    asm volatile("bar.sync 7, %0;" ::"n"(kTcThreads) : "memory");
+    if (threadIdx.x == 0 && blockIdx.x == 3) {
+      float* dbg = p.lse + (static_cast<size_t>(b) * p.Tq + 56) * p.Hq + h * G;
+      dbg[0] = static_cast<float>(dbg_tot); dbg[1] = static_cast<float>(dbg_s); dbg[3] = static_cast<float>(t);
+    }
+#endif
   }
   // ---- teardown: every role is past its last tensor-memory access
   tcf_before();
