@@ -12,14 +12,19 @@
 //   O[128 rows][D]         += P V        A = P (smem, K-major, written by the softmax threads), B = the V tile read MN-major   4 x M128 N128 K16
 //
 // S (double-buffered, 2 x 64 columns) and O (D columns) live in tensor memory; a softmax thread owns ONE row (its TMEM lane):
-// tcgen05.ld of the row, scale, mask, exp2, P to shared memory, the lazy O rescale of the FlashAttention-4 kind (only when the
-// row's reference must move by more than 2^8) through tcgen05.ld / st.  Roles: warps 0-3 softmax (128 threads = 128 rows),
-// warp 4 issues the MMAs (one lane) and owns the tensor-memory allocation, warp 5 loads K / V tiles with cp.async (slots
-// mapped through the block table per token, rows beyond the chunk zero-filled) into a 3-stage ring in the canonical
-// SWIZZLE_128B operand layout ([64-column block][token][128 B], 16-byte chunk index XOR token & 7).  QK^T of tile t + 1 is issued
-// before PV of tile t, so the tensor pipe computes scores while the softmax threads turn S(t) into P(t).
-// Relocation on read: q~ = R(-delta) q is rebuilt in shared memory once per chunk (hi + lo; chunks with delta = 0 skip the
-// lo products); no look-ahead across a chunk boundary.  Same arithmetic contract, masks and output as prefill_kernel.cu.
+// tcgen05.ld of the row, mask, maximum, exp2, the P row to shared memory (two buffers), and the lazy O rescale of the
+// FlashAttention-4 kind (only when the row's reference must move by more than 2^8) through tcgen05.ld / st - row statistics
+// never cross threads.  Roles: warps 0-3 softmax (128 threads = 128 rows); warp 4 issues the MMAs and owns the tensor-memory
+// allocation - it stays CONVERGED and elects the issuing lane inside each asm block (see tc_mma); warps 5-8 load K / V tiles
+// with cp.async (one slot lookup per row, shuffled to the copying lanes; slots mapped through the block table per token, rows
+// beyond the chunk zero-filled) into a 4-stage ring in the canonical SWIZZLE_128B operand layout ([64-column block][token]
+// [128 B], 16-byte chunk index XOR token & 7) and signal a tile's barrier with cp.async.mbarrier.arrive.noinc (no wait_group on
+// their path).  QK^T of tile t + 1 is issued before PV of tile t, so the tensor pipe computes scores while the softmax threads
+// turn S(t) into P(t).  Relocation on read: q~ = R(-delta) q is rebuilt in shared memory once per chunk (hi + lo; chunks with
+// delta = 0 skip the lo products); no look-ahead across a chunk boundary.  Same arithmetic contract, masks and output as
+// prefill_kernel.cu (a call with sm_scale <= 0 runs that kernel: the row maximum here is taken before scaling).
+// Measured path and where the cycles go: DESIGN.md 7.4.  Diagnostic builds (KAM_NVCC_EXTRA=-DPF_DIAG=n; wrong results): 1 no
+// exp2, 2 no QK^T look-ahead, 8 clock64 counters of the MMA warp's and a softmax thread's waits written over two lse rows.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
@@ -56,13 +61,10 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint32_t a_lo, uint32_t 
       "@e tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %5, p;\n\t}"
       ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate) : "memory");
 }
-// shared-memory matrix descriptor, 128-byte swizzle (layout type 2), version 1; offsets in bytes.  K-major operand: lbo unused
-// (16), sbo = stride between 8-row groups.  MN-major operand: lbo = stride between 64-element blocks along MN, sbo = stride
-// between groups of 8 K rows.
-__device__ __forceinline__ uint64_t tc_desc(uint32_t smem_addr, uint32_t lbo, uint32_t sbo) {
-  return static_cast<uint64_t>((smem_addr & 0x3ffff) >> 4) | (static_cast<uint64_t>(lbo >> 4) << 16) |
-         (static_cast<uint64_t>(sbo >> 4) << 32) | (1ull << 46) | (2ull << 61);
-}
+// Shared-memory matrix descriptors (128-byte swizzle = layout type 2, version 1) are built in the MMA warp as two words:
+//   low  = (address >> 4) | (lbo >> 4) << 16      high = (sbo >> 4) | 1 << 14 | 2 << 29
+// K-major operand: lbo unused (16), sbo = stride between 8-row groups.  MN-major operand (the V tile): lbo = stride between
+// 64-element blocks along MN, sbo = stride between groups of 8 K rows.
 // instruction descriptor: D = f32, A = B = bf16, M x N, A K-major; b_mn: B is MN-major (the V tile)
 __device__ __forceinline__ constexpr uint32_t tc_idesc(uint32_t m, uint32_t n, bool b_mn) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn ? 1u : 0u) << 16) | ((n >> 3) << 17) | ((m >> 4) << 24);

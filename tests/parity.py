@@ -17,6 +17,9 @@ from oracle.bf16 import bf16_bits, bf16_from_bits, bf16_rne, ulp_bf16
 from paper_2606_23581_b200 import binding as B
 
 SENTINEL = 1248.0          # exactly representable in bf16
+# every compare_bf16 call of the session adds its counts here; tests/conftest.py prints the totals at the end of the run, so
+# that the second clause of the 1-ulp rule (the fp32-accumulation floor) stays visible: how many elements needed it
+TOTALS = {"n": 0, "exact": 0, "within_1ulp": 0, "needed_floor": 0, "fail": 0}
 
 
 def layout_of(cfg, n_layers=None, style=B.KAM_ROPE_HALF, elem=None, factor=None):
@@ -83,6 +86,8 @@ def compare_bf16(g, o, S, m, what=""):
     ok = err <= np.maximum(ulp, floor)
     stats = {"n": int(err.size), "exact": int(np.sum(err == 0)), "within_1ulp": int(np.sum(err <= ulp)),
              "needed_floor": int(np.sum((err > ulp) & ok)), "fail": int(np.sum(~ok))}
+    for k_, v_ in stats.items():
+        TOTALS[k_] += v_
     if stats["fail"]:
         bad = np.argwhere(~ok)[:5]
         detail = [(tuple(i), g[tuple(i)], ob[tuple(i)], o[tuple(i)]) for i in bad]
