@@ -653,8 +653,11 @@ def extras(wl, device, peak):
     ctx3.kam_decode_set_max_patch_rank(16)
     Lr = 2
     refs3 = [B.patch_refs([[(rnd((T3, 1, m3)), rnd((1, m3, D3), c3.w_std), None, None, m3) for _ in range(nch3)] for _ in range(nb3)], device) for _ in range(Lr)]
-    for name, pr in (("mla_decode_absorbed", None), ("mla_decode_on_read_patch_m16", refs3)):
+    # (the two per-call-plan entries first: profiles/ncu_extras_r02.md counts launches of this kernel from the start of the extras)
+    for name, pr, pin in (("mla_decode_absorbed", None, False), ("mla_decode_on_read_patch_m16", refs3, False),
+                          ("mla_decode_absorbed_pinned_plan", None, True), ("mla_decode_on_read_patch_m16_pinned_plan", refs3, True)):
         it = [0]
+        ctx3.kam_paged_decode_plan(bt3b if pin else None, st3, None, nc3, has_patches=pr is not None)
 
         def launch():
             l = it[0] % L3
@@ -663,8 +666,9 @@ def extras(wl, device, peak):
         ms = _time_ms(torch, launch, 27)
         nbytes = nb3 * nch3 * T3 * (D3 + (m3 if pr else 0)) * 2
         out[name] = entry(nbytes, ms, bytes="every latent+rope row once (it is both key and value)" + (" + its U row" if pr else ""), batch=nb3, tokens=nch3 * T3,
-                          what="stateless call = plan + kam_mla_ts_decode_kernel (token-split) + merge",
+                          what=("kam_paged_decode_plan once, then " if pin else "stateless call = plan + ") + "kam_mla_ts_decode_kernel (token-split) + merge",
                           tflops=nb3 * nch3 * T3 * c3.n_q_heads * (D3 + c3.v_dim) * 2 / ms / 1e9)
+    ctx3.kam_paged_decode_plan(None, None, None, None)
     ctx3.close()
     return out
 
