@@ -9,10 +9,11 @@
 // space of one KV head and walks the request's cached tokens in 64-token tiles:
 //
 //   S[128 rows][64 tokens]  = q~ K^T     A = q~ (smem, K-major), B = the K tile (smem, K-major)          8 x tcgen05.mma M128 N64 K16
-//   O[128 rows][D]         += P V        A = P (smem, K-major, written by the softmax threads), B = the V tile read MN-major   4 x M128 N128 K16
+//   O[128 rows][D]         += P V        A = P (TENSOR MEMORY: written by the softmax threads over S), B = the V tile read MN-major   4 x M128 N128 K16
 //
 // S (double-buffered, 2 x 64 columns) and O (D columns) live in tensor memory; a softmax thread owns ONE row (its TMEM lane):
-// tcgen05.ld of the row, mask, maximum, exp2, the P row to shared memory (two buffers), and the lazy O rescale of the
+// tcgen05.ld of the row, mask, maximum, exp2, the P row (bf16 pairs) stored with tcgen05.st over the first 32 columns of the
+// S buffer it came from - PV reads its A operand from there, no shared-memory round trip and no proxy fence -, and the lazy O rescale of the
 // FlashAttention-4 kind (only when the row's reference must move by more than 2^8) through tcgen05.ld / st - row statistics
 // never cross threads.  Roles: warps 0-3 softmax (128 threads = 128 rows); warp 4 issues the MMAs and owns the tensor-memory
 // allocation - it stays CONVERGED and elects the issuing lane inside each asm block (see tc_mma); warps 5-8 load K / V tiles
@@ -38,6 +39,7 @@ namespace {
 constexpr int kTcRows = 128;               // rows per CTA (= TMEM lanes)
 constexpr int kTcTile = 64;                // cached tokens per tile
 constexpr int kTcStages = 4;
+constexpr bool kTcPInTmem = true;         // P(t) is written over the first 32 columns of S(t) in tensor memory and read from there by PV
 constexpr int kTcLoaders = 4;              // loader warps: each takes a quarter of a tile's rows
 constexpr int kTcThreads = (5 + kTcLoaders) * 32;   // 4 softmax warps + MMA warp + loader warps
 enum : int { BAR_KV_FULL = 0, BAR_KV_EMPTY = kTcStages, BAR_S_FULL = 2 * kTcStages /* x2 */, BAR_P_FULL = 2 * kTcStages + 2 /* x2 */, BAR_O_DONE = 2 * kTcStages + 4,
@@ -60,6 +62,21 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint32_t a_lo, uint32_t 
       "elect.sync _|e, 0xffffffff;\n\t"
       "@e tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %5, p;\n\t}"
       ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate) : "memory");
+}
+// the same with the A operand in TENSOR MEMORY (the P row block: lane = row, 16 bf16 of K in 8 columns)
+__device__ __forceinline__ void tc_mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p, e;\n\t.reg .b64 db;\n\tsetp.ne.b32 p, %5, 0;\n\tmov.b64 db, {%2, %3};\n\t"
+      "elect.sync _|e, 0xffffffff;\n\t"
+      "@e tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %4, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {      // this thread's lane, 32 consecutive columns
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+               ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]),
+                 "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
+                 "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+               : "memory");
 }
 // Shared-memory matrix descriptors (128-byte swizzle = layout type 2, version 1) are built in the MMA warp as two words:
 //   low  = (address >> 4) | (lbo >> 4) << 16      high = (sbo >> 4) | 1 << 14 | 2 << 29
@@ -139,7 +156,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
   constexpr int QBYTES = kTcRows * D * 2;                  // one q~ operand (hi or lo): [DB][128 rows][128 B]
   constexpr int PBYTES = kTcRows * kTcTile * 2;            // P: [128 rows][128 B], two buffers
   constexpr int KVB = kTcTile * D * 2;                     // one K (or V) tile: [DB][64 tokens][128 B]
-  constexpr int OFF_Q = 1024, OFF_QLO = OFF_Q + QBYTES, OFF_P = OFF_QLO + QBYTES, OFF_KV = OFF_P + 2 * PBYTES;
+  constexpr int OFF_Q = 1024, OFF_QLO = OFF_Q + QBYTES, OFF_P = OFF_QLO + QBYTES, OFF_KV = OFF_P + (kTcPInTmem ? 0 : 2 * PBYTES);
   constexpr uint32_t TM_S = 0, TM_O = 2 * kTcTile, TM_COLS = (TM_O + D <= 256) ? 256 : 512;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
@@ -189,7 +206,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
     constexpr int RPP = 32 / CPR;                           // rows per pass of the warp (2 at D = 128, 4 at D = 64)
     constexpr int RPW = kTcTile / kTcLoaders;               // rows per loader warp
     const int lc = lane % CPR;
-    static_assert(RPW == 16, "one slot per lane of a half warp");
+    static_assert(RPW <= 32 && (RPW & (RPW - 1)) == 0, "one slot per lane");
     const uint32_t dst_c = static_cast<uint32_t>((lc >> 3) * (kTcTile * 128));       // the chunk's 64-column block
     int issued = 0;
     const char* kbase = pool_k + head_off + lc * 16;
@@ -273,7 +290,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       const uint32_t pa_lo = p_lo + (t & 1) * (PBYTES >> 4);
 #pragma unroll
       for (int kk = 0; kk < kTcTile / 16; ++kk)
-        tc_mma(tmem + TM_O, pa_lo + ((kk * 32) >> 4), kHiK, v_lo + ((kk * 2048) >> 4), kHiK, idesc_pv, (t > 0 || kk > 0) ? 1u : 0u);
+        if (kTcPInTmem) tc_mma_ts(tmem + TM_O, tmem + TM_S + kTcTile * (t & 1) + 8 * kk, v_lo + ((kk * 2048) >> 4), kHiK, idesc_pv, (t > 0 || kk > 0) ? 1u : 0u);
+        else tc_mma(tmem + TM_O, pa_lo + ((kk * 32) >> 4), kHiK, v_lo + ((kk * 2048) >> 4), kHiK, idesc_pv, (t > 0 || kk > 0) ? 1u : 0u);
       tc_commit(&bars[BAR_KV_EMPTY + st]);                  // the stage returns to the loader
       tc_commit(&bars[BAR_O_DONE]);
     };
@@ -432,6 +450,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       // ---- P row (bf16) as the A operand of PV: [128 rows][128 B], swizzled
       const float nref = m_ref == -CUDART_INF_F ? 0.f : -m_ref;
       float ls0 = 0.f, ls1 = 0.f;
+      [[maybe_unused]] uint32_t pw[kTcTile / 2];
 #pragma unroll
       for (int c = 0; c < kTcTile / 8; ++c) {
         float pv[8];
@@ -442,10 +461,20 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
         for (int e = 0; e < 8; ++e) pv[e] = ex2a(fmaf(s[8 * c + e], scale_log2, nref));     // e^{s - m}: -inf -> 0
 #endif
         ls0 += (pv[0] + pv[1]) + (pv[2] + pv[3]); ls1 += (pv[4] + pv[5]) + (pv[6] + pv[7]);
-        *reinterpret_cast<uint4*>(smem + OFF_P + (t & 1) * PBYTES + sw_chunk(r, c)) = pack8(pv);
+        const uint4 pk = pack8(pv);
+        if (kTcPInTmem) { pw[4 * c] = pk.x; pw[4 * c + 1] = pk.y; pw[4 * c + 2] = pk.z; pw[4 * c + 3] = pk.w; }
+        else *reinterpret_cast<uint4*>(smem + OFF_P + (t & 1) * PBYTES + sw_chunk(r, c)) = pk;
       }
       l_sum += ls0 + ls1;
-      fence_proxy_async();
+      if (kTcPInTmem) {
+        // P(t) over the first 32 columns of S(t): this thread has its S row in registers; the next writer of these columns is
+        // QK^T of tile t + 2, issued after PV(t) and executed behind it
+#pragma unroll
+        for (int j = 0; j < kTcTile / 64; ++j) tmem_st32(trow + TM_S + kTcTile * (t & 1) + 32 * j, pw + 32 * j);
+        tmem_st_wait();
+      } else {
+        fence_proxy_async();
+      }
       tcf_before();
       mbar_arrive(&bars[BAR_P_FULL + (t & 1)]);
       if (o_pending) { mbar_wait(&bars[BAR_O_DONE], o_phase); o_phase ^= 1; tcf_after(); }
@@ -485,7 +514,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
   if (warp == 4) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TM_COLS) : "memory");
 }
 
-int prefill_tc_smem_bytes(int D) { return 1024 + 2 * kTcRows * D * 2 + 2 * kTcRows * kTcTile * 2 + kTcStages * 2 * kTcTile * D * 2; }
+int prefill_tc_smem_bytes(int D) { return 1024 + 2 * kTcRows * D * 2 + (kTcPInTmem ? 0 : 2 * kTcRows * kTcTile * 2) + kTcStages * 2 * kTcTile * D * 2; }
 
 void launch_prefill_tc(const PrefillParams& p, int D, cudaStream_t st) {
   const int smem = prefill_tc_smem_bytes(D);
