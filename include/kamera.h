@@ -149,7 +149,7 @@ typedef struct kam_stats {
 kam_status kam_create(const kam_layout *layout, const kam_pool *pool, int32_t max_requests,
                       int32_t max_chunks_per_request, int32_t max_pages_per_chunk, kam_ctx **out);
 kam_status kam_destroy(kam_ctx *ctx);
-const char *kam_last_error(const kam_ctx *ctx);     /* ctx may be NULL: error of the last failed kam_create */
+const char *kam_last_error(const kam_ctx *ctx);     /* ctx may be NULL: error of this thread's last failed kam_create (or context-free call) */
 const char *kam_version(void);
 /* Tunables, per context; the defaults are the measured choices and nothing reads the environment.  Keys:
  *   reloc_stages 0..8 (0 = automatic)   reloc_head_group 0..4   reloc_head_group_cap 1..8   reloc_kv_split 0 never / 1 automatic / 2 always
@@ -343,6 +343,45 @@ kam_status kam_paged_decode_merge_host(kam_ctx *ctx, const void *q_host, const k
                                        const int64_t *chunk_offsets, const int32_t *n_chunks, int32_t max_chunks,
                                        const kam_patch_ref *patches, int32_t layer, int32_t batch, float sm_scale,
                                        void *out_host, float *lse_host, void *stream);
+
+/* ---- the fused decode for callers that must not allocate device memory (same readout as kam_paged_decode_merge) -----
+ * Who needs this: every other decode entry hangs off a kam_ctx, and a context cudaMallocs - at kam_create (frequency table,
+ * error counter, tensor maps) and again whenever a call needs a bigger plan / partials workspace or names a new pool.  Some
+ * hosts cannot live with that: a serving engine that hands ALL free HBM to its own KV-pool / caching allocator at start-up (a
+ * later cudaMalloc from a library then simply fails with out-of-memory), a plug-in loaded into a process whose memory budget
+ * is enforced from outside, a latency-critical loop where cudaMalloc's implicit device-wide synchronisation is not
+ * acceptable.  This ONE call needs no context and calls no cudaMalloc / cudaFree / cudaMallocAsync or any other allocating
+ * routine, on its first use or later: its plan, its cos/sin tables, its frequency table and the per-segment softmax partials
+ * live in a file-scope `static __device__` array of KAM_STATIC_SCRATCH_BYTES inside libkamera.so.
+ * The cost: every GPU on which a process loads the library carries that array until the process exits, used or not.
+ *
+ * Arguments as kam_paged_decode_merge (q, block_tables, chunk_starts, chunk_offsets, n_chunks, out, lse: caller-owned DEVICE
+ * memory, same shapes, same alignment rules), with the layout and the pool passed directly instead of through a context.
+ * Restrictions: bf16 MHA / GQA pools with head_dim 64 or 128 and at most 16 query heads per KV head, rope_dim <= 256; no on-read
+ * patch (materialise patches with kam_relocate_patch first); MLA is KAM_ERR_UNSUPPORTED (its kernel needs tensor maps, which
+ * need device memory of their own).  Pool pages are fetched by per-token bulk copies (what option decode_tma = 0 selects on the
+ * context path), so any page_size works; the arithmetic, the work split and the merge order are those of the context path.
+ *
+ * Size limit: the scratch a call needs grows with batch * max_chunks (about (444 + batch * max_chunks) * n_q_heads * (head_dim + 1)
+ * * 4 bytes of partials for a 4-KV-head layout, plus the plan); a call that needs more than KAM_STATIC_SCRATCH_BYTES returns
+ * KAM_ERR_INVALID_ARG with both figures in kam_last_error(NULL), and nothing is launched.  16 MiB covers BASELINE.json's
+ * configs[1] decode step (32 requests x 9 chunks, 28 query heads, head_dim 128: about 11 MB).
+ *
+ * First call on a device: the library looks up the array's device address (cudaGetSymbolAddress with that device current,
+ * once per device, cached).  That lookup may initialise the CUDA module, so make the first call on each device before any
+ * stream capture is begun on it and outside any region that must not synchronise; later calls only launch kernels.
+ * Sharing: there is ONE array per device, not one per stream or per caller.  Every call overwrites it and finds the previous
+ * call's contents in it; the call itself re-writes what it reads (the plan is rebuilt every time, the error word and the frequency
+ * table are reset by a small set-up kernel at the head of the call), so calls issued one after another on ONE stream are safe.  Two
+ * calls that may run concurrently on the GPU - different streams, or different threads / contexts of one process on the same
+ * device - race on the array and give garbage: serialise them (one stream, or an event between them).
+ * Errors: INVALID_ARG (NULL / misaligned pointers, bad sizes, scratch limit), UNSUPPORTED (layout), CUDA.  The reason is read with
+ * kam_last_error(NULL) (the slot kam_create's failures use: the calling thread's last context-free failure). */
+#define KAM_STATIC_SCRATCH_BYTES (16u << 20)
+kam_status kam_paged_decode_merge_static(const kam_layout *layout, const void *q, const kam_pool *pool,
+                                         const int32_t *block_tables, int32_t max_pages, const int32_t *chunk_starts,
+                                         const int64_t *chunk_offsets, const int32_t *n_chunks, int32_t max_chunks,
+                                         int32_t layer, int32_t batch, float sm_scale, void *out, float *lse, void *stream);
 
 #ifdef __cplusplus
 }

@@ -94,7 +94,10 @@ SIGNATURES = {
     "kam_window_decode": (i32, [vp, vp, C.POINTER(i32), i32, i32, C.c_float, vp, vp, vp]),
     "kam_paged_decode_merge_host": (i32, [vp, vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, vp, i32, i32,
                                           C.c_float, vp, vp, vp]),
+    "kam_paged_decode_merge_static": (i32, [C.POINTER(kam_layout), vp, C.POINTER(kam_pool), vp, i32, vp, vp, vp, i32, i32, i32,
+                                            C.c_float, vp, vp, vp]),
 }
+KAM_STATIC_SCRATCH_BYTES = 16 << 20
 
 _lib = None
 
@@ -371,6 +374,18 @@ class Context:
                                                  _ptr(n_chunks), max_chunks, _ptr(patches), int(layer), batch,
                                                  float(sm_scale), _ptr(out_host), _ptr(lse_host), _stream_ptr(stream)),
                self.h)
+
+
+def kam_paged_decode_merge_static(layout, q, pool, block_tables, chunk_starts, chunk_offsets, n_chunks, layer, sm_scale, out, lse,
+                                  stream=None):
+    """The fused decode without a context and without any device allocation inside the library (kamera.h): for hosts that have
+    given all their HBM to an allocator of their own, or that may not pay cudaMalloc's device-wide synchronisation.  Scratch is
+    the library's static 16 MiB device array - shared by every caller on the device, so calls must be ordered on one stream."""
+    batch, max_pages = block_tables.shape
+    max_chunks = chunk_starts.shape[1] - 1
+    _check(lib().kam_paged_decode_merge_static(C.byref(layout), _ptr(q), C.byref(pool.c), _ptr(block_tables), max_pages,
+                                               _ptr(chunk_starts), _ptr(chunk_offsets), _ptr(n_chunks), max_chunks, int(layer),
+                                               batch, float(sm_scale), _ptr(out), _ptr(lse), _stream_ptr(stream)), None)
 
 
 def patch_refs(refs, device, max_chunks=None):

@@ -1,7 +1,9 @@
 // Decode entry points: geometry, workspace, plan -> decode -> merge launches.  All arithmetic is in decode_kernel.cu.
 #include <algorithm>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "ctx.h"
@@ -445,3 +447,132 @@ kam_status kam_paged_decode_merge_host(kam_ctx* c, const void* q_host, const kam
 }
 
 }  // extern "C"
+
+// =====================================================================================================================
+// kam_paged_decode_merge_static: the fused decode for callers that may not allocate device memory (kamera.h).
+//
+// Everything the decode needs beyond the caller's inputs and outputs - frequency table, plan, cos/sin rows, per-segment
+// partials - is carved out of ONE file-scope device array.  In this file's HOST code the name `g_static_scratch` is only a
+// handle for the runtime (handing it to a kernel as a pointer would pass a host address): the device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current.  DEVICE code of this file (the set-up kernel below)
+// names the array directly.
+namespace {
+
+constexpr size_t kStaticHdrBytes = 256;           // [0] int32: malformed-record counter the decode kernels may bump
+constexpr int kStaticMaxFreq = 128;               // rope_dim <= 256
+constexpr size_t kStaticFreqOff = kStaticHdrBytes;
+constexpr size_t kStaticWsOff = 4096;             // plan | cos/sin | partials start here (ws_layout offsets are relative to it)
+static_assert(kStaticFreqOff + kStaticMaxFreq * sizeof(double) <= kStaticWsOff, "header region");
+
+static __device__ __align__(256) unsigned char g_static_scratch[KAM_STATIC_SCRATCH_BYTES];
+
+struct StaticFreq { double f[kStaticMaxFreq]; int32_t n; };
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;                           // guards the two caches below (the entry may be called from several threads)
+void* g_static_dev_ptr[kStaticMaxDevices] = {};   // device address of g_static_scratch, per device ordinal
+struct StaticGeomCache { bool ok = false; int dev = -1; int sm_count = 0; kam_layout lay{}; DecodeGeom g{}; } g_static_geom;
+
+}  // namespace
+
+namespace kam {
+// Head of every call: the array keeps whatever the previous call (any caller, any layout) left in it, so the two things the
+// later kernels read without writing first are reset here - the error word to zero, the frequency table to this layout's.
+__global__ void __launch_bounds__(kStaticMaxFreq) kam_static_setup_kernel(const __grid_constant__ StaticFreq t) {
+  if (threadIdx.x == 0) *reinterpret_cast<int32_t*>(g_static_scratch) = 0;
+  if (threadIdx.x < t.n) reinterpret_cast<double*>(g_static_scratch + kStaticFreqOff)[threadIdx.x] = t.f[threadIdx.x];
+}
+}  // namespace kam
+
+extern "C" kam_status kam_paged_decode_merge_static(const kam_layout* layout, const void* q, const kam_pool* pool,
+                                                    const int32_t* block_tables, int32_t max_pages, const int32_t* chunk_starts,
+                                                    const int64_t* chunk_offsets, const int32_t* n_chunks, int32_t max_chunks,
+                                                    int32_t layer, int32_t batch, float sm_scale, void* out, float* lse,
+                                                    void* stream) {
+  // ---- arguments (errors go to the context-free slot kam_last_error(NULL) reads)
+  if (!layout || !pool) return fail(nullptr, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge_static: layout / pool is NULL");
+  const kam_layout& L = *layout;
+  if (L.n_layers < 1 || L.n_layers > KAM_MAX_LAYERS || L.n_kv_heads < 1 || L.n_q_heads < 1 || L.n_q_heads % L.n_kv_heads ||
+      L.page_size < 1 || L.rope_dim < 0 || L.rope_dim % 2 || L.rope_off < 0 || L.rope_off + L.rope_dim > L.row_dim ||
+      (L.rope_style != KAM_ROPE_HALF && L.rope_style != KAM_ROPE_INTERLEAVED) || !(L.rope_theta > 0))
+    return fail(nullptr, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge_static: malformed layout");
+  if (!L.has_v) return fail(nullptr, KAM_ERR_UNSUPPORTED, "kam_paged_decode_merge_static: MLA decode needs tensor maps in device memory; use a context");
+  if (L.rope_dim / 2 > kStaticMaxFreq) return fail(nullptr, KAM_ERR_UNSUPPORTED, "kam_paged_decode_merge_static: rope_dim > %d", 2 * kStaticMaxFreq);
+  if (!pool->k_layers || !pool->v_layers || pool->num_pages < 1) return fail(nullptr, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge_static: bad pool");
+  if (!q || !out || !lse || !block_tables || !chunk_starts || !n_chunks) return fail(nullptr, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge_static: NULL argument");
+  if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(nullptr, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge_static: q and out must be 16-byte aligned");
+  if (layer < 0 || layer >= L.n_layers) return fail(nullptr, KAM_ERR_INVALID_ARG, "layer %d outside [0, %d)", layer, L.n_layers);
+  if (batch < 0 || max_pages < 1 || max_chunks < 1) return fail(nullptr, KAM_ERR_INVALID_ARG, "bad batch / max_pages / max_chunks");
+  if (batch == 0) return KAM_OK;
+  if ((long long)batch * max_chunks > (1ll << 24)) return fail(nullptr, KAM_ERR_INVALID_ARG, "batch * max_chunks too large");
+
+  // ---- once per device: where the array lives; per (device, layout): the kernel geometry.  No allocation in either.
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "no CUDA device: libkamera has no CPU fallback");
+  if (dev < 0 || dev >= kStaticMaxDevices) return fail(nullptr, KAM_ERR_UNSUPPORTED, "device ordinal %d beyond %d", dev, kStaticMaxDevices - 1);
+  void* base = nullptr;
+  DecodeGeom g;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_dev_ptr[dev]) {
+      void* ptr = nullptr;
+      e = cudaGetSymbolAddress(&ptr, g_static_scratch);        // the current device's copy of the array
+      if (e != cudaSuccess || !ptr) return cuda_fail(nullptr, e, "cudaGetSymbolAddress(static decode scratch)");
+      g_static_dev_ptr[dev] = ptr;
+    }
+    base = g_static_dev_ptr[dev];
+    if (!(g_static_geom.ok && g_static_geom.dev == dev && memcmp(&g_static_geom.lay, &L, sizeof L) == 0)) {
+      // decode_geom wants a context for the layout, the options and the SM count: a host-only one on the stack, with the
+      // tensor-map path switched off (maps would need device memory) - it owns nothing on the device
+      kam_ctx tmp;
+      tmp.lay = L; tmp.cuda_ok = true; tmp.opt.dec_tma = 0;
+      if ((e = cudaDeviceGetAttribute(&tmp.sm_count, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+        return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(SM count)");
+      const void* tmaps = nullptr;
+      const kam_status s = decode_geom(&tmp, pool, 0, &g, &tmaps);
+      if (s != KAM_OK) return fail(nullptr, s, "kam_paged_decode_merge_static: %s", tmp.err.c_str());
+      g_static_geom.ok = true; g_static_geom.dev = dev; g_static_geom.sm_count = tmp.sm_count; g_static_geom.lay = L; g_static_geom.g = g;
+    }
+    g = g_static_geom.g;
+  }
+
+  // ---- the size limit, checked before anything is launched
+  const int N = batch * max_chunks;
+  const WsLayout w = ws_layout(g, N, batch);
+  if (kStaticWsOff + w.total > (size_t)KAM_STATIC_SCRATCH_BYTES)
+    return fail(nullptr, KAM_ERR_INVALID_ARG, "kam_paged_decode_merge_static: batch %d x max_chunks %d needs %zu bytes of scratch, the static array has %u "
+                "(KAM_STATIC_SCRATCH_BYTES); split the batch or use a context", batch, max_chunks, kStaticWsOff + w.total, KAM_STATIC_SCRATCH_BYTES);
+
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  char* ws = static_cast<char*>(base) + kStaticWsOff;
+  StaticFreq fr{};
+  fr.n = L.rope_dim / 2;
+  for (int i = 0; i < fr.n; ++i) fr.f[i] = pow(L.rope_theta, -2.0 * (double)i / L.rope_dim);     // f_i as kam_create writes it (R-2)
+  kam_static_setup_kernel<<<1, kStaticMaxFreq, 0, st>>>(fr);
+
+  DecodeParams p{};
+  p.q = q; p.pool_k_layers = pool->k_layers; p.pool_v_layers = pool->v_layers; p.layer = layer;
+  p.block_tables = block_tables; p.tmaps = nullptr;
+  {
+    kam_ctx tmp;                                                   // plan_of only takes the frequency table from it
+    tmp.d_inv_freq = reinterpret_cast<double*>(static_cast<char*>(base) + kStaticFreqOff);
+    p.plan = plan_of(&tmp, ws, w, N, batch);
+  }
+  p.plan.block_tables = block_tables;
+  p.patches = nullptr; p.err = static_cast<int32_t*>(base);
+  p.part_o = reinterpret_cast<float*>(ws + w.part_o);
+  p.part_lse = reinterpret_cast<float*>(ws + w.part_lse);
+  p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.out_f32 = 0;
+  p.plan_fresh = 1;
+  DecodeCsr csr{};
+  csr.chunk_starts = chunk_starts; csr.chunk_offsets = reinterpret_cast<const long long*>(chunk_offsets); csr.n_chunks = n_chunks;
+  csr.max_chunks = max_chunks; csr.max_pages = max_pages; csr.enabled = 1; csr.has_patches = 0;
+  // plain stream order between the four kernels (no programmatic dependent launch): each one starts after the one before it has
+  // finished writing the array
+  launch_decode_plan(g, p.plan, csr, st);
+  launch_decode(g, p, false, st);
+  launch_decode_merge(g, p, false, st);
+  if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(nullptr, e, "kam_paged_decode_merge_static launch");
+  return KAM_OK;
+}

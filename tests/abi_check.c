@@ -27,6 +27,7 @@ int main(void) {
   SZ(kam_stats); OFF(kam_stats, pages_free); OFF(kam_stats, pages_total); OFF(kam_stats, table_entries_written);
   OFF(kam_stats, chunks_live); OFF(kam_stats, kernels_launched); OFF(kam_stats, device_errors); OFF(kam_stats, generic_launches);
   printf("const KAM_MAX_RANK %d\nconst KAM_MAX_LAYERS %d\n", KAM_MAX_RANK, KAM_MAX_LAYERS);
+  printf("const KAM_STATIC_SCRATCH_BYTES %u\n", KAM_STATIC_SCRATCH_BYTES);
   printf("enum KAM_ERR_CUDA %d\nenum KAM_MLA %d\nenum KAM_ROPE_INTERLEAVED %d\nenum KAM_PATCH_CANONICAL_FRAME %d\nenum KAM_BACK %d\nenum KAM_F32 %d\n",
          (int)KAM_ERR_CUDA, (int)KAM_MLA, (int)KAM_ROPE_INTERLEAVED, (int)KAM_PATCH_CANONICAL_FRAME, (int)KAM_BACK, (int)KAM_F32);
 
