@@ -192,9 +192,13 @@ kam_status kam_rotate_inplace(kam_ctx *ctx, const kam_pool *pool, const int32_t 
  * (U contiguous [T][H][rank]).  The library copies them to device staging it owns (H2D on `stream`), then runs
  * kam_relocate_patch.  Pinned host memory makes the copies asynchronous.  Copies whose host source continues the previous
  * one are merged: a chunk kept as ONE slab in the order (per layer: K, V, U_k, W_k, U_v, W_v) crosses PCIe in one transfer.
- * The copies run on a stream of the library's own into one of two staging buffers, so the transfer of one call overlaps the
- * kernel of the previous one; the kernel is ordered behind its copies on `stream` as usual (option host_copy_overlap = 0:
- * one buffer, everything on `stream`).  The host arrays must stay valid until `stream` has passed this call. */
+ * By default the copies are enqueued on `stream` like everything else, so host arrays that earlier work on `stream` is still
+ * filling (the D2H copy of an eviction to the host store, followed by its recall) are read in stream order.
+ * Option host_copy_overlap = 1 (opt-in) moves the copies to a stream of the library's own and alternates two staging buffers, so
+ * the transfer of one call overlaps the kernel of the previous one; the kernel still waits for its copies on `stream`.  That copy
+ * stream is NOT ordered behind `stream`: with the option on, the CONTENTS of the host arrays must be final when the call is made
+ * (written by the host, or by device work the caller has already synchronised with).
+ * Either way the host arrays must stay valid until `stream` has passed this call. */
 kam_status kam_relocate_patch_host(kam_ctx *ctx, const kam_pool *pool, const int32_t *block_table /* device */,
                                    int64_t dst_token_start, int32_t n_tokens, int64_t p_base, int64_t p_target,
                                    const void *const *k_host, const void *const *v_host,
@@ -302,6 +306,8 @@ kam_status kam_paged_decode_plan(kam_ctx *ctx, const kam_pool *pool, const int32
  *               (n_q_tokens > N_b) gives out = 0, lse = -inf.
  * The per-chunk softmax states are merged in registers by the same log-sum-exp state merge as the decode, online.
  * No on-read patch here: on this path the patches were materialised by kam_relocate_patch / kam_admit.
+ * Inconsistent paging metadata is never dereferenced: a cached token whose page index is >= max_pages or whose block-table entry
+ * lies outside [0, pool->num_pages) reads as a zero key / value row and is counted (at least once) in kam_stats.device_errors.
  * Requires a bf16 MHA / GQA pool, head_dim 64 or 128 rotated over the whole head; else KAM_ERR_UNSUPPORTED.
  * Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
 kam_status kam_paged_prefill_merge(kam_ctx *ctx, const void *q, const kam_pool *pool, const int32_t *block_tables,

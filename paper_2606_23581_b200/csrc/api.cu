@@ -672,8 +672,7 @@ kam_status kam_relocate_patch_host(kam_ctx* c, const kam_pool* pool, const int32
   // copies -> event; caller's stream: wait for that event -> kernel -> event "consumed".   ("host_copy_overlap" = 0: one
   // buffer, everything on the caller's stream.)
   const bool overlap = c->opt.host_copy_overlap && c->copy_stream;
-  const int hb = overlap ? c->hstage_next : 0;
-  if (overlap) c->hstage_next ^= 1;
+  const int hb = overlap ? c->hstage_next : 0;      // the buffers alternate only once a call got as far as its kernel (below)
   if ((s = grow_device(c, &c->d_hstage[hb], &c->hstage_cap[hb], per_layer * L.n_layers, "cudaMalloc(host-chunk staging)", st)) != KAM_OK) return s;
   cudaStream_t cs = overlap ? c->copy_stream : st;
   cudaError_t e = cudaSuccess;
@@ -726,7 +725,10 @@ kam_status kam_relocate_patch_host(kam_ctx* c, const kam_pool* pool, const int32
   hs[0] = HostReloc{block_table, dst_token_start, p_target - p_base, ch.k_layers, ch.v_layers, rank ? &pa : nullptr, rank, n_tokens, 0};
   s = run_reloc(c, pool, hs, st);
   staging_release(sg, st);          // the pointer tables are released behind the kernel that reads them
-  if (overlap && cudaEventRecord(c->ev_consumed[hb], st) == cudaSuccess) c->hstage_used[hb] = true;
+  if (overlap) {
+    if (cudaEventRecord(c->ev_consumed[hb], st) == cudaSuccess) c->hstage_used[hb] = true;
+    c->hstage_next = hb ^ 1;
+  }
   return s;
 }
 

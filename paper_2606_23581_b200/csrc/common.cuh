@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace kam {
 
 // ---------------------------------------------------------------- mbarrier + bulk async copy (TMA engine, 1-D)
@@ -117,6 +119,16 @@ __device__ __forceinline__ void ldmatrix_x4_trans(uint32_t& r0, uint32_t& r1, ui
 // streaming 128-bit global store (the pool page is written once and not re-read by this kernel)
 __device__ __forceinline__ void st_global_v4(void* p, const uint4& v) {
   asm volatile("st.global.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// Function attributes (cudaFuncSetAttribute) belong to a kernel ON ONE DEVICE: a process that uses the library on several GPUs must
+// set them on each.  `done` is the caller's per-kernel-family bit mask of device ordinals already served; true = the current
+// device has not been served yet (ordinals beyond 63 and a failing cudaGetDevice answer true every time: setting again is harmless).
+inline bool first_launch_on_this_device(std::atomic<uint64_t>& done) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev > 63) return true;
+  const uint64_t bit = 1ull << dev;
+  return (done.fetch_or(bit, std::memory_order_relaxed) & bit) == 0;
 }
 
 }  // namespace kam

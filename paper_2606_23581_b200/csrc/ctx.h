@@ -39,7 +39,8 @@ struct Options {
   int use_pdl = 1;             // "decode_pdl": programmatic dependent launch between plan, decode and merge
   int dec_tma = 1;             // "decode_tma": pool pages arrive as TMA tensor-map boxes (0: per-token bulk copies)
   int prefill_tc = 1;          // "prefill_tcgen05": the multi-query readout runs on tcgen05 / tensor memory (0: the mma.sync kernel)
-  int host_copy_overlap = 1;   // "host_copy_overlap": kam_relocate_patch_host copies chunk c+1 under the kernel of chunk c
+  int host_copy_overlap = 0;   // "host_copy_overlap": kam_relocate_patch_host copies chunk c+1 under the kernel of chunk c, on a stream
+                               // of the library's own that is NOT ordered behind the caller's stream - opt-in, for host data that is final
   int host_sync = 0;           // "host_entries_sync": kam_paged_decode_merge_host ends with a stream synchronise
 };
 
@@ -78,6 +79,9 @@ struct kam_ctx {
   size_t ws_cap = 0;
   bool decplan_valid = false;                  // a plan pinned by kam_paged_decode_plan sits in d_ws
   alignas(8) unsigned char decplan_key[64] = {};
+  bool decplan_unread = false;                 // the pinned plan's kernel was enqueued and no decode has been launched behind it yet:
+                                               // that first decode may not read the plan before griddepcontrol.wait
+  bool winplan_unread = false;                 // same for the window plan (kam_window_plan followed by kam_window_decode)
   void* d_ws_win = nullptr;                    // window calls: laid out once for max_requests x max_chunks (graph-stable)
   size_t ws_win_cap = 0;
   uint64_t winplan_epoch = ~0ull;              // window epoch the plan in d_ws was built for (~0 = none)

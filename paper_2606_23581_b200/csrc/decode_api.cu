@@ -200,13 +200,15 @@ static kam_status decode_stateless(kam_ctx* c, const void* q, const kam_pool* po
     launch_decode_plan(g, p.plan, csr, st);
     ++c->kernels_launched;
     c->decplan_valid = plan_only;
-    if (plan_only) memcpy(c->decplan_key, &key, sizeof key);
+    if (plan_only) { memcpy(c->decplan_key, &key, sizeof key); c->decplan_unread = true; }
   }
   if (!plan_only) {
     // a plan written by the kernel just before this one: with programmatic dependent launch only the decode kernel's prologue
     // (barrier setup, shared-memory carve-up, launch latency) overlaps the plan kernel - plan_fresh makes it wait before the
-    // first plan read.  A reused plan is older than anything on the stream that could still be writing it.
-    p.plan_fresh = reuse ? 0 : 1;
+    // first plan read.  A reused plan is older than anything on the stream that could still be writing it - except on the FIRST
+    // decode behind kam_paged_decode_plan, whose plan kernel may be the launch right before this one and still running.
+    p.plan_fresh = (reuse && !c->decplan_unread) ? 0 : 1;
+    c->decplan_unread = false;
     if (g.mla) launch_mla_ts_decode(g, p, pdl, st);
     else launch_decode(g, p, pdl, st);
     launch_decode_merge(g, p, pdl, st);
@@ -325,6 +327,7 @@ static kam_status window_plan(kam_ctx* c, const int32_t* req_ids, int32_t batch,
   launch_decode_plan(g, pl, csr, st);
   ++c->kernels_launched;
   if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(c, e, "decode plan launch");
+  c->winplan_unread = true;
   c->winplan_epoch = c->win->epoch();
   c->winplan_reqs.assign(req_ids, req_ids + batch);
   c->winplan_chunks = N;
@@ -370,9 +373,13 @@ kam_status kam_window_decode(kam_ctx* c, const void* q, const int32_t* req_ids, 
   p.part_lse = reinterpret_cast<float*>(static_cast<char*>(c->d_ws_win) + w.part_lse);
   p.sm_scale = sm_scale; p.out = out; p.lse = lse; p.err = c->d_err;
   const bool pdl = c->opt.use_pdl != 0;
-  // with a plan from an earlier call the decode prologue may overlap whatever precedes it on the stream (it only reads the plan)
-  if (g.mla) launch_mla_ts_decode(g, p, cached && pdl, st);
-  else launch_decode(g, p, cached && pdl, st);
+  // with a plan an earlier decode already ran on, the decode prologue may overlap whatever precedes it on the stream (it only reads
+  // the plan).  The first decode behind a plan kernel - built by this call, or by kam_window_plan just before it - starts in plain
+  // stream order: that kernel may be the launch right before this one and still writing the plan.
+  const bool settled = cached && !c->winplan_unread;
+  c->winplan_unread = false;
+  if (g.mla) launch_mla_ts_decode(g, p, settled && pdl, st);
+  else launch_decode(g, p, settled && pdl, st);
   launch_decode_merge(g, p, pdl, st);
   c->kernels_launched += 2;
   cudaError_t e = cudaGetLastError();
@@ -407,6 +414,7 @@ kam_status kam_paged_prefill_merge(kam_ctx* c, const void* q, const kam_pool* po
   p.P = L.page_size; p.P_shift = -1;
   for (int sft = 0; sft < 31; ++sft) if ((1 << sft) == p.P) p.P_shift = sft;
   p.max_pages = max_pages; p.max_chunks = max_chunks; p.causal = causal; p.rope_style = L.rope_style; p.sm_scale = sm_scale;
+  p.num_pages = pool->num_pages; p.err = c->d_err;
   if (c->opt.prefill_tc && sm_scale > 0.f) launch_prefill_tc(p, L.row_dim, static_cast<cudaStream_t>(stream));
   else launch_prefill(p, L.row_dim, static_cast<cudaStream_t>(stream));
   ++c->kernels_launched;

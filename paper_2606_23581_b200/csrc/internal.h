@@ -265,6 +265,9 @@ struct PrefillParams {
   const double* inv_freq;        // [D / 2]
   int32_t layer, batch, Tq, Hq, H, G, P, P_shift, max_pages, max_chunks, causal, rope_style;
   float sm_scale;
+  int32_t num_pages;             // pool pages: a token whose page index is >= max_pages or whose table entry lies outside
+                                 // [0, num_pages) is never dereferenced - it reads as a zero row and is counted in *err
+  int32_t* err;                  // device counter (kam_stats.device_errors)
 };
 void launch_prefill(const PrefillParams& p, int D, cudaStream_t st);        // mma.sync formulation (prefill_kernel.cu)
 void launch_prefill_tc(const PrefillParams& p, int D, cudaStream_t st);     // tcgen05 / tensor-memory formulation (prefill_tc_kernel.cu)

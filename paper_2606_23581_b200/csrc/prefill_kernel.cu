@@ -125,11 +125,17 @@ __global__ void __launch_bounds__(kPfThreads, 2) kam_paged_prefill_kernel(const 
     for (int i = 0; i < kPfN / RPP; ++i) {
       const int r = lr0 + i * RPP;
       const int tok = tl.pos + r;
-      const bool valid = tok < tl.hi;
+      bool valid = tok < tl.hi;
       size_t src = 0;
       if (valid) {
         const int pg = p.P_shift >= 0 ? (tok >> p.P_shift) : tok / p.P;
-        src = (static_cast<size_t>(bt[pg]) * p.P + (tok - pg * p.P)) * tok_bytes + head_off + lc * 16;     // A1 slot mapping
+        const int page = pg < p.max_pages ? bt[pg] : -1;
+        if (page >= 0 && page < p.num_pages) {
+          src = (static_cast<size_t>(page) * p.P + (tok - pg * p.P)) * tok_bytes + head_off + lc * 16;     // A1 slot mapping
+        } else {                                              // inconsistent metadata: a zero row, never a wild read
+          valid = false;
+          if (lc == 0 && (tok == tl.pos || tok == pg * p.P)) atomicAdd(p.err, 1);
+        }
       }
       const uint32_t d = static_cast<uint32_t>(buf * TILEB + r * ROWB + ((lc ^ (r & 7)) << 4));
       cp_async_16(sK_u + d, pool_k + src, valid);
@@ -317,11 +323,10 @@ int prefill_smem_bytes(int D) { return kPfM * D * 2 + 4 * kPfN * D * 2 + (D / 2)
 void launch_prefill(const PrefillParams& p, int D, cudaStream_t st) {
   const int smem = prefill_smem_bytes(D);
   dim3 grid((p.Tq * p.G + kPfM - 1) / kPfM, p.H, p.batch);
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<uint64_t> attr_done{0};          // per device: the attribute is not shared between GPUs
+  if (first_launch_on_this_device(attr_done)) {
     cudaFuncSetAttribute(kam_paged_prefill_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, prefill_smem_bytes(128));
     cudaFuncSetAttribute(kam_paged_prefill_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, prefill_smem_bytes(64));
-    attr_set = true;
   }
   if (D == 128) kam_paged_prefill_kernel<128><<<grid, kPfThreads, smem, st>>>(p);
   else kam_paged_prefill_kernel<64><<<grid, kPfThreads, smem, st>>>(p);

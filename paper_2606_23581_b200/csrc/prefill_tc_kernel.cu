@@ -220,7 +220,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
         const int tok = cur.pos + wrow0 + (lane & (RPW - 1));
         if (tok < cur.hi) {
           const int pg = p.P_shift >= 0 ? (tok >> p.P_shift) : tok / p.P;
-          myslot = bt[pg] * p.P + (tok - pg * p.P);
+          const int page = pg < p.max_pages ? bt[pg] : -1;
+          if (page >= 0 && page < p.num_pages) myslot = page * p.P + (tok - pg * p.P);
+          else if (lane < RPW && (tok == cur.pos + wrow0 || tok == pg * p.P)) atomicAdd(p.err, 1);   // a zero row, never a wild read
         }
       }
       if (issued >= kTcStages) mbar_wait(&bars[BAR_KV_EMPTY + st], ((issued / kTcStages) - 1) & 1);
@@ -475,9 +477,13 @@ __global__ void __launch_bounds__(kTcThreads, 1) kam_paged_prefill_tc_kernel(con
       } else {
         fence_proxy_async();
       }
+      // O_DONE is ONE barrier read by parity: PV(t - 1)'s completion must be observed BEFORE this thread lets PV(t) go (its P_FULL
+      // arrival below).  In the other order a thread held up between the two could see PV(t - 1) and PV(t) both complete - the
+      // parity back where it was - and wait for PV(t + 1), which needs this thread's own next arrival: a hang.  Behind the P
+      // write the wait has long been satisfied, so it costs one poll.
+      if (o_pending) { mbar_wait(&bars[BAR_O_DONE], o_phase); o_phase ^= 1; tcf_after(); }
       tcf_before();
       mbar_arrive(&bars[BAR_P_FULL + (t & 1)]);
-      if (o_pending) { mbar_wait(&bars[BAR_O_DONE], o_phase); o_phase ^= 1; tcf_after(); }
       more = cur.next();
       ++t;
     }
@@ -519,11 +525,10 @@ int prefill_tc_smem_bytes(int D) { return 1024 + 2 * kTcRows * D * 2 + (kTcPInTm
 void launch_prefill_tc(const PrefillParams& p, int D, cudaStream_t st) {
   const int smem = prefill_tc_smem_bytes(D);
   dim3 grid((p.Tq * p.G + kTcRows - 1) / kTcRows, p.H, p.batch);
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<uint64_t> attr_done{0};          // per device: the attribute is not shared between GPUs
+  if (first_launch_on_this_device(attr_done)) {
     cudaFuncSetAttribute(kam_paged_prefill_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, prefill_tc_smem_bytes(128));
     cudaFuncSetAttribute(kam_paged_prefill_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, prefill_tc_smem_bytes(64));
-    attr_set = true;
   }
   if (D == 128) kam_paged_prefill_tc_kernel<128><<<grid, kTcThreads, smem, st>>>(p);
   else kam_paged_prefill_tc_kernel<64><<<grid, kTcThreads, smem, st>>>(p);

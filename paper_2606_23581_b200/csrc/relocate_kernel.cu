@@ -598,11 +598,10 @@ kam_relocate_admit_kernel(const __grid_constant__ RelocGeom g, const __grid_cons
 }
 
 void launch_relocate_fast(const RelocGeom& g, const RelocParams& p, const RelocInline& inl, const RelocPages* pages, int grid, bool pdl, cudaStream_t st) {
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<uint64_t> attr_done{0};          // per device: the attribute is not shared between GPUs
+  if (first_launch_on_this_device(attr_done)) {
     cudaFuncSetAttribute(kam_relocate_patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     cudaFuncSetAttribute(kam_relocate_admit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    attr_set = true;
   }
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kRelocThreads); cfg.dynamicSmemBytes = g.smem_bytes; cfg.stream = st;

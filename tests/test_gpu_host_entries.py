@@ -35,9 +35,9 @@ def _host_lists(ch, mode):
     return [out.get(x) or None for x in names], out
 
 
-@pytest.mark.parametrize("mode", ["pinned", "slab", "pageable"])
+@pytest.mark.parametrize("mode,overlap", [("pinned", 0), ("pinned", 1), ("slab", 0), ("slab", 1), ("pageable", 0)])
 @pytest.mark.parametrize("cfg_id,m", [(2, 16), (3, 16), (2, 0)])
-def test_relocate_patch_host_matches_oracle(cfg_id, m, mode):
+def test_relocate_patch_host_matches_oracle(cfg_id, m, mode, overlap):
     cfg = CONFIGS[cfg_id]
     L, T, P = 3, 272, cfg.page_size
     rng = np.random.Generator(np.random.PCG64(400 + cfg_id + m))
@@ -47,14 +47,42 @@ def test_relocate_patch_host_matches_oracle(cfg_id, m, mode):
     bt_h = make_block_table(rng, n_pages, n_pages + 3)
     pool = par.make_pool(cfg, L, n_pages + 3, torch.bfloat16)
     ctx = kam.Context(par.layout_of(cfg, L), pool)
+    ctx.kam_set_option("host_copy_overlap", overlap)                # 1: the library's own copy stream + two staging buffers (opt-in)
     (k, v, uk, wk, uv, wv), keep = _host_lists(ch, mode)
     p_target = 31337
-    for _ in range(2):                                             # twice: the staging buffer and its pointer tables are reused
+    for _ in range(2 + overlap):                                             # twice: the staging buffer and its pointer tables are reused
         ctx.kam_relocate_patch_host(torch.from_numpy(bt_h).cuda(), dst0, T, 0, p_target, k, v, uk, wk, uv, wv, m)
     torch.cuda.synchronize()
     st = par.check_relocated(cfg, pool, ch, bt_h, dst0, p_target, m)
     assert st["fail"] == 0
     assert par.untouched_pages_intact(pool, bt_h, L)
+    ctx.close()
+
+
+def test_relocate_patch_host_reads_stream_ordered_host_data_in_stream_order():
+    """The evict-to-host-then-recall pattern of P:88: the pinned host slab is still being FILLED by a device-to-host copy enqueued on
+    the caller's stream (held back behind a long kernel) when kam_relocate_patch_host is called.  With the default options the
+    library's copies are ordered on that stream, so the recall must see the evicted bits, not the slab's stale contents."""
+    cfg = CONFIGS[2]
+    L, T, P, m = 2, 256, cfg.page_size, 16
+    rng = np.random.Generator(np.random.PCG64(77))
+    ch = make_chunk(cfg, rng, n_tokens=T, n_layers=L, rank=m)
+    n_pages = T // P
+    bt_h = make_block_table(rng, n_pages, n_pages + 2)
+    pool = par.make_pool(cfg, L, n_pages + 2, torch.bfloat16)
+    ctx = kam.Context(par.layout_of(cfg, L), pool)
+    names = ("K", "V", "Uk", "Wk", "Uv", "Wv")
+    dev = {x: [ch[x][l].contiguous().cuda() for l in range(L)] for x in names}
+    host = {x: [torch.full(ch[x][l].shape, 3.0, dtype=ch[x][l].dtype).pin_memory() for l in range(L)] for x in names}   # stale contents
+    bt_d = torch.from_numpy(bt_h).cuda()
+    torch.cuda.synchronize()
+    torch.cuda._sleep(200_000_000)                                  # ~0.1 s of device time in front of the eviction copies
+    for x in names:
+        for l in range(L):
+            host[x][l].copy_(dev[x][l], non_blocking=True)          # "evict to the host store", stream-ordered
+    ctx.kam_relocate_patch_host(bt_d, 0, T, 0, 4242, *[host[x] for x in names], m)
+    torch.cuda.synchronize()
+    assert par.check_relocated(cfg, pool, ch, bt_h, 0, 4242, m)["fail"] == 0
     ctx.close()
 
 

@@ -279,3 +279,97 @@ def test_decode_over_a_callers_pool_gqa_and_mla():
                 o, l = att.attend_bruteforce(par.to_f64(q[b]), chunks, scale, par.rope_kw(cfg), **kw)
                 check_attention(par.to_f64(out)[b], par.to_f64(lse)[b], o, l, "%s request %d" % ("MLA" if mla else "GQA", b))
         ctx.close()
+
+
+@pytest.mark.parametrize("cfg_id", [2, 3])
+def test_first_decode_right_behind_the_plan_kernel(cfg_id):
+    """kam_paged_decode_plan followed AT ONCE by kam_paged_decode_merge on a fresh context (fresh workspace, no kernel between the
+    two): the plan kernel releases its dependents at its first instruction, so the decode launched behind it with programmatic
+    dependent launch must still not read the plan before it is complete.  Many chunks make the plan kernel long.  The result must
+    carry the bits of an unpinned call on another context, for GQA and for absorbed MLA, on repeated fresh contexts."""
+    cfg = CONFIGS[cfg_id].scaled(n_layers=1)
+    mla = not cfg.has_v
+    rng = _rng(70 + cfg_id)
+    P, D = cfg.page_size, cfg.row_dim
+    Dv = cfg.v_dim if mla else D
+    batch, max_chunks = 24, 40
+    lens = [[int(x) for x in rng.integers(1, 90, size=int(rng.integers(1, max_chunks + 1)))] for _ in range(batch)]
+    max_pages = max((sum(r) + P - 1) // P for r in lens) + 1
+    num_pages = batch * max_pages + 2
+    from synth import randn_device
+    shape = (num_pages, P, cfg.n_kv_heads, D)
+    pool = kam.Pool([randn_device(shape, 77, 1.0, torch.bfloat16, "cuda")], None if mla else [randn_device(shape, 78, 1.0, torch.bfloat16, "cuda")])
+    perm = make_block_table(rng, batch * max_pages, num_pages).reshape(batch, max_pages)
+    starts = np.zeros((batch, max_chunks + 1), np.int32); offs = np.zeros((batch, max_chunks), np.int64)
+    for b, row in enumerate(lens):
+        for c, n in enumerate(row):
+            starts[b, c + 1] = starts[b, c] + n; offs[b, c] = int(rng.integers(-5000, 5000)) * (c % 3 != 0)
+        starts[b, len(row) + 1:] = starts[b, len(row)]
+    ncs = torch.tensor([len(r) for r in lens], dtype=torch.int32, device="cuda")
+    bt_d, st_d, of_d = torch.from_numpy(perm).cuda(), torch.from_numpy(starts).cuda(), torch.from_numpy(offs).cuda()
+    q = torch.from_numpy(rng.standard_normal((batch, cfg.n_q_heads, D), dtype=np.float32)).to(torch.bfloat16).cuda()
+    scale = 192 ** -0.5 if mla else D ** -0.5
+    ref_o = torch.zeros((batch, cfg.n_q_heads, Dv), dtype=torch.bfloat16, device="cuda")
+    ref_s = torch.zeros((batch, cfg.n_q_heads), dtype=torch.float32, device="cuda")
+    ctx = kam.Context(par.layout_of(cfg, 1), pool)
+    ctx.kam_paged_decode_merge(q, bt_d, st_d, of_d, ncs, 0, scale, ref_o, ref_s)      # unpinned: plan, decode and merge in one call
+    torch.cuda.synchronize()
+    ctx.close()
+    b0 = int(np.argmax([len(r) for r in lens]))                                       # and the reference itself against the oracle
+    chunks, t0 = [], 0
+    for c, n in enumerate(lens[b0]):
+        chunks.append({"k": par.pool_rows(pool.k_layers[0], perm[b0], t0, n),
+                       "v": None if mla else par.pool_rows(pool.v_layers[0], perm[b0], t0, n), "delta": int(offs[b0, c])})
+        t0 += n
+    o, l = att.attend_bruteforce(par.to_f64(q[b0].cpu()), chunks, scale, par.rope_kw(cfg), **(dict(v_dim=Dv) if mla else {}))
+    check_attention(par.to_f64(ref_o)[b0], par.to_f64(ref_s)[b0], o, l, "reference request %d" % b0)
+    for rep in range(6):
+        ctx = kam.Context(par.layout_of(cfg, 1), pool)                                # fresh context: its workspace holds no older plan
+        out = torch.full_like(ref_o, 7.0); lse = torch.full_like(ref_s, 7.0)
+        torch.cuda.synchronize()
+        ctx.kam_paged_decode_plan(bt_d, st_d, of_d, ncs)
+        ctx.kam_paged_decode_merge(q, bt_d, st_d, of_d, ncs, 0, scale, out, lse)      # nothing between the plan kernel and this
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref_o) and torch.equal(lse, ref_s), "repetition %d" % rep
+        ctx.kam_paged_decode_merge(q, bt_d, st_d, of_d, ncs, 0, scale, out, lse)      # the settled plan: same bits again
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref_o) and torch.equal(lse, ref_s)
+        ctx.close()
+
+
+def test_first_window_decode_right_behind_kam_window_plan():
+    """The same sequence on the window path: an explicit kam_window_plan followed at once by kam_window_decode (the plan counts as
+    cached there, so the decode used to start under the plan kernel); against the oracle, on fresh contexts."""
+    cfg = CONFIGS[2].scaled(n_layers=1)
+    P, T, m, R, C = cfg.page_size, 64, 16, 8, 12
+    rng = _rng(91)
+    canon = [make_chunk(cfg, rng, n_tokens=T, n_layers=1) for _ in range(3)]
+    up = [par.upload_chunk(c) for c in canon]
+    n_pages = R * C * (T // P)
+    q = make_query(cfg, rng, R)
+    qd = q.cuda()
+    scale = cfg.row_dim ** -0.5
+    for rep in range(3):
+        pool = par.make_pool(cfg, 1, n_pages, torch.bfloat16)
+        ctx = kam.Context(par.layout_of(cfg, 1), pool, max_requests=R, max_chunks_per_request=C, max_pages_per_chunk=T // P)
+        ws = WindowStore(n_pages, P)
+        for r in range(R):
+            ctx.kam_window_open(r, 0); ws.open(r, 0)
+            for i in range(C - (r % 3)):
+                ctx.kam_admit(r, BACK, up[(r + i) % 3][0], up[(r + i) % 3][1], m, 1); ws.admit(r, BACK, T, 1)
+            ctx.kam_evict(r, FRONT, 0); ws.evict(r, FRONT, 0)                         # lazy: a pending offset rides in the plan
+        out = torch.full((R, cfg.n_q_heads, cfg.row_dim), 7.0, dtype=torch.bfloat16, device="cuda")
+        lse = torch.full((R, cfg.n_q_heads), 7.0, dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        ctx.kam_window_plan(list(range(R)))
+        ctx.kam_window_decode(qd, list(range(R)), 0, scale, out, lse)
+        torch.cuda.synchronize()
+        for r in (0, R - 1):
+            w = ws.export(r)
+            chunks = [{"k": par.pool_rows(pool.k_layers[0], w["block_table"], w["chunk_starts"][c], T),
+                       "v": par.pool_rows(pool.v_layers[0], w["block_table"], w["chunk_starts"][c], T), "delta": w["chunk_offsets"][c]}
+                      for c in range(len(w["chunk_offsets"]))]
+            o, l = att.attend_bruteforce(par.to_f64(q[r]), chunks, scale, par.rope_kw(cfg))
+            check_attention(par.to_f64(out)[r], par.to_f64(lse)[r], o, l, "repetition %d request %d" % (rep, r))
+        assert not bool((lse == 7.0).any())                                           # every (request, head) was written
+        ctx.close()
