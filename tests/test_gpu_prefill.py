@@ -119,6 +119,67 @@ def test_head_dim_64_and_interleaved_pairs(kernel):
     _run(CONFIGS[2].scaled(n_q_heads=8, n_kv_heads=4), [[90, 40]], [[-555, 0]], 40, 1, 509, style=reuse.INTERLEAVED, kernel=kernel)
 
 
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_bench_shape_many_waves_sampled(kernel):
+    """The shape bench.py's extras time (8 requests x 512 appended rows over 8 recalled 1024-token chunks + the turn, config 2's
+    28 / 4 heads): 896 CTAs of the tcgen05 kernel (one per SM: 6 waves, so tensor memory is allocated after an earlier CTA's
+    dealloc and the barrier words are re-initialised over used shared memory), 1792 of the mma.sync kernel.  The oracle evaluates
+    8 rows of EVERY request (first / last row tiles included): 64 (request, row) pairs."""
+    cfg = CONFIGS[2]
+    lens = [[1024] * 8 + [512] for _ in range(8)]
+    deltas = [[(-1) ** c * (1000 * b + 37 * c) for c in range(8)] + [0] for b in range(8)]
+    rows = [0, 1, 17, 18, 255, 300, 493, 511]                     # G = 7: rows 0-18 sit in row tile 0, 493-511 in the last one
+    _run(cfg, lens, deltas, 512, 1, 510, rows=rows, kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_three_waves_with_chunk_ends_inside_tiles(kernel):
+    """11 requests x 200 rows x 7 query heads per KV head = 11 row tiles x 4 KV heads x 11 requests = 484 CTAs (> 3 x 148), ragged
+    chunks whose ends fall inside 64-token tiles in every request, offsets pending on most of them."""
+    cfg = CONFIGS[2]
+    rng = np.random.Generator(np.random.PCG64(511))
+    lens, deltas = [], []
+    for b in range(11):
+        n = [int(x) for x in rng.integers(1, 400, size=4)] + [200]
+        lens.append(n)
+        deltas.append([int(x) for x in rng.integers(-30000, 30000, size=4)] + [0])
+    _run(cfg, lens, deltas, 200, 1, 512, rows=[0, 9, 10, 100, 191, 199], kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_out_of_range_block_table_entries_read_as_zero_rows(kernel):
+    """Inconsistent paging metadata must never be dereferenced (kamera.h): a block-table entry outside [0, num_pages) - here far
+    beyond the pool and negative - reads as zero key / value rows and is counted in kam_stats.device_errors.  Checked without the
+    oracle: the result must carry the bits of the same call with those entries pointing at a page that IS all zeros."""
+    cfg = CONFIGS[2].scaled(n_q_heads=8, n_kv_heads=4)
+    P, D, Hq, Tq = cfg.page_size, cfg.row_dim, cfg.n_q_heads, 40
+    rng = np.random.Generator(np.random.PCG64(513))
+    n_tok, max_pages = 300, 20                                    # 19 pages used
+    num_pages = max_pages + 2
+    pool = _fill_pool(cfg, 1, num_pages, 513)
+    zero_page = num_pages - 1
+    pool.k_layers[0][zero_page].zero_(); pool.v_layers[0][zero_page].zero_()
+    ctx = kam.Context(par.layout_of(cfg, 1), pool)
+    ctx.kam_set_option("prefill_tcgen05", KERNELS[kernel])
+    perm = make_block_table(rng, max_pages, num_pages - 1).reshape(1, max_pages)
+    starts = torch.tensor([[0, 130, n_tok]], dtype=torch.int32, device="cuda")
+    offs = torch.tensor([[777, 0]], dtype=torch.int64, device="cuda")
+    ncs = torch.tensor([2], dtype=torch.int32, device="cuda")
+    q = torch.from_numpy(rng.standard_normal((1, Tq, Hq, D), dtype=np.float32)).to(torch.bfloat16).cuda()
+    res = []
+    for bad in ((zero_page, zero_page), (num_pages + 1000, -3)):
+        bt = perm.copy()
+        bt[0, 2], bt[0, 11] = bad
+        out = torch.full((1, Tq, Hq, D), 7.0, dtype=torch.bfloat16, device="cuda")
+        lse = torch.full((1, Tq, Hq), 7.0, dtype=torch.float32, device="cuda")
+        ctx.kam_paged_prefill_merge(q, torch.from_numpy(bt).cuda(), starts, offs, ncs, 0, 1, D ** -0.5, out, lse)
+        torch.cuda.synchronize()
+        res.append((out, lse, ctx.kam_get_stats()["device_errors"]))
+    assert res[0][2] == 0 and res[1][2] >= 2
+    assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])
+    ctx.close()
+
+
 def test_unsupported_and_invalid_arguments():
     cfg = CONFIGS[3]                                              # MLA: not covered by the multi-query kernel
     pool = kam.Pool([torch.zeros((4, cfg.page_size, 1, cfg.row_dim), dtype=torch.bfloat16, device="cuda")], None)
