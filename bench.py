@@ -670,16 +670,232 @@ def extras(wl, device, peak):
                           tflops=nb3 * nch3 * T3 * c3.n_q_heads * (D3 + c3.v_dim) * 2 / ms / 1e9)
     ctx3.kam_paged_decode_plan(None, None, None, None)
     ctx3.close()
+    del pool3, ctx3, ch3, refs3, q3, o3
     return out
 
 
+_PROFILE_LEGS = False            # --profile-legs: one representative call of every as-stated phase runs between cudaProfilerStart / Stop
+
+
+def _prof(torch, fn):
+    if _PROFILE_LEGS:
+        torch.cuda.synchronize(); torch.cuda.profiler.start()
+        fn()
+        torch.cuda.synchronize(); torch.cuda.profiler.stop()
+
+
+def as_stated_legs(wl, device, peak):
+    """After the extras: kam_form_patch timed (f3), and BASELINE.json configs[3] / configs[4] at their stated sizes (not reduced
+    shapes).  Each leg frees what it allocated; a leg that cannot run (memory) says so instead of taking the line down."""
+    import torch
+    from synth import randn_device
+    out, seed = {}, [192837]
+
+    def rnd(shape, std=1.0):
+        seed[0] += 1
+        return randn_device(shape, seed[0], std, torch.bfloat16, device)
+    for name, leg in (("form_patch_config2_chunk_m16", lambda: _form_patch_leg(wl, device, rnd)),
+                      ("config5_as_stated", lambda: _config5_leg(wl, device, peak, rnd)),
+                      ("config4_as_stated", lambda: _config4_leg(wl, device, peak, rnd))):
+        torch.cuda.synchronize(); torch.cuda.empty_cache()
+        try:
+            out[name] = leg()
+        except Exception as e:
+            out[name] = {"error": repr(e)[:300]}
+    torch.cuda.synchronize(); torch.cuda.empty_cache()
+    out["note_on_frac"] = ("frac = algorithmic bytes / device time / MEASURED_PEAKS.json hbm_gbs, which is a COPY rate (read + write); a stream that mostly "
+                           "reads (decode) or runs for milliseconds (no ramp, no tail) can exceed it: ncu's dram__throughput %% in profiles/ncu_legs_r03.md "
+                           "is the figure to hold against the hardware")
+    return out
+
+
+def _time_queued_ms(torch, fn, reps, sleep_cycles=120_000_000):
+    """Device time of `reps` calls of fn whose HOST side (marshalling a few hundred descriptors in Python) is slower than their
+    kernels: the calls are enqueued while the GPU sits in a sleep kernel, so the events bracket back-to-back device work."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    fn(); torch.cuda.synchronize()
+    torch.cuda._sleep(sleep_cycles)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record(); torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def _form_patch_leg(wl, device, rnd):
+    import torch
+    cfg = wl.cfg
+    L, H, D, T, m = cfg.n_layers, cfg.n_kv_heads, cfg.row_dim, cfg.chunk_tokens, cfg.rank
+    solo = [rnd((T, H, D)) for _ in range(L)]
+    # conditioned rows = rotated solo rows + an exactly rank-m perturbation would need the oracle; for TIMING any rows do
+    cond = [rnd((T, H, D)) for _ in range(L)]
+    ms = _time_ms(torch, lambda: wl.ctx_a.kam_form_patch(cond, solo, 4096, 1, m), 3)
+    _prof(torch, lambda: wl.ctx_a.kam_form_patch(cond, solo, 4096, 1, m))
+    sweeps = 6
+    b = m + 8
+    flops = L * H * (2.0 * T * D * D + sweeps * 2 * (2.0 * D * D * b)) + L * H * 2.0 * T * D * b       # Gram + sweeps on D x D + U = Delta V
+    return {"ms": ms, "ms_per_chunk_k_and_v": 2 * ms, "gflops": flops / ms / 1e6,
+            "what": "kam_form_patch(is_key = 1) for one 1024-token chunk x 28 layers x 4 KV heads, rank 16 (+8 oversampling), 6 sweeps of block "
+                    "subspace iteration on Delta^T Delta; flops = Gram product + sweeps + U = Delta V; CUDA cores (fp32), not tuned: paid once per chunk at "
+                    "compile time (P:56), not on the serve path"}
+
+
+def _config5_leg(wl, device, peak, rnd):
+    """BASELINE.json configs[4]: GQA 64 q / 8 kv heads, head_dim 128, chunks of 2048 tokens, m = 32, page size 16; 64 requests x 32
+    chunks.  The stated pool (~150 GB) holds 8 of the 80 layers at a time; the bench keeps 2 layers resident (34 GB) beside its own
+    workload: ONE launch relocates 256 chunks (8 requests x 32 chunks) from 256 distinct canonical chunks (5.4 GB; with fewer sources
+    than relocations two CTAs read the same source at the same moment and the second read is an L2 hit - measured: DRAM reads fell to
+    half the algorithmic bytes), and the fused decode reads batch 64 x 65536 tokens (17.2 GB per layer)."""
+    import torch
+    kam, B = wl.kam, wl.B
+    from synth import CONFIGS
+    cx = CONFIGS[5]
+    H, D, P, T, m, Hq = cx.n_kv_heads, cx.row_dim, cx.page_size, cx.chunk_tokens, cx.rank, cx.n_q_heads
+    Lx, NREQ, NCH, NSRC, PER = 2, 64, 32, 256, 256
+    ppr = NCH * T // P
+    need = 2 * Lx * NREQ * ppr * P * H * D * 2 + NSRC * Lx * 2 * (T * H * D * 2 + T * H * m * 2) + 2e9
+    free = torch.cuda.mem_get_info()[0]
+    if free < need:
+        return {"skipped": "needs %.0f GB of free HBM, %.0f GB free" % (need / 1e9, free / 1e9)}
+    pool = kam.Pool([torch.zeros((NREQ * ppr, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(Lx)],
+                    [torch.zeros((NREQ * ppr, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(Lx)])
+    ctx = kam.Context(kam.make_layout(B.KAM_GQA, Lx, Hq, H, D, 0, D, True, P, cx.theta), pool)
+    srcs = [(kam.Chunk([rnd((T, H, D)) for _ in range(Lx)], [rnd((T, H, D)) for _ in range(Lx)]),
+             kam.Patch([rnd((T, H, m)) for _ in range(Lx)], [rnd((H, m, D), cx.w_std) for _ in range(Lx)],
+                       [rnd((T, H, m)) for _ in range(Lx)], [rnd((H, m, D), cx.w_std) for _ in range(Lx)])) for _ in range(NSRC)]
+    bt = torch.randperm(NREQ * ppr, device=device, dtype=torch.int32)
+    gen = torch.Generator().manual_seed(5)
+    targets = torch.randint(0, cx.max_pos, (NREQ * NCH,), generator=gen).tolist()
+    it = [0]
+
+    def launch():
+        g0 = (it[0] * PER) % (NREQ * NCH)
+        it[0] += 1
+        ctx.kam_relocate_patch_batch([(bt, (g0 + c) * T, srcs[(g0 + c) % NSRC][0], targets[g0 + c], srcs[(g0 + c) % NSRC][1], m) for c in range(PER)])
+    for _ in range(NREQ * NCH // PER):                            # fill the whole pool once (8 launches): the decode reads relocated rows
+        launch()
+    ms = _time_queued_ms(torch, launch, 4)
+    _prof(torch, launch)
+    nbytes = PER * Lx * algorithmic_bytes_relocate(T, H, D, m, P)
+    res = {"relocate": {"ms_per_launch": ms, "GB/s": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak, "chunks_per_launch": PER, "layers_resident": Lx,
+                        "us_per_1024tok_chunk_80_layers": 1e3 * ms / PER * 1024 / T * cx.n_layers / Lx,
+                        "ms_all_2048_chunks_80_layers_extrapolated": ms * (NREQ * NCH / PER) * cx.n_layers / Lx,
+                        "tiled_kernel": ctx.kam_get_stats()["generic_launches"] == 0,
+                        "what": "one kam_relocate_patch_batch of 256 chunk-relocations (m = 32) into 2 resident layers; 256 distinct sources (5.4 GB), every launch reads each once"}}
+    btd = bt.reshape(NREQ, ppr)
+    starts = torch.arange(0, (NCH + 1) * T, T, dtype=torch.int32, device=device).repeat(NREQ, 1)
+    nc = torch.full((NREQ,), NCH, dtype=torch.int32, device=device)
+    q = rnd((NREQ, Hq, D))
+    o, l = torch.zeros_like(q), torch.zeros((NREQ, Hq), dtype=torch.float32, device=device)
+    jt = [0]
+
+    def dec():
+        jt[0] += 1
+        ctx.kam_paged_decode_merge(q, btd, starts, None, nc, jt[0] % Lx, D ** -0.5, o, l)
+    msd = _time_ms(torch, dec, 4)
+    _prof(torch, dec)
+    nb = NREQ * NCH * T * H * 2 * D * 2
+    res["decode"] = {"ms_per_layer": msd, "GB/s": nb / msd / 1e6, "frac": nb / msd / 1e6 / peak, "batch": NREQ, "tokens_per_request": NCH * T,
+                     "tok_per_s_80_layers_extrapolated": NREQ / (msd * cx.n_layers / 1e3),
+                     "roofline_tok_per_s_80_layers": NREQ / (nb * cx.n_layers / (peak * 1e9)),
+                     "what": "kam_paged_decode_merge (plan + decode + merge per call), batch 64 over 32 chunks x 2048 tokens, one layer = 17.2 GB"}
+    ctx.close()
+    return res
+
+
+def _config4_leg(wl, device, peak, rnd):
+    """BASELINE.json configs[3] at its stated size: MHA 32 layers x 32 heads x 128, 32 requests, each a pinned 512-token text prefix + a
+    window of 3 screenshots of 1280 tokens (pool 73 GB).  One slide step = every request evicts its oldest screenshot and recalls
+    one by relocate+patch (m = 16) from 8 canonical chunks (5.5 GB) while the two survivors rotate in place by -1280; then
+    the fused decode, batch 32, over window + prefix (4352 tokens) x 32 layers."""
+    import torch
+    kam, B = wl.kam, wl.B
+    from synth import CONFIGS
+    cx = CONFIGS[4]
+    L, H, D, P, T, m = cx.n_layers, cx.n_kv_heads, cx.row_dim, cx.page_size, cx.chunk_tokens, cx.rank
+    NREQ, TP, NCAN = 32, 512, 8
+    ppc = T // P
+    n_pages = NREQ * (TP // P + 4 * ppc)
+    need = 2 * L * n_pages * P * H * D * 2 + NCAN * L * 2 * (T * H * D * 2 + T * H * m * 2) + 3e9
+    free = torch.cuda.mem_get_info()[0]
+    if free < need:
+        return {"skipped": "needs %.0f GB of free HBM, %.0f GB free" % (need / 1e9, free / 1e9)}
+    pool = kam.Pool([torch.zeros((n_pages, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(L)],
+                    [torch.zeros((n_pages, P, H, D), dtype=torch.bfloat16, device=device) for _ in range(L)])
+    ctx = kam.Context(kam.make_layout(B.KAM_MHA, L, cx.n_q_heads, H, D, 0, D, True, P, cx.theta), pool, max_requests=NREQ,
+                      max_chunks_per_request=5, max_pages_per_chunk=ppc)
+    canon = [(kam.Chunk([rnd((T, H, D)) for _ in range(L)], [rnd((T, H, D)) for _ in range(L)]),
+              kam.Patch([rnd((T, H, m)) for _ in range(L)], [rnd((H, m, D), cx.w_std) for _ in range(L)],
+                        [rnd((T, H, m)) for _ in range(L)], [rnd((H, m, D), cx.w_std) for _ in range(L)])) for _ in range(NCAN)]
+    prefix = kam.Chunk([rnd((TP, H, D)) for _ in range(L)], [rnd((TP, H, D)) for _ in range(L)])
+    for r in range(NREQ):
+        ctx.kam_window_open(r, 0)
+        ctx.kam_admit(r, B.KAM_BACK, prefix, None, 0, 1)
+        ctx.kam_window_pin(r, 1)
+        for c in range(3):
+            ctx.kam_admit(r, B.KAM_BACK, canon[(r + c) % NCAN][0], canon[(r + c) % NCAN][1], m, 1)
+    torch.cuda.synchronize()
+    it = [0]
+
+    def slide_step():                                            # ONE launch per request: 2 survivors in place + the recalled chunk
+        s = it[0]
+        it[0] += 1
+        for r in range(NREQ):
+            ci = (r + 3 + s) % NCAN
+            ctx.kam_slide(r, B.KAM_FRONT, B.KAM_BACK, canon[ci][0], canon[ci][1], m, 1)
+    ms_slide = _time_ms(torch, slide_step, 3)
+    _prof(torch, lambda: ctx.kam_slide(0, B.KAM_FRONT, B.KAM_BACK, canon[1][0], canon[1][1], m, 1))
+    _prof(torch, lambda: ctx.kam_evict(1, B.KAM_FRONT, 1))
+    _prof(torch, lambda: ctx.kam_admit(1, B.KAM_BACK, canon[2][0], canon[2][1], m, 1))
+    b_surv = 2 * L * (2 * T * H * D * 2)                           # two survivors: K rows read + written, V untouched
+    b_rec = L * algorithmic_bytes_relocate(T, H, D, m, P)
+    # the two halves separately (the two-call form: kam_evict rotates the survivors, kam_admit recalls)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ms_e = ms_a = 0.0
+    for rep in range(3):
+        ev[0].record()
+        for r in range(NREQ):
+            ctx.kam_evict(r, B.KAM_FRONT, 1)
+        ev[1].record()
+        for r in range(NREQ):
+            ci = (r + 5 + rep) % NCAN
+            ctx.kam_admit(r, B.KAM_BACK, canon[ci][0], canon[ci][1], m, 1)
+        ev[2].record(); torch.cuda.synchronize()
+        if rep:                                                   # the first repetition warms up
+            ms_e += ev[0].elapsed_time(ev[1]) / 2; ms_a += ev[1].elapsed_time(ev[2]) / 2
+    res = {"slide_step": {"ms": ms_slide, "GB/s": NREQ * (b_surv + b_rec) / ms_slide / 1e6, "frac": NREQ * (b_surv + b_rec) / ms_slide / 1e6 / peak,
+                          "roofline_ms": NREQ * (b_surv + b_rec) / (peak * 1e6), "launches": NREQ,
+                          "what": "32 x kam_slide(FRONT, BACK, m = 16): per request 2 x 1280 survivor tokens rotated in place (K only) + 1280 tokens recalled by Eq. 1, 32 layers"},
+           "survivors_alone": {"ms": ms_e, "GB/s": NREQ * b_surv / ms_e / 1e6, "frac": NREQ * b_surv / ms_e / 1e6 / peak,
+                               "us_per_1024tok_chunk": 1e3 * ms_e / (NREQ * 2 * T / 1024), "what": "32 x kam_evict(FRONT, materialize = 1)"},
+           "recall_alone": {"ms": ms_a, "GB/s": NREQ * b_rec / ms_a / 1e6, "frac": NREQ * b_rec / ms_a / 1e6 / peak,
+                            "us_per_1024tok_chunk": 1e3 * ms_a / (NREQ * T / 1024), "what": "32 x kam_admit(BACK, m = 16)"}}
+    q = rnd((NREQ, cx.n_q_heads, D))
+    o, l = torch.zeros_like(q), torch.zeros((NREQ, cx.n_q_heads), dtype=torch.float32, device=device)
+    reqs = list(range(NREQ))
+
+    def decode_step():
+        ctx.kam_window_plan(reqs)
+        for layer in range(L):
+            ctx.kam_window_decode(q, reqs, layer, D ** -0.5, o, l)
+    ms_d = _time_ms(torch, decode_step, 3)
+    _prof(torch, lambda: ctx.kam_window_decode(q, reqs, 7, D ** -0.5, o, l))
+    nb = NREQ * (TP + 3 * T) * H * 2 * D * 2 * L
+    res["decode_step"] = {"ms": ms_d, "GB/s": nb / ms_d / 1e6, "frac": nb / ms_d / 1e6 / peak, "tok_per_s": NREQ / (ms_d / 1e3),
+                          "roofline_tok_per_s": NREQ / (nb / (peak * 1e9)), "batch": NREQ, "tokens_per_request": TP + 3 * T,
+                          "what": "kam_window_plan + 32 x kam_window_decode (eager), 73 GB read per step"}
+    res["pool_GB"] = 2 * L * n_pages * P * H * D * 2 / 1e9
+    ctx.close()
+    return res
+
+
 # ------------------------------------------------------------------------------------------------------- ncu evidence
-NCU_SUMMARY = "profiles/ncu_step_r02.json"
+NCU_SUMMARY = "profiles/ncu_step_r03.json"
 
 
 def ncu_evidence(kernel_key):
     """DRAM bytes per launch and ncu's own dram__throughput % for the named kernel, from the committed summary of ONE
-    `ncu --set full` capture of a bench step (profiles/ncu_step_r02.md names the command and the commit).  None if absent."""
+    `ncu --set full` capture of a bench step (profiles/ncu_step_r03.md names the command and the commit).  None if absent."""
     path = os.path.join(ROOT, NCU_SUMMARY)
     if not os.path.exists(path):
         return None
@@ -835,11 +1051,15 @@ def main():
                     help="bracket the first timed step with cudaProfilerStart/Stop (for `ncu --profile-from-start off`)")
     ap.add_argument("--profile-extras", action="store_true",
                     help="bracket the extras leg with cudaProfilerStart/Stop instead of a timed step")
+    ap.add_argument("--profile-legs", action="store_true",
+                    help="skip the other extras and bracket ONE call of every phase of the as-stated config 4 / 5 legs with cudaProfilerStart/Stop")
     ap.add_argument("--no-graph", action="store_true", help="launch the per-layer decode calls eagerly instead of replaying a CUDA graph")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     args.warmup = max(3, args.warmup)
+    global _PROFILE_LEGS
+    _PROFILE_LEGS = args.profile_legs
 
     import torch
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -901,9 +1121,10 @@ def main():
         if rank == 0 and world == 1 and not args.no_extras and not args.profile_step:
             if args.profile_extras:
                 torch.cuda.profiler.start()
-            legs["extras"] = extras(wl, device, peak)
+            legs["extras"] = {} if args.profile_legs else extras(wl, device, peak)
             if args.profile_extras:
                 torch.cuda.profiler.stop()
+            legs["extras"].update(as_stated_legs(wl, device, peak))
         return legs
 
     run(args, world, rank, wl, clock, wl_info, sampler=ClockSampler(local), after=after)
