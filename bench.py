@@ -1103,7 +1103,7 @@ def main():
             legs["e2e"] = {"value": by / res["pipelined"] / 1e9, "unit": "GB/s", "h2d_bytes_per_step": ee.h2d, "d2h_bytes_per_step": ee.d2h,
                            "ms_per_step": res["pipelined"] * 1e3, "serial_value": by / res["serial"] / 1e9, "serial_ms_per_step": res["serial"] * 1e3,
                            "what": "8 x kam_relocate_patch_host (one pinned host slab per chunk: rows + factors of 28 layers -> one merged H2D on the "
-                                   "library's copy stream -> kernel; the copy of chunk c+1 runs under the kernel of chunk c) + kam_paged_decode_plan + 28 x "
+                                   "library's copy stream (option host_copy_overlap = 1, opt-in: the slabs are final before the call) -> kernel; the copy of chunk c+1 runs under the kernel of chunk c) + kam_paged_decode_plan + 28 x "
                                    "kam_paged_decode_merge_host (q H2D, out/lse D2H) + ONE synchronise per step, after which the host reads out/lse; "
                                    "relocate+patch bytes / whole region.  serial_*: options host_copy_overlap=0, host_entries_sync=1 (a synchronise per decode call)"}
         if rank == 0 and world == 1 and not args.no_cpu:
